@@ -1,0 +1,328 @@
+"""fp64 CPU oracle for the fast Eikonal Phase Retrieval (EPR) hot path.
+
+TEST INFRASTRUCTURE ONLY.  This module is a plain, slow, obviously-correct numpy
+restatement of what the paper defines.  It shares no code with the CUDA path and must
+never be imported by the product (`paper_2601_22793_b200/`); only `tests/`,
+`__graft_entry__.smoke()` and `bench.py`'s `cpu_baseline` / `--impl reference` legs may
+import it.
+
+Every function cites the PAPER.md passage (line, section / equation) it follows.  Where the
+paper is silent the reading taken is the one listed in DESIGN.md ("Readings", R1..R15, which
+restate SURVEY.md §8(c)).
+
+Conventions: pixel units; arrays are `[row = y][col = x]`, x fastest
+(PAPER.md:185-191 write `P_s(y0, x0)`); every index is periodic (R7).
+
+Parity pins: every function below is pinned by `tests/test_oracle_pins.py` against closed
+forms, invariants, brute force or a library routine used in a different way (see the table in
+DESIGN.md).  The *discretisation readings* R1..R14 themselves are "parity unpinned" against
+the paper's own (unavailable) implementation: the paper prints no numeric intermediate or
+final value.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+
+import numpy as np
+
+HC_KEV_M = 1.2398419843e-9  # h*c in keV*m  (lambda = hc / E)
+
+
+# --------------------------------------------------------------------------------------
+# physical constants per spectral line
+# --------------------------------------------------------------------------------------
+@dataclass
+class Lines:
+    """Per-line scalars of the spectral discretisation (§4.3-4.4)."""
+
+    n_bins: int
+    energy_keV: np.ndarray
+    k: np.ndarray        # wavenumber 2*pi/lambda, 1/m
+    alpha: np.ndarray    # eps_s / p^2 = L/(k_s p^2), dimensionless
+    db: np.ndarray       # delta_s / beta_s
+    a: np.ndarray        # alpha_s * db_s / 2  (Paganin length^2 in px^2)
+    f: np.ndarray        # spectral fraction, sum = 1
+    gamma: np.ndarray    # per-line attenuation scaling, sum f*gamma = 1      PAPER.md:227-229 (R11)
+
+    @property
+    def abar(self) -> float:
+        """Weighted-mean Paganin coefficient used by the initial guess (R9)."""
+        return float(np.sum(self.f * self.a))
+
+
+def derive_lines(pixel_m, L_m, energy_keV, weight, delta_over_beta, mu_rel=None) -> Lines:
+    """k_s = 2 pi E_s/(hc); eps_s = L/k_s (Eq. (2), (S8) PAPER.md:349);
+    in pixel units alpha_s = eps_s/p^2.  phi_s = (db_s/2) ln I_s (Eq. (6)
+    PAPER.md:216) gives a_s = alpha_s db_s/2.  gamma_s (Eq. (7)) is not a plan
+    argument; reading R11: mu_s ∝ 1/(E_s db_s), normalised so that sum_s f_s gamma_s = 1."""
+    E = np.atleast_1d(np.asarray(energy_keV, dtype=np.float64))
+    w = np.atleast_1d(np.asarray(weight, dtype=np.float64))
+    db = np.atleast_1d(np.asarray(delta_over_beta, dtype=np.float64))
+    n = E.size
+    assert w.size == n and db.size == n
+    k = 2.0 * np.pi * E / HC_KEV_M
+    alpha = L_m / (k * pixel_m * pixel_m)
+    a = alpha * db / 2.0
+    f = w / w.sum()
+    g = (1.0 / (E * db)) if mu_rel is None else np.asarray(mu_rel, dtype=np.float64)
+    gamma = g / np.sum(f * g)
+    return Lines(n, E, k, alpha, db, a, f, gamma)
+
+
+# --------------------------------------------------------------------------------------
+# periodic finite differences (R1-R3, R7)
+# --------------------------------------------------------------------------------------
+def _xp(g):  # g[y][x+1]
+    return np.roll(g, -1, axis=1)
+
+
+def _xm(g):  # g[y][x-1]
+    return np.roll(g, 1, axis=1)
+
+
+def _yp(g):  # g[y+1][x]
+    return np.roll(g, -1, axis=0)
+
+
+def _ym(g):  # g[y-1][x]
+    return np.roll(g, 1, axis=0)
+
+
+def d0x(g):
+    return (_xp(g) - _xm(g)) / 2.0
+
+
+def d0y(g):
+    return (_yp(g) - _ym(g)) / 2.0
+
+
+def d2x(g):
+    return _xp(g) - 2.0 * g + _xm(g)
+
+
+def d2y(g):
+    return _yp(g) - 2.0 * g + _ym(g)
+
+
+def lap5(g):
+    return d2x(g) + d2y(g)
+
+
+# --------------------------------------------------------------------------------------
+# a1-L  local O(L^2) closure, Eq. (1)
+# --------------------------------------------------------------------------------------
+def closure(I, a, alpha, order=2, wkb1=True):
+    """P = I − eps ∂i(I ∂iφ) + (eps²/2) ∂i∂j(I ∂iφ ∂jφ) − (eps²/4) ∂i(I ∂iQ)   Eq. (1) PAPER.md:146.
+
+    With Eq. (6) I ∂φ = (db/2) ∂I, so the O(L) term is −a ∇²I (R1, 5-point).
+    WKB0 O(L²): g = D⁰ ln I, S_ij = I g_i g_j, coefficient a²/2 (R2).
+    WKB1: Q = ∇²√I/√I (Eq. (S15)), flux form, coefficient alpha²/4 (R3).
+    `order=1` is the L¹ truncation."""
+    I = np.asarray(I, dtype=np.float64)
+    P = I - a * lap5(I)
+    if order == 2:
+        lnI = np.log(I)
+        gx = d0x(lnI)
+        gy = d0y(lnI)
+        Sxx = I * gx * gx
+        Syy = I * gy * gy
+        Sxy = I * gx * gy
+        P = P + 0.5 * a * a * (d2x(Sxx) + d2y(Syy) + 2.0 * d0x(d0y(Sxy)))
+        if wkb1:
+            A = np.sqrt(I)
+            Q = lap5(A) / A
+            Fx = 0.5 * (_xp(I) + I) * (_xp(Q) - Q)   # flux through the face x+1/2
+            Fy = 0.5 * (_yp(I) + I) * (_yp(Q) - Q)   # flux through the face y+1/2
+            div = (Fx - _xm(Fx)) + (Fy - _ym(Fy))
+            P = P - 0.25 * alpha * alpha * div
+    return P
+
+
+# --------------------------------------------------------------------------------------
+# a1-N  eikonal ray map, Eq. (2), and splat
+# --------------------------------------------------------------------------------------
+def ray_map(I, a, S):
+    """u_s = Δ_s/p = (eps_s/p²) ∇φ_s with φ_s = (db_s/2) ln I_s  →  u = a · D⁰ ln I
+    (Eq. (2), Eq. (6)), each component clamped
+    to [−S, S] (R6)."""
+    lnI = np.log(np.asarray(I, dtype=np.float64))
+    ux = np.clip(a * d0x(lnI), -S, S)
+    uy = np.clip(a * d0y(lnI), -S, S)
+    return ux, uy
+
+
+def _bilinear_targets(ux, uy):
+    """x_t = x + u_x, y_t = y + u_y; x0 = ⌊x_t⌋, y0 = ⌊y_t⌋, d = x_t − x0; the four weights of
+    PAPER.md:177-181.  Indices wrap (R7)."""
+    ny, nx = ux.shape
+    Y, X = np.meshgrid(np.arange(ny, dtype=np.float64), np.arange(nx, dtype=np.float64), indexing="ij")
+    xt = X + ux
+    yt = Y + uy
+    x0f = np.floor(xt)
+    y0f = np.floor(yt)
+    dx = xt - x0f
+    dy = yt - y0f
+    x0 = np.mod(x0f.astype(np.int64), nx)
+    y0 = np.mod(y0f.astype(np.int64), ny)
+    x1 = np.mod(x0 + 1, nx)
+    y1 = np.mod(y0 + 1, ny)
+    w00 = (1.0 - dx) * (1.0 - dy)
+    w10 = dx * (1.0 - dy)
+    w01 = (1.0 - dx) * dy
+    w11 = dx * dy
+    return (y0, y1, x0, x1), (w00, w10, w01, w11)
+
+
+def splat(I, ux, uy):
+    """Mass-conserving bilinear redistribution ℳ_s (Eq. (3), discrete form
+    PAPER.md:175-191):  P(y0,x0) += I w00;  P(y0,x0+1) += I w10;  P(y0+1,x0) += I w01;
+    P(y0+1,x0+1) += I w11."""
+    I = np.asarray(I, dtype=np.float64)
+    ny, nx = I.shape
+    (y0, y1, x0, x1), (w00, w10, w01, w11) = _bilinear_targets(ux, uy)
+    P = np.zeros(ny * nx, dtype=np.float64)
+    for yy, xx, w in ((y0, x0, w00), (y0, x1, w10), (y1, x0, w01), (y1, x1, w11)):
+        P += np.bincount((yy * nx + xx).ravel(), weights=(I * w).ravel(), minlength=ny * nx)
+    return P.reshape(ny, nx)
+
+
+def gather(e, ux, uy):
+    """Adjoint ℳ*_s, Eq. (4) PAPER.md:197-203:
+    (ℳ* e)(x,y) = w00 e(y0,x0) + w10 e(y0,x0+1) + w01 e(y0+1,x0) + w11 e(y0+1,x0+1)."""
+    e = np.asarray(e, dtype=np.float64)
+    (y0, y1, x0, x1), (w00, w10, w01, w11) = _bilinear_targets(ux, uy)
+    return w00 * e[y0, x0] + w10 * e[y0, x1] + w01 * e[y1, x0] + w11 * e[y1, x1]
+
+
+# --------------------------------------------------------------------------------------
+# a4  FFT-diagonal Paganin-type preconditioner
+# --------------------------------------------------------------------------------------
+def symbol_lambda(ny, nx, symbol=0):
+    """λ(θ): Fourier symbol of −∇² on the pixel grid.  symbol=0: discrete 5-point
+    (2−2cosθx)+(2−2cosθy) (default, R5: makes P⁻¹₁ the exact inverse of the R1 O(L) operator);
+    symbol=1: continuous θx²+θy² (textbook Paganin filter)."""
+    thx = 2.0 * np.pi * np.fft.fftfreq(nx)
+    thy = 2.0 * np.pi * np.fft.fftfreq(ny)
+    if symbol == 0:
+        lx = 2.0 - 2.0 * np.cos(thx)
+        ly = 2.0 - 2.0 * np.cos(thy)
+    else:
+        lx = thx * thx
+        ly = thy * thy
+    return ly[:, None] + lx[None, :]
+
+
+def precondition(r, a, symbol=0):
+    """q = IFFT2( FFT2(r) / (1 + a λ) ): the FFT-diagonal inverse of the linearised O(L)
+    per-line operator I ↦ I − a∇²I ("Paganin-type filter")."""
+    r = np.asarray(r, dtype=np.float64)
+    H = 1.0 / (1.0 + a * symbol_lambda(r.shape[0], r.shape[1], symbol))
+    return np.real(np.fft.ifft2(np.fft.fft2(r) * H))
+
+
+# --------------------------------------------------------------------------------------
+# a6  projection to the single-thickness manifold, Eq. (7) PAPER.md:227, PAPER.md:233 (R10)
+# --------------------------------------------------------------------------------------
+def line_intensities(tau, lines: Lines):
+    """I_s = f_s exp(−γ_s τ)   Eq. (7) PAPER.md:227."""
+    tau = np.asarray(tau, dtype=np.float64)
+    return [lines.f[s] * np.exp(-lines.gamma[s] * tau) for s in range(lines.n_bins)]
+
+
+def project(T, lines: Lines, tol=1e-14, max_iter=200):
+    """Solve Σ_s f_s exp(−γ_s τ) = T per pixel (R10: the projection keeps the total object-plane
+    intensity).  Newton from τ0 = −ln(T/Σf)/γ̄, γ̄ = Σ f γ / Σ f; monotone by convexity."""
+    T = np.asarray(T, dtype=np.float64)
+    f, g = lines.f, lines.gamma
+    gbar = np.sum(f * g) / np.sum(f)
+    tau = -np.log(T / np.sum(f)) / gbar
+    if lines.n_bins == 1:
+        return -np.log(T / f[0]) / g[0]
+    for _ in range(max_iter):
+        F = -T.copy()
+        dF = np.zeros_like(T)
+        for s in range(lines.n_bins):
+            E = f[s] * np.exp(-g[s] * tau)
+            F += E
+            dF -= g[s] * E
+        step = F / dF
+        tau = tau - step
+        if np.max(np.abs(step)) < tol:
+            break
+    return tau
+
+
+# --------------------------------------------------------------------------------------
+# forward model  τ → Σ_s F_s[I_s]   Eq. (5)
+# --------------------------------------------------------------------------------------
+def forward(tau, lines: Lines, solver="local", order=2, wkb1=True, S=16.0):
+    """I_det ≈ Σ_s F_s[I_s], F_s ∈ {P_{m,s}, ℳ_s} (Eq. (5)) with
+    I_s = f_s e^{−γ_s τ} (Eq. (7)).  Returns (P_sum, [P_s], [(ux_s, uy_s)] or None)."""
+    Is = line_intensities(tau, lines)
+    P_bins, maps = [], []
+    for s in range(lines.n_bins):
+        if solver == "local":
+            P_bins.append(closure(Is[s], lines.a[s], lines.alpha[s], order=order, wkb1=wkb1))
+        else:
+            ux, uy = ray_map(Is[s], lines.a[s], S)
+            maps.append((ux, uy))
+            P_bins.append(splat(Is[s], ux, uy))
+    P = np.sum(P_bins, axis=0)
+    return P, P_bins, (maps if solver != "local" else None)
+
+
+def split_weights(P_bins, lines: Lines):
+    """"positivity-weighted weights", reading R8: w_s = P_s⁺ / Σ_t P_t⁺,
+    falling back to f_s where the denominator is not positive."""
+    Pp = [np.maximum(P, 0.0) for P in P_bins]
+    den = np.sum(Pp, axis=0)
+    ok = den > 0.0
+    safe = np.where(ok, den, 1.0)
+    return [np.where(ok, Pp[s] / safe, lines.f[s]) for s in range(lines.n_bins)]
+
+
+# --------------------------------------------------------------------------------------
+# the iteration
+# --------------------------------------------------------------------------------------
+def paganin_init(d, lines: Lines, symbol=0, i_min=1e-6):
+    """Initial guess (R9): one linear Paganin solve with the weighted-mean coefficient ā,
+    floored at i_min, projected onto the manifold Eq. (7).  `iterations = 0` returns this —
+    the L¹ / Paganin result of PAPER.md:124."""
+    T0 = precondition(d, lines.abar, symbol)
+    T0 = np.maximum(T0, i_min)
+    return project(T0, lines)
+
+
+def retrieve(d, lines: Lines, solver="local", iterations=10, step=1.0, order=2, wkb1=True,
+             symbol=0, S=16.0, i_min=1e-6, tau0=None, history=None):
+    """The batched per-projection correction loop for one projection:
+    per-line predictions and their sum, detector residual, positivity-weighted split, transport
+    back (identity | adjoint Eq. (4)), per-line FFT-diagonal preconditioner update, projection
+    to the single-thickness manifold.  Returns τ."""
+    d = np.asarray(d, dtype=np.float64)
+    tau = paganin_init(d, lines, symbol, i_min) if tau0 is None else np.asarray(tau0, np.float64).copy()
+    n = lines.n_bins
+    for _ in range(iterations):
+        Is = line_intensities(tau, lines)
+        P, P_bins, maps = forward(tau, lines, solver, order, wkb1, S)
+        e = d - P
+        if history is not None:
+            history.append(float(np.sqrt(np.mean(e * e))))
+        w = split_weights(P_bins, lines)
+        for s in range(n):
+            r = w[s] * e
+            if solver != "local":
+                r = gather(r, maps[s][0], maps[s][1])
+            Is[s] = Is[s] + step * precondition(r, lines.a[s], symbol)
+        if n > 1:
+            T = np.maximum(np.sum(Is, axis=0), i_min)
+            tau = project(T, lines)
+        else:
+            I1 = np.maximum(Is[0], i_min)
+            tau = -np.log(I1 / lines.f[0]) / lines.gamma[0]
+    return tau
+
+
+def phase(tau, lines: Lines, s=0):
+    """φ_s = (db_s/2) ln(I_s/f_s) = −(db_s/2) γ_s τ   Eq. (6) PAPER.md:216 with Eq. (7)."""
+    return -(lines.db[s] / 2.0) * lines.gamma[s] * np.asarray(tau, dtype=np.float64)

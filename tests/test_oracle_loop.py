@@ -1,0 +1,127 @@
+"""Pins for the fp64 oracle's iteration (CPU only): special cases, limits, self-consistency."""
+import numpy as np
+import pytest
+
+from oracle import epr_oracle as O
+
+RNG = np.random.default_rng(777)
+
+
+def _smooth(ny, nx, seed, scale=1.0):
+    """Smooth periodic random field in [-scale, scale] (few low Fourier modes)."""
+    rng = np.random.default_rng(seed)
+    y, x = np.meshgrid(np.arange(ny) * 2 * np.pi / ny, np.arange(nx) * 2 * np.pi / nx, indexing="ij")
+    f = np.zeros((ny, nx))
+    for _ in range(6):
+        m, n = rng.integers(-3, 4, size=2)
+        f += rng.normal() * np.cos(m * x + n * y + rng.uniform(0, 2 * np.pi))
+    return scale * f / np.max(np.abs(f))
+
+
+def _mono(a_target=60.0):
+    p, E, db = 6.5e-6, 100.0, 1000.0
+    k = 2 * np.pi * E / O.HC_KEV_M
+    L = a_target * 2.0 / db * k * p * p
+    return O.derive_lines(p, L, [E], [1.0], [db])
+
+
+def test_L1_mono_one_iteration_equals_paganin():
+    """L1 mono is the Paganin single-distance retrieval.  With order=1, step=1 one
+    iteration from ANY start gives IFFT(FFT(d)/(1+a lambda)) (discrete symbol, R5)."""
+    lines = _mono()
+    d = 1.0 + 0.2 * _smooth(32, 48, 1)
+    tau0 = 0.3 * RNG.uniform(size=d.shape)
+    tau = O.retrieve(d, lines, "local", iterations=1, step=1.0, order=1, tau0=tau0)
+    pag = O.precondition(d, lines.a[0], 0)
+    assert np.max(np.abs(np.exp(-tau) - pag)) < 1e-13
+    # and iterations=0 returns exactly that Paganin result (R9)
+    tau_init = O.retrieve(d, lines, "local", iterations=0)
+    assert np.max(np.abs(np.exp(-tau_init) - pag)) < 1e-14
+
+
+def test_weak_phase_limit_converges_to_paganin_linearly():
+    """north_star pin: in the weak-phase limit the local-closure solution tends to the linear Paganin
+    retrieval; the relative difference is proportional to the object strength eps."""
+    lines = _mono(40.0)
+    b = _smooth(48, 48, 2)
+    ratios = []
+    for eps in (1e-2, 1e-3, 1e-4):
+        truth = eps * (1.0 + 0.5 * b)
+        d, _, _ = O.forward(truth, lines, "local")
+        tau = O.retrieve(d, lines, "local", iterations=12, step=1.0)
+        pag = O.retrieve(d, lines, "local", iterations=0)
+        assert np.max(np.abs(tau - truth)) < 1e-9 * max(1.0, eps / 1e-4)     # recovers its own data
+        ratios.append(np.linalg.norm(tau - pag) / np.linalg.norm(pag - pag.mean()))
+    assert ratios[0] < 5e-2
+    assert 8.0 < ratios[0] / ratios[1] < 12.0
+    assert 8.0 < ratios[1] / ratios[2] < 12.0
+
+
+@pytest.mark.parametrize("solver,step,iters,bound", [("local", 1.0, 12, 1e-4), ("nonlocal", 0.4, 12, 0.15)])
+def test_self_consistent_data_drive_residual_down(solver, step, iters, bound):
+    """Noise-free data made by the same operator: the residual history falls monotonically over the
+    first dozen iterations and the largest gain is at the first one.  (The non-local
+    iteration is only slowly contractive: its residual stalls near 10 % — the bilinear "quantisation
+    effect" of PAPER.md:79 — which is why the bound differs.)"""
+    lines = _mono(50.0)
+    truth = 0.05 * (1.0 + 0.8 * _smooth(64, 64, 3))
+    d, _, _ = O.forward(truth, lines, solver)
+    hist = []
+    tau = O.retrieve(d, lines, solver, iterations=iters, step=step, history=hist)
+    assert all(h1 < h0 for h0, h1 in zip(hist, hist[1:]))
+    assert hist[-1] < bound * hist[0]
+    drops = [h0 - h1 for h0, h1 in zip(hist, hist[1:])]
+    assert drops[0] == max(drops)
+    assert np.linalg.norm(tau - truth) < np.linalg.norm(O.retrieve(d, lines, solver, iterations=0) - truth)
+
+
+def test_poly_with_identical_lines_reduces_to_mono():
+    """Eq. (5)/(7): N_s copies of the same line (equal gamma, db, E) must reproduce the mono result."""
+    p, E, db, L = 6.5e-6, 100.0, 1000.0, 2.0
+    mono = O.derive_lines(p, L, [E], [1.0], [db])
+    poly = O.derive_lines(p, L, [E, E, E], [0.2, 0.5, 0.3], [db, db, db])
+    assert np.allclose(poly.gamma, 1.0)
+    d = 1.0 + 0.1 * _smooth(32, 32, 4)
+    for solver, step in (("local", 1.0), ("nonlocal", 0.4)):
+        t1 = O.retrieve(d, mono, solver, iterations=4, step=step)
+        t3 = O.retrieve(d, poly, solver, iterations=4, step=step)
+        assert np.max(np.abs(t1 - t3)) < 1e-12
+
+
+def test_fourier_sum_identity_R10():
+    """R10 consequence: only the SUM of the per-line updates enters the projection, so summing the
+    filtered residuals in Fourier space and inverse-transforming once changes nothing."""
+    E = np.array([70.0, 100.0, 130.0])
+    lines = O.derive_lines(6.5e-6, 3.0, E, [0.3, 0.4, 0.3], [900.0, 1000.0, 1100.0])
+    assert np.ptp(lines.a) > 1.0                                   # unequal a_s
+    r = [RNG.normal(size=(16, 20)) for _ in range(3)]
+    per_line = sum(O.precondition(r[s], lines.a[s]) for s in range(3))
+    lam = O.symbol_lambda(16, 20, 0)
+    fused = np.real(np.fft.ifft2(sum(np.fft.fft2(r[s]) / (1 + lines.a[s] * lam) for s in range(3))))
+    assert np.max(np.abs(per_line - fused)) < 1e-13
+
+
+def test_split_weights_sum_to_one_and_fallback():
+    lines = O.derive_lines(6.5e-6, 3.0, [80.0, 120.0], [0.4, 0.6], [800.0, 1200.0])
+    P = [RNG.uniform(-0.2, 1.0, size=(8, 8)), RNG.uniform(-0.2, 1.0, size=(8, 8))]
+    P[0][0, 0] = P[1][0, 0] = -1.0                                 # both negative: fallback to f_s
+    w = O.split_weights(P, lines)
+    assert np.max(np.abs(w[0] + w[1] - 1.0)) < 1e-15
+    assert w[0][0, 0] == lines.f[0] and w[1][0, 0] == lines.f[1]
+    assert (w[0] >= 0).all() and (w[1] >= 0).all()
+
+
+def test_local_solver_degrades_beyond_one_pixel_nonlocal_stays_stable():
+    """PAPER.md:97 (qualitative): with multi-pixel shifts the local closure diverges while the
+    non-local solver with relaxation 0.4 stays stable."""
+    lines = _mono(400.0)
+    truth = 0.15 * (1.0 + _smooth(64, 64, 5))
+    ux, _ = O.ray_map(np.exp(-truth), lines.a[0], 16.0)
+    assert np.max(np.abs(ux)) > 1.5
+    d, _, _ = O.forward(truth, lines, "nonlocal")
+    h_loc, h_non = [], []
+    with np.errstate(all="ignore"):
+        O.retrieve(d, lines, "local", iterations=8, step=1.0, history=h_loc)
+    O.retrieve(d, lines, "nonlocal", iterations=8, step=0.4, history=h_non)
+    assert h_non[-1] < h_non[0]
+    assert not (h_loc[-1] < h_non[-1])
