@@ -1,0 +1,118 @@
+/* epr.h — C-ABI of the B200-native fast Eikonal Phase Retrieval (EPR) hot path.
+ *
+ * One library, libepr.so, hand-written CUDA for sm_100a.  It implements the batched per-projection
+ * iterative correction loop of arxiv 2601.22793 (§4.4) and the three operators of one
+ * iteration.  No CPU fallback, no other backend.  Notation follows the paper; the readings R1..R15 of the
+ * points the paper leaves open are listed in DESIGN.md.
+ *
+ * Conventions
+ *  - Arrays are row-major [y][x], x fastest; every index is periodic (R7).
+ *  - ALL array arguments are DEVICE pointers owned by the caller, contiguous, 16-byte aligned.  The library
+ *    never allocates or frees them and keeps no reference once the work enqueued on `stream` has completed.
+ *    (epr_retrieve_host is the one exception: it takes HOST pointers and does the copies itself.)
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Calls only ENQUEUE work and
+ *    return; epr_plan / epr_destroy / epr_retrieve_host may synchronise.
+ *  - Every call returns an epr_status; nothing throws or exits.  On EPR_EINVAL / EPR_ESIZE nothing has been
+ *    enqueued.  epr_last_error(plan) gives a NUL-terminated message owned by the plan.
+ *  - A plan is not thread-safe; distinct plans are independent.
+ *  - d is the flat-field-normalised detector intensity (≈ 1 in the empty beam; Σ_s f_s = 1).
+ *  - The state of the iteration is the nominal thickness field τ of Eq. (7):
+ *    I_s = f_s exp(−γ_s τ).  The phase of line s is φ_s = −(δ_s/2β_s) γ_s τ (Eq. (6)).
+ */
+#ifndef EPR_H
+#define EPR_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct epr_plan_s* epr_plan_t;
+
+typedef enum {
+  EPR_OK = 0,
+  EPR_EINVAL = 1, /* bad argument (NULL pointer, non-positive size / energy / weight / step, batch > max_batch …) */
+  EPR_ESIZE = 2,  /* unsupported grid: nx, ny must be multiples of 4 whose prime factors are in {2,3,5}, ≥ 16 */
+  EPR_ECUDA = 3,  /* a CUDA runtime call failed; message in epr_last_error */
+  EPR_ENOMEM = 4  /* device allocation failed */
+} epr_status;
+
+typedef enum { EPR_LOCAL = 0, EPR_NONLOCAL = 1 } epr_solver;
+
+/* All optional: pass NULL for the defaults, or fill with epr_default_options() first. */
+typedef struct {
+  int order;          /* local solver: truncation order m of P_{m,s}, 1 or 2 (default 2) */
+  int wkb1;           /* local solver: include the −(ε²/4)∂(I∂Q) term of Eq. (1) (default 1) */
+  int symbol;         /* Fourier symbol λ of the filter: 0 discrete 5-point (default), 1 θ²       R5 */
+  float max_shift_px; /* S: clamp of each ray-map component and splat halo (default 16, ≤ 30)    R6 */
+  float i_min;        /* positivity floor of the total object-plane intensity (default 1e-6) */
+  int newton_iters;   /* Newton steps of the single-thickness projection (default 4)             R10 */
+  int init;           /* 0: Paganin initial guess (default); 1: `out` holds τ⁰ on entry          R9 */
+  int output;         /* 0: τ (default); 1: phase φ of line out_bin; 2: total intensity Σ_s I_s */
+  int out_bin;
+  const double* mu_rel; /* γ_s override (relative attenuation per line, length n_bins) or NULL   R11 */
+} epr_options;
+
+void epr_default_options(epr_options* opt);
+
+/* epr_plan — derive the per-line scalars and build tables / workspaces.          PAPER.md:225-233, Eq. (2),(6),(7)
+ *   nx, ny        grid (x fastest).  pixel_m: detector pixel p [m].  L_m: propagation distance [m].
+ *   n_bins        number of spectral lines N_s (1 = monochromatic), ≤ 16.
+ *   energy_keV, weight, delta_over_beta   HOST arrays of length n_bins: E_s, spectral weight (normalised
+ *                 internally to Σ f_s = 1), δ_s/β_s.
+ *   solver        EPR_LOCAL: Taylor/WKB closure Eq. (1); EPR_NONLOCAL: ray map Eq. (2) + splat Eq. (3).
+ *   max_batch     largest `batch` later calls may pass (workspaces are sized for it).
+ * Derived: k_s = 2πE_s/(hc); α_s = L/(k_s p²); a_s = α_s δ_s/(2β_s); γ_s ∝ 1/(E_s δ_s/β_s), Σ f_s γ_s = 1. */
+epr_status epr_plan(epr_plan_t* plan, int nx, int ny, double pixel_m, double L_m, int n_bins,
+                    const double* energy_keV, const double* weight, const double* delta_over_beta,
+                    epr_solver solver, int max_batch, const epr_options* opt);
+
+/* epr_forward — the non-linear forward model τ → Σ_s F_s[f_s e^{−γ_s τ}]         Eq. (5)
+ *   tau    [batch][ny][nx]            in
+ *   P_sum  [batch][ny][nx]            out: predicted detector intensity Σ_s P_s
+ *   P_bins [batch][n_bins][ny][nx]    out or NULL: per-line predictions P_s
+ * Local: P_s = closure Eq. (1).  Non-local: u_s = clamp(a_s D⁰ ln I_s, ±S) (Eq. (2)) and the
+ * mass-conserving bilinear splat; the ray map is kept in the plan for epr_adjoint /
+ * epr_transport (storage for max_batch · n_bins maps is allocated on the first non-local call). */
+epr_status epr_forward(epr_plan_t plan, int batch, const float* tau, float* P_sum, float* P_bins, void* stream);
+
+/* epr_adjoint — back-transport of per-line detector residuals                     Eq. (4)
+ *   e_bins, r_bins [batch][n_bins][ny][nx].  Non-local: bilinear gather with the ray map of the last
+ *   epr_forward on this plan (same batch).  Local: identity copy. */
+epr_status epr_adjoint(epr_plan_t plan, int batch, const float* e_bins, float* r_bins, void* stream);
+
+/* epr_transport — the LINEAR operator ℳ_s: splat arbitrary per-line planes with the stored ray map
+ *   (Eq. (3)).  I_bins, P_bins [batch][n_bins][ny][nx].  Non-local plans only (EPR_EINVAL
+ *   otherwise).  Lets ⟨ℳx,y⟩ = ⟨x,ℳ*y⟩ and mass conservation be checked on the device. */
+epr_status epr_transport(epr_plan_t plan, int batch, const float* I_bins, float* P_bins, void* stream);
+
+/* epr_precondition — q_s = IFFT2( FFT2(r_s) / (1 + a_s λ) ) per line
+ *   r_bins, q_bins [batch][n_bins][ny][nx]; may alias. */
+epr_status epr_precondition(epr_plan_t plan, int batch, const float* r_bins, float* q_bins, void* stream);
+
+/* epr_retrieve — the correction loop
+ *   d   [batch][ny][nx] in;  out [batch][ny][nx] out (τ, or what opt.output selects; τ⁰ in if opt.init = 1).
+ *   iterations ≥ 0 correction iterations after the initial Paganin solve (0 returns the L¹/Paganin result,
+ *   PAPER.md:124); step > 0 relaxation factor. */
+epr_status epr_retrieve(epr_plan_t plan, int batch, const float* d, float* out, int iterations, float step,
+                        void* stream);
+
+/* epr_retrieve_host — same, with HOST buffers (pinned for full speed): copies d host→device, runs the loop,
+ *   copies the result device→host, in chunks of max_batch projections with copies overlapped with compute;
+ *   returns after the last copy has completed.  `batch` may exceed max_batch. */
+epr_status epr_retrieve_host(epr_plan_t plan, int batch, const float* d_host, float* out_host, int iterations,
+                             float step);
+
+/* Per-line scalars the plan derived (HOST arrays of length n_bins, any may be NULL): f_s, γ_s, a_s, α_s. */
+epr_status epr_plan_lines(epr_plan_t plan, double* f, double* gamma, double* a, double* alpha);
+
+/* Number of kernel launches the plan has enqueued so far (for bench.py's gpu_launches). */
+long long epr_launch_count(epr_plan_t plan);
+
+epr_status epr_destroy(epr_plan_t plan);
+const char* epr_last_error(epr_plan_t plan);
+const char* epr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EPR_H */

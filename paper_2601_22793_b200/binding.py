@@ -1,0 +1,198 @@
+"""ctypes binding of include/epr.h — same names, argument marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+EPR_LOCAL, EPR_NONLOCAL = 0, 1
+_STATUS = {0: "EPR_OK", 1: "EPR_EINVAL", 2: "EPR_ESIZE", 3: "EPR_ECUDA", 4: "EPR_ENOMEM"}
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+EXPORTS = ["epr_default_options", "epr_plan", "epr_forward", "epr_adjoint", "epr_transport", "epr_precondition",
+           "epr_retrieve", "epr_retrieve_host", "epr_plan_lines", "epr_launch_count", "epr_destroy",
+           "epr_last_error", "epr_version"]
+
+
+class EprError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{_STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+class Options(C.Structure):
+    """Mirror of `epr_options` (include/epr.h)."""
+    _fields_ = [("order", C.c_int), ("wkb1", C.c_int), ("symbol", C.c_int), ("max_shift_px", C.c_float),
+                ("i_min", C.c_float), ("newton_iters", C.c_int), ("init", C.c_int), ("output", C.c_int),
+                ("out_bin", C.c_int), ("mu_rel", C.POINTER(C.c_double))]
+
+
+def lib_path():
+    return os.path.join(_HERE, "libepr.so")
+
+
+def load_library():
+    """dlopen libepr.so (built by paper_2601_22793_b200.build).  Raises if it is missing — no fallback."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = lib_path()
+    if not os.path.exists(path):
+        raise EprError(3, f"{path} not built: run `python -m paper_2601_22793_b200.build` (needs nvcc)")
+    lib = C.CDLL(path)
+    vp, ci, cf, cd = C.c_void_p, C.c_int, C.c_float, C.c_double
+    lib.epr_default_options.argtypes = [C.POINTER(Options)]
+    lib.epr_default_options.restype = None
+    lib.epr_plan.argtypes = [C.POINTER(vp), ci, ci, cd, cd, ci, C.POINTER(cd), C.POINTER(cd), C.POINTER(cd), ci, ci,
+                             C.POINTER(Options)]
+    lib.epr_forward.argtypes = [vp, ci, vp, vp, vp, vp]
+    lib.epr_adjoint.argtypes = [vp, ci, vp, vp, vp]
+    lib.epr_transport.argtypes = [vp, ci, vp, vp, vp]
+    lib.epr_precondition.argtypes = [vp, ci, vp, vp, vp]
+    lib.epr_retrieve.argtypes = [vp, ci, vp, vp, ci, cf, vp]
+    lib.epr_retrieve_host.argtypes = [vp, ci, vp, vp, ci, cf]
+    lib.epr_plan_lines.argtypes = [vp, C.POINTER(cd), C.POINTER(cd), C.POINTER(cd), C.POINTER(cd)]
+    lib.epr_launch_count.argtypes = [vp]
+    lib.epr_launch_count.restype = C.c_longlong
+    lib.epr_destroy.argtypes = [vp]
+    lib.epr_last_error.argtypes = [vp]
+    lib.epr_last_error.restype = C.c_char_p
+    lib.epr_version.restype = C.c_char_p
+    for name in ("epr_plan", "epr_forward", "epr_adjoint", "epr_transport", "epr_precondition", "epr_retrieve",
+                 "epr_retrieve_host", "epr_plan_lines", "epr_destroy"):
+        getattr(lib, name).restype = ci
+    _LIB = lib
+    return lib
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev(t, shape=None, name="tensor"):
+    import torch
+    if t is None:
+        return C.c_void_p(0)
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError(f"{name}: expected a contiguous float32 CUDA tensor")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    return C.c_void_p(t.data_ptr())
+
+
+class Plan:
+    """Owner of an `epr_plan_t`.  Create with `epr_plan(...)`."""
+
+    def __init__(self, handle, nx, ny, n_bins, solver, max_batch):
+        self._h, self.nx, self.ny, self.n_bins, self.solver, self.max_batch = handle, nx, ny, n_bins, solver, max_batch
+
+    def _check(self, status):
+        if status != 0:
+            raise EprError(status, load_library().epr_last_error(self._h).decode())
+
+    def lines(self):
+        """Per-line scalars derived by the plan: dict of float64 arrays f, gamma, a, alpha."""
+        arrs = [np.zeros(self.n_bins) for _ in range(4)]
+        ptrs = [a.ctypes.data_as(C.POINTER(C.c_double)) for a in arrs]
+        self._check(load_library().epr_plan_lines(self._h, *ptrs))
+        return dict(zip(("f", "gamma", "a", "alpha"), arrs))
+
+    @property
+    def launches(self):
+        return int(load_library().epr_launch_count(self._h))
+
+    def destroy(self):
+        if self._h is not None:
+            load_library().epr_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def epr_plan(nx, ny, pixel_m, L_m, energy_keV, weight, delta_over_beta, solver="local", max_batch=1, **opts):
+    """epr_plan of include/epr.h.  `opts`: fields of epr_options (order, wkb1, symbol, max_shift_px, i_min,
+    newton_iters, init, output, out_bin, mu_rel)."""
+    lib = load_library()
+    E = np.ascontiguousarray(np.atleast_1d(energy_keV), dtype=np.float64)
+    w = np.ascontiguousarray(np.atleast_1d(weight), dtype=np.float64)
+    db = np.ascontiguousarray(np.atleast_1d(delta_over_beta), dtype=np.float64)
+    if not (E.size == w.size == db.size):
+        raise ValueError("energy_keV, weight, delta_over_beta must have the same length")
+    sv = {"local": EPR_LOCAL, "nonlocal": EPR_NONLOCAL}.get(solver, solver)
+    o = Options()
+    lib.epr_default_options(C.byref(o))
+    keep = None
+    for k, v in opts.items():
+        if k == "mu_rel":
+            keep = np.ascontiguousarray(v, dtype=np.float64)
+            o.mu_rel = keep.ctypes.data_as(C.POINTER(C.c_double))
+        elif hasattr(o, k):
+            setattr(o, k, v)
+        else:
+            raise TypeError(f"unknown option {k}")
+    h = C.c_void_p(0)
+    dp = C.POINTER(C.c_double)
+    st = lib.epr_plan(C.byref(h), int(nx), int(ny), float(pixel_m), float(L_m), int(E.size), E.ctypes.data_as(dp),
+                      w.ctypes.data_as(dp), db.ctypes.data_as(dp), int(sv), int(max_batch), C.byref(o))
+    if st != 0:
+        msg = lib.epr_last_error(h).decode() if h.value else "invalid argument or unsupported size"
+        if h.value:
+            lib.epr_destroy(h)
+        raise EprError(st, msg)
+    return Plan(h, int(nx), int(ny), int(E.size), sv, int(max_batch))
+
+
+def epr_forward(plan, tau, P_sum, P_bins=None):
+    b = tau.shape[0]
+    plan._check(load_library().epr_forward(plan._h, b, _dev(tau, (b, plan.ny, plan.nx), "tau"),
+                                           _dev(P_sum, (b, plan.ny, plan.nx), "P_sum"),
+                                           _dev(P_bins, (b, plan.n_bins, plan.ny, plan.nx), "P_bins"), _stream()))
+
+
+def epr_adjoint(plan, e_bins, r_bins):
+    b = e_bins.shape[0]
+    sh = (b, plan.n_bins, plan.ny, plan.nx)
+    plan._check(load_library().epr_adjoint(plan._h, b, _dev(e_bins, sh, "e_bins"), _dev(r_bins, sh, "r_bins"), _stream()))
+
+
+def epr_transport(plan, I_bins, P_bins):
+    b = I_bins.shape[0]
+    sh = (b, plan.n_bins, plan.ny, plan.nx)
+    plan._check(load_library().epr_transport(plan._h, b, _dev(I_bins, sh, "I_bins"), _dev(P_bins, sh, "P_bins"), _stream()))
+
+
+def epr_precondition(plan, r_bins, q_bins):
+    b = r_bins.shape[0]
+    sh = (b, plan.n_bins, plan.ny, plan.nx)
+    plan._check(load_library().epr_precondition(plan._h, b, _dev(r_bins, sh, "r_bins"), _dev(q_bins, sh, "q_bins"), _stream()))
+
+
+def epr_retrieve(plan, d, out, iterations, step):
+    b = d.shape[0]
+    sh = (b, plan.ny, plan.nx)
+    plan._check(load_library().epr_retrieve(plan._h, b, _dev(d, sh, "d"), _dev(out, sh, "out"), int(iterations),
+                                            float(step), _stream()))
+
+
+def epr_retrieve_host(plan, d_host, out_host, iterations, step):
+    """HOST buffers (pinned float32 torch tensors or C-contiguous numpy arrays), copies inside the call."""
+    def hp(a, name):
+        if isinstance(a, np.ndarray):
+            if a.dtype != np.float32 or not a.flags.c_contiguous:
+                raise TypeError(f"{name}: expected C-contiguous float32")
+            return C.c_void_p(a.ctypes.data), a.shape
+        if a.is_cuda or a.dtype.is_floating_point is False or not a.is_contiguous():
+            raise TypeError(f"{name}: expected a contiguous float32 host tensor")
+        return C.c_void_p(a.data_ptr()), tuple(a.shape)
+    pd, sd = hp(d_host, "d_host")
+    po, so = hp(out_host, "out_host")
+    if tuple(sd) != tuple(so) or tuple(sd[1:]) != (plan.ny, plan.nx):
+        raise ValueError("d_host / out_host must both be [batch][ny][nx]")
+    plan._check(load_library().epr_retrieve_host(plan._h, int(sd[0]), pd, po, int(iterations), float(step)))

@@ -1,0 +1,363 @@
+// epr_api.cu — the C-ABI of include/epr.h: plan, operators, the retrieval loop, host-streaming wrapper.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <vector>
+
+#include "epr_internal.h"
+
+extern "C" int epr_fft_size_supported(int n);
+
+static const double HC_KEV_M = 1.2398419843e-9;
+
+#define FAIL(p, code, ...)                         \
+  do {                                             \
+    snprintf((p)->err, sizeof((p)->err), __VA_ARGS__); \
+    return (code);                                 \
+  } while (0)
+#define CU(p, call)                                                                     \
+  do {                                                                                  \
+    cudaError_t e_ = (call);                                                            \
+    if (e_ != cudaSuccess) FAIL(p, EPR_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+#define KL(p, call)      \
+  do {                   \
+    CU(p, call);         \
+    (p)->launches += 1;  \
+  } while (0)
+
+extern "C" void epr_default_options(epr_options* o) {
+  if (!o) return;
+  o->order = 2; o->wkb1 = 1; o->symbol = 0; o->max_shift_px = 16.f; o->i_min = 1e-6f; o->newton_iters = 4;
+  o->init = 0; o->output = 0; o->out_bin = 0; o->mu_rel = NULL;
+}
+
+extern "C" const char* epr_version(void) { return "epr-b200 0.1 (sm_100a)"; }
+
+extern "C" const char* epr_last_error(epr_plan_t p) { return p ? p->err : "null plan"; }
+
+extern "C" long long epr_launch_count(epr_plan_t p) { return p ? p->launches : 0; }
+
+template <typename T> static cudaError_t upload(T** dst, const std::vector<T>& v) {
+  cudaError_t e = cudaMalloc((void**)dst, v.size() * sizeof(T));
+  if (e != cudaSuccess) return e;
+  return cudaMemcpy(*dst, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice);
+}
+
+static std::vector<float2> twiddles(int n, int count) {
+  std::vector<float2> v(count);
+  for (int m = 0; m < count; ++m) {
+    const double th = -2.0 * M_PI * (double)m / (double)n;
+    v[m] = make_float2((float)cos(th), (float)sin(th));
+  }
+  return v;
+}
+
+static std::vector<float> lambda_table(int n, int count, int symbol) {
+  std::vector<float> v(count);
+  for (int k = 0; k < count; ++k) {
+    const int kk = (k <= n / 2) ? k : k - n;
+    const double th = 2.0 * M_PI * (double)kk / (double)n;
+    v[k] = (float)(symbol == 0 ? 2.0 - 2.0 * cos(th) : th * th);
+  }
+  return v;
+}
+
+extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, double L_m, int n_bins,
+                               const double* energy_keV, const double* weight, const double* delta_over_beta,
+                               epr_solver solver, int max_batch, const epr_options* opt) {
+  if (!out) return EPR_EINVAL;
+  *out = NULL;
+  if (!energy_keV || !weight || !delta_over_beta) return EPR_EINVAL;
+  if (n_bins < 1 || n_bins > EPR_MAX_BINS || max_batch < 1 || !(pixel_m > 0) || !(L_m > 0)) return EPR_EINVAL;
+  if (solver != EPR_LOCAL && solver != EPR_NONLOCAL) return EPR_EINVAL;
+  if (nx < 16 || ny < 16) return EPR_EINVAL;
+  double wsum = 0;
+  for (int s = 0; s < n_bins; ++s) {
+    if (!(energy_keV[s] > 0) || !(weight[s] > 0) || !(delta_over_beta[s] > 0)) return EPR_EINVAL;
+    wsum += weight[s];
+  }
+  epr_options o;
+  epr_default_options(&o);
+  if (opt) o = *opt;
+  if ((o.order != 1 && o.order != 2) || (o.symbol != 0 && o.symbol != 1) || !(o.max_shift_px >= 0) ||
+      o.max_shift_px > 30.f || !(o.i_min > 0) || o.newton_iters < 0 || o.newton_iters > 32 || o.output < 0 ||
+      o.output > 2 || o.out_bin < 0 || o.out_bin >= n_bins)
+    return EPR_EINVAL;
+  if (!epr_fft_size_supported(nx) || !epr_fft_size_supported(ny)) return EPR_ESIZE;
+
+  epr_plan_s* p = (epr_plan_s*)calloc(1, sizeof(epr_plan_s));
+  if (!p) return EPR_ENOMEM;
+  *out = p;                                   // returned even on failure so that the caller can read the message
+  p->nx = nx; p->ny = ny; p->n_bins = n_bins; p->max_batch = max_batch; p->solver = (int)solver; p->opt = o;
+  p->opt.mu_rel = NULL;
+
+  // per-line scalars: k_s = 2πE/(hc); α_s = L/(k_s p²) (Eq. (2)); a_s = α_s db_s/2 (Eq. (6));
+  // γ_s ∝ 1/(E_s db_s) normalised to Σ f γ = 1 (R11)
+  double gsum = 0;
+  for (int s = 0; s < n_bins; ++s) {
+    const double k = 2.0 * M_PI * energy_keV[s] / HC_KEV_M;
+    p->h_alpha[s] = L_m / (k * pixel_m * pixel_m);
+    p->h_db[s] = delta_over_beta[s];
+    p->h_a[s] = p->h_alpha[s] * delta_over_beta[s] / 2.0;
+    p->h_f[s] = weight[s] / wsum;
+    p->h_gamma[s] = o.mu_rel ? o.mu_rel[s] : 1.0 / (energy_keV[s] * delta_over_beta[s]);
+    if (!(p->h_gamma[s] > 0)) FAIL(p, EPR_EINVAL, "mu_rel must be positive");
+    gsum += p->h_f[s] * p->h_gamma[s];
+  }
+  EprLines& L = p->lines;
+  L.n_bins = n_bins;
+  double abar = 0;
+  for (int s = 0; s < n_bins; ++s) {
+    p->h_gamma[s] /= gsum;
+    L.f[s] = (float)p->h_f[s];
+    L.gamma[s] = (float)p->h_gamma[s];
+    L.a[s] = (float)p->h_a[s];
+    L.a2h[s] = (float)(0.5 * p->h_a[s] * p->h_a[s]);
+    L.q4[s] = (float)(0.25 * p->h_alpha[s] * p->h_alpha[s]);
+    // the device uses the fp32-rounded f_s consistently (deviation form): P_s − f_s with f_s = (float)
+    L.fixF[s] = (double)L.f[s] * EPR_FIX_ONE;
+    L.fixFi[s] = (unsigned)llrint(L.fixF[s]);
+    L.fixCorr[s] = (float)((double)L.fixFi[s] / EPR_FIX_ONE - (double)L.f[s]);
+    abar += p->h_f[s] * p->h_a[s];
+  }
+  L.abar = (float)abar;
+  double fs = 0;
+  for (int s = 0; s < n_bins; ++s) fs += (double)L.f[s];
+  L.fsum_dev = (float)(fs - 1.0);
+
+  const int M = nx / 2;
+  CU(p, upload(&p->tw_row, twiddles(M, M)));
+  CU(p, upload(&p->tw_r2c, twiddles(nx, M)));
+  CU(p, upload(&p->tw_col, twiddles(ny, ny)));
+  CU(p, upload(&p->lam_x, lambda_table(nx, M + 1, o.symbol)));
+  CU(p, upload(&p->lam_y, lambda_table(ny, ny, o.symbol)));
+
+  // workspaces, sized for `work` projections at a time (≤ max_batch; bounded so that they stay within ~12 GB)
+  const size_t plane = (size_t)nx * ny;
+  size_t per_proj = plane * sizeof(float) * ((size_t)n_bins * (solver == EPR_NONLOCAL ? 4 : 3) + 2);
+  int work = max_batch;
+  const char* env = getenv("EPR_WORK_BATCH");
+  size_t cap = (size_t)12 << 30;
+  if (per_proj * (size_t)work > cap) work = (int)(cap / per_proj);
+  if (env && atoi(env) > 0) work = atoi(env) < max_batch ? atoi(env) : max_batch;
+  if (work < 1) work = 1;
+  p->work_batch = work;
+  const size_t wb = (size_t)work;
+  cudaError_t e = cudaSuccess;
+  if (e == cudaSuccess) e = cudaMalloc((void**)&p->tau, wb * plane * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&p->pred, wb * n_bins * plane * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&p->res, wb * n_bins * plane * sizeof(float));
+  if (e == cudaSuccess && solver == EPR_NONLOCAL) e = cudaMalloc((void**)&p->res2, wb * n_bins * plane * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&p->spec, wb * n_bins * plane * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&p->spec_sum, wb * plane * sizeof(float));
+  if (e != cudaSuccess) FAIL(p, e == cudaErrorMemoryAllocation ? EPR_ENOMEM : EPR_ECUDA, "workspace: %s", cudaGetErrorString(e));
+  return EPR_OK;
+}
+
+extern "C" epr_status epr_plan_lines(epr_plan_t p, double* f, double* gamma, double* a, double* alpha) {
+  if (!p) return EPR_EINVAL;
+  for (int s = 0; s < p->n_bins; ++s) {
+    if (f) f[s] = p->h_f[s];
+    if (gamma) gamma[s] = p->h_gamma[s];
+    if (a) a[s] = p->h_a[s];
+    if (alpha) alpha[s] = p->h_alpha[s];
+  }
+  return EPR_OK;
+}
+
+extern "C" epr_status epr_destroy(epr_plan_t p) {
+  if (!p) return EPR_EINVAL;
+  cudaDeviceSynchronize();
+  cudaFree(p->tw_row); cudaFree(p->tw_r2c); cudaFree(p->tw_col); cudaFree(p->lam_x); cudaFree(p->lam_y);
+  cudaFree(p->tau); cudaFree(p->pred); cudaFree(p->res); cudaFree(p->res2); cudaFree(p->spec); cudaFree(p->spec_sum);
+  cudaFree(p->raymap);
+  for (int i = 0; i < 2; ++i) { cudaFree(p->stage_in[i]); cudaFree(p->stage_out[i]); }
+  for (int i = 0; i < 3; ++i) if (p->hstream[i]) cudaStreamDestroy(p->hstream[i]);
+  for (int i = 0; i < 6; ++i) if (p->hev[i]) cudaEventDestroy(p->hev[i]);
+  free(p);
+  return EPR_OK;
+}
+
+static epr_status check_call(epr_plan_t p, int batch) {
+  if (!p) return EPR_EINVAL;
+  if (batch < 1 || batch > p->max_batch) FAIL(p, EPR_EINVAL, "batch %d outside [1, max_batch = %d]", batch, p->max_batch);
+  return EPR_OK;
+}
+
+// ----------------------------------------------------------------------------------------------- operators
+static epr_status ensure_raymap(epr_plan_t p) {
+  if (p->raymap) return EPR_OK;
+  const size_t n = (size_t)p->work_batch * p->n_bins * p->nx * p->ny;
+  cudaError_t e = cudaMalloc((void**)&p->raymap, n * sizeof(float2));
+  if (e != cudaSuccess) FAIL(p, EPR_ENOMEM, "ray map storage: %s", cudaGetErrorString(e));
+  return EPR_OK;
+}
+
+extern "C" epr_status epr_forward(epr_plan_t p, int batch, const float* tau, float* P_sum, float* P_bins, void* stream) {
+  epr_status st = check_call(p, batch);
+  if (st != EPR_OK) return st;
+  if (!tau || !P_sum) FAIL(p, EPR_EINVAL, "epr_forward: NULL tau or P_sum");
+  if (batch > p->work_batch) FAIL(p, EPR_EINVAL, "epr_forward: batch %d exceeds the plan's work batch %d", batch, p->work_batch);
+  cudaStream_t cs = (cudaStream_t)stream;
+  const size_t plane = (size_t)p->nx * p->ny;
+  if (p->solver == EPR_LOCAL) {
+    KL(p, epr_launch_forward_local(p, batch, tau, p->pred, cs));
+    KL(p, epr_launch_pred_out(p, batch, p->pred, 0, 0, P_sum, P_bins, cs));
+  } else {
+    if ((st = ensure_raymap(p)) != EPR_OK) return st;
+    CU(p, epr_launch_zero(p->pred, (size_t)batch * p->n_bins * plane * sizeof(unsigned), cs));
+    KL(p, epr_launch_splat(p, batch, tau, NULL, NULL, p->raymap, (unsigned*)p->pred, cs));
+    KL(p, epr_launch_pred_out(p, batch, p->pred, 1, 0, P_sum, P_bins, cs));
+    p->raymap_batch = batch;
+  }
+  return EPR_OK;
+}
+
+extern "C" epr_status epr_adjoint(epr_plan_t p, int batch, const float* e_bins, float* r_bins, void* stream) {
+  epr_status st = check_call(p, batch);
+  if (st != EPR_OK) return st;
+  if (!e_bins || !r_bins) FAIL(p, EPR_EINVAL, "epr_adjoint: NULL pointer");
+  cudaStream_t cs = (cudaStream_t)stream;
+  const size_t n = (size_t)batch * p->n_bins * p->nx * p->ny;
+  if (p->solver == EPR_LOCAL) {
+    if (e_bins != r_bins) CU(p, cudaMemcpyAsync(r_bins, e_bins, n * sizeof(float), cudaMemcpyDeviceToDevice, cs));
+    return EPR_OK;
+  }
+  if (e_bins == r_bins) FAIL(p, EPR_EINVAL, "epr_adjoint: the gather cannot run in place");
+  if (!p->raymap || p->raymap_batch < batch) FAIL(p, EPR_EINVAL, "epr_adjoint: no ray map stored for batch %d (call epr_forward first)", batch);
+  KL(p, epr_launch_gather(p, batch, NULL, p->raymap, e_bins, r_bins, cs));
+  return EPR_OK;
+}
+
+extern "C" epr_status epr_transport(epr_plan_t p, int batch, const float* I_bins, float* P_bins, void* stream) {
+  epr_status st = check_call(p, batch);
+  if (st != EPR_OK) return st;
+  if (!I_bins || !P_bins) FAIL(p, EPR_EINVAL, "epr_transport: NULL pointer");
+  if (p->solver != EPR_NONLOCAL) FAIL(p, EPR_EINVAL, "epr_transport: non-local plans only");
+  if (!p->raymap || p->raymap_batch < batch) FAIL(p, EPR_EINVAL, "epr_transport: no ray map stored for batch %d (call epr_forward first)", batch);
+  cudaStream_t cs = (cudaStream_t)stream;
+  const size_t plane = (size_t)p->nx * p->ny;
+  CU(p, epr_launch_zero(p->pred, (size_t)batch * p->n_bins * plane * sizeof(unsigned), cs));
+  KL(p, epr_launch_splat(p, batch, NULL, I_bins, p->raymap, NULL, (unsigned*)p->pred, cs));
+  KL(p, epr_launch_pred_out(p, batch, p->pred, 1, 1, NULL, P_bins, cs));
+  return EPR_OK;
+}
+
+extern "C" epr_status epr_precondition(epr_plan_t p, int batch, const float* r_bins, float* q_bins, void* stream) {
+  epr_status st = check_call(p, batch);
+  if (st != EPR_OK) return st;
+  if (!r_bins || !q_bins) FAIL(p, EPR_EINVAL, "epr_precondition: NULL pointer");
+  cudaStream_t cs = (cudaStream_t)stream;
+  const size_t plane = (size_t)p->nx * p->ny;
+  for (int b0 = 0; b0 < batch; b0 += p->work_batch) {
+    const int nb = (batch - b0 < p->work_batch) ? batch - b0 : p->work_batch;
+    const int planes = nb * p->n_bins;
+    const size_t off = (size_t)b0 * p->n_bins * plane;
+    KL(p, epr_launch_rows_r2c(p, planes, r_bins + off, 0.f, p->spec, cs));
+    KL(p, epr_launch_cols(p, planes, 0, p->spec, p->spec, cs));
+    KL(p, epr_launch_rows_c2r(p, planes, p->spec, 0, 1.f, 0, q_bins + off, cs));
+  }
+  return EPR_OK;
+}
+
+// ----------------------------------------------------------------------------------------------- the loop
+// One pass over `nb` ≤ work_batch projections.  tau is the state (device, [nb][ny][nx]).
+static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* tau, int iterations, float step,
+                                 cudaStream_t cs) {
+  const size_t plane = (size_t)p->nx * p->ny;
+  const int planes = nb * p->n_bins;
+  if (p->opt.init == 0) {
+    // initial guess (R9): τ⁰ = project( max(IFFT(FFT(d)/(1+āλ)), i_min) ), in deviation form from d − 1
+    KL(p, epr_launch_rows_r2c(p, nb, d, -1.f, p->spec, cs));
+    KL(p, epr_launch_cols(p, nb, 2, p->spec, p->spec_sum, cs));
+    KL(p, epr_launch_rows_c2r(p, nb, p->spec_sum, 1, 1.f, 1, tau, cs));
+  }
+  for (int it = 0; it < iterations; ++it) {
+    const float* r;
+    if (p->solver == EPR_LOCAL) {
+      KL(p, epr_launch_forward_local(p, nb, tau, p->pred, cs));                 // a0 + a1-L
+      KL(p, epr_launch_residual(p, nb, d, p->pred, 0, p->res, cs));             // a2 (a3 = identity)
+      r = p->res;
+    } else {
+      CU(p, epr_launch_zero(p->pred, (size_t)planes * plane * sizeof(unsigned), cs));
+      KL(p, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, (unsigned*)p->pred, cs));   // a0 + a1-N
+      KL(p, epr_launch_residual(p, nb, d, p->pred, 1, p->res, cs));             // a2
+      KL(p, epr_launch_gather(p, nb, tau, NULL, p->res, p->res2, cs));          // a3
+      r = p->res2;
+    }
+    KL(p, epr_launch_rows_r2c(p, planes, r, 0.f, p->spec, cs));                 // a4
+    KL(p, epr_launch_cols(p, planes, 1, p->spec, p->spec_sum, cs));             // a4 (Σ_s in Fourier space, R10)
+    KL(p, epr_launch_rows_c2r(p, nb, p->spec_sum, 1, step, 0, tau, cs));        // a4 + a5 + a6
+  }
+  return EPR_OK;
+}
+
+static epr_status retrieve_device(epr_plan_t p, int batch, const float* d, float* out, int iterations, float step,
+                                  cudaStream_t cs) {
+  const size_t plane = (size_t)p->nx * p->ny;
+  for (int b0 = 0; b0 < batch; b0 += p->work_batch) {
+    const int nb = (batch - b0 < p->work_batch) ? batch - b0 : p->work_batch;
+    float* o = out + (size_t)b0 * plane;
+    float* tau = (p->opt.output == 0) ? o : p->tau;
+    if (p->opt.init == 1 && tau != o) CU(p, cudaMemcpyAsync(tau, o, (size_t)nb * plane * sizeof(float), cudaMemcpyDeviceToDevice, cs));
+    epr_status st = retrieve_chunk(p, nb, d + (size_t)b0 * plane, tau, iterations, step, cs);
+    if (st != EPR_OK) return st;
+    if (p->opt.output != 0) KL(p, epr_launch_output(p, nb, tau, o, cs));
+  }
+  return EPR_OK;
+}
+
+extern "C" epr_status epr_retrieve(epr_plan_t p, int batch, const float* d, float* out, int iterations, float step,
+                                   void* stream) {
+  epr_status st = check_call(p, batch);
+  if (st != EPR_OK) return st;
+  if (!d || !out) FAIL(p, EPR_EINVAL, "epr_retrieve: NULL pointer");
+  if (iterations < 0 || !(step > 0.f)) FAIL(p, EPR_EINVAL, "epr_retrieve: iterations must be >= 0 and step > 0");
+  return retrieve_device(p, batch, d, out, iterations, step, (cudaStream_t)stream);
+}
+
+extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_host, float* out_host, int iterations,
+                                        float step) {
+  if (!p) return EPR_EINVAL;
+  if (batch < 1 || !d_host || !out_host) FAIL(p, EPR_EINVAL, "epr_retrieve_host: bad batch or NULL pointer");
+  if (iterations < 0 || !(step > 0.f)) FAIL(p, EPR_EINVAL, "epr_retrieve_host: iterations must be >= 0 and step > 0");
+  const size_t plane = (size_t)p->nx * p->ny;
+  const int wbch = p->work_batch;
+  if (!p->stage_in[0]) {
+    for (int i = 0; i < 2; ++i) {
+      CU(p, cudaMalloc((void**)&p->stage_in[i], (size_t)wbch * plane * sizeof(float)));
+      CU(p, cudaMalloc((void**)&p->stage_out[i], (size_t)wbch * plane * sizeof(float)));
+    }
+    for (int i = 0; i < 3; ++i) CU(p, cudaStreamCreateWithFlags(&p->hstream[i], cudaStreamNonBlocking));
+    for (int i = 0; i < 6; ++i) CU(p, cudaEventCreateWithFlags(&p->hev[i], cudaEventDisableTiming));
+  }
+  cudaStream_t s_in = p->hstream[0], s_cmp = p->hstream[1], s_out = p->hstream[2];
+  int chunk = 0;
+  for (int b0 = 0; b0 < batch; b0 += wbch, ++chunk) {
+    const int nb = (batch - b0 < wbch) ? batch - b0 : wbch;
+    const int buf = chunk & 1;
+    cudaEvent_t ev_in = p->hev[buf * 3 + 0], ev_cmp = p->hev[buf * 3 + 1], ev_out = p->hev[buf * 3 + 2];
+    const size_t bytes = (size_t)nb * plane * sizeof(float);
+    if (chunk >= 2) {                       // buffers of chunk-2 must be free: its compute read stage_in, its D2H read stage_out
+      CU(p, cudaStreamWaitEvent(s_in, ev_cmp, 0));
+      CU(p, cudaStreamWaitEvent(s_cmp, ev_out, 0));
+    }
+    CU(p, cudaMemcpyAsync(p->stage_in[buf], d_host + (size_t)b0 * plane, bytes, cudaMemcpyHostToDevice, s_in));
+    if (p->opt.init == 1)
+      CU(p, cudaMemcpyAsync(p->stage_out[buf], out_host + (size_t)b0 * plane, bytes, cudaMemcpyHostToDevice, s_in));
+    CU(p, cudaEventRecord(ev_in, s_in));
+    CU(p, cudaStreamWaitEvent(s_cmp, ev_in, 0));
+    epr_status st = retrieve_device(p, nb, p->stage_in[buf], p->stage_out[buf], iterations, step, s_cmp);
+    if (st != EPR_OK) return st;
+    CU(p, cudaEventRecord(ev_cmp, s_cmp));
+    CU(p, cudaStreamWaitEvent(s_out, ev_cmp, 0));
+    CU(p, cudaMemcpyAsync(out_host + (size_t)b0 * plane, p->stage_out[buf], bytes, cudaMemcpyDeviceToHost, s_out));
+    CU(p, cudaEventRecord(ev_out, s_out));
+  }
+  CU(p, cudaStreamSynchronize(s_out));
+  CU(p, cudaStreamSynchronize(s_cmp));
+  return EPR_OK;
+}

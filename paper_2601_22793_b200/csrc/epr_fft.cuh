@@ -1,0 +1,157 @@
+// epr_fft.cuh — shared-memory mixed-radix Stockham FFT engine (radices 16/8/4/2/5/3), sm_100a.
+//
+// Used by the FFT-diagonal Paganin-type preconditioner P^{-1}_{1,s}: row R2C,
+// column FFT · H_s · column IFFT, row C2R.  The data of one transform live in shared memory as float2
+// at  s[pad(i) * STRIDE + off];  each pass is done by TPC cooperating threads which hold their
+// butterflies in registers (read all → barrier → write all → barrier), so no ping-pong buffer is needed.
+// Natural order in, natural order out (autosort).  Forward sign e^{-i…}; INV gives the unnormalised inverse.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace eprfft {
+
+__host__ __device__ constexpr int pick_radix(int rem) {
+  return (rem % 16 == 0) ? 16 : (rem % 8 == 0) ? 8 : (rem % 4 == 0) ? 4 : (rem % 2 == 0) ? 2
+       : (rem % 5 == 0) ? 5 : (rem % 3 == 0) ? 3 : 0;
+}
+__host__ __device__ constexpr bool supported(int n) {
+  while (n > 1) { int r = pick_radix(n); if (!r) return false; n /= r; }
+  return true;
+}
+// shared-memory padding: one extra element every 16 keeps stride-R first-pass writes off a single bank
+__host__ __device__ constexpr int padi(int i) { return i + (i >> 4); }
+__host__ __device__ constexpr int padded_len(int n) { return padi(n - 1) + 1; }
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+  return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+}
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+template <bool INV> __device__ __forceinline__ float2 rot90(float2 a) {   // multiply by -i (fwd) / +i (inv)
+  return INV ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
+}
+template <bool INV> __device__ __forceinline__ float2 conj_if(float2 a) { return INV ? make_float2(a.x, -a.y) : a; }
+
+template <bool INV> __device__ __forceinline__ void dft2(float2* v) {
+  float2 a = v[0], b = v[1];
+  v[0] = cadd(a, b); v[1] = csub(a, b);
+}
+template <bool INV> __device__ __forceinline__ void dft4(float2& a0, float2& a1, float2& a2, float2& a3) {
+  float2 t0 = cadd(a0, a2), t1 = csub(a0, a2), t2 = cadd(a1, a3), t3 = rot90<INV>(csub(a1, a3));
+  a0 = cadd(t0, t2); a2 = csub(t0, t2); a1 = cadd(t1, t3); a3 = csub(t1, t3);
+}
+template <bool INV> __device__ __forceinline__ void dft3(float2* v) {
+  const float s = INV ? 0.86602540378443864676f : -0.86602540378443864676f;   // Im of w3
+  float2 t = cadd(v[1], v[2]), d = csub(v[1], v[2]);
+  float2 m = make_float2(fmaf(-0.5f, t.x, v[0].x), fmaf(-0.5f, t.y, v[0].y));
+  float2 r = make_float2(-s * d.y, s * d.x);                                  // i*s*d
+  v[0] = cadd(v[0], t); v[1] = cadd(m, r); v[2] = csub(m, r);
+}
+template <bool INV> __device__ __forceinline__ void dft5(float2* v) {
+  const float c1 = 0.30901699437494742410f, c2 = -0.80901699437494742410f;
+  const float s1 = INV ? 0.95105651629515357212f : -0.95105651629515357212f;
+  const float s2 = INV ? 0.58778525229247312917f : -0.58778525229247312917f;
+  float2 a = cadd(v[1], v[4]), b = csub(v[1], v[4]), c = cadd(v[2], v[3]), d = csub(v[2], v[3]);
+  float2 m1 = make_float2(v[0].x + c1 * a.x + c2 * c.x, v[0].y + c1 * a.y + c2 * c.y);
+  float2 m2 = make_float2(v[0].x + c2 * a.x + c1 * c.x, v[0].y + c2 * a.y + c1 * c.y);
+  float2 r1 = make_float2(-(s1 * b.y + s2 * d.y), s1 * b.x + s2 * d.x);       // i*(s1 b + s2 d)
+  float2 r2 = make_float2(-(s2 * b.y - s1 * d.y), s2 * b.x - s1 * d.x);       // i*(s2 b - s1 d)
+  v[0] = cadd(v[0], cadd(a, c));
+  v[1] = cadd(m1, r1); v[4] = csub(m1, r1); v[2] = cadd(m2, r2); v[3] = csub(m2, r2);
+}
+template <bool INV> __device__ __forceinline__ void dft8(float2* v) {
+  const float h = 0.70710678118654752440f;
+  float2 e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1], o1 = v[3], o2 = v[5], o3 = v[7];
+  dft4<INV>(e0, e1, e2, e3);
+  dft4<INV>(o0, o1, o2, o3);
+  // o_k *= w8^k, w8 = e^{∓iπ/4}
+  float2 p1 = INV ? make_float2(h * (o1.x - o1.y), h * (o1.x + o1.y)) : make_float2(h * (o1.x + o1.y), h * (o1.y - o1.x));
+  float2 p2 = rot90<INV>(o2);
+  float2 p3 = INV ? make_float2(-h * (o3.x + o3.y), h * (o3.x - o3.y)) : make_float2(h * (o3.y - o3.x), -h * (o3.x + o3.y));
+  v[0] = cadd(e0, o0); v[4] = csub(e0, o0);
+  v[1] = cadd(e1, p1); v[5] = csub(e1, p1);
+  v[2] = cadd(e2, p2); v[6] = csub(e2, p2);
+  v[3] = cadd(e3, p3); v[7] = csub(e3, p3);
+}
+template <bool INV> __device__ __forceinline__ void dft16(float2* v) {
+  // X[k1 + 4 k2] = Σ_{n2} w16^{n2 k1} ( Σ_{n1} x[4 n1 + n2] w4^{n1 k1} ) w4^{n2 k2}
+  const float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f, h = 0.70710678118654752440f;
+#pragma unroll
+  for (int n2 = 0; n2 < 4; ++n2) dft4<INV>(v[n2], v[4 + n2], v[8 + n2], v[12 + n2]);   // v[4 k1 + n2] = Y[n2][k1]
+  // twiddles w16^{n2 k1}, w16 = e^{∓iπ/8}
+  const float2 w1 = conj_if<INV>(make_float2(c1, -s1)), w2 = conj_if<INV>(make_float2(h, -h)),
+               w3 = conj_if<INV>(make_float2(s1, -c1)), w6 = conj_if<INV>(make_float2(-h, -h)),
+               w9 = conj_if<INV>(make_float2(-c1, s1));
+  v[4 + 1] = cmul(v[4 + 1], w1); v[4 + 2] = cmul(v[4 + 2], w2); v[4 + 3] = cmul(v[4 + 3], w3);
+  v[8 + 1] = cmul(v[8 + 1], w2); v[8 + 2] = rot90<INV>(v[8 + 2]); v[8 + 3] = cmul(v[8 + 3], w6);
+  v[12 + 1] = cmul(v[12 + 1], w3); v[12 + 2] = cmul(v[12 + 2], w6); v[12 + 3] = cmul(v[12 + 3], w9);
+#pragma unroll
+  for (int k1 = 0; k1 < 4; ++k1) dft4<INV>(v[4 * k1], v[4 * k1 + 1], v[4 * k1 + 2], v[4 * k1 + 3]);   // → v[4 k1 + k2]
+  // natural order X[k1 + 4 k2] ← v[4 k1 + k2]: transpose the 4x4
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = i + 1; j < 4; ++j) { float2 t = v[4 * i + j]; v[4 * i + j] = v[4 * j + i]; v[4 * j + i] = t; }
+}
+template <int R, bool INV> __device__ __forceinline__ void dft(float2* v) {
+  if constexpr (R == 2) dft2<INV>(v);
+  else if constexpr (R == 3) dft3<INV>(v);
+  else if constexpr (R == 4) dft4<INV>(v[0], v[1], v[2], v[3]);
+  else if constexpr (R == 5) dft5<INV>(v);
+  else if constexpr (R == 8) dft8<INV>(v);
+  else dft16<INV>(v);
+}
+
+// One Stockham pass of radix R with P = product of the previous radices.
+template <int N, int P, int R, int TPC, int STRIDE, bool INV>
+__device__ __forceinline__ void pass(float2* s, int off, int t, const float2* __restrict__ tw) {
+  constexpr int T = N / R;
+  constexpr int CNT = (T + TPC - 1) / TPC;
+  float2 u[CNT][R];
+#pragma unroll
+  for (int c = 0; c < CNT; ++c) {
+    const int j = t + c * TPC;
+    if (CNT * TPC == T || j < T) {
+#pragma unroll
+      for (int r = 0; r < R; ++r) u[c][r] = s[padi(j + r * T) * STRIDE + off];
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int c = 0; c < CNT; ++c) {
+    const int j = t + c * TPC;
+    if (CNT * TPC == T || j < T) {
+      const int k = (P == 1) ? 0 : (j % P);
+      if constexpr (P > 1) {
+        constexpr int TWS = N / (P * R);
+#pragma unroll
+        for (int r = 1; r < R; ++r) u[c][r] = cmul(u[c][r], conj_if<INV>(__ldg(&tw[r * k * TWS])));
+      }
+      dft<R, INV>(u[c]);
+      const int j0 = (j - k) * R + k;
+#pragma unroll
+      for (int q = 0; q < R; ++q) s[padi(j0 + q * P) * STRIDE + off] = u[c][q];
+    }
+  }
+  __syncthreads();
+}
+
+template <int N, int P, int TPC, int STRIDE, bool INV>
+__device__ __forceinline__ void passes(float2* s, int off, int t, const float2* __restrict__ tw) {
+  if constexpr (P < N) {
+    constexpr int R = pick_radix(N / P);
+    static_assert(R != 0, "unsupported FFT length");
+    pass<N, P, R, TPC, STRIDE, INV>(s, off, t, tw);
+    passes<N, P * R, TPC, STRIDE, INV>(s, off, t, tw);
+  }
+}
+
+// In-place length-N transform of the sequence s[padi(i)*STRIDE + off], done by TPC threads (t = 0..TPC-1).
+// Must be called by every thread of the CTA (it contains __syncthreads); the data must be visible
+// (barrier) before the call and are visible after it.  tw[m] = exp(-2πi m/N), m < N.
+template <int N, int TPC, int STRIDE, bool INV>
+__device__ __forceinline__ void fft_smem(float2* s, int off, int t, const float2* __restrict__ tw) {
+  passes<N, 1, TPC, STRIDE, INV>(s, off, t, tw);
+}
+
+}  // namespace eprfft

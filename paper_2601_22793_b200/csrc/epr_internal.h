@@ -1,0 +1,78 @@
+// epr_internal.h — plan layout and launcher prototypes shared by the C-ABI and the kernels.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/epr.h"
+
+#define EPR_MAX_BINS 16
+#define EPR_FIX_BITS 26                       /* splat accumulators: u32 fixed point, 1.0 = 2^26 */
+#define EPR_FIX_ONE 67108864.0                /* 2^26 */
+
+// Per-line scalars, passed to kernels by value (fits the 4 KB parameter space).
+struct EprLines {
+  int n_bins;
+  float f[EPR_MAX_BINS];        // spectral fraction f_s                       Eq. (7)
+  float gamma[EPR_MAX_BINS];    // attenuation scaling γ_s                      Eq. (7)
+  float a[EPR_MAX_BINS];        // a_s = α_s db_s / 2                           Eq. (1)+(6)
+  float a2h[EPR_MAX_BINS];      // a_s² / 2                                     Eq. (1) WKB0
+  float q4[EPR_MAX_BINS];       // α_s² / 4                                     Eq. (1) WKB1
+  double fixF[EPR_MAX_BINS];    // f_s · 2^26 (double, for the splat)
+  unsigned fixFi[EPR_MAX_BINS]; // rint(f_s · 2^26)
+  float fixCorr[EPR_MAX_BINS];  // rint(f_s 2^26)·2^-26 − f_s
+  float abar;                   // Σ f_s a_s (initial guess, R9)
+  float fsum_dev;               // Σ_s (float)f_s − 1: rounding of the fp32 fractions, removed from the residual
+};
+
+struct epr_plan_s {
+  int nx, ny, n_bins, max_batch;
+  int work_batch;              // projections processed per pass of the loop (workspaces are sized for it)
+  int solver;                  // EPR_LOCAL / EPR_NONLOCAL
+  epr_options opt;
+  double h_f[EPR_MAX_BINS], h_gamma[EPR_MAX_BINS], h_a[EPR_MAX_BINS], h_alpha[EPR_MAX_BINS], h_db[EPR_MAX_BINS];
+  EprLines lines;
+  // tables
+  float2* tw_row;              // exp(-2πi m/(nx/2)), m < nx/2
+  float2* tw_r2c;              // exp(-2πi k/nx),     k < nx/2
+  float2* tw_col;              // exp(-2πi m/ny),     m < ny
+  float* lam_x;                // λ_x[kx], kx = 0..nx/2
+  float* lam_y;                // λ_y[ky], ky < ny
+  // workspaces (sized for max_batch)
+  float* tau;                  // [work_batch][ny][nx]        state τ (when `out` is not τ) / scratch
+  float* pred;                 // [work_batch][n_bins][ny][nx] float: P_s − f_s (local) ; u32 fixed point (non-local)
+  float* res;                  // [work_batch][n_bins][ny][nx] e_s then r_s
+  float* res2;                 // [work_batch][n_bins][ny][nx] r_s (non-local gather output)
+  float2* spec;                // [work_batch][n_bins][ny][nx/2] half spectra (packed Nyquist)
+  float2* spec_sum;            // [work_batch][ny][nx/2]
+  float2* raymap;              // [work_batch][n_bins][ny][nx] stored u_s (lazy, epr_forward non-local)
+  int raymap_batch;            // batch of the stored map (0 = none)
+  // host staging for epr_retrieve_host
+  float* stage_in[2];
+  float* stage_out[2];
+  cudaStream_t hstream[3];     // copy-in, compute, copy-out
+  cudaEvent_t hev[6];          // per buffer: in-done, compute-done, out-done
+  long long launches;
+  char err[256];
+};
+
+// ---- launchers (epr_kernels.cu / epr_fftk.cu); all return cudaGetLastError() ----
+// planes = batch * n_bins unless stated.
+cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float* tau, float* pred, cudaStream_t st);
+cudaError_t epr_launch_splat(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
+                             float2* map_out, unsigned* pfix, cudaStream_t st);
+cudaError_t epr_launch_residual(const epr_plan_s* p, int batch, const float* d, const void* pred, int fixed,
+                                float* es, cudaStream_t st);
+cudaError_t epr_launch_pred_out(const epr_plan_s* p, int batch, const void* pred, int fixed, int linear, float* P_sum,
+                                float* P_bins, cudaStream_t st);
+cudaError_t epr_launch_gather(const epr_plan_s* p, int batch, const float* tau, const float2* map_in, const float* es,
+                              float* r, cudaStream_t st);
+cudaError_t epr_launch_rows_r2c(const epr_plan_s* p, int planes, const float* in, float in_offset, float2* spec,
+                                cudaStream_t st);
+// mode 0: per-plane filter with bin = plane % n_bins (out has `planes` planes);
+// mode 1: sum over bins (out has planes / n_bins planes);  mode 2: single filter with abar (init).
+cudaError_t epr_launch_cols(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st);
+// epilogue 0: write q; 1: τ update (Newton projection) with step; init0: treat τ as 0 (initial guess)
+cudaError_t epr_launch_rows_c2r(const epr_plan_s* p, int planes, const float2* spec, int epilogue, float step,
+                                int tau_is_zero, float* q_or_tau, cudaStream_t st);
+cudaError_t epr_launch_output(const epr_plan_s* p, int batch, const float* tau, float* out, cudaStream_t st);
+cudaError_t epr_launch_zero(void* ptr, size_t bytes, cudaStream_t st);

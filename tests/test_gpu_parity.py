@@ -1,0 +1,225 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the fp64 oracle, element by element, on the
+same seeded inputs.  Tolerances are north_star's: per-operator relative L2 <= 1e-5, retrieved phase <= 1e-4,
+splat mass conservation <= 1e-6 relative."""
+import numpy as np
+import pytest
+
+from epr_inputs import make_workload
+from oracle import epr_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+TOL_OP = 1e-5
+TOL_PHASE = 1e-4
+TOL_MASS = 1e-6
+
+
+def rel_l2(got, ref):
+    got = np.asarray(got, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    return float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
+
+
+@pytest.fixture(scope="module")
+def E():
+    import torch
+    import paper_2601_22793_b200 as epr
+    assert torch.cuda.is_available()
+    epr.load_library()
+    return epr
+
+
+def _dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def _tau_field(ny, nx, seed, amp=0.05):
+    """Smooth + rough thickness-like field (fp32-representable)."""
+    rng = np.random.default_rng(seed)
+    y, x = np.meshgrid(np.arange(ny) * 2 * np.pi / ny, np.arange(nx) * 2 * np.pi / nx, indexing="ij")
+    t = amp * (1.2 + np.cos(2 * x + 0.3) * np.sin(3 * y) + 0.5 * np.cos(5 * x - 4 * y))
+    t += 0.02 * amp * rng.normal(size=(ny, nx))
+    return t.astype(np.float32)
+
+
+POLY = dict(energy=np.linspace(60.0, 140.0, 8), weight=np.exp(-0.5 * ((np.linspace(60.0, 140.0, 8) - 100.0) / 20.0) ** 2))
+SPECTRA = {
+    "mono": (np.array([100.0]), np.array([1.0]), np.array([1000.0])),
+    "poly8": (POLY["energy"], POLY["weight"], 200.0 * POLY["energy"] / 100.0),
+    "poly3_unequal_a": (np.array([70.0, 100.0, 130.0]), np.array([0.3, 0.4, 0.3]), np.array([900.0, 1000.0, 1100.0])),
+}
+SIZES = [(256, 256), (48, 80), (160, 96), (320, 512)]          # (ny, nx): powers of two and radix-3/5 lengths
+
+
+@pytest.mark.parametrize("ny,nx", SIZES)
+@pytest.mark.parametrize("spec", ["mono", "poly3_unequal_a"])
+@pytest.mark.parametrize("symbol", [0, 1])
+def test_precondition(E, ny, nx, spec, symbol):
+    import torch
+    en, w, db = SPECTRA[spec]
+    L = 3.0
+    plan = E.epr_plan(nx, ny, 6.5e-6, L, en, w, db, "local", max_batch=2, symbol=symbol)
+    lines = O.derive_lines(6.5e-6, L, en, w, db)
+    rng = np.random.default_rng(5)
+    r = rng.normal(size=(2, len(en), ny, nx)).astype(np.float32)
+    q = torch.empty_like(_dev(r))
+    E.epr_precondition(plan, _dev(r), q)
+    q = q.cpu().numpy()
+    for b in range(2):
+        for s in range(len(en)):
+            ref = O.precondition(r[b, s].astype(np.float64), lines.a[s], symbol)
+            assert rel_l2(q[b, s], ref) < TOL_OP
+    plan.destroy()
+
+
+@pytest.mark.parametrize("ny,nx", [(256, 256), (160, 96)])
+@pytest.mark.parametrize("spec", ["mono", "poly8"])
+@pytest.mark.parametrize("order,wkb1", [(2, 1), (2, 0), (1, 0)])
+def test_forward_local(E, ny, nx, spec, order, wkb1):
+    import torch
+    en, w, db = SPECTRA[spec]
+    L = 2.0
+    plan = E.epr_plan(nx, ny, 6.5e-6, L, en, w, db, "local", max_batch=2, order=order, wkb1=wkb1)
+    lines = O.derive_lines(6.5e-6, L, en, w, db)
+    tau = np.stack([_tau_field(ny, nx, 1), _tau_field(ny, nx, 2, amp=0.3)])
+    P = torch.empty((2, ny, nx), device="cuda")
+    Pb = torch.empty((2, len(en), ny, nx), device="cuda")
+    E.epr_forward(plan, _dev(tau), P, Pb)
+    P, Pb = P.cpu().numpy(), Pb.cpu().numpy()
+    for b in range(2):
+        ref, ref_bins, _ = O.forward(tau[b].astype(np.float64), lines, "local", order=order, wkb1=bool(wkb1))
+        assert rel_l2(P[b], ref) < TOL_OP
+        assert rel_l2(P[b] - 1.0, ref - 1.0) < 20 * TOL_OP       # the propagation signal itself
+        for s in range(len(en)):
+            assert rel_l2(Pb[b, s], ref_bins[s]) < TOL_OP
+    plan.destroy()
+
+
+@pytest.mark.parametrize("ny,nx", [(256, 256), (160, 96)])
+@pytest.mark.parametrize("spec,L", [("mono", 30.0), ("poly8", 60.0)])
+def test_forward_nonlocal_splat_mass_and_adjoint(E, ny, nx, spec, L):
+    import torch
+    en, w, db = SPECTRA[spec]
+    nb = len(en)
+    S = 12.0
+    plan = E.epr_plan(nx, ny, 6.5e-6, L, en, w, db, "nonlocal", max_batch=2, max_shift_px=S)
+    lines = O.derive_lines(6.5e-6, L, en, w, db)
+    tau = np.stack([_tau_field(ny, nx, 3, amp=0.2), _tau_field(ny, nx, 4, amp=0.6)])
+    P = torch.empty((2, ny, nx), device="cuda")
+    Pb = torch.empty((2, nb, ny, nx), device="cuda")
+    E.epr_forward(plan, _dev(tau), P, Pb)
+    Ph, Pbh = P.cpu().numpy(), Pb.cpu().numpy()
+    rng = np.random.default_rng(9)
+    e = rng.normal(size=(2, nb, ny, nx)).astype(np.float32)
+    x = rng.uniform(0.0, 2.0, size=(2, nb, ny, nx)).astype(np.float32)
+    r = torch.empty_like(Pb)
+    E.epr_adjoint(plan, _dev(e), r)
+    Mx = torch.empty_like(Pb)
+    E.epr_transport(plan, _dev(x), Mx)
+    rh, Mxh = r.cpu().numpy(), Mx.cpu().numpy()
+    saw_multi_pixel = False
+    for b in range(2):
+        ref, ref_bins, maps = O.forward(tau[b].astype(np.float64), lines, "nonlocal", S=S)
+        Is = O.line_intensities(tau[b].astype(np.float64), lines)
+        assert rel_l2(Ph[b], ref) < TOL_OP
+        for s in range(nb):
+            saw_multi_pixel |= max(np.abs(maps[s][0]).max(), np.abs(maps[s][1]).max()) > 2.0
+            assert rel_l2(Pbh[b, s], ref_bins[s]) < TOL_OP
+            # mass conservation of the GPU splat (north_star: <= 1e-6 relative)
+            assert abs(Pbh[b, s].astype(np.float64).sum() - Is[s].sum()) <= TOL_MASS * Is[s].sum()
+            assert rel_l2(rh[b, s], O.gather(e[b, s].astype(np.float64), *maps[s])) < TOL_OP
+            assert rel_l2(Mxh[b, s], O.splat(x[b, s].astype(np.float64), *maps[s])) < TOL_OP
+        # <Mx, y> = <x, M*y> on the device results
+        lhs = float(np.sum(Mxh[b].astype(np.float64) * e[b]))
+        rhs = float(np.sum(x[b].astype(np.float64) * rh[b]))
+        assert abs(lhs - rhs) <= 1e-5 * np.sqrt(np.sum(Mxh[b].astype(np.float64) ** 2) * np.sum(e[b].astype(np.float64) ** 2))
+    assert saw_multi_pixel
+    plan.destroy()
+
+
+def test_splat_is_deterministic(E):
+    """Fixed-point accumulation: two runs give bit-identical planes regardless of atomic ordering."""
+    import torch
+    en, w, db = SPECTRA["mono"]
+    plan = E.epr_plan(256, 256, 6.5e-6, 40.0, en, w, db, "nonlocal", max_batch=1)
+    tau = _dev(_tau_field(256, 256, 8, amp=0.5)[None])
+    P1 = torch.empty((1, 256, 256), device="cuda")
+    P2 = torch.empty_like(P1)
+    E.epr_forward(plan, tau, P1)
+    E.epr_forward(plan, tau, P2)
+    assert torch.equal(P1, P2)
+    plan.destroy()
+
+
+def _run_retrieve(E, w, iterations=None, batch_idx=(0,), **opts):
+    import torch
+    it = w.iterations if iterations is None else iterations
+    plan = E.epr_plan(w.nx, w.ny, w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
+                      max_batch=len(batch_idx), max_shift_px=w.max_shift_px, **opts)
+    d = _dev(w.d[list(batch_idx)])
+    out = torch.empty_like(d)
+    E.epr_retrieve(plan, d, out, it, w.step)
+    torch.cuda.synchronize()
+    plan.destroy()
+    lines = O.derive_lines(w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta)
+    refs = [O.retrieve(w.d[j].astype(np.float64), lines, w.solver, it, w.step, S=w.max_shift_px) for j in batch_idx]
+    return out.cpu().numpy(), refs
+
+
+@pytest.mark.parametrize("name,n", [("C1", None), ("C2", 512), ("C3", 512), ("C4", 256), ("C5", (160, 320))])
+def test_retrieve_parity(E, name, n):
+    """Retrieved phase after the stated iteration count within 1e-4 relative L2 (phase ∝ τ, Eq. (6))."""
+    w = make_workload(name, n=n, batch=2 if name == "C5" else 1)
+    got, refs = _run_retrieve(E, w, batch_idx=tuple(range(w.batch)))
+    for j, ref in enumerate(refs):
+        assert rel_l2(got[j], ref) < TOL_PHASE
+
+
+def test_retrieve_zero_iterations_is_paganin(E):
+    w = make_workload("C1")
+    got, refs = _run_retrieve(E, w, iterations=0)
+    assert rel_l2(got[0], refs[0]) < TOL_OP
+
+
+def test_retrieve_unequal_a_lines(E):
+    """The implementation must not rely on 'all a_s equal' (a coincidence of C4/C5): db_s constant here."""
+    w = make_workload("C4", n=256)
+    w.delta_over_beta = np.full(8, 200.0)
+    got, refs = _run_retrieve(E, w, iterations=8)
+    assert rel_l2(got[0], refs[0]) < TOL_PHASE
+
+
+def test_retrieve_outputs_and_host_path(E):
+    import torch
+    w = make_workload("C1")
+    lines = O.derive_lines(w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta)
+    ref = O.retrieve(w.d[0].astype(np.float64), lines, w.solver, w.iterations, w.step)
+    got_phi, _ = _run_retrieve(E, w, output=1)
+    assert rel_l2(got_phi[0], O.phase(ref, lines)) < TOL_PHASE
+    plan = E.epr_plan(w.nx, w.ny, w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver, max_batch=2)
+    d3 = np.concatenate([w.d, w.d, w.d]).astype(np.float32)          # batch 3 > max_batch 2: chunked + double buffered
+    dh = torch.from_numpy(d3).pin_memory()
+    oh = torch.empty_like(dh).pin_memory()
+    E.epr_retrieve_host(plan, dh, oh, w.iterations, w.step)
+    for j in range(3):
+        assert rel_l2(oh[j].numpy(), ref) < TOL_PHASE
+    plan.destroy()
+
+
+def test_argument_errors(E):
+    import torch
+    en, w, db = SPECTRA["mono"]
+    with pytest.raises(E.EprError) as ei:
+        E.epr_plan(250, 256, 6.5e-6, 1.0, en, w, db)            # 250 = 2·5³ is not in the supported size table
+    assert ei.value.status == 2
+    with pytest.raises(E.EprError):
+        E.epr_plan(256, 256, -1.0, 1.0, en, w, db)
+    plan = E.epr_plan(256, 256, 6.5e-6, 1.0, en, w, db, max_batch=1)
+    d = torch.ones((2, 256, 256), device="cuda")
+    with pytest.raises(E.EprError):
+        E.epr_retrieve(plan, d, torch.empty_like(d), 1, 1.0)   # batch > max_batch
+    d = torch.ones((1, 256, 256), device="cuda")
+    with pytest.raises(E.EprError):
+        E.epr_retrieve(plan, d, torch.empty_like(d), 1, 0.0)   # step <= 0
+    plan.destroy()
