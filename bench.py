@@ -1,0 +1,285 @@
+#!/usr/bin/env python
+"""bench.py — EPR projections/s on B200 (BASELINE.json metric), with roofline, e2e and the oracle baseline.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--batch B] [--impl ours|reference]
+
+A step = one pass of the whole hot path (epr_retrieve: Paganin init + `iterations` correction iterations) over
+one batch of B synthetic projections of the named config (default C2: 2048x2048, monochromatic, local O(L^2)
+solver, 20 iterations — the configuration the metric is quoted on).  B distinct noisy projections (B x plane
+>> L2) are resident in HBM when the timed region starts.  N > 1 (torchrun): every rank runs its own batch on
+its own GPU (projections are independent units: weak scaling, no data-path collective); the time is the max
+over ranks.  `--impl reference` times the fp64 numpy oracle on the host cores instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "EPR projections/s (2048^2, 20 iters) on 1 B200; % HBM roofline per kernel"
+UNIT = "projections/s"
+
+
+# ---- algorithmic bytes per pixel per LAUNCH of each kernel family (fp32) ----
+def kernel_bytes_per_px(name, nb, solver):
+    return {
+        "k_forward_local": 4 + 4 * nb,          # R tau, W (P_s - f_s) x nb
+        "k_splat": 4 + 4 * nb,                  # R tau, RED fixed-point planes x nb
+        "k_residual": 4 + 8 * nb,               # R d, R pred x nb, W e_s x nb
+        "k_gather": 4 + 8 * nb,                 # R tau, R e_s x nb, W r_s x nb
+        "k_rows_r2c": 8,                        # per plane: R 4, W half spectrum 4
+        "k_cols": 4 * nb + 4,                   # R nb spectra, W summed spectrum
+        "k_rows_c2r": 12,                       # R spectrum 4, R tau 4, W tau 4
+        "k_output": 8,
+        "k_pred_out": 4 * nb + 4,
+    }[name]
+
+
+def kernel_px_per_launch(name, nb, batch, plane, launches_init_share):
+    # rows_r2c runs on nb planes per projection in the loop (1 in the init); cols/c2r on 1 output plane.
+    return batch * plane
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.25)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = max(mx, float(r[1]))
+                for n, v in zip(names, r[2:6]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_time_one(w, j=0):
+    """The oracle as it stands, one projection of the workload, on the host cores (numpy: 1 thread)."""
+    from oracle import epr_oracle as O
+    lines = O.derive_lines(w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta)
+    t0 = time.perf_counter()
+    O.retrieve(w.d[j].astype(np.float64), lines, w.solver, w.iterations, w.step, S=w.max_shift_px)
+    return time.perf_counter() - t0
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    from epr_inputs import make_workload
+    w = make_workload(args.config, batch=1, distinct=1)
+    for _ in range(args.warmup):
+        oracle_time_one(w)
+    t = [oracle_time_one(w) for _ in range(args.steps)]
+    tot = float(np.sum(t))
+    val = args.steps / tot
+    sample = f"1 projection {w.ny}x{w.nx} per step, all {w.iterations} iterations, numpy fp64 oracle"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{args.config}: {w.ny}x{w.nx}, {w.n_bins} line(s), {w.solver}, {w.iterations} iterations"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C2")
+    ap.add_argument("--batch", type=int, default=16)
+    ap.add_argument("--distinct", type=int, default=2, help="distinct simulated projections (rest: new noise only)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_2601_22793_b200 as epr
+    from epr_inputs import make_workload
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    args.warmup = max(args.warmup, 3)
+
+    B = args.batch
+    w = make_workload(args.config, batch=B, distinct=min(args.distinct, B))
+    if world > 1:                                   # every rank gets its own noise realisations
+        rng = np.random.default_rng(4000 + rank)
+        w.d = np.ascontiguousarray(w.d[rng.permutation(B)])
+    plane = w.nx * w.ny
+    nb = w.n_bins
+    plan = epr.epr_plan(w.nx, w.ny, w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
+                        max_batch=B, max_shift_px=w.max_shift_px)
+    d_host = torch.from_numpy(w.d).pin_memory()
+    out_host = torch.empty_like(d_host).pin_memory()
+    d = d_host.cuda()
+    out = torch.empty_like(d)
+
+    def step():
+        epr.epr_retrieve(plan, d, out, w.iterations, w.step)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    l0 = plan.launches
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        ev0.record()
+        for _ in range(args.steps):
+            step()
+        ev1.record()
+        barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = plan.launches - l0
+    if world > 1:
+        t = torch.tensor([ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * B * args.steps / (ms * 1e-3)
+
+    # ---- end to end through the public host API: pinned host buffers, H2D + loop + D2H inside the timed region
+    epr.epr_retrieve_host(plan, d_host, out_host, w.iterations, w.step)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        epr.epr_retrieve_host(plan, d_host, out_host, w.iterations, w.step)
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e = world * B * args.steps / e2e_s
+
+    # ---- per-kernel device times (CUDA events around every launch, on the launch stream), same K steps
+    plan.profile(True)
+    for _ in range(args.steps):
+        step()
+    prof = plan.profile_read()
+    plan.profile(False)
+
+    if rank == 0:
+        peak, peak_src = peaks()
+        per_kernel = []
+        for name, (tot_ms, cnt) in prof.items():
+            bpp = kernel_bytes_per_px(name, nb, w.solver)
+            # px per launch: every launch covers the whole batch; r2c covers nb planes per projection in the loop
+            launches_per_step = cnt / args.steps
+            px = B * plane
+            if name == "k_rows_r2c":
+                # (iterations launches of nb planes + 1 init launch of 1 plane) per step
+                px = B * plane * (w.iterations * nb + 1) / (w.iterations + 1)
+            avg_ms = tot_ms / cnt
+            gbs = bpp * px / (avg_ms * 1e-3) / 1e9
+            per_kernel.append({"kernel": name, "launches_per_step": launches_per_step, "avg_ms": avg_ms,
+                               "share": None, "algorithmic_bytes_per_launch": bpp * px, "achieved_gbs": gbs,
+                               "frac": gbs / peak})
+        tot = sum(k["avg_ms"] * k["launches_per_step"] for k in per_kernel)
+        for k in per_kernel:
+            k["share"] = k["avg_ms"] * k["launches_per_step"] / tot
+        per_kernel.sort(key=lambda k: -k["share"])
+        dom = per_kernel[0]
+        roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved_gbs"], "peak": peak,
+                    "unit": "GB/s", "frac": dom["frac"], "traffic": None, "peak_source": peak_src,
+                    "per_kernel": per_kernel}
+        result = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{args.config}: {w.ny}x{w.nx}, {nb} line(s), {w.solver} solver, "
+                                   f"{w.iterations} iterations, step {w.step}",
+                       "batch_per_gpu": B, "work_batch": None,
+                       "l2": f"inputs {B * plane * 4 / 1e6:.0f} MB per step > 126 MB L2 (no flush needed)",
+                       "ms_per_iteration_per_projection": ms / args.steps / B / (w.iterations + 1)},
+            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": B * plane * 4, "d2h_bytes_per_step": B * plane * 4},
+            "gpu_launches": int(launches) * world,
+            "clocks": clk.summary(),
+            "roofline": roofline,
+        }
+        if not args.no_cpu_baseline:
+            t1 = oracle_time_one(w)
+            result["cpu_baseline"] = {"value": 1.0 / t1, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                      "sample": f"1 of the {B} projections ({w.ny}x{w.nx}, all {w.iterations} "
+                                                f"iterations) in {t1:.1f} s, numpy fp64, host has {os.cpu_count()} cores"}
+        print(json.dumps(result))
+    plan.destroy()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

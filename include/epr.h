@@ -108,6 +108,13 @@ epr_status epr_plan_lines(epr_plan_t plan, double* f, double* gamma, double* a, 
 /* Number of kernel launches the plan has enqueued so far (for bench.py's gpu_launches). */
 long long epr_launch_count(epr_plan_t plan);
 
+/* Optional per-kernel timing for bench.py's roofline: while enabled, CUDA events are recorded on the launch
+ * stream around every kernel launch.  epr_profile_read synchronises the device and returns, per kernel family
+ * that ran, its name, total milliseconds and launch count (up to max_kernels entries; the return value is the
+ * number written); reset != 0 clears the accumulators. */
+epr_status epr_profile_enable(epr_plan_t plan, int on);
+int epr_profile_read(epr_plan_t plan, int max_kernels, const char** names, double* total_ms, long long* count, int reset);
+
 epr_status epr_destroy(epr_plan_t plan);
 const char* epr_last_error(epr_plan_t plan);
 const char* epr_version(void);

@@ -13,7 +13,7 @@ _LIB = None
 
 EXPORTS = ["epr_default_options", "epr_plan", "epr_forward", "epr_adjoint", "epr_transport", "epr_precondition",
            "epr_retrieve", "epr_retrieve_host", "epr_plan_lines", "epr_launch_count", "epr_destroy",
-           "epr_last_error", "epr_version"]
+           "epr_last_error", "epr_version", "epr_profile_enable", "epr_profile_read"]
 
 
 class EprError(RuntimeError):
@@ -57,6 +57,10 @@ def load_library():
     lib.epr_launch_count.argtypes = [vp]
     lib.epr_launch_count.restype = C.c_longlong
     lib.epr_destroy.argtypes = [vp]
+    lib.epr_profile_enable.argtypes = [vp, ci]
+    lib.epr_profile_enable.restype = ci
+    lib.epr_profile_read.argtypes = [vp, ci, C.POINTER(C.c_char_p), C.POINTER(cd), C.POINTER(C.c_longlong), ci]
+    lib.epr_profile_read.restype = ci
     lib.epr_last_error.argtypes = [vp]
     lib.epr_last_error.restype = C.c_char_p
     lib.epr_version.restype = C.c_char_p
@@ -103,6 +107,19 @@ class Plan:
     @property
     def launches(self):
         return int(load_library().epr_launch_count(self._h))
+
+    def profile(self, on):
+        """Enable / disable per-kernel CUDA-event timing inside the library."""
+        self._check(load_library().epr_profile_enable(self._h, 1 if on else 0))
+
+    def profile_read(self, reset=True):
+        """{kernel family: (total_ms, launches)} accumulated while profiling was enabled (synchronises)."""
+        n = 16
+        names = (C.c_char_p * n)()
+        ms = (C.c_double * n)()
+        cnt = (C.c_longlong * n)()
+        k = load_library().epr_profile_read(self._h, n, names, ms, cnt, 1 if reset else 0)
+        return {names[i].decode(): (float(ms[i]), int(cnt[i])) for i in range(k)}
 
     def destroy(self):
         if self._h is not None:

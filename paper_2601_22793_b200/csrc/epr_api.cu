@@ -22,10 +22,32 @@ static const double HC_KEV_M = 1.2398419843e-9;
     cudaError_t e_ = (call);                                                            \
     if (e_ != cudaSuccess) FAIL(p, EPR_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
   } while (0)
-#define KL(p, call)      \
-  do {                   \
-    CU(p, call);         \
-    (p)->launches += 1;  \
+// Kernel families, for launch counting and the optional per-kernel CUDA-event timing (epr_profile_*).
+enum { K_FWD_LOCAL = 0, K_SPLAT, K_RESIDUAL, K_GATHER, K_ROWS_R2C, K_COLS, K_ROWS_C2R, K_PRED_OUT, K_OUTPUT, K_COUNT };
+static const char* const K_NAMES[K_COUNT] = {"k_forward_local", "k_splat", "k_residual", "k_gather", "k_rows_r2c",
+                                              "k_cols", "k_rows_c2r", "k_pred_out", "k_output"};
+struct EprProf {
+  struct Rec { int tag; cudaEvent_t a, b; };
+  std::vector<Rec> recs;
+  double ms[K_COUNT];
+  long long n[K_COUNT];
+};
+
+#define KL(p, ktag, st, call)                                                   \
+  do {                                                                         \
+    EprProf::Rec rec_;                                                         \
+    if ((p)->prof_on) {                                                        \
+      rec_.tag = (ktag);                                                        \
+      CU(p, cudaEventCreate(&rec_.a));                                         \
+      CU(p, cudaEventCreate(&rec_.b));                                         \
+      CU(p, cudaEventRecord(rec_.a, (st)));                                    \
+    }                                                                          \
+    CU(p, call);                                                               \
+    (p)->launches += 1;                                                        \
+    if ((p)->prof_on) {                                                        \
+      CU(p, cudaEventRecord(rec_.b, (st)));                                    \
+      ((EprProf*)(p)->prof)->recs.push_back(rec_);                             \
+    }                                                                          \
   } while (0)
 
 extern "C" void epr_default_options(epr_options* o) {
@@ -157,6 +179,43 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
   return EPR_OK;
 }
 
+// Optional per-kernel timing: CUDA events are recorded around every kernel launch on the launch stream while
+// enabled; epr_profile_read synchronises, accumulates and returns total ms and launch count per kernel family.
+extern "C" epr_status epr_profile_enable(epr_plan_t p, int on) {
+  if (!p) return EPR_EINVAL;
+  if (!p->prof) {
+    EprProf* pr = new EprProf();
+    for (int i = 0; i < K_COUNT; ++i) { pr->ms[i] = 0; pr->n[i] = 0; }
+    p->prof = pr;
+  }
+  p->prof_on = on ? 1 : 0;
+  return EPR_OK;
+}
+
+extern "C" int epr_profile_read(epr_plan_t p, int max_kernels, const char** names, double* total_ms, long long* count,
+                                int reset) {
+  if (!p || !p->prof) return 0;
+  EprProf* pr = (EprProf*)p->prof;
+  cudaDeviceSynchronize();
+  for (auto& r : pr->recs) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess) { pr->ms[r.tag] += ms; pr->n[r.tag] += 1; }
+    cudaEventDestroy(r.a);
+    cudaEventDestroy(r.b);
+  }
+  pr->recs.clear();
+  int k = 0;
+  for (int i = 0; i < K_COUNT && k < max_kernels; ++i) {
+    if (!pr->n[i]) continue;
+    if (names) names[k] = K_NAMES[i];
+    if (total_ms) total_ms[k] = pr->ms[i];
+    if (count) count[k] = pr->n[i];
+    ++k;
+  }
+  if (reset) for (int i = 0; i < K_COUNT; ++i) { pr->ms[i] = 0; pr->n[i] = 0; }
+  return k;
+}
+
 extern "C" epr_status epr_plan_lines(epr_plan_t p, double* f, double* gamma, double* a, double* alpha) {
   if (!p) return EPR_EINVAL;
   for (int s = 0; s < p->n_bins; ++s) {
@@ -174,6 +233,7 @@ extern "C" epr_status epr_destroy(epr_plan_t p) {
   cudaFree(p->tw_row); cudaFree(p->tw_r2c); cudaFree(p->tw_col); cudaFree(p->lam_x); cudaFree(p->lam_y);
   cudaFree(p->tau); cudaFree(p->pred); cudaFree(p->res); cudaFree(p->res2); cudaFree(p->spec); cudaFree(p->spec_sum);
   cudaFree(p->raymap);
+  if (p->prof) { epr_profile_read(p, 0, NULL, NULL, NULL, 1); delete (EprProf*)p->prof; }
   for (int i = 0; i < 2; ++i) { cudaFree(p->stage_in[i]); cudaFree(p->stage_out[i]); }
   for (int i = 0; i < 3; ++i) if (p->hstream[i]) cudaStreamDestroy(p->hstream[i]);
   for (int i = 0; i < 6; ++i) if (p->hev[i]) cudaEventDestroy(p->hev[i]);
@@ -204,13 +264,13 @@ extern "C" epr_status epr_forward(epr_plan_t p, int batch, const float* tau, flo
   cudaStream_t cs = (cudaStream_t)stream;
   const size_t plane = (size_t)p->nx * p->ny;
   if (p->solver == EPR_LOCAL) {
-    KL(p, epr_launch_forward_local(p, batch, tau, p->pred, cs));
-    KL(p, epr_launch_pred_out(p, batch, p->pred, 0, 0, P_sum, P_bins, cs));
+    KL(p, K_FWD_LOCAL, cs, epr_launch_forward_local(p, batch, tau, p->pred, cs));
+    KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, 0, 0, P_sum, P_bins, cs));
   } else {
     if ((st = ensure_raymap(p)) != EPR_OK) return st;
     CU(p, epr_launch_zero(p->pred, (size_t)batch * p->n_bins * plane * sizeof(unsigned), cs));
-    KL(p, epr_launch_splat(p, batch, tau, NULL, NULL, p->raymap, (unsigned*)p->pred, cs));
-    KL(p, epr_launch_pred_out(p, batch, p->pred, 1, 0, P_sum, P_bins, cs));
+    KL(p, K_SPLAT, cs, epr_launch_splat(p, batch, tau, NULL, NULL, p->raymap, (unsigned*)p->pred, cs));
+    KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, 1, 0, P_sum, P_bins, cs));
     p->raymap_batch = batch;
   }
   return EPR_OK;
@@ -228,7 +288,7 @@ extern "C" epr_status epr_adjoint(epr_plan_t p, int batch, const float* e_bins, 
   }
   if (e_bins == r_bins) FAIL(p, EPR_EINVAL, "epr_adjoint: the gather cannot run in place");
   if (!p->raymap || p->raymap_batch < batch) FAIL(p, EPR_EINVAL, "epr_adjoint: no ray map stored for batch %d (call epr_forward first)", batch);
-  KL(p, epr_launch_gather(p, batch, NULL, p->raymap, e_bins, r_bins, cs));
+  KL(p, K_GATHER, cs, epr_launch_gather(p, batch, NULL, p->raymap, e_bins, r_bins, cs));
   return EPR_OK;
 }
 
@@ -241,8 +301,8 @@ extern "C" epr_status epr_transport(epr_plan_t p, int batch, const float* I_bins
   cudaStream_t cs = (cudaStream_t)stream;
   const size_t plane = (size_t)p->nx * p->ny;
   CU(p, epr_launch_zero(p->pred, (size_t)batch * p->n_bins * plane * sizeof(unsigned), cs));
-  KL(p, epr_launch_splat(p, batch, NULL, I_bins, p->raymap, NULL, (unsigned*)p->pred, cs));
-  KL(p, epr_launch_pred_out(p, batch, p->pred, 1, 1, NULL, P_bins, cs));
+  KL(p, K_SPLAT, cs, epr_launch_splat(p, batch, NULL, I_bins, p->raymap, NULL, (unsigned*)p->pred, cs));
+  KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, 1, 1, NULL, P_bins, cs));
   return EPR_OK;
 }
 
@@ -256,9 +316,9 @@ extern "C" epr_status epr_precondition(epr_plan_t p, int batch, const float* r_b
     const int nb = (batch - b0 < p->work_batch) ? batch - b0 : p->work_batch;
     const int planes = nb * p->n_bins;
     const size_t off = (size_t)b0 * p->n_bins * plane;
-    KL(p, epr_launch_rows_r2c(p, planes, r_bins + off, 0.f, p->spec, cs));
-    KL(p, epr_launch_cols(p, planes, 0, p->spec, p->spec, cs));
-    KL(p, epr_launch_rows_c2r(p, planes, p->spec, 0, 1.f, 0, q_bins + off, cs));
+    KL(p, K_ROWS_R2C, cs, epr_launch_rows_r2c(p, planes, r_bins + off, 0.f, p->spec, cs));
+    KL(p, K_COLS, cs, epr_launch_cols(p, planes, 0, p->spec, p->spec, cs));
+    KL(p, K_ROWS_C2R, cs, epr_launch_rows_c2r(p, planes, p->spec, 0, 1.f, 0, q_bins + off, cs));
   }
   return EPR_OK;
 }
@@ -271,26 +331,26 @@ static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* ta
   const int planes = nb * p->n_bins;
   if (p->opt.init == 0) {
     // initial guess (R9): τ⁰ = project( max(IFFT(FFT(d)/(1+āλ)), i_min) ), in deviation form from d − 1
-    KL(p, epr_launch_rows_r2c(p, nb, d, -1.f, p->spec, cs));
-    KL(p, epr_launch_cols(p, nb, 2, p->spec, p->spec_sum, cs));
-    KL(p, epr_launch_rows_c2r(p, nb, p->spec_sum, 1, 1.f, 1, tau, cs));
+    KL(p, K_ROWS_R2C, cs, epr_launch_rows_r2c(p, nb, d, -1.f, p->spec, cs));
+    KL(p, K_COLS, cs, epr_launch_cols(p, nb, 2, p->spec, p->spec_sum, cs));
+    KL(p, K_ROWS_C2R, cs, epr_launch_rows_c2r(p, nb, p->spec_sum, 1, 1.f, 1, tau, cs));
   }
   for (int it = 0; it < iterations; ++it) {
     const float* r;
     if (p->solver == EPR_LOCAL) {
-      KL(p, epr_launch_forward_local(p, nb, tau, p->pred, cs));                 // a0 + a1-L
-      KL(p, epr_launch_residual(p, nb, d, p->pred, 0, p->res, cs));             // a2 (a3 = identity)
+      KL(p, K_FWD_LOCAL, cs, epr_launch_forward_local(p, nb, tau, p->pred, cs));                 // a0 + a1-L
+      KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, 0, p->res, cs));             // a2 (a3 = identity)
       r = p->res;
     } else {
       CU(p, epr_launch_zero(p->pred, (size_t)planes * plane * sizeof(unsigned), cs));
-      KL(p, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, (unsigned*)p->pred, cs));   // a0 + a1-N
-      KL(p, epr_launch_residual(p, nb, d, p->pred, 1, p->res, cs));             // a2
-      KL(p, epr_launch_gather(p, nb, tau, NULL, p->res, p->res2, cs));          // a3
+      KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, (unsigned*)p->pred, cs));   // a0 + a1-N
+      KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, 1, p->res, cs));             // a2
+      KL(p, K_GATHER, cs, epr_launch_gather(p, nb, tau, NULL, p->res, p->res2, cs));          // a3
       r = p->res2;
     }
-    KL(p, epr_launch_rows_r2c(p, planes, r, 0.f, p->spec, cs));                 // a4
-    KL(p, epr_launch_cols(p, planes, 1, p->spec, p->spec_sum, cs));             // a4 (Σ_s in Fourier space, R10)
-    KL(p, epr_launch_rows_c2r(p, nb, p->spec_sum, 1, step, 0, tau, cs));        // a4 + a5 + a6
+    KL(p, K_ROWS_R2C, cs, epr_launch_rows_r2c(p, planes, r, 0.f, p->spec, cs));                 // a4
+    KL(p, K_COLS, cs, epr_launch_cols(p, planes, 1, p->spec, p->spec_sum, cs));             // a4 (Σ_s in Fourier space, R10)
+    KL(p, K_ROWS_C2R, cs, epr_launch_rows_c2r(p, nb, p->spec_sum, 1, step, 0, tau, cs));        // a4 + a5 + a6
   }
   return EPR_OK;
 }
@@ -305,7 +365,7 @@ static epr_status retrieve_device(epr_plan_t p, int batch, const float* d, float
     if (p->opt.init == 1 && tau != o) CU(p, cudaMemcpyAsync(tau, o, (size_t)nb * plane * sizeof(float), cudaMemcpyDeviceToDevice, cs));
     epr_status st = retrieve_chunk(p, nb, d + (size_t)b0 * plane, tau, iterations, step, cs);
     if (st != EPR_OK) return st;
-    if (p->opt.output != 0) KL(p, epr_launch_output(p, nb, tau, o, cs));
+    if (p->opt.output != 0) KL(p, K_OUTPUT, cs, epr_launch_output(p, nb, tau, o, cs));
   }
   return EPR_OK;
 }

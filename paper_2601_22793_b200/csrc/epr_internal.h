@@ -52,6 +52,8 @@ struct epr_plan_s {
   cudaStream_t hstream[3];     // copy-in, compute, copy-out
   cudaEvent_t hev[6];          // per buffer: in-done, compute-done, out-done
   long long launches;
+  int prof_on;                 // per-kernel event timing enabled
+  void* prof;                  // EprProf*
   char err[256];
 };
 
