@@ -264,7 +264,7 @@ extern "C" epr_status epr_forward(epr_plan_t p, int batch, const float* tau, flo
   cudaStream_t cs = (cudaStream_t)stream;
   const size_t plane = (size_t)p->nx * p->ny;
   if (p->solver == EPR_LOCAL) {
-    KL(p, K_FWD_LOCAL, cs, epr_launch_forward_local(p, batch, tau, p->pred, cs));
+    KL(p, K_FWD_LOCAL, cs, epr_launch_forward_local(p, batch, tau, NULL, p->pred, cs));
     KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, 0, 0, P_sum, P_bins, cs));
   } else {
     if ((st = ensure_raymap(p)) != EPR_OK) return st;
@@ -338,8 +338,12 @@ static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* ta
   for (int it = 0; it < iterations; ++it) {
     const float* r;
     if (p->solver == EPR_LOCAL) {
-      KL(p, K_FWD_LOCAL, cs, epr_launch_forward_local(p, nb, tau, p->pred, cs));                 // a0 + a1-L
-      KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, 0, p->res, cs));             // a2 (a3 = identity)
+      if (p->n_bins == 1) {
+        KL(p, K_FWD_LOCAL, cs, epr_launch_forward_local(p, nb, tau, d, p->res, cs));             // a0 + a1-L + a2 fused
+      } else {
+        KL(p, K_FWD_LOCAL, cs, epr_launch_forward_local(p, nb, tau, NULL, p->pred, cs));         // a0 + a1-L
+        KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, 0, p->res, cs));           // a2 (a3 = identity)
+      }
       r = p->res;
     } else {
       CU(p, epr_launch_zero(p->pred, (size_t)planes * plane * sizeof(unsigned), cs));

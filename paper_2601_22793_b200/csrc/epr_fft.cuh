@@ -102,6 +102,120 @@ template <int R, bool INV> __device__ __forceinline__ void dft(float2* v) {
   else dft16<INV>(v);
 }
 
+// ---- radix schedule: forward order greedy (16,…,8,4,2,5,3); the inverse uses the REVERSED order, so that the
+// last forward pass and the first inverse pass act on the same butterflies (indices j + r·N/R) and a diagonal
+// filter can be applied between them in registers. ----
+__host__ __device__ constexpr int num_passes(int n) { int c = 0; while (n > 1) { n /= pick_radix(n); ++c; } return c; }
+__host__ __device__ constexpr int fwd_radix(int n, int i) {
+  int r = pick_radix(n);
+  while (i-- > 0) { n /= r; r = pick_radix(n); }
+  return r;
+}
+// radix of pass i (0-based) in schedule DIR (false: forward order, true: reversed order)
+__host__ __device__ constexpr int sched_radix(int n, int i, bool rev) { return fwd_radix(n, rev ? num_passes(n) - 1 - i : i); }
+__host__ __device__ constexpr int sched_P(int n, int i, bool rev) {   // product of the radices before pass i
+  int p = 1;
+  for (int k = 0; k < i; ++k) p *= sched_radix(n, k, rev);
+  return p;
+}
+
+template <int N, int R, int TPC> struct PassGeom {
+  static constexpr int T = N / R;                       // butterflies per transform
+  static constexpr int CNT = (T + TPC - 1) / TPC;       // butterflies per thread
+  static constexpr bool FULL = (CNT * TPC == T);
+};
+
+// Butterfly + Stockham scatter of one thread's butterflies held in u[c][r] (inputs x[j + r·T], j = t + c·TPC):
+// twiddle (P > 1), radix-R DFT; afterwards u[c][q] is output element j0 + q·P, j0 = (j − j%P)·R + j%P.
+template <int N, int P, int R, int TPC, bool INV>
+__device__ __forceinline__ void bfly(float2 (&u)[PassGeom<N, R, TPC>::CNT][R], int t, const float2* __restrict__ tw) {
+  using G = PassGeom<N, R, TPC>;
+#pragma unroll
+  for (int c = 0; c < G::CNT; ++c) {
+    const int j = t + c * TPC;
+    if (G::FULL || j < G::T) {
+      if constexpr (P > 1) {
+        const int k = j % P;
+        constexpr int TWS = N / (P * R);
+#pragma unroll
+        for (int r = 1; r < R; ++r) u[c][r] = cmul(u[c][r], conj_if<INV>(__ldg(&tw[r * k * TWS])));
+      }
+      dft<R, INV>(u[c]);
+    }
+  }
+}
+template <int N, int R, int TPC, int STRIDE>
+__device__ __forceinline__ void smem_gather(float2 (&u)[PassGeom<N, R, TPC>::CNT][R], const float2* s, int off, int t) {
+  using G = PassGeom<N, R, TPC>;
+#pragma unroll
+  for (int c = 0; c < G::CNT; ++c) {
+    const int j = t + c * TPC;
+    if (G::FULL || j < G::T) {
+#pragma unroll
+      for (int r = 0; r < R; ++r) u[c][r] = s[padi(j + r * G::T) * STRIDE + off];
+    }
+  }
+}
+template <int N, int P, int R, int TPC, int STRIDE>
+__device__ __forceinline__ void smem_scatter(const float2 (&u)[PassGeom<N, R, TPC>::CNT][R], float2* s, int off, int t) {
+  using G = PassGeom<N, R, TPC>;
+#pragma unroll
+  for (int c = 0; c < G::CNT; ++c) {
+    const int j = t + c * TPC;
+    if (G::FULL || j < G::T) {
+      const int k = (P == 1) ? 0 : j % P;
+      const int j0 = (j - k) * R + k;
+#pragma unroll
+      for (int q = 0; q < R; ++q) s[padi(j0 + q * P) * STRIDE + off] = u[c][q];
+    }
+  }
+}
+
+// Engine for one transform size/schedule.  REV selects the reversed radix order (used for inverses).
+// Usage (n = NP passes):  first pass inputs come from registers (filled by the caller from global memory:
+// element index of u[c][r] is (t + c·TPC) + r·T0), last pass outputs stay in registers (element index of
+// u[c][q] is (t + c·TPC) + q·PL).  Passes in between go through shared memory.
+template <int N, int TPC, int STRIDE, bool INV, bool REV> struct Engine {
+  static constexpr int NP = num_passes(N);
+  static constexpr int R0 = sched_radix(N, 0, REV);                 // first radix
+  static constexpr int RL = sched_radix(N, NP - 1, REV);            // last radix
+  static constexpr int PL = sched_P(N, NP - 1, REV);                // = N / RL
+  using G0 = PassGeom<N, R0, TPC>;
+  using GL = PassGeom<N, RL, TPC>;
+
+  template <int I> __device__ static __forceinline__ void middle(float2* s, int off, int t, const float2* __restrict__ tw) {
+    if constexpr (I < NP - 1) {
+      constexpr int R = sched_radix(N, I, REV), P = sched_P(N, I, REV);
+      float2 u[PassGeom<N, R, TPC>::CNT][R];
+      smem_gather<N, R, TPC, STRIDE>(u, s, off, t);
+      __syncthreads();
+      bfly<N, P, R, TPC, INV>(u, t, tw);
+      smem_scatter<N, P, R, TPC, STRIDE>(u, s, off, t);
+      __syncthreads();
+      middle<I + 1>(s, off, t, tw);
+    }
+  }
+  // u0: first-pass inputs (registers) → … → uL: last-pass outputs (registers).  For NP == 1, u0 and uL are the
+  // same butterflies: pass the same array type (R0 == RL) and the result is left in uL.
+  __device__ static __forceinline__ void run(float2 (&u0)[G0::CNT][R0], float2 (&uL)[GL::CNT][RL], float2* s, int off, int t,
+                                             const float2* __restrict__ tw) {
+    if constexpr (NP == 1) {
+      bfly<N, 1, R0, TPC, INV>(u0, t, tw);
+#pragma unroll
+      for (int c = 0; c < G0::CNT; ++c)
+#pragma unroll
+        for (int r = 0; r < R0; ++r) uL[c][r] = u0[c][r];
+    } else {
+      bfly<N, 1, R0, TPC, INV>(u0, t, tw);
+      smem_scatter<N, 1, R0, TPC, STRIDE>(u0, s, off, t);
+      __syncthreads();
+      middle<1>(s, off, t, tw);
+      smem_gather<N, RL, TPC, STRIDE>(uL, s, off, t);
+      bfly<N, PL, RL, TPC, INV>(uL, t, tw);
+    }
+  }
+};
+
 // One Stockham pass of radix R with P = product of the previous radices.
 template <int N, int P, int R, int TPC, int STRIDE, bool INV>
 __device__ __forceinline__ void pass(float2* s, int off, int t, const float2* __restrict__ tw) {

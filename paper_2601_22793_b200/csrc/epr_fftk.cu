@@ -19,45 +19,62 @@ template <int M> struct RowCfg {                // M = nx/2 complex points per r
 };
 
 // ------------------------------------------------------------------------------------------------ rows R2C
+// global → registers (first pass) → shared-memory passes → registers (last pass) → pair exchange → global
 template <int M>
 __global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_r2c(int ny, const float* __restrict__ in, float in_offset,
                                                             const float2* __restrict__ tw, const float2* __restrict__ tw2,
                                                             float2* __restrict__ spec) {
   using C = RowCfg<M>;
+  using EF = Engine<M, C::TPC, 1, false, false>;
   __shared__ float2 sm[C::ROWS * C::PL];
   const int lr = threadIdx.x / C::TPC, t = threadIdx.x - lr * C::TPC;
   const int row = blockIdx.x * C::ROWS + lr;
   const bool live = row < ny;
-  const size_t plane = blockIdx.y;
+  const size_t rowoff = ((size_t)blockIdx.y * ny + (live ? row : 0)) * (size_t)M;
   float2* s = sm + lr * C::PL;
-  if (live) {
-    const float2* src = reinterpret_cast<const float2*>(in + (plane * ny + row) * (size_t)(2 * M));
-    for (int j = t; j < M; j += C::TPC) {
-      float2 v = __ldg(&src[j]);
-      s[padi(j)] = make_float2(v.x + in_offset, v.y + in_offset);
+  const float2* src = reinterpret_cast<const float2*>(in) + rowoff;
+  float2 u0[EF::G0::CNT][EF::R0], uL[EF::GL::CNT][EF::RL];
+#pragma unroll
+  for (int c = 0; c < EF::G0::CNT; ++c) {
+    const int j = t + c * C::TPC;
+#pragma unroll
+    for (int r = 0; r < EF::R0; ++r) {
+      float2 v = make_float2(0.f, 0.f);
+      if ((EF::G0::FULL || j < EF::G0::T) && live) v = __ldg(&src[j + r * EF::G0::T]);
+      u0[c][r] = make_float2(v.x + in_offset, v.y + in_offset);
+    }
+  }
+  EF::run(u0, uL, s, 0, t, tw);
+  __syncthreads();
+#pragma unroll
+  for (int c = 0; c < EF::GL::CNT; ++c) {
+    const int j = t + c * C::TPC;
+    if (EF::GL::FULL || j < EF::GL::T) {
+#pragma unroll
+      for (int q = 0; q < EF::RL; ++q) s[padi(j + q * EF::PL)] = uL[c][q];
     }
   }
   __syncthreads();
-  fft_smem<M, C::TPC, 1, false>(s, 0, t, tw);
-  // post-process pairs (k, M-k):  X[k] = ½(Z[k] + Z*[M−k]) − (i/2) w^k (Z[k] − Z*[M−k]),  w = e^{−2πi/nx}
-  float2* dst = spec + (plane * ny + row) * (size_t)M;
+  // X[k] = ½(Z[k] + Z*[M−k]) − (i/2) w^k (Z[k] − Z*[M−k]),  w = e^{−2πi/nx};  k = 0: packed (X[0], X[M])
   if (live) {
-    for (int k = t; k <= M / 2; k += C::TPC) {
-      if (k == 0) {
-        const float2 z = s[0];
-        dst[0] = make_float2(z.x + z.y, z.x - z.y);          // packed: re = X[0], im = X[M]
-      } else {
-        const float2 zk = s[padi(k)], zm = s[padi(M - k)];
-        const float2 wk = __ldg(&tw2[k]), wm = __ldg(&tw2[M - k]);
-        {
-          const float2 e = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
-          const float2 o = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));   // −(i/2)(zk − zm*)
-          dst[k] = cadd(e, cmul(wk, o));
-        }
-        if (k != M - k) {
-          const float2 e = make_float2(0.5f * (zm.x + zk.x), 0.5f * (zm.y - zk.y));
-          const float2 o = make_float2(0.5f * (zm.y + zk.y), -0.5f * (zm.x - zk.x));
-          dst[M - k] = cadd(e, cmul(wm, o));
+    float2* dst = spec + rowoff;
+#pragma unroll
+    for (int c = 0; c < EF::GL::CNT; ++c) {
+      const int j = t + c * C::TPC;
+      if (EF::GL::FULL || j < EF::GL::T) {
+#pragma unroll
+        for (int q = 0; q < EF::RL; ++q) {
+          const int k = j + q * EF::PL;
+          const float2 zk = uL[c][q];
+          if (k == 0) {
+            dst[0] = make_float2(zk.x + zk.y, zk.x - zk.y);
+          } else {
+            const float2 zm = s[padi(M - k)];
+            const float2 wk = __ldg(&tw2[k]);
+            const float2 e = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
+            const float2 o = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));
+            dst[k] = cadd(e, cmul(wk, o));
+          }
         }
       }
     }
@@ -72,50 +89,58 @@ __global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_c2r(EprLines L, int ny, 
                                                             int epilogue, float step, int tau_is_zero, int newton_iters,
                                                             float i_min, float* __restrict__ out) {
   using C = RowCfg<M>;
+  using EI = Engine<M, C::TPC, 1, true, false>;
   __shared__ float2 sm[C::ROWS * C::PL];
   const int lr = threadIdx.x / C::TPC, t = threadIdx.x - lr * C::TPC;
   const int row = blockIdx.x * C::ROWS + lr;
   const bool live = row < ny;
-  const size_t plane = blockIdx.y;
+  const size_t rowoff = ((size_t)blockIdx.y * ny + (live ? row : 0)) * (size_t)M;
   float2* s = sm + lr * C::PL;
-  const float2* src = spec + (plane * ny + row) * (size_t)M;
+  const float2* src = spec + rowoff;
+  float2 u0[EI::G0::CNT][EI::R0], uL[EI::GL::CNT][EI::RL];
   // Z2[k] = (X[k] + X*[M−k]) + i w^{−k} (X[k] − X*[M−k]);  Z2[0] = (x0 + xM) + i (x0 − xM)
-  if (live) {
-    for (int k = t; k <= M / 2; k += C::TPC) {
-      if (k == 0) {
-        const float2 x = __ldg(&src[0]);
-        s[0] = make_float2(x.x + x.y, x.x - x.y);
-      } else {
-        const float2 xk = __ldg(&src[k]), xm = __ldg(&src[M - k]);
-        const float2 wk = __ldg(&tw2[k]), wm = __ldg(&tw2[M - k]);
-        {
+#pragma unroll
+  for (int c = 0; c < EI::G0::CNT; ++c) {
+    const int j = t + c * C::TPC;
+#pragma unroll
+    for (int r = 0; r < EI::R0; ++r) {
+      const int k = j + r * EI::G0::T;
+      float2 z = make_float2(0.f, 0.f);
+      if ((EI::G0::FULL || j < EI::G0::T) && live) {
+        const float2 xk = __ldg(&src[k]);
+        if (k == 0) {
+          z = make_float2(xk.x + xk.y, xk.x - xk.y);
+        } else {
+          const float2 xm = __ldg(&src[M - k]);
+          const float2 wk = __ldg(&tw2[k]);
           const float2 e = make_float2(xk.x + xm.x, xk.y - xm.y);
-          const float2 dlt = make_float2(xk.x - xm.x, xk.y + xm.y);            // xk − xm*
-          const float2 o = make_float2(-dlt.y, dlt.x);                          // i (xk − xm*)
-          s[padi(k)] = cadd(e, cmul(make_float2(wk.x, -wk.y), o));
-        }
-        if (k != M - k) {
-          const float2 e = make_float2(xm.x + xk.x, xm.y - xk.y);
-          const float2 dlt = make_float2(xm.x - xk.x, xm.y + xk.y);
-          const float2 o = make_float2(-dlt.y, dlt.x);
-          s[padi(M - k)] = cadd(e, cmul(make_float2(wm.x, -wm.y), o));
+          const float2 o = make_float2(-(xk.y + xm.y), xk.x - xm.x);            // i (xk − xm*)
+          z = cadd(e, cmul(make_float2(wk.x, -wk.y), o));
         }
       }
+      u0[c][r] = z;
     }
   }
-  __syncthreads();
-  fft_smem<M, C::TPC, 1, true>(s, 0, t, tw);
+  EI::run(u0, uL, s, 0, t, tw);
   if (live) {
-    float2* dst = reinterpret_cast<float2*>(out + (plane * ny + row) * (size_t)(2 * M));
-    for (int j = t; j < M; j += C::TPC) {
-      float2 q = s[padi(j)];
-      if (epilogue == 1) {
-        float2 tau = tau_is_zero ? make_float2(0.f, 0.f) : dst[j];
-        tau.x += epr_project_increment(tau.x, step * q.x, L, newton_iters, i_min);
-        tau.y += epr_project_increment(tau.y, step * q.y, L, newton_iters, i_min);
-        q = tau;
+    float2* dst = reinterpret_cast<float2*>(out) + rowoff;
+#pragma unroll
+    for (int c = 0; c < EI::GL::CNT; ++c) {
+      const int j = t + c * C::TPC;
+      if (EI::GL::FULL || j < EI::GL::T) {
+#pragma unroll
+        for (int q = 0; q < EI::RL; ++q) {
+          const int idx = j + q * EI::PL;
+          float2 v = uL[c][q];
+          if (epilogue == 1) {
+            float2 tau = tau_is_zero ? make_float2(0.f, 0.f) : dst[idx];
+            tau.x += epr_project_increment(tau.x, step * v.x, L, newton_iters, i_min);
+            tau.y += epr_project_increment(tau.y, step * v.y, L, newton_iters, i_min);
+            v = tau;
+          }
+          dst[idx] = v;
+        }
       }
-      dst[j] = q;
     }
   }
 }
@@ -126,82 +151,123 @@ template <int N> struct ColCfg {
   static constexpr int TPC = (N + 15) / 16;      // threads per column
   static constexpr int NT = TPC * W;
   static constexpr int PL = padded_len(N);
-  static constexpr int OWN = (N + TPC - 1) / TPC;
   static constexpr size_t SMEM = (size_t)PL * W * sizeof(float2);
 };
 
 // mode 0: out[plane] = IFFT( H_{plane % nb} FFT(spec[plane]) )      (per-line, epr_precondition)
 // mode 1: out[b]     = IFFT( Σ_s H_s FFT(spec[b·nb + s]) )           (Fourier-space sum, R10 identity)
 // mode 2: out[plane] = IFFT( H_ā FFT(spec[plane]) )                  (initial guess, R9)
-template <int N>
-__global__ void __launch_bounds__(ColCfg<N>::NT) k_cols(EprLines L, int M, int mode, float scale,
-                                                        const float* __restrict__ lam_x, const float* __restrict__ lam_y,
-                                                        const float2* __restrict__ tw, const float2* __restrict__ spec,
-                                                        float2* __restrict__ out) {
+// SUM (template) = mode 1 with more than one line: accumulators in registers.
+// The forward transform uses the radix order (16,…), the inverse the reversed order, so the last forward pass,
+// the diagonal filter and the first inverse pass all happen in registers on the same butterflies.
+template <int N, bool SUM>
+__global__ void __launch_bounds__(ColCfg<N>::NT, (SUM || ColCfg<N>::NT > 512) ? 1 : 2)
+k_cols(EprLines L, int M, int mode, float scale, const float* __restrict__ lam_x, const float* __restrict__ lam_y,
+       const float2* __restrict__ tw, const float2* __restrict__ spec, float2* __restrict__ out) {
   using C = ColCfg<N>;
+  using EF = Engine<N, C::TPC, C::W, false, false>;
+  using EI = Engine<N, C::TPC, C::W, true, true>;
+  static_assert(EF::RL == EI::R0 && EF::GL::CNT == EI::G0::CNT && EF::PL == EI::G0::T, "schedules must mirror");
   extern __shared__ float2 sm[];
   const int c = threadIdx.x % C::W, t = threadIdx.x / C::W;
   const int kx = blockIdx.x * C::W + c;
   const int oplane = blockIdx.y;
   const int nb = L.n_bins;
-  const int nloop = (mode == 1) ? nb : 1;
+  const int nloop = SUM ? nb : 1;
   const bool live = kx < M;
   const float lx = live ? __ldg(&lam_x[kx]) : 0.f;
-  const float lxN = __ldg(&lam_x[M]);            // λx at the Nyquist column (packed into kx = 0)
-  float2 acc[C::OWN];
+  float2 acc[EF::GL::CNT][EF::RL];
+  if (SUM) {
 #pragma unroll
-  for (int m = 0; m < C::OWN; ++m) acc[m] = make_float2(0.f, 0.f);
-
+    for (int cc = 0; cc < EF::GL::CNT; ++cc)
+#pragma unroll
+      for (int q = 0; q < EF::RL; ++q) acc[cc][q] = make_float2(0.f, 0.f);
+  }
   for (int sl = 0; sl < nloop; ++sl) {
     const size_t iplane = (mode == 1) ? (size_t)oplane * nb + sl : (size_t)oplane;
     const float a = (mode == 2) ? L.abar : L.a[(mode == 1) ? sl : (oplane % nb)];
-    const float2* src = spec + iplane * (size_t)N * M;
-    for (int i = threadIdx.x; i < N * C::W; i += C::NT) {
-      const int ky = i / C::W, cc = i - ky * C::W;
-      const int k2 = blockIdx.x * C::W + cc;
-      sm[padi(ky) * C::W + cc] = (k2 < M) ? __ldg(&src[(size_t)ky * M + k2]) : make_float2(0.f, 0.f);
-    }
-    __syncthreads();
-    fft_smem<N, C::TPC, C::W, false>(sm, c, t, tw);
-    if (kx == 0) {
-      // packed column: C = F0 + i FM with F0, FM Hermitian in ky.  A = ½(C[ky] + C*[−ky]), B = −(i/2)(C[ky] − C*[−ky]);
-      // C'[ky] = H(0,ky) A + i H(M,ky) B,  C'[−ky] = H(0,ky) A* + i H(M,ky) B*
-      for (int ky = t; ky <= N / 2; ky += C::TPC) {
-        const int km = (ky == 0) ? 0 : N - ky;
-        const float2 ck = sm[padi(ky) * C::W], cm = sm[padi(km) * C::W];
-        const float ly = __ldg(&lam_y[ky]);
-        const float h0 = scale / (1.f + a * (lx + ly)), hN = scale / (1.f + a * (lxN + ly));
-        const float2 A = make_float2(0.5f * (ck.x + cm.x), 0.5f * (ck.y - cm.y));
-        const float2 B = make_float2(0.5f * (ck.y + cm.y), -0.5f * (ck.x - cm.x));
-        sm[padi(ky) * C::W] = make_float2(h0 * A.x - hN * B.y, h0 * A.y + hN * B.x);
-        if (km != ky) sm[padi(km) * C::W] = make_float2(h0 * A.x + hN * B.y, -h0 * A.y + hN * B.x);
+    const float2* src = spec + iplane * (size_t)N * M + (live ? kx : 0);
+    float2 u0[EF::G0::CNT][EF::R0], uL[EF::GL::CNT][EF::RL];
+#pragma unroll
+    for (int cc = 0; cc < EF::G0::CNT; ++cc) {
+      const int j = t + cc * C::TPC;
+#pragma unroll
+      for (int r = 0; r < EF::R0; ++r) {
+        float2 v = make_float2(0.f, 0.f);
+        if ((EF::G0::FULL || j < EF::G0::T) && live) v = __ldg(&src[(size_t)(j + r * EF::G0::T) * M]);
+        u0[cc][r] = v;
       }
     }
-    __syncthreads();
+    EF::run(u0, uL, sm, c, t, tw);
+    if (blockIdx.x == 0) {
+      // tile 0 holds the packed column kx = 0: C = F0 + i FM (both Hermitian in ky).  With A = ½(C[ky] + C*[−ky]),
+      // B = −(i/2)(C[ky] − C*[−ky]):  C'[ky] = H(0,ky) A + i H(M,ky) B,  C'[−ky] = H(0,ky) A* + i H(M,ky) B*.
+      __syncthreads();
 #pragma unroll
-    for (int m = 0; m < C::OWN; ++m) {
-      const int ky = t + m * C::TPC;
-      if (C::OWN * C::TPC == N || ky < N) {
-        const float2 v = sm[padi(ky) * C::W + c];
-        const float h = (kx == 0) ? 1.f : scale / (1.f + a * (lx + __ldg(&lam_y[ky])));
-        acc[m].x = fmaf(h, v.x, acc[m].x);
-        acc[m].y = fmaf(h, v.y, acc[m].y);
+      for (int cc = 0; cc < EF::GL::CNT; ++cc) {
+        const int j = t + cc * C::TPC;
+        if (EF::GL::FULL || j < EF::GL::T) {
+#pragma unroll
+          for (int q = 0; q < EF::RL; ++q) sm[padi(j + q * EF::PL) * C::W + c] = uL[cc][q];
+        }
+      }
+      __syncthreads();
+      if (c == 0) {
+        const float lxN = __ldg(&lam_x[M]);
+        for (int ky = t; ky <= N / 2; ky += C::TPC) {
+          const int km = (ky == 0) ? 0 : N - ky;
+          const float2 ck = sm[padi(ky) * C::W], cm = sm[padi(km) * C::W];
+          const float ly = __ldg(&lam_y[ky]);
+          const float h0 = scale / (1.f + a * (lx + ly)), hN = scale / (1.f + a * (lxN + ly));
+          const float2 A = make_float2(0.5f * (ck.x + cm.x), 0.5f * (ck.y - cm.y));
+          const float2 B = make_float2(0.5f * (ck.y + cm.y), -0.5f * (ck.x - cm.x));
+          sm[padi(ky) * C::W] = make_float2(h0 * A.x - hN * B.y, h0 * A.y + hN * B.x);
+          if (km != ky) sm[padi(km) * C::W] = make_float2(h0 * A.x + hN * B.y, -h0 * A.y + hN * B.x);
+        }
+      }
+      __syncthreads();
+#pragma unroll
+      for (int cc = 0; cc < EF::GL::CNT; ++cc) {
+        const int j = t + cc * C::TPC;
+        if (EF::GL::FULL || j < EF::GL::T) {
+#pragma unroll
+          for (int q = 0; q < EF::RL; ++q) uL[cc][q] = sm[padi(j + q * EF::PL) * C::W + c];
+        }
       }
     }
-    __syncthreads();
-  }
+    const float alx = fmaf(a, lx, 1.f);
 #pragma unroll
-  for (int m = 0; m < C::OWN; ++m) {
-    const int ky = t + m * C::TPC;
-    if (C::OWN * C::TPC == N || ky < N) sm[padi(ky) * C::W + c] = acc[m];
+    for (int cc = 0; cc < EF::GL::CNT; ++cc) {
+      const int j = t + cc * C::TPC;
+      if (EF::GL::FULL || j < EF::GL::T) {
+#pragma unroll
+        for (int q = 0; q < EF::RL; ++q) {
+          const float h = (kx == 0) ? 1.f : __fdividef(scale, fmaf(a, __ldg(&lam_y[j + q * EF::PL]), alx));
+          if (SUM) { acc[cc][q].x = fmaf(h, uL[cc][q].x, acc[cc][q].x); acc[cc][q].y = fmaf(h, uL[cc][q].y, acc[cc][q].y); }
+          else { uL[cc][q].x *= h; uL[cc][q].y *= h; }
+        }
+      }
+    }
+    __syncthreads();                       // all reads of shared memory done before the next transform writes it
+    if (!SUM) {
+#pragma unroll
+      for (int cc = 0; cc < EF::GL::CNT; ++cc)
+#pragma unroll
+        for (int q = 0; q < EF::RL; ++q) acc[cc][q] = uL[cc][q];
+    }
   }
-  __syncthreads();
-  fft_smem<N, C::TPC, C::W, true>(sm, c, t, tw);
-  float2* dst = out + (size_t)oplane * N * M;
-  for (int i = threadIdx.x; i < N * C::W; i += C::NT) {
-    const int ky = i / C::W, cc = i - ky * C::W;
-    const int k2 = blockIdx.x * C::W + cc;
-    if (k2 < M) dst[(size_t)ky * M + k2] = sm[padi(ky) * C::W + cc];
+  float2 uo[EI::GL::CNT][EI::RL];
+  EI::run(acc, uo, sm, c, t, tw);
+  if (live) {
+    float2* dst = out + (size_t)oplane * N * M + kx;
+#pragma unroll
+    for (int cc = 0; cc < EI::GL::CNT; ++cc) {
+      const int j = t + cc * C::TPC;
+      if (EI::GL::FULL || j < EI::GL::T) {
+#pragma unroll
+        for (int q = 0; q < EI::RL; ++q) dst[(size_t)(j + q * EI::PL) * M] = uo[cc][q];
+      }
+    }
   }
 }
 
@@ -257,9 +323,16 @@ cudaError_t epr_launch_cols(const epr_plan_s* p, int planes, int mode, const flo
   case n_: {                                                                                                    \
     using C = ColCfg<n_>;                                                                                       \
     static bool attr = false;                                                                                   \
-    if (!attr) { cudaFuncSetAttribute(k_cols<n_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM); attr = true; } \
+    if (!attr) {                                                                                                \
+      cudaFuncSetAttribute(k_cols<n_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);       \
+      cudaFuncSetAttribute(k_cols<n_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);        \
+      attr = true;                                                                                              \
+    }                                                                                                           \
     dim3 grid((M + C::W - 1) / C::W, oplanes);                                                                  \
-    k_cols<n_><<<grid, C::NT, C::SMEM, st>>>(p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, spec, out); \
+    if (mode == 1 && p->n_bins > 1)                                                                             \
+      k_cols<n_, true><<<grid, C::NT, C::SMEM, st>>>(p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, spec, out); \
+    else                                                                                                        \
+      k_cols<n_, false><<<grid, C::NT, C::SMEM, st>>>(p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, spec, out); \
   } break;
     EPR_FFT_SIZES(X)
 #undef X

@@ -59,7 +59,9 @@ struct epr_plan_s {
 
 // ---- launchers (epr_kernels.cu / epr_fftk.cu); all return cudaGetLastError() ----
 // planes = batch * n_bins unless stated.
-cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float* tau, float* pred, cudaStream_t st);
+// d_fuse != NULL (one line only): out = e = (d-1) - (P-1) directly; else out = pred[b][s] = P_s - f_s
+cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float* tau, const float* d_fuse, float* out,
+                                     cudaStream_t st);
 cudaError_t epr_launch_splat(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
                              float2* map_out, unsigned* pfix, cudaStream_t st);
 cudaError_t epr_launch_residual(const epr_plan_s* p, int batch, const float* d, const void* pred, int fixed,

@@ -3,88 +3,167 @@
 #include "epr_math.cuh"
 
 // =====================================================================================================
-// a1-L  local O(L²) closure, Eq. (1) PAPER.md:146 (readings R1-R3), in deviation form.
-//   out: pred[b][s][y][x] = P_s − f_s
+// a1-L  local O(L²) closure, Eq. (1) PAPER.md:146 (readings R1-R3), in deviation form, fused (one line) with
+// a2, the detector residual (a3 is the identity for the local solver).
 //   P_s/f_s − 1 = J − a ∇²₅J + (a²/2)[D²x(Î gx²) + D²y(Î gy²) + 2 D⁰xD⁰y(Î gx gy)] − (α²/4) Σ_i D⁻_i(Ī_i D⁺_i Q)
 //   with A = exp(−γτ/2) = 1 + Ad,  Î = I/f = A²,  J = Î − 1 = Ad(2+Ad),  g = −γ D⁰τ,  Q = ∇²₅A / A.
-// One CTA = 64x16 output pixels; τ and Ad staged in shared memory with a 2-pixel halo, g and Q with 1.
+//   FUSE (n_bins == 1): out = e = (d − 1) − (P − 1);  otherwise out[b][s] = P_s − f_s for k_residual.
+// One CTA = 128x8 output pixels, each thread a strip of 4 in x.  Stage 1: τ and Ad (halo 2) in shared memory;
+// stage 2: Î gx², Î gy², Î gx gy, Q (halo 1); stage 3: the closure from float4 shared loads.  The kernel is
+// bound by fp32 issue (≈ 100 instructions per pixel), not by HBM (12 B/px): see DESIGN.md.
 // =====================================================================================================
-#define FL_TX 64
-#define FL_TY 16
-#define FL_SX (FL_TX + 4)
-#define FL_SY (FL_TY + 4)
+#define FL_TX 128
+#define FL_TY 8
+#define FL_PW (FL_TX + 8)            // row pitch: 4 columns of (aligned) halo on each side, 2 used
+#define FL_R1 (FL_TY + 4)            // rows with halo 2
+#define FL_R2 (FL_TY + 2)            // rows with halo 1
 
+struct Strip6 { float m, v0, v1, v2, v3, p; };     // values at columns c-1, c..c+3, c+4 of one row
+__device__ __forceinline__ Strip6 ld6(const float* row, int c) {
+  const float4 v = *reinterpret_cast<const float4*>(row + c);
+  return Strip6{row[c - 1], v.x, v.y, v.z, v.w, row[c + 4]};
+}
+__device__ __forceinline__ float4 ld4(const float* row, int c) { return *reinterpret_cast<const float4*>(row + c); }
+
+template <bool FUSE>
 __global__ void __launch_bounds__(256) k_forward_local(EprLines L, int nx, int ny, int order, int wkb1,
-                                                       const float* __restrict__ tau, float* __restrict__ pred) {
-  __shared__ float s_tau[FL_SY][FL_SX], s_ad[FL_SY][FL_SX], s_gx[FL_SY][FL_SX], s_gy[FL_SY][FL_SX], s_q[FL_SY][FL_SX];
-  const int b = blockIdx.z;
-  const int x0 = blockIdx.x * FL_TX - 2, y0 = blockIdx.y * FL_TY - 2;
-  const size_t plane = (size_t)nx * ny;
+                                                       const float* __restrict__ tau, const float* __restrict__ d,
+                                                       float* __restrict__ out) {
+  __shared__ __align__(16) float s_tau[FL_R1][FL_PW], s_ad[FL_R1][FL_PW];
+  __shared__ __align__(16) float s_sxx[FL_R2][FL_PW], s_syy[FL_R2][FL_PW], s_sxy[FL_R2][FL_PW], s_q[FL_R2][FL_PW];
+  const int b = blockIdx.z, tid = threadIdx.x;
+  const int x0 = blockIdx.x * FL_TX, y0 = blockIdx.y * FL_TY;
+  const unsigned plane = (unsigned)nx * (unsigned)ny;
   const float* tb = tau + (size_t)b * plane;
-  const int tid = threadIdx.x;
 
-  for (int i = tid; i < FL_SX * FL_SY; i += 256) {
-    const int ly = i / FL_SX, lx = i - ly * FL_SX;
-    int gx_ = x0 + lx, gy_ = y0 + ly;
-    gx_ = wrapm(gx_, nx);
-    gy_ = wrapm(gy_, ny);
-    s_tau[ly][lx] = __ldg(&tb[(size_t)gy_ * nx + gx_]);
+  // stage 0: τ tile, rows y0-2 .. y0+TY+1, columns x0-4 .. x0+TX+3 as whole float4 groups (nx % 4 == 0)
+  for (int i = tid; i < FL_R1 * (FL_PW / 4); i += 256) {
+    const int ly = i / (FL_PW / 4), g = i - ly * (FL_PW / 4);
+    const int gy = wrapm(y0 - 2 + ly, ny), gx = wrapm(x0 - 4 + 4 * g, nx);
+    *reinterpret_cast<float4*>(&s_tau[ly][4 * g]) = __ldg(reinterpret_cast<const float4*>(tb + (unsigned)gy * nx + gx));
   }
   for (int s = 0; s < L.n_bins; ++s) {
-    const float gam = L.gamma[s];
+    const float gam = L.gamma[s], cg = -0.5f * gam;
     __syncthreads();
-    for (int i = tid; i < FL_SX * FL_SY; i += 256) {
-      const int ly = i / FL_SX, lx = i - ly * FL_SX;
-      s_ad[ly][lx] = expm1f(-0.5f * gam * s_tau[ly][lx]);
+    // stage 1: Ad = expm1(−γτ/2)
+    for (int i = tid; i < FL_R1 * (FL_PW / 4); i += 256) {
+      const int ly = i / (FL_PW / 4), g = i - ly * (FL_PW / 4);
+      const float4 t = *reinterpret_cast<const float4*>(&s_tau[ly][4 * g]);
+      *reinterpret_cast<float4*>(&s_ad[ly][4 * g]) =
+          make_float4(epr_expm1(cg * t.x), epr_expm1(cg * t.y), epr_expm1(cg * t.z), epr_expm1(cg * t.w));
     }
     __syncthreads();
     if (order == 2) {
-      for (int i = tid; i < (FL_SX - 2) * (FL_SY - 2); i += 256) {
-        const int ly = i / (FL_SX - 2) + 1, lx = i - (ly - 1) * (FL_SX - 2) + 1;
-        s_gx[ly][lx] = -0.5f * gam * (s_tau[ly][lx + 1] - s_tau[ly][lx - 1]);
-        s_gy[ly][lx] = -0.5f * gam * (s_tau[ly + 1][lx] - s_tau[ly - 1][lx]);
-        const float c = s_ad[ly][lx];
-        s_q[ly][lx] = ((s_ad[ly][lx + 1] - c) + (s_ad[ly][lx - 1] - c) + (s_ad[ly + 1][lx] - c) + (s_ad[ly - 1][lx] - c)) / (1.f + c);
+      // stage 2 on rows 1..TY+2 (halo 1): interior float4 groups 1..TX/4, plus the two halo columns 3 and TX+4
+      for (int i = tid; i < FL_R2 * (FL_TX / 4 + 1); i += 256) {
+        const int r2 = i / (FL_TX / 4 + 1), g = i - r2 * (FL_TX / 4 + 1);
+        const int ly = r2 + 1;
+        if (g < FL_TX / 4) {
+          const int c = 4 * (g + 1);
+          const Strip6 t0 = ld6(s_tau[ly], c), a0 = ld6(s_ad[ly], c);
+          const float4 tn = ld4(s_tau[ly - 1], c), ts = ld4(s_tau[ly + 1], c);
+          const float4 an = ld4(s_ad[ly - 1], c), as = ld4(s_ad[ly + 1], c);
+          float4 oxx, oyy, oxy, oq;
+#define ST2(o, tw, te, tnn, tss, aw, ac, ae, ann, ass)                                  \
+          {                                                                              \
+            const float gx = cg * ((te) - (tw)), gy = cg * ((tss) - (tnn));              \
+            const float A = 1.f + (ac), I = A * A, igx = I * gx;                          \
+            oxx.o = igx * gx; oxy.o = igx * gy; oyy.o = I * gy * gy;                      \
+            oq.o = __fdividef((((ae) - (ac)) + ((aw) - (ac))) + (((ann) - (ac)) + ((ass) - (ac))), A); \
+          }
+          ST2(x, t0.m, t0.v1, tn.x, ts.x, a0.m, a0.v0, a0.v1, an.x, as.x)
+          ST2(y, t0.v0, t0.v2, tn.y, ts.y, a0.v0, a0.v1, a0.v2, an.y, as.y)
+          ST2(z, t0.v1, t0.v3, tn.z, ts.z, a0.v1, a0.v2, a0.v3, an.z, as.z)
+          ST2(w, t0.v2, t0.p, tn.w, ts.w, a0.v2, a0.v3, a0.p, an.w, as.w)
+          *reinterpret_cast<float4*>(&s_sxx[r2][c]) = oxx;
+          *reinterpret_cast<float4*>(&s_syy[r2][c]) = oyy;
+          *reinterpret_cast<float4*>(&s_sxy[r2][c]) = oxy;
+          *reinterpret_cast<float4*>(&s_q[r2][c]) = oq;
+        } else {
+#pragma unroll
+          for (int side = 0; side < 2; ++side) {
+            const int c = side ? FL_TX + 4 : 3;
+            const float gx = cg * (s_tau[ly][c + 1] - s_tau[ly][c - 1]), gy = cg * (s_tau[ly + 1][c] - s_tau[ly - 1][c]);
+            const float ac = s_ad[ly][c], A = 1.f + ac, I = A * A, igx = I * gx;
+            s_sxx[r2][c] = igx * gx; s_sxy[r2][c] = igx * gy; s_syy[r2][c] = I * gy * gy;
+            s_q[r2][c] = __fdividef(((s_ad[ly][c + 1] - ac) + (s_ad[ly][c - 1] - ac)) + ((s_ad[ly - 1][c] - ac) + (s_ad[ly + 1][c] - ac)), A);
+          }
+        }
       }
     }
     __syncthreads();
-    float* out = pred + ((size_t)b * L.n_bins + s) * plane;
-    for (int i = tid; i < FL_TX * FL_TY; i += 256) {
-      const int ty = i / FL_TX, tx = i - ty * FL_TX;
-      const int gxx = x0 + 2 + tx, gyy = y0 + 2 + ty;
-      if (gxx >= nx || gyy >= ny) continue;
-      const int ly = ty + 2, lx = tx + 2;
-#define AD(dy, dx) s_ad[ly + (dy)][lx + (dx)]
-#define IH(dy, dx) ((1.f + AD(dy, dx)) * (1.f + AD(dy, dx)))
-#define JJ(dy, dx) (AD(dy, dx) * (2.f + AD(dy, dx)))
-      const float Jc = JJ(0, 0);
-      const float lapJ = (JJ(0, 1) - Jc) + (JJ(0, -1) - Jc) + (JJ(1, 0) - Jc) + (JJ(-1, 0) - Jc);
-      float v = Jc - L.a[s] * lapJ;
-      if (order == 2) {
-#define GX(dy, dx) s_gx[ly + (dy)][lx + (dx)]
-#define GY(dy, dx) s_gy[ly + (dy)][lx + (dx)]
-#define QQ(dy, dx) s_q[ly + (dy)][lx + (dx)]
-        const float Ic = IH(0, 0), Ixp = IH(0, 1), Ixm = IH(0, -1), Iyp = IH(1, 0), Iym = IH(-1, 0);
-        const float sxx = Ixp * GX(0, 1) * GX(0, 1) - 2.f * Ic * GX(0, 0) * GX(0, 0) + Ixm * GX(0, -1) * GX(0, -1);
-        const float syy = Iyp * GY(1, 0) * GY(1, 0) - 2.f * Ic * GY(0, 0) * GY(0, 0) + Iym * GY(-1, 0) * GY(-1, 0);
-        const float sxy = 0.25f * (IH(1, 1) * GX(1, 1) * GY(1, 1) - IH(1, -1) * GX(1, -1) * GY(1, -1)
-                                   - IH(-1, 1) * GX(-1, 1) * GY(-1, 1) + IH(-1, -1) * GX(-1, -1) * GY(-1, -1));
-        v = fmaf(L.a2h[s], sxx + syy + 2.f * sxy, v);
-        if (wkb1) {
-          const float Qc = QQ(0, 0);
-          const float div = 0.5f * ((Ixp + Ic) * (QQ(0, 1) - Qc) - (Ic + Ixm) * (Qc - QQ(0, -1))
-                                    + (Iyp + Ic) * (QQ(1, 0) - Qc) - (Ic + Iym) * (Qc - QQ(-1, 0)));
-          v = fmaf(-L.q4[s], div, v);
+    // stage 3: one strip of 4 outputs per thread (TX/4 = 32 strips per row x TY rows = 256)
+    {
+      const int ty = tid >> 5, c = 4 * ((tid & 31) + 1);
+      const int gx0 = x0 + c - 4, gyy = y0 + ty;
+      if (gx0 < nx && gyy < ny) {
+        const int l1 = ty + 2, l2 = ty + 1;
+        const Strip6 a0 = ld6(s_ad[l1], c);
+        const float4 an = ld4(s_ad[l1 - 1], c), as = ld4(s_ad[l1 + 1], c);
+        const float av[6] = {a0.m, a0.v0, a0.v1, a0.v2, a0.v3, a0.p};
+        const float anv[4] = {an.x, an.y, an.z, an.w}, asv[4] = {as.x, as.y, as.z, as.w};
+        float v[4];
+        float Jr[6], Ir[6];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) { Jr[k] = av[k] * (2.f + av[k]); Ir[k] = Jr[k] + 1.f; }
+        float Jn[4], Js[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { Jn[k] = anv[k] * (2.f + anv[k]); Js[k] = asv[k] * (2.f + asv[k]); }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const float Jc = Jr[k + 1];
+          const float lapJ = ((Jr[k + 2] - Jc) + (Jr[k] - Jc)) + ((Jn[k] - Jc) + (Js[k] - Jc));
+          v[k] = fmaf(-L.a[s], lapJ, Jc);
+        }
+        if (order == 2) {
+          const Strip6 xx = ld6(s_sxx[l2], c);
+          const float4 yn = ld4(s_syy[l2 - 1], c), yc = ld4(s_syy[l2], c), ys = ld4(s_syy[l2 + 1], c);
+          const Strip6 xyn = ld6(s_sxy[l2 - 1], c), xys = ld6(s_sxy[l2 + 1], c);
+          const float xxv[6] = {xx.m, xx.v0, xx.v1, xx.v2, xx.v3, xx.p};
+          const float ynv[4] = {yn.x, yn.y, yn.z, yn.w}, ycv[4] = {yc.x, yc.y, yc.z, yc.w}, ysv[4] = {ys.x, ys.y, ys.z, ys.w};
+          const float xnv[6] = {xyn.m, xyn.v0, xyn.v1, xyn.v2, xyn.v3, xyn.p}, xsv[6] = {xys.m, xys.v0, xys.v1, xys.v2, xys.v3, xys.p};
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const float sxx = (xxv[k + 2] - xxv[k + 1]) + (xxv[k] - xxv[k + 1]);
+            const float syy = (ysv[k] - ycv[k]) + (ynv[k] - ycv[k]);
+            const float sxy2 = 0.5f * ((xsv[k + 2] - xsv[k]) - (xnv[k + 2] - xnv[k]));      // 2 · D⁰xD⁰y
+            v[k] = fmaf(L.a2h[s], (sxx + syy) + sxy2, v[k]);
+          }
+          if (wkb1) {
+            const Strip6 q0 = ld6(s_q[l2], c);
+            const float4 qn = ld4(s_q[l2 - 1], c), qs = ld4(s_q[l2 + 1], c);
+            const float qv[6] = {q0.m, q0.v0, q0.v1, q0.v2, q0.v3, q0.p};
+            const float qnv[4] = {qn.x, qn.y, qn.z, qn.w}, qsv[4] = {qs.x, qs.y, qs.z, qs.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              const float Ic = Ir[k + 1], Qc = qv[k + 1];
+              const float In = Jn[k] + 1.f, Is = Js[k] + 1.f;
+              const float div = 0.5f * (((Ir[k + 2] + Ic) * (qv[k + 2] - Qc) - (Ic + Ir[k]) * (Qc - qv[k]))
+                                        + ((Is + Ic) * (qsv[k] - Qc) - (Ic + In) * (Qc - qnv[k])));
+              v[k] = fmaf(-L.q4[s], div, v[k]);
+            }
+          }
+        }
+        const unsigned o = (unsigned)gyy * nx + gx0;
+        if (FUSE) {
+          const float4 dd = __ldg(reinterpret_cast<const float4*>(d + (size_t)b * plane + o));
+          *reinterpret_cast<float4*>(out + (size_t)b * plane + o) =
+              make_float4((dd.x - 1.f) - v[0], (dd.y - 1.f) - v[1], (dd.z - 1.f) - v[2], (dd.w - 1.f) - v[3]);
+        } else {
+          const float f = L.f[s];
+          *reinterpret_cast<float4*>(out + ((size_t)b * L.n_bins + s) * plane + o) =
+              make_float4(f * v[0], f * v[1], f * v[2], f * v[3]);
         }
       }
-      out[(size_t)gyy * nx + gxx] = L.f[s] * v;
     }
   }
 }
 
-cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float* tau, float* pred, cudaStream_t st) {
+cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float* tau, const float* d_fuse, float* out,
+                                     cudaStream_t st) {
   dim3 grid((p->nx + FL_TX - 1) / FL_TX, (p->ny + FL_TY - 1) / FL_TY, batch);
-  k_forward_local<<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, pred);
+  if (d_fuse) k_forward_local<true><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, d_fuse, out);
+  else k_forward_local<false><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, nullptr, out);
   return cudaGetLastError();
 }
 
@@ -213,30 +292,53 @@ __device__ __forceinline__ float pred_dev(const void* pred, size_t idx, int fixe
   return __ldg(&((const float*)pred)[idx]);
 }
 
-__global__ void __launch_bounds__(256) k_residual(EprLines L, size_t plane, const float* __restrict__ d,
+__device__ __forceinline__ float4 pred_dev4(const void* pred, size_t idx, int fixed, const EprLines& L, int s) {
+  if (fixed) {
+    const uint4 v = __ldg(reinterpret_cast<const uint4*>((const unsigned*)pred + idx));
+    const float sc = 1.0f / (float)EPR_FIX_ONE, c = L.fixCorr[s];
+    const unsigned F = L.fixFi[s];
+    return make_float4(fmaf((float)(int)(v.x - F), sc, c), fmaf((float)(int)(v.y - F), sc, c),
+                       fmaf((float)(int)(v.z - F), sc, c), fmaf((float)(int)(v.w - F), sc, c));
+  }
+  return __ldg(reinterpret_cast<const float4*>((const float*)pred + idx));
+}
+
+// one thread = 4 consecutive pixels (plane % 4 == 0)
+__global__ void __launch_bounds__(256) k_residual(EprLines L, unsigned plane, const float* __restrict__ d,
                                                   const void* __restrict__ pred, int fixed, float* __restrict__ es) {
-  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
+  const unsigned i = (blockIdx.x * 256u + threadIdx.x) * 4u;
   const int b = blockIdx.y;
   if (i >= plane) return;
   const size_t base = (size_t)b * L.n_bins * plane + i;
-  float sum = 0.f, den = 0.f;
+  float4 sum = make_float4(0.f, 0.f, 0.f, 0.f), den = sum;
   for (int s = 0; s < L.n_bins; ++s) {
-    const float pd = pred_dev(pred, base + s * plane, fixed, L, s);
-    sum += pd;
-    den += fmaxf(L.f[s] + pd, 0.f);
+    const float4 pd = pred_dev4(pred, base + (size_t)s * plane, fixed, L, s);
+    const float f = L.f[s];
+    sum.x += pd.x; sum.y += pd.y; sum.z += pd.z; sum.w += pd.w;
+    den.x += fmaxf(f + pd.x, 0.f); den.y += fmaxf(f + pd.y, 0.f); den.z += fmaxf(f + pd.z, 0.f); den.w += fmaxf(f + pd.w, 0.f);
   }
-  const float e = (__ldg(&d[(size_t)b * plane + i]) - 1.f) - sum - L.fsum_dev;
+  const float4 dd = __ldg(reinterpret_cast<const float4*>(d + (size_t)b * plane + i));
+  const float off = 1.f + L.fsum_dev;
+  const float4 e = make_float4((dd.x - off) - sum.x, (dd.y - off) - sum.y, (dd.z - off) - sum.z, (dd.w - off) - sum.w);
+  // e/den once per pixel; w_s e = P_s⁺ (e/den), fallback f_s e where den <= 0
+  const float4 q = make_float4(den.x > 0.f ? e.x / den.x : 0.f, den.y > 0.f ? e.y / den.y : 0.f,
+                               den.z > 0.f ? e.z / den.z : 0.f, den.w > 0.f ? e.w / den.w : 0.f);
   for (int s = 0; s < L.n_bins; ++s) {
-    const float pd = pred_dev(pred, base + s * plane, fixed, L, s);
-    const float w = den > 0.f ? fmaxf(L.f[s] + pd, 0.f) / den : L.f[s];
-    es[base + s * plane] = w * e;
+    const float4 pd = pred_dev4(pred, base + (size_t)s * plane, fixed, L, s);
+    const float f = L.f[s];
+    float4 o;
+    o.x = den.x > 0.f ? fmaxf(f + pd.x, 0.f) * q.x : f * e.x;
+    o.y = den.y > 0.f ? fmaxf(f + pd.y, 0.f) * q.y : f * e.y;
+    o.z = den.z > 0.f ? fmaxf(f + pd.z, 0.f) * q.z : f * e.z;
+    o.w = den.w > 0.f ? fmaxf(f + pd.w, 0.f) * q.w : f * e.w;
+    *reinterpret_cast<float4*>(es + base + (size_t)s * plane) = o;
   }
 }
 
 cudaError_t epr_launch_residual(const epr_plan_s* p, int batch, const float* d, const void* pred, int fixed,
                                 float* es, cudaStream_t st) {
-  const size_t plane = (size_t)p->nx * p->ny;
-  dim3 grid((unsigned)((plane + 255) / 256), batch);
+  const unsigned plane = (unsigned)p->nx * p->ny;
+  dim3 grid((plane / 4 + 255) / 256, batch);
   k_residual<<<grid, 256, 0, st>>>(p->lines, plane, d, pred, fixed, es);
   return cudaGetLastError();
 }

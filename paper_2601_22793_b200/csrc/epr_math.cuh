@@ -10,31 +10,66 @@
 __device__ __forceinline__ int wrap1(int i, int n) { return i < 0 ? i + n : (i >= n ? i - n : i); }   // -n <= i < 2n
 __device__ __forceinline__ int wrapm(int i, int n) { i %= n; return i < 0 ? i + n : i; }               // any i
 
+// expm1 to ~2 ulp RELATIVE accuracy without the slow path of expm1f: Taylor (degree 8) for |x| < 0.35
+// (truncation x^8/9! < 1e-9 relative), exp(x) − 1 with the MUFU exponential beyond (|result| > 0.29 there, so
+// the 2^-22 relative error of ex2.approx stays below 1e-6 relative).  Both branches are evaluated (no divergence).
+__device__ __forceinline__ float epr_expm1(float x) {
+  float q = fmaf(x, 2.48015873e-5f, 1.98412698e-4f);
+  q = fmaf(x, q, 1.38888889e-3f);
+  q = fmaf(x, q, 8.33333333e-3f);
+  q = fmaf(x, q, 4.16666667e-2f);
+  q = fmaf(x, q, 1.66666667e-1f);
+  q = fmaf(x, q, 0.5f);
+  const float small = fmaf(x * x, q, x);
+  const float big = __expf(x) - 1.f;
+  return fabsf(x) < 0.35f ? small : big;
+}
+
+// log1p to ~2 ulp relative accuracy: 2 atanh(z/(2+z)) series for |z| < 0.25 (s^10/11 < 1e-10), log(1+z) beyond.
+__device__ __forceinline__ float epr_log1p(float z) {
+  const float s = __fdividef(z, 2.f + z);
+  const float s2 = s * s;
+  float q = fmaf(s2, 0.111111111f, 0.142857143f);
+  q = fmaf(s2, q, 0.2f);
+  q = fmaf(s2, q, 0.333333333f);
+  q = fmaf(s2, q, 1.f);
+  const float small = 2.f * s * q;
+  const float big = __logf(1.f + z);
+  return fabsf(z) < 0.25f ? small : big;
+}
+
 // Projection to the single-thickness manifold, Eq. (7) + PAPER.md:233 (R10), as an increment:
 //   given τ and ΔT, find δ with Σ_s I_s(τ) expm1(−γ_s δ) = ΔT, clamped so that Σ_s I_s + ΔT ≥ i_min.
 // Newton from the Jensen bound δ0 = −log1p(ΔT/ΣI)/γ̄_I (monotone; exact for one line).
 __device__ __forceinline__ float epr_project_increment(float tau, float dT, const EprLines& L, int newton_iters,
                                                        float i_min) {
   const int nb = L.n_bins;
+  if (nb == 1) {
+    // one line: f = γ = 1, I = e^{−τ};  δ = −log1p(ΔT e^{τ}), floor I + ΔT ≥ i_min  ⇔  1 + z ≥ i_min e^{τ}
+    const float E = __expf(tau);
+    float z = dT * E;
+    if (1.f + z < i_min * E) z = i_min * E - 1.f;
+    return -epr_log1p(z);
+  }
   float Tsum = 0.f, G = 0.f;
   for (int s = 0; s < nb; ++s) {
-    const float I = L.f[s] * expf(-L.gamma[s] * tau);
+    const float I = L.f[s] * __expf(-L.gamma[s] * tau);
     Tsum += I;
     G = fmaf(L.gamma[s], I, G);
   }
   if (Tsum + dT < i_min) dT = i_min - Tsum;
-  float delta = -log1pf(dT / Tsum) * (Tsum / G);
-  if (nb > 1) {
-    for (int it = 0; it < newton_iters; ++it) {
-      float F = -dT, dF = 0.f;
-      for (int s = 0; s < nb; ++s) {
-        const float I = L.f[s] * expf(-L.gamma[s] * tau);
-        const float x = -L.gamma[s] * delta;
-        F = fmaf(I, expm1f(x), F);
-        dF = fmaf(-L.gamma[s] * I, expf(x), dF);
-      }
-      delta -= F / dF;
+  float delta = -epr_log1p(__fdividef(dT, Tsum)) * __fdividef(Tsum, G);
+  for (int it = 0; it < newton_iters; ++it) {
+    float F = -dT, dF = 0.f;
+    for (int s = 0; s < nb; ++s) {
+      const float I = L.f[s] * __expf(-L.gamma[s] * tau);
+      const float em = epr_expm1(-L.gamma[s] * delta);
+      F = fmaf(I, em, F);
+      dF = fmaf(-L.gamma[s] * I, 1.f + em, dF);
     }
+    const float stp = __fdividef(F, dF);
+    delta -= stp;
+    if (fabsf(stp) <= 1e-7f * fabsf(delta) + 1e-12f) break;      // converged to fp32 (Newton is quadratic)
   }
   return delta;
 }
