@@ -6,6 +6,7 @@
 
 #include <vector>
 
+#include "epr_fft.cuh"
 #include "epr_internal.h"
 
 extern "C" int epr_fft_size_supported(int n);
@@ -73,6 +74,22 @@ static std::vector<float2> twiddles(int n, int count) {
   for (int m = 0; m < count; ++m) {
     const double th = -2.0 * M_PI * (double)m / (double)n;
     v[m] = make_float2((float)cos(th), (float)sin(th));
+  }
+  return v;
+}
+
+// per-pass tables of epr_fft.cuh: tab[off_i + (r−1)·P_i + k] = exp(−2πi r k/(P_i R_i))
+static std::vector<float2> pass_twiddles(int n, bool rev) {
+  using namespace eprfft;
+  std::vector<float2> v(tw_total(n, rev) > 0 ? tw_total(n, rev) : 1, make_float2(1.f, 0.f));
+  const int np = num_passes(n);
+  for (int i = 1; i < np; ++i) {
+    const int R = sched_radix(n, i, rev), P = sched_P(n, i, rev), off = tw_offset(n, i, rev);
+    for (int r = 1; r < R; ++r)
+      for (int k = 0; k < P; ++k) {
+        const double th = -2.0 * M_PI * (double)r * (double)k / ((double)P * (double)R);
+        v[off + (r - 1) * P + k] = make_float2((float)cos(th), (float)sin(th));
+      }
   }
   return v;
 }
@@ -151,9 +168,10 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
   L.fsum_dev = (float)(fs - 1.0);
 
   const int M = nx / 2;
-  CU(p, upload(&p->tw_row, twiddles(M, M)));
+  CU(p, upload(&p->tw_row, pass_twiddles(M, false)));
   CU(p, upload(&p->tw_r2c, twiddles(nx, M)));
-  CU(p, upload(&p->tw_col, twiddles(ny, ny)));
+  CU(p, upload(&p->tw_col, pass_twiddles(ny, false)));
+  CU(p, upload(&p->tw_col_inv, pass_twiddles(ny, true)));
   CU(p, upload(&p->lam_x, lambda_table(nx, M + 1, o.symbol)));
   CU(p, upload(&p->lam_y, lambda_table(ny, ny, o.symbol)));
 
@@ -230,7 +248,7 @@ extern "C" epr_status epr_plan_lines(epr_plan_t p, double* f, double* gamma, dou
 extern "C" epr_status epr_destroy(epr_plan_t p) {
   if (!p) return EPR_EINVAL;
   cudaDeviceSynchronize();
-  cudaFree(p->tw_row); cudaFree(p->tw_r2c); cudaFree(p->tw_col); cudaFree(p->lam_x); cudaFree(p->lam_y);
+  cudaFree(p->tw_row); cudaFree(p->tw_r2c); cudaFree(p->tw_col); cudaFree(p->tw_col_inv); cudaFree(p->lam_x); cudaFree(p->lam_y);
   cudaFree(p->tau); cudaFree(p->pred); cudaFree(p->res); cudaFree(p->res2); cudaFree(p->spec); cudaFree(p->spec_sum);
   cudaFree(p->raymap);
   if (p->prof) { epr_profile_read(p, 0, NULL, NULL, NULL, 1); delete (EprProf*)p->prof; }

@@ -25,6 +25,8 @@ __host__ __device__ constexpr int padded_len(int n) { return padi(n - 1) + 1; }
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
   return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
 }
+// (packed add.f32x2 / fma.rn.f32x2 were tried here: fewer FP instructions but more register-pair moves and
+// address arithmetic; the column kernel got 10 % slower, so the scalar forms stay)
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 template <bool INV> __device__ __forceinline__ float2 rot90(float2 a) {   // multiply by -i (fwd) / +i (inv)
@@ -119,6 +121,16 @@ __host__ __device__ constexpr int sched_P(int n, int i, bool rev) {   // product
   return p;
 }
 
+// Per-pass twiddle tables: pass i ≥ 1 of a schedule uses tab[off_i + (r−1)·P_i + k] = exp(−2πi r k /(P_i R_i)),
+// k < P_i, 1 ≤ r < R_i — laid out so that threads with consecutive k read consecutive addresses (one or two
+// 128-byte lines per warp load instead of up to 4r lines with a single stride-indexed table).
+__host__ __device__ constexpr int tw_offset(int n, int i, bool rev) {
+  int off = 0;
+  for (int k = 1; k < i; ++k) off += (sched_radix(n, k, rev) - 1) * sched_P(n, k, rev);
+  return off;
+}
+__host__ __device__ constexpr int tw_total(int n, bool rev) { return tw_offset(n, num_passes(n), rev); }
+
 template <int N, int R, int TPC> struct PassGeom {
   static constexpr int T = N / R;                       // butterflies per transform
   static constexpr int CNT = (T + TPC - 1) / TPC;       // butterflies per thread
@@ -136,9 +148,8 @@ __device__ __forceinline__ void bfly(float2 (&u)[PassGeom<N, R, TPC>::CNT][R], i
     if (G::FULL || j < G::T) {
       if constexpr (P > 1) {
         const int k = j % P;
-        constexpr int TWS = N / (P * R);
 #pragma unroll
-        for (int r = 1; r < R; ++r) u[c][r] = cmul(u[c][r], conj_if<INV>(__ldg(&tw[r * k * TWS])));
+        for (int r = 1; r < R; ++r) u[c][r] = cmul(u[c][r], conj_if<INV>(__ldg(&tw[(r - 1) * P + k])));
       }
       dft<R, INV>(u[c]);
     }
@@ -189,7 +200,7 @@ template <int N, int TPC, int STRIDE, bool INV, bool REV> struct Engine {
       float2 u[PassGeom<N, R, TPC>::CNT][R];
       smem_gather<N, R, TPC, STRIDE>(u, s, off, t);
       __syncthreads();
-      bfly<N, P, R, TPC, INV>(u, t, tw);
+      bfly<N, P, R, TPC, INV>(u, t, tw + tw_offset(N, I, REV));
       smem_scatter<N, P, R, TPC, STRIDE>(u, s, off, t);
       __syncthreads();
       middle<I + 1>(s, off, t, tw);
@@ -211,61 +222,9 @@ template <int N, int TPC, int STRIDE, bool INV, bool REV> struct Engine {
       __syncthreads();
       middle<1>(s, off, t, tw);
       smem_gather<N, RL, TPC, STRIDE>(uL, s, off, t);
-      bfly<N, PL, RL, TPC, INV>(uL, t, tw);
+      bfly<N, PL, RL, TPC, INV>(uL, t, tw + tw_offset(N, NP - 1, REV));
     }
   }
 };
-
-// One Stockham pass of radix R with P = product of the previous radices.
-template <int N, int P, int R, int TPC, int STRIDE, bool INV>
-__device__ __forceinline__ void pass(float2* s, int off, int t, const float2* __restrict__ tw) {
-  constexpr int T = N / R;
-  constexpr int CNT = (T + TPC - 1) / TPC;
-  float2 u[CNT][R];
-#pragma unroll
-  for (int c = 0; c < CNT; ++c) {
-    const int j = t + c * TPC;
-    if (CNT * TPC == T || j < T) {
-#pragma unroll
-      for (int r = 0; r < R; ++r) u[c][r] = s[padi(j + r * T) * STRIDE + off];
-    }
-  }
-  __syncthreads();
-#pragma unroll
-  for (int c = 0; c < CNT; ++c) {
-    const int j = t + c * TPC;
-    if (CNT * TPC == T || j < T) {
-      const int k = (P == 1) ? 0 : (j % P);
-      if constexpr (P > 1) {
-        constexpr int TWS = N / (P * R);
-#pragma unroll
-        for (int r = 1; r < R; ++r) u[c][r] = cmul(u[c][r], conj_if<INV>(__ldg(&tw[r * k * TWS])));
-      }
-      dft<R, INV>(u[c]);
-      const int j0 = (j - k) * R + k;
-#pragma unroll
-      for (int q = 0; q < R; ++q) s[padi(j0 + q * P) * STRIDE + off] = u[c][q];
-    }
-  }
-  __syncthreads();
-}
-
-template <int N, int P, int TPC, int STRIDE, bool INV>
-__device__ __forceinline__ void passes(float2* s, int off, int t, const float2* __restrict__ tw) {
-  if constexpr (P < N) {
-    constexpr int R = pick_radix(N / P);
-    static_assert(R != 0, "unsupported FFT length");
-    pass<N, P, R, TPC, STRIDE, INV>(s, off, t, tw);
-    passes<N, P * R, TPC, STRIDE, INV>(s, off, t, tw);
-  }
-}
-
-// In-place length-N transform of the sequence s[padi(i)*STRIDE + off], done by TPC threads (t = 0..TPC-1).
-// Must be called by every thread of the CTA (it contains __syncthreads); the data must be visible
-// (barrier) before the call and are visible after it.  tw[m] = exp(-2πi m/N), m < N.
-template <int N, int TPC, int STRIDE, bool INV>
-__device__ __forceinline__ void fft_smem(float2* s, int off, int t, const float2* __restrict__ tw) {
-  passes<N, 1, TPC, STRIDE, INV>(s, off, t, tw);
-}
 
 }  // namespace eprfft

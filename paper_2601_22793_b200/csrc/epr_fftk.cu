@@ -82,11 +82,12 @@ __global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_r2c(int ny, const float*
 }
 
 // ------------------------------------------------------------------------------------------------ rows C2R
-// epilogue 0: out[plane][y][x] = q.   epilogue 1: τ[plane][y][x] += δ(τ, step·q)  (projection increment, R10)
-template <int M>
+// EPI 0: out[plane][y][x] = q.   EPI 1 / 2: τ[plane][y][x] += δ(τ, step·q)  (projection increment, R10) for
+// one line (closed form) / several lines (Newton).
+template <int M, int EPI>
 __global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_c2r(EprLines L, int ny, const float2* __restrict__ spec,
                                                             const float2* __restrict__ tw, const float2* __restrict__ tw2,
-                                                            int epilogue, float step, int tau_is_zero, int newton_iters,
+                                                            float step, int tau_is_zero, int newton_iters,
                                                             float i_min, float* __restrict__ out) {
   using C = RowCfg<M>;
   using EI = Engine<M, C::TPC, 1, true, false>;
@@ -121,9 +122,20 @@ __global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_c2r(EprLines L, int ny, 
       u0[c][r] = z;
     }
   }
+  // prefetch the τ values the epilogue will update, so that their latency hides behind the transform
+  float2* dst = reinterpret_cast<float2*>(out) + rowoff;
+  float2 tpre[EI::GL::CNT][EI::RL];
+#pragma unroll
+  for (int c = 0; c < EI::GL::CNT; ++c) {
+    const int j = t + c * C::TPC;
+#pragma unroll
+    for (int q = 0; q < EI::RL; ++q) {
+      tpre[c][q] = make_float2(0.f, 0.f);
+      if (EPI != 0 && !tau_is_zero && live && (EI::GL::FULL || j < EI::GL::T)) tpre[c][q] = dst[j + q * EI::PL];
+    }
+  }
   EI::run(u0, uL, s, 0, t, tw);
   if (live) {
-    float2* dst = reinterpret_cast<float2*>(out) + rowoff;
 #pragma unroll
     for (int c = 0; c < EI::GL::CNT; ++c) {
       const int j = t + c * C::TPC;
@@ -132,8 +144,13 @@ __global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_c2r(EprLines L, int ny, 
         for (int q = 0; q < EI::RL; ++q) {
           const int idx = j + q * EI::PL;
           float2 v = uL[c][q];
-          if (epilogue == 1) {
-            float2 tau = tau_is_zero ? make_float2(0.f, 0.f) : dst[idx];
+          if (EPI == 1) {
+            float2 tau = tpre[c][q];
+            tau.x += epr_project_increment_mono(tau.x, step * v.x, i_min);
+            tau.y += epr_project_increment_mono(tau.y, step * v.y, i_min);
+            v = tau;
+          } else if (EPI == 2) {
+            float2 tau = tpre[c][q];
             tau.x += epr_project_increment(tau.x, step * v.x, L, newton_iters, i_min);
             tau.y += epr_project_increment(tau.y, step * v.y, L, newton_iters, i_min);
             v = tau;
@@ -163,7 +180,8 @@ template <int N> struct ColCfg {
 template <int N, bool SUM>
 __global__ void __launch_bounds__(ColCfg<N>::NT, (SUM || ColCfg<N>::NT > 512) ? 1 : 2)
 k_cols(EprLines L, int M, int mode, float scale, const float* __restrict__ lam_x, const float* __restrict__ lam_y,
-       const float2* __restrict__ tw, const float2* __restrict__ spec, float2* __restrict__ out) {
+       const float2* __restrict__ tw, const float2* __restrict__ tw_inv, const float2* __restrict__ spec,
+       float2* __restrict__ out) {
   using C = ColCfg<N>;
   using EF = Engine<N, C::TPC, C::W, false, false>;
   using EI = Engine<N, C::TPC, C::W, true, true>;
@@ -257,7 +275,7 @@ k_cols(EprLines L, int M, int mode, float scale, const float* __restrict__ lam_x
     }
   }
   float2 uo[EI::GL::CNT][EI::RL];
-  EI::run(acc, uo, sm, c, t, tw);
+  EI::run(acc, uo, sm, c, t, tw_inv);
   if (live) {
     float2* dst = out + (size_t)oplane * N * M + kx;
 #pragma unroll
@@ -304,8 +322,15 @@ cudaError_t epr_launch_rows_c2r(const epr_plan_s* p, int planes, const float2* s
   case n_: {                                                                                                    \
     using C = RowCfg<n_ / 2>;                                                                                   \
     dim3 grid((p->ny + C::ROWS - 1) / C::ROWS, planes);                                                         \
-    k_rows_c2r<n_ / 2><<<grid, C::NT, 0, st>>>(p->lines, p->ny, spec, p->tw_row, p->tw_r2c, epilogue, step,       \
-                                               tau_is_zero, p->opt.newton_iters, p->opt.i_min, q_or_tau);       \
+    if (epilogue == 0)                                                                                          \
+      k_rows_c2r<n_ / 2, 0><<<grid, C::NT, 0, st>>>(p->lines, p->ny, spec, p->tw_row, p->tw_r2c, step, tau_is_zero, \
+                                                    p->opt.newton_iters, p->opt.i_min, q_or_tau);               \
+    else if (p->n_bins == 1)                                                                                    \
+      k_rows_c2r<n_ / 2, 1><<<grid, C::NT, 0, st>>>(p->lines, p->ny, spec, p->tw_row, p->tw_r2c, step, tau_is_zero, \
+                                                    p->opt.newton_iters, p->opt.i_min, q_or_tau);               \
+    else                                                                                                        \
+      k_rows_c2r<n_ / 2, 2><<<grid, C::NT, 0, st>>>(p->lines, p->ny, spec, p->tw_row, p->tw_r2c, step, tau_is_zero, \
+                                                    p->opt.newton_iters, p->opt.i_min, q_or_tau);               \
   } break;
     EPR_FFT_SIZES(X)
 #undef X
@@ -330,9 +355,9 @@ cudaError_t epr_launch_cols(const epr_plan_s* p, int planes, int mode, const flo
     }                                                                                                           \
     dim3 grid((M + C::W - 1) / C::W, oplanes);                                                                  \
     if (mode == 1 && p->n_bins > 1)                                                                             \
-      k_cols<n_, true><<<grid, C::NT, C::SMEM, st>>>(p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, spec, out); \
+      k_cols<n_, true><<<grid, C::NT, C::SMEM, st>>>(p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv, spec, out); \
     else                                                                                                        \
-      k_cols<n_, false><<<grid, C::NT, C::SMEM, st>>>(p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, spec, out); \
+      k_cols<n_, false><<<grid, C::NT, C::SMEM, st>>>(p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv, spec, out); \
   } break;
     EPR_FFT_SIZES(X)
 #undef X

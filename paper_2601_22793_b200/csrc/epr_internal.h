@@ -32,9 +32,10 @@ struct epr_plan_s {
   double h_f[EPR_MAX_BINS], h_gamma[EPR_MAX_BINS], h_a[EPR_MAX_BINS], h_alpha[EPR_MAX_BINS], h_db[EPR_MAX_BINS];
   EprLines lines;
   // tables
-  float2* tw_row;              // exp(-2πi m/(nx/2)), m < nx/2
-  float2* tw_r2c;              // exp(-2πi k/nx),     k < nx/2
-  float2* tw_col;              // exp(-2πi m/ny),     m < ny
+  float2* tw_row;              // per-pass twiddles of the nx/2-point row transform (forward radix order)
+  float2* tw_r2c;              // exp(-2πi k/nx), k < nx/2 (real<->complex split)
+  float2* tw_col;              // per-pass twiddles of the ny-point column transform, forward radix order
+  float2* tw_col_inv;          //   … reversed radix order (inverse)
   float* lam_x;                // λ_x[kx], kx = 0..nx/2
   float* lam_y;                // λ_y[ky], ky < ny
   // workspaces (sized for max_batch)

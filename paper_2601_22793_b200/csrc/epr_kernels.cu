@@ -159,11 +159,145 @@ __global__ void __launch_bounds__(256) k_forward_local(EprLines L, int nx, int n
   }
 }
 
+// -----------------------------------------------------------------------------------------------------
+// Register-marching variant of the fused closure + residual for one spectral line (the hot configuration).
+// A warp owns a band of 128 columns (lane l: 4 consecutive pixels; lanes 0 and 31 are halo providers, lanes
+// 1..30 write 120 output columns) and marches down MR output rows.  Every row of τ is loaded ONCE from global
+// memory as a float4 per lane; all x-neighbours come from warp shuffles and all y-neighbours from rolling
+// registers, so the kernel uses no shared memory and no barriers and is bound by fp32 issue.
+// Pipeline per step (new τ row n): Ad[n] → stage-2 row m = n−1 (Î gx², Î gy², Î gx gy, Q) → output row o = n−2.
+// -----------------------------------------------------------------------------------------------------
+#define LM_MR 32                     // output rows per warp
+#define LM_BW 120                    // output columns per warp
+
+struct F4 { float v[4]; };
+__device__ __forceinline__ float shfl_l(float x) { return __shfl_up_sync(0xffffffffu, x, 1); }     // from lane-1
+__device__ __forceinline__ float shfl_r(float x) { return __shfl_down_sync(0xffffffffu, x, 1); }   // from lane+1
+
+__global__ void __launch_bounds__(128) k_local_march(EprLines L, int nx, int ny, int order, int wkb1,
+                                                     const float* __restrict__ tau, const float* __restrict__ d,
+                                                     float* __restrict__ out) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int band = blockIdx.x * 4 + warp;
+  const int xs = band * LM_BW - 4 + 4 * lane;              // first of this lane's 4 columns (may be < 0 or >= nx)
+  if (band * LM_BW >= nx) return;                          // whole warp out of range (no barriers in this kernel)
+  const int y0 = blockIdx.y * LM_MR;
+  const unsigned plane = (unsigned)nx * (unsigned)ny;
+  const float* tb = tau + (size_t)blockIdx.z * plane;
+  const float* db = d + (size_t)blockIdx.z * plane;
+  float* ob = out + (size_t)blockIdx.z * plane;
+  const int xw = wrapm(xs, nx);
+  const bool writer = lane >= 1 && lane <= 30 && xs < nx;
+  const float cg = -0.5f * L.gamma[0], a = L.a[0], a2h = L.a2h[0], q4 = L.q4[0];
+
+  // rolling registers (suffix: row relative to the output row o):  p1 = o+1 (= m), 0 = o, m1 = o−1
+  F4 t_m1, t_0, t_p1;                       // τ rows m−1.. for stage 2 (t_p1 is the newest row n after the shift)
+  F4 A_m1, A_0, A_p1, A_p2;                 // Ad rows o−1, o, o+1, o+2 (A_p2 = newest)
+  float A0_l = 0.f, A0_r = 0.f, Ap1_l = 0.f, Ap1_r = 0.f;      // x-halo of Ad rows o and o+1
+  F4 sxx_0, syy_m1, syy_0, syy_p1, sxy_m1, sxy_0, sxy_p1, q_m1, q_0, q_p1;
+  float sxx0_l = 0.f, sxx0_r = 0.f, sxxp1_l = 0.f, sxxp1_r = 0.f;
+  float sxym1_l = 0.f, sxym1_r = 0.f, sxy0_l = 0.f, sxy0_r = 0.f, sxyp1_l = 0.f, sxyp1_r = 0.f;
+  float q0_l = 0.f, q0_r = 0.f, qp1_l = 0.f, qp1_r = 0.f;
+  F4 sxx_p1;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    t_m1.v[k] = t_0.v[k] = t_p1.v[k] = 0.f; A_m1.v[k] = A_0.v[k] = A_p1.v[k] = A_p2.v[k] = 0.f;
+    sxx_0.v[k] = sxx_p1.v[k] = syy_m1.v[k] = syy_0.v[k] = syy_p1.v[k] = 0.f;
+    sxy_m1.v[k] = sxy_0.v[k] = sxy_p1.v[k] = q_m1.v[k] = q_0.v[k] = q_p1.v[k] = 0.f;
+  }
+
+  // rows n = y0−2 … y0+MR+1; output row o = n−2 is valid once n ≥ y0+2
+  for (int step = 0; step < LM_MR + 4; ++step) {
+    const int n = y0 - 2 + step;
+    // ---- shift the windows ----
+    t_m1 = t_0; t_0 = t_p1;
+    A_m1 = A_0; A_0 = A_p1; A_p1 = A_p2; A0_l = Ap1_l; A0_r = Ap1_r;
+    sxx_0 = sxx_p1; sxx0_l = sxxp1_l; sxx0_r = sxxp1_r;
+    syy_m1 = syy_0; syy_0 = syy_p1;
+    sxy_m1 = sxy_0; sxy_0 = sxy_p1; sxym1_l = sxy0_l; sxym1_r = sxy0_r; sxy0_l = sxyp1_l; sxy0_r = sxyp1_r;
+    q_m1 = q_0; q_0 = q_p1; q0_l = qp1_l; q0_r = qp1_r;
+    // ---- new row n: τ and Ad ----
+    {
+      const float4 tv = __ldg(reinterpret_cast<const float4*>(tb + (unsigned)wrapm(n, ny) * nx + xw));
+      t_p1.v[0] = tv.x; t_p1.v[1] = tv.y; t_p1.v[2] = tv.z; t_p1.v[3] = tv.w;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) A_p2.v[k] = epr_expm1(cg * t_p1.v[k]);
+    }
+    // after the shift: stage-2 row m = n−1 has τ rows (t_m1, t_0, t_p1) = (m−1, m, m+1) and Ad rows (A_0, A_p1, A_p2)
+    // — careful: A_p1 is row m (= o+1), A_0 is row m−1, A_p2 is row m+1.
+    {
+      const float tl = shfl_l(t_0.v[3]), tr = shfl_r(t_0.v[0]);
+      Ap1_l = shfl_l(A_p1.v[3]); Ap1_r = shfl_r(A_p1.v[0]);
+      if (order == 2) {
+        const float tw_[6] = {tl, t_0.v[0], t_0.v[1], t_0.v[2], t_0.v[3], tr};
+        const float aw_[6] = {Ap1_l, A_p1.v[0], A_p1.v[1], A_p1.v[2], A_p1.v[3], Ap1_r};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const float gx = cg * (tw_[k + 2] - tw_[k]), gy = cg * (t_p1.v[k] - t_m1.v[k]);
+          const float ac = aw_[k + 1], A = 1.f + ac, I = A * A, igx = I * gx;
+          sxx_p1.v[k] = igx * gx; sxy_p1.v[k] = igx * gy; syy_p1.v[k] = I * gy * gy;
+          q_p1.v[k] = __fdividef(((aw_[k + 2] - ac) + (aw_[k] - ac)) + ((A_0.v[k] - ac) + (A_p2.v[k] - ac)), A);
+        }
+        sxxp1_l = shfl_l(sxx_p1.v[3]); sxxp1_r = shfl_r(sxx_p1.v[0]);
+        sxyp1_l = shfl_l(sxy_p1.v[3]); sxyp1_r = shfl_r(sxy_p1.v[0]);
+        qp1_l = shfl_l(q_p1.v[3]); qp1_r = shfl_r(q_p1.v[0]);
+      }
+    }
+    // ---- output row o = n − 2: Ad rows (A_m1, A_0, A_p1) = (o−1, o, o+1); halo of row o in A0_l/A0_r ----
+    const int o = n - 2;
+    if (step >= 4 && o < ny && writer) {
+      const float aw_[6] = {A0_l, A_0.v[0], A_0.v[1], A_0.v[2], A_0.v[3], A0_r};
+      float Jr[6], Ir[6];
+#pragma unroll
+      for (int k = 0; k < 6; ++k) { Jr[k] = aw_[k] * (2.f + aw_[k]); Ir[k] = Jr[k] + 1.f; }
+      float v[4];
+      float Jn[4], Js[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        Jn[k] = A_m1.v[k] * (2.f + A_m1.v[k]); Js[k] = A_p1.v[k] * (2.f + A_p1.v[k]);
+        const float Jc = Jr[k + 1];
+        v[k] = fmaf(-a, ((Jr[k + 2] - Jc) + (Jr[k] - Jc)) + ((Jn[k] - Jc) + (Js[k] - Jc)), Jc);
+      }
+      if (order == 2) {
+        const float xx[6] = {sxx0_l, sxx_0.v[0], sxx_0.v[1], sxx_0.v[2], sxx_0.v[3], sxx0_r};
+        const float xn[6] = {sxym1_l, sxy_m1.v[0], sxy_m1.v[1], sxy_m1.v[2], sxy_m1.v[3], sxym1_r};
+        const float xs_[6] = {sxyp1_l, sxy_p1.v[0], sxy_p1.v[1], sxy_p1.v[2], sxy_p1.v[3], sxyp1_r};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const float sxx = (xx[k + 2] - xx[k + 1]) + (xx[k] - xx[k + 1]);
+          const float syy = (syy_p1.v[k] - syy_0.v[k]) + (syy_m1.v[k] - syy_0.v[k]);
+          const float sxy2 = 0.5f * ((xs_[k + 2] - xs_[k]) - (xn[k + 2] - xn[k]));
+          v[k] = fmaf(a2h, (sxx + syy) + sxy2, v[k]);
+        }
+        if (wkb1) {
+          const float qq[6] = {q0_l, q_0.v[0], q_0.v[1], q_0.v[2], q_0.v[3], q0_r};
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const float Ic = Ir[k + 1], Qc = qq[k + 1], In = Jn[k] + 1.f, Is = Js[k] + 1.f;
+            const float div = 0.5f * (((Ir[k + 2] + Ic) * (qq[k + 2] - Qc) - (Ic + Ir[k]) * (Qc - qq[k]))
+                                      + ((Is + Ic) * (q_p1.v[k] - Qc) - (Ic + In) * (Qc - q_m1.v[k])));
+            v[k] = fmaf(-q4, div, v[k]);
+          }
+        }
+      }
+      const unsigned off = (unsigned)o * nx + xs;
+      const float4 dd = __ldg(reinterpret_cast<const float4*>(db + off));
+      *reinterpret_cast<float4*>(ob + off) =
+          make_float4((dd.x - 1.f) - v[0], (dd.y - 1.f) - v[1], (dd.z - 1.f) - v[2], (dd.w - 1.f) - v[3]);
+    }
+  }
+}
+
 cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float* tau, const float* d_fuse, float* out,
                                      cudaStream_t st) {
+  if (d_fuse) {
+    const int bands = (p->nx + LM_BW - 1) / LM_BW;
+    dim3 grid((bands + 3) / 4, (p->ny + LM_MR - 1) / LM_MR, batch);
+    k_local_march<<<grid, 128, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, d_fuse, out);
+    return cudaGetLastError();
+  }
   dim3 grid((p->nx + FL_TX - 1) / FL_TX, (p->ny + FL_TY - 1) / FL_TY, batch);
-  if (d_fuse) k_forward_local<true><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, d_fuse, out);
-  else k_forward_local<false><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, nullptr, out);
+  k_forward_local<false><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, nullptr, out);
   return cudaGetLastError();
 }
 

@@ -38,19 +38,34 @@ __device__ __forceinline__ float epr_log1p(float z) {
   return fabsf(z) < 0.25f ? small : big;
 }
 
+// out-of-line copy for rare paths (keeps the unrolled epilogues small)
+static __device__ __noinline__ float epr_log1p_cold(float z) { return epr_log1p(z); }
+
+// One spectral line (f = γ = 1, I = e^{−τ}):  δ = −log1p(ΔT e^{τ}), with the floor I + ΔT ≥ i_min ⇔ 1 + z ≥ i_min e^{τ}.
+// log1p: alternating series (degree 8, |z| < 0.1: z^9/9 < 1.2e-10) on the common path, atanh series / log beyond.
+__device__ __forceinline__ float epr_project_increment_mono(float tau, float dT, float i_min) {
+  const float E = __expf(tau);
+  float z = dT * E;
+  z = fmaxf(z, fmaf(i_min, E, -1.f));
+  if (fabsf(z) < 0.1f) {
+    float q = fmaf(z, -0.125f, 0.142857143f);
+    q = fmaf(z, q, -0.166666667f);
+    q = fmaf(z, q, 0.2f);
+    q = fmaf(z, q, -0.25f);
+    q = fmaf(z, q, 0.333333333f);
+    q = fmaf(z, q, -0.5f);
+    return -fmaf(z * z, q, z);
+  }
+  return -epr_log1p_cold(z);
+}
+
 // Projection to the single-thickness manifold, Eq. (7) + PAPER.md:233 (R10), as an increment:
 //   given τ and ΔT, find δ with Σ_s I_s(τ) expm1(−γ_s δ) = ΔT, clamped so that Σ_s I_s + ΔT ≥ i_min.
 // Newton from the Jensen bound δ0 = −log1p(ΔT/ΣI)/γ̄_I (monotone; exact for one line).
 __device__ __forceinline__ float epr_project_increment(float tau, float dT, const EprLines& L, int newton_iters,
                                                        float i_min) {
   const int nb = L.n_bins;
-  if (nb == 1) {
-    // one line: f = γ = 1, I = e^{−τ};  δ = −log1p(ΔT e^{τ}), floor I + ΔT ≥ i_min  ⇔  1 + z ≥ i_min e^{τ}
-    const float E = __expf(tau);
-    float z = dT * E;
-    if (1.f + z < i_min * E) z = i_min * E - 1.f;
-    return -epr_log1p(z);
-  }
+  if (nb == 1) return epr_project_increment_mono(tau, dT, i_min);
   float Tsum = 0.f, G = 0.f;
   for (int s = 0; s < nb; ++s) {
     const float I = L.f[s] * __expf(-L.gamma[s] * tau);
