@@ -206,9 +206,15 @@ __global__ void __launch_bounds__(128) k_local_march(EprLines L, int nx, int ny,
     sxy_m1.v[k] = sxy_0.v[k] = sxy_p1.v[k] = q_m1.v[k] = q_0.v[k] = q_p1.v[k] = 0.f;
   }
 
+  // software prefetch: τ row of the NEXT step and d row of the next output are in flight during this step
+  float4 tnext = __ldg(reinterpret_cast<const float4*>(tb + (unsigned)wrapm(y0 - 2, ny) * nx + xw));
+  float4 dnext = make_float4(0.f, 0.f, 0.f, 0.f);
   // rows n = y0−2 … y0+MR+1; output row o = n−2 is valid once n ≥ y0+2
   for (int step = 0; step < LM_MR + 4; ++step) {
     const int n = y0 - 2 + step;
+    const float4 tv = tnext, dd = dnext;
+    if (step + 1 < LM_MR + 4) tnext = __ldg(reinterpret_cast<const float4*>(tb + (unsigned)wrapm(n + 1, ny) * nx + xw));
+    if (step >= 3 && n - 1 < ny && writer) dnext = __ldg(reinterpret_cast<const float4*>(db + (unsigned)(n - 1) * nx + xs));
     // ---- shift the windows ----
     t_m1 = t_0; t_0 = t_p1;
     A_m1 = A_0; A_0 = A_p1; A_p1 = A_p2; A0_l = Ap1_l; A0_r = Ap1_r;
@@ -218,7 +224,6 @@ __global__ void __launch_bounds__(128) k_local_march(EprLines L, int nx, int ny,
     q_m1 = q_0; q_0 = q_p1; q0_l = qp1_l; q0_r = qp1_r;
     // ---- new row n: τ and Ad ----
     {
-      const float4 tv = __ldg(reinterpret_cast<const float4*>(tb + (unsigned)wrapm(n, ny) * nx + xw));
       t_p1.v[0] = tv.x; t_p1.v[1] = tv.y; t_p1.v[2] = tv.z; t_p1.v[3] = tv.w;
 #pragma unroll
       for (int k = 0; k < 4; ++k) A_p2.v[k] = epr_expm1(cg * t_p1.v[k]);
@@ -281,7 +286,6 @@ __global__ void __launch_bounds__(128) k_local_march(EprLines L, int nx, int ny,
         }
       }
       const unsigned off = (unsigned)o * nx + xs;
-      const float4 dd = __ldg(reinterpret_cast<const float4*>(db + off));
       *reinterpret_cast<float4*>(ob + off) =
           make_float4((dd.x - 1.f) - v[0], (dd.y - 1.f) - v[1], (dd.z - 1.f) - v[2], (dd.w - 1.f) - v[3]);
     }
