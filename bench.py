@@ -44,9 +44,15 @@ def kernel_bytes_per_px(name, nb, solver):
     }[name]
 
 
-def kernel_px_per_launch(name, nb, batch, plane, launches_init_share):
-    # rows_r2c runs on nb planes per projection in the loop (1 in the init); cols/c2r on 1 output plane.
-    return batch * plane
+def max_over_ranks(value, device):
+    """Max over ranks of a per-rank scalar (the timing reduction of the N > 1 path; works on gloo and nccl)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
 
 
 def peaks():
@@ -205,10 +211,7 @@ def main():
         barrier()
     ms = ev0.elapsed_time(ev1)
     launches = plan.launches - l0
-    if world > 1:
-        t = torch.tensor([ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, torch.device("cuda", local))
     value = world * B * args.steps / (ms * 1e-3)
 
     # ---- end to end through the public host API: pinned host buffers, H2D + loop + D2H inside the timed region
@@ -218,10 +221,7 @@ def main():
     for _ in range(args.steps):
         epr.epr_retrieve_host(plan, d_host, out_host, w.iterations, w.step)
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, torch.device("cuda", local))
     e2e = world * B * args.steps / e2e_s
 
     # ---- per-kernel device times (CUDA events around every launch, on the launch stream), same K steps

@@ -9,6 +9,6 @@ which the method itself never evaluates) plus Poisson noise.
 
 The recipe is stated in DESIGN.md §"Synthetic inputs".
 """
-from .configs import CONFIGS, Workload, make_workload  # noqa: F401
+from .configs import CONFIGS, Workload, make_workload, shard_range  # noqa: F401
 from .phantom import ellipsoid_phantom  # noqa: F401
 from .simulate import fresnel_detector, poisson_noise  # noqa: F401

@@ -110,3 +110,11 @@ def make_workload(name, n=None, batch=None, noise=True, distinct=None):
                     delta_over_beta=db, solver=c["solver"], iterations=c["iterations"], step=c["step"],
                     max_shift_px=c["S"], target_shift_px=c["target"], d=d, thickness_px=phantoms[0],
                     seed_noise=2000 + num)
+
+
+def shard_range(total, rank, world):
+    """Contiguous, balanced split of `total` independent projections over `world` ranks (no exchange step:
+    PAPER.md:231 is per radiograph).  Returns (start, stop) for `rank`."""
+    base, rem = divmod(int(total), int(world))
+    start = rank * base + min(rank, rem)
+    return start, start + base + (1 if rank < rem else 0)
