@@ -1,37 +1,58 @@
-"""Build libepr.so (hand-written CUDA, sm_100a) in-tree with nvcc.  `python -m paper_2601_22793_b200.build`."""
+"""Build libepr.so (hand-written CUDA, sm_100a) in-tree with nvcc.  `python -m paper_2601_22793_b200.build`.
+
+Every translation unit is compiled to an object in parallel (the FFT kernels are instantiated in
+FFT_GROUPS units from the same source, -DEPR_FFT_GROUP=g), then linked into one shared library."""
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libepr.so")
-SOURCES = ["epr_api.cu", "epr_kernels.cu", "epr_fftk.cu"]
-HEADERS = ["epr_internal.h", "epr_math.cuh", "epr_fft.cuh", os.path.join("..", "..", "include", "epr.h")]
+FFT_GROUPS = 6
+# (source, object stem, extra flags)
+UNITS = [("epr_api.cu", "epr_api", []), ("epr_kernels.cu", "epr_kernels", []), ("epr_fftd.cu", "epr_fftd", [])] + \
+        [("epr_fftk.cu", f"epr_fftk_g{g}", [f"-DEPR_FFT_GROUP={g}"]) for g in range(FFT_GROUPS)]
+HEADERS = ["epr_internal.h", "epr_math.cuh", "epr_fft.cuh", "epr_tma.cuh", os.path.join("..", "..", "include", "epr.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared"]
+              "-Xcompiler", "-fPIC"]
 
 
-def _stale():
-    if not os.path.exists(LIB):
-        return True
-    t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + HEADERS)
+def _newest_header():
+    return max(os.path.getmtime(os.path.join(CSRC, h)) for h in HEADERS)
+
+
+def _compile(unit, nvcc, force, verbose, hdr_t):
+    src, stem, extra = unit
+    obj = os.path.join(OBJ, stem + ".o")
+    src_p = os.path.join(CSRC, src)
+    if not force and os.path.exists(obj) and os.path.getmtime(obj) > max(os.path.getmtime(src_p), hdr_t):
+        return obj, ""
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + extra + ["-c", src, "-o", obj]
+    res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
+    if res.returncode != 0:
+        raise RuntimeError(f"nvcc failed on {src} {extra}:\n" + res.stdout + res.stderr)
+    return obj, res.stderr
 
 
 def build(force=False, verbose=False):
-    """Compile the library if it is missing or older than its sources.  Returns the path."""
-    if not force and not _stale():
-        return LIB
+    """Compile what is missing or older than its sources, link, return the library path."""
+    os.makedirs(OBJ, exist_ok=True)
     nvcc = os.environ.get("NVCC", "nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + SOURCES + ["-o", LIB]
-    res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
-    if res.returncode != 0:
-        raise RuntimeError("nvcc failed:\n" + res.stdout + res.stderr)
+    hdr_t = _newest_header()
+    with ThreadPoolExecutor(max_workers=min(len(UNITS), os.cpu_count() or 4)) as ex:
+        results = list(ex.map(lambda u: _compile(u, nvcc, force, verbose, hdr_t), UNITS))
+    objs = [o for o, _ in results]
     if verbose:
-        sys.stderr.write(res.stderr)
+        sys.stderr.write("".join(log for _, log in results))
+    if force or not os.path.exists(LIB) or any(os.path.getmtime(o) > os.path.getmtime(LIB) for o in objs):
+        res = subprocess.run([nvcc, "-shared", "-o", LIB] + objs, capture_output=True, text=True)
+        if res.returncode != 0:
+            raise RuntimeError("link failed:\n" + res.stdout + res.stderr)
     return LIB
 
 

@@ -8,6 +8,7 @@
 #include "epr_fft.cuh"
 #include "epr_internal.h"
 #include "epr_math.cuh"
+#include "epr_tma.cuh"
 
 using namespace eprfft;
 
@@ -16,149 +17,203 @@ template <int M> struct RowCfg {                // M = nx/2 complex points per r
   static constexpr int ROWS = (TPC >= 128) ? 1 : (128 + TPC - 1) / TPC;   // rows per CTA (≥128 threads)
   static constexpr int NT = TPC * ROWS;
   static constexpr int PL = padded_len(M);
+  static constexpr int STAGE = ROWS * M;        // float2 per staging buffer (ROWS whole rows, contiguous in HBM)
+  // dynamic shared memory: [2 mbarriers | pad to 128 B][stage 0][stage 1][FFT work ROWS x PL]
+  static constexpr size_t OFF_STAGE = 128;
+  static constexpr size_t OFF_WORK = OFF_STAGE + 2 * (size_t)STAGE * sizeof(float2);
+  static constexpr size_t SMEM = OFF_WORK + (size_t)ROWS * PL * sizeof(float2);
+};
+
+// Both row kernels are PERSISTENT and TMA-staged: a CTA walks over groups of ROWS consecutive rows (rows of all
+// planes are contiguous, so one group is one contiguous chunk of HBM); while it transforms group i out of one
+// shared-memory stage, one bulk asynchronous copy (cp.async.bulk, completion on an mbarrier) is already filling
+// the other stage with group i + gridDim.x.  No warp waits on a global load inside the transform.
+struct RowPipe {
+  uint64_t* bar;
+  float2* stage;
+  const float2* src;
+  int nrows, rows_per_group, M, stage_elems;
+  __device__ __forceinline__ void issue(int grp, int buf) const {
+    const int r0 = grp * rows_per_group;
+    const int nr = min(rows_per_group, nrows - r0);
+    const unsigned bytes = (unsigned)nr * (unsigned)M * (unsigned)sizeof(float2);
+    eprtma::fence_proxy_async();
+    eprtma::mbar_expect_tx(&bar[buf], bytes);
+    eprtma::bulk_g2s(stage + (size_t)buf * stage_elems, src + (size_t)r0 * M, bytes, &bar[buf]);
+  }
 };
 
 // ------------------------------------------------------------------------------------------------ rows R2C
-// global → registers (first pass) → shared-memory passes → registers (last pass) → pair exchange → global
+// stage (TMA) → registers (first pass) → shared-memory passes → registers (last pass) → pair exchange → global
 template <int M>
-__global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_r2c(int ny, const float* __restrict__ in, float in_offset,
+__global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_r2c(int nrows, const float* __restrict__ in, float in_offset,
                                                             const float2* __restrict__ tw, const float2* __restrict__ tw2,
                                                             float2* __restrict__ spec) {
   using C = RowCfg<M>;
   using EF = Engine<M, C::TPC, 1, false, false>;
-  __shared__ float2 sm[C::ROWS * C::PL];
-  const int lr = threadIdx.x / C::TPC, t = threadIdx.x - lr * C::TPC;
-  const int row = blockIdx.x * C::ROWS + lr;
-  const bool live = row < ny;
-  const size_t rowoff = ((size_t)blockIdx.y * ny + (live ? row : 0)) * (size_t)M;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
+  float2* stage = reinterpret_cast<float2*>(smem_raw + C::OFF_STAGE);
+  float2* sm = reinterpret_cast<float2*>(smem_raw + C::OFF_WORK);
+  const int tid = threadIdx.x;
+  const int lr = tid / C::TPC, t = tid - lr * C::TPC;
+  const int ngroups = (nrows + C::ROWS - 1) / C::ROWS;
+  const RowPipe pipe{bar, stage, reinterpret_cast<const float2*>(in), nrows, C::ROWS, M, C::STAGE};
+  if (tid == 0) { eprtma::mbar_init(&bar[0], 1); eprtma::mbar_init(&bar[1], 1); eprtma::mbar_fence_init(); }
+  __syncthreads();
+  if (tid == 0 && (int)blockIdx.x < ngroups) pipe.issue(blockIdx.x, 0);
   float2* s = sm + lr * C::PL;
-  const float2* src = reinterpret_cast<const float2*>(in) + rowoff;
-  float2 u0[EF::G0::CNT][EF::R0], uL[EF::GL::CNT][EF::RL];
+  int it = 0;
+  for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x, ++it) {
+    const int buf = it & 1;
+    if (tid == 0 && grp + (int)gridDim.x < ngroups) pipe.issue(grp + gridDim.x, buf ^ 1);
+    eprtma::mbar_wait(&bar[buf], (it >> 1) & 1);
+    const int row = grp * C::ROWS + lr;
+    const bool live = row < nrows;
+    const float2* src = stage + (size_t)buf * C::STAGE + lr * M;
+    float2 u0[EF::G0::CNT][EF::R0], uL[EF::GL::CNT][EF::RL];
 #pragma unroll
-  for (int c = 0; c < EF::G0::CNT; ++c) {
-    const int j = t + c * C::TPC;
+    for (int c = 0; c < EF::G0::CNT; ++c) {
+      const int j = t + c * C::TPC;
 #pragma unroll
-    for (int r = 0; r < EF::R0; ++r) {
-      float2 v = make_float2(0.f, 0.f);
-      if ((EF::G0::FULL || j < EF::G0::T) && live) v = __ldg(&src[j + r * EF::G0::T]);
-      u0[c][r] = make_float2(v.x + in_offset, v.y + in_offset);
+      for (int r = 0; r < EF::R0; ++r) {
+        float2 v = make_float2(0.f, 0.f);
+        if ((EF::G0::FULL || j < EF::G0::T) && live) v = src[j + r * EF::G0::T];
+        u0[c][r] = make_float2(v.x + in_offset, v.y + in_offset);
+      }
     }
-  }
-  EF::run(u0, uL, s, 0, t, tw);
-  __syncthreads();
-#pragma unroll
-  for (int c = 0; c < EF::GL::CNT; ++c) {
-    const int j = t + c * C::TPC;
-    if (EF::GL::FULL || j < EF::GL::T) {
-#pragma unroll
-      for (int q = 0; q < EF::RL; ++q) s[padi(j + q * EF::PL)] = uL[c][q];
-    }
-  }
-  __syncthreads();
-  // X[k] = ½(Z[k] + Z*[M−k]) − (i/2) w^k (Z[k] − Z*[M−k]),  w = e^{−2πi/nx};  k = 0: packed (X[0], X[M])
-  if (live) {
-    float2* dst = spec + rowoff;
+    EF::run(u0, uL, s, 0, t, tw);
+    __syncthreads();
 #pragma unroll
     for (int c = 0; c < EF::GL::CNT; ++c) {
       const int j = t + c * C::TPC;
       if (EF::GL::FULL || j < EF::GL::T) {
 #pragma unroll
-        for (int q = 0; q < EF::RL; ++q) {
-          const int k = j + q * EF::PL;
-          const float2 zk = uL[c][q];
-          if (k == 0) {
-            dst[0] = make_float2(zk.x + zk.y, zk.x - zk.y);
-          } else {
-            const float2 zm = s[padi(M - k)];
-            const float2 wk = __ldg(&tw2[k]);
-            const float2 e = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
-            const float2 o = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));
-            dst[k] = cadd(e, cmul(wk, o));
+        for (int q = 0; q < EF::RL; ++q) s[padi(j + q * EF::PL)] = uL[c][q];
+      }
+    }
+    __syncthreads();
+    // X[k] = ½(Z[k] + Z*[M−k]) − (i/2) w^k (Z[k] − Z*[M−k]),  w = e^{−2πi/nx};  k = 0: packed (X[0], X[M])
+    if (live) {
+      float2* dst = spec + (size_t)row * M;
+#pragma unroll
+      for (int c = 0; c < EF::GL::CNT; ++c) {
+        const int j = t + c * C::TPC;
+        if (EF::GL::FULL || j < EF::GL::T) {
+#pragma unroll
+          for (int q = 0; q < EF::RL; ++q) {
+            const int k = j + q * EF::PL;
+            const float2 zk = uL[c][q];
+            if (k == 0) {
+              dst[0] = make_float2(zk.x + zk.y, zk.x - zk.y);
+            } else {
+              const float2 zm = s[padi(M - k)];
+              const float2 wk = __ldg(&tw2[k]);
+              const float2 e = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
+              const float2 o = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));
+              dst[k] = cadd(e, cmul(wk, o));
+            }
           }
         }
       }
     }
+    __syncthreads();                       // work buffer and stage[buf] are free for the next group
   }
 }
 
 // ------------------------------------------------------------------------------------------------ rows C2R
-// EPI 0: out[plane][y][x] = q.   EPI 1 / 2: τ[plane][y][x] += δ(τ, step·q)  (projection increment, R10) for
+// EPI 0: out[row][x] = q.   EPI 1 / 2: τ[row][x] += δ(τ, step·q)  (projection increment, R10) for
 // one line (closed form) / several lines (Newton).
 template <int M, int EPI>
-__global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_c2r(EprLines L, int ny, const float2* __restrict__ spec,
+__global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_c2r(EprLines L, int nrows, const float2* __restrict__ spec,
                                                             const float2* __restrict__ tw, const float2* __restrict__ tw2,
                                                             float step, int tau_is_zero, int newton_iters,
                                                             float i_min, float* __restrict__ out) {
   using C = RowCfg<M>;
   using EI = Engine<M, C::TPC, 1, true, false>;
-  __shared__ float2 sm[C::ROWS * C::PL];
-  const int lr = threadIdx.x / C::TPC, t = threadIdx.x - lr * C::TPC;
-  const int row = blockIdx.x * C::ROWS + lr;
-  const bool live = row < ny;
-  const size_t rowoff = ((size_t)blockIdx.y * ny + (live ? row : 0)) * (size_t)M;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
+  float2* stage = reinterpret_cast<float2*>(smem_raw + C::OFF_STAGE);
+  float2* sm = reinterpret_cast<float2*>(smem_raw + C::OFF_WORK);
+  const int tid = threadIdx.x;
+  const int lr = tid / C::TPC, t = tid - lr * C::TPC;
+  const int ngroups = (nrows + C::ROWS - 1) / C::ROWS;
+  const RowPipe pipe{bar, stage, spec, nrows, C::ROWS, M, C::STAGE};
+  if (tid == 0) { eprtma::mbar_init(&bar[0], 1); eprtma::mbar_init(&bar[1], 1); eprtma::mbar_fence_init(); }
+  __syncthreads();
+  if (tid == 0 && (int)blockIdx.x < ngroups) pipe.issue(blockIdx.x, 0);
   float2* s = sm + lr * C::PL;
-  const float2* src = spec + rowoff;
-  float2 u0[EI::G0::CNT][EI::R0], uL[EI::GL::CNT][EI::RL];
-  // Z2[k] = (X[k] + X*[M−k]) + i w^{−k} (X[k] − X*[M−k]);  Z2[0] = (x0 + xM) + i (x0 − xM)
-#pragma unroll
-  for (int c = 0; c < EI::G0::CNT; ++c) {
-    const int j = t + c * C::TPC;
-#pragma unroll
-    for (int r = 0; r < EI::R0; ++r) {
-      const int k = j + r * EI::G0::T;
-      float2 z = make_float2(0.f, 0.f);
-      if ((EI::G0::FULL || j < EI::G0::T) && live) {
-        const float2 xk = __ldg(&src[k]);
-        if (k == 0) {
-          z = make_float2(xk.x + xk.y, xk.x - xk.y);
-        } else {
-          const float2 xm = __ldg(&src[M - k]);
-          const float2 wk = __ldg(&tw2[k]);
-          const float2 e = make_float2(xk.x + xm.x, xk.y - xm.y);
-          const float2 o = make_float2(-(xk.y + xm.y), xk.x - xm.x);            // i (xk − xm*)
-          z = cadd(e, cmul(make_float2(wk.x, -wk.y), o));
-        }
-      }
-      u0[c][r] = z;
-    }
-  }
-  // prefetch the τ values the epilogue will update, so that their latency hides behind the transform
-  float2* dst = reinterpret_cast<float2*>(out) + rowoff;
-  float2 tpre[EI::GL::CNT][EI::RL];
-#pragma unroll
-  for (int c = 0; c < EI::GL::CNT; ++c) {
-    const int j = t + c * C::TPC;
-#pragma unroll
-    for (int q = 0; q < EI::RL; ++q) {
-      tpre[c][q] = make_float2(0.f, 0.f);
-      if (EPI != 0 && !tau_is_zero && live && (EI::GL::FULL || j < EI::GL::T)) tpre[c][q] = dst[j + q * EI::PL];
-    }
-  }
-  EI::run(u0, uL, s, 0, t, tw);
-  if (live) {
+  int it = 0;
+  for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x, ++it) {
+    const int buf = it & 1;
+    if (tid == 0 && grp + (int)gridDim.x < ngroups) pipe.issue(grp + gridDim.x, buf ^ 1);
+    const int row = grp * C::ROWS + lr;
+    const bool live = row < nrows;
+    // the τ values the epilogue will update: requested now, consumed after the transform
+    float2* dst = reinterpret_cast<float2*>(out) + (size_t)(live ? row : 0) * M;
+    float2 tpre[EI::GL::CNT][EI::RL];
 #pragma unroll
     for (int c = 0; c < EI::GL::CNT; ++c) {
       const int j = t + c * C::TPC;
-      if (EI::GL::FULL || j < EI::GL::T) {
 #pragma unroll
-        for (int q = 0; q < EI::RL; ++q) {
-          const int idx = j + q * EI::PL;
-          float2 v = uL[c][q];
-          if (EPI == 1) {
-            float2 tau = tpre[c][q];
-            tau.x += epr_project_increment_mono(tau.x, step * v.x, i_min);
-            tau.y += epr_project_increment_mono(tau.y, step * v.y, i_min);
-            v = tau;
-          } else if (EPI == 2) {
-            float2 tau = tpre[c][q];
-            tau.x += epr_project_increment(tau.x, step * v.x, L, newton_iters, i_min);
-            tau.y += epr_project_increment(tau.y, step * v.y, L, newton_iters, i_min);
-            v = tau;
+      for (int q = 0; q < EI::RL; ++q) {
+        tpre[c][q] = make_float2(0.f, 0.f);
+        if (EPI != 0 && !tau_is_zero && live && (EI::GL::FULL || j < EI::GL::T)) tpre[c][q] = dst[j + q * EI::PL];
+      }
+    }
+    eprtma::mbar_wait(&bar[buf], (it >> 1) & 1);
+    const float2* src = stage + (size_t)buf * C::STAGE + lr * M;
+    float2 u0[EI::G0::CNT][EI::R0], uL[EI::GL::CNT][EI::RL];
+    // Z2[k] = (X[k] + X*[M−k]) + i w^{−k} (X[k] − X*[M−k]);  Z2[0] = (x0 + xM) + i (x0 − xM)
+#pragma unroll
+    for (int c = 0; c < EI::G0::CNT; ++c) {
+      const int j = t + c * C::TPC;
+#pragma unroll
+      for (int r = 0; r < EI::R0; ++r) {
+        const int k = j + r * EI::G0::T;
+        float2 z = make_float2(0.f, 0.f);
+        if ((EI::G0::FULL || j < EI::G0::T) && live) {
+          const float2 xk = src[k];
+          if (k == 0) {
+            z = make_float2(xk.x + xk.y, xk.x - xk.y);
+          } else {
+            const float2 xm = src[M - k];
+            const float2 wk = __ldg(&tw2[k]);
+            const float2 e = make_float2(xk.x + xm.x, xk.y - xm.y);
+            const float2 o = make_float2(-(xk.y + xm.y), xk.x - xm.x);            // i (xk − xm*)
+            z = cadd(e, cmul(make_float2(wk.x, -wk.y), o));
           }
-          dst[idx] = v;
+        }
+        u0[c][r] = z;
+      }
+    }
+    EI::run(u0, uL, s, 0, t, tw);
+    if (live) {
+#pragma unroll
+      for (int c = 0; c < EI::GL::CNT; ++c) {
+        const int j = t + c * C::TPC;
+        if (EI::GL::FULL || j < EI::GL::T) {
+#pragma unroll
+          for (int q = 0; q < EI::RL; ++q) {
+            const int idx = j + q * EI::PL;
+            float2 v = uL[c][q];
+            if (EPI == 1) {
+              float2 tau = tpre[c][q];
+              tau.x += epr_project_increment_mono(tau.x, step * v.x, i_min);
+              tau.y += epr_project_increment_mono(tau.y, step * v.y, i_min);
+              v = tau;
+            } else if (EPI == 2) {
+              float2 tau = tpre[c][q];
+              tau.x += epr_project_increment(tau.x, step * v.x, L, newton_iters, i_min);
+              tau.y += epr_project_increment(tau.y, step * v.y, L, newton_iters, i_min);
+              v = tau;
+            }
+            dst[idx] = v;
+          }
         }
       }
     }
+    __syncthreads();                       // work buffer and stage[buf] are free for the next group
   }
 }
 
@@ -290,23 +345,58 @@ k_cols(EprLines L, int M, int mode, float scale, const float* __restrict__ lam_x
 }
 
 // ------------------------------------------------------------------------------------------------ dispatch
-#define EPR_FFT_SIZES(X) X(16) X(32) X(48) X(64) X(80) X(96) X(128) X(160) X(256) X(320) X(512) X(1024) X(2048) X(2160) X(2560)
+// The instantiations are split into EPR_FFT_NGROUPS translation units (this file compiled once per group with
+// -DEPR_FFT_GROUP=g, in parallel: see build.py); epr_fftd.cu routes a size to the group that holds it.
+#ifndef EPR_FFT_GROUP
+#error "compile with -DEPR_FFT_GROUP=<0..5> (paper_2601_22793_b200/build.py does)"
+#endif
+#if EPR_FFT_GROUP == 0
+#define EPR_FFT_SIZES(X) X(2048) X(16) X(32)
+#elif EPR_FFT_GROUP == 1
+#define EPR_FFT_SIZES(X) X(2560) X(48)
+#elif EPR_FFT_GROUP == 2
+#define EPR_FFT_SIZES(X) X(2160) X(64)
+#elif EPR_FFT_GROUP == 3
+#define EPR_FFT_SIZES(X) X(1024) X(80) X(96)
+#elif EPR_FFT_GROUP == 4
+#define EPR_FFT_SIZES(X) X(512) X(320) X(128)
+#else
+#define EPR_FFT_SIZES(X) X(256) X(160)
+#endif
+#define EPR_CAT2(a, b) a##b
+#define EPR_CAT(a, b) EPR_CAT2(a, b)
+#define GFN(name) EPR_CAT(name, EPR_FFT_GROUP)
 
-extern "C" int epr_fft_size_supported(int n) {
+int GFN(epr_fftg_has_)(int n) {
 #define X(n_) if (n == n_) return 1;
   EPR_FFT_SIZES(X)
 #undef X
   return 0;
 }
 
-cudaError_t epr_launch_rows_r2c(const epr_plan_s* p, int planes, const float* in, float in_offset, float2* spec,
-                                cudaStream_t st) {
+// persistent grid: as many CTAs as are resident at once (occupancy x SMs), at most one per row group
+template <typename K> static int row_grid(K kernel, int nt, size_t smem, int ngroups) {
+  int dev = 0, sms = 0, occ = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, nt, smem);
+  const int g = sms * (occ > 0 ? occ : 1);
+  return ngroups < g ? ngroups : g;
+}
+
+cudaError_t GFN(epr_fftg_rows_r2c_)(const epr_plan_s* p, int planes, const float* in, float in_offset, float2* spec,
+                                    cudaStream_t st) {
+  const int nrows = planes * p->ny;
   switch (p->nx) {
 #define X(n_)                                                                                                   \
   case n_: {                                                                                                    \
     using C = RowCfg<n_ / 2>;                                                                                   \
-    dim3 grid((p->ny + C::ROWS - 1) / C::ROWS, planes);                                                         \
-    k_rows_r2c<n_ / 2><<<grid, C::NT, 0, st>>>(p->ny, in, in_offset, p->tw_row, p->tw_r2c, spec);                \
+    static int full = 0;                                                                                        \
+    if (!full) full = row_grid(k_rows_r2c<n_ / 2>, C::NT, C::SMEM, 1 << 30);                                    \
+    const int ngroups = (nrows + C::ROWS - 1) / C::ROWS;                                                        \
+    k_rows_r2c<n_ / 2><<<ngroups < full ? ngroups : full, C::NT, C::SMEM, st>>>(nrows, in, in_offset, p->tw_row, \
+                                                                                 p->tw_r2c, spec);              \
   } break;
     EPR_FFT_SIZES(X)
 #undef X
@@ -315,22 +405,26 @@ cudaError_t epr_launch_rows_r2c(const epr_plan_s* p, int planes, const float* in
   return cudaGetLastError();
 }
 
-cudaError_t epr_launch_rows_c2r(const epr_plan_s* p, int planes, const float2* spec, int epilogue, float step,
-                                int tau_is_zero, float* q_or_tau, cudaStream_t st) {
+template <int M, int EPI>
+static void launch_c2r(const epr_plan_s* p, int nrows, const float2* spec, float step, int tau_is_zero, float* q_or_tau,
+                       cudaStream_t st) {
+  using C = RowCfg<M>;
+  static int full = 0;
+  if (!full) full = row_grid(k_rows_c2r<M, EPI>, C::NT, C::SMEM, 1 << 30);
+  const int ngroups = (nrows + C::ROWS - 1) / C::ROWS;
+  k_rows_c2r<M, EPI><<<ngroups < full ? ngroups : full, C::NT, C::SMEM, st>>>(
+      p->lines, nrows, spec, p->tw_row, p->tw_r2c, step, tau_is_zero, p->opt.newton_iters, p->opt.i_min, q_or_tau);
+}
+
+cudaError_t GFN(epr_fftg_rows_c2r_)(const epr_plan_s* p, int planes, const float2* spec, int epilogue, float step,
+                                    int tau_is_zero, float* q_or_tau, cudaStream_t st) {
+  const int nrows = planes * p->ny;
   switch (p->nx) {
 #define X(n_)                                                                                                   \
   case n_: {                                                                                                    \
-    using C = RowCfg<n_ / 2>;                                                                                   \
-    dim3 grid((p->ny + C::ROWS - 1) / C::ROWS, planes);                                                         \
-    if (epilogue == 0)                                                                                          \
-      k_rows_c2r<n_ / 2, 0><<<grid, C::NT, 0, st>>>(p->lines, p->ny, spec, p->tw_row, p->tw_r2c, step, tau_is_zero, \
-                                                    p->opt.newton_iters, p->opt.i_min, q_or_tau);               \
-    else if (p->n_bins == 1)                                                                                    \
-      k_rows_c2r<n_ / 2, 1><<<grid, C::NT, 0, st>>>(p->lines, p->ny, spec, p->tw_row, p->tw_r2c, step, tau_is_zero, \
-                                                    p->opt.newton_iters, p->opt.i_min, q_or_tau);               \
-    else                                                                                                        \
-      k_rows_c2r<n_ / 2, 2><<<grid, C::NT, 0, st>>>(p->lines, p->ny, spec, p->tw_row, p->tw_r2c, step, tau_is_zero, \
-                                                    p->opt.newton_iters, p->opt.i_min, q_or_tau);               \
+    if (epilogue == 0) launch_c2r<n_ / 2, 0>(p, nrows, spec, step, tau_is_zero, q_or_tau, st);                  \
+    else if (p->n_bins == 1) launch_c2r<n_ / 2, 1>(p, nrows, spec, step, tau_is_zero, q_or_tau, st);            \
+    else launch_c2r<n_ / 2, 2>(p, nrows, spec, step, tau_is_zero, q_or_tau, st);                                \
   } break;
     EPR_FFT_SIZES(X)
 #undef X
@@ -339,7 +433,7 @@ cudaError_t epr_launch_rows_c2r(const epr_plan_s* p, int planes, const float2* s
   return cudaGetLastError();
 }
 
-cudaError_t epr_launch_cols(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st) {
+cudaError_t GFN(epr_fftg_cols_)(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st) {
   const int M = p->nx / 2;
   const int oplanes = (mode == 1) ? planes / p->n_bins : planes;
   const float scale = (float)(1.0 / ((double)p->nx * (double)p->ny));

@@ -169,6 +169,11 @@ __global__ void __launch_bounds__(256) k_forward_local(EprLines L, int nx, int n
 // -----------------------------------------------------------------------------------------------------
 #define LM_MR 32                     // output rows per warp
 #define LM_BW 120                    // output columns per warp
+#ifndef LM_UNROLL
+#define LM_UNROLL 1
+#endif
+#define EPR_PRAGMA(x) _Pragma(#x)
+#define EPR_UNROLL(n) EPR_PRAGMA(unroll n)
 
 struct F4 { float v[4]; };
 __device__ __forceinline__ float shfl_l(float x) { return __shfl_up_sync(0xffffffffu, x, 1); }     // from lane-1
@@ -210,6 +215,7 @@ __global__ void __launch_bounds__(128) k_local_march(EprLines L, int nx, int ny,
   float4 tnext = __ldg(reinterpret_cast<const float4*>(tb + (unsigned)wrapm(y0 - 2, ny) * nx + xw));
   float4 dnext = make_float4(0.f, 0.f, 0.f, 0.f);
   // rows n = y0−2 … y0+MR+1; output row o = n−2 is valid once n ≥ y0+2
+  EPR_UNROLL(LM_UNROLL)
   for (int step = 0; step < LM_MR + 4; ++step) {
     const int n = y0 - 2 + step;
     const float4 tv = tnext, dd = dnext;
