@@ -32,7 +32,7 @@ UNIT = "projections/s"
 # ---- algorithmic bytes per pixel per LAUNCH of each kernel family (fp32) ----
 def kernel_bytes_per_px(name, nb, solver):
     return {
-        "k_forward_local": 4 + 4 * nb,          # R tau, W (P_s - f_s) x nb
+        "k_forward_local": 12 if nb == 1 else 4 + 4 * nb,   # 1 line: fused march R tau, R d, W e; else R tau, W (P_s - f_s) x nb
         "k_splat": 4 + 4 * nb,                  # R tau, RED fixed-point planes x nb
         "k_residual": 4 + 8 * nb,               # R d, R pred x nb, W e_s x nb
         "k_gather": 4 + 8 * nb,                 # R tau, R e_s x nb, W r_s x nb

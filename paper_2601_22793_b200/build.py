@@ -39,17 +39,22 @@ def _compile(unit, nvcc, force, verbose, hdr_t):
     return obj, res.stderr
 
 
-def build(force=False, verbose=False):
-    """Compile what is missing or older than its sources, link, return the library path."""
+def build(force=False, verbose=False, dev=False):
+    """Compile what is missing or older than its sources, link, return the library path.
+    dev=True: developer build with FFT group 0 only (2048, 16, 32) — seconds instead of a minute; never ship it."""
     os.makedirs(OBJ, exist_ok=True)
     nvcc = os.environ.get("NVCC", "nvcc")
     hdr_t = _newest_header()
-    with ThreadPoolExecutor(max_workers=min(len(UNITS), os.cpu_count() or 4)) as ex:
-        results = list(ex.map(lambda u: _compile(u, nvcc, force, verbose, hdr_t), UNITS))
+    units = UNITS
+    if dev:
+        units = [u for u in UNITS if u[0] != "epr_fftk.cu" or u[1].endswith("_g0")]
+        units = [(s, st + "_dev", ex + ["-DEPR_FFT_DEV"]) if s == "epr_fftd.cu" else (s, st, ex) for s, st, ex in units]
+    with ThreadPoolExecutor(max_workers=min(len(units), os.cpu_count() or 4)) as ex:
+        results = list(ex.map(lambda u: _compile(u, nvcc, force, verbose, hdr_t), units))
     objs = [o for o, _ in results]
     if verbose:
         sys.stderr.write("".join(log for _, log in results))
-    if force or not os.path.exists(LIB) or any(os.path.getmtime(o) > os.path.getmtime(LIB) for o in objs):
+    if True:  # always relink: a dev and a full build share the output name
         res = subprocess.run([nvcc, "-shared", "-o", LIB] + objs, capture_output=True, text=True)
         if res.returncode != 0:
             raise RuntimeError("link failed:\n" + res.stdout + res.stderr)
@@ -57,4 +62,4 @@ def build(force=False, verbose=False):
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, dev="--dev" in sys.argv))

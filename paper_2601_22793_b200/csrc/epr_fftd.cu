@@ -2,7 +2,11 @@
 // epr_fftk.cu is compiled EPR_FFT_NGROUPS times (-DEPR_FFT_GROUP=g), each with a subset of the supported sizes.
 #include "epr_internal.h"
 
+#ifdef EPR_FFT_DEV          /* developer build: only group 0 (2048, 16, 32) is compiled */
+#define EPR_FFT_GROUPS(G) G(0)
+#else
 #define EPR_FFT_GROUPS(G) G(0) G(1) G(2) G(3) G(4) G(5)
+#endif
 
 #define G(g)                                                                                                          \
   int epr_fftg_has_##g(int n);                                                                                        \

@@ -160,17 +160,24 @@ __global__ void __launch_bounds__(256) k_forward_local(EprLines L, int nx, int n
 }
 
 // -----------------------------------------------------------------------------------------------------
-// Register-marching variant of the fused closure + residual for one spectral line (the hot configuration).
+// k_local_march — the fused closure + residual for one spectral line (the hot configuration), register marching.
 // A warp owns a band of 128 columns (lane l: 4 consecutive pixels; lanes 0 and 31 are halo providers, lanes
-// 1..30 write 120 output columns) and marches down MR output rows.  Every row of τ is loaded ONCE from global
-// memory as a float4 per lane; all x-neighbours come from warp shuffles and all y-neighbours from rolling
-// registers, so the kernel uses no shared memory and no barriers and is bound by fp32 issue.
-// Pipeline per step (new τ row n): Ad[n] → stage-2 row m = n−1 (Î gx², Î gy², Î gx gy, Q) → output row o = n−2.
+// 1..30 write 120 output columns) and marches down LM_MR output rows.  Every row of τ and d is fetched ONCE
+// (cp.async ring, see below); all x-neighbours come from warp shuffles and all y-neighbours from rolling
+// registers; no barriers.  The arithmetic is organised so that every neighbour difference is formed once:
+//   * each stage-2 row m SCATTERS its contributions into three rolling accumulator rows (m−1, m, m+1) instead of
+//     every output row gathering from three stored rows of Î gx², Î gy², Î gx gy and Q;
+//   * y-differences (J, A, Q, fluxes) are shared between the two rows they separate, x-differences between the
+//     two pixels they separate;
+//   * constant factors are folded: S'_ij = c2 Î ∂_iτ ∂_jτ with c2 = (a²/2)(γ/2)², H = ½Î (the flux mean).
+//   v[o] = J[o] − a ∇²₅J + [D²x S'xx + D²y S'yy + 2 D⁰xD⁰y S'xy] − (α²/4) Σ_i D⁻_i(Ī_i D⁺_i Q),  out = (d − 1) − v.
+// Rolling rows (suffix a = m−1, b = m, c = m+1 = newest row n); output row o = m − 1 is final after stage 2 of m.
+// ≈ 62 fp32 instructions per pixel: bound by fp32 issue, not by HBM (12 B/px) — DESIGN.md §7.
 // -----------------------------------------------------------------------------------------------------
 #define LM_MR 32                     // output rows per warp
 #define LM_BW 120                    // output columns per warp
 #ifndef LM_UNROLL
-#define LM_UNROLL 1
+#define LM_UNROLL 4
 #endif
 #define EPR_PRAGMA(x) _Pragma(#x)
 #define EPR_UNROLL(n) EPR_PRAGMA(unroll n)
@@ -179,13 +186,28 @@ struct F4 { float v[4]; };
 __device__ __forceinline__ float shfl_l(float x) { return __shfl_up_sync(0xffffffffu, x, 1); }     // from lane-1
 __device__ __forceinline__ float shfl_r(float x) { return __shfl_down_sync(0xffffffffu, x, 1); }   // from lane+1
 
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+struct W6 { float w[6]; };
+__device__ __forceinline__ W6 window(const F4& v) {
+  W6 r;
+  r.w[0] = shfl_l(v.v[3]);
+  r.w[1] = v.v[0]; r.w[2] = v.v[1]; r.w[3] = v.v[2]; r.w[4] = v.v[3];
+  r.w[5] = shfl_r(v.v[0]);
+  return r;
+}
+
 __global__ void __launch_bounds__(128) k_local_march(EprLines L, int nx, int ny, int order, int wkb1,
                                                      const float* __restrict__ tau, const float* __restrict__ d,
                                                      float* __restrict__ out) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int band = blockIdx.x * 4 + warp;
-  const int xs = band * LM_BW - 4 + 4 * lane;              // first of this lane's 4 columns (may be < 0 or >= nx)
-  if (band * LM_BW >= nx) return;                          // whole warp out of range (no barriers in this kernel)
+  const int xs = band * LM_BW - 4 + 4 * lane;
+  if (band * LM_BW >= nx) return;
   const int y0 = blockIdx.y * LM_MR;
   const unsigned plane = (unsigned)nx * (unsigned)ny;
   const float* tb = tau + (size_t)blockIdx.z * plane;
@@ -193,108 +215,140 @@ __global__ void __launch_bounds__(128) k_local_march(EprLines L, int nx, int ny,
   float* ob = out + (size_t)blockIdx.z * plane;
   const int xw = wrapm(xs, nx);
   const bool writer = lane >= 1 && lane <= 30 && xs < nx;
-  const float cg = -0.5f * L.gamma[0], a = L.a[0], a2h = L.a2h[0], q4 = L.q4[0];
+  const float cg = -0.5f * L.gamma[0], a = L.a[0], q4 = L.q4[0];
+  const float c2 = L.a2h[0] * cg * cg;
+  const bool o2 = order == 2, wk = o2 && wkb1;
 
-  // rolling registers (suffix: row relative to the output row o):  p1 = o+1 (= m), 0 = o, m1 = o−1
-  F4 t_m1, t_0, t_p1;                       // τ rows m−1.. for stage 2 (t_p1 is the newest row n after the shift)
-  F4 A_m1, A_0, A_p1, A_p2;                 // Ad rows o−1, o, o+1, o+2 (A_p2 = newest)
-  float A0_l = 0.f, A0_r = 0.f, Ap1_l = 0.f, Ap1_r = 0.f;      // x-halo of Ad rows o and o+1
-  F4 sxx_0, syy_m1, syy_0, syy_p1, sxy_m1, sxy_0, sxy_p1, q_m1, q_0, q_p1;
-  float sxx0_l = 0.f, sxx0_r = 0.f, sxxp1_l = 0.f, sxxp1_r = 0.f;
-  float sxym1_l = 0.f, sxym1_r = 0.f, sxy0_l = 0.f, sxy0_r = 0.f, sxyp1_l = 0.f, sxyp1_r = 0.f;
-  float q0_l = 0.f, q0_r = 0.f, qp1_l = 0.f, qp1_r = 0.f;
-  F4 sxx_p1;
+  F4 t_a, t_b, t_c, A_b, dA_lo, J_a, J_b, H_a, Q_a, ACC_a, ACC_b;
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
-    t_m1.v[k] = t_0.v[k] = t_p1.v[k] = 0.f; A_m1.v[k] = A_0.v[k] = A_p1.v[k] = A_p2.v[k] = 0.f;
-    sxx_0.v[k] = sxx_p1.v[k] = syy_m1.v[k] = syy_0.v[k] = syy_p1.v[k] = 0.f;
-    sxy_m1.v[k] = sxy_0.v[k] = sxy_p1.v[k] = q_m1.v[k] = q_0.v[k] = q_p1.v[k] = 0.f;
+    t_a.v[k] = t_b.v[k] = t_c.v[k] = A_b.v[k] = dA_lo.v[k] = J_a.v[k] = J_b.v[k] = 0.f;
+    H_a.v[k] = 0.5f; Q_a.v[k] = ACC_a.v[k] = ACC_b.v[k] = 0.f;
   }
-
-  // software prefetch: τ row of the NEXT step and d row of the next output are in flight during this step
-  float4 tnext = __ldg(reinterpret_cast<const float4*>(tb + (unsigned)wrapm(y0 - 2, ny) * nx + xw));
-  float4 dnext = make_float4(0.f, 0.f, 0.f, 0.f);
-  // rows n = y0−2 … y0+MR+1; output row o = n−2 is valid once n ≥ y0+2
+  __shared__ float4 ring_t[LM_D][128], ring_d[LM_D][128];
+  const unsigned tid = threadIdx.x;
+  // row pointers advance by one row per request (τ rows wrap periodically, d / out rows never leave the plane)
+  int yr = wrapm(y0 - 2, ny);
+  const float* tp = tb + (unsigned)yr * nx + xw;
+  const float* dp = db + (unsigned)y0 * nx + xs;
+  float* op = ob + (unsigned)y0 * nx + xs;
+#pragma unroll
+  for (int i = 0; i < LM_D - 1; ++i) {
+    cp_async16(&ring_t[i][tid], tp);
+    tp += nx;
+    if (++yr == ny) { yr = 0; tp -= plane; }
+    cp_async_commit();                             // (no d row is due before step 4 > LM_D − 2)
+  }
+  static_assert(LM_D <= 5, "d rows of the prologue are not requested");
   EPR_UNROLL(LM_UNROLL)
   for (int step = 0; step < LM_MR + 4; ++step) {
     const int n = y0 - 2 + step;
-    const float4 tv = tnext, dd = dnext;
-    if (step + 1 < LM_MR + 4) tnext = __ldg(reinterpret_cast<const float4*>(tb + (unsigned)wrapm(n + 1, ny) * nx + xw));
-    if (step >= 3 && n - 1 < ny && writer) dnext = __ldg(reinterpret_cast<const float4*>(db + (unsigned)(n - 1) * nx + xs));
-    // ---- shift the windows ----
-    t_m1 = t_0; t_0 = t_p1;
-    A_m1 = A_0; A_0 = A_p1; A_p1 = A_p2; A0_l = Ap1_l; A0_r = Ap1_r;
-    sxx_0 = sxx_p1; sxx0_l = sxxp1_l; sxx0_r = sxxp1_r;
-    syy_m1 = syy_0; syy_0 = syy_p1;
-    sxy_m1 = sxy_0; sxy_0 = sxy_p1; sxym1_l = sxy0_l; sxym1_r = sxy0_r; sxy0_l = sxyp1_l; sxy0_r = sxyp1_r;
-    q_m1 = q_0; q_0 = q_p1; q0_l = qp1_l; q0_r = qp1_r;
-    // ---- new row n: τ and Ad ----
     {
-      t_p1.v[0] = tv.x; t_p1.v[1] = tv.y; t_p1.v[2] = tv.z; t_p1.v[3] = tv.w;
-#pragma unroll
-      for (int k = 0; k < 4; ++k) A_p2.v[k] = epr_expm1(cg * t_p1.v[k]);
-    }
-    // after the shift: stage-2 row m = n−1 has τ rows (t_m1, t_0, t_p1) = (m−1, m, m+1) and Ad rows (A_0, A_p1, A_p2)
-    // — careful: A_p1 is row m (= o+1), A_0 is row m−1, A_p2 is row m+1.
-    {
-      const float tl = shfl_l(t_0.v[3]), tr = shfl_r(t_0.v[0]);
-      Ap1_l = shfl_l(A_p1.v[3]); Ap1_r = shfl_r(A_p1.v[0]);
-      if (order == 2) {
-        const float tw_[6] = {tl, t_0.v[0], t_0.v[1], t_0.v[2], t_0.v[3], tr};
-        const float aw_[6] = {Ap1_l, A_p1.v[0], A_p1.v[1], A_p1.v[2], A_p1.v[3], Ap1_r};
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const float gx = cg * (tw_[k + 2] - tw_[k]), gy = cg * (t_p1.v[k] - t_m1.v[k]);
-          const float ac = aw_[k + 1], A = 1.f + ac, I = A * A, igx = I * gx;
-          sxx_p1.v[k] = igx * gx; sxy_p1.v[k] = igx * gy; syy_p1.v[k] = I * gy * gy;
-          q_p1.v[k] = __fdividef(((aw_[k + 2] - ac) + (aw_[k] - ac)) + ((A_0.v[k] - ac) + (A_p2.v[k] - ac)), A);
+      const int sl = (step + LM_D - 1) % LM_D, ahead = step + LM_D - 1;
+      if (ahead < LM_MR + 4) {
+        cp_async16(&ring_t[sl][tid], tp);
+        tp += nx;
+        if (++yr == ny) { yr = 0; tp -= plane; }
+        if (ahead >= 4) {                            // d row of output row y0 − 4 + ahead
+          if (y0 - 4 + ahead < ny && writer) cp_async16(&ring_d[sl][tid], dp);
+          dp += nx;
         }
-        sxxp1_l = shfl_l(sxx_p1.v[3]); sxxp1_r = shfl_r(sxx_p1.v[0]);
-        sxyp1_l = shfl_l(sxy_p1.v[3]); sxyp1_r = shfl_r(sxy_p1.v[0]);
-        qp1_l = shfl_l(q_p1.v[3]); qp1_r = shfl_r(q_p1.v[0]);
+      }
+      cp_async_commit();
+      cp_async_wait<LM_D - 1>();
+    }
+    const float4 tv = ring_t[step % LM_D][tid], dd = ring_d[step % LM_D][tid];
+    // ---- rotate ----
+    t_a = t_b; t_b = t_c;
+    t_c.v[0] = tv.x; t_c.v[1] = tv.y; t_c.v[2] = tv.z; t_c.v[3] = tv.w;
+    // ---- stage 1 on the new row n: A, J, and the y-difference of A towards row m ----
+    F4 A_c, J_c, dA_hi;
+    {
+      const float x0 = cg * t_c.v[0], x1 = cg * t_c.v[1], x2 = cg * t_c.v[2], x3 = cg * t_c.v[3];
+      const float mx = fmaxf(fmaxf(fabsf(x0), fabsf(x1)), fmaxf(fabsf(x2), fabsf(x3)));
+      if (__any_sync(0xffffffffu, mx >= 0.35f)) {        // rare (thick object): both branches of epr_expm1
+        A_c.v[0] = epr_expm1(x0); A_c.v[1] = epr_expm1(x1); A_c.v[2] = epr_expm1(x2); A_c.v[3] = epr_expm1(x3);
+      } else {
+        A_c.v[0] = epr_expm1_small(x0); A_c.v[1] = epr_expm1_small(x1);
+        A_c.v[2] = epr_expm1_small(x2); A_c.v[3] = epr_expm1_small(x3);
       }
     }
-    // ---- output row o = n − 2: Ad rows (A_m1, A_0, A_p1) = (o−1, o, o+1); halo of row o in A0_l/A0_r ----
-    const int o = n - 2;
-    if (step >= 4 && o < ny && writer) {
-      const float aw_[6] = {A0_l, A_0.v[0], A_0.v[1], A_0.v[2], A_0.v[3], A0_r};
-      float Jr[6], Ir[6];
 #pragma unroll
-      for (int k = 0; k < 6; ++k) { Jr[k] = aw_[k] * (2.f + aw_[k]); Ir[k] = Jr[k] + 1.f; }
-      float v[4];
-      float Jn[4], Js[4];
+    for (int k = 0; k < 4; ++k) {
+      J_c.v[k] = A_c.v[k] * (2.f + A_c.v[k]);
+      dA_hi.v[k] = A_c.v[k] - A_b.v[k];
+    }
+    // ---- stage 2 on row m = n − 1: scatter into ACC_a (row m−1, final after this), ACC_b (row m), ACC_c (row m+1) ----
+    F4 ACC_c, H_b, Q_b;
+    {
+      const W6 Jw = window(J_b);
+      float dJ[5];
+#pragma unroll
+      for (int i = 0; i < 5; ++i) dJ[i] = Jw.w[i + 1] - Jw.w[i];
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
-        Jn[k] = A_m1.v[k] * (2.f + A_m1.v[k]); Js[k] = A_p1.v[k] * (2.f + A_p1.v[k]);
-        const float Jc = Jr[k + 1];
-        v[k] = fmaf(-a, ((Jr[k + 2] - Jc) + (Jr[k] - Jc)) + ((Jn[k] - Jc) + (Js[k] - Jc)), Jc);
+        const float g = J_b.v[k] - J_a.v[k];                       // y-difference of J across m−½
+        ACC_b.v[k] = fmaf(-a, dJ[k + 1] - dJ[k], fmaf(a, g, ACC_b.v[k]));
+        ACC_a.v[k] = fmaf(-a, g, ACC_a.v[k]);
+        ACC_c.v[k] = 0.f;
+        H_b.v[k] = fmaf(0.5f, J_b.v[k], 0.5f);
+        Q_b.v[k] = 0.f;
       }
-      if (order == 2) {
-        const float xx[6] = {sxx0_l, sxx_0.v[0], sxx_0.v[1], sxx_0.v[2], sxx_0.v[3], sxx0_r};
-        const float xn[6] = {sxym1_l, sxy_m1.v[0], sxy_m1.v[1], sxy_m1.v[2], sxy_m1.v[3], sxym1_r};
-        const float xs_[6] = {sxyp1_l, sxy_p1.v[0], sxy_p1.v[1], sxy_p1.v[2], sxy_p1.v[3], sxyp1_r};
+      if (o2) {
+        const W6 tw = window(t_b);
+        F4 Sxx, Sxy;
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-          const float sxx = (xx[k + 2] - xx[k + 1]) + (xx[k] - xx[k + 1]);
-          const float syy = (syy_p1.v[k] - syy_0.v[k]) + (syy_m1.v[k] - syy_0.v[k]);
-          const float sxy2 = 0.5f * ((xs_[k + 2] - xs_[k]) - (xn[k + 2] - xn[k]));
-          v[k] = fmaf(a2h, (sxx + syy) + sxy2, v[k]);
+          const float dx = tw.w[k + 2] - tw.w[k], dy = t_c.v[k] - t_a.v[k];
+          const float Ic = fmaf(c2, J_b.v[k], c2), tt = Ic * dx, Syy = Ic * dy * dy;
+          Sxx.v[k] = tt * dx; Sxy.v[k] = tt * dy;
+          ACC_c.v[k] = Syy;
+          ACC_b.v[k] = fmaf(-2.f, Syy, ACC_b.v[k]);
+          ACC_a.v[k] += Syy;
         }
-        if (wkb1) {
-          const float qq[6] = {q0_l, q_0.v[0], q_0.v[1], q_0.v[2], q_0.v[3], q0_r};
+        const W6 xw6 = window(Sxx), yw6 = window(Sxy);
+        float dS[5];
+#pragma unroll
+        for (int i = 0; i < 5; ++i) dS[i] = xw6.w[i + 1] - xw6.w[i];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const float cx = yw6.w[k + 2] - yw6.w[k];
+          ACC_b.v[k] += dS[k + 1] - dS[k];
+          ACC_c.v[k] = fmaf(-0.5f, cx, ACC_c.v[k]);
+          ACC_a.v[k] = fmaf(0.5f, cx, ACC_a.v[k]);
+        }
+        if (wk) {
+          const W6 Aw = window(A_b);
+          float dAx[5];
+#pragma unroll
+          for (int i = 0; i < 5; ++i) dAx[i] = Aw.w[i + 1] - Aw.w[i];
+#pragma unroll
+          for (int k = 0; k < 4; ++k)
+            Q_b.v[k] = __fdividef((dAx[k + 1] - dAx[k]) + (dA_hi.v[k] - dA_lo.v[k]), 1.f + A_b.v[k]);
+          const W6 Qw = window(Q_b);
+          float Hw[6], Fx[5];
+#pragma unroll
+          for (int i = 0; i < 6; ++i) Hw[i] = fmaf(0.5f, Jw.w[i], 0.5f);
+#pragma unroll
+          for (int i = 0; i < 5; ++i) Fx[i] = (Hw[i + 1] + Hw[i]) * (Qw.w[i + 1] - Qw.w[i]);
 #pragma unroll
           for (int k = 0; k < 4; ++k) {
-            const float Ic = Ir[k + 1], Qc = qq[k + 1], In = Jn[k] + 1.f, Is = Js[k] + 1.f;
-            const float div = 0.5f * (((Ir[k + 2] + Ic) * (qq[k + 2] - Qc) - (Ic + Ir[k]) * (Qc - qq[k]))
-                                      + ((Is + Ic) * (q_p1.v[k] - Qc) - (Ic + In) * (Qc - q_m1.v[k])));
-            v[k] = fmaf(-q4, div, v[k]);
+            const float Fy = (H_b.v[k] + H_a.v[k]) * (Q_b.v[k] - Q_a.v[k]);    // flux across m−½
+            ACC_b.v[k] = fmaf(-q4, Fx[k + 1] - Fx[k], fmaf(q4, Fy, ACC_b.v[k]));
+            ACC_a.v[k] = fmaf(-q4, Fy, ACC_a.v[k]);
           }
         }
       }
-      const unsigned off = (unsigned)o * nx + xs;
-      *reinterpret_cast<float4*>(ob + off) =
-          make_float4((dd.x - 1.f) - v[0], (dd.y - 1.f) - v[1], (dd.z - 1.f) - v[2], (dd.w - 1.f) - v[3]);
     }
+    // ---- output row o = n − 2 = m − 1 ----
+    const int o = n - 2;
+    if (step >= 4 && o < ny && writer) {
+      *reinterpret_cast<float4*>(op + (unsigned)(step - 4) * nx) =
+          make_float4((dd.x - 1.f) - (J_a.v[0] + ACC_a.v[0]), (dd.y - 1.f) - (J_a.v[1] + ACC_a.v[1]),
+                      (dd.z - 1.f) - (J_a.v[2] + ACC_a.v[2]), (dd.w - 1.f) - (J_a.v[3] + ACC_a.v[3]));
+    }
+    // ---- rotate the row windows ----
+    A_b = A_c; dA_lo = dA_hi; J_a = J_b; J_b = J_c; H_a = H_b; Q_a = Q_b; ACC_a = ACC_b; ACC_b = ACC_c;
   }
 }
 

@@ -13,6 +13,17 @@ __device__ __forceinline__ int wrapm(int i, int n) { i %= n; return i < 0 ? i + 
 // expm1 to ~2 ulp RELATIVE accuracy without the slow path of expm1f: Taylor (degree 8) for |x| < 0.35
 // (truncation x^8/9! < 1e-9 relative), exp(x) − 1 with the MUFU exponential beyond (|result| > 0.29 there, so
 // the 2^-22 relative error of ex2.approx stays below 1e-6 relative).  Both branches are evaluated (no divergence).
+// Taylor branch alone (valid for |x| < 0.35): callers test the range once per warp and row.
+__device__ __forceinline__ float epr_expm1_small(float x) {
+  float q = fmaf(x, 2.48015873e-5f, 1.98412698e-4f);
+  q = fmaf(x, q, 1.38888889e-3f);
+  q = fmaf(x, q, 8.33333333e-3f);
+  q = fmaf(x, q, 4.16666667e-2f);
+  q = fmaf(x, q, 1.66666667e-1f);
+  q = fmaf(x, q, 0.5f);
+  return fmaf(x * x, q, x);
+}
+
 __device__ __forceinline__ float epr_expm1(float x) {
   float q = fmaf(x, 2.48015873e-5f, 1.98412698e-4f);
   q = fmaf(x, q, 1.38888889e-3f);
