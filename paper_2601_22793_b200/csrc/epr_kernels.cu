@@ -176,6 +176,9 @@ __global__ void __launch_bounds__(256) k_forward_local(EprLines L, int nx, int n
 // -----------------------------------------------------------------------------------------------------
 #define LM_MR 32                     // output rows per warp
 #define LM_BW 120                    // output columns per warp
+#ifndef LM_D
+#define LM_D 4                       // cp.async ring depth: rows are requested LM_D − 1 steps ahead
+#endif
 #ifndef LM_UNROLL
 #define LM_UNROLL 4
 #endif
