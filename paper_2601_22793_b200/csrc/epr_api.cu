@@ -286,9 +286,8 @@ extern "C" epr_status epr_forward(epr_plan_t p, int batch, const float* tau, flo
     KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, 0, 0, P_sum, P_bins, cs));
   } else {
     if ((st = ensure_raymap(p)) != EPR_OK) return st;
-    CU(p, epr_launch_zero(p->pred, (size_t)batch * p->n_bins * plane * sizeof(unsigned), cs));
-    KL(p, K_SPLAT, cs, epr_launch_splat(p, batch, tau, NULL, NULL, p->raymap, (unsigned*)p->pred, cs));
-    KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, 1, 0, P_sum, P_bins, cs));
+    KL(p, K_SPLAT, cs, epr_launch_splat(p, batch, tau, NULL, NULL, p->raymap, p->pred, 0, NULL, cs));
+    KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, 0, 0, P_sum, P_bins, cs));
     p->raymap_batch = batch;
   }
   return EPR_OK;
@@ -318,9 +317,8 @@ extern "C" epr_status epr_transport(epr_plan_t p, int batch, const float* I_bins
   if (!p->raymap || p->raymap_batch < batch) FAIL(p, EPR_EINVAL, "epr_transport: no ray map stored for batch %d (call epr_forward first)", batch);
   cudaStream_t cs = (cudaStream_t)stream;
   const size_t plane = (size_t)p->nx * p->ny;
-  CU(p, epr_launch_zero(p->pred, (size_t)batch * p->n_bins * plane * sizeof(unsigned), cs));
-  KL(p, K_SPLAT, cs, epr_launch_splat(p, batch, NULL, I_bins, p->raymap, NULL, (unsigned*)p->pred, cs));
-  KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, 1, 1, NULL, P_bins, cs));
+  if (I_bins == P_bins) FAIL(p, EPR_EINVAL, "epr_transport: the splat cannot run in place");
+  KL(p, K_SPLAT, cs, epr_launch_splat(p, batch, NULL, I_bins, p->raymap, NULL, P_bins, 1, NULL, cs));
   return EPR_OK;
 }
 
@@ -364,9 +362,12 @@ static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* ta
       }
       r = p->res;
     } else {
-      CU(p, epr_launch_zero(p->pred, (size_t)planes * plane * sizeof(unsigned), cs));
-      KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, (unsigned*)p->pred, cs));   // a0 + a1-N
-      KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, 1, p->res, cs));             // a2
+      if (p->n_bins == 1) {
+        KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->res, 2, d, cs));       // a0 + a1-N + a2 fused
+      } else {
+        KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->pred, 0, NULL, cs));   // a0 + a1-N
+        KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, 0, p->res, cs));           // a2
+      }
       KL(p, K_GATHER, cs, epr_launch_gather(p, nb, tau, NULL, p->res, p->res2, cs));          // a3
       r = p->res2;
     }

@@ -63,8 +63,9 @@ struct epr_plan_s {
 // d_fuse != NULL (one line only): out = e = (d-1) - (P-1) directly; else out = pred[b][s] = P_s - f_s
 cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float* tau, const float* d_fuse, float* out,
                                      cudaStream_t st);
+// out_mode 0: out[b][s] = P_s − f_s;  1: out[b][s] = P_s (linear transport);  2 (one line): out[b] = e = (d−1) − (P−f)
 cudaError_t epr_launch_splat(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
-                             float2* map_out, unsigned* pfix, cudaStream_t st);
+                             float2* map_out, float* out, int out_mode, const float* d, cudaStream_t st);
 cudaError_t epr_launch_residual(const epr_plan_s* p, int batch, const float* d, const void* pred, int fixed,
                                 float* es, cudaStream_t st);
 cudaError_t epr_launch_pred_out(const epr_plan_s* p, int batch, const void* pred, int fixed, int linear, float* P_sum,

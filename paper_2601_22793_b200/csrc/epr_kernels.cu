@@ -369,115 +369,194 @@ cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float
 }
 
 // =====================================================================================================
-// a1-N  ray map (Eq. (2), clamp R6) + mass-conserving bilinear splat.
-//   One CTA = 64x32 source pixels.  The 4-way scatter is resolved with NATIVE u32 shared-memory atomics on a
-//   fixed-point (2^-26) accumulator tile that covers the source tile plus the halo actually reached by this
-//   tile's rays (h = 1 + max |floor u|, found by a block reduction), then flushed once to the global
-//   fixed-point plane with RED.ADD.  Integer accumulation makes the result independent of the order of the
-//   atomics (deterministic) and conserves mass exactly: the 4th corner gets rint(I·2^26) minus the other three.
-//   Sources: I_s = f_s(1+J) from τ (I_bins == NULL) or an arbitrary plane (epr_transport);
-//            u from τ (map_in == NULL; optionally written to map_out) or from a stored map.
+// a1-N  ray map (Eq. (2), clamp R6) + mass-conserving bilinear splat,
+//       DETECTOR-TILE-OWNED: one CTA owns ST_W x ST_H detector pixels of one projection and walks over every
+//       source pixel that can reach them (the tile grown by H = ceil(S) + 1), so the 4-way scatter is resolved
+//       entirely by NATIVE u32 shared-memory atomics on the CTA's own accumulator tile: no global atomics, no
+//       zero-initialised global plane, no second pass over the prediction.
+//   Accumulation is u32 fixed point (unit 2^-26): independent of the order of the atomics (bit-reproducible) and
+//   exactly mass conserving — the 4th corner receives the source mass minus the other three corners, in integers.
+//   Source mass: tot = rint(f_s 2^26) + rint(f_s 2^26 J), J = expm1(−γ_s τ) (deviation form: the fp32 rounding
+//   acts on the small J only), or rint(I 2^26) for an arbitrary plane (epr_transport).  Corner masses:
+//   (tot · rint(w 2^24) + 2^23) >> 24 in 64-bit integers.
+//   Sources: I_s from τ (I_bins == NULL) or a given plane; u from τ (map_in == NULL; written to map_out by the
+//   tile that owns the source pixel) or from a stored map.
+//   Output (out_mode): 0  out[b][s] = P_s − f_s (float);  1  out[b][s] = P_s;  2 (one line)  out[b] = e =
+//   (d − 1) − (P − f): the detector residual a2 fused into the flush.
 // =====================================================================================================
-#define SP_TX 64
-#define SP_TY 32
-#define SP_PX ((SP_TX * SP_TY) / 256)
+#define ST_W 128
+#define ST_H 64
+#ifndef ST_NT
+#define ST_NT 512                     // threads per CTA
+#endif
 
-__global__ void __launch_bounds__(256) k_splat(EprLines L, int nx, int ny, float S, int hmax,
-                                               const float* __restrict__ tau, const float* __restrict__ I_bins,
-                                               const float2* __restrict__ map_in, float2* __restrict__ map_out,
-                                               unsigned* __restrict__ pfix) {
-  extern __shared__ unsigned s_acc[];                 // (SP_TY + 2 hmax) x (SP_TX + 2 hmax)
-  __shared__ float s_tau[SP_TY + 2][SP_TX + 2];
-  __shared__ int s_h;
-  const int b = blockIdx.z, tid = threadIdx.x;
-  const int x0 = blockIdx.x * SP_TX, y0 = blockIdx.y * SP_TY;
-  const size_t plane = (size_t)nx * ny;
-  const int aw = SP_TX + 2 * hmax;
+// FROM_TAU: sources and ray map from the τ tile staged in shared memory (the loop's configuration);
+// otherwise (epr_transport) both are read from global planes.
+// predicated shared-memory reduction (no branch, no convergence barrier around the atomic)
+__device__ __forceinline__ void red_shared_if(bool p, unsigned* addr, unsigned v) {
+  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %2, 0;\n\t@q red.shared.add.u32 [%0], %1;\n\t}" ::"r"(
+                   (unsigned)__cvta_generic_to_shared(addr)),
+               "r"(v), "r"((unsigned)p)
+               : "memory");
+}
 
-  if (tau) {
+template <bool FROM_TAU, bool MAP_OUT>
+__global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny, float S, int H,
+                                                    const float* __restrict__ tau, const float* __restrict__ I_bins,
+                                                    const float2* __restrict__ map_in, float2* __restrict__ map_out,
+                                                    float* __restrict__ out, int out_mode, const float* __restrict__ d) {
+  extern __shared__ __align__(16) unsigned char st_raw[];
+  unsigned* s_acc = reinterpret_cast<unsigned*>(st_raw);                              // [ST_H][ST_W]
+  float* s_tau = reinterpret_cast<float*>(st_raw + ST_W * ST_H * sizeof(unsigned));   // [RH + 2][TP]
+  const int b = blockIdx.z, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  constexpr int NW = ST_NT / 32;
+  const int x0 = blockIdx.x * ST_W, y0 = blockIdx.y * ST_H;
+  const int RW = ST_W + 2 * H, RH = ST_H + 2 * H;      // source region: columns x0 − H …, rows y0 − H …
+  const int Ha = (H + 1 + 3) & ~3;                     // τ tile halo in x, rounded up to whole 16-byte chunks
+  const int TP = ST_W + 2 * Ha;                        // τ tile pitch; tile column of tile-relative x is x + Ha
+  const unsigned plane = (unsigned)nx * (unsigned)ny;
+
+  if (FROM_TAU) {
+    // τ tile rows y0 − H − 1 …, columns x0 − Ha …: 16-byte cp.async chunks (nx % 4 == 0: a chunk never straddles the wrap)
     const float* tb = tau + (size_t)b * plane;
-    for (int i = tid; i < (SP_TX + 2) * (SP_TY + 2); i += 256) {
-      const int ly = i / (SP_TX + 2), lx = i - ly * (SP_TX + 2);
-      s_tau[ly][lx] = __ldg(&tb[(size_t)wrapm(y0 - 1 + ly, ny) * nx + wrapm(x0 - 1 + lx, nx)]);
+    const int step_x = 128 % nx, step_y = NW % ny;
+    int gy = wrapm(y0 - H - 1 + warp, ny);
+    const int gx0 = wrapm(x0 - Ha + 4 * lane, nx);
+    for (int ly = warp; ly < RH + 2; ly += NW) {
+      const float* row = tb + (unsigned)gy * nx;
+      int gx = gx0;
+      for (int cx = lane; cx < TP / 4; cx += 32) {
+        cp_async16(s_tau + ly * TP + 4 * cx, row + gx);
+        gx += step_x;
+        if (gx >= nx) gx -= nx;
+      }
+      gy += step_y;
+      if (gy >= ny) gy -= ny;
     }
+    cp_async_commit();
   }
+  // Largest |D⁰τ| (times 2) among the sources OUTSIDE the tile: bounds how far away a source can be and still
+  // reach the tile, so that the walk below covers the tile grown by He ≤ H only.
+  __shared__ unsigned s_maxd;
+  if (tid == 0) s_maxd = 0u;
   for (int s = 0; s < L.n_bins; ++s) {
     const size_t pl = ((size_t)b * L.n_bins + s) * plane;
-    if (tid == 0) s_h = 0;
-    __syncthreads();                                   // also orders the previous bin's flush before re-zeroing
-    float ux[SP_PX], uy[SP_PX];
-    int hloc = 0;
-#pragma unroll
-    for (int k = 0; k < SP_PX; ++k) {
-      const int i = tid + k * 256, ty = i / SP_TX, tx = i - ty * SP_TX;
-      const int gx = x0 + tx, gy = y0 + ty;
-      ux[k] = uy[k] = 0.f;
-      if (gx < nx && gy < ny) {
-        if (map_in) {
-          const float2 m = __ldg(&map_in[pl + (size_t)gy * nx + gx]);
-          ux[k] = m.x; uy[k] = m.y;
-        } else {
-          // u = a D⁰ ln I_s = −a γ D⁰τ, clamped to ±S
-          const float c = -0.5f * L.a[s] * L.gamma[s];
-          ux[k] = fminf(fmaxf(c * (s_tau[ty + 1][tx + 2] - s_tau[ty + 1][tx]), -S), S);
-          uy[k] = fminf(fmaxf(c * (s_tau[ty + 2][tx + 1] - s_tau[ty][tx + 1]), -S), S);
-          if (map_out) map_out[pl + (size_t)gy * nx + gx] = make_float2(ux[k], uy[k]);
+    __syncthreads();                                   // previous bin flushed
+    for (int i = tid; i < ST_W * ST_H / 4; i += ST_NT) reinterpret_cast<uint4*>(s_acc)[i] = make_uint4(0u, 0u, 0u, 0u);
+    if (FROM_TAU && s == 0) {
+      cp_async_wait<0>();
+      __syncthreads();
+      float md = 0.f;
+      for (int sy = warp; sy < RH; sy += NW) {
+        const bool yin = sy >= H && sy < H + ST_H;
+        const float* trow = s_tau + (sy + 1) * TP + (Ha - H);
+        for (int sx = lane; sx < RW; sx += 32) {
+          if (yin && sx >= H && sx < H + ST_W) continue;                          // the tile itself is always walked
+          md = fmaxf(md, fmaxf(fabsf(trow[sx + 1] - trow[sx - 1]), fabsf(trow[sx + TP] - trow[sx - TP])));
         }
-        const int fx = (int)floorf(ux[k]), fy = (int)floorf(uy[k]);
-        hloc = max(hloc, max(max(-fx, fx + 1), max(-fy, fy + 1)));
       }
-    }
-    atomicMax(&s_h, hloc);
-    __syncthreads();
-    const int h = min(s_h, hmax);
-    const int rw = SP_TX + 2 * h, rh = SP_TY + 2 * h;
-    for (int i = tid; i < rw * rh; i += 256) { const int ry = i / rw; s_acc[ry * aw + (i - ry * rw)] = 0u; }
-    __syncthreads();
 #pragma unroll
-    for (int k = 0; k < SP_PX; ++k) {
-      const int i = tid + k * 256, ty = i / SP_TX, tx = i - ty * SP_TX;
-      const int gx = x0 + tx, gy = y0 + ty;
-      if (gx < nx && gy < ny) {
-        const float fxf = floorf(ux[k]), fyf = floorf(uy[k]);
-        const double dx = (double)(ux[k] - fxf), dy = (double)(uy[k] - fyf);
-        double Id;                                     // source mass in fixed-point units
-        if (I_bins) Id = (double)__ldg(&I_bins[pl + (size_t)gy * nx + gx]) * EPR_FIX_ONE;
-        else Id = L.fixF[s] * (1.0 + (double)expm1f(-L.gamma[s] * s_tau[ty + 1][tx + 1]));
-        const long long tot = __double2ll_rn(Id);
-        const long long c00 = __double2ll_rn(Id * (1.0 - dx) * (1.0 - dy));
-        const long long c10 = __double2ll_rn(Id * dx * (1.0 - dy));
-        const long long c01 = __double2ll_rn(Id * (1.0 - dx) * dy);
-        const long long c11 = tot - c00 - c10 - c01;
-        const int ax = tx + h + (int)fxf, ay = ty + h + (int)fyf;
-        unsigned* a0 = &s_acc[ay * aw + ax];
-        atomicAdd(a0, (unsigned)c00);
-        atomicAdd(a0 + 1, (unsigned)c10);
-        atomicAdd(a0 + aw, (unsigned)c01);
-        atomicAdd(a0 + aw + 1, (unsigned)c11);
-      }
+      for (int o = 16; o > 0; o >>= 1) md = fmaxf(md, __shfl_xor_sync(0xffffffffu, md, o));
+      if (lane == 0) atomicMax(&s_maxd, __float_as_uint(md));
     }
     __syncthreads();
-    unsigned* pb = pfix + pl;
-    for (int i = tid; i < rw * rh; i += 256) {
-      const int ry = i / rw, rx = i - ry * rw;
-      const unsigned v = s_acc[ry * aw + rx];
-      if (v) atomicAdd(&pb[(size_t)wrapm(y0 - h + ry, ny) * nx + wrapm(x0 - h + rx, nx)], v);
+    const float cs = -0.5f * L.a[s] * L.gamma[s], gam = L.gamma[s], fixFf = (float)L.fixF[s];
+    const int Fi = (int)L.fixFi[s];
+    // a source at distance D from the tile reaches it only if ⌊|u|⌋ + 1 ≥ D
+    int He = H;
+    if (FROM_TAU) He = min(H, (int)fminf(fabsf(cs) * __uint_as_float(s_maxd), S) + 1);
+    const int RWe = ST_W + 2 * He, RHe = ST_H + 2 * He;
+    // Every periodic image of a source pixel inside the region is a distinct candidate: its targets differ by whole
+    // periods, and exactly one image puts a given corner on a given detector pixel — that IS the periodic wrap (R7).
+    // the CTA's 256 threads walk the region in row-major order, 256 sources per pass: (sx, sy) advance incrementally
+    const int adv_y = ST_NT / RWe, adv_x = ST_NT - adv_y * RWe;
+    int sy = tid / RWe, sx = tid - sy * RWe;
+    for (; sy < RHe; sx += adv_x, sy += adv_y) {
+      if (sx >= RWe) { sx -= RWe; ++sy; if (sy >= RHe) break; }
+      const int tx0 = sx - He, ty0 = sy - He;          // source pixel relative to the tile
+      float ux, uy, tc = 0.f;
+      unsigned gidx = 0;
+      if (FROM_TAU) {
+        // u = a D⁰ ln I_s = −a γ D⁰τ, clamped to ±S
+        const float* tp = s_tau + (ty0 + H + 1) * TP + (tx0 + Ha);
+        tc = tp[0];
+        ux = fminf(fmaxf(cs * (tp[1] - tp[-1]), -S), S);
+        uy = fminf(fmaxf(cs * (tp[TP] - tp[-TP]), -S), S);
+        if (MAP_OUT && (unsigned)tx0 < ST_W && (unsigned)ty0 < ST_H && x0 + tx0 < nx && y0 + ty0 < ny)
+          map_out[pl + (unsigned)(y0 + ty0) * nx + (x0 + tx0)] = make_float2(ux, uy);
+      } else {
+        gidx = (unsigned)wrapm(y0 + ty0, ny) * nx + wrapm(x0 + tx0, nx);
+        const float2 m = __ldg(&map_in[pl + gidx]);
+        ux = m.x; uy = m.y;
+      }
+      const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
+      const int ax = tx0 + fx, ay = ty0 + fy;          // top-left target, tile coordinates
+      if ((unsigned)(ax + 1) > ST_W || (unsigned)(ay + 1) > ST_H) continue;      // cannot touch this tile
+      const float dx = ux - (float)fx, dy = uy - (float)fy;
+      int tot;                                         // signed: epr_transport accepts planes of either sign
+      if (FROM_TAU) tot = Fi + __float2int_rn(fixFf * epr_expm1(-gam * tc));
+      else tot = __float2int_rn(__ldg(&I_bins[pl + gidx]) * 67108864.f);
+      // corner masses in fp32 (± 2 units of 2^-26), the 4th corner takes the exact remainder
+      const float totf = (float)tot, ex = 1.f - dx, ey = 1.f - dy;
+      const int c00 = __float2int_rn(totf * ex * ey), c10 = __float2int_rn(totf * dx * ey),
+                c01 = __float2int_rn(totf * ex * dy);
+      const int c11 = tot - c00 - c10 - c01;
+      const bool xin0 = ax >= 0, xin1 = ax + 1 < ST_W, yin0 = ay >= 0, yin1 = ay + 1 < ST_H;
+      unsigned* a0 = s_acc + ay * ST_W + ax;
+      red_shared_if(yin0 && xin0, a0, (unsigned)c00);
+      red_shared_if(yin0 && xin1, a0 + 1, (unsigned)c10);
+      red_shared_if(yin1 && xin0, a0 + ST_W, (unsigned)c01);
+      red_shared_if(yin1 && xin1, a0 + ST_W + 1, (unsigned)c11);
+    }
+    __syncthreads();
+    // flush the tile: 4 pixels per thread per pass
+    const float sc = 1.0f / (float)EPR_FIX_ONE, corr = L.fixCorr[s];
+    for (int i = tid; i < ST_W * ST_H / 4; i += ST_NT) {
+      const int ty = i / (ST_W / 4), tx = 4 * (i - ty * (ST_W / 4));
+      const int gx = x0 + tx, gy = y0 + ty;
+      if (gx >= nx || gy >= ny) continue;
+      const uint4 v = reinterpret_cast<const uint4*>(s_acc)[i];
+      const unsigned g = (unsigned)gy * nx + gx;
+      float4 o;
+      if (out_mode == 1) {
+        o = make_float4((float)(int)v.x * sc, (float)(int)v.y * sc, (float)(int)v.z * sc, (float)(int)v.w * sc);
+      } else {
+        o = make_float4(fmaf((float)((int)v.x - Fi), sc, corr), fmaf((float)((int)v.y - Fi), sc, corr),
+                        fmaf((float)((int)v.z - Fi), sc, corr), fmaf((float)((int)v.w - Fi), sc, corr));
+        if (out_mode == 2) {
+          const float4 dd = __ldg(reinterpret_cast<const float4*>(d + (size_t)b * plane + g));
+          const float off = 1.f + L.fsum_dev;
+          o = make_float4((dd.x - off) - o.x, (dd.y - off) - o.y, (dd.z - off) - o.z, (dd.w - off) - o.w);
+        }
+      }
+      *reinterpret_cast<float4*>(out + pl + g) = o;
     }
   }
 }
 
-cudaError_t epr_launch_splat(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
-                             float2* map_out, unsigned* pfix, cudaStream_t st) {
-  const int hmax = (int)ceilf(p->opt.max_shift_px) + 1;
-  const size_t smem = (size_t)(SP_TX + 2 * hmax) * (SP_TY + 2 * hmax) * sizeof(unsigned);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(k_splat, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
-    attr_set = true;
+template <bool FROM_TAU, bool MAP_OUT>
+static cudaError_t launch_splat_t(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
+                                  float2* map_out, float* out, int out_mode, const float* d, cudaStream_t st) {
+  const int H = (int)ceilf(p->opt.max_shift_px) + 1;
+  const int Ha = (H + 1 + 3) & ~3;
+  const size_t smem = (size_t)ST_W * ST_H * sizeof(unsigned) +
+                      (FROM_TAU ? (size_t)(ST_W + 2 * Ha) * (ST_H + 2 * H + 2) * sizeof(float) : 0);
+  static size_t attr = 0;
+  if (smem > attr) {
+    cudaFuncSetAttribute(k_splat_tile<FROM_TAU, MAP_OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attr = smem;
   }
-  dim3 grid((p->nx + SP_TX - 1) / SP_TX, (p->ny + SP_TY - 1) / SP_TY, batch);
-  k_splat<<<grid, 256, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, hmax, tau, I_bins, map_in, map_out, pfix);
+  dim3 grid((p->nx + ST_W - 1) / ST_W, (p->ny + ST_H - 1) / ST_H, batch);
+  k_splat_tile<FROM_TAU, MAP_OUT><<<grid, ST_NT, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, H, tau, I_bins,
+                                                           map_in, map_out, out, out_mode, d);
   return cudaGetLastError();
+}
+
+cudaError_t epr_launch_splat(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
+                             float2* map_out, float* out, int out_mode, const float* d, cudaStream_t st) {
+  if (!tau) return launch_splat_t<false, false>(p, batch, tau, I_bins, map_in, map_out, out, out_mode, d, st);
+  if (map_out) return launch_splat_t<true, true>(p, batch, tau, I_bins, map_in, map_out, out, out_mode, d, st);
+  return launch_splat_t<true, false>(p, batch, tau, I_bins, map_in, map_out, out, out_mode, d, st);
 }
 
 // =====================================================================================================
@@ -574,46 +653,55 @@ cudaError_t epr_launch_pred_out(const epr_plan_s* p, int batch, const void* pred
 // a3  adjoint ℳ*_s: bilinear gather at the mapped coordinates, Eq. (4), with the SAME
 //     x0, y0, w as the splat of this iteration (ray map recomputed from τ, or the stored one).
 // =====================================================================================================
+template <bool BIG>          // BIG: nx, ny > 32 ≥ |shift| + 1, so one conditional add wraps an index
 __global__ void __launch_bounds__(256) k_gather(EprLines L, int nx, int ny, float S, const float* __restrict__ tau,
                                                 const float2* __restrict__ map_in, const float* __restrict__ es,
                                                 float* __restrict__ r) {
   const int x = blockIdx.x * 64 + (threadIdx.x & 63), y = blockIdx.y * 4 + (threadIdx.x >> 6);
   const int b = blockIdx.z;
   if (x >= nx || y >= ny) return;
-  const size_t plane = (size_t)nx * ny;
-  const int xm = wrap1(x - 1, nx), xp = wrap1(x + 1, nx), ym = wrap1(y - 1, ny), yp = wrap1(y + 1, ny);
+  const unsigned plane = (unsigned)nx * (unsigned)ny, row = (unsigned)y * nx;
   float dtx = 0.f, dty = 0.f;
   if (!map_in) {
     const float* tb = tau + (size_t)b * plane;
-    dtx = __ldg(&tb[(size_t)y * nx + xp]) - __ldg(&tb[(size_t)y * nx + xm]);
-    dty = __ldg(&tb[(size_t)yp * nx + x]) - __ldg(&tb[(size_t)ym * nx + x]);
+    const int xm = wrap1(x - 1, nx), xp = wrap1(x + 1, nx), ym = wrap1(y - 1, ny), yp = wrap1(y + 1, ny);
+    dtx = __ldg(tb + row + xp) - __ldg(tb + row + xm);
+    dty = __ldg(tb + (unsigned)yp * nx + x) - __ldg(tb + (unsigned)ym * nx + x);
   }
-  for (int s = 0; s < L.n_bins; ++s) {
-    const size_t pl = ((size_t)b * L.n_bins + s) * plane;
+  const size_t p0 = (size_t)b * L.n_bins * plane;
+  const float* eb = es + p0;
+  float* rb = r + p0 + row + x;
+  const float2* mb = map_in ? map_in + p0 + row + x : nullptr;
+  for (int s = 0; s < L.n_bins; ++s, eb += plane, rb += plane) {
     float ux, uy;
     if (map_in) {
-      const float2 m = __ldg(&map_in[pl + (size_t)y * nx + x]);
+      const float2 m = __ldg(mb);
+      mb += plane;
       ux = m.x; uy = m.y;
     } else {
       const float c = -0.5f * L.a[s] * L.gamma[s];
       ux = fminf(fmaxf(c * dtx, -S), S);
       uy = fminf(fmaxf(c * dty, -S), S);
     }
-    const float fx = floorf(ux), fy = floorf(uy);
-    const float dx = ux - fx, dy = uy - fy;
-    const int ix0 = wrapm(x + (int)fx, nx), iy0 = wrapm(y + (int)fy, ny);
-    const int ix1 = wrap1(ix0 + 1, nx), iy1 = wrap1(iy0 + 1, ny);
-    const float* eb = es + pl;
-    const float e00 = __ldg(&eb[(size_t)iy0 * nx + ix0]), e10 = __ldg(&eb[(size_t)iy0 * nx + ix1]);
-    const float e01 = __ldg(&eb[(size_t)iy1 * nx + ix0]), e11 = __ldg(&eb[(size_t)iy1 * nx + ix1]);
-    r[pl + (size_t)y * nx + x] = (1.f - dx) * (1.f - dy) * e00 + dx * (1.f - dy) * e10 + (1.f - dx) * dy * e01 + dx * dy * e11;
+    const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
+    const float dx = ux - (float)fx, dy = uy - (float)fy;
+    const int ix0 = BIG ? wrap1(x + fx, nx) : wrapm(x + fx, nx);
+    const int iy0 = BIG ? wrap1(y + fy, ny) : wrapm(y + fy, ny);
+    const int ix1 = ix0 + 1 == nx ? 0 : ix0 + 1, iy1 = iy0 + 1 == ny ? 0 : iy0 + 1;
+    const float* e0 = eb + (unsigned)iy0 * nx;
+    const float* e1 = eb + (unsigned)iy1 * nx;
+    const float e00 = __ldg(e0 + ix0), e10 = __ldg(e0 + ix1), e01 = __ldg(e1 + ix0), e11 = __ldg(e1 + ix1);
+    // Eq. (4): Σ_ab w_ab e[y0+b][x0+a], w00 = (1−dx)(1−dy), w10 = dx(1−dy), w01 = (1−dx)dy, w11 = dx dy
+    const float ex = 1.f - dx, ey = 1.f - dy;
+    *rb = ey * (ex * e00 + dx * e10) + dy * (ex * e01 + dx * e11);
   }
 }
 
 cudaError_t epr_launch_gather(const epr_plan_s* p, int batch, const float* tau, const float2* map_in, const float* es,
                               float* r, cudaStream_t st) {
   dim3 grid((p->nx + 63) / 64, (p->ny + 3) / 4, batch);
-  k_gather<<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, tau, map_in, es, r);
+  if (p->nx > 32 && p->ny > 32) k_gather<true><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, tau, map_in, es, r);
+  else k_gather<false><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, tau, map_in, es, r);
   return cudaGetLastError();
 }
 
