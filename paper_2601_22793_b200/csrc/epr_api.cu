@@ -163,6 +163,8 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
     abar += p->h_f[s] * p->h_a[s];
   }
   L.abar = (float)abar;
+  L.gamma_max = 0.f;
+  for (int s = 0; s < n_bins; ++s) L.gamma_max = fmaxf(L.gamma_max, L.gamma[s]);
   double fs = 0;
   for (int s = 0; s < n_bins; ++s) fs += (double)L.f[s];
   L.fsum_dev = (float)(fs - 1.0);

@@ -139,6 +139,8 @@ __global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_c2r(EprLines L, int nrow
   const int lr = tid / C::TPC, t = tid - lr * C::TPC;
   const int ngroups = (nrows + C::ROWS - 1) / C::ROWS;
   const RowPipe pipe{bar, stage, spec, nrows, C::ROWS, M, C::STAGE};
+  __shared__ float s_f[EPR_MAX_BINS], s_gamma[EPR_MAX_BINS];
+  if (EPI == 2 && tid < L.n_bins) { s_f[tid] = L.f[tid]; s_gamma[tid] = L.gamma[tid]; }
   if (tid == 0) { eprtma::mbar_init(&bar[0], 1); eprtma::mbar_init(&bar[1], 1); eprtma::mbar_fence_init(); }
   __syncthreads();
   if (tid == 0 && (int)blockIdx.x < ngroups) pipe.issue(blockIdx.x, 0);
@@ -204,8 +206,8 @@ __global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_c2r(EprLines L, int nrow
               v = tau;
             } else if (EPI == 2) {
               float2 tau = tpre[c][q];
-              tau.x += epr_project_increment(tau.x, step * v.x, L, newton_iters, i_min);
-              tau.y += epr_project_increment(tau.y, step * v.y, L, newton_iters, i_min);
+              tau.x += epr_project_increment(tau.x, step * v.x, s_f, s_gamma, L.n_bins, L.gamma_max, newton_iters, i_min);
+              tau.y += epr_project_increment(tau.y, step * v.y, s_f, s_gamma, L.n_bins, L.gamma_max, newton_iters, i_min);
               v = tau;
             }
             dst[idx] = v;

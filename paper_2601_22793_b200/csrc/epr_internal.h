@@ -21,6 +21,7 @@ struct EprLines {
   unsigned fixFi[EPR_MAX_BINS]; // rint(f_s · 2^26)
   float fixCorr[EPR_MAX_BINS];  // rint(f_s 2^26)·2^-26 − f_s
   float abar;                   // Σ f_s a_s (initial guess, R9)
+  float gamma_max;              // max_s γ_s (range test of the projection's polynomial form)
   float fsum_dev;               // Σ_s (float)f_s − 1: rounding of the fp32 fractions, removed from the residual
 };
 

@@ -657,49 +657,60 @@ template <bool BIG>          // BIG: nx, ny > 32 ≥ |shift| + 1, so one conditi
 __global__ void __launch_bounds__(256) k_gather(EprLines L, int nx, int ny, float S, const float* __restrict__ tau,
                                                 const float2* __restrict__ map_in, const float* __restrict__ es,
                                                 float* __restrict__ r) {
-  const int x = blockIdx.x * 64 + (threadIdx.x & 63), y = blockIdx.y * 4 + (threadIdx.x >> 6);
+  // one thread = 4 consecutive pixels of one row (nx % 4 == 0)
+  const int x = 4 * (blockIdx.x * 64 + (threadIdx.x & 63)), y = blockIdx.y * 4 + (threadIdx.x >> 6);
   const int b = blockIdx.z;
   if (x >= nx || y >= ny) return;
   const unsigned plane = (unsigned)nx * (unsigned)ny, row = (unsigned)y * nx;
-  float dtx = 0.f, dty = 0.f;
+  float dtx[4] = {0.f, 0.f, 0.f, 0.f}, dty[4] = {0.f, 0.f, 0.f, 0.f};
   if (!map_in) {
     const float* tb = tau + (size_t)b * plane;
-    const int xm = wrap1(x - 1, nx), xp = wrap1(x + 1, nx), ym = wrap1(y - 1, ny), yp = wrap1(y + 1, ny);
-    dtx = __ldg(tb + row + xp) - __ldg(tb + row + xm);
-    dty = __ldg(tb + (unsigned)yp * nx + x) - __ldg(tb + (unsigned)ym * nx + x);
+    const int xm = x == 0 ? nx - 1 : x - 1, xp = x + 4 == nx ? 0 : x + 4;
+    const int ym = y == 0 ? ny - 1 : y - 1, yp = y + 1 == ny ? 0 : y + 1;
+    const float4 c = __ldg(reinterpret_cast<const float4*>(tb + row + x));
+    const float4 n = __ldg(reinterpret_cast<const float4*>(tb + (unsigned)ym * nx + x));
+    const float4 s4 = __ldg(reinterpret_cast<const float4*>(tb + (unsigned)yp * nx + x));
+    const float l = __ldg(tb + row + xm), rr = __ldg(tb + row + xp);
+    dtx[0] = c.y - l; dtx[1] = c.z - c.x; dtx[2] = c.w - c.y; dtx[3] = rr - c.z;
+    dty[0] = s4.x - n.x; dty[1] = s4.y - n.y; dty[2] = s4.z - n.z; dty[3] = s4.w - n.w;
   }
   const size_t p0 = (size_t)b * L.n_bins * plane;
   const float* eb = es + p0;
   float* rb = r + p0 + row + x;
   const float2* mb = map_in ? map_in + p0 + row + x : nullptr;
   for (int s = 0; s < L.n_bins; ++s, eb += plane, rb += plane) {
-    float ux, uy;
-    if (map_in) {
-      const float2 m = __ldg(mb);
-      mb += plane;
-      ux = m.x; uy = m.y;
-    } else {
-      const float c = -0.5f * L.a[s] * L.gamma[s];
-      ux = fminf(fmaxf(c * dtx, -S), S);
-      uy = fminf(fmaxf(c * dty, -S), S);
+    const float c = -0.5f * L.a[s] * L.gamma[s];
+    float o[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      float ux, uy;
+      if (map_in) {
+        const float2 m = __ldg(mb + k);
+        ux = m.x; uy = m.y;
+      } else {
+        ux = fminf(fmaxf(c * dtx[k], -S), S);
+        uy = fminf(fmaxf(c * dty[k], -S), S);
+      }
+      const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
+      const float dx = ux - (float)fx, dy = uy - (float)fy;
+      const int ix0 = BIG ? wrap1(x + k + fx, nx) : wrapm(x + k + fx, nx);
+      const int iy0 = BIG ? wrap1(y + fy, ny) : wrapm(y + fy, ny);
+      const int ix1 = ix0 + 1 == nx ? 0 : ix0 + 1, iy1 = iy0 + 1 == ny ? 0 : iy0 + 1;
+      const unsigned r0 = (unsigned)iy0 * nx, r1 = (unsigned)iy1 * nx;
+      const float e00 = __ldg(eb + (r0 + ix0)), e10 = __ldg(eb + (r0 + ix1));
+      const float e01 = __ldg(eb + (r1 + ix0)), e11 = __ldg(eb + (r1 + ix1));
+      // Eq. (4): Σ_ab w_ab e[y0+b][x0+a], w00 = (1−dx)(1−dy), w10 = dx(1−dy), w01 = (1−dx)dy, w11 = dx dy
+      const float ex = 1.f - dx, ey = 1.f - dy;
+      o[k] = ey * (ex * e00 + dx * e10) + dy * (ex * e01 + dx * e11);
     }
-    const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
-    const float dx = ux - (float)fx, dy = uy - (float)fy;
-    const int ix0 = BIG ? wrap1(x + fx, nx) : wrapm(x + fx, nx);
-    const int iy0 = BIG ? wrap1(y + fy, ny) : wrapm(y + fy, ny);
-    const int ix1 = ix0 + 1 == nx ? 0 : ix0 + 1, iy1 = iy0 + 1 == ny ? 0 : iy0 + 1;
-    const float* e0 = eb + (unsigned)iy0 * nx;
-    const float* e1 = eb + (unsigned)iy1 * nx;
-    const float e00 = __ldg(e0 + ix0), e10 = __ldg(e0 + ix1), e01 = __ldg(e1 + ix0), e11 = __ldg(e1 + ix1);
-    // Eq. (4): Σ_ab w_ab e[y0+b][x0+a], w00 = (1−dx)(1−dy), w10 = dx(1−dy), w01 = (1−dx)dy, w11 = dx dy
-    const float ex = 1.f - dx, ey = 1.f - dy;
-    *rb = ey * (ex * e00 + dx * e10) + dy * (ex * e01 + dx * e11);
+    if (map_in) mb += plane;
+    *reinterpret_cast<float4*>(rb) = make_float4(o[0], o[1], o[2], o[3]);
   }
 }
 
 cudaError_t epr_launch_gather(const epr_plan_s* p, int batch, const float* tau, const float2* map_in, const float* es,
                               float* r, cudaStream_t st) {
-  dim3 grid((p->nx + 63) / 64, (p->ny + 3) / 4, batch);
+  dim3 grid((p->nx / 4 + 63) / 64, (p->ny + 3) / 4, batch);
   if (p->nx > 32 && p->ny > 32) k_gather<true><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, tau, map_in, es, r);
   else k_gather<false><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, tau, map_in, es, r);
   return cudaGetLastError();
