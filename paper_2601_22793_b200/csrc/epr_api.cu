@@ -410,12 +410,25 @@ extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_
   if (batch < 1 || !d_host || !out_host) FAIL(p, EPR_EINVAL, "epr_retrieve_host: bad batch or NULL pointer");
   if (iterations < 0 || !(step > 0.f)) FAIL(p, EPR_EINVAL, "epr_retrieve_host: iterations must be >= 0 and step > 0");
   const size_t plane = (size_t)p->nx * p->ny;
-  const int wbch = p->work_batch;
+  // Host chunks are smaller than the device work batch so that the copies of chunk i±1 overlap the loop of chunk i:
+  // about 64 MB of input per chunk (EPR_HOST_CHUNK overrides), at least 4 chunks per call when the batch allows.
+  int wbch = (int)(((size_t)64 << 20) / (plane * sizeof(float)));
+  if (wbch > (batch + 3) / 4) wbch = (batch + 3) / 4;
+  { const char* env = getenv("EPR_HOST_CHUNK"); if (env && atoi(env) > 0) wbch = atoi(env); }
+  if (wbch < 1) wbch = 1;
+  if (wbch > p->work_batch) wbch = p->work_batch;
+  if (p->stage_in[0] && p->stage_chunk < wbch) {           // staging buffers too small for this call: re-allocate
+    CU(p, cudaDeviceSynchronize());
+    for (int i = 0; i < 2; ++i) { cudaFree(p->stage_in[i]); cudaFree(p->stage_out[i]); p->stage_in[i] = p->stage_out[i] = NULL; }
+  }
   if (!p->stage_in[0]) {
     for (int i = 0; i < 2; ++i) {
       CU(p, cudaMalloc((void**)&p->stage_in[i], (size_t)wbch * plane * sizeof(float)));
       CU(p, cudaMalloc((void**)&p->stage_out[i], (size_t)wbch * plane * sizeof(float)));
     }
+    p->stage_chunk = wbch;
+  }
+  if (!p->hstream[0]) {
     for (int i = 0; i < 3; ++i) CU(p, cudaStreamCreateWithFlags(&p->hstream[i], cudaStreamNonBlocking));
     for (int i = 0; i < 6; ++i) CU(p, cudaEventCreateWithFlags(&p->hev[i], cudaEventDisableTiming));
   }

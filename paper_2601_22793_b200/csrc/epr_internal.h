@@ -51,6 +51,7 @@ struct epr_plan_s {
   // host staging for epr_retrieve_host
   float* stage_in[2];
   float* stage_out[2];
+  int stage_chunk;             // projections the staging buffers hold
   cudaStream_t hstream[3];     // copy-in, compute, copy-out
   cudaEvent_t hev[6];          // per buffer: in-done, compute-done, out-done
   long long launches;
