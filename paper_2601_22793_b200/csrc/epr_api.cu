@@ -104,6 +104,29 @@ static std::vector<float> lambda_table(int n, int count, int symbol) {
   return v;
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time dependency on libcuda)
+static bool make_spec_map(CUtensorMap* map, void* base, int nx, size_t rows) {
+  typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static encode_fn fn = NULL;
+  if (!fn) {
+    void* ptr = NULL;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) != cudaSuccess || !ptr ||
+        qres != cudaDriverEntryPointSuccess)
+      return false;
+    fn = (encode_fn)ptr;
+  }
+  if (rows > 0xffffffffull) return false;
+  const cuuint64_t dims[2] = {(cuuint64_t)nx, (cuuint64_t)rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)nx * sizeof(float)};
+  const cuuint32_t box[2] = {8, 256};
+  const cuuint32_t estr[2] = {1, 1};
+  return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, double L_m, int n_bins,
                                const double* energy_keV, const double* weight, const double* delta_over_beta,
                                epr_solver solver, int max_batch, const epr_options* opt) {
@@ -127,8 +150,9 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
     return EPR_EINVAL;
   if (!epr_fft_size_supported(nx) || !epr_fft_size_supported(ny)) return EPR_ESIZE;
 
-  epr_plan_s* p = (epr_plan_s*)calloc(1, sizeof(epr_plan_s));
+  epr_plan_s* p = (epr_plan_s*)aligned_alloc(64, (sizeof(epr_plan_s) + 63) / 64 * 64);   // CUtensorMap members: 64-byte aligned
   if (!p) return EPR_ENOMEM;
+  memset(p, 0, sizeof(epr_plan_s));
   *out = p;                                   // returned even on failure so that the caller can read the message
   p->nx = nx; p->ny = ny; p->n_bins = n_bins; p->max_batch = max_batch; p->solver = (int)solver; p->opt = o;
   p->opt.mu_rel = NULL;
@@ -196,6 +220,14 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->spec, wb * n_bins * plane * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->spec_sum, wb * plane * sizeof(float));
   if (e != cudaSuccess) FAIL(p, e == cudaErrorMemoryAllocation ? EPR_ENOMEM : EPR_ECUDA, "workspace: %s", cudaGetErrorString(e));
+  // TMA descriptors for the column kernel (power-of-two ny ≥ 256, whole 4-column tiles): the spectra seen as
+  // [rows = planes·ny][nx floats], box = 8 floats (4 complex columns) x 256 rows, no swizzle.
+  p->tma_ok = 0;
+  if (ny >= 256 && (ny & (ny - 1)) == 0 && nx % 8 == 0) {
+    if (make_spec_map(&p->map_spec, p->spec, nx, (size_t)wb * n_bins * ny) &&
+        make_spec_map(&p->map_spec_sum, p->spec_sum, nx, (size_t)wb * ny))
+      p->tma_ok = 1;
+  }
   return EPR_OK;
 }
 

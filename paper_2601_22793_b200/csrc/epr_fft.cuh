@@ -228,3 +228,95 @@ template <int N, int TPC, int STRIDE, bool INV, bool REV> struct Engine {
 };
 
 }  // namespace eprfft
+
+// =====================================================================================================
+// Swizzled in-place variant for power-of-two column transforms whose tile is staged by TMA.
+// A tile is N rows of W = 4 complex columns (32 bytes per row), exactly as the TMA box lands it: LINEAR layout,
+// element (row, c) at float2 index row·4 + c, no padding (N·32 bytes in all).  After the first pass the data live
+// in the SAME N·32 bytes in a SWIZZLED layout  (row ^ h(row))·4 + c  with
+//     h(row) = ((row>>3 ^ row>>5) & 1) | ((row>>4 & 1) << 1),
+// a bijection that only permutes the 4 rows of a 128-byte group.  A warp is 8 butterflies x 4 columns, and a
+// 64-bit shared access is served per half-warp (4 butterflies x 4 columns = 128 bytes if the 4 rows differ mod 4):
+// with h, the 4 rows are distinct mod 4 for consecutive rows and for rows 8 or 16 apart — every gather / scatter
+// pattern of the (16,16,8 | 8,16,16) schedules — so all passes are bank-conflict free without padding.
+// Addresses: a thread's rows in one pass are rb + off with rb (run time) and off (compile time) on disjoint bits, so
+// (rb + off) ^ h(rb + off) = [rb ^ h(rb)] ^ h(off) + off: ONE base register per pass (xor-ed with a 2-bit
+// constant) plus immediate offsets — no per-access index arithmetic.
+// =====================================================================================================
+namespace eprfft {
+
+__host__ __device__ constexpr int hsw(int row) { return (((row >> 3) ^ (row >> 5)) & 1) | (((row >> 4) & 1) << 1); }
+
+// float2 index of row (rb + OFF), given e0 = ((rb ^ h(rb)) << 2) + c
+template <int OFF> __device__ __forceinline__ int sw_index(int e0) {
+  constexpr int x = (OFF & 3) ^ hsw(OFF);
+  return (e0 ^ (x << 2)) + ((OFF & ~3) << 2);
+}
+__device__ __forceinline__ int sw_base(int rb, int c) { return ((rb ^ hsw(rb)) << 2) + c; }
+
+template <int N, int R, int TPC, int CC, int RR>
+__device__ __forceinline__ void sw_gather_one(float2 (&u)[PassGeom<N, R, TPC>::CNT][R], const float2* s, int e0) {
+  using G = PassGeom<N, R, TPC>;
+  u[CC][RR] = s[sw_index<CC * TPC + RR * G::T>(e0)];
+  if constexpr (RR + 1 < R) sw_gather_one<N, R, TPC, CC, RR + 1>(u, s, e0);
+  else if constexpr (CC + 1 < G::CNT) sw_gather_one<N, R, TPC, CC + 1, 0>(u, s, e0);
+}
+// rows t + cc·TPC + r·T: rb = t
+template <int N, int R, int TPC>
+__device__ __forceinline__ void sw_gather(float2 (&u)[PassGeom<N, R, TPC>::CNT][R], const float2* s, int c, int t) {
+  static_assert(PassGeom<N, R, TPC>::FULL, "power-of-two sizes only");
+  sw_gather_one<N, R, TPC, 0, 0>(u, s, sw_base(t, c));
+}
+template <int N, int P, int R, int TPC, int CC, int Q>
+__device__ __forceinline__ void sw_scatter_q(const float2 (&u)[PassGeom<N, R, TPC>::CNT][R], float2* s, int e0) {
+  s[sw_index<Q * P>(e0)] = u[CC][Q];
+  if constexpr (Q + 1 < R) sw_scatter_q<N, P, R, TPC, CC, Q + 1>(u, s, e0);
+}
+template <int N, int P, int R, int TPC, int CC>
+__device__ __forceinline__ void sw_scatter_cc(const float2 (&u)[PassGeom<N, R, TPC>::CNT][R], float2* s, int c, int t) {
+  using G = PassGeom<N, R, TPC>;
+  const int j = t + CC * TPC;
+  const int k = (P == 1) ? 0 : j % P;
+  const int j0 = (j - k) * R + k;                 // rows j0 + q·P: rb = j0
+  sw_scatter_q<N, P, R, TPC, CC, 0>(u, s, sw_base(j0, c));
+  if constexpr (CC + 1 < G::CNT) sw_scatter_cc<N, P, R, TPC, CC + 1>(u, s, c, t);
+}
+template <int N, int P, int R, int TPC>
+__device__ __forceinline__ void sw_scatter(const float2 (&u)[PassGeom<N, R, TPC>::CNT][R], float2* s, int c, int t) {
+  sw_scatter_cc<N, P, R, TPC, 0>(u, s, c, t);
+}
+
+// Same pass structure as Engine (STRIDE = 4 columns per tile), on the swizzled layout.
+//  run_first: first-pass inputs already in registers (read by the caller from the LINEAR tile, followed by a barrier)
+//  the last pass leaves its outputs in registers (element index of uL[c][q] is (t + c·TPC) + q·PL).
+template <int N, int TPC, bool INV, bool REV> struct EngineSw {
+  using E = Engine<N, TPC, 4, INV, REV>;
+  static constexpr int NP = E::NP, R0 = E::R0, RL = E::RL, PL = E::PL;
+  using G0 = typename E::G0;
+  using GL = typename E::GL;
+  static_assert(NP >= 2, "at least two passes");
+
+  template <int I> __device__ static __forceinline__ void middle(float2* s, int c, int t, const float2* __restrict__ tw) {
+    if constexpr (I < NP - 1) {
+      constexpr int R = sched_radix(N, I, REV), P = sched_P(N, I, REV);
+      float2 u[PassGeom<N, R, TPC>::CNT][R];
+      sw_gather<N, R, TPC>(u, s, c, t);
+      __syncthreads();
+      bfly<N, P, R, TPC, INV>(u, t, tw + tw_offset(N, I, REV));
+      sw_scatter<N, P, R, TPC>(u, s, c, t);
+      __syncthreads();
+      middle<I + 1>(s, c, t, tw);
+    }
+  }
+  __device__ static __forceinline__ void run(float2 (&u0)[G0::CNT][R0], float2 (&uL)[GL::CNT][RL], float2* s, int c, int t,
+                                             const float2* __restrict__ tw) {
+    bfly<N, 1, R0, TPC, INV>(u0, t, tw);
+    sw_scatter<N, 1, R0, TPC>(u0, s, c, t);
+    __syncthreads();
+    middle<1>(s, c, t, tw);
+    sw_gather<N, RL, TPC>(uL, s, c, t);
+    bfly<N, PL, RL, TPC, INV>(uL, t, tw + tw_offset(N, NP - 1, REV));
+  }
+};
+
+}  // namespace eprfft

@@ -346,6 +346,123 @@ k_cols(EprLines L, int M, int mode, float scale, const float* __restrict__ lam_x
   }
 }
 
+// ------------------------------------------------------------------------------------------------ columns, TMA
+// Power-of-two ny ≥ 256, nx % 8 == 0: the 4-column tile (ny rows of 32 bytes) is moved by the TMA unit
+// (cp.async.bulk.tensor.2d, boxes of 256 rows) straight into shared memory and back, so the 32-byte row segments
+// never pass through the LSU, registers or a scoreboard; the transform runs IN PLACE in those ny·32 bytes on the
+// swizzled layout of epr_fft.cuh (no padding, conflict-free), which leaves room for two CTAs per SM.
+template <int N> struct ColTmaCfg {
+  static constexpr int W = 4;
+  static constexpr int TPC = N / 16;
+  static constexpr int NT = TPC * W;
+  static constexpr int BOX = 256;                          // rows per TMA box (hardware limit)
+  static constexpr size_t TILE = (size_t)N * W * sizeof(float2);
+  static constexpr size_t SMEM = TILE + 16;                // + one mbarrier
+};
+
+template <int N, bool SUM>
+__global__ void __launch_bounds__(ColTmaCfg<N>::NT, SUM ? 1 : 2)
+k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_out, EprLines L, int M,
+           int mode, float scale, const float* __restrict__ lam_x, const float* __restrict__ lam_y,
+           const float2* __restrict__ tw, const float2* __restrict__ tw_inv) {
+  using C = ColTmaCfg<N>;
+  using EF = EngineSw<N, C::TPC, false, false>;
+  using EI = EngineSw<N, C::TPC, true, true>;
+  static_assert(EF::RL == EI::R0 && EF::GL::CNT == EI::G0::CNT && EF::PL == EI::G0::T, "schedules must mirror");
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  float2* sm = reinterpret_cast<float2*>(smem_raw);
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + C::TILE);
+  const int c = threadIdx.x % C::W, t = threadIdx.x / C::W;
+  const int kx0 = blockIdx.x * C::W, kx = kx0 + c;
+  const int oplane = blockIdx.y;
+  const int nb = L.n_bins;
+  const int nloop = SUM ? nb : 1;
+  const float lx = __ldg(&lam_x[kx]);
+  if (threadIdx.x == 0) { eprtma::mbar_init(bar, 1); eprtma::mbar_fence_init(); }
+  __syncthreads();
+  float2 acc[EF::GL::CNT][EF::RL];
+  if (SUM) {
+#pragma unroll
+    for (int cc = 0; cc < EF::GL::CNT; ++cc)
+#pragma unroll
+      for (int q = 0; q < EF::RL; ++q) acc[cc][q] = make_float2(0.f, 0.f);
+  }
+  for (int sl = 0; sl < nloop; ++sl) {
+    const int iplane = (mode == 1) ? oplane * nb + sl : oplane;
+    const float a = (mode == 2) ? L.abar : L.a[(mode == 1) ? sl : (oplane % nb)];
+    if (threadIdx.x == 0) {
+      eprtma::fence_proxy_async();
+      eprtma::mbar_expect_tx(bar, (unsigned)C::TILE);
+#pragma unroll
+      for (int bx = 0; bx < N / C::BOX; ++bx)
+        eprtma::tensor_g2s_2d(sm + bx * C::BOX * C::W, &map_in, 2 * kx0, iplane * N + bx * C::BOX, bar);
+    }
+    eprtma::mbar_wait(bar, sl & 1);
+    float2 u0[EF::G0::CNT][EF::R0], uL[EF::GL::CNT][EF::RL];
+#pragma unroll
+    for (int cc = 0; cc < EF::G0::CNT; ++cc)
+#pragma unroll
+      for (int r = 0; r < EF::R0; ++r) u0[cc][r] = sm[(t + cc * C::TPC + r * EF::G0::T) * C::W + c];   // LINEAR tile
+    __syncthreads();                       // every thread has its inputs: the tile may be overwritten in place
+    EF::run(u0, uL, sm, c, t, tw);
+    if (blockIdx.x == 0) {
+      // tile 0 holds the packed column kx = 0: C = F0 + i FM (both Hermitian in ky).  With A = ½(C[ky] + C*[−ky]),
+      // B = −(i/2)(C[ky] − C*[−ky]):  C'[ky] = H(0,ky) A + i H(M,ky) B,  C'[−ky] = H(0,ky) A* + i H(M,ky) B*.
+      __syncthreads();
+#pragma unroll
+      for (int cc = 0; cc < EF::GL::CNT; ++cc)
+#pragma unroll
+        for (int q = 0; q < EF::RL; ++q) sm[(t + cc * C::TPC + q * EF::PL) * C::W + c] = uL[cc][q];
+      __syncthreads();
+      if (c == 0) {
+        const float lxN = __ldg(&lam_x[M]);
+        for (int ky = t; ky <= N / 2; ky += C::TPC) {
+          const int km = (ky == 0) ? 0 : N - ky;
+          const float2 ck = sm[ky * C::W], cm = sm[km * C::W];
+          const float ly = __ldg(&lam_y[ky]);
+          const float h0 = scale / (1.f + a * (lx + ly)), hN = scale / (1.f + a * (lxN + ly));
+          const float2 A = make_float2(0.5f * (ck.x + cm.x), 0.5f * (ck.y - cm.y));
+          const float2 B = make_float2(0.5f * (ck.y + cm.y), -0.5f * (ck.x - cm.x));
+          sm[ky * C::W] = make_float2(h0 * A.x - hN * B.y, h0 * A.y + hN * B.x);
+          if (km != ky) sm[km * C::W] = make_float2(h0 * A.x + hN * B.y, -h0 * A.y + hN * B.x);
+        }
+      }
+      __syncthreads();
+#pragma unroll
+      for (int cc = 0; cc < EF::GL::CNT; ++cc)
+#pragma unroll
+        for (int q = 0; q < EF::RL; ++q) uL[cc][q] = sm[(t + cc * C::TPC + q * EF::PL) * C::W + c];
+    }
+    const float alx = fmaf(a, lx, 1.f);
+#pragma unroll
+    for (int cc = 0; cc < EF::GL::CNT; ++cc) {
+#pragma unroll
+      for (int q = 0; q < EF::RL; ++q) {
+        const float h = (kx == 0) ? 1.f : __fdividef(scale, fmaf(a, __ldg(&lam_y[t + cc * C::TPC + q * EF::PL]), alx));
+        if (SUM) { acc[cc][q].x = fmaf(h, uL[cc][q].x, acc[cc][q].x); acc[cc][q].y = fmaf(h, uL[cc][q].y, acc[cc][q].y); }
+        else { acc[cc][q].x = h * uL[cc][q].x; acc[cc][q].y = h * uL[cc][q].y; }
+      }
+    }
+    __syncthreads();                       // all reads of the tile done before the next load / the inverse writes it
+  }
+  float2 uo[EI::GL::CNT][EI::RL];
+  EI::run(acc, uo, sm, c, t, tw_inv);
+  __syncthreads();                         // last-pass gathers done: the tile is rewritten in LINEAR order for the TMA store
+#pragma unroll
+  for (int cc = 0; cc < EI::GL::CNT; ++cc)
+#pragma unroll
+    for (int q = 0; q < EI::RL; ++q) sm[(t + cc * C::TPC + q * EI::PL) * C::W + c] = uo[cc][q];
+  eprtma::fence_proxy_async();             // generic-proxy writes → visible to the async proxy
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int bx = 0; bx < N / C::BOX; ++bx)
+      eprtma::tensor_s2g_2d(&map_out, 2 * kx0, oplane * N + bx * C::BOX, sm + bx * C::BOX * C::W);
+    eprtma::bulk_commit();
+    eprtma::bulk_wait<0>();                // the CTA's shared memory must outlive the store
+  }
+}
+
 // ------------------------------------------------------------------------------------------------ dispatch
 // The instantiations are split into EPR_FFT_NGROUPS translation units (this file compiled once per group with
 // -DEPR_FFT_GROUP=g, in parallel: see build.py); epr_fftd.cu routes a size to the group that holds it.
@@ -435,6 +552,31 @@ cudaError_t GFN(epr_fftg_rows_c2r_)(const epr_plan_s* p, int planes, const float
   return cudaGetLastError();
 }
 
+template <int N>
+static bool launch_cols_tma(const epr_plan_s* p, int oplanes, int mode, const float2* spec, float2* out, float scale,
+                            cudaStream_t st) {
+  if constexpr (N >= 256 && (N & (N - 1)) == 0) {
+    using C = ColTmaCfg<N>;
+    const int M = p->nx / 2;
+    if (!p->tma_ok || M % C::W != 0 || spec != p->spec || (out != p->spec && out != p->spec_sum)) return false;
+    static bool attr = false;
+    if (!attr) {
+      cudaFuncSetAttribute(k_cols_tma<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+      cudaFuncSetAttribute(k_cols_tma<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+      attr = true;
+    }
+    const CUtensorMap& mo = (out == p->spec) ? p->map_spec : p->map_spec_sum;
+    dim3 grid(M / C::W, oplanes);
+    if (mode == 1 && p->n_bins > 1)
+      k_cols_tma<N, true><<<grid, C::NT, C::SMEM, st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+    else
+      k_cols_tma<N, false><<<grid, C::NT, C::SMEM, st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+    return true;
+  } else {
+    return false;
+  }
+}
+
 cudaError_t GFN(epr_fftg_cols_)(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st) {
   const int M = p->nx / 2;
   const int oplanes = (mode == 1) ? planes / p->n_bins : planes;
@@ -443,6 +585,7 @@ cudaError_t GFN(epr_fftg_cols_)(const epr_plan_s* p, int planes, int mode, const
 #define X(n_)                                                                                                   \
   case n_: {                                                                                                    \
     using C = ColCfg<n_>;                                                                                       \
+    if (launch_cols_tma<n_>(p, oplanes, mode, spec, out, scale, st)) break;                                     \
     static bool attr = false;                                                                                   \
     if (!attr) {                                                                                                \
       cudaFuncSetAttribute(k_cols<n_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);       \

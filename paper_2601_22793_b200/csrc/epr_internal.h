@@ -1,5 +1,6 @@
 // epr_internal.h — plan layout and launcher prototypes shared by the C-ABI and the kernels.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -46,6 +47,9 @@ struct epr_plan_s {
   float* res2;                 // [work_batch][n_bins][ny][nx] r_s (non-local gather output)
   float2* spec;                // [work_batch][n_bins][ny][nx/2] half spectra (packed Nyquist)
   float2* spec_sum;            // [work_batch][ny][nx/2]
+  CUtensorMap map_spec;        // TMA descriptors of spec / spec_sum as [rows][nx floats], box 8 floats x 256 rows
+  CUtensorMap map_spec_sum;
+  int tma_ok;                  // descriptors valid (power-of-two ny ≥ 256, nx % 8 == 0)
   float2* raymap;              // [work_batch][n_bins][ny][nx] stored u_s (lazy, epr_forward non-local)
   int raymap_batch;            // batch of the stored map (0 = none)
   // host staging for epr_retrieve_host

@@ -55,3 +55,19 @@ template <int N> __device__ __forceinline__ void bulk_wait_read() {
 template <int N> __device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
 
 }  // namespace eprtma
+
+// ---- 2-D tiled tensor copies (TMA proper): coordinates are element indices {x (fastest), y} of the tensor map ----
+namespace eprtma {
+__device__ __forceinline__ void tensor_g2s_2d(void* dst_smem, const void* tmap, int x, int y, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+          smem_u32(dst_smem)),
+      "l"(tmap), "r"(x), "r"(y), "r"(smem_u32(bar))
+      : "memory");
+}
+__device__ __forceinline__ void tensor_s2g_2d(const void* tmap, int x, int y, const void* src_smem) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group [%0, {%1, %2}], [%3];" ::"l"(tmap), "r"(x), "r"(y),
+               "r"(smem_u32(src_smem))
+               : "memory");
+}
+}  // namespace eprtma
