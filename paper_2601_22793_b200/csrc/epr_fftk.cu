@@ -357,7 +357,8 @@ template <int N> struct ColTmaCfg {
   static constexpr int NT = TPC * W;
   static constexpr int BOX = 256;                          // rows per TMA box (hardware limit)
   static constexpr size_t TILE = (size_t)N * W * sizeof(float2);
-  static constexpr size_t SMEM = TILE + 16;                // + one mbarrier
+  // SUM (several lines per output tile): two tiles, so that the load of line s+1 overlaps the transform of line s
+  static constexpr size_t smem(bool sum) { return (sum ? 2 : 1) * TILE + 16; }   // + two mbarriers
 };
 
 template <int N, bool SUM>
@@ -370,16 +371,26 @@ k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
   using EI = EngineSw<N, C::TPC, true, true>;
   static_assert(EF::RL == EI::R0 && EF::GL::CNT == EI::G0::CNT && EF::PL == EI::G0::T, "schedules must mirror");
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  float2* sm = reinterpret_cast<float2*>(smem_raw);
-  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + C::TILE);
+  constexpr int NBUF = SUM ? 2 : 1;
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + NBUF * C::TILE);
   const int c = threadIdx.x % C::W, t = threadIdx.x / C::W;
   const int kx0 = blockIdx.x * C::W, kx = kx0 + c;
   const int oplane = blockIdx.y;
   const int nb = L.n_bins;
   const int nloop = SUM ? nb : 1;
   const float lx = __ldg(&lam_x[kx]);
-  if (threadIdx.x == 0) { eprtma::mbar_init(bar, 1); eprtma::mbar_fence_init(); }
+  if (threadIdx.x == 0) { eprtma::mbar_init(&bar[0], 1); eprtma::mbar_init(&bar[1], 1); eprtma::mbar_fence_init(); }
   __syncthreads();
+  auto load_tile = [&](int sl) {            // one thread: request line sl of this output tile into buffer sl % NBUF
+    const int iplane = (mode == 1) ? oplane * nb + sl : oplane;
+    float2* dst = reinterpret_cast<float2*>(smem_raw + (sl % NBUF) * C::TILE);
+    eprtma::fence_proxy_async();
+    eprtma::mbar_expect_tx(&bar[sl % NBUF], (unsigned)C::TILE);
+#pragma unroll
+    for (int bx = 0; bx < N / C::BOX; ++bx)
+      eprtma::tensor_g2s_2d(dst + bx * C::BOX * C::W, &map_in, 2 * kx0, iplane * N + bx * C::BOX, &bar[sl % NBUF]);
+  };
+  if (threadIdx.x == 0) load_tile(0);
   float2 acc[EF::GL::CNT][EF::RL];
   if (SUM) {
 #pragma unroll
@@ -388,16 +399,11 @@ k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
       for (int q = 0; q < EF::RL; ++q) acc[cc][q] = make_float2(0.f, 0.f);
   }
   for (int sl = 0; sl < nloop; ++sl) {
-    const int iplane = (mode == 1) ? oplane * nb + sl : oplane;
     const float a = (mode == 2) ? L.abar : L.a[(mode == 1) ? sl : (oplane % nb)];
-    if (threadIdx.x == 0) {
-      eprtma::fence_proxy_async();
-      eprtma::mbar_expect_tx(bar, (unsigned)C::TILE);
-#pragma unroll
-      for (int bx = 0; bx < N / C::BOX; ++bx)
-        eprtma::tensor_g2s_2d(sm + bx * C::BOX * C::W, &map_in, 2 * kx0, iplane * N + bx * C::BOX, bar);
-    }
-    eprtma::mbar_wait(bar, sl & 1);
+    float2* sm = reinterpret_cast<float2*>(smem_raw + (sl % NBUF) * C::TILE);
+    // the other buffer was last read during line sl − 1, which every thread left through the barrier closing it
+    if (SUM && threadIdx.x == 0 && sl + 1 < nloop) load_tile(sl + 1);
+    eprtma::mbar_wait(&bar[sl % NBUF], (sl / NBUF) & 1);
     float2 u0[EF::G0::CNT][EF::R0], uL[EF::GL::CNT][EF::RL];
 #pragma unroll
     for (int cc = 0; cc < EF::G0::CNT; ++cc)
@@ -445,6 +451,7 @@ k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     }
     __syncthreads();                       // all reads of the tile done before the next load / the inverse writes it
   }
+  float2* sm = reinterpret_cast<float2*>(smem_raw);
   float2 uo[EI::GL::CNT][EI::RL];
   EI::run(acc, uo, sm, c, t, tw_inv);
   __syncthreads();                         // last-pass gathers done: the tile is rewritten in LINEAR order for the TMA store
@@ -561,16 +568,16 @@ static bool launch_cols_tma(const epr_plan_s* p, int oplanes, int mode, const fl
     if (!p->tma_ok || M % C::W != 0 || spec != p->spec || (out != p->spec && out != p->spec_sum)) return false;
     static bool attr = false;
     if (!attr) {
-      cudaFuncSetAttribute(k_cols_tma<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-      cudaFuncSetAttribute(k_cols_tma<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+      cudaFuncSetAttribute(k_cols_tma<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem(false));
+      cudaFuncSetAttribute(k_cols_tma<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem(true));
       attr = true;
     }
     const CUtensorMap& mo = (out == p->spec) ? p->map_spec : p->map_spec_sum;
     dim3 grid(M / C::W, oplanes);
     if (mode == 1 && p->n_bins > 1)
-      k_cols_tma<N, true><<<grid, C::NT, C::SMEM, st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+      k_cols_tma<N, true><<<grid, C::NT, C::smem(true), st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
     else
-      k_cols_tma<N, false><<<grid, C::NT, C::SMEM, st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+      k_cols_tma<N, false><<<grid, C::NT, C::smem(false), st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
     return true;
   } else {
     return false;
