@@ -24,7 +24,7 @@ template <int M> struct RowCfg {                // M = nx/2 complex points per r
   static constexpr size_t SMEM = OFF_WORK + (size_t)ROWS * PL * sizeof(float2);
 };
 
-// Both row kernels are PERSISTENT and TMA-staged: a CTA walks over groups of ROWS consecutive rows (rows of all
+// The C2R row kernel is PERSISTENT and TMA-staged: a CTA walks over groups of ROWS consecutive rows (rows of all
 // planes are contiguous, so one group is one contiguous chunk of HBM); while it transforms group i out of one
 // shared-memory stage, one bulk asynchronous copy (cp.async.bulk, completion on an mbarrier) is already filling
 // the other stage with group i + gridDim.x.  No warp waits on a global load inside the transform.
@@ -43,81 +43,68 @@ struct RowPipe {
   }
 };
 
-// ------------------------------------------------------------------------------------------------ rows R2C
-// stage (TMA) → registers (first pass) → shared-memory passes → registers (last pass) → pair exchange → global
+// ------------------------------------------------------------------------------------------------ rows R2C, direct
+// global → registers (first pass) → shared-memory passes → registers (last pass) → pair exchange → global.
+// One row group per CTA, many CTAs per SM: the forward row transform has no epilogue to hide a load behind and
+// measures faster this way (6.7 vs 7.3 us per 2048² plane) than through the TMA stage, which is kept for C2R.
 template <int M>
-__global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_r2c(int nrows, const float* __restrict__ in, float in_offset,
+__global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_r2c_direct(int ny, const float* __restrict__ in, float in_offset,
                                                             const float2* __restrict__ tw, const float2* __restrict__ tw2,
                                                             float2* __restrict__ spec) {
   using C = RowCfg<M>;
   using EF = Engine<M, C::TPC, 1, false, false>;
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
-  float2* stage = reinterpret_cast<float2*>(smem_raw + C::OFF_STAGE);
-  float2* sm = reinterpret_cast<float2*>(smem_raw + C::OFF_WORK);
-  const int tid = threadIdx.x;
-  const int lr = tid / C::TPC, t = tid - lr * C::TPC;
-  const int ngroups = (nrows + C::ROWS - 1) / C::ROWS;
-  const RowPipe pipe{bar, stage, reinterpret_cast<const float2*>(in), nrows, C::ROWS, M, C::STAGE};
-  if (tid == 0) { eprtma::mbar_init(&bar[0], 1); eprtma::mbar_init(&bar[1], 1); eprtma::mbar_fence_init(); }
-  __syncthreads();
-  if (tid == 0 && (int)blockIdx.x < ngroups) pipe.issue(blockIdx.x, 0);
+  extern __shared__ float2 sm[];           // C::ROWS * C::PL
+  const int lr = threadIdx.x / C::TPC, t = threadIdx.x - lr * C::TPC;
+  const int row = blockIdx.x * C::ROWS + lr;
+  const bool live = row < ny;
+  const size_t rowoff = ((size_t)blockIdx.y * ny + (live ? row : 0)) * (size_t)M;
   float2* s = sm + lr * C::PL;
-  int it = 0;
-  for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x, ++it) {
-    const int buf = it & 1;
-    if (tid == 0 && grp + (int)gridDim.x < ngroups) pipe.issue(grp + gridDim.x, buf ^ 1);
-    eprtma::mbar_wait(&bar[buf], (it >> 1) & 1);
-    const int row = grp * C::ROWS + lr;
-    const bool live = row < nrows;
-    const float2* src = stage + (size_t)buf * C::STAGE + lr * M;
-    float2 u0[EF::G0::CNT][EF::R0], uL[EF::GL::CNT][EF::RL];
+  const float2* src = reinterpret_cast<const float2*>(in) + rowoff;
+  float2 u0[EF::G0::CNT][EF::R0], uL[EF::GL::CNT][EF::RL];
 #pragma unroll
-    for (int c = 0; c < EF::G0::CNT; ++c) {
-      const int j = t + c * C::TPC;
+  for (int c = 0; c < EF::G0::CNT; ++c) {
+    const int j = t + c * C::TPC;
 #pragma unroll
-      for (int r = 0; r < EF::R0; ++r) {
-        float2 v = make_float2(0.f, 0.f);
-        if ((EF::G0::FULL || j < EF::G0::T) && live) v = src[j + r * EF::G0::T];
-        u0[c][r] = make_float2(v.x + in_offset, v.y + in_offset);
-      }
+    for (int r = 0; r < EF::R0; ++r) {
+      float2 v = make_float2(0.f, 0.f);
+      if ((EF::G0::FULL || j < EF::G0::T) && live) v = __ldg(&src[j + r * EF::G0::T]);
+      u0[c][r] = make_float2(v.x + in_offset, v.y + in_offset);
     }
-    EF::run(u0, uL, s, 0, t, tw);
-    __syncthreads();
+  }
+  EF::run(u0, uL, s, 0, t, tw);
+  __syncthreads();
+#pragma unroll
+  for (int c = 0; c < EF::GL::CNT; ++c) {
+    const int j = t + c * C::TPC;
+    if (EF::GL::FULL || j < EF::GL::T) {
+#pragma unroll
+      for (int q = 0; q < EF::RL; ++q) s[padi(j + q * EF::PL)] = uL[c][q];
+    }
+  }
+  __syncthreads();
+  // X[k] = ½(Z[k] + Z*[M−k]) − (i/2) w^k (Z[k] − Z*[M−k]),  w = e^{−2πi/nx};  k = 0: packed (X[0], X[M])
+  if (live) {
+    float2* dst = spec + rowoff;
 #pragma unroll
     for (int c = 0; c < EF::GL::CNT; ++c) {
       const int j = t + c * C::TPC;
       if (EF::GL::FULL || j < EF::GL::T) {
 #pragma unroll
-        for (int q = 0; q < EF::RL; ++q) s[padi(j + q * EF::PL)] = uL[c][q];
-      }
-    }
-    __syncthreads();
-    // X[k] = ½(Z[k] + Z*[M−k]) − (i/2) w^k (Z[k] − Z*[M−k]),  w = e^{−2πi/nx};  k = 0: packed (X[0], X[M])
-    if (live) {
-      float2* dst = spec + (size_t)row * M;
-#pragma unroll
-      for (int c = 0; c < EF::GL::CNT; ++c) {
-        const int j = t + c * C::TPC;
-        if (EF::GL::FULL || j < EF::GL::T) {
-#pragma unroll
-          for (int q = 0; q < EF::RL; ++q) {
-            const int k = j + q * EF::PL;
-            const float2 zk = uL[c][q];
-            if (k == 0) {
-              dst[0] = make_float2(zk.x + zk.y, zk.x - zk.y);
-            } else {
-              const float2 zm = s[padi(M - k)];
-              const float2 wk = __ldg(&tw2[k]);
-              const float2 e = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
-              const float2 o = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));
-              dst[k] = cadd(e, cmul(wk, o));
-            }
+        for (int q = 0; q < EF::RL; ++q) {
+          const int k = j + q * EF::PL;
+          const float2 zk = uL[c][q];
+          if (k == 0) {
+            dst[0] = make_float2(zk.x + zk.y, zk.x - zk.y);
+          } else {
+            const float2 zm = s[padi(M - k)];
+            const float2 wk = __ldg(&tw2[k]);
+            const float2 e = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
+            const float2 o = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));
+            dst[k] = cadd(e, cmul(wk, o));
           }
         }
       }
     }
-    __syncthreads();                       // work buffer and stage[buf] are free for the next group
   }
 }
 
@@ -518,11 +505,14 @@ cudaError_t GFN(epr_fftg_rows_r2c_)(const epr_plan_s* p, int planes, const float
 #define X(n_)                                                                                                   \
   case n_: {                                                                                                    \
     using C = RowCfg<n_ / 2>;                                                                                   \
-    static int full = 0;                                                                                        \
-    if (!full) full = row_grid(k_rows_r2c<n_ / 2>, C::NT, C::SMEM, 1 << 30);                                    \
-    const int ngroups = (nrows + C::ROWS - 1) / C::ROWS;                                                        \
-    k_rows_r2c<n_ / 2><<<ngroups < full ? ngroups : full, C::NT, C::SMEM, st>>>(nrows, in, in_offset, p->tw_row, \
-                                                                                 p->tw_r2c, spec);              \
+    constexpr size_t smem = (size_t)C::ROWS * C::PL * sizeof(float2);                                           \
+    static bool attr = false;                                                                                   \
+    if (!attr) {                                                                                                \
+      cudaFuncSetAttribute(k_rows_r2c_direct<n_ / 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);   \
+      attr = true;                                                                                              \
+    }                                                                                                           \
+    dim3 grid((p->ny + C::ROWS - 1) / C::ROWS, planes);                                                         \
+    k_rows_r2c_direct<n_ / 2><<<grid, C::NT, smem, st>>>(p->ny, in, in_offset, p->tw_row, p->tw_r2c, spec);      \
   } break;
     EPR_FFT_SIZES(X)
 #undef X
