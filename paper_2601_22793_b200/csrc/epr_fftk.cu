@@ -17,29 +17,32 @@ template <int M> struct RowCfg {                // M = nx/2 complex points per r
   static constexpr int ROWS = (TPC >= 128) ? 1 : (128 + TPC - 1) / TPC;   // rows per CTA (≥128 threads)
   static constexpr int NT = TPC * ROWS;
   static constexpr int PL = padded_len(M);
-  static constexpr int STAGE = ROWS * M;        // float2 per staging buffer (ROWS whole rows, contiguous in HBM)
-  // dynamic shared memory: [2 mbarriers | pad to 128 B][stage 0][stage 1][FFT work ROWS x PL]
+  static constexpr int PLA = (PL + 1) & ~1;      // row pitch of a stage: padded length, 16-byte aligned
+  static constexpr int STAGE = ROWS * PLA;      // float2 per stage (ROWS rows; a stage is also the FFT work buffer)
+  // dynamic shared memory: [2 mbarriers | pad to 128 B][stage 0][stage 1]
   static constexpr size_t OFF_STAGE = 128;
-  static constexpr size_t OFF_WORK = OFF_STAGE + 2 * (size_t)STAGE * sizeof(float2);
-  static constexpr size_t SMEM = OFF_WORK + (size_t)ROWS * PL * sizeof(float2);
+  static constexpr size_t SMEM = OFF_STAGE + 2 * (size_t)STAGE * sizeof(float2);
 };
 
 // The C2R row kernel is PERSISTENT and TMA-staged: a CTA walks over groups of ROWS consecutive rows (rows of all
 // planes are contiguous, so one group is one contiguous chunk of HBM); while it transforms group i out of one
 // shared-memory stage, one bulk asynchronous copy (cp.async.bulk, completion on an mbarrier) is already filling
-// the other stage with group i + gridDim.x.  No warp waits on a global load inside the transform.
+// the other stage with group i + gridDim.x.  No warp waits on a global load inside the transform.  A stage row
+// (M points, linear) is read into registers by the first pass and then REUSED in place as the padded work buffer
+// of the remaining passes, so two stages are all the shared memory a CTA needs.
 struct RowPipe {
   uint64_t* bar;
   float2* stage;
   const float2* src;
-  int nrows, rows_per_group, M, stage_elems;
+  int nrows, rows_per_group, M, row_pitch, stage_elems;
   __device__ __forceinline__ void issue(int grp, int buf) const {
     const int r0 = grp * rows_per_group;
     const int nr = min(rows_per_group, nrows - r0);
-    const unsigned bytes = (unsigned)nr * (unsigned)M * (unsigned)sizeof(float2);
+    const unsigned row_bytes = (unsigned)M * (unsigned)sizeof(float2);
     eprtma::fence_proxy_async();
-    eprtma::mbar_expect_tx(&bar[buf], bytes);
-    eprtma::bulk_g2s(stage + (size_t)buf * stage_elems, src + (size_t)r0 * M, bytes, &bar[buf]);
+    eprtma::mbar_expect_tx(&bar[buf], (unsigned)nr * row_bytes);
+    for (int r = 0; r < nr; ++r)
+      eprtma::bulk_g2s(stage + (size_t)buf * stage_elems + (size_t)r * row_pitch, src + (size_t)(r0 + r) * M, row_bytes, &bar[buf]);
   }
 };
 
@@ -111,8 +114,11 @@ __global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_r2c_direct(int ny, const
 // ------------------------------------------------------------------------------------------------ rows C2R
 // EPI 0: out[row][x] = q.   EPI 1 / 2: τ[row][x] += δ(τ, step·q)  (projection increment, R10) for
 // one line (closed form) / several lines (Newton).
+#ifndef C2R_MINB
+#define C2R_MINB 5
+#endif
 template <int M, int EPI>
-__global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_c2r(EprLines L, int nrows, const float2* __restrict__ spec,
+__global__ void __launch_bounds__(RowCfg<M>::NT, (RowCfg<M>::NT <= 128 && EPI != 2) ? C2R_MINB : 1) k_rows_c2r(EprLines L, int nrows, const float2* __restrict__ spec,
                                                             const float2* __restrict__ tw, const float2* __restrict__ tw2,
                                                             float step, int tau_is_zero, int newton_iters,
                                                             float i_min, float* __restrict__ out) {
@@ -121,21 +127,20 @@ __global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_c2r(EprLines L, int nrow
   extern __shared__ __align__(128) unsigned char smem_raw[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
   float2* stage = reinterpret_cast<float2*>(smem_raw + C::OFF_STAGE);
-  float2* sm = reinterpret_cast<float2*>(smem_raw + C::OFF_WORK);
   const int tid = threadIdx.x;
   const int lr = tid / C::TPC, t = tid - lr * C::TPC;
   const int ngroups = (nrows + C::ROWS - 1) / C::ROWS;
-  const RowPipe pipe{bar, stage, spec, nrows, C::ROWS, M, C::STAGE};
+  const RowPipe pipe{bar, stage, spec, nrows, C::ROWS, M, C::PLA, C::STAGE};
   __shared__ float s_f[EPR_MAX_BINS], s_gamma[EPR_MAX_BINS];
   if (EPI == 2 && tid < L.n_bins) { s_f[tid] = L.f[tid]; s_gamma[tid] = L.gamma[tid]; }
   if (tid == 0) { eprtma::mbar_init(&bar[0], 1); eprtma::mbar_init(&bar[1], 1); eprtma::mbar_fence_init(); }
   __syncthreads();
   if (tid == 0 && (int)blockIdx.x < ngroups) pipe.issue(blockIdx.x, 0);
-  float2* s = sm + lr * C::PL;
   int it = 0;
   for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x, ++it) {
     const int buf = it & 1;
     if (tid == 0 && grp + (int)gridDim.x < ngroups) pipe.issue(grp + gridDim.x, buf ^ 1);
+    float2* s = stage + (size_t)buf * C::STAGE + lr * C::PLA;
     const int row = grp * C::ROWS + lr;
     const bool live = row < nrows;
     // the τ values the epilogue will update: requested now, consumed after the transform
@@ -151,7 +156,7 @@ __global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_c2r(EprLines L, int nrow
       }
     }
     eprtma::mbar_wait(&bar[buf], (it >> 1) & 1);
-    const float2* src = stage + (size_t)buf * C::STAGE + lr * M;
+    const float2* src = s;
     float2 u0[EI::G0::CNT][EI::R0], uL[EI::GL::CNT][EI::RL];
     // Z2[k] = (X[k] + X*[M−k]) + i w^{−k} (X[k] − X*[M−k]);  Z2[0] = (x0 + xM) + i (x0 − xM)
 #pragma unroll
@@ -176,6 +181,7 @@ __global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_c2r(EprLines L, int nrow
         u0[c][r] = z;
       }
     }
+    __syncthreads();                       // every input is in registers: the stage row becomes the work buffer
     EI::run(u0, uL, s, 0, t, tw);
     if (live) {
 #pragma unroll
