@@ -174,7 +174,8 @@ __global__ void __launch_bounds__(256) k_forward_local(EprLines L, int nx, int n
 // Rolling rows (suffix a = m−1, b = m, c = m+1 = newest row n); output row o = m − 1 is final after stage 2 of m.
 // ≈ 62 fp32 instructions per pixel: bound by fp32 issue, not by HBM (12 B/px) — DESIGN.md §7.
 // -----------------------------------------------------------------------------------------------------
-#define LM_MR 32                     // output rows per warp
+// LM_MR output rows per warp and LM_WPC warps (bands) per CTA are template parameters: (128, 1) when the launch has
+// enough bands x row blocks x projections to fill the GPU (row halo 4/128, 12.4 us per 2048² plane), (32, 4) otherwise.
 #define LM_BW 120                    // output columns per warp
 #ifndef LM_D
 #define LM_D 4                       // cp.async ring depth: rows are requested LM_D − 1 steps ahead
@@ -204,11 +205,12 @@ __device__ __forceinline__ W6 window(const F4& v) {
   return r;
 }
 
-__global__ void __launch_bounds__(128) k_local_march(EprLines L, int nx, int ny, int order, int wkb1,
+template <int LM_MR, int LM_WPC>
+__global__ void __launch_bounds__(32 * LM_WPC) k_local_march(EprLines L, int nx, int ny, int order, int wkb1,
                                                      const float* __restrict__ tau, const float* __restrict__ d,
                                                      float* __restrict__ out) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int band = blockIdx.x * 4 + warp;
+  const int band = blockIdx.x * LM_WPC + warp;
   const int xs = band * LM_BW - 4 + 4 * lane;
   if (band * LM_BW >= nx) return;
   const int y0 = blockIdx.y * LM_MR;
@@ -228,7 +230,7 @@ __global__ void __launch_bounds__(128) k_local_march(EprLines L, int nx, int ny,
     t_a.v[k] = t_b.v[k] = t_c.v[k] = A_b.v[k] = dA_lo.v[k] = J_a.v[k] = J_b.v[k] = 0.f;
     H_a.v[k] = 0.5f; Q_a.v[k] = ACC_a.v[k] = ACC_b.v[k] = 0.f;
   }
-  __shared__ float4 ring_t[LM_D][128], ring_d[LM_D][128];
+  __shared__ float4 ring_t[LM_D][32 * LM_WPC], ring_d[LM_D][32 * LM_WPC];
   const unsigned tid = threadIdx.x;
   // row pointers advance by one row per request (τ rows wrap periodically, d / out rows never leave the plane)
   int yr = wrapm(y0 - 2, ny);
@@ -359,8 +361,15 @@ cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float
                                      cudaStream_t st) {
   if (d_fuse) {
     const int bands = (p->nx + LM_BW - 1) / LM_BW;
-    dim3 grid((bands + 3) / 4, (p->ny + LM_MR - 1) / LM_MR, batch);
-    k_local_march<<<grid, 128, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, d_fuse, out);
+    static int sms = 0;
+    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+    if ((long long)bands * ((p->ny + 127) / 128) * batch >= 16ll * sms) {          // ≥ 16 one-warp CTAs per SM
+      dim3 grid(bands, (p->ny + 127) / 128, batch);
+      k_local_march<128, 1><<<grid, 32, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, d_fuse, out);
+    } else {
+      dim3 grid((bands + 3) / 4, (p->ny + 31) / 32, batch);
+      k_local_march<32, 4><<<grid, 128, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, d_fuse, out);
+    }
     return cudaGetLastError();
   }
   dim3 grid((p->nx + FL_TX - 1) / FL_TX, (p->ny + FL_TY - 1) / FL_TY, batch);
