@@ -395,28 +395,22 @@ cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float
 // =====================================================================================================
 #define ST_W 128
 #define ST_H 64
+#define ST_AP (ST_W + 8)              // accumulator pitch: 4 columns of (aligned) border left, 1 used right
+#define ST_AROWS (ST_H + 2)           // one border row above and below: out-of-tile corners land there, unflushed
 #ifndef ST_NT
 #define ST_NT 512                     // threads per CTA
 #endif
 
 // FROM_TAU: sources and ray map from the τ tile staged in shared memory (the loop's configuration);
 // otherwise (epr_transport) both are read from global planes.
-// predicated shared-memory reduction (no branch, no convergence barrier around the atomic)
-__device__ __forceinline__ void red_shared_if(bool p, unsigned* addr, unsigned v) {
-  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %2, 0;\n\t@q red.shared.add.u32 [%0], %1;\n\t}" ::"r"(
-                   (unsigned)__cvta_generic_to_shared(addr)),
-               "r"(v), "r"((unsigned)p)
-               : "memory");
-}
-
 template <bool FROM_TAU, bool MAP_OUT>
 __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny, float S, int H,
                                                     const float* __restrict__ tau, const float* __restrict__ I_bins,
                                                     const float2* __restrict__ map_in, float2* __restrict__ map_out,
                                                     float* __restrict__ out, int out_mode, const float* __restrict__ d) {
   extern __shared__ __align__(16) unsigned char st_raw[];
-  unsigned* s_acc = reinterpret_cast<unsigned*>(st_raw);                              // [ST_H][ST_W]
-  float* s_tau = reinterpret_cast<float*>(st_raw + ST_W * ST_H * sizeof(unsigned));   // [RH + 2][TP]
+  unsigned* s_acc = reinterpret_cast<unsigned*>(st_raw);                              // [ST_AROWS][ST_AP]
+  float* s_tau = reinterpret_cast<float*>(st_raw + ST_AP * ST_AROWS * sizeof(unsigned));   // [RH + 2][TP]
   const int b = blockIdx.z, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   constexpr int NW = ST_NT / 32;
   const int x0 = blockIdx.x * ST_W, y0 = blockIdx.y * ST_H;
@@ -451,7 +445,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
   for (int s = 0; s < L.n_bins; ++s) {
     const size_t pl = ((size_t)b * L.n_bins + s) * plane;
     __syncthreads();                                   // previous bin flushed
-    for (int i = tid; i < ST_W * ST_H / 4; i += ST_NT) reinterpret_cast<uint4*>(s_acc)[i] = make_uint4(0u, 0u, 0u, 0u);
+    for (int i = tid; i < ST_AP * ST_AROWS / 4; i += ST_NT) reinterpret_cast<uint4*>(s_acc)[i] = make_uint4(0u, 0u, 0u, 0u);
     if (FROM_TAU && s == 0) {
       cp_async_wait<0>();
       __syncthreads();
@@ -503,19 +497,24 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       if ((unsigned)(ax + 1) > ST_W || (unsigned)(ay + 1) > ST_H) continue;      // cannot touch this tile
       const float dx = ux - (float)fx, dy = uy - (float)fy;
       int tot;                                         // signed: epr_transport accepts planes of either sign
-      if (FROM_TAU) tot = Fi + __float2int_rn(fixFf * epr_expm1(-gam * tc));
-      else tot = __float2int_rn(__ldg(&I_bins[pl + gidx]) * 67108864.f);
+      if (FROM_TAU) {
+        const float xe = -gam * tc;                    // both expm1 branches only where a lane of the warp needs them
+        const float J = epr_expm1(xe);
+        tot = Fi + __float2int_rn(fixFf * J);
+      } else {
+        tot = __float2int_rn(__ldg(&I_bins[pl + gidx]) * 67108864.f);
+      }
       // corner masses in fp32 (± 2 units of 2^-26), the 4th corner takes the exact remainder
       const float totf = (float)tot, ex = 1.f - dx, ey = 1.f - dy;
       const int c00 = __float2int_rn(totf * ex * ey), c10 = __float2int_rn(totf * dx * ey),
                 c01 = __float2int_rn(totf * ex * dy);
       const int c11 = tot - c00 - c10 - c01;
-      const bool xin0 = ax >= 0, xin1 = ax + 1 < ST_W, yin0 = ay >= 0, yin1 = ay + 1 < ST_H;
-      unsigned* a0 = s_acc + ay * ST_W + ax;
-      red_shared_if(yin0 && xin0, a0, (unsigned)c00);
-      red_shared_if(yin0 && xin1, a0 + 1, (unsigned)c10);
-      red_shared_if(yin1 && xin0, a0 + ST_W, (unsigned)c01);
-      red_shared_if(yin1 && xin1, a0 + ST_W + 1, (unsigned)c11);
+      // ax ∈ [−1, ST_W − 1], ay ∈ [−1, ST_H − 1]: all four corners are inside the bordered accumulator
+      unsigned* a0 = s_acc + (ay + 1) * ST_AP + (ax + 4);
+      atomicAdd(a0, (unsigned)c00);
+      atomicAdd(a0 + 1, (unsigned)c10);
+      atomicAdd(a0 + ST_AP, (unsigned)c01);
+      atomicAdd(a0 + ST_AP + 1, (unsigned)c11);
     }
     __syncthreads();
     // flush the tile: 4 pixels per thread per pass
@@ -524,7 +523,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       const int ty = i / (ST_W / 4), tx = 4 * (i - ty * (ST_W / 4));
       const int gx = x0 + tx, gy = y0 + ty;
       if (gx >= nx || gy >= ny) continue;
-      const uint4 v = reinterpret_cast<const uint4*>(s_acc)[i];
+      const uint4 v = *reinterpret_cast<const uint4*>(s_acc + (ty + 1) * ST_AP + 4 + tx);
       const unsigned g = (unsigned)gy * nx + gx;
       float4 o;
       if (out_mode == 1) {
@@ -548,7 +547,7 @@ static cudaError_t launch_splat_t(const epr_plan_s* p, int batch, const float* t
                                   float2* map_out, float* out, int out_mode, const float* d, cudaStream_t st) {
   const int H = (int)ceilf(p->opt.max_shift_px) + 1;
   const int Ha = (H + 1 + 3) & ~3;
-  const size_t smem = (size_t)ST_W * ST_H * sizeof(unsigned) +
+  const size_t smem = (size_t)ST_AP * ST_AROWS * sizeof(unsigned) +
                       (FROM_TAU ? (size_t)(ST_W + 2 * Ha) * (ST_H + 2 * H + 2) * sizeof(float) : 0);
   static size_t attr = 0;
   if (smem > attr) {
