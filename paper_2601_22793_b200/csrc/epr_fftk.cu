@@ -208,7 +208,8 @@ __global__ void __launch_bounds__(RowCfg<M>::NT, (RowCfg<M>::NT <= 128 && EPI !=
         }
       }
     }
-    __syncthreads();                       // work buffer and stage[buf] are free for the next group
+    eprtma::fence_proxy_async();           // this thread's generic writes of the stage are ordered before the TMA refill
+    __syncthreads();                       // stage[buf] is free for the group after next
   }
 }
 
@@ -442,6 +443,7 @@ k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
         else { acc[cc][q].x = h * uL[cc][q].x; acc[cc][q].y = h * uL[cc][q].y; }
       }
     }
+    if (SUM) eprtma::fence_proxy_async();  // generic writes of this tile are ordered before its TMA refill (line sl + 2)
     __syncthreads();                       // all reads of the tile done before the next load / the inverse writes it
   }
   float2* sm = reinterpret_cast<float2*>(smem_raw);
