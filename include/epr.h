@@ -92,7 +92,10 @@ epr_status epr_precondition(epr_plan_t plan, int batch, const float* r_bins, flo
 /* epr_retrieve — the correction loop
  *   d   [batch][ny][nx] in;  out [batch][ny][nx] out (τ, or what opt.output selects; τ⁰ in if opt.init = 1).
  *   iterations ≥ 0 correction iterations after the initial Paganin solve (0 returns the L¹/Paganin result,
- *   PAPER.md:124); step > 0 relaxation factor. */
+ *   PAPER.md:124); step > 0 relaxation factor.
+ *   Launch-bound calls (batch · n_bins · nx · ny ≤ 2^20) on a non-default stream are captured into a CUDA graph on
+ *   their second occurrence and replayed while (d, out, batch, iterations, step) stay the same; the buffers' CONTENTS
+ *   may change between calls.  Environment EPR_GRAPH = 0 disables this, 2 applies it to every size. */
 epr_status epr_retrieve(epr_plan_t plan, int batch, const float* d, float* out, int iterations, float step,
                         void* stream);
 

@@ -156,6 +156,8 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
   *out = p;                                   // returned even on failure so that the caller can read the message
   p->nx = nx; p->ny = ny; p->n_bins = n_bins; p->max_batch = max_batch; p->solver = (int)solver; p->opt = o;
   p->opt.mu_rel = NULL;
+  p->graph_mode = 1;
+  { const char* g = getenv("EPR_GRAPH"); if (g) p->graph_mode = atoi(g); }
 
   // per-line scalars: k_s = 2πE/(hc); α_s = L/(k_s p²) (Eq. (2)); a_s = α_s db_s/2 (Eq. (6));
   // γ_s ∝ 1/(E_s db_s) normalised to Σ f γ = 1 (R11)
@@ -285,6 +287,7 @@ extern "C" epr_status epr_destroy(epr_plan_t p) {
   cudaFree(p->tw_row); cudaFree(p->tw_r2c); cudaFree(p->tw_col); cudaFree(p->tw_col_inv); cudaFree(p->lam_x); cudaFree(p->lam_y);
   cudaFree(p->tau); cudaFree(p->pred); cudaFree(p->res); cudaFree(p->res2); cudaFree(p->spec); cudaFree(p->spec_sum);
   cudaFree(p->raymap);
+  if (p->graph_exec) cudaGraphExecDestroy(p->graph_exec);
   if (p->prof) { epr_profile_read(p, 0, NULL, NULL, NULL, 1); delete (EprProf*)p->prof; }
   for (int i = 0; i < 2; ++i) { cudaFree(p->stage_in[i]); cudaFree(p->stage_out[i]); }
   for (int i = 0; i < 3; ++i) if (p->hstream[i]) cudaStreamDestroy(p->hstream[i]);
@@ -433,7 +436,39 @@ extern "C" epr_status epr_retrieve(epr_plan_t p, int batch, const float* d, floa
   if (st != EPR_OK) return st;
   if (!d || !out) FAIL(p, EPR_EINVAL, "epr_retrieve: NULL pointer");
   if (iterations < 0 || !(step > 0.f)) FAIL(p, EPR_EINVAL, "epr_retrieve: iterations must be >= 0 and step > 0");
-  return retrieve_device(p, batch, d, out, iterations, step, (cudaStream_t)stream);
+  cudaStream_t cs = (cudaStream_t)stream;
+  // Launch-bound sizes (a few hundred thousand pixels per launch: the kernels last microseconds): the whole loop is
+  // captured once into a CUDA graph and replayed while the call's arguments stay the same.  Never under profiling
+  // (events are recorded around every launch) and never on the legacy default stream (capture is illegal there).
+  const size_t work = (size_t)batch * p->n_bins * p->nx * p->ny;
+  const bool use_graph = !p->prof_on && cs != 0 && (p->graph_mode == 2 || (p->graph_mode == 1 && work <= ((size_t)1 << 20)));
+  if (!use_graph) return retrieve_device(p, batch, d, out, iterations, step, cs);
+  if (p->graph_exec && p->graph_d == d && p->graph_out == out && p->graph_batch == batch && p->graph_iters == iterations &&
+      p->graph_step == step) {
+    CU(p, cudaGraphLaunch(p->graph_exec, cs));
+    p->launches += p->graph_launches;
+    return EPR_OK;
+  }
+  if (p->graph_exec) { cudaGraphExecDestroy(p->graph_exec); p->graph_exec = NULL; }
+  // one eager pass first: launchers set function attributes / query occupancy on their first call
+  if (!p->graph_warm) {
+    p->graph_warm = 1;
+    return retrieve_device(p, batch, d, out, iterations, step, cs);
+  }
+  const long long l0 = p->launches;
+  CU(p, cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal));
+  st = retrieve_device(p, batch, d, out, iterations, step, cs);
+  cudaGraph_t graph = NULL;
+  cudaError_t ce = cudaStreamEndCapture(cs, &graph);
+  if (st != EPR_OK) { if (graph) cudaGraphDestroy(graph); return st; }
+  if (ce != cudaSuccess || !graph) FAIL(p, EPR_ECUDA, "graph capture: %s", cudaGetErrorString(ce));
+  ce = cudaGraphInstantiate(&p->graph_exec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (ce != cudaSuccess) { p->graph_exec = NULL; FAIL(p, EPR_ECUDA, "graph instantiate: %s", cudaGetErrorString(ce)); }
+  p->graph_d = d; p->graph_out = out; p->graph_batch = batch; p->graph_iters = iterations; p->graph_step = step;
+  p->graph_launches = p->launches - l0;
+  CU(p, cudaGraphLaunch(p->graph_exec, cs));
+  return EPR_OK;
 }
 
 extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_host, float* out_host, int iterations,

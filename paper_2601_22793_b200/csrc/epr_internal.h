@@ -58,6 +58,15 @@ struct epr_plan_s {
   int stage_chunk;             // projections the staging buffers hold
   cudaStream_t hstream[3];     // copy-in, compute, copy-out
   cudaEvent_t hev[6];          // per buffer: in-done, compute-done, out-done
+  // CUDA graph of the last epr_retrieve (same buffers, batch, iterations, step): replayed instead of re-enqueued
+  cudaGraphExec_t graph_exec;
+  const float* graph_d;
+  float* graph_out;
+  int graph_batch, graph_iters;
+  float graph_step;
+  long long graph_launches;    // kernel launches inside the graph
+  int graph_warm;              // an eager pass has run (function attributes are set)
+  int graph_mode;              // 0 off, 1 on for launch-bound sizes (default), 2 always (EPR_GRAPH)
   long long launches;
   int prof_on;                 // per-kernel event timing enabled
   void* prof;                  // EprProf*

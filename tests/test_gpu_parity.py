@@ -222,6 +222,43 @@ def test_full_size_periodic_tiling(E, name):
     assert np.array_equal(got[0], got[1])                      # batch entries are independent and deterministic
 
 
+def test_retrieve_graph_replay_matches_eager(E):
+    """On a non-default stream a launch-bound retrieval is captured into a CUDA graph (second call) and replayed
+    (third call, with NEW data in the same buffers): all three must equal the eager result bit for bit."""
+    import torch
+    w = make_workload("C1")
+    w2 = make_workload("C3", n=256)
+    for wk in (w, w2):
+        plan = E.epr_plan(wk.nx, wk.ny, wk.pixel_m, wk.L_m, wk.energy_keV, wk.weight, wk.delta_over_beta, wk.solver,
+                          max_batch=1, max_shift_px=wk.max_shift_px)
+        d = _dev(wk.d[:1])
+        ref = torch.empty_like(d)
+        E.epr_retrieve(plan, d, ref, wk.iterations, wk.step)            # default stream: eager
+        d_alt = _dev(np.roll(wk.d[:1], 5, axis=2))
+        ref_alt = torch.empty_like(d)
+        E.epr_retrieve(plan, d_alt, ref_alt, wk.iterations, wk.step)
+        torch.cuda.synchronize()
+        side = torch.cuda.Stream()
+        out = torch.empty_like(d)
+        buf = d.clone()
+        l0 = plan.launches
+        with torch.cuda.stream(side):
+            E.epr_retrieve(plan, buf, out, wk.iterations, wk.step)      # eager warm pass
+            side.synchronize()
+            per_call = plan.launches - l0
+            assert torch.equal(out, ref)
+            out.zero_()
+            E.epr_retrieve(plan, buf, out, wk.iterations, wk.step)      # capture + launch
+            side.synchronize()
+            assert torch.equal(out, ref)
+            buf.copy_(d_alt)
+            E.epr_retrieve(plan, buf, out, wk.iterations, wk.step)      # replay on new contents
+            side.synchronize()
+            assert torch.equal(out, ref_alt)
+        assert plan.launches - l0 == 3 * per_call
+        plan.destroy()
+
+
 def test_retrieve_zero_iterations_is_paganin(E):
     w = make_workload("C1")
     got, refs = _run_retrieve(E, w, iterations=0)
