@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_r2c_direct(int ny, const
 #define C2R_MINB 5
 #endif
 template <int M, int EPI>
-__global__ void __launch_bounds__(RowCfg<M>::NT, (RowCfg<M>::NT <= 128 && EPI != 2) ? C2R_MINB : 1) k_rows_c2r(EprLines L, int nrows, const float2* __restrict__ spec,
+__global__ void __launch_bounds__(RowCfg<M>::NT, (RowCfg<M>::NT <= 128) ? C2R_MINB : (RowCfg<M>::NT <= 192) ? 3 : 1) k_rows_c2r(EprLines L, int nrows, const float2* __restrict__ spec,
                                                             const float2* __restrict__ tw, const float2* __restrict__ tw2,
                                                             float step, int tau_is_zero, int newton_iters,
                                                             float i_min, float* __restrict__ out) {
@@ -152,7 +152,7 @@ __global__ void __launch_bounds__(RowCfg<M>::NT, (RowCfg<M>::NT <= 128 && EPI !=
 #pragma unroll
       for (int q = 0; q < EI::RL; ++q) {
         tpre[c][q] = make_float2(0.f, 0.f);
-        if (EPI != 0 && !tau_is_zero && live && (EI::GL::FULL || j < EI::GL::T)) tpre[c][q] = dst[j + q * EI::PL];
+        if (EPI == 1 && !tau_is_zero && live && (EI::GL::FULL || j < EI::GL::T)) tpre[c][q] = dst[j + q * EI::PL];
       }
     }
     eprtma::mbar_wait(&bar[buf], (it >> 1) & 1);
@@ -183,7 +183,33 @@ __global__ void __launch_bounds__(RowCfg<M>::NT, (RowCfg<M>::NT <= 128 && EPI !=
     }
     __syncthreads();                       // every input is in registers: the stage row becomes the work buffer
     EI::run(u0, uL, s, 0, t, tw);
-    if (live) {
+    if (EPI == 2) {
+      // Several lines: the projection costs hundreds of instructions per pixel.  The row goes back to shared memory in
+      // natural order and is updated in a rolled loop (2 pixels per thread per pass, τ of the next pass in flight), so
+      // that neither the FFT's register arrays nor 32 unrolled copies of the solver are alive in the epilogue.
+      __syncthreads();                     // last-pass gathers of the row are done
+#pragma unroll
+      for (int c = 0; c < EI::GL::CNT; ++c) {
+        const int j = t + c * C::TPC;
+        if (EI::GL::FULL || j < EI::GL::T) {
+#pragma unroll
+          for (int q = 0; q < EI::RL; ++q) s[j + q * EI::PL] = uL[c][q];
+        }
+      }
+      __syncthreads();
+      if (live) {
+        float2 tnext = tau_is_zero ? make_float2(0.f, 0.f) : dst[t];
+#pragma unroll 1
+        for (int i = t; i < M; i += C::TPC) {
+          float2 tau = tnext;
+          if (i + C::TPC < M && !tau_is_zero) tnext = dst[i + C::TPC];
+          const float2 v = s[i];
+          tau.x += epr_project_increment(tau.x, step * v.x, s_f, s_gamma, L.n_bins, L.gamma_max, newton_iters, i_min);
+          tau.y += epr_project_increment(tau.y, step * v.y, s_f, s_gamma, L.n_bins, L.gamma_max, newton_iters, i_min);
+          dst[i] = tau;
+        }
+      }
+    } else if (live) {
 #pragma unroll
       for (int c = 0; c < EI::GL::CNT; ++c) {
         const int j = t + c * C::TPC;
@@ -196,11 +222,6 @@ __global__ void __launch_bounds__(RowCfg<M>::NT, (RowCfg<M>::NT <= 128 && EPI !=
               float2 tau = tpre[c][q];
               tau.x += epr_project_increment_mono(tau.x, step * v.x, i_min);
               tau.y += epr_project_increment_mono(tau.y, step * v.y, i_min);
-              v = tau;
-            } else if (EPI == 2) {
-              float2 tau = tpre[c][q];
-              tau.x += epr_project_increment(tau.x, step * v.x, s_f, s_gamma, L.n_bins, L.gamma_max, newton_iters, i_min);
-              tau.y += epr_project_increment(tau.y, step * v.y, s_f, s_gamma, L.n_bins, L.gamma_max, newton_iters, i_min);
               v = tau;
             }
             dst[idx] = v;
