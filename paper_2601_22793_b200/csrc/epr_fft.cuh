@@ -10,9 +10,11 @@
 
 namespace eprfft {
 
+// Greedy radix choice.  The composite odd / semi-odd radices 15, 10, 9, 6 (nested 3x5, 2x5, 3x3, 2x3 butterflies in
+// registers) keep the mixed sizes at three passes: 2160 = 16·15·9, 2560 = 16·16·10, 1080 = 8·15·9.
 __host__ __device__ constexpr int pick_radix(int rem) {
-  return (rem % 16 == 0) ? 16 : (rem % 8 == 0) ? 8 : (rem % 4 == 0) ? 4 : (rem % 2 == 0) ? 2
-       : (rem % 5 == 0) ? 5 : (rem % 3 == 0) ? 3 : 0;
+  return (rem % 16 == 0) ? 16 : (rem % 8 == 0) ? 8 : (rem % 4 == 0) ? 4 : (rem % 15 == 0) ? 15 : (rem % 10 == 0) ? 10
+       : (rem % 9 == 0) ? 9 : (rem % 6 == 0) ? 6 : (rem % 2 == 0) ? 2 : (rem % 5 == 0) ? 5 : (rem % 3 == 0) ? 3 : 0;
 }
 __host__ __device__ constexpr bool supported(int n) {
   while (n > 1) { int r = pick_radix(n); if (!r) return false; n /= r; }
@@ -95,12 +97,96 @@ template <bool INV> __device__ __forceinline__ void dft16(float2* v) {
 #pragma unroll
     for (int j = i + 1; j < 4; ++j) { float2 t = v[4 * i + j]; v[4 * i + j] = v[4 * j + i]; v[4 * j + i] = t; }
 }
+// e^{∓iθ} from (cos θ, sin θ): forward sign −, inverse +
+template <bool INV> __device__ __forceinline__ float2 wconst(float c, float sn) { return make_float2(c, INV ? sn : -sn); }
+
+// Composite radix N1·N2 by Cooley-Tukey in registers: n = N2 n1 + n2, k = k1 + N1 k2,
+//   X[k1 + N1 k2] = Σ_{n2} w_{N2}^{n2 k2} · w_N^{n2 k1} · ( Σ_{n1} x[N2 n1 + n2] w_{N1}^{n1 k1} ).
+template <bool INV> __device__ __forceinline__ void dft6(float2* v) {          // 2 x 3
+  float2 y[6];
+#pragma unroll
+  for (int n2 = 0; n2 < 3; ++n2) { float2 a[2] = {v[n2], v[3 + n2]}; dft2<INV>(a); y[n2] = a[0]; y[3 + n2] = a[1]; }
+  y[3 + 1] = cmul(y[3 + 1], wconst<INV>(0.5f, 0.86602540378443864676f));
+  y[3 + 2] = cmul(y[3 + 2], wconst<INV>(-0.5f, 0.86602540378443864676f));
+#pragma unroll
+  for (int k1 = 0; k1 < 2; ++k1) {
+    float2 a[3] = {y[3 * k1], y[3 * k1 + 1], y[3 * k1 + 2]};
+    dft3<INV>(a);
+#pragma unroll
+    for (int k2 = 0; k2 < 3; ++k2) v[k1 + 2 * k2] = a[k2];
+  }
+}
+template <bool INV> __device__ __forceinline__ void dft9(float2* v) {          // 3 x 3
+  float2 y[9];
+#pragma unroll
+  for (int n2 = 0; n2 < 3; ++n2) {
+    float2 a[3] = {v[n2], v[3 + n2], v[6 + n2]};
+    dft3<INV>(a);
+    y[n2] = a[0]; y[3 + n2] = a[1]; y[6 + n2] = a[2];
+  }
+  y[3 + 1] = cmul(y[3 + 1], wconst<INV>(0.76604444311897803520f, 0.64278760968653932632f));    // w9^1
+  y[3 + 2] = cmul(y[3 + 2], wconst<INV>(0.17364817766693034885f, 0.98480775301220805937f));    // w9^2
+  y[6 + 1] = cmul(y[6 + 1], wconst<INV>(0.17364817766693034885f, 0.98480775301220805937f));    // w9^2
+  y[6 + 2] = cmul(y[6 + 2], wconst<INV>(-0.93969262078590838405f, 0.34202014332566873304f));   // w9^4
+#pragma unroll
+  for (int k1 = 0; k1 < 3; ++k1) {
+    float2 a[3] = {y[3 * k1], y[3 * k1 + 1], y[3 * k1 + 2]};
+    dft3<INV>(a);
+#pragma unroll
+    for (int k2 = 0; k2 < 3; ++k2) v[k1 + 3 * k2] = a[k2];
+  }
+}
+template <bool INV> __device__ __forceinline__ void dft10(float2* v) {         // 2 x 5
+  float2 y[10];
+#pragma unroll
+  for (int n2 = 0; n2 < 5; ++n2) { float2 a[2] = {v[n2], v[5 + n2]}; dft2<INV>(a); y[n2] = a[0]; y[5 + n2] = a[1]; }
+  y[5 + 1] = cmul(y[5 + 1], wconst<INV>(0.80901699437494742410f, 0.58778525229247312917f));    // w10^1
+  y[5 + 2] = cmul(y[5 + 2], wconst<INV>(0.30901699437494742410f, 0.95105651629515357212f));    // w10^2
+  y[5 + 3] = cmul(y[5 + 3], wconst<INV>(-0.30901699437494742410f, 0.95105651629515357212f));   // w10^3
+  y[5 + 4] = cmul(y[5 + 4], wconst<INV>(-0.80901699437494742410f, 0.58778525229247312917f));   // w10^4
+#pragma unroll
+  for (int k1 = 0; k1 < 2; ++k1) {
+    float2 a[5] = {y[5 * k1], y[5 * k1 + 1], y[5 * k1 + 2], y[5 * k1 + 3], y[5 * k1 + 4]};
+    dft5<INV>(a);
+#pragma unroll
+    for (int k2 = 0; k2 < 5; ++k2) v[k1 + 2 * k2] = a[k2];
+  }
+}
+template <bool INV> __device__ __forceinline__ void dft15(float2* v) {         // 3 x 5
+  float2 y[15];
+#pragma unroll
+  for (int n2 = 0; n2 < 5; ++n2) {
+    float2 a[3] = {v[n2], v[5 + n2], v[10 + n2]};
+    dft3<INV>(a);
+    y[n2] = a[0]; y[5 + n2] = a[1]; y[10 + n2] = a[2];
+  }
+  // w15^{n2 k1}: k1 = 1 → exponents 1..4; k1 = 2 → 2, 4, 6, 8
+  y[5 + 1] = cmul(y[5 + 1], wconst<INV>(0.91354545764260089550f, 0.40673664307580020775f));
+  y[5 + 2] = cmul(y[5 + 2], wconst<INV>(0.66913060635885821383f, 0.74314482547739423501f));
+  y[5 + 3] = cmul(y[5 + 3], wconst<INV>(0.30901699437494742410f, 0.95105651629515357212f));
+  y[5 + 4] = cmul(y[5 + 4], wconst<INV>(-0.10452846326765347140f, 0.99452189536827333692f));
+  y[10 + 1] = cmul(y[10 + 1], wconst<INV>(0.66913060635885821383f, 0.74314482547739423501f));
+  y[10 + 2] = cmul(y[10 + 2], wconst<INV>(-0.10452846326765347140f, 0.99452189536827333692f));
+  y[10 + 3] = cmul(y[10 + 3], wconst<INV>(-0.80901699437494742410f, 0.58778525229247312917f));
+  y[10 + 4] = cmul(y[10 + 4], wconst<INV>(-0.97814760073380563793f, -0.20791169081775933710f));
+#pragma unroll
+  for (int k1 = 0; k1 < 3; ++k1) {
+    float2 a[5] = {y[5 * k1], y[5 * k1 + 1], y[5 * k1 + 2], y[5 * k1 + 3], y[5 * k1 + 4]};
+    dft5<INV>(a);
+#pragma unroll
+    for (int k2 = 0; k2 < 5; ++k2) v[k1 + 3 * k2] = a[k2];
+  }
+}
 template <int R, bool INV> __device__ __forceinline__ void dft(float2* v) {
   if constexpr (R == 2) dft2<INV>(v);
   else if constexpr (R == 3) dft3<INV>(v);
   else if constexpr (R == 4) dft4<INV>(v[0], v[1], v[2], v[3]);
   else if constexpr (R == 5) dft5<INV>(v);
+  else if constexpr (R == 6) dft6<INV>(v);
   else if constexpr (R == 8) dft8<INV>(v);
+  else if constexpr (R == 9) dft9<INV>(v);
+  else if constexpr (R == 10) dft10<INV>(v);
+  else if constexpr (R == 15) dft15<INV>(v);
   else dft16<INV>(v);
 }
 
@@ -130,6 +216,15 @@ __host__ __device__ constexpr int tw_offset(int n, int i, bool rev) {
   return off;
 }
 __host__ __device__ constexpr int tw_total(int n, bool rev) { return tw_offset(n, num_passes(n), rev); }
+
+// Threads cooperating on one transform: 16 points each, but never fewer than the butterflies of a radix-15 pass
+// (N/15 > N/16 would otherwise cost a whole second, almost empty, round of 15-point butterflies).
+__host__ __device__ constexpr int threads_per_transform(int n) {
+  int t = (n + 15) / 16;
+  for (int i = 0; i < num_passes(n); ++i)
+    if (fwd_radix(n, i) == 15 && n / 15 > t) t = n / 15;
+  return t;
+}
 
 template <int N, int R, int TPC> struct PassGeom {
   static constexpr int T = N / R;                       // butterflies per transform

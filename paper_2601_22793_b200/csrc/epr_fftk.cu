@@ -13,7 +13,7 @@
 using namespace eprfft;
 
 template <int M> struct RowCfg {                // M = nx/2 complex points per row
-  static constexpr int TPC = (M + 15) / 16;     // threads per row
+  static constexpr int TPC = threads_per_transform(M);   // threads per row
   static constexpr int ROWS = (TPC >= 128) ? 1 : (128 + TPC - 1) / TPC;   // rows per CTA (≥128 threads)
   static constexpr int NT = TPC * ROWS;
   static constexpr int PL = padded_len(M);
@@ -237,7 +237,7 @@ __global__ void __launch_bounds__(RowCfg<M>::NT, (RowCfg<M>::NT <= 128) ? C2R_MI
 // ------------------------------------------------------------------------------------------------ columns
 template <int N> struct ColCfg {
   static constexpr int W = 4;                    // columns per CTA (32 B per row segment)
-  static constexpr int TPC = (N + 15) / 16;      // threads per column
+  static constexpr int TPC = threads_per_transform(N);    // threads per column
   static constexpr int NT = TPC * W;
   static constexpr int PL = padded_len(N);
   static constexpr size_t SMEM = (size_t)PL * W * sizeof(float2);

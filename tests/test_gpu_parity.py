@@ -50,7 +50,9 @@ SPECTRA = {
     "poly3_unequal_a": (np.array([70.0, 100.0, 130.0]), np.array([0.3, 0.4, 0.3]), np.array([900.0, 1000.0, 1100.0])),
 }
 # (ny, nx): powers of two and radix-3/5 lengths; ny = 256 … 2048 with nx % 8 == 0 take the TMA-staged column kernel
-SIZES = [(256, 256), (48, 80), (160, 96), (320, 512), (512, 128), (1024, 64), (2048, 32)]
+# 2160 = 16·15·9, 2560 = 16·16·10, 1080 = 8·15·9 exercise the composite radices
+SIZES = [(256, 256), (48, 80), (160, 96), (320, 512), (512, 128), (1024, 64), (2048, 32), (2160, 32), (32, 2160),
+         (2560, 16), (16, 2560)]
 
 
 @pytest.mark.parametrize("ny,nx", SIZES)
