@@ -397,13 +397,11 @@ cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float
 #define ST_H 64
 #define ST_AP (ST_W + 8)              // accumulator pitch: 4 columns of (aligned) border left, 1 used right
 #define ST_AROWS (ST_H + 2)           // one border row above and below: out-of-tile corners land there, unflushed
-#ifndef ST_NT
-#define ST_NT 512                     // threads per CTA
-#endif
 
 // FROM_TAU: sources and ray map from the τ tile staged in shared memory (the loop's configuration);
 // otherwise (epr_transport) both are read from global planes.
-template <bool FROM_TAU, bool MAP_OUT>
+// ST_NT threads per CTA: 512 when two CTAs fit an SM, 1024 when the halo (large S) leaves room for one only
+template <bool FROM_TAU, bool MAP_OUT, int ST_NT>
 __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny, float S, int H,
                                                     const float* __restrict__ tau, const float* __restrict__ I_bins,
                                                     const float2* __restrict__ map_in, float2* __restrict__ map_out,
@@ -549,14 +547,20 @@ static cudaError_t launch_splat_t(const epr_plan_s* p, int batch, const float* t
   const int Ha = (H + 1 + 3) & ~3;
   const size_t smem = (size_t)ST_AP * ST_AROWS * sizeof(unsigned) +
                       (FROM_TAU ? (size_t)(ST_W + 2 * Ha) * (ST_H + 2 * H + 2) * sizeof(float) : 0);
-  static size_t attr = 0;
-  if (smem > attr) {
-    cudaFuncSetAttribute(k_splat_tile<FROM_TAU, MAP_OUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr = smem;
+  static size_t attr[2] = {0, 0};
+  const int big = smem > 113 * 1024 ? 1 : 0;            // more than half of the 227 KB an SM offers
+  if (smem > attr[big]) {
+    if (big) cudaFuncSetAttribute(k_splat_tile<FROM_TAU, MAP_OUT, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    else cudaFuncSetAttribute(k_splat_tile<FROM_TAU, MAP_OUT, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attr[big] = smem;
   }
   dim3 grid((p->nx + ST_W - 1) / ST_W, (p->ny + ST_H - 1) / ST_H, batch);
-  k_splat_tile<FROM_TAU, MAP_OUT><<<grid, ST_NT, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, H, tau, I_bins,
-                                                           map_in, map_out, out, out_mode, d);
+  if (big)
+    k_splat_tile<FROM_TAU, MAP_OUT, 1024><<<grid, 1024, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, H, tau, I_bins,
+                                                                    map_in, map_out, out, out_mode, d);
+  else
+    k_splat_tile<FROM_TAU, MAP_OUT, 512><<<grid, 512, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, H, tau, I_bins,
+                                                                  map_in, map_out, out, out_mode, d);
   return cudaGetLastError();
 }
 
