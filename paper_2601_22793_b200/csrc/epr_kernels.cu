@@ -363,9 +363,14 @@ cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float
     const int bands = (p->nx + LM_BW - 1) / LM_BW;
     static int sms = 0;
     if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
-    if ((long long)bands * ((p->ny + 127) / 128) * batch >= 16ll * sms) {          // ≥ 16 one-warp CTAs per SM
+    // the tallest row block that still gives every SM about a dozen warps (all CTAs resident at once: no tail wave)
+    const long long need = 12ll * sms;
+    if ((long long)bands * ((p->ny + 127) / 128) * batch >= need) {
       dim3 grid(bands, (p->ny + 127) / 128, batch);
       k_local_march<128, 1><<<grid, 32, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, d_fuse, out);
+    } else if ((long long)bands * ((p->ny + 63) / 64) * batch >= need) {
+      dim3 grid((bands + 1) / 2, (p->ny + 63) / 64, batch);
+      k_local_march<64, 2><<<grid, 64, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, d_fuse, out);
     } else {
       dim3 grid((bands + 3) / 4, (p->ny + 31) / 32, batch);
       k_local_march<32, 4><<<grid, 128, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, d_fuse, out);
