@@ -320,11 +320,11 @@ extern "C" epr_status epr_forward(epr_plan_t p, int batch, const float* tau, flo
   const size_t plane = (size_t)p->nx * p->ny;
   if (p->solver == EPR_LOCAL) {
     KL(p, K_FWD_LOCAL, cs, epr_launch_forward_local(p, batch, tau, NULL, p->pred, cs));
-    KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, 0, 0, P_sum, P_bins, cs));
+    KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, P_sum, P_bins, cs));
   } else {
     if ((st = ensure_raymap(p)) != EPR_OK) return st;
     KL(p, K_SPLAT, cs, epr_launch_splat(p, batch, tau, NULL, NULL, p->raymap, p->pred, 0, NULL, cs));
-    KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, 0, 0, P_sum, P_bins, cs));
+    KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, P_sum, P_bins, cs));
     p->raymap_batch = batch;
   }
   return EPR_OK;
@@ -395,7 +395,7 @@ static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* ta
         KL(p, K_FWD_LOCAL, cs, epr_launch_forward_local(p, nb, tau, d, p->res, cs));             // a0 + a1-L + a2 fused
       } else {
         KL(p, K_FWD_LOCAL, cs, epr_launch_forward_local(p, nb, tau, NULL, p->pred, cs));         // a0 + a1-L
-        KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, 0, p->res, cs));           // a2 (a3 = identity)
+        KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, p->res, cs));           // a2 (a3 = identity)
       }
       r = p->res;
     } else {
@@ -403,7 +403,7 @@ static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* ta
         KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->res, 2, d, cs));       // a0 + a1-N + a2 fused
       } else {
         KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->pred, 0, NULL, cs));   // a0 + a1-N
-        KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, 0, p->res, cs));           // a2
+        KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, p->res, cs));           // a2
       }
       KL(p, K_GATHER, cs, epr_launch_gather(p, nb, tau, NULL, p->res, p->res2, cs));          // a3
       r = p->res2;

@@ -42,7 +42,7 @@ struct epr_plan_s {
   float* lam_y;                // λ_y[ky], ky < ny
   // workspaces (sized for max_batch)
   float* tau;                  // [work_batch][ny][nx]        state τ (when `out` is not τ) / scratch
-  float* pred;                 // [work_batch][n_bins][ny][nx] float: P_s − f_s (local) ; u32 fixed point (non-local)
+  float* pred;                 // [work_batch][n_bins][ny][nx] P_s − f_s
   float* res;                  // [work_batch][n_bins][ny][nx] e_s then r_s
   float* res2;                 // [work_batch][n_bins][ny][nx] r_s (non-local gather output)
   float2* spec;                // [work_batch][n_bins][ny][nx/2] half spectra (packed Nyquist)
@@ -81,10 +81,10 @@ cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float
 // out_mode 0: out[b][s] = P_s − f_s;  1: out[b][s] = P_s (linear transport);  2 (one line): out[b] = e = (d−1) − (P−f)
 cudaError_t epr_launch_splat(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
                              float2* map_out, float* out, int out_mode, const float* d, cudaStream_t st);
-cudaError_t epr_launch_residual(const epr_plan_s* p, int batch, const float* d, const void* pred, int fixed,
-                                float* es, cudaStream_t st);
-cudaError_t epr_launch_pred_out(const epr_plan_s* p, int batch, const void* pred, int fixed, int linear, float* P_sum,
-                                float* P_bins, cudaStream_t st);
+cudaError_t epr_launch_residual(const epr_plan_s* p, int batch, const float* d, const float* pred, float* es,
+                                cudaStream_t st);
+cudaError_t epr_launch_pred_out(const epr_plan_s* p, int batch, const float* pred, float* P_sum, float* P_bins,
+                                cudaStream_t st);
 cudaError_t epr_launch_gather(const epr_plan_s* p, int batch, const float* tau, const float2* map_in, const float* es,
                               float* r, cudaStream_t st);
 cudaError_t epr_launch_rows_r2c(const epr_plan_s* p, int planes, const float* in, float in_offset, float2* spec,
@@ -96,4 +96,3 @@ cudaError_t epr_launch_cols(const epr_plan_s* p, int planes, int mode, const flo
 cudaError_t epr_launch_rows_c2r(const epr_plan_s* p, int planes, const float2* spec, int epilogue, float step,
                                 int tau_is_zero, float* q_or_tau, cudaStream_t st);
 cudaError_t epr_launch_output(const epr_plan_s* p, int batch, const float* tau, float* out, cudaStream_t st);
-cudaError_t epr_launch_zero(void* ptr, size_t bytes, cudaStream_t st);

@@ -579,37 +579,18 @@ cudaError_t epr_launch_splat(const epr_plan_s* p, int batch, const float* tau, c
 // =====================================================================================================
 // a2  detector residual and positivity-weighted split (reading R8), deviation form:
 //   e = (d − 1) − Σ_s (P_s − f_s);   w_s = P_s⁺ / Σ_t P_t⁺ (fallback f_s);   es_s = w_s e
-//   pred is either float P_s − f_s (local) or the u32 fixed-point splat plane (non-local).
+//   pred holds P_s − f_s (float), written by k_forward_local or k_splat_tile.
 // =====================================================================================================
-__device__ __forceinline__ float pred_dev(const void* pred, size_t idx, int fixed, const EprLines& L, int s) {
-  if (fixed) {
-    const unsigned v = __ldg(&((const unsigned*)pred)[idx]);
-    return (float)(int)(v - L.fixFi[s]) * (1.0f / (float)EPR_FIX_ONE) + L.fixCorr[s];
-  }
-  return __ldg(&((const float*)pred)[idx]);
-}
-
-__device__ __forceinline__ float4 pred_dev4(const void* pred, size_t idx, int fixed, const EprLines& L, int s) {
-  if (fixed) {
-    const uint4 v = __ldg(reinterpret_cast<const uint4*>((const unsigned*)pred + idx));
-    const float sc = 1.0f / (float)EPR_FIX_ONE, c = L.fixCorr[s];
-    const unsigned F = L.fixFi[s];
-    return make_float4(fmaf((float)(int)(v.x - F), sc, c), fmaf((float)(int)(v.y - F), sc, c),
-                       fmaf((float)(int)(v.z - F), sc, c), fmaf((float)(int)(v.w - F), sc, c));
-  }
-  return __ldg(reinterpret_cast<const float4*>((const float*)pred + idx));
-}
-
 // one thread = 4 consecutive pixels (plane % 4 == 0)
 __global__ void __launch_bounds__(256) k_residual(EprLines L, unsigned plane, const float* __restrict__ d,
-                                                  const void* __restrict__ pred, int fixed, float* __restrict__ es) {
+                                                  const float* __restrict__ pred, float* __restrict__ es) {
   const unsigned i = (blockIdx.x * 256u + threadIdx.x) * 4u;
   const int b = blockIdx.y;
   if (i >= plane) return;
   const size_t base = (size_t)b * L.n_bins * plane + i;
   float4 sum = make_float4(0.f, 0.f, 0.f, 0.f), den = sum;
   for (int s = 0; s < L.n_bins; ++s) {
-    const float4 pd = pred_dev4(pred, base + (size_t)s * plane, fixed, L, s);
+    const float4 pd = __ldg(reinterpret_cast<const float4*>(pred + base + (size_t)s * plane));
     const float f = L.f[s];
     sum.x += pd.x; sum.y += pd.y; sum.z += pd.z; sum.w += pd.w;
     den.x += fmaxf(f + pd.x, 0.f); den.y += fmaxf(f + pd.y, 0.f); den.z += fmaxf(f + pd.z, 0.f); den.w += fmaxf(f + pd.w, 0.f);
@@ -621,7 +602,7 @@ __global__ void __launch_bounds__(256) k_residual(EprLines L, unsigned plane, co
   const float4 q = make_float4(den.x > 0.f ? e.x / den.x : 0.f, den.y > 0.f ? e.y / den.y : 0.f,
                                den.z > 0.f ? e.z / den.z : 0.f, den.w > 0.f ? e.w / den.w : 0.f);
   for (int s = 0; s < L.n_bins; ++s) {
-    const float4 pd = pred_dev4(pred, base + (size_t)s * plane, fixed, L, s);
+    const float4 pd = __ldg(reinterpret_cast<const float4*>(pred + base + (size_t)s * plane));
     const float f = L.f[s];
     float4 o;
     o.x = den.x > 0.f ? fmaxf(f + pd.x, 0.f) * q.x : f * e.x;
@@ -632,37 +613,35 @@ __global__ void __launch_bounds__(256) k_residual(EprLines L, unsigned plane, co
   }
 }
 
-cudaError_t epr_launch_residual(const epr_plan_s* p, int batch, const float* d, const void* pred, int fixed,
-                                float* es, cudaStream_t st) {
+cudaError_t epr_launch_residual(const epr_plan_s* p, int batch, const float* d, const float* pred, float* es,
+                                cudaStream_t st) {
   const unsigned plane = (unsigned)p->nx * p->ny;
   dim3 grid((plane / 4 + 255) / 256, batch);
-  k_residual<<<grid, 256, 0, st>>>(p->lines, plane, d, pred, fixed, es);
+  k_residual<<<grid, 256, 0, st>>>(p->lines, plane, d, pred, es);
   return cudaGetLastError();
 }
 
-// epr_forward / epr_transport output: P_s = f_s + (P_s − f_s) (linear = 1: plain fixed-point value), P = Σ_s P_s.
-__global__ void __launch_bounds__(256) k_pred_out(EprLines L, size_t plane, const void* __restrict__ pred, int fixed,
-                                                  int linear, float* __restrict__ P_sum, float* __restrict__ P_bins) {
+// epr_forward output: P_s = f_s + (P_s − f_s), P = Σ_s P_s.
+__global__ void __launch_bounds__(256) k_pred_out(EprLines L, size_t plane, const float* __restrict__ pred,
+                                                  float* __restrict__ P_sum, float* __restrict__ P_bins) {
   const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
   const int b = blockIdx.y;
   if (i >= plane) return;
   const size_t base = (size_t)b * L.n_bins * plane + i;
   float sum = 0.f;
   for (int s = 0; s < L.n_bins; ++s) {
-    float v;
-    if (linear) v = (float)(int)__ldg(&((const unsigned*)pred)[base + s * plane]) * (1.0f / (float)EPR_FIX_ONE);
-    else v = L.f[s] + pred_dev(pred, base + s * plane, fixed, L, s);
+    const float v = L.f[s] + __ldg(&pred[base + s * plane]);
     sum += v;
     if (P_bins) P_bins[base + s * plane] = v;
   }
   if (P_sum) P_sum[(size_t)b * plane + i] = sum;
 }
 
-cudaError_t epr_launch_pred_out(const epr_plan_s* p, int batch, const void* pred, int fixed, int linear, float* P_sum,
-                                float* P_bins, cudaStream_t st) {
+cudaError_t epr_launch_pred_out(const epr_plan_s* p, int batch, const float* pred, float* P_sum, float* P_bins,
+                                cudaStream_t st) {
   const size_t plane = (size_t)p->nx * p->ny;
   dim3 grid((unsigned)((plane + 255) / 256), batch);
-  k_pred_out<<<grid, 256, 0, st>>>(p->lines, plane, pred, fixed, linear, P_sum, P_bins);
+  k_pred_out<<<grid, 256, 0, st>>>(p->lines, plane, pred, P_sum, P_bins);
   return cudaGetLastError();
 }
 
@@ -755,5 +734,3 @@ cudaError_t epr_launch_output(const epr_plan_s* p, int batch, const float* tau, 
   k_output<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p->lines, n, p->opt.output, coef, tau, out);
   return cudaGetLastError();
 }
-
-cudaError_t epr_launch_zero(void* ptr, size_t bytes, cudaStream_t st) { return cudaMemsetAsync(ptr, 0, bytes, st); }
