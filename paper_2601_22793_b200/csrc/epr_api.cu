@@ -500,14 +500,27 @@ extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_
     for (int i = 0; i < 6; ++i) CU(p, cudaEventCreateWithFlags(&p->hev[i], cudaEventDisableTiming));
   }
   cudaStream_t s_in = p->hstream[0], s_cmp = p->hstream[1], s_out = p->hstream[2];
-  int chunk = 0;
-  for (int b0 = 0; b0 < batch; b0 += wbch, ++chunk) {
-    const int nb = (batch - b0 < wbch) ? batch - b0 : wbch;
+  // Tapered schedule: the first copy in and the last copy out cannot overlap any compute, so the first and the last
+  // chunks are small (wbch/4, wbch/2, wbch, …, wbch, wbch/2, wbch/4) when the batch holds at least three full chunks.
+  const bool taper = wbch >= 4 && batch >= 3 * wbch;
+  const int head[2] = {wbch / 4, wbch / 2};
+  int chunk = 0, nb = 0;
+  for (int b0 = 0; b0 < batch; b0 += nb, ++chunk) {
+    const int left = batch - b0;
+    nb = wbch;
+    if (taper) {
+      if (chunk < 2) nb = head[chunk];
+      else if (left <= wbch / 4) nb = left;
+      else if (left <= wbch / 4 + wbch / 2) nb = left - wbch / 4;
+      else if (left < wbch + wbch / 4 + wbch / 2) nb = left - (wbch / 4 + wbch / 2);
+    }
+    if (nb > left) nb = left;
     const int buf = chunk & 1;
     cudaEvent_t ev_in = p->hev[buf * 3 + 0], ev_cmp = p->hev[buf * 3 + 1], ev_out = p->hev[buf * 3 + 2];
     const size_t bytes = (size_t)nb * plane * sizeof(float);
     if (chunk >= 2) {                       // buffers of chunk-2 must be free: its compute read stage_in, its D2H read stage_out
       CU(p, cudaStreamWaitEvent(s_in, ev_cmp, 0));
+      if (p->opt.init == 1) CU(p, cudaStreamWaitEvent(s_in, ev_out, 0));
       CU(p, cudaStreamWaitEvent(s_cmp, ev_out, 0));
     }
     CU(p, cudaMemcpyAsync(p->stage_in[buf], d_host + (size_t)b0 * plane, bytes, cudaMemcpyHostToDevice, s_in));
