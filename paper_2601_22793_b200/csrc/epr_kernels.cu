@@ -193,6 +193,16 @@ __device__ __forceinline__ float shfl_r(float x) { return __shfl_down_sync(0xfff
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
 }
+// shared-memory access by 32-bit shared address (volatile: program order among themselves is kept, so a kernel can
+// place the loads of the next step before the atomics of the current one)
+__device__ __forceinline__ float lds_f32(unsigned a) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ void red_shared_u32(unsigned a, unsigned v) {
+  asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
@@ -474,11 +484,63 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
     const int RWe = ST_W + 2 * He, RHe = ST_H + 2 * He;
     // Every periodic image of a source pixel inside the region is a distinct candidate: its targets differ by whole
     // periods, and exactly one image puts a given corner on a given detector pixel — that IS the periodic wrap (R7).
-    // the CTA's 256 threads walk the region in row-major order, 256 sources per pass: (sx, sy) advance incrementally
-    const int adv_y = ST_NT / RWe, adv_x = ST_NT - adv_y * RWe;
-    int sy = tid / RWe, sx = tid - sy * RWe;
-    for (; sy < RHe; sx += adv_x, sy += adv_y) {
-      if (sx >= RWe) { sx -= RWe; ++sy; if (sy >= RHe) break; }
+    if (FROM_TAU) {
+      // (1) The tile's own ST_W x ST_H sources (nearly all of them hit): a warp owns a 32-column strip and marches
+      // down its rows with the column's τ values in registers (3 shared loads per source instead of 5, no index
+      // arithmetic: one address per array advances by a row); the loads of row r + 1 are issued before the atomics
+      // of row r.  32-bit shared addresses are formed once (the compiler otherwise rebuilds them per source).
+      constexpr int RG = NW / 4, ROWS = ST_H / RG;
+      const int x = (warp & 3) * 32 + lane, yb = (warp >> 2) * ROWS;
+      const unsigned TP4 = 4u * TP;
+      unsigned rb = (unsigned)__cvta_generic_to_shared(s_tau) + 4u * (unsigned)((yb + H + 1) * TP + x + Ha);
+      unsigned ab = (unsigned)__cvta_generic_to_shared(s_acc) + 4u * (unsigned)((yb + 1) * ST_AP + x + 4);
+      float tn = lds_f32(rb - TP4), tc = lds_f32(rb), ts = lds_f32(rb + TP4), tl = lds_f32(rb - 4), tr = lds_f32(rb + 4);
+      float2* mo = MAP_OUT ? map_out + pl + (size_t)(y0 + yb) * nx + (x0 + x) : nullptr;
+#pragma unroll 2
+      for (int r = 0; r < ROWS; ++r) {
+        rb += TP4;                                     // one row beyond the strip at the last r: still inside the τ tile
+        const float ts2 = lds_f32(rb + TP4), tl2 = lds_f32(rb - 4), tr2 = lds_f32(rb + 4);
+        const float ux = fminf(fmaxf(cs * (tr - tl), -S), S), uy = fminf(fmaxf(cs * (ts - tn), -S), S);
+        if (MAP_OUT) {
+          if (x0 + x < nx && y0 + yb + r < ny) *mo = make_float2(ux, uy);
+          mo += nx;
+        }
+        const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
+        const float dx = ux - (float)fx, dy = uy - (float)fy;
+        const float xe = -gam * tc;
+        float J = epr_expm1_small(xe);                 // MUFU branch only where a lane of the warp needs it
+        if (__any_sync(0xffffffffu, fabsf(xe) >= 0.35f)) J = fabsf(xe) < 0.35f ? J : __expf(xe) - 1.f;
+        const int tot = Fi + __float2int_rn(fixFf * J);
+        const float totf = (float)tot, te = totf * (1.f - dy), td = totf * dy, ex = 1.f - dx;
+        const int c00 = __float2int_rn(te * ex), c10 = __float2int_rn(te * dx), c01 = __float2int_rn(td * ex);
+        const int c11 = tot - c00 - c10 - c01;
+        // ax = x + fx ∈ [−1, ST_W − 1], ay ∈ [−1, ST_H − 1]: all four corners are inside the bordered accumulator
+        if ((unsigned)(x + fx + 1) <= ST_W && (unsigned)(yb + r + fy + 1) <= ST_H) {
+          const unsigned a0 = ab + 4u * (unsigned)(fy * ST_AP + fx);
+          red_shared_u32(a0, (unsigned)c00);
+          red_shared_u32(a0 + 4, (unsigned)c10);
+          red_shared_u32(a0 + 4 * ST_AP, (unsigned)c01);
+          red_shared_u32(a0 + 4 * ST_AP + 4, (unsigned)c11);
+        }
+        tn = tc; tc = ts; ts = ts2; tl = tl2; tr = tr2;
+        ab += 4u * ST_AP;
+      }
+    }
+    // (2) FROM_TAU: the ring of width He around the tile (two bands of He rows, two of He columns), few of whose
+    // sources reach the tile; otherwise (epr_transport): the whole region, row-major.
+    const int n_tb = 2 * He * RWe, n_walk = FROM_TAU ? n_tb + 2 * ST_H * He : RWe * RHe;
+    const float inv_rw = 1.f / (float)RWe, inv_2he = 1.f / (float)(2 * He);
+    for (int i = tid; i < n_walk; i += ST_NT) {
+      int sx, sy;                                      // quotients by float reciprocal: exact for these ranges
+      if (!FROM_TAU || i < n_tb) {
+        sy = (int)(((float)i + 0.5f) * inv_rw); sx = i - sy * RWe;
+        if (FROM_TAU && sy >= He) sy += ST_H;
+      } else {
+        const int j = i - n_tb;
+        sy = (int)(((float)j + 0.5f) * inv_2he); sx = j - sy * 2 * He;
+        sy += He;
+        if (sx >= He) sx += ST_W;
+      }
       const int tx0 = sx - He, ty0 = sy - He;          // source pixel relative to the tile
       float ux, uy, tc = 0.f;
       unsigned gidx = 0;
