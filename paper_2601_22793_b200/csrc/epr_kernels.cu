@@ -1,4 +1,5 @@
 // epr_kernels.cu — stencil, splat, gather and pointwise kernels of the EPR iteration (sm_100a).
+#include <type_traits>
 #include "epr_internal.h"
 #include "epr_math.cuh"
 
@@ -453,8 +454,8 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
   }
   // Largest |D⁰τ| (times 2) among the sources OUTSIDE the tile: bounds how far away a source can be and still
   // reach the tile, so that the walk below covers the tile grown by He ≤ H only.
-  __shared__ unsigned s_maxd;
-  if (tid == 0) s_maxd = 0u;
+  __shared__ unsigned s_maxd, s_maxd_in;
+  if (tid == 0) { s_maxd = 0u; s_maxd_in = 0u; }
   for (int s = 0; s < L.n_bins; ++s) {
     const size_t pl = ((size_t)b * L.n_bins + s) * plane;
     __syncthreads();                                   // previous bin flushed
@@ -463,12 +464,17 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       cp_async_wait<0>();
       __syncthreads();
       float md = 0.f;
+      // ring of width H around the tile only: whole rows above and below, two H-column segments beside it
       for (int sy = warp; sy < RH; sy += NW) {
-        const bool yin = sy >= H && sy < H + ST_H;
         const float* trow = s_tau + (sy + 1) * TP + (Ha - H);
-        for (int sx = lane; sx < RW; sx += 32) {
-          if (yin && sx >= H && sx < H + ST_W) continue;                          // the tile itself is always walked
-          md = fmaxf(md, fmaxf(fabsf(trow[sx + 1] - trow[sx - 1]), fabsf(trow[sx + TP] - trow[sx - TP])));
+        if (sy < H || sy >= H + ST_H) {
+          for (int sx = lane; sx < RW; sx += 32)
+            md = fmaxf(md, fmaxf(fabsf(trow[sx + 1] - trow[sx - 1]), fabsf(trow[sx + TP] - trow[sx - TP])));
+        } else {
+          for (int l = lane; l < 2 * H; l += 32) {
+            const int sx = l < H ? l : l + ST_W;
+            md = fmaxf(md, fmaxf(fabsf(trow[sx + 1] - trow[sx - 1]), fabsf(trow[sx + TP] - trow[sx - TP])));
+          }
         }
       }
 #pragma unroll
@@ -489,42 +495,62 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       // down its rows with the column's τ values in registers (3 shared loads per source instead of 5, no index
       // arithmetic: one address per array advances by a row); the loads of row r + 1 are issued before the atomics
       // of row r.  32-bit shared addresses are formed once (the compiler otherwise rebuilds them per source).
+      // Line 0 also records the largest |D⁰τ| of the tile itself; the later lines then skip the clamp of u when
+      // |c_s| · max|D⁰τ| over the whole region cannot exceed S.
       constexpr int RG = NW / 4, ROWS = ST_H / RG;
       const int x = (warp & 3) * 32 + lane, yb = (warp >> 2) * ROWS;
       const unsigned TP4 = 4u * TP;
-      unsigned rb = (unsigned)__cvta_generic_to_shared(s_tau) + 4u * (unsigned)((yb + H + 1) * TP + x + Ha);
-      unsigned ab = (unsigned)__cvta_generic_to_shared(s_acc) + 4u * (unsigned)((yb + 1) * ST_AP + x + 4);
-      float tn = lds_f32(rb - TP4), tc = lds_f32(rb), ts = lds_f32(rb + TP4), tl = lds_f32(rb - 4), tr = lds_f32(rb + 4);
-      float2* mo = MAP_OUT ? map_out + pl + (size_t)(y0 + yb) * nx + (x0 + x) : nullptr;
+      const unsigned rb0 = (unsigned)__cvta_generic_to_shared(s_tau) + 4u * (unsigned)((yb + H + 1) * TP + x + Ha);
+      const unsigned ab0 = (unsigned)__cvta_generic_to_shared(s_acc) + 4u * (unsigned)((yb + 1) * ST_AP + x + 4);
+      auto interior = [&](auto clamp_tag) {
+        constexpr bool CLAMP = decltype(clamp_tag)::value;      // CLAMP is also "line 0": track the tile's max|D⁰τ|
+        unsigned rb = rb0, ab = ab0;
+        float tn = lds_f32(rb - TP4), tc = lds_f32(rb), ts = lds_f32(rb + TP4), tl = lds_f32(rb - 4), tr = lds_f32(rb + 4);
+        float2* mo = MAP_OUT ? map_out + pl + (size_t)(y0 + yb) * nx + (x0 + x) : nullptr;
+        float md_in = 0.f;
 #pragma unroll 2
-      for (int r = 0; r < ROWS; ++r) {
-        rb += TP4;                                     // one row beyond the strip at the last r: still inside the τ tile
-        const float ts2 = lds_f32(rb + TP4), tl2 = lds_f32(rb - 4), tr2 = lds_f32(rb + 4);
-        const float ux = fminf(fmaxf(cs * (tr - tl), -S), S), uy = fminf(fmaxf(cs * (ts - tn), -S), S);
-        if (MAP_OUT) {
-          if (x0 + x < nx && y0 + yb + r < ny) *mo = make_float2(ux, uy);
-          mo += nx;
+        for (int r = 0; r < ROWS; ++r) {
+          rb += TP4;                                   // one row beyond the strip at the last r: still inside the τ tile
+          const float ts2 = lds_f32(rb + TP4), tl2 = lds_f32(rb - 4), tr2 = lds_f32(rb + 4);
+          const float gx = tr - tl, gy = ts - tn;
+          float ux = cs * gx, uy = cs * gy;
+          if (CLAMP) {
+            md_in = fmaxf(md_in, fmaxf(fabsf(gx), fabsf(gy)));
+            ux = fminf(fmaxf(ux, -S), S); uy = fminf(fmaxf(uy, -S), S);
+          }
+          if (MAP_OUT) {
+            if (x0 + x < nx && y0 + yb + r < ny) *mo = make_float2(ux, uy);
+            mo += nx;
+          }
+          const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
+          const float dx = ux - (float)fx, dy = uy - (float)fy;
+          const float xe = -gam * tc;
+          float J = epr_expm1_small(xe);               // MUFU branch only where a lane of the warp needs it
+          if (__any_sync(0xffffffffu, fabsf(xe) >= 0.35f)) J = fabsf(xe) < 0.35f ? J : epr_exp_fast(xe) - 1.f;
+          const int tot = Fi + __float2int_rn(fixFf * J);
+          const float totf = (float)tot, te = totf * (1.f - dy), td = totf * dy, ex = 1.f - dx;
+          const int c00 = __float2int_rn(te * ex), c10 = __float2int_rn(te * dx), c01 = __float2int_rn(td * ex);
+          const int c11 = tot - c00 - c10 - c01;
+          // ax = x + fx ∈ [−1, ST_W − 1], ay ∈ [−1, ST_H − 1]: all four corners are inside the bordered accumulator
+          if ((unsigned)(x + fx + 1) <= ST_W && (unsigned)(yb + r + fy + 1) <= ST_H) {
+            const unsigned a0 = ab + 4u * (unsigned)(fy * ST_AP + fx);
+            red_shared_u32(a0, (unsigned)c00);
+            red_shared_u32(a0 + 4, (unsigned)c10);
+            red_shared_u32(a0 + 4 * ST_AP, (unsigned)c01);
+            red_shared_u32(a0 + 4 * ST_AP + 4, (unsigned)c11);
+          }
+          tn = tc; tc = ts; ts = ts2; tl = tl2; tr = tr2;
+          ab += 4u * ST_AP;
         }
-        const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
-        const float dx = ux - (float)fx, dy = uy - (float)fy;
-        const float xe = -gam * tc;
-        float J = epr_expm1_small(xe);                 // MUFU branch only where a lane of the warp needs it
-        if (__any_sync(0xffffffffu, fabsf(xe) >= 0.35f)) J = fabsf(xe) < 0.35f ? J : __expf(xe) - 1.f;
-        const int tot = Fi + __float2int_rn(fixFf * J);
-        const float totf = (float)tot, te = totf * (1.f - dy), td = totf * dy, ex = 1.f - dx;
-        const int c00 = __float2int_rn(te * ex), c10 = __float2int_rn(te * dx), c01 = __float2int_rn(td * ex);
-        const int c11 = tot - c00 - c10 - c01;
-        // ax = x + fx ∈ [−1, ST_W − 1], ay ∈ [−1, ST_H − 1]: all four corners are inside the bordered accumulator
-        if ((unsigned)(x + fx + 1) <= ST_W && (unsigned)(yb + r + fy + 1) <= ST_H) {
-          const unsigned a0 = ab + 4u * (unsigned)(fy * ST_AP + fx);
-          red_shared_u32(a0, (unsigned)c00);
-          red_shared_u32(a0 + 4, (unsigned)c10);
-          red_shared_u32(a0 + 4 * ST_AP, (unsigned)c01);
-          red_shared_u32(a0 + 4 * ST_AP + 4, (unsigned)c11);
+        if (CLAMP) {
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) md_in = fmaxf(md_in, __shfl_xor_sync(0xffffffffu, md_in, o));
+          if (lane == 0) atomicMax(&s_maxd_in, __float_as_uint(md_in));
         }
-        tn = tc; tc = ts; ts = ts2; tl = tl2; tr = tr2;
-        ab += 4u * ST_AP;
-      }
+      };
+      // s_maxd_in is complete after line 0 (two barriers lie between its last update and the first read below)
+      if (s > 0 && fabsf(cs) * fmaxf(__uint_as_float(s_maxd), __uint_as_float(s_maxd_in)) <= S) interior(std::false_type{});
+      else interior(std::true_type{});
     }
     // (2) FROM_TAU: the ring of width He around the tile (two bands of He rows, two of He columns), few of whose
     // sources reach the tile; otherwise (epr_transport): the whole region, row-major.

@@ -24,6 +24,13 @@ __device__ __forceinline__ float epr_expm1_small(float x) {
   return fmaf(x * x, q, x);
 }
 
+// e^x by the MUFU exponential alone (ex2.approx.ftz, 2^-22 relative; no denormal rescue: callers' results saturate)
+__device__ __forceinline__ float epr_exp_fast(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x * 1.4426950408889634f));
+  return y;
+}
+
 __device__ __forceinline__ float epr_expm1(float x) {
   float q = fmaf(x, 2.48015873e-5f, 1.98412698e-4f);
   q = fmaf(x, q, 1.38888889e-3f);
