@@ -219,6 +219,7 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->pred, wb * n_bins * plane * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->res, wb * n_bins * plane * sizeof(float));
   if (e == cudaSuccess && solver == EPR_NONLOCAL) e = cudaMalloc((void**)&p->res2, wb * n_bins * plane * sizeof(float));
+  if (e == cudaSuccess && solver == EPR_NONLOCAL) e = cudaMalloc((void**)&p->gmax, wb * (size_t)(nx / 16) * (ny / 16) * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->spec, wb * n_bins * plane * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->spec_sum, wb * plane * sizeof(float));
   if (e != cudaSuccess) FAIL(p, e == cudaErrorMemoryAllocation ? EPR_ENOMEM : EPR_ECUDA, "workspace: %s", cudaGetErrorString(e));
@@ -286,7 +287,7 @@ extern "C" epr_status epr_destroy(epr_plan_t p) {
   cudaDeviceSynchronize();
   cudaFree(p->tw_row); cudaFree(p->tw_r2c); cudaFree(p->tw_col); cudaFree(p->tw_col_inv); cudaFree(p->lam_x); cudaFree(p->lam_y);
   cudaFree(p->tau); cudaFree(p->pred); cudaFree(p->res); cudaFree(p->res2); cudaFree(p->spec); cudaFree(p->spec_sum);
-  cudaFree(p->raymap);
+  cudaFree(p->raymap); cudaFree(p->gmax);
   if (p->graph_exec) cudaGraphExecDestroy(p->graph_exec);
   if (p->prof) { epr_profile_read(p, 0, NULL, NULL, NULL, 1); delete (EprProf*)p->prof; }
   for (int i = 0; i < 2; ++i) { cudaFree(p->stage_in[i]); cudaFree(p->stage_out[i]); }
@@ -324,6 +325,7 @@ extern "C" epr_status epr_forward(epr_plan_t p, int batch, const float* tau, flo
   } else {
     if ((st = ensure_raymap(p)) != EPR_OK) return st;
     KL(p, K_SPLAT, cs, epr_launch_splat(p, batch, tau, NULL, NULL, p->raymap, p->pred, 0, NULL, cs));
+    p->launches += 1;                                  // k_grad_blockmax, launched ahead of the splat
     KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, P_sum, P_bins, cs));
     p->raymap_batch = batch;
   }
@@ -401,8 +403,10 @@ static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* ta
     } else {
       if (p->n_bins == 1) {
         KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->res, 2, d, cs));       // a0 + a1-N + a2 fused
+        p->launches += 1;                                  // k_grad_blockmax, launched ahead of the splat
       } else {
         KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->pred, 0, NULL, cs));   // a0 + a1-N
+        p->launches += 1;                                  // k_grad_blockmax, launched ahead of the splat
         KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, p->res, cs));           // a2
       }
       KL(p, K_GATHER, cs, epr_launch_gather(p, nb, tau, NULL, p->res, p->res2, cs));          // a3

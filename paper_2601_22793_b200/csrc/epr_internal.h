@@ -50,6 +50,7 @@ struct epr_plan_s {
   CUtensorMap map_spec;        // TMA descriptors of spec / spec_sum as [rows][nx floats], box 8 floats x 256 rows
   CUtensorMap map_spec_sum;
   int tma_ok;                  // descriptors valid (power-of-two ny ≥ 256, nx % 8 == 0)
+  float* gmax;                 // [work_batch][ny/16][nx/16] block maxima of |D⁰τ| (non-local: k_grad_blockmax)
   float2* raymap;              // [work_batch][n_bins][ny][nx] stored u_s (lazy, epr_forward non-local)
   int raymap_batch;            // batch of the stored map (0 = none)
   // host staging for epr_retrieve_host
@@ -81,6 +82,8 @@ cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float
 // out_mode 0: out[b][s] = P_s − f_s;  1: out[b][s] = P_s (linear transport);  2 (one line): out[b] = e = (d−1) − (P−f)
 cudaError_t epr_launch_splat(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
                              float2* map_out, float* out, int out_mode, const float* d, cudaStream_t st);
+// block maxima of |D⁰τ| into p->gmax (launched by epr_launch_splat when the sources come from τ)
+cudaError_t epr_launch_grad_blockmax(const epr_plan_s* p, int batch, const float* tau, cudaStream_t st);
 cudaError_t epr_launch_residual(const epr_plan_s* p, int batch, const float* d, const float* pred, float* es,
                                 cudaStream_t st);
 cudaError_t epr_launch_pred_out(const epr_plan_s* p, int batch, const float* pred, float* P_sum, float* P_bins,

@@ -394,6 +394,51 @@ cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float
 }
 
 // =====================================================================================================
+// Helper of a1-N / a3: gmax[b][y/16][x/16] = max over the 16x16-pixel block of max(|τ[x+1] − τ[x−1]|, |τ[y+1] − τ[y−1]|)
+// (periodic; nx, ny are multiples of 16).  With u_s = c_s D⁰τ (Eq. (2)) it bounds the ray shifts of a
+// block, which tells the splat how wide a ring of foreign sources can reach a detector tile and the gather how wide a
+// halo of the residual a tile needs — before either loads anything.  One pass over τ (4 B/px).
+// CTA: 128 columns x 16 rows = 8 blocks; thread: one strip of 4 pixels in rows ry and ry + 8.
+// =====================================================================================================
+__global__ void __launch_bounds__(256) k_grad_blockmax(int nx, int ny, const float* __restrict__ tau, float* __restrict__ gmax) {
+  __shared__ unsigned s_m[8];
+  const int tid = threadIdx.x, lane = tid & 31;
+  if (tid < 8) s_m[tid] = 0u;
+  __syncthreads();
+  const int x = blockIdx.x * 128 + 4 * lane;
+  float m = 0.f;
+  if (x < nx) {
+    const float* tb = tau + (size_t)blockIdx.z * nx * ny;
+    const int xm = x == 0 ? nx - 1 : x - 1, xp = x + 4 == nx ? 0 : x + 4;
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const int y = blockIdx.y * 16 + (tid >> 5) + 8 * k;
+      const int ym = y == 0 ? ny - 1 : y - 1, yp = y + 1 == ny ? 0 : y + 1;
+      const float* row = tb + (size_t)y * nx;
+      const float4 c = __ldg(reinterpret_cast<const float4*>(row + x));
+      const float4 n = __ldg(reinterpret_cast<const float4*>(tb + (size_t)ym * nx + x));
+      const float4 s4 = __ldg(reinterpret_cast<const float4*>(tb + (size_t)yp * nx + x));
+      const float l = __ldg(row + xm), r = __ldg(row + xp);
+      m = fmaxf(m, fmaxf(fmaxf(fabsf(c.y - l), fabsf(c.z - c.x)), fmaxf(fabsf(c.w - c.y), fabsf(r - c.z))));
+      m = fmaxf(m, fmaxf(fmaxf(fabsf(s4.x - n.x), fabsf(s4.y - n.y)), fmaxf(fabsf(s4.z - n.z), fabsf(s4.w - n.w))));
+    }
+  }
+  m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
+  m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
+  if ((lane & 3) == 0) atomicMax(&s_m[lane >> 2], __float_as_uint(m));
+  __syncthreads();
+  const int nbx = nx >> 4;
+  if (tid < 8 && blockIdx.x * 8 + tid < nbx)
+    gmax[((size_t)blockIdx.z * (ny >> 4) + blockIdx.y) * nbx + blockIdx.x * 8 + tid] = __uint_as_float(s_m[tid]);
+}
+
+cudaError_t epr_launch_grad_blockmax(const epr_plan_s* p, int batch, const float* tau, cudaStream_t st) {
+  dim3 grid((p->nx + 127) / 128, p->ny / 16, batch);
+  k_grad_blockmax<<<grid, 256, 0, st>>>(p->nx, p->ny, tau, p->gmax);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
 // a1-N  ray map (Eq. (2), clamp R6) + mass-conserving bilinear splat,
 //       DETECTOR-TILE-OWNED: one CTA owns ST_W x ST_H detector pixels of one projection and walks over every
 //       source pixel that can reach them (the tile grown by H = ceil(S) + 1), so the 4-way scatter is resolved
@@ -421,7 +466,8 @@ template <bool FROM_TAU, bool MAP_OUT, int ST_NT>
 __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny, float S, int H,
                                                     const float* __restrict__ tau, const float* __restrict__ I_bins,
                                                     const float2* __restrict__ map_in, float2* __restrict__ map_out,
-                                                    float* __restrict__ out, int out_mode, const float* __restrict__ d) {
+                                                    float* __restrict__ out, int out_mode, const float* __restrict__ d,
+                                                    const float* __restrict__ gmax) {
   extern __shared__ __align__(16) unsigned char st_raw[];
   unsigned* s_acc = reinterpret_cast<unsigned*>(st_raw);                              // [ST_AROWS][ST_AP]
   float* s_tau = reinterpret_cast<float*>(st_raw + ST_AP * ST_AROWS * sizeof(unsigned));   // [RH + 2][TP]
@@ -433,54 +479,47 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
   const int TP = ST_W + 2 * Ha;                        // τ tile pitch; tile column of tile-relative x is x + Ha
   const unsigned plane = (unsigned)nx * (unsigned)ny;
 
+  // Largest |D⁰τ| (times 2) among the sources in the ring of width H around the tile (s_maxd) and in the tile itself
+  // (s_maxd_in), from the 16x16-block maxima of k_grad_blockmax: a source at distance D from the tile reaches it only
+  // if ⌊|u|⌋ + 1 ≥ D, so the ring that has to be walked (and loaded) is He ≤ H wide.
+  __shared__ unsigned s_maxd, s_maxd_in;
   if (FROM_TAU) {
-    // τ tile rows y0 − H − 1 …, columns x0 − Ha …: 16-byte cp.async chunks (nx % 4 == 0: a chunk never straddles the wrap)
+    if (tid == 0) { s_maxd = 0u; s_maxd_in = 0u; }
+    __syncthreads();
+    const int nbx = nx >> 4, nby = ny >> 4;
+    const int nsx = (ST_W + 2 * H + 15) / 16 + 1, nsy = (ST_H + 2 * H + 15) / 16 + 1;
+    const float* gm = gmax + (size_t)b * nbx * nby;
+    for (int i = tid; i < nsx * nsy; i += ST_NT) {
+      const int j = i / nsx, ii = i - j * nsx;
+      const int px = min(-H + 16 * ii, ST_W - 1 + H), py = min(-H + 16 * j, ST_H - 1 + H);   // tile-relative sample
+      const bool inside = (unsigned)px < ST_W && (unsigned)py < ST_H;
+      const float v = __ldg(&gm[(wrapm(y0 + py, ny) >> 4) * nbx + (wrapm(x0 + px, nx) >> 4)]);
+      atomicMax(inside ? &s_maxd_in : &s_maxd, __float_as_uint(v));
+    }
+    __syncthreads();
+    float csmax = 0.f;
+    for (int s = 0; s < L.n_bins; ++s) csmax = fmaxf(csmax, 0.5f * L.a[s] * L.gamma[s]);
+    const int Hl = min(H, (int)fminf(csmax * __uint_as_float(s_maxd), S) + 1);      // widest ring of any line
+    // τ tile rows y0 − Hl − 1 … y0 + ST_H + Hl (tile rows H − Hl … H + ST_H + 1 + Hl), columns x0 − Ha …:
+    // 16-byte cp.async chunks (nx % 4 == 0: a chunk never straddles the wrap), spread evenly over the threads
     const float* tb = tau + (size_t)b * plane;
-    const int step_x = 128 % nx, step_y = NW % ny;
-    int gy = wrapm(y0 - H - 1 + warp, ny);
-    const int gx0 = wrapm(x0 - Ha + 4 * lane, nx);
-    for (int ly = warp; ly < RH + 2; ly += NW) {
-      const float* row = tb + (unsigned)gy * nx;
-      int gx = gx0;
-      for (int cx = lane; cx < TP / 4; cx += 32) {
-        cp_async16(s_tau + ly * TP + 4 * cx, row + gx);
-        gx += step_x;
-        if (gx >= nx) gx -= nx;
-      }
-      gy += step_y;
-      if (gy >= ny) gy -= ny;
+    const int cpr = TP / 4, nrows = ST_H + 2 + 2 * Hl;
+    const float inv_cpr = 1.f / (float)cpr;
+    const bool big = nx >= 2 * (ST_W + 2 * Ha) && ny >= 2 * (ST_H + 2 * H + 2);
+    for (int i = tid; i < nrows * cpr; i += ST_NT) {
+      const int r = (int)(((float)i + 0.5f) * inv_cpr), cx = i - r * cpr;
+      const int ly = H - Hl + r;
+      int gy = y0 - H - 1 + ly, gx = x0 - Ha + 4 * cx;
+      if (big) { gy = wrap1(gy, ny); gx = wrap1(gx, nx); } else { gy = wrapm(gy, ny); gx = wrapm(gx, nx); }
+      cp_async16(s_tau + ly * TP + 4 * cx, tb + (unsigned)gy * nx + gx);
     }
     cp_async_commit();
   }
-  // Largest |D⁰τ| (times 2) among the sources OUTSIDE the tile: bounds how far away a source can be and still
-  // reach the tile, so that the walk below covers the tile grown by He ≤ H only.
-  __shared__ unsigned s_maxd, s_maxd_in;
-  if (tid == 0) { s_maxd = 0u; s_maxd_in = 0u; }
   for (int s = 0; s < L.n_bins; ++s) {
     const size_t pl = ((size_t)b * L.n_bins + s) * plane;
     __syncthreads();                                   // previous bin flushed
     for (int i = tid; i < ST_AP * ST_AROWS / 4; i += ST_NT) reinterpret_cast<uint4*>(s_acc)[i] = make_uint4(0u, 0u, 0u, 0u);
-    if (FROM_TAU && s == 0) {
-      cp_async_wait<0>();
-      __syncthreads();
-      float md = 0.f;
-      // ring of width H around the tile only: whole rows above and below, two H-column segments beside it
-      for (int sy = warp; sy < RH; sy += NW) {
-        const float* trow = s_tau + (sy + 1) * TP + (Ha - H);
-        if (sy < H || sy >= H + ST_H) {
-          for (int sx = lane; sx < RW; sx += 32)
-            md = fmaxf(md, fmaxf(fabsf(trow[sx + 1] - trow[sx - 1]), fabsf(trow[sx + TP] - trow[sx - TP])));
-        } else {
-          for (int l = lane; l < 2 * H; l += 32) {
-            const int sx = l < H ? l : l + ST_W;
-            md = fmaxf(md, fmaxf(fabsf(trow[sx + 1] - trow[sx - 1]), fabsf(trow[sx + TP] - trow[sx - TP])));
-          }
-        }
-      }
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) md = fmaxf(md, __shfl_xor_sync(0xffffffffu, md, o));
-      if (lane == 0) atomicMax(&s_maxd, __float_as_uint(md));
-    }
+    if (FROM_TAU && s == 0) cp_async_wait<0>();
     __syncthreads();
     const float cs = -0.5f * L.a[s] * L.gamma[s], gam = L.gamma[s], fixFf = (float)L.fixF[s];
     const int Fi = (int)L.fixFi[s];
@@ -495,29 +534,24 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       // down its rows with the column's τ values in registers (3 shared loads per source instead of 5, no index
       // arithmetic: one address per array advances by a row); the loads of row r + 1 are issued before the atomics
       // of row r.  32-bit shared addresses are formed once (the compiler otherwise rebuilds them per source).
-      // Line 0 also records the largest |D⁰τ| of the tile itself; the later lines then skip the clamp of u when
-      // |c_s| · max|D⁰τ| over the whole region cannot exceed S.
+      // The clamp of u is skipped when |c_s| · max|D⁰τ| over the tile cannot exceed S.
       constexpr int RG = NW / 4, ROWS = ST_H / RG;
       const int x = (warp & 3) * 32 + lane, yb = (warp >> 2) * ROWS;
       const unsigned TP4 = 4u * TP;
       const unsigned rb0 = (unsigned)__cvta_generic_to_shared(s_tau) + 4u * (unsigned)((yb + H + 1) * TP + x + Ha);
       const unsigned ab0 = (unsigned)__cvta_generic_to_shared(s_acc) + 4u * (unsigned)((yb + 1) * ST_AP + x + 4);
       auto interior = [&](auto clamp_tag) {
-        constexpr bool CLAMP = decltype(clamp_tag)::value;      // CLAMP is also "line 0": track the tile's max|D⁰τ|
+        constexpr bool CLAMP = decltype(clamp_tag)::value;
         unsigned rb = rb0, ab = ab0;
         float tn = lds_f32(rb - TP4), tc = lds_f32(rb), ts = lds_f32(rb + TP4), tl = lds_f32(rb - 4), tr = lds_f32(rb + 4);
         float2* mo = MAP_OUT ? map_out + pl + (size_t)(y0 + yb) * nx + (x0 + x) : nullptr;
-        float md_in = 0.f;
 #pragma unroll 2
         for (int r = 0; r < ROWS; ++r) {
           rb += TP4;                                   // one row beyond the strip at the last r: still inside the τ tile
           const float ts2 = lds_f32(rb + TP4), tl2 = lds_f32(rb - 4), tr2 = lds_f32(rb + 4);
           const float gx = tr - tl, gy = ts - tn;
           float ux = cs * gx, uy = cs * gy;
-          if (CLAMP) {
-            md_in = fmaxf(md_in, fmaxf(fabsf(gx), fabsf(gy)));
-            ux = fminf(fmaxf(ux, -S), S); uy = fminf(fmaxf(uy, -S), S);
-          }
+          if (CLAMP) { ux = fminf(fmaxf(ux, -S), S); uy = fminf(fmaxf(uy, -S), S); }
           if (MAP_OUT) {
             if (x0 + x < nx && y0 + yb + r < ny) *mo = make_float2(ux, uy);
             mo += nx;
@@ -542,14 +576,8 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
           tn = tc; tc = ts; ts = ts2; tl = tl2; tr = tr2;
           ab += 4u * ST_AP;
         }
-        if (CLAMP) {
-#pragma unroll
-          for (int o = 16; o > 0; o >>= 1) md_in = fmaxf(md_in, __shfl_xor_sync(0xffffffffu, md_in, o));
-          if (lane == 0) atomicMax(&s_maxd_in, __float_as_uint(md_in));
-        }
       };
-      // s_maxd_in is complete after line 0 (two barriers lie between its last update and the first read below)
-      if (s > 0 && fabsf(cs) * fmaxf(__uint_as_float(s_maxd), __uint_as_float(s_maxd_in)) <= S) interior(std::false_type{});
+      if (fabsf(cs) * __uint_as_float(s_maxd_in) <= S) interior(std::false_type{});
       else interior(std::true_type{});
     }
     // (2) FROM_TAU: the ring of width He around the tile (two bands of He rows, two of He columns), few of whose
@@ -648,12 +676,16 @@ static cudaError_t launch_splat_t(const epr_plan_s* p, int batch, const float* t
     attr[big] = smem;
   }
   dim3 grid((p->nx + ST_W - 1) / ST_W, (p->ny + ST_H - 1) / ST_H, batch);
+  if (FROM_TAU) {                                      // block maxima of |D⁰τ| (also used by the gather of this τ)
+    const cudaError_t e = epr_launch_grad_blockmax(p, batch, tau, st);
+    if (e != cudaSuccess) return e;
+  }
   if (big)
     k_splat_tile<FROM_TAU, MAP_OUT, 1024><<<grid, 1024, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, H, tau, I_bins,
-                                                                    map_in, map_out, out, out_mode, d);
+                                                                    map_in, map_out, out, out_mode, d, p->gmax);
   else
     k_splat_tile<FROM_TAU, MAP_OUT, 512><<<grid, 512, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, H, tau, I_bins,
-                                                                  map_in, map_out, out, out_mode, d);
+                                                                  map_in, map_out, out, out_mode, d, p->gmax);
   return cudaGetLastError();
 }
 
