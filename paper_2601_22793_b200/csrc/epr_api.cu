@@ -344,7 +344,7 @@ extern "C" epr_status epr_adjoint(epr_plan_t p, int batch, const float* e_bins, 
   }
   if (e_bins == r_bins) FAIL(p, EPR_EINVAL, "epr_adjoint: the gather cannot run in place");
   if (!p->raymap || p->raymap_batch < batch) FAIL(p, EPR_EINVAL, "epr_adjoint: no ray map stored for batch %d (call epr_forward first)", batch);
-  KL(p, K_GATHER, cs, epr_launch_gather(p, batch, NULL, p->raymap, e_bins, r_bins, cs));
+  KL(p, K_GATHER, cs, epr_launch_gather(p, batch, NULL, p->raymap, e_bins, r_bins, 0, cs));
   return EPR_OK;
 }
 
@@ -409,7 +409,7 @@ static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* ta
         p->launches += 1;                                  // k_grad_blockmax, launched ahead of the splat
         KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, p->res, cs));           // a2
       }
-      KL(p, K_GATHER, cs, epr_launch_gather(p, nb, tau, NULL, p->res, p->res2, cs));          // a3
+      KL(p, K_GATHER, cs, epr_launch_gather(p, nb, tau, NULL, p->res, p->res2, 1, cs));          // a3
       r = p->res2;
     }
     KL(p, K_ROWS_R2C, cs, epr_launch_rows_r2c(p, planes, r, 0.f, p->spec, cs));                 // a4

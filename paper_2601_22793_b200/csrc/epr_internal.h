@@ -88,8 +88,9 @@ cudaError_t epr_launch_residual(const epr_plan_s* p, int batch, const float* d, 
                                 cudaStream_t st);
 cudaError_t epr_launch_pred_out(const epr_plan_s* p, int batch, const float* pred, float* P_sum, float* P_bins,
                                 cudaStream_t st);
+// gmax_fresh: p->gmax holds the block maxima of this tau (epr_launch_splat ran on it) -> shared-memory tile kernel
 cudaError_t epr_launch_gather(const epr_plan_s* p, int batch, const float* tau, const float2* map_in, const float* es,
-                              float* r, cudaStream_t st);
+                              float* r, int gmax_fresh, cudaStream_t st);
 cudaError_t epr_launch_rows_r2c(const epr_plan_s* p, int planes, const float* in, float in_offset, float2* spec,
                                 cudaStream_t st);
 // mode 0: per-plane filter with bin = plane % n_bins (out has `planes` planes);

@@ -824,8 +824,145 @@ __global__ void __launch_bounds__(256) k_gather(EprLines L, int nx, int ny, floa
   }
 }
 
+// -----------------------------------------------------------------------------------------------------
+// a3 through shared memory (the loop's configuration: ray map recomputed from τ, block maxima of |D⁰τ| at hand).
+// One CTA = GT_W x GT_H pixels of one projection.  The tile's own max|u_s| (from p->gmax) gives the halo Hg of the
+// residual it can touch; e_s[tile + Hg] is staged by 16-byte cp.async (line s + 1 under the gather of line s) and the
+// four corners are plain shared loads at consecutive lanes — one wavefront each instead of the ~4.5 lines a scattered
+// global load touches.  The τ differences are formed once and reused for every line.  Lines whose halo exceeds
+// GT_HG fall back to global loads inside the same kernel.
+#define GT_W 128
+#define GT_H 64
+#define GT_HG 8                        // largest halo served from shared memory (multiple of 4)
+#define GT_EP (GT_W + 2 * GT_HG)       // pitch of a staged tile
+#define GT_ER (GT_H + 2 * GT_HG)
+#define GT_NT 512
+#define GT_PPT (GT_W * GT_H / GT_NT)   // pixels per thread (rows y = (tid >> 7) + 4 k of column tid & 127)
+
+template <bool BIG>          // BIG: nx, ny ≥ 2 (tile + halo), so one conditional add wraps an index
+__global__ void __launch_bounds__(GT_NT, 2) k_gather_tile(EprLines L, int nx, int ny, float S, const float* __restrict__ tau,
+                                                        const float* __restrict__ gmax, const float* __restrict__ es,
+                                                        float* __restrict__ r) {
+  extern __shared__ __align__(16) float s_e[];        // [2][GT_ER][GT_EP]
+  __shared__ unsigned s_max;
+  const int tid = threadIdx.x, b = blockIdx.z;
+  const int x0 = blockIdx.x * GT_W, y0 = blockIdx.y * GT_H;
+  const unsigned plane = (unsigned)nx * (unsigned)ny;
+  if (tid == 0) s_max = 0u;
+  __syncthreads();
+  if (tid < 32) {
+    const int px = x0 + 16 * (tid & 7), py = y0 + 16 * (tid >> 3);
+    if (px < nx && py < ny) atomicMax(&s_max, __float_as_uint(__ldg(&gmax[((size_t)b * (ny >> 4) + (py >> 4)) * (nx >> 4) + (px >> 4)])));
+  }
+  __syncthreads();
+  const float maxd = __uint_as_float(s_max);
+  const size_t p0 = (size_t)b * L.n_bins * plane;
+  // reads reach x + fx … x + fx + 1 with fx ∈ [−Hg, Hg − 1], Hg = ⌊max|u|⌋ + 1
+  auto halo = [&](int s) { return (int)fminf(0.5f * L.a[s] * L.gamma[s] * maxd, S) + 1; };
+  auto stage = [&](int s) {                           // request e_s[tile + halo] into buffer s & 1
+    const int Hg = halo(s);
+    if (Hg <= GT_HG) {
+      const int Hga = (Hg + 3) & ~3, rows = GT_H + 2 * Hg, cpr = (GT_W + 2 * Hga) / 4;
+      const float inv_cpr = 1.f / (float)cpr;
+      const float* eb = es + p0 + (size_t)s * plane;
+      float* dst = s_e + (s & 1) * (GT_ER * GT_EP) + (GT_HG - Hg) * GT_EP + (GT_HG - Hga);
+      for (int i = tid; i < rows * cpr; i += GT_NT) {
+        const int rr = (int)(((float)i + 0.5f) * inv_cpr), c = i - rr * cpr;
+        int gy = y0 - Hg + rr, gx = x0 - Hga + 4 * c;
+        if (BIG) { gy = wrap1(gy, ny); gx = wrap1(gx, nx); } else { gy = wrapm(gy, ny); gx = wrapm(gx, nx); }
+        cp_async16(dst + rr * GT_EP + 4 * c, eb + (unsigned)gy * nx + gx);
+      }
+    }
+    cp_async_commit();
+  };
+  stage(0);
+  // τ differences of this thread's pixels (column x, rows yy + 4 k), formed once for all lines
+  const int x = tid & (GT_W - 1), yy = tid >> 7;
+  const bool xin = x0 + x < nx;
+  float dtx[GT_PPT], dty[GT_PPT];
+  {
+    const float* tb = tau + (size_t)b * plane;
+    const int gx = xin ? x0 + x : 0;
+    const int xm = gx == 0 ? nx - 1 : gx - 1, xp = gx + 1 == nx ? 0 : gx + 1;
+#pragma unroll
+    for (int k = 0; k < GT_PPT; ++k) {
+      const int gy = min(y0 + yy + 4 * k, ny - 1);
+      const int ym = gy == 0 ? ny - 1 : gy - 1, yp = gy + 1 == ny ? 0 : gy + 1;
+      const float* row = tb + (unsigned)gy * nx;
+      dtx[k] = __ldg(row + xp) - __ldg(row + xm);
+      dty[k] = __ldg(tb + (unsigned)yp * nx + gx) - __ldg(tb + (unsigned)ym * nx + gx);
+    }
+  }
+  for (int s = 0; s < L.n_bins; ++s) {
+    if (s + 1 < L.n_bins) { stage(s + 1); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
+    __syncthreads();                                   // line s is staged (every thread's chunks have landed)
+    const float c = -0.5f * L.a[s] * L.gamma[s];
+    const int Hg = halo(s);
+    float* rb = r + p0 + (size_t)s * plane + (size_t)(y0 + yy) * nx + (x0 + x);
+    if (Hg <= GT_HG) {
+      const unsigned base = (unsigned)__cvta_generic_to_shared(s_e + (s & 1) * (GT_ER * GT_EP)) +
+                            4u * (unsigned)((yy + GT_HG) * GT_EP + x + GT_HG);
+      const size_t nx4 = 4 * (size_t)nx;
+      // CLAMP: some |u| of the tile may exceed S;  FULL: the whole tile lies inside the image (no per-pixel test)
+      auto body = [&](auto clamp_tag, auto full_tag) {
+        constexpr bool CLAMP = decltype(clamp_tag)::value, FULL = decltype(full_tag)::value;
+#pragma unroll
+        for (int k = 0; k < GT_PPT; ++k) {
+          float ux = c * dtx[k], uy = c * dty[k];
+          if (CLAMP) { ux = fminf(fmaxf(ux, -S), S); uy = fminf(fmaxf(uy, -S), S); }
+          const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
+          const float dx = ux - (float)fx, dy = uy - (float)fy;
+          const unsigned a = base + 4u * (unsigned)(fy * GT_EP + fx);
+          // the row offsets 16 k GT_EP are compile-time after unrolling: ptxas folds them into the load
+          const float e00 = lds_f32(a + 16 * k * GT_EP), e10 = lds_f32(a + 16 * k * GT_EP + 4);
+          const float e01 = lds_f32(a + (16 * k + 4) * GT_EP), e11 = lds_f32(a + (16 * k + 4) * GT_EP + 4);
+          // Eq. (4): Σ_ab w_ab e[y0+b][x0+a], w00 = (1−dx)(1−dy), w10 = dx(1−dy), w01 = (1−dx)dy, w11 = dx dy
+          const float t0 = fmaf(dx, e10 - e00, e00), t1 = fmaf(dx, e11 - e01, e01);
+          if (FULL || (xin && y0 + yy + 4 * k < ny)) rb[k * nx4] = fmaf(dy, t1 - t0, t0);
+        }
+      };
+      const bool clamp = fabsf(c) * maxd > S, full = x0 + GT_W <= nx && y0 + GT_H <= ny;
+      if (clamp) { if (full) body(std::true_type{}, std::true_type{}); else body(std::true_type{}, std::false_type{}); }
+      else { if (full) body(std::false_type{}, std::true_type{}); else body(std::false_type{}, std::false_type{}); }
+    } else if (xin) {
+      const float* eb = es + p0 + (size_t)s * plane;
+      for (int k = 0; k < GT_PPT; ++k) {
+        const int gy = y0 + yy + 4 * k;
+        if (gy >= ny) break;
+        const float ux = fminf(fmaxf(c * dtx[k], -S), S), uy = fminf(fmaxf(c * dty[k], -S), S);
+        const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
+        const float dx = ux - (float)fx, dy = uy - (float)fy;
+        const int ix0 = wrapm(x0 + x + fx, nx), iy0 = wrapm(gy + fy, ny);
+        const int ix1 = ix0 + 1 == nx ? 0 : ix0 + 1, iy1 = iy0 + 1 == ny ? 0 : iy0 + 1;
+        const unsigned r0 = (unsigned)iy0 * nx, r1 = (unsigned)iy1 * nx;
+        const float e00 = __ldg(eb + (r0 + ix0)), e10 = __ldg(eb + (r0 + ix1));
+        const float e01 = __ldg(eb + (r1 + ix0)), e11 = __ldg(eb + (r1 + ix1));
+        const float ex = 1.f - dx, ey = 1.f - dy;
+        rb[(size_t)(4 * k) * nx] = ey * (ex * e00 + dx * e10) + dy * (ex * e01 + dx * e11);
+      }
+    }
+    __syncthreads();                                   // buffer s & 1 is free for line s + 2
+  }
+}
+
 cudaError_t epr_launch_gather(const epr_plan_s* p, int batch, const float* tau, const float2* map_in, const float* es,
-                              float* r, cudaStream_t st) {
+                              float* r, int gmax_fresh, cudaStream_t st) {
+  if (tau && !map_in && gmax_fresh && p->gmax) {
+    // the loop: p->gmax holds the block maxima of this τ (written ahead of the splat of the same iteration)
+    constexpr size_t smem = 2 * (size_t)GT_ER * GT_EP * sizeof(float);
+    static bool attr = false;
+    if (!attr) {
+      cudaFuncSetAttribute(k_gather_tile<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      cudaFuncSetAttribute(k_gather_tile<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      attr = true;
+    }
+    dim3 grid((p->nx + GT_W - 1) / GT_W, (p->ny + GT_H - 1) / GT_H, batch);
+    if (p->nx >= 2 * GT_EP && p->ny >= 2 * GT_ER)
+      k_gather_tile<true><<<grid, GT_NT, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, tau, p->gmax, es, r);
+    else
+      k_gather_tile<false><<<grid, GT_NT, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, tau, p->gmax, es, r);
+    return cudaGetLastError();
+  }
   dim3 grid((p->nx / 4 + 63) / 64, (p->ny + 3) / 4, batch);
   if (p->nx > 32 && p->ny > 32) k_gather<true><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, tau, map_in, es, r);
   else k_gather<false><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, tau, map_in, es, r);
