@@ -405,9 +405,8 @@ static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* ta
         KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->res, 2, d, cs));       // a0 + a1-N + a2 fused
         p->launches += 1;                                  // k_grad_blockmax, launched ahead of the splat
       } else {
-        KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->pred, 0, NULL, cs));   // a0 + a1-N
+        KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->res, 3, d, cs));       // a0 + a1-N + a2 fused
         p->launches += 1;                                  // k_grad_blockmax, launched ahead of the splat
-        KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, p->res, cs));           // a2
       }
       KL(p, K_GATHER, cs, epr_launch_gather(p, nb, tau, NULL, p->res, p->res2, 1, cs));          // a3
       r = p->res2;

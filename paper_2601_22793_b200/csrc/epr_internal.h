@@ -79,7 +79,8 @@ struct epr_plan_s {
 // d_fuse != NULL (one line only): out = e = (d-1) - (P-1) directly; else out = pred[b][s] = P_s - f_s
 cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float* tau, const float* d_fuse, float* out,
                                      cudaStream_t st);
-// out_mode 0: out[b][s] = P_s − f_s;  1: out[b][s] = P_s (linear transport);  2 (one line): out[b] = e = (d−1) − (P−f)
+// out_mode 0: out[b][s] = P_s − f_s;  1: out[b][s] = P_s (linear transport);  2 (one line): out[b] = e = (d−1) − (P−f);
+// 3 (several lines): out[b][s] = e_s = w_s e, the residual split fused into the splat (needs d)
 cudaError_t epr_launch_splat(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
                              float2* map_out, float* out, int out_mode, const float* d, cudaStream_t st);
 // block maxima of |D⁰τ| into p->gmax (launched by epr_launch_splat when the sources come from τ)

@@ -452,7 +452,8 @@ cudaError_t epr_launch_grad_blockmax(const epr_plan_s* p, int batch, const float
 //   (tot · rint(w 2^24) + 2^23) >> 24 in 64-bit integers.
 //   Sources: I_s from τ (I_bins == NULL) or a given plane; u from τ (map_in == NULL; written to map_out by the
 //   tile that owns the source pixel) or from a stored map.
-//   Output (out_mode): 0  out[b][s] = P_s − f_s (float);  1  out[b][s] = P_s;  2 (one line)  out[b] = e =
+//   Output (out_mode): 0  out[b][s] = P_s − f_s (float);  1  out[b][s] = P_s;  3  out[b][s] = e_s = w_s e (the residual
+//   split a2 of several lines, fused: see the end of the kernel);  2 (one line)  out[b] = e =
 //   (d − 1) − (P − f): the detector residual a2 fused into the flush.
 // =====================================================================================================
 #define ST_W 128
@@ -618,16 +619,17 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       const float dx = ux - (float)fx, dy = uy - (float)fy;
       int tot;                                         // signed: epr_transport accepts planes of either sign
       if (FROM_TAU) {
-        const float xe = -gam * tc;                    // both expm1 branches only where a lane of the warp needs them
-        const float J = epr_expm1(xe);
+        // the same arithmetic as the interior walk, operation for operation: a source is an interior source of its
+        // own tile and a ring source of its neighbours, and all of them must agree on its four corner masses
+        const float xe = -gam * tc;
+        const float J = fabsf(xe) < 0.35f ? epr_expm1_small(xe) : epr_exp_fast(xe) - 1.f;
         tot = Fi + __float2int_rn(fixFf * J);
       } else {
         tot = __float2int_rn(__ldg(&I_bins[pl + gidx]) * 67108864.f);
       }
       // corner masses in fp32 (± 2 units of 2^-26), the 4th corner takes the exact remainder
-      const float totf = (float)tot, ex = 1.f - dx, ey = 1.f - dy;
-      const int c00 = __float2int_rn(totf * ex * ey), c10 = __float2int_rn(totf * dx * ey),
-                c01 = __float2int_rn(totf * ex * dy);
+      const float totf = (float)tot, te = totf * (1.f - dy), td = totf * dy, ex = 1.f - dx;
+      const int c00 = __float2int_rn(te * ex), c10 = __float2int_rn(te * dx), c01 = __float2int_rn(td * ex);
       const int c11 = tot - c00 - c10 - c01;
       // ax ∈ [−1, ST_W − 1], ay ∈ [−1, ST_H − 1]: all four corners are inside the bordered accumulator
       unsigned* a0 = s_acc + (ay + 1) * ST_AP + (ax + 4);
@@ -658,6 +660,41 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
         }
       }
       *reinterpret_cast<float4*>(out + pl + g) = o;
+    }
+  }
+  if (out_mode == 3) {
+    // a2 fused (several lines): e = (d − 1) − Σ_s (P_s − f_s), e_s = w_s e with w_s = P_s⁺ / Σ_t P_t⁺ (fallback f_s),
+    // PAPER.md:231, reading R8 — the arithmetic of k_residual, in place.  Every thread re-reads exactly the values
+    // P_s − f_s it stored above (same thread, same addresses: program order makes them visible; they are still in L2)
+    // and overwrites them with e_s, so the N prediction planes never come back from HBM.
+    const float off = 1.f + L.fsum_dev;
+    float* ob = out + (size_t)b * L.n_bins * plane;
+    for (int i = tid; i < ST_W * ST_H / 4; i += ST_NT) {
+      const int ty = i / (ST_W / 4), tx = 4 * (i - ty * (ST_W / 4));
+      const int gx = x0 + tx, gy = y0 + ty;
+      if (gx >= nx || gy >= ny) continue;
+      float* og = ob + (unsigned)gy * nx + gx;
+      float4 sum = make_float4(0.f, 0.f, 0.f, 0.f), den = sum;
+      for (int s = 0; s < L.n_bins; ++s) {
+        const float4 pd = __ldcg(reinterpret_cast<const float4*>(og + (size_t)s * plane));
+        const float f = L.f[s];
+        sum.x += pd.x; sum.y += pd.y; sum.z += pd.z; sum.w += pd.w;
+        den.x += fmaxf(f + pd.x, 0.f); den.y += fmaxf(f + pd.y, 0.f); den.z += fmaxf(f + pd.z, 0.f); den.w += fmaxf(f + pd.w, 0.f);
+      }
+      const float4 dd = __ldg(reinterpret_cast<const float4*>(d + (size_t)b * plane + (unsigned)gy * nx + gx));
+      const float4 e = make_float4((dd.x - off) - sum.x, (dd.y - off) - sum.y, (dd.z - off) - sum.z, (dd.w - off) - sum.w);
+      const float4 q = make_float4(den.x > 0.f ? e.x / den.x : 0.f, den.y > 0.f ? e.y / den.y : 0.f,
+                                   den.z > 0.f ? e.z / den.z : 0.f, den.w > 0.f ? e.w / den.w : 0.f);
+      for (int s = 0; s < L.n_bins; ++s) {
+        const float4 pd = __ldcg(reinterpret_cast<const float4*>(og + (size_t)s * plane));
+        const float f = L.f[s];
+        float4 o;
+        o.x = den.x > 0.f ? fmaxf(f + pd.x, 0.f) * q.x : f * e.x;
+        o.y = den.y > 0.f ? fmaxf(f + pd.y, 0.f) * q.y : f * e.y;
+        o.z = den.z > 0.f ? fmaxf(f + pd.z, 0.f) * q.z : f * e.z;
+        o.w = den.w > 0.f ? fmaxf(f + pd.w, 0.f) * q.w : f * e.w;
+        *reinterpret_cast<float4*>(og + (size_t)s * plane) = o;
+      }
     }
   }
 }
