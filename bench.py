@@ -33,7 +33,9 @@ UNIT = "projections/s"
 def kernel_bytes_per_px(name, nb, solver):
     return {
         "k_forward_local": 12 if nb == 1 else 4 + 4 * nb,   # 1 line: fused march R tau, R d, W e; else R tau, W (P_s - f_s) x nb
-        "k_splat": 12 if nb == 1 else 4 + 4 * nb,   # 1 line: fused residual R tau, R d, W e; else R tau, W (P_s - f_s) x nb
+        # splat with the residual (a2) fused: R tau, R d, W e_s x nb.  Not counted: the second read of tau by the
+        # block-maximum prepass and the N prediction planes that stay in L2 between flush and split (design overheads)
+        "k_splat": 8 + 4 * nb,
         "k_residual": 4 + 8 * nb,               # R d, R pred x nb, W e_s x nb
         "k_gather": 4 + 8 * nb,                 # R tau, R e_s x nb, W r_s x nb
         "k_rows_r2c": 8,                        # per plane: R 4, W half spectrum 4
