@@ -189,6 +189,12 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
     abar += p->h_f[s] * p->h_a[s];
   }
   L.abar = (float)abar;
+  for (int s = 0; s < n_bins; ++s) {
+    L.pj_a[s] = (float)(-p->h_gamma[s] * 1.4426950408889634);
+    L.pj_b[s] = (float)log2(p->h_f[s]);
+    L.pj_g2[s] = (float)(p->h_gamma[s] * p->h_gamma[s]);
+    L.pj_g3[s] = (float)(p->h_gamma[s] * p->h_gamma[s] * p->h_gamma[s]);
+  }
   L.gamma_max = 0.f;
   for (int s = 0; s < n_bins; ++s) L.gamma_max = fmaxf(L.gamma_max, L.gamma[s]);
   double fs = 0;

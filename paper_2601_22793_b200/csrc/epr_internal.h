@@ -21,6 +21,10 @@ struct EprLines {
   double fixF[EPR_MAX_BINS];    // f_s · 2^26 (double, for the splat)
   unsigned fixFi[EPR_MAX_BINS]; // rint(f_s · 2^26)
   float fixCorr[EPR_MAX_BINS];  // rint(f_s 2^26)·2^-26 − f_s
+  float pj_a[EPR_MAX_BINS];     // −γ_s log2(e)          projection moments: f_s e^{−γ_s τ} = 2^(pj_a τ + pj_b)
+  float pj_b[EPR_MAX_BINS];     // log2(f_s)
+  float pj_g2[EPR_MAX_BINS];    // γ_s²
+  float pj_g3[EPR_MAX_BINS];    // γ_s³
   float abar;                   // Σ f_s a_s (initial guess, R9)
   float gamma_max;              // max_s γ_s (range test of the projection's polynomial form)
   float fsum_dev;               // Σ_s (float)f_s − 1: rounding of the fp32 fractions, removed from the residual

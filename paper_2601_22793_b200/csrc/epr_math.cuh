@@ -77,6 +77,49 @@ __device__ __forceinline__ float epr_project_increment_mono(float tau, float dT,
   return -epr_log1p_cold(z);
 }
 
+// Converging iterations of the projection (R10) for a compile-time number of lines: |γ_max δ| < 0.01, where the cubic
+// Taylor polynomial of F(δ) = Σ_s I_s expm1(−γ_s δ) − ΔT is exact to (γδ)³/24 < 5e-8 relative.  The per-line constants
+// are read straight from the kernel's parameter bank (L by value, s unrolled): one FFMA + one MUFU.EX2 for I_s and one
+// FFMA per moment, no table loads.  Returns false when the step is too large or the floor could bind: the caller then
+// takes the general routine below.
+template <int NB>
+__device__ __forceinline__ bool epr_project_increment_small(const EprLines& L, float tau, float dT, int newton_iters,
+                                                            float i_min, float& delta_out) {
+  float G0 = 0.f, G1 = 0.f, G2 = 0.f, G3 = 0.f;
+#pragma unroll
+  for (int s = 0; s < NB; ++s) {
+    float p;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(p) : "f"(fmaf(tau, L.pj_a[s], L.pj_b[s])));
+    G0 += p;
+    G1 = fmaf(p, L.gamma[s], G1);
+    G2 = fmaf(p, L.pj_g2[s], G2);
+    G3 = fmaf(p, L.pj_g3[s], G3);
+  }
+  float delta = -__fdividef(dT, G1);
+  if (!(fabsf(delta) * L.gamma_max < 0.01f && G0 + dT >= i_min)) return false;
+  const float c1 = -G1, c2 = 0.5f * G2, c3 = -1.66666667e-1f * G3;
+  for (int it = 0; it < newton_iters; ++it) {
+    const float F = fmaf(fmaf(fmaf(c3, delta, c2), delta, c1), delta, -dT);
+    const float dF = fmaf(fmaf(3.f * c3, delta, 2.f * c2), delta, c1);
+    const float stp = __fdividef(F, dF);
+    delta -= stp;
+    if (fabsf(stp) <= 1e-7f * fabsf(delta) + 1e-12f) break;
+  }
+  delta_out = delta;
+  return true;
+}
+
+// the line counts with an unrolled instance: 8 (BASELINE configs C4, C5), 5 and 10 (the paper's own runs)
+__device__ __forceinline__ bool epr_project_increment_small_nb(const EprLines& L, float tau, float dT, int newton_iters,
+                                                               float i_min, float& delta_out) {
+  switch (L.n_bins) {
+    case 8: return epr_project_increment_small<8>(L, tau, dT, newton_iters, i_min, delta_out);
+    case 5: return epr_project_increment_small<5>(L, tau, dT, newton_iters, i_min, delta_out);
+    case 10: return epr_project_increment_small<10>(L, tau, dT, newton_iters, i_min, delta_out);
+    default: return false;
+  }
+}
+
 // Projection to the single-thickness manifold, Eq. (7) + PAPER.md:233 (R10), as an increment:
 //   given τ and ΔT, find δ with Σ_s I_s(τ) expm1(−γ_s δ) = ΔT, clamped so that Σ_s I_s + ΔT ≥ i_min.
 // Newton from the Jensen bound δ0 = −log1p(ΔT/ΣI)/γ̄_I (monotone; exact for one line).

@@ -202,7 +202,7 @@ def test_retrieve_parity(E, name, n):
         assert rel_l2(got[j], ref) < TOL_PHASE
 
 
-@pytest.mark.parametrize("name", ["C2", "C3"])
+@pytest.mark.parametrize("name", ["C2", "C3", "C4"])
 def test_full_size_periodic_tiling(E, name):
     """Full 2048 x 2048 grid, in the launch configuration bench.py times (batched epr_retrieve, 20 iterations).
     Every operator is periodic on the (nx, ny) grid (R7), so the retrieval of a 4 x 4 tiling of a 512 x 512 detector
@@ -271,6 +271,19 @@ def test_retrieve_unequal_a_lines(E):
     """The implementation must not rely on 'all a_s equal' (a coincidence of C4/C5): db_s constant here."""
     w = make_workload("C4", n=256)
     w.delta_over_beta = np.full(8, 200.0)
+    got, refs = _run_retrieve(E, w, iterations=8)
+    assert rel_l2(got[0], refs[0]) < TOL_PHASE
+
+
+@pytest.mark.parametrize("n_lines", [3, 5, 10])
+def test_retrieve_other_line_counts(E, n_lines):
+    """Line counts other than 8: 5 and 10 lines (the paper's own runs) take the unrolled small-step
+    projection, 3 lines the general routine; the gather tile kernel and the fused residual split serve all of them.
+    The detector image is C4's; only the retrieval's spectral discretisation changes."""
+    w = make_workload("C4", n=256)
+    e = np.linspace(60.0, 140.0, n_lines)
+    wt = np.exp(-0.5 * ((e - 100.0) / 20.0) ** 2)
+    w.energy_keV, w.weight, w.delta_over_beta = e, wt / wt.sum(), 200.0 * e / 100.0
     got, refs = _run_retrieve(E, w, iterations=8)
     assert rel_l2(got[0], refs[0]) < TOL_PHASE
 
