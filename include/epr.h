@@ -31,7 +31,7 @@ typedef struct epr_plan_s* epr_plan_t;
 typedef enum {
   EPR_OK = 0,
   EPR_EINVAL = 1, /* bad argument (NULL pointer, non-positive size / energy / weight / step, batch > max_batch …) */
-  EPR_ESIZE = 2,  /* unsupported grid: nx, ny must be multiples of 4 whose prime factors are in {2,3,5}, ≥ 16 */
+  EPR_ESIZE = 2,  /* unsupported grid: nx, ny must be one of the sizes with a compiled FFT (16 … 4096) */
   EPR_ECUDA = 3,  /* a CUDA runtime call failed; message in epr_last_error */
   EPR_ENOMEM = 4  /* device allocation failed */
 } epr_status;
@@ -98,6 +98,20 @@ epr_status epr_precondition(epr_plan_t plan, int batch, const float* r_bins, flo
  *   may change between calls.  Environment EPR_GRAPH = 0 disables this, 2 applies it to every size. */
 epr_status epr_retrieve(epr_plan_t plan, int batch, const float* d, float* out, int iterations, float step,
                         void* stream);
+
+/* epr_retrieve_oversampled — the loop on an oversampled computational grid          PAPER.md:79 (reading R16)
+ *   "All reconstructions ... were computed on oversampled grids ... the local solver uses an oversampling factor of
+ *   2 (i.e. a pixel size reduced by a factor 2), while the non-local solver uses an oversampling factor of 4."
+ *   `plan` is the plan of the FINE grid: nx = factor · nx_d, ny = factor · ny_d, pixel_m = p / factor (so that shifts
+ *   and max_shift_px count fine pixels).
+ *   d   [batch][ny/factor][nx/factor] in  (detector grid);  out  same shape, out.
+ *   The detector image reaches the fine grid by pixel replication (a detector pixel measures the mean intensity over
+ *   its area), epr_retrieve runs there, and the result (τ, or what opt.output selects) returns as the mean over each
+ *   factor x factor block — the exact left inverse of the replication.  factor ∈ 1..8 must divide nx and ny with
+ *   nx / factor a multiple of 4; opt.init must be 0.  The fine-grid buffers (two planes per projection of the plan's
+ *   work batch) are allocated on the first call and owned by the plan. */
+epr_status epr_retrieve_oversampled(epr_plan_t plan, int factor, int batch, const float* d, float* out, int iterations,
+                                    float step, void* stream);
 
 /* epr_retrieve_host — same, with HOST buffers (pinned for full speed): copies d host→device, runs the loop,
  *   copies the result device→host, in chunks of max_batch projections with copies overlapped with compute;

@@ -326,3 +326,32 @@ def retrieve(d, lines: Lines, solver="local", iterations=10, step=1.0, order=2, 
 def phase(tau, lines: Lines, s=0):
     """φ_s = (db_s/2) ln(I_s/f_s) = −(db_s/2) γ_s τ   Eq. (6) PAPER.md:216 with Eq. (7)."""
     return -(lines.db[s] / 2.0) * lines.gamma[s] * np.asarray(tau, dtype=np.float64)
+
+
+# --------------------------------------------------------------------------------------
+# oversampled computational grid (PAPER.md:79; SURVEY.md §8(f) rank 1; reading R16)
+# --------------------------------------------------------------------------------------
+def upsample(d, m):
+    """Detector image on the grid refined m times ("a pixel size reduced by a factor 2").
+    The paper does not say how the data reach the fine grid; reading R16: each detector pixel measures the mean
+    intensity over its area, so the fine image is constant over it — pixel replication."""
+    d = np.asarray(d, dtype=np.float64)
+    return np.repeat(np.repeat(d, m, axis=0), m, axis=1)
+
+
+def downsample(t, m):
+    """Back to the detector grid: mean over each m x m block of fine pixels (R16), the exact left inverse of
+    `upsample` and mean-preserving."""
+    t = np.asarray(t, dtype=np.float64)
+    ny, nx = t.shape
+    return t.reshape(ny // m, m, nx // m, m).mean(axis=(1, 3))
+
+
+def retrieve_oversampled(d, lines_fine: Lines, m, solver="local", iterations=10, step=1.0, order=2, wkb1=True,
+                         symbol=0, S=16.0, i_min=1e-6):
+    """The correction loop on the m-times oversampled grid (factor 2 for the local solver, 4 for the
+    non-local one): up-sample d, run `retrieve` with the per-line scalars of the FINE pixel (`lines_fine` =
+    derive_lines(pixel/m, ...), so that shifts are counted in fine pixels; S is in fine pixels too),
+    down-sample τ.  m = 1 is `retrieve`."""
+    tau = retrieve(upsample(d, m), lines_fine, solver, iterations, step, order, wkb1, symbol, S, i_min)
+    return downsample(tau, m)

@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
 EXPORTS = ["epr_default_options", "epr_plan", "epr_forward", "epr_adjoint", "epr_transport", "epr_precondition",
-           "epr_retrieve", "epr_retrieve_host", "epr_plan_lines", "epr_launch_count", "epr_destroy",
+           "epr_retrieve", "epr_retrieve_oversampled", "epr_retrieve_host", "epr_plan_lines", "epr_launch_count", "epr_destroy",
            "epr_last_error", "epr_version", "epr_profile_enable", "epr_profile_read"]
 
 
@@ -52,6 +52,7 @@ def load_library():
     lib.epr_transport.argtypes = [vp, ci, vp, vp, vp]
     lib.epr_precondition.argtypes = [vp, ci, vp, vp, vp]
     lib.epr_retrieve.argtypes = [vp, ci, vp, vp, ci, cf, vp]
+    lib.epr_retrieve_oversampled.argtypes = [vp, ci, ci, vp, vp, ci, cf, vp]
     lib.epr_retrieve_host.argtypes = [vp, ci, vp, vp, ci, cf]
     lib.epr_plan_lines.argtypes = [vp, C.POINTER(cd), C.POINTER(cd), C.POINTER(cd), C.POINTER(cd)]
     lib.epr_launch_count.argtypes = [vp]
@@ -65,7 +66,7 @@ def load_library():
     lib.epr_last_error.restype = C.c_char_p
     lib.epr_version.restype = C.c_char_p
     for name in ("epr_plan", "epr_forward", "epr_adjoint", "epr_transport", "epr_precondition", "epr_retrieve",
-                 "epr_retrieve_host", "epr_plan_lines", "epr_destroy"):
+                 "epr_retrieve_oversampled", "epr_retrieve_host", "epr_plan_lines", "epr_destroy"):
         getattr(lib, name).restype = ci
     _LIB = lib
     return lib
@@ -196,6 +197,17 @@ def epr_retrieve(plan, d, out, iterations, step):
     sh = (b, plan.ny, plan.nx)
     plan._check(load_library().epr_retrieve(plan._h, b, _dev(d, sh, "d"), _dev(out, sh, "out"), int(iterations),
                                             float(step), _stream()))
+
+
+def epr_retrieve_oversampled(plan, factor, d, out, iterations, step):
+    """`plan` is the FINE grid's plan; d, out are [batch][ny / factor][nx / factor] (include/epr.h)."""
+    b = d.shape[0]
+    factor = int(factor)
+    if factor < 1 or plan.ny % factor or plan.nx % factor:
+        raise ValueError("factor must divide the plan's grid")
+    sh = (b, plan.ny // factor, plan.nx // factor)
+    plan._check(load_library().epr_retrieve_oversampled(plan._h, factor, b, _dev(d, sh, "d"), _dev(out, sh, "out"),
+                                                        int(iterations), float(step), _stream()))
 
 
 def epr_retrieve_host(plan, d_host, out_host, iterations, step):

@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libepr.so")
-FFT_GROUPS = 6
+FFT_GROUPS = 7
 # (source, object stem, extra flags)
 UNITS = [("epr_api.cu", "epr_api", []), ("epr_kernels.cu", "epr_kernels", []), ("epr_fftd.cu", "epr_fftd", [])] + \
         [("epr_fftk.cu", f"epr_fftk_g{g}", [f"-DEPR_FFT_GROUP={g}"]) for g in range(FFT_GROUPS)]

@@ -24,9 +24,9 @@ static const double HC_KEV_M = 1.2398419843e-9;
     if (e_ != cudaSuccess) FAIL(p, EPR_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
   } while (0)
 // Kernel families, for launch counting and the optional per-kernel CUDA-event timing (epr_profile_*).
-enum { K_FWD_LOCAL = 0, K_SPLAT, K_RESIDUAL, K_GATHER, K_ROWS_R2C, K_COLS, K_ROWS_C2R, K_PRED_OUT, K_OUTPUT, K_COUNT };
+enum { K_FWD_LOCAL = 0, K_SPLAT, K_RESIDUAL, K_GATHER, K_ROWS_R2C, K_COLS, K_ROWS_C2R, K_PRED_OUT, K_OUTPUT, K_RESAMPLE, K_COUNT };
 static const char* const K_NAMES[K_COUNT] = {"k_forward_local", "k_splat", "k_residual", "k_gather", "k_rows_r2c",
-                                              "k_cols", "k_rows_c2r", "k_pred_out", "k_output"};
+                                              "k_cols", "k_rows_c2r", "k_pred_out", "k_output", "k_resample"};
 struct EprProf {
   struct Rec { int tag; cudaEvent_t a, b; };
   std::vector<Rec> recs;
@@ -293,7 +293,7 @@ extern "C" epr_status epr_destroy(epr_plan_t p) {
   cudaDeviceSynchronize();
   cudaFree(p->tw_row); cudaFree(p->tw_r2c); cudaFree(p->tw_col); cudaFree(p->tw_col_inv); cudaFree(p->lam_x); cudaFree(p->lam_y);
   cudaFree(p->tau); cudaFree(p->pred); cudaFree(p->res); cudaFree(p->res2); cudaFree(p->spec); cudaFree(p->spec_sum);
-  cudaFree(p->raymap); cudaFree(p->gmax);
+  cudaFree(p->raymap); cudaFree(p->gmax); cudaFree(p->os_d); cudaFree(p->os_out);
   if (p->graph_exec) cudaGraphExecDestroy(p->graph_exec);
   if (p->prof) { epr_profile_read(p, 0, NULL, NULL, NULL, 1); delete (EprProf*)p->prof; }
   for (int i = 0; i < 2; ++i) { cudaFree(p->stage_in[i]); cudaFree(p->stage_out[i]); }
@@ -435,6 +435,33 @@ static epr_status retrieve_device(epr_plan_t p, int batch, const float* d, float
     epr_status st = retrieve_chunk(p, nb, d + (size_t)b0 * plane, tau, iterations, step, cs);
     if (st != EPR_OK) return st;
     if (p->opt.output != 0) KL(p, K_OUTPUT, cs, epr_launch_output(p, nb, tau, o, cs));
+  }
+  return EPR_OK;
+}
+
+// The loop on an oversampled grid (reading R16): the plan is the FINE grid's.
+extern "C" epr_status epr_retrieve_oversampled(epr_plan_t p, int factor, int batch, const float* d, float* out,
+                                               int iterations, float step, void* stream) {
+  epr_status st = check_call(p, batch);
+  if (st != EPR_OK) return st;
+  if (!d || !out) FAIL(p, EPR_EINVAL, "epr_retrieve_oversampled: NULL pointer");
+  if (iterations < 0 || !(step > 0.f)) FAIL(p, EPR_EINVAL, "epr_retrieve_oversampled: iterations must be >= 0 and step > 0");
+  if (factor < 1 || factor > 8 || p->nx % (4 * factor) != 0 || p->ny % factor != 0)
+    FAIL(p, EPR_EINVAL, "epr_retrieve_oversampled: factor %d must be in 1..8 and divide the plan's grid %d x %d (nx / factor a multiple of 4)", factor, p->nx, p->ny);
+  if (p->opt.init != 0) FAIL(p, EPR_EINVAL, "epr_retrieve_oversampled: opt.init = 1 (caller-supplied start) is not supported");
+  cudaStream_t cs = (cudaStream_t)stream;
+  const size_t plane = (size_t)p->nx * p->ny, cplane = plane / ((size_t)factor * factor);
+  if (!p->os_d) {
+    cudaError_t e = cudaMalloc((void**)&p->os_d, (size_t)p->work_batch * plane * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&p->os_out, (size_t)p->work_batch * plane * sizeof(float));
+    if (e != cudaSuccess) FAIL(p, e == cudaErrorMemoryAllocation ? EPR_ENOMEM : EPR_ECUDA, "oversampling buffers: %s", cudaGetErrorString(e));
+  }
+  for (int b0 = 0; b0 < batch; b0 += p->work_batch) {
+    const int nb = (batch - b0 < p->work_batch) ? batch - b0 : p->work_batch;
+    KL(p, K_RESAMPLE, cs, epr_launch_upsample(p, nb, factor, d + (size_t)b0 * cplane, p->os_d, cs));
+    st = retrieve_device(p, nb, p->os_d, p->os_out, iterations, step, cs);
+    if (st != EPR_OK) return st;
+    KL(p, K_RESAMPLE, cs, epr_launch_downsample(p, nb, factor, p->os_out, out + (size_t)b0 * cplane, cs));
   }
   return EPR_OK;
 }

@@ -5,7 +5,7 @@
 #ifdef EPR_FFT_DEV          /* developer build: only group 0 (2048, 16, 32) is compiled */
 #define EPR_FFT_GROUPS(G) G(0)
 #else
-#define EPR_FFT_GROUPS(G) G(0) G(1) G(2) G(3) G(4) G(5)
+#define EPR_FFT_GROUPS(G) G(0) G(1) G(2) G(3) G(4) G(5) G(6)
 #endif
 
 #define G(g)                                                                                                          \

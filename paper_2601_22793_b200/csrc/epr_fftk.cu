@@ -381,7 +381,7 @@ template <int N> struct ColTmaCfg {
 };
 
 template <int N, bool SUM>
-__global__ void __launch_bounds__(ColTmaCfg<N>::NT, SUM ? 1 : 2)
+__global__ void __launch_bounds__(ColTmaCfg<N>::NT, (SUM || ColTmaCfg<N>::NT > 512) ? 1 : 2)
 k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_out, EprLines L, int M,
            int mode, float scale, const float* __restrict__ lam_x, const float* __restrict__ lam_y,
            const float2* __restrict__ tw, const float2* __restrict__ tw_inv) {
@@ -494,7 +494,7 @@ k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
 // The instantiations are split into EPR_FFT_NGROUPS translation units (this file compiled once per group with
 // -DEPR_FFT_GROUP=g, in parallel: see build.py); epr_fftd.cu routes a size to the group that holds it.
 #ifndef EPR_FFT_GROUP
-#error "compile with -DEPR_FFT_GROUP=<0..5> (paper_2601_22793_b200/build.py does)"
+#error "compile with -DEPR_FFT_GROUP=<0..6> (paper_2601_22793_b200/build.py does)"
 #endif
 #if EPR_FFT_GROUP == 0
 #define EPR_FFT_SIZES(X) X(2048) X(16) X(32)
@@ -506,8 +506,10 @@ k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
 #define EPR_FFT_SIZES(X) X(1024) X(80) X(96)
 #elif EPR_FFT_GROUP == 4
 #define EPR_FFT_SIZES(X) X(512) X(320) X(128)
-#else
+#elif EPR_FFT_GROUP == 5
 #define EPR_FFT_SIZES(X) X(256) X(160)
+#else
+#define EPR_FFT_SIZES(X) X(4096)
 #endif
 #define EPR_CAT2(a, b) a##b
 #define EPR_CAT(a, b) EPR_CAT2(a, b)
@@ -589,10 +591,12 @@ static bool launch_cols_tma(const epr_plan_s* p, int oplanes, int mode, const fl
     using C = ColTmaCfg<N>;
     const int M = p->nx / 2;
     if (!p->tma_ok || M % C::W != 0 || spec != p->spec || (out != p->spec && out != p->spec_sum)) return false;
+    if (mode == 1 && p->n_bins > 1 && C::smem(true) > 227 * 1024) return false;     // two tiles of 4096 rows do not fit an SM
     static bool attr = false;
     if (!attr) {
       cudaFuncSetAttribute(k_cols_tma<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem(false));
-      cudaFuncSetAttribute(k_cols_tma<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem(true));
+      if (C::smem(true) <= 227 * 1024)
+        cudaFuncSetAttribute(k_cols_tma<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem(true));
       attr = true;
     }
     const CUtensorMap& mo = (out == p->spec) ? p->map_spec : p->map_spec_sum;

@@ -55,6 +55,8 @@ struct epr_plan_s {
   CUtensorMap map_spec_sum;
   int tma_ok;                  // descriptors valid (power-of-two ny ≥ 256, nx % 8 == 0)
   float* gmax;                 // [work_batch][ny/16][nx/16] block maxima of |D⁰τ| (non-local: k_grad_blockmax)
+  float* os_d;                 // [work_batch][ny][nx] up-sampled detector images (lazy, epr_retrieve_oversampled)
+  float* os_out;               // [work_batch][ny][nx] fine-grid result before down-sampling (lazy)
   float2* raymap;              // [work_batch][n_bins][ny][nx] stored u_s (lazy, epr_forward non-local)
   int raymap_batch;            // batch of the stored map (0 = none)
   // host staging for epr_retrieve_host
@@ -104,4 +106,7 @@ cudaError_t epr_launch_cols(const epr_plan_s* p, int planes, int mode, const flo
 // epilogue 0: write q; 1: τ update (Newton projection) with step; init0: treat τ as 0 (initial guess)
 cudaError_t epr_launch_rows_c2r(const epr_plan_s* p, int planes, const float2* spec, int epilogue, float step,
                                 int tau_is_zero, float* q_or_tau, cudaStream_t st);
+// oversampled grid (R16): the plan's (nx, ny) is the FINE grid; coarse planes are (ny/m) x (nx/m)
+cudaError_t epr_launch_upsample(const epr_plan_s* p, int batch, int m, const float* coarse, float* fine, cudaStream_t st);
+cudaError_t epr_launch_downsample(const epr_plan_s* p, int batch, int m, const float* fine, float* coarse, cudaStream_t st);
 cudaError_t epr_launch_output(const epr_plan_s* p, int batch, const float* tau, float* out, cudaStream_t st);

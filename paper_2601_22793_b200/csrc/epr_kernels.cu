@@ -1039,3 +1039,50 @@ cudaError_t epr_launch_output(const epr_plan_s* p, int batch, const float* tau, 
   k_output<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p->lines, n, p->opt.output, coef, tau, out);
   return cudaGetLastError();
 }
+
+// =====================================================================================================
+// Oversampled computational grid (reading R16): the loop runs on a grid refined m times; the detector
+// image reaches it by pixel replication (a detector pixel measures the mean intensity over its area) and the result
+// returns by the mean over each m x m block — the exact left inverse.  Both kernels are plain HBM streams.
+// =====================================================================================================
+// fine[b][Y][X] = coarse[b][Y / m][X / m];  one thread = 4 consecutive fine pixels (nx_f % 4 == 0)
+__global__ void __launch_bounds__(256) k_upsample(int nx_f, int ny_f, int m, const float* __restrict__ coarse,
+                                                  float* __restrict__ fine) {
+  const int X = 4 * (blockIdx.x * 256 + threadIdx.x), Y = blockIdx.y, b = blockIdx.z;
+  if (X >= nx_f) return;
+  const int nx_c = nx_f / m, ny_c = ny_f / m;
+  const float* row = coarse + ((size_t)b * ny_c + Y / m) * nx_c;
+  float4 o;
+  if (m == 2) { const float2 v = __ldg(reinterpret_cast<const float2*>(row + X / 2)); o = make_float4(v.x, v.x, v.y, v.y); }
+  else if (m % 4 == 0) { const float v = __ldg(row + X / m); o = make_float4(v, v, v, v); }
+  else o = make_float4(__ldg(row + X / m), __ldg(row + (X + 1) / m), __ldg(row + (X + 2) / m), __ldg(row + (X + 3) / m));
+  *reinterpret_cast<float4*>(fine + ((size_t)b * ny_f + Y) * nx_f + X) = o;
+}
+
+// coarse[b][y][x] = mean of fine[b][m y + j][m x + i], i, j < m;  one thread = one coarse pixel
+__global__ void __launch_bounds__(256) k_downsample(int nx_c, int ny_c, int m, const float* __restrict__ fine,
+                                                    float* __restrict__ coarse) {
+  const int x = blockIdx.x * 256 + threadIdx.x, y = blockIdx.y, b = blockIdx.z;
+  if (x >= nx_c) return;
+  const int nx_f = nx_c * m;
+  const float* src = fine + ((size_t)b * ny_c * m + (size_t)y * m) * nx_f + (size_t)x * m;
+  float acc = 0.f;
+  for (int j = 0; j < m; ++j) {
+    float r = 0.f;
+    for (int i = 0; i < m; ++i) r += __ldg(src + (size_t)j * nx_f + i);
+    acc += r;
+  }
+  coarse[((size_t)b * ny_c + y) * nx_c + x] = acc / (float)(m * m);
+}
+
+cudaError_t epr_launch_upsample(const epr_plan_s* p, int batch, int m, const float* coarse, float* fine, cudaStream_t st) {
+  dim3 grid((p->nx / 4 + 255) / 256, p->ny, batch);
+  k_upsample<<<grid, 256, 0, st>>>(p->nx, p->ny, m, coarse, fine);
+  return cudaGetLastError();
+}
+
+cudaError_t epr_launch_downsample(const epr_plan_s* p, int batch, int m, const float* fine, float* coarse, cudaStream_t st) {
+  dim3 grid((p->nx / m + 255) / 256, p->ny / m, batch);
+  k_downsample<<<grid, 256, 0, st>>>(p->nx / m, p->ny / m, m, fine, coarse);
+  return cudaGetLastError();
+}

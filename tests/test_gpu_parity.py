@@ -288,6 +288,42 @@ def test_retrieve_other_line_counts(E, n_lines):
     assert rel_l2(got[0], refs[0]) < TOL_PHASE
 
 
+@pytest.mark.parametrize("name,n,m,S", [("C1", None, 2, 16.0), ("C2", 256, 2, 16.0), ("C3", 128, 4, 28.0), ("C4", 128, 2, 24.0)])
+def test_retrieve_oversampled_parity(E, name, n, m, S):
+    """PAPER.md:79 (reading R16): the loop on the grid refined m times (2 for the local solver, 4 for the non-local
+    one), plan built for the fine pixel; replication in, block mean out.  S counts fine pixels."""
+    import torch
+    w = make_workload(name, n=n, batch=2)
+    plan = E.epr_plan(m * w.nx, m * w.ny, w.pixel_m / m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
+                      max_batch=2, max_shift_px=S)
+    d = _dev(w.d)
+    out = torch.empty_like(d)
+    E.epr_retrieve_oversampled(plan, m, d, out, w.iterations, w.step)
+    got = out.cpu().numpy()
+    plan.destroy()
+    lines = O.derive_lines(w.pixel_m / m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta)
+    for j in range(2):
+        ref = O.retrieve_oversampled(w.d[j].astype(np.float64), lines, m, w.solver, w.iterations, w.step, S=S)
+        assert got[j].shape == ref.shape == (w.ny, w.nx)
+        assert rel_l2(got[j], ref) < TOL_PHASE
+
+
+def test_resampling_round_trip_is_exact(E):
+    """Zero iterations of a plan whose filter is the identity (L -> 0): out = −ln(block mean … ) is not exact, so the
+    round trip is checked on the intensity output instead: output = 2 returns T = e^{−τ}; with a vanishing propagation
+    distance the Paganin solve is the identity and mean(replicate(d)) = d up to the fp32 rounding of exp/log."""
+    import torch
+    rng = np.random.default_rng(5)
+    dn = (1.0 + 0.2 * rng.uniform(-1, 1, size=(2, 40, 64))).astype(np.float32)      # fine grids 80 x 128, 160 x 256
+    for m in (2, 4):
+        plan = E.epr_plan(m * 64, m * 40, 6.5e-6 / m, 1e-9, [100.0], [1.0], [1000.0], "local", max_batch=2, output=2)
+        d = _dev(dn)
+        out = torch.empty_like(d)
+        E.epr_retrieve_oversampled(plan, m, d, out, 0, 1.0)
+        plan.destroy()
+        assert np.max(np.abs(out.cpu().numpy() - dn)) < 5e-7
+
+
 def test_retrieve_outputs_and_host_path(E):
     import torch
     w = make_workload("C1")
