@@ -42,6 +42,7 @@ def kernel_bytes_per_px(name, nb, solver):
         "k_cols": 4 * nb + 4,                   # R nb spectra, W summed spectrum
         "k_rows_c2r": 12,                       # R spectrum 4, R tau 4, W tau 4
         "k_output": 8,
+        "k_resample": 8,                        # replaced per call by 4 + 4/m² (see main)
         "k_pred_out": 4 * nb + 4,
     }[name]
 
@@ -132,12 +133,20 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_time_one(w, j=0):
+def fine_shift_clamp(w, m):
+    """S in pixels of the grid refined m times (the library accepts at most 30)."""
+    return float(min(30.0, m * w.max_shift_px))
+
+
+def oracle_time_one(w, j=0, m=1):
     """The oracle as it stands, one projection of the workload, on the host cores (numpy: 1 thread)."""
     from oracle import epr_oracle as O
-    lines = O.derive_lines(w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta)
+    lines = O.derive_lines(w.pixel_m / m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta)
     t0 = time.perf_counter()
-    O.retrieve(w.d[j].astype(np.float64), lines, w.solver, w.iterations, w.step, S=w.max_shift_px)
+    if m == 1:
+        O.retrieve(w.d[j].astype(np.float64), lines, w.solver, w.iterations, w.step, S=w.max_shift_px)
+    else:
+        O.retrieve_oversampled(w.d[j].astype(np.float64), lines, m, w.solver, w.iterations, w.step, S=fine_shift_clamp(w, m))
     return time.perf_counter() - t0
 
 
@@ -147,8 +156,8 @@ def run_reference(args, rank):
     from epr_inputs import make_workload
     w = make_workload(args.config, batch=1, distinct=1)
     for _ in range(args.warmup):
-        oracle_time_one(w)
-    t = [oracle_time_one(w) for _ in range(args.steps)]
+        oracle_time_one(w, m=args.oversample)
+    t = [oracle_time_one(w, m=args.oversample) for _ in range(args.steps)]
     tot = float(np.sum(t))
     val = args.steps / tot
     sample = f"1 projection {w.ny}x{w.nx} per step, all {w.iterations} iterations, numpy fp64 oracle"
@@ -156,7 +165,8 @@ def run_reference(args, rank):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{args.config}: {w.ny}x{w.nx}, {w.n_bins} line(s), {w.solver}, {w.iterations} iterations"},
+        "config": {"workload": f"{args.config}: {w.ny}x{w.nx}, {w.n_bins} line(s), {w.solver}, {w.iterations} iterations"
+                               + (f", oversampling {args.oversample}" if args.oversample > 1 else "")},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
@@ -172,6 +182,8 @@ def main():
     ap.add_argument("--distinct", type=int, default=2, help="distinct simulated projections (rest: new noise only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--oversample", type=int, default=1,
+                    help="run the loop on the grid refined this many times (PAPER.md:79; epr_retrieve_oversampled)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -201,15 +213,28 @@ def main():
         w.d = np.ascontiguousarray(w.d[rng.permutation(B)])
     plane = w.nx * w.ny
     nb = w.n_bins
-    plan = epr.epr_plan(w.nx, w.ny, w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
-                        max_batch=B, max_shift_px=w.max_shift_px)
+    m = args.oversample
+    plan = epr.epr_plan(m * w.nx, m * w.ny, w.pixel_m / m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
+                        max_batch=B, max_shift_px=w.max_shift_px if m == 1 else fine_shift_clamp(w, m))
     d_host = torch.from_numpy(w.d).pin_memory()
     out_host = torch.empty_like(d_host).pin_memory()
     d = d_host.cuda()
     out = torch.empty_like(d)
 
     def step():
-        epr.epr_retrieve(plan, d, out, w.iterations, w.step)
+        if m == 1:
+            epr.epr_retrieve(plan, d, out, w.iterations, w.step)
+        else:
+            epr.epr_retrieve_oversampled(plan, m, d, out, w.iterations, w.step)
+
+    def step_host():
+        if m == 1:
+            epr.epr_retrieve_host(plan, d_host, out_host, w.iterations, w.step)
+        else:                                       # no chunked host variant of the oversampled call: plain copies
+            d.copy_(d_host, non_blocking=True)
+            step()
+            out_host.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
 
     def barrier():
         torch.cuda.synchronize()
@@ -243,11 +268,11 @@ def main():
     value = world * B * args.steps / (ms * 1e-3)
 
     # ---- end to end through the public host API: pinned host buffers, H2D + loop + D2H inside the timed region
-    epr.epr_retrieve_host(plan, d_host, out_host, w.iterations, w.step)
+    step_host()
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        epr.epr_retrieve_host(plan, d_host, out_host, w.iterations, w.step)
+        step_host()
     e2e_s = time.perf_counter() - t0
     e2e_s = max_over_ranks(e2e_s, torch.device("cuda", local))
     e2e = world * B * args.steps / e2e_s
@@ -266,10 +291,12 @@ def main():
             bpp = kernel_bytes_per_px(name, nb, w.solver)
             # px per launch: every launch covers the whole batch; r2c covers nb planes per projection in the loop
             launches_per_step = cnt / args.steps
-            px = B * plane
+            px = B * plane * m * m                  # pixels of the computational grid
             if name == "k_rows_r2c":
                 # (iterations launches of nb planes + 1 init launch of 1 plane) per step
-                px = B * plane * (w.iterations * nb + 1) / (w.iterations + 1)
+                px = px * (w.iterations * nb + 1) / (w.iterations + 1)
+            if name == "k_resample":                # replication: R 4/m² + W 4; block mean: R 4 + W 4/m²; one launch each
+                bpp = 4.0 + 4.0 / (m * m)
             avg_ms = tot_ms / cnt
             gbs = bpp * px / (avg_ms * 1e-3) / 1e9
             per_kernel.append({"kernel": name, "launches_per_step": launches_per_step, "avg_ms": avg_ms,
@@ -290,7 +317,8 @@ def main():
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"{args.config}: {w.ny}x{w.nx}, {nb} line(s), {w.solver} solver, "
-                                   f"{w.iterations} iterations, step {w.step}",
+                                   f"{w.iterations} iterations, step {w.step}"
+                                   + (f", oversampling {m} (computational grid {m * w.ny}x{m * w.nx})" if m > 1 else ""),
                        "batch_per_gpu": B, "work_batch": None,
                        "l2": (f"inputs {in_bytes / 1e6:.0f} MB per step > 2 x 126 MB L2: no flush needed" if flush is None else
                               f"inputs {in_bytes / 1e6:.0f} MB per step: L2 flushed (256 MB overwrite) between timed steps"),
@@ -301,7 +329,7 @@ def main():
             "roofline": roofline,
         }
         if not args.no_cpu_baseline:
-            t1 = oracle_time_one(w)
+            t1 = oracle_time_one(w, m=m)
             result["cpu_baseline"] = {"value": 1.0 / t1, "unit": UNIT, "cores": 1, "kind": "oracle",
                                       "sample": f"1 of the {B} projections ({w.ny}x{w.nx}, all {w.iterations} "
                                                 f"iterations) in {t1:.1f} s, numpy fp64, host has {os.cpu_count()} cores"}
