@@ -2,7 +2,7 @@
  *
  * One library, libepr.so, hand-written CUDA for sm_100a.  It implements the batched per-projection
  * iterative correction loop of arxiv 2601.22793 (§4.4) and the three operators of one
- * iteration.  No CPU fallback, no other backend.  Notation follows the paper; the readings R1..R15 of the
+ * iteration.  No CPU fallback, no other backend.  Notation follows the paper; the readings R1..R16 of the
  * points the paper leaves open are listed in DESIGN.md.
  *
  * Conventions
