@@ -399,42 +399,42 @@ cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float
 // (periodic; nx, ny are multiples of 16).  With u_s = c_s D⁰τ (Eq. (2)) it bounds the ray shifts of a
 // block, which tells the splat how wide a ring of foreign sources can reach a detector tile and the gather how wide a
 // halo of the residual a tile needs — before either loads anything.  One pass over τ (4 B/px).
-// CTA: 128 columns x 16 rows = 8 blocks; thread: one strip of 4 pixels in rows ry and ry + 8.
+// A warp owns 128 columns x 16 rows = 8 blocks and walks down the rows with the column's three current rows in registers
+// (18 row loads of 512 B for 16 rows; x-neighbours by shuffles, the two strip edges by one scalar load each);
+// CTA = 8 warps stacked in y.
 // =====================================================================================================
 __global__ void __launch_bounds__(256) k_grad_blockmax(int nx, int ny, const float* __restrict__ tau, float* __restrict__ gmax) {
-  __shared__ unsigned s_m[8];
-  const int tid = threadIdx.x, lane = tid & 31;
-  if (tid < 8) s_m[tid] = 0u;
-  __syncthreads();
-  const int x = blockIdx.x * 128 + 4 * lane;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int x = blockIdx.x * 128 + 4 * lane, by = blockIdx.y * 8 + warp;       // block row
+  if (by * 16 >= ny) return;
+  const bool xin = x < nx;
+  const int xs = xin ? x : 0;
+  const float* tb = tau + (size_t)blockIdx.z * nx * ny;
+  const int xm = xs == 0 ? nx - 1 : xs - 1, xp = xs + 4 >= nx ? 0 : xs + 4;
+  const int y0 = by * 16;
+  auto row4 = [&](int y) { return __ldg(reinterpret_cast<const float4*>(tb + (size_t)(y < 0 ? y + ny : (y >= ny ? y - ny : y)) * nx + xs)); };
+  float4 n = row4(y0 - 1), c = row4(y0);
   float m = 0.f;
-  if (x < nx) {
-    const float* tb = tau + (size_t)blockIdx.z * nx * ny;
-    const int xm = x == 0 ? nx - 1 : x - 1, xp = x + 4 == nx ? 0 : x + 4;
-#pragma unroll
-    for (int k = 0; k < 2; ++k) {
-      const int y = blockIdx.y * 16 + (tid >> 5) + 8 * k;
-      const int ym = y == 0 ? ny - 1 : y - 1, yp = y + 1 == ny ? 0 : y + 1;
-      const float* row = tb + (size_t)y * nx;
-      const float4 c = __ldg(reinterpret_cast<const float4*>(row + x));
-      const float4 n = __ldg(reinterpret_cast<const float4*>(tb + (size_t)ym * nx + x));
-      const float4 s4 = __ldg(reinterpret_cast<const float4*>(tb + (size_t)yp * nx + x));
-      const float l = __ldg(row + xm), r = __ldg(row + xp);
-      m = fmaxf(m, fmaxf(fmaxf(fabsf(c.y - l), fabsf(c.z - c.x)), fmaxf(fabsf(c.w - c.y), fabsf(r - c.z))));
-      m = fmaxf(m, fmaxf(fmaxf(fabsf(s4.x - n.x), fabsf(s4.y - n.y)), fmaxf(fabsf(s4.z - n.z), fabsf(s4.w - n.w))));
-    }
+#pragma unroll 4
+  for (int r = 0; r < 16; ++r) {
+    const float4 s4 = row4(y0 + r + 1);
+    float l = __shfl_up_sync(0xffffffffu, c.w, 1), rr = __shfl_down_sync(0xffffffffu, c.x, 1);
+    const float* row = tb + (size_t)(y0 + r) * nx;
+    if (lane == 0 || x == 0) l = __ldg(row + xm);
+    if (lane == 31 || x + 4 >= nx) rr = __ldg(row + xp);
+    m = fmaxf(m, fmaxf(fmaxf(fabsf(c.y - l), fabsf(c.z - c.x)), fmaxf(fabsf(c.w - c.y), fabsf(rr - c.z))));
+    m = fmaxf(m, fmaxf(fmaxf(fabsf(s4.x - n.x), fabsf(s4.y - n.y)), fmaxf(fabsf(s4.z - n.z), fabsf(s4.w - n.w))));
+    n = c; c = s4;
   }
+  if (!xin) m = 0.f;
   m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
   m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
-  if ((lane & 3) == 0) atomicMax(&s_m[lane >> 2], __float_as_uint(m));
-  __syncthreads();
   const int nbx = nx >> 4;
-  if (tid < 8 && blockIdx.x * 8 + tid < nbx)
-    gmax[((size_t)blockIdx.z * (ny >> 4) + blockIdx.y) * nbx + blockIdx.x * 8 + tid] = __uint_as_float(s_m[tid]);
+  if ((lane & 3) == 0 && xin) gmax[((size_t)blockIdx.z * (ny >> 4) + by) * nbx + (x >> 4)] = m;
 }
 
 cudaError_t epr_launch_grad_blockmax(const epr_plan_s* p, int batch, const float* tau, cudaStream_t st) {
-  dim3 grid((p->nx + 127) / 128, p->ny / 16, batch);
+  dim3 grid((p->nx + 127) / 128, (p->ny / 16 + 7) / 8, batch);
   k_grad_blockmax<<<grid, 256, 0, st>>>(p->nx, p->ny, tau, p->gmax);
   return cudaGetLastError();
 }
@@ -516,6 +516,20 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       cp_async16(s_tau + ly * TP + 4 * cx, tb + (unsigned)gy * nx + gx);
     }
     cp_async_commit();
+  }
+  // one line with the residual fused (out_mode 2): the d values of this thread's flush groups are requested now, so that
+  // the flush does not wait on them (the load used to be 21 % of the kernel's stall samples)
+  constexpr int NFL = ST_W * ST_H / 4 / ST_NT;         // flush groups (4 pixels) per thread
+  float4 dpre[NFL];
+  if (out_mode == 2) {
+#pragma unroll
+    for (int k = 0; k < NFL; ++k) {
+      const int i = tid + k * ST_NT;
+      const int ty = i / (ST_W / 4), tx = 4 * (i - ty * (ST_W / 4));
+      dpre[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (x0 + tx < nx && y0 + ty < ny)
+        dpre[k] = __ldg(reinterpret_cast<const float4*>(d + (size_t)b * plane + (unsigned)(y0 + ty) * nx + (x0 + tx)));
+    }
   }
   for (int s = 0; s < L.n_bins; ++s) {
     const size_t pl = ((size_t)b * L.n_bins + s) * plane;
@@ -641,7 +655,9 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
     __syncthreads();
     // flush the tile: 4 pixels per thread per pass
     const float sc = 1.0f / (float)EPR_FIX_ONE, corr = L.fixCorr[s];
-    for (int i = tid; i < ST_W * ST_H / 4; i += ST_NT) {
+#pragma unroll
+    for (int k = 0; k < NFL; ++k) {
+      const int i = tid + k * ST_NT;
       const int ty = i / (ST_W / 4), tx = 4 * (i - ty * (ST_W / 4));
       const int gx = x0 + tx, gy = y0 + ty;
       if (gx >= nx || gy >= ny) continue;
@@ -654,7 +670,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
         o = make_float4(fmaf((float)((int)v.x - Fi), sc, corr), fmaf((float)((int)v.y - Fi), sc, corr),
                         fmaf((float)((int)v.z - Fi), sc, corr), fmaf((float)((int)v.w - Fi), sc, corr));
         if (out_mode == 2) {
-          const float4 dd = __ldg(reinterpret_cast<const float4*>(d + (size_t)b * plane + g));
+          const float4 dd = dpre[k];
           const float off = 1.f + L.fsum_dev;
           o = make_float4((dd.x - off) - o.x, (dd.y - off) - o.y, (dd.z - off) - o.z, (dd.w - off) - o.w);
         }
