@@ -105,7 +105,7 @@ static std::vector<float> lambda_table(int n, int count, int symbol) {
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time dependency on libcuda)
-static bool make_spec_map(CUtensorMap* map, void* base, int nx, size_t rows) {
+static bool make_spec_map(CUtensorMap* map, void* base, int nx, size_t rows, int box_rows) {
   typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -121,7 +121,7 @@ static bool make_spec_map(CUtensorMap* map, void* base, int nx, size_t rows) {
   if (rows > 0xffffffffull) return false;
   const cuuint64_t dims[2] = {(cuuint64_t)nx, (cuuint64_t)rows};
   const cuuint64_t strides[1] = {(cuuint64_t)nx * sizeof(float)};
-  const cuuint32_t box[2] = {8, 256};
+  const cuuint32_t box[2] = {8, (cuuint32_t)box_rows};
   const cuuint32_t estr[2] = {1, 1};
   return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
@@ -232,9 +232,12 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
   // TMA descriptors for the column kernel (power-of-two ny ≥ 256, whole 4-column tiles): the spectra seen as
   // [rows = planes·ny][nx floats], box = 8 floats (4 complex columns) x 256 rows, no swizzle.
   p->tma_ok = 0;
-  if (ny >= 256 && (ny & (ny - 1)) == 0 && nx % 8 == 0) {
-    if (make_spec_map(&p->map_spec, p->spec, nx, (size_t)wb * n_bins * ny) &&
-        make_spec_map(&p->map_spec_sum, p->spec_sum, nx, (size_t)wb * ny))
+  if (ny >= 256 && nx % 8 == 0) {
+    int br = 256;
+    while (ny % br != 0) --br;                       // 256 for powers of two, 240 for 2160, 160 for 320
+    p->tma_box_rows = br;
+    if (br >= 64 && make_spec_map(&p->map_spec, p->spec, nx, (size_t)wb * n_bins * ny, br) &&
+        make_spec_map(&p->map_spec_sum, p->spec_sum, nx, (size_t)wb * ny, br))
       p->tma_ok = 1;
   }
   return EPR_OK;

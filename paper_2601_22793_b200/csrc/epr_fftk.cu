@@ -490,6 +490,146 @@ k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
   }
 }
 
+// ------------------------------------------------------------------------------------------------ columns, TMA, any ny
+// ny ≥ 256 that is not a power of two (2160 = 9 boxes of 240 rows): the 4-column tile arrives by TMA in LINEAR order in
+// its own buffer(s) and the padded engine of k_cols works beside it, so that — several lines — the load of line s + 1
+// runs under the transform of line s and no 32-byte row segment goes through the LSU.  The result leaves through
+// tile 0 by a TMA store.  (k_cols itself has one CTA per SM at these sizes and overlaps nothing.)
+template <int N> struct ColTmaPadCfg {
+  using C = ColCfg<N>;
+  static constexpr size_t LIN = (size_t)N * C::W * sizeof(float2);
+  static constexpr size_t WORK = (C::SMEM + 15) / 16 * 16;
+  static constexpr size_t smem(bool sum) { return (sum ? 2 : 1) * LIN + WORK + 16; }
+};
+
+template <int N, bool SUM>
+__global__ void __launch_bounds__(ColCfg<N>::NT, 1)
+k_cols_tmap(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_out, EprLines L, int M,
+            int mode, float scale, int box_rows, const float* __restrict__ lam_x, const float* __restrict__ lam_y,
+            const float2* __restrict__ tw, const float2* __restrict__ tw_inv) {
+  using C = ColCfg<N>;
+  using P = ColTmaPadCfg<N>;
+  using EF = Engine<N, C::TPC, C::W, false, false>;
+  using EI = Engine<N, C::TPC, C::W, true, true>;
+  static_assert(EF::RL == EI::R0 && EF::GL::CNT == EI::G0::CNT && EF::PL == EI::G0::T, "schedules must mirror");
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  constexpr int NBUF = SUM ? 2 : 1;
+  float2* work = reinterpret_cast<float2*>(smem_raw + NBUF * P::LIN);
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + NBUF * P::LIN + P::WORK);
+  const int c = threadIdx.x % C::W, t = threadIdx.x / C::W;
+  const int kx0 = blockIdx.x * C::W, kx = kx0 + c;
+  const int oplane = blockIdx.y;
+  const int nb = L.n_bins;
+  const int nloop = SUM ? nb : 1;
+  const int nbox = N / box_rows;
+  const float lx = __ldg(&lam_x[kx]);
+  if (threadIdx.x == 0) { eprtma::mbar_init(&bar[0], 1); eprtma::mbar_init(&bar[1], 1); eprtma::mbar_fence_init(); }
+  __syncthreads();
+  auto load_tile = [&](int sl) {            // one thread: request line sl of this output tile into buffer sl % NBUF
+    const int iplane = (mode == 1) ? oplane * nb + sl : oplane;
+    float2* dst = reinterpret_cast<float2*>(smem_raw + (sl % NBUF) * P::LIN);
+    eprtma::fence_proxy_async();
+    eprtma::mbar_expect_tx(&bar[sl % NBUF], (unsigned)P::LIN);
+    for (int bx = 0; bx < nbox; ++bx)
+      eprtma::tensor_g2s_2d(dst + bx * box_rows * C::W, &map_in, 2 * kx0, iplane * N + bx * box_rows, &bar[sl % NBUF]);
+  };
+  if (threadIdx.x == 0) load_tile(0);
+  float2 acc[EF::GL::CNT][EF::RL];
+#pragma unroll
+  for (int cc = 0; cc < EF::GL::CNT; ++cc)
+#pragma unroll
+    for (int q = 0; q < EF::RL; ++q) acc[cc][q] = make_float2(0.f, 0.f);
+  for (int sl = 0; sl < nloop; ++sl) {
+    const float a = (mode == 2) ? L.abar : L.a[(mode == 1) ? sl : (oplane % nb)];
+    const float2* lin = reinterpret_cast<const float2*>(smem_raw + (sl % NBUF) * P::LIN);
+    // the other buffer was last read during line sl − 1, which every thread left through the barrier closing it
+    if (SUM && threadIdx.x == 0 && sl + 1 < nloop) load_tile(sl + 1);
+    eprtma::mbar_wait(&bar[sl % NBUF], (sl / NBUF) & 1);
+    float2 u0[EF::G0::CNT][EF::R0], uL[EF::GL::CNT][EF::RL];
+#pragma unroll
+    for (int cc = 0; cc < EF::G0::CNT; ++cc) {
+      const int j = t + cc * C::TPC;
+#pragma unroll
+      for (int r = 0; r < EF::R0; ++r) {
+        float2 v = make_float2(0.f, 0.f);
+        if (EF::G0::FULL || j < EF::G0::T) v = lin[(j + r * EF::G0::T) * C::W + c];
+        u0[cc][r] = v;
+      }
+    }
+    EF::run(u0, uL, work, c, t, tw);
+    if (blockIdx.x == 0) {
+      // tile 0 holds the packed column kx = 0: C = F0 + i FM (both Hermitian in ky).  With A = ½(C[ky] + C*[−ky]),
+      // B = −(i/2)(C[ky] − C*[−ky]):  C'[ky] = H(0,ky) A + i H(M,ky) B,  C'[−ky] = H(0,ky) A* + i H(M,ky) B*.
+      __syncthreads();
+#pragma unroll
+      for (int cc = 0; cc < EF::GL::CNT; ++cc) {
+        const int j = t + cc * C::TPC;
+        if (EF::GL::FULL || j < EF::GL::T) {
+#pragma unroll
+          for (int q = 0; q < EF::RL; ++q) work[padi(j + q * EF::PL) * C::W + c] = uL[cc][q];
+        }
+      }
+      __syncthreads();
+      if (c == 0) {
+        const float lxN = __ldg(&lam_x[M]);
+        for (int ky = t; ky <= N / 2; ky += C::TPC) {
+          const int km = (ky == 0) ? 0 : N - ky;
+          const float2 ck = work[padi(ky) * C::W], cm = work[padi(km) * C::W];
+          const float ly = __ldg(&lam_y[ky]);
+          const float h0 = scale / (1.f + a * (lx + ly)), hN = scale / (1.f + a * (lxN + ly));
+          const float2 A = make_float2(0.5f * (ck.x + cm.x), 0.5f * (ck.y - cm.y));
+          const float2 B = make_float2(0.5f * (ck.y + cm.y), -0.5f * (ck.x - cm.x));
+          work[padi(ky) * C::W] = make_float2(h0 * A.x - hN * B.y, h0 * A.y + hN * B.x);
+          if (km != ky) work[padi(km) * C::W] = make_float2(h0 * A.x + hN * B.y, -h0 * A.y + hN * B.x);
+        }
+      }
+      __syncthreads();
+#pragma unroll
+      for (int cc = 0; cc < EF::GL::CNT; ++cc) {
+        const int j = t + cc * C::TPC;
+        if (EF::GL::FULL || j < EF::GL::T) {
+#pragma unroll
+          for (int q = 0; q < EF::RL; ++q) uL[cc][q] = work[padi(j + q * EF::PL) * C::W + c];
+        }
+      }
+    }
+    const float alx = fmaf(a, lx, 1.f);
+#pragma unroll
+    for (int cc = 0; cc < EF::GL::CNT; ++cc) {
+      const int j = t + cc * C::TPC;
+      if (EF::GL::FULL || j < EF::GL::T) {
+#pragma unroll
+        for (int q = 0; q < EF::RL; ++q) {
+          const float h = (kx == 0) ? 1.f : __fdividef(scale, fmaf(a, __ldg(&lam_y[j + q * EF::PL]), alx));
+          acc[cc][q].x = fmaf(h, uL[cc][q].x, acc[cc][q].x);
+          acc[cc][q].y = fmaf(h, uL[cc][q].y, acc[cc][q].y);
+        }
+      }
+    }
+    if (SUM) eprtma::fence_proxy_async();  // generic reads of this tile are ordered before its TMA refill (line sl + 2)
+    __syncthreads();                       // all reads of the tile and of the work buffer done
+  }
+  float2 uo[EI::GL::CNT][EI::RL];
+  EI::run(acc, uo, work, c, t, tw_inv);
+  float2* lin0 = reinterpret_cast<float2*>(smem_raw);     // free: every line has been consumed
+#pragma unroll
+  for (int cc = 0; cc < EI::GL::CNT; ++cc) {
+    const int j = t + cc * C::TPC;
+    if (EI::GL::FULL || j < EI::GL::T) {
+#pragma unroll
+      for (int q = 0; q < EI::RL; ++q) lin0[(j + q * EI::PL) * C::W + c] = uo[cc][q];
+    }
+  }
+  eprtma::fence_proxy_async();             // generic-proxy writes → visible to the async proxy
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int bx = 0; bx < nbox; ++bx)
+      eprtma::tensor_s2g_2d(&map_out, 2 * kx0, oplane * N + bx * box_rows, lin0 + bx * box_rows * C::W);
+    eprtma::bulk_commit();
+    eprtma::bulk_wait<0>();                // the CTA's shared memory must outlive the store
+  }
+}
+
 // ------------------------------------------------------------------------------------------------ dispatch
 // The instantiations are split into EPR_FFT_NGROUPS translation units (this file compiled once per group with
 // -DEPR_FFT_GROUP=g, in parallel: see build.py); epr_fftd.cu routes a size to the group that holds it.
@@ -605,6 +745,28 @@ static bool launch_cols_tma(const epr_plan_s* p, int oplanes, int mode, const fl
       k_cols_tma<N, true><<<grid, C::NT, C::smem(true), st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
     else
       k_cols_tma<N, false><<<grid, C::NT, C::smem(false), st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+    return true;
+  } else if constexpr (N >= 256) {
+    using C = ColCfg<N>;
+    using P = ColTmaPadCfg<N>;
+    const int M = p->nx / 2;
+    const bool sum = mode == 1 && p->n_bins > 1;
+    if (!p->tma_ok || M % C::W != 0 || spec != p->spec || (out != p->spec && out != p->spec_sum)) return false;
+    if (P::smem(sum) > 227 * 1024) return false;
+    static bool attr = false;
+    if (!attr) {
+      if (P::smem(false) <= 227 * 1024)
+        cudaFuncSetAttribute(k_cols_tmap<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::smem(false));
+      if (P::smem(true) <= 227 * 1024)
+        cudaFuncSetAttribute(k_cols_tmap<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::smem(true));
+      attr = true;
+    }
+    const CUtensorMap& mo = (out == p->spec) ? p->map_spec : p->map_spec_sum;
+    dim3 grid(M / C::W, oplanes);
+    if (sum)
+      k_cols_tmap<N, true><<<grid, C::NT, P::smem(true), st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->tma_box_rows, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+    else
+      k_cols_tmap<N, false><<<grid, C::NT, P::smem(false), st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->tma_box_rows, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
     return true;
   } else {
     return false;

@@ -53,7 +53,8 @@ struct epr_plan_s {
   float2* spec_sum;            // [work_batch][ny][nx/2]
   CUtensorMap map_spec;        // TMA descriptors of spec / spec_sum as [rows][nx floats], box 8 floats x 256 rows
   CUtensorMap map_spec_sum;
-  int tma_ok;                  // descriptors valid (power-of-two ny ≥ 256, nx % 8 == 0)
+  int tma_ok;                  // descriptors valid (ny ≥ 256, nx % 8 == 0)
+  int tma_box_rows;            // rows per TMA box: the largest divisor of ny that is ≤ 256 (256 for powers of two, 240 for 2160)
   float* gmax;                 // [work_batch][ny/16][nx/16] block maxima of |D⁰τ| (non-local: k_grad_blockmax)
   float* os_d;                 // [work_batch][ny][nx] up-sampled detector images (lazy, epr_retrieve_oversampled)
   float* os_out;               // [work_batch][ny][nx] fine-grid result before down-sampling (lazy)

@@ -324,6 +324,30 @@ def test_resampling_round_trip_is_exact(E):
         assert np.max(np.abs(out.cpu().numpy() - dn)) < 5e-7
 
 
+@pytest.mark.parametrize("ny,nx,n_lines", [(2160, 32, 3), (2160, 64, 8), (320, 64, 5), (2560, 32, 3)])
+def test_retrieve_non_power_of_two_columns_several_lines(E, ny, nx, n_lines):
+    """The Fourier-space sum over lines (R10) on column lengths that are not powers of two: 2160 and 320 take the
+    TMA-staged padded column kernel with two tiles in flight, 2560 (two tiles would not fit an SM) the direct one."""
+    import torch
+    rng = np.random.default_rng(ny + nx + n_lines)
+    y, x = np.meshgrid(np.arange(ny) * 2 * np.pi / ny, np.arange(nx) * 2 * np.pi / nx, indexing="ij")
+    d = 1.0 + sum(0.02 * rng.normal() * np.cos(rng.integers(1, 9) * y + rng.integers(0, 4) * x + rng.uniform(0, 6.28))
+                  for _ in range(8)) + 0.003 * rng.normal(size=(ny, nx))
+    d = d.astype(np.float32)[None]
+    e = np.linspace(60.0, 140.0, n_lines)
+    wt = np.exp(-0.5 * ((e - 100.0) / 20.0) ** 2)
+    db = 1000.0 * e / 100.0
+    plan = E.epr_plan(nx, ny, 6.5e-6, 0.5, e, wt, db, "local", max_batch=1)
+    dd = _dev(d)
+    out = torch.empty_like(dd)
+    E.epr_retrieve(plan, dd, out, 4, 1.0)
+    got = out.cpu().numpy()[0]
+    plan.destroy()
+    lines = O.derive_lines(6.5e-6, 0.5, e, wt, db)
+    ref = O.retrieve(d[0].astype(np.float64), lines, "local", 4, 1.0)
+    assert rel_l2(got, ref) < TOL_PHASE
+
+
 def test_retrieve_outputs_and_host_path(E):
     import torch
     w = make_workload("C1")
