@@ -113,6 +113,17 @@ epr_status epr_retrieve(epr_plan_t plan, int batch, const float* d, float* out, 
 epr_status epr_retrieve_oversampled(epr_plan_t plan, int factor, int batch, const float* d, float* out, int iterations,
                                     float step, void* stream);
 
+/* epr_set_diagnostics — per-iteration diagnostics of the retrievals that follow
+ *   diag: DEVICE array [batch][capacity_iters][2] of floats owned by the caller, or NULL to switch diagnostics off
+ *   (the default).  For projection b of a later epr_retrieve / epr_retrieve_oversampled / epr_retrieve_host call and
+ *   correction iteration n < capacity_iters:
+ *     diag[b][n][0] = RMS over the pixels of the detector residual e = d − Σ_s P_s at iteration n;
+ *     diag[b][n][1] = the regime indicator η of PAPER.md:53 in the sup norm: the largest unclamped shift component
+ *                     max_s max_r |a_s D⁰ ln I_s| in pixels of the plan's grid (η < 1: local regime).
+ *   Costs two small kernels and one pass over the residual planes per iteration; keep it off in timed runs.  While it
+ *   is on, retrievals are not captured into CUDA graphs. */
+epr_status epr_set_diagnostics(epr_plan_t plan, float* diag, int capacity_iters);
+
 /* epr_retrieve_host — same, with HOST buffers (pinned for full speed): copies d host→device, runs the loop,
  *   copies the result device→host, in chunks of max_batch projections with copies overlapped with compute;
  *   returns after the last copy has completed.  `batch` may exceed max_batch. */

@@ -294,8 +294,20 @@ def paganin_init(d, lines: Lines, symbol=0, i_min=1e-6):
     return project(T0, lines)
 
 
+def max_shift(tau, lines: Lines):
+    """Regime indicator of PAPER.md:53-55 in the sup norm: the largest component of the eikonal shift
+    u_s = a_s D⁰ ln I_s (Eq. (2), Eq. (6)) over pixels and lines, in pixels, NOT clamped
+    (η(r) = ‖Δ(r)‖/p is its Euclidean version: η_sup ≤ η ≤ √2 η_sup)."""
+    Is = line_intensities(tau, lines)
+    m = 0.0
+    for s in range(lines.n_bins):
+        ux, uy = ray_map(Is[s], lines.a[s], np.inf)
+        m = max(m, float(np.max(np.abs(ux))), float(np.max(np.abs(uy))))
+    return m
+
+
 def retrieve(d, lines: Lines, solver="local", iterations=10, step=1.0, order=2, wkb1=True,
-             symbol=0, S=16.0, i_min=1e-6, tau0=None, history=None):
+             symbol=0, S=16.0, i_min=1e-6, tau0=None, history=None, shift_history=None):
     """The batched per-projection correction loop for one projection:
     per-line predictions and their sum, detector residual, positivity-weighted split, transport
     back (identity | adjoint Eq. (4)), per-line FFT-diagonal preconditioner update, projection
@@ -309,6 +321,8 @@ def retrieve(d, lines: Lines, solver="local", iterations=10, step=1.0, order=2, 
         e = d - P
         if history is not None:
             history.append(float(np.sqrt(np.mean(e * e))))
+        if shift_history is not None:
+            shift_history.append(max_shift(tau, lines))
         w = split_weights(P_bins, lines)
         for s in range(n):
             r = w[s] * e

@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
 EXPORTS = ["epr_default_options", "epr_plan", "epr_forward", "epr_adjoint", "epr_transport", "epr_precondition",
-           "epr_retrieve", "epr_retrieve_oversampled", "epr_retrieve_host", "epr_plan_lines", "epr_launch_count", "epr_destroy",
+           "epr_retrieve", "epr_retrieve_oversampled", "epr_set_diagnostics", "epr_retrieve_host", "epr_plan_lines", "epr_launch_count", "epr_destroy",
            "epr_last_error", "epr_version", "epr_profile_enable", "epr_profile_read"]
 
 
@@ -53,6 +53,7 @@ def load_library():
     lib.epr_precondition.argtypes = [vp, ci, vp, vp, vp]
     lib.epr_retrieve.argtypes = [vp, ci, vp, vp, ci, cf, vp]
     lib.epr_retrieve_oversampled.argtypes = [vp, ci, ci, vp, vp, ci, cf, vp]
+    lib.epr_set_diagnostics.argtypes = [vp, vp, ci]
     lib.epr_retrieve_host.argtypes = [vp, ci, vp, vp, ci, cf]
     lib.epr_plan_lines.argtypes = [vp, C.POINTER(cd), C.POINTER(cd), C.POINTER(cd), C.POINTER(cd)]
     lib.epr_launch_count.argtypes = [vp]
@@ -66,7 +67,7 @@ def load_library():
     lib.epr_last_error.restype = C.c_char_p
     lib.epr_version.restype = C.c_char_p
     for name in ("epr_plan", "epr_forward", "epr_adjoint", "epr_transport", "epr_precondition", "epr_retrieve",
-                 "epr_retrieve_oversampled", "epr_retrieve_host", "epr_plan_lines", "epr_destroy"):
+                 "epr_retrieve_oversampled", "epr_set_diagnostics", "epr_retrieve_host", "epr_plan_lines", "epr_destroy"):
         getattr(lib, name).restype = ci
     _LIB = lib
     return lib
@@ -208,6 +209,16 @@ def epr_retrieve_oversampled(plan, factor, d, out, iterations, step):
     sh = (b, plan.ny // factor, plan.nx // factor)
     plan._check(load_library().epr_retrieve_oversampled(plan._h, factor, b, _dev(d, sh, "d"), _dev(out, sh, "out"),
                                                         int(iterations), float(step), _stream()))
+
+
+def epr_set_diagnostics(plan, diag):
+    """diag: contiguous float32 CUDA tensor [batch][capacity_iters][2] (kept alive by the caller), or None to switch off."""
+    if diag is None:
+        plan._check(load_library().epr_set_diagnostics(plan._h, C.c_void_p(0), 0))
+        return
+    if diag.dim() != 3 or diag.shape[2] != 2:
+        raise ValueError("diag: expected [batch][capacity_iters][2]")
+    plan._check(load_library().epr_set_diagnostics(plan._h, _dev(diag, None, "diag"), int(diag.shape[1])))
 
 
 def epr_retrieve_host(plan, d_host, out_host, iterations, step):

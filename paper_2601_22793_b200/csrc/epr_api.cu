@@ -24,9 +24,9 @@ static const double HC_KEV_M = 1.2398419843e-9;
     if (e_ != cudaSuccess) FAIL(p, EPR_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
   } while (0)
 // Kernel families, for launch counting and the optional per-kernel CUDA-event timing (epr_profile_*).
-enum { K_FWD_LOCAL = 0, K_SPLAT, K_RESIDUAL, K_GATHER, K_ROWS_R2C, K_COLS, K_ROWS_C2R, K_PRED_OUT, K_OUTPUT, K_RESAMPLE, K_COUNT };
+enum { K_FWD_LOCAL = 0, K_SPLAT, K_RESIDUAL, K_GATHER, K_ROWS_R2C, K_COLS, K_ROWS_C2R, K_PRED_OUT, K_OUTPUT, K_RESAMPLE, K_DIAG, K_COUNT };
 static const char* const K_NAMES[K_COUNT] = {"k_forward_local", "k_splat", "k_residual", "k_gather", "k_rows_r2c",
-                                              "k_cols", "k_rows_c2r", "k_pred_out", "k_output", "k_resample"};
+                                              "k_cols", "k_rows_c2r", "k_pred_out", "k_output", "k_resample", "k_diagnostics"};
 struct EprProf {
   struct Rec { int tag; cudaEvent_t a, b; };
   std::vector<Rec> recs;
@@ -296,7 +296,7 @@ extern "C" epr_status epr_destroy(epr_plan_t p) {
   cudaDeviceSynchronize();
   cudaFree(p->tw_row); cudaFree(p->tw_r2c); cudaFree(p->tw_col); cudaFree(p->tw_col_inv); cudaFree(p->lam_x); cudaFree(p->lam_y);
   cudaFree(p->tau); cudaFree(p->pred); cudaFree(p->res); cudaFree(p->res2); cudaFree(p->spec); cudaFree(p->spec_sum);
-  cudaFree(p->raymap); cudaFree(p->gmax); cudaFree(p->os_d); cudaFree(p->os_out);
+  cudaFree(p->raymap); cudaFree(p->gmax); cudaFree(p->os_d); cudaFree(p->os_out); cudaFree(p->diag_partial);
   if (p->graph_exec) cudaGraphExecDestroy(p->graph_exec);
   if (p->prof) { epr_profile_read(p, 0, NULL, NULL, NULL, 1); delete (EprProf*)p->prof; }
   for (int i = 0; i < 2; ++i) { cudaFree(p->stage_in[i]); cudaFree(p->stage_out[i]); }
@@ -389,8 +389,9 @@ extern "C" epr_status epr_precondition(epr_plan_t p, int batch, const float* r_b
 
 // ----------------------------------------------------------------------------------------------- the loop
 // One pass over `nb` ≤ work_batch projections.  tau is the state (device, [nb][ny][nx]).
+// b_first: index of the chunk's first projection within the caller's batch (row of the diagnostics array).
 static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* tau, int iterations, float step,
-                                 cudaStream_t cs) {
+                                 int b_first, cudaStream_t cs) {
   const size_t plane = (size_t)p->nx * p->ny;
   const int planes = nb * p->n_bins;
   if (p->opt.init == 0) {
@@ -409,6 +410,8 @@ static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* ta
         KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, p->res, cs));           // a2 (a3 = identity)
       }
       r = p->res;
+      if (p->diag && it < p->diag_cap)
+        KL(p, K_DIAG, cs, epr_launch_diagnostics(p, nb, tau, p->res, p->diag + ((size_t)b_first * p->diag_cap + it) * 2, p->diag_cap * 2, cs));
     } else {
       if (p->n_bins == 1) {
         KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->res, 2, d, cs));       // a0 + a1-N + a2 fused
@@ -417,6 +420,8 @@ static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* ta
         KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->res, 3, d, cs));       // a0 + a1-N + a2 fused
         p->launches += 1;                                  // k_grad_blockmax, launched ahead of the splat
       }
+      if (p->diag && it < p->diag_cap)
+        KL(p, K_DIAG, cs, epr_launch_diagnostics(p, nb, tau, p->res, p->diag + ((size_t)b_first * p->diag_cap + it) * 2, p->diag_cap * 2, cs));
       KL(p, K_GATHER, cs, epr_launch_gather(p, nb, tau, NULL, p->res, p->res2, 1, cs));          // a3
       r = p->res2;
     }
@@ -428,17 +433,33 @@ static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* ta
 }
 
 static epr_status retrieve_device(epr_plan_t p, int batch, const float* d, float* out, int iterations, float step,
-                                  cudaStream_t cs) {
+                                  int b_first, cudaStream_t cs) {
   const size_t plane = (size_t)p->nx * p->ny;
   for (int b0 = 0; b0 < batch; b0 += p->work_batch) {
     const int nb = (batch - b0 < p->work_batch) ? batch - b0 : p->work_batch;
     float* o = out + (size_t)b0 * plane;
     float* tau = (p->opt.output == 0) ? o : p->tau;
     if (p->opt.init == 1 && tau != o) CU(p, cudaMemcpyAsync(tau, o, (size_t)nb * plane * sizeof(float), cudaMemcpyDeviceToDevice, cs));
-    epr_status st = retrieve_chunk(p, nb, d + (size_t)b0 * plane, tau, iterations, step, cs);
+    epr_status st = retrieve_chunk(p, nb, d + (size_t)b0 * plane, tau, iterations, step, b_first + b0, cs);
     if (st != EPR_OK) return st;
     if (p->opt.output != 0) KL(p, K_OUTPUT, cs, epr_launch_output(p, nb, tau, o, cs));
   }
+  return EPR_OK;
+}
+
+// Per-iteration diagnostics of the following retrievals: residual RMS and largest shift component (device array).
+extern "C" epr_status epr_set_diagnostics(epr_plan_t p, float* diag, int capacity_iters) {
+  if (!p) return EPR_EINVAL;
+  if (diag && capacity_iters < 1) FAIL(p, EPR_EINVAL, "epr_set_diagnostics: capacity_iters must be >= 1");
+  if (diag) {
+    cudaError_t e = cudaSuccess;
+    if (!p->diag_partial) e = cudaMalloc((void**)&p->diag_partial, (size_t)p->work_batch * 64 * sizeof(double));
+    if (e == cudaSuccess && !p->gmax)
+      e = cudaMalloc((void**)&p->gmax, (size_t)p->work_batch * (p->nx / 16) * (p->ny / 16) * sizeof(float));
+    if (e != cudaSuccess) FAIL(p, e == cudaErrorMemoryAllocation ? EPR_ENOMEM : EPR_ECUDA, "diagnostics buffers: %s", cudaGetErrorString(e));
+  }
+  p->diag = diag;
+  p->diag_cap = diag ? capacity_iters : 0;
   return EPR_OK;
 }
 
@@ -462,7 +483,7 @@ extern "C" epr_status epr_retrieve_oversampled(epr_plan_t p, int factor, int bat
   for (int b0 = 0; b0 < batch; b0 += p->work_batch) {
     const int nb = (batch - b0 < p->work_batch) ? batch - b0 : p->work_batch;
     KL(p, K_RESAMPLE, cs, epr_launch_upsample(p, nb, factor, d + (size_t)b0 * cplane, p->os_d, cs));
-    st = retrieve_device(p, nb, p->os_d, p->os_out, iterations, step, cs);
+    st = retrieve_device(p, nb, p->os_d, p->os_out, iterations, step, b0, cs);
     if (st != EPR_OK) return st;
     KL(p, K_RESAMPLE, cs, epr_launch_downsample(p, nb, factor, p->os_out, out + (size_t)b0 * cplane, cs));
   }
@@ -480,8 +501,8 @@ extern "C" epr_status epr_retrieve(epr_plan_t p, int batch, const float* d, floa
   // captured once into a CUDA graph and replayed while the call's arguments stay the same.  Never under profiling
   // (events are recorded around every launch) and never on the legacy default stream (capture is illegal there).
   const size_t work = (size_t)batch * p->n_bins * p->nx * p->ny;
-  const bool use_graph = !p->prof_on && cs != 0 && (p->graph_mode == 2 || (p->graph_mode == 1 && work <= ((size_t)1 << 20)));
-  if (!use_graph) return retrieve_device(p, batch, d, out, iterations, step, cs);
+  const bool use_graph = !p->prof_on && !p->diag && cs != 0 && (p->graph_mode == 2 || (p->graph_mode == 1 && work <= ((size_t)1 << 20)));
+  if (!use_graph) return retrieve_device(p, batch, d, out, iterations, step, 0, cs);
   if (p->graph_exec && p->graph_d == d && p->graph_out == out && p->graph_batch == batch && p->graph_iters == iterations &&
       p->graph_step == step) {
     CU(p, cudaGraphLaunch(p->graph_exec, cs));
@@ -492,11 +513,11 @@ extern "C" epr_status epr_retrieve(epr_plan_t p, int batch, const float* d, floa
   // one eager pass first: launchers set function attributes / query occupancy on their first call
   if (!p->graph_warm) {
     p->graph_warm = 1;
-    return retrieve_device(p, batch, d, out, iterations, step, cs);
+    return retrieve_device(p, batch, d, out, iterations, step, 0, cs);
   }
   const long long l0 = p->launches;
   CU(p, cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal));
-  st = retrieve_device(p, batch, d, out, iterations, step, cs);
+  st = retrieve_device(p, batch, d, out, iterations, step, 0, cs);
   cudaGraph_t graph = NULL;
   cudaError_t ce = cudaStreamEndCapture(cs, &graph);
   if (st != EPR_OK) { if (graph) cudaGraphDestroy(graph); return st; }
@@ -567,7 +588,7 @@ extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_
       CU(p, cudaMemcpyAsync(p->stage_out[buf], out_host + (size_t)b0 * plane, bytes, cudaMemcpyHostToDevice, s_in));
     CU(p, cudaEventRecord(ev_in, s_in));
     CU(p, cudaStreamWaitEvent(s_cmp, ev_in, 0));
-    epr_status st = retrieve_device(p, nb, p->stage_in[buf], p->stage_out[buf], iterations, step, s_cmp);
+    epr_status st = retrieve_device(p, nb, p->stage_in[buf], p->stage_out[buf], iterations, step, b0, s_cmp);
     if (st != EPR_OK) return st;
     CU(p, cudaEventRecord(ev_cmp, s_cmp));
     CU(p, cudaStreamWaitEvent(s_out, ev_cmp, 0));

@@ -56,6 +56,9 @@ struct epr_plan_s {
   int tma_ok;                  // descriptors valid (ny ≥ 256, nx % 8 == 0)
   int tma_box_rows;            // rows per TMA box: the largest divisor of ny that is ≤ 256 (256 for powers of two, 240 for 2160)
   float* gmax;                 // [work_batch][ny/16][nx/16] block maxima of |D⁰τ| (non-local: k_grad_blockmax)
+  float* diag;                 // caller's diagnostics array [batch][diag_cap][2] (device) or NULL (epr_set_diagnostics)
+  int diag_cap;
+  double* diag_partial;        // [work_batch][64] partial sums of squares
   float* os_d;                 // [work_batch][ny][nx] up-sampled detector images (lazy, epr_retrieve_oversampled)
   float* os_out;               // [work_batch][ny][nx] fine-grid result before down-sampling (lazy)
   float2* raymap;              // [work_batch][n_bins][ny][nx] stored u_s (lazy, epr_forward non-local)
@@ -110,4 +113,7 @@ cudaError_t epr_launch_rows_c2r(const epr_plan_s* p, int planes, const float2* s
 // oversampled grid (R16): the plan's (nx, ny) is the FINE grid; coarse planes are (ny/m) x (nx/m)
 cudaError_t epr_launch_upsample(const epr_plan_s* p, int batch, int m, const float* coarse, float* fine, cudaStream_t st);
 cudaError_t epr_launch_downsample(const epr_plan_s* p, int batch, int m, const float* fine, float* coarse, cudaStream_t st);
+// diag[b·stride + 0] = RMS_px(Σ_s es[b][s]), diag[b·stride + 1] = max_s |c_s| · max|D⁰τ| (unclamped shift, px)
+cudaError_t epr_launch_diagnostics(const epr_plan_s* p, int batch, const float* tau, const float* es, float* diag,
+                                   int stride, cudaStream_t st);
 cudaError_t epr_launch_output(const epr_plan_s* p, int batch, const float* tau, float* out, cudaStream_t st);

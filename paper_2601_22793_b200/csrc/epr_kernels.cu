@@ -1102,3 +1102,67 @@ cudaError_t epr_launch_downsample(const epr_plan_s* p, int batch, int m, const f
   k_downsample<<<grid, 256, 0, st>>>(p->nx / m, p->ny / m, m, fine, coarse);
   return cudaGetLastError();
 }
+
+// =====================================================================================================
+// Diagnostics of the loop (off unless epr_set_diagnostics was called; never in timed runs): per projection and
+// iteration, the RMS of the detector residual e = d − Σ_s P_s = Σ_s e_s and the regime indicator
+// η as the largest unclamped shift component max_s |c_s| · max|D⁰τ| from the block maxima.
+// Two launches, fixed summation order (bit-reproducible).
+// =====================================================================================================
+#define DG_BLK 64
+__global__ void __launch_bounds__(256) k_diag_partial(int n_bins, unsigned plane, const float* __restrict__ es,
+                                                      double* __restrict__ partial) {
+  __shared__ double s_sum[256];
+  const int b = blockIdx.y;
+  const float* eb = es + (size_t)b * n_bins * plane;
+  double acc = 0.0;
+  for (unsigned i = (blockIdx.x * 256u + threadIdx.x) * 4u; i < plane; i += DG_BLK * 256u * 4u) {
+    float4 e = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int s = 0; s < n_bins; ++s) {
+      const float4 v = __ldg(reinterpret_cast<const float4*>(eb + (size_t)s * plane + i));
+      e.x += v.x; e.y += v.y; e.z += v.z; e.w += v.w;
+    }
+    acc += (double)e.x * e.x + (double)e.y * e.y + (double)e.z * e.z + (double)e.w * e.w;
+  }
+  s_sum[threadIdx.x] = acc;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (threadIdx.x < o) s_sum[threadIdx.x] += s_sum[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) partial[(size_t)b * DG_BLK + blockIdx.x] = s_sum[0];
+}
+
+__global__ void __launch_bounds__(256) k_diag_final(unsigned plane, int nblocks, float cmax, const double* __restrict__ partial,
+                                                    const float* __restrict__ gmax, float* __restrict__ diag, int stride) {
+  __shared__ float s_max[256];
+  const int b = blockIdx.x;
+  float m = 0.f;
+  for (int i = threadIdx.x; i < nblocks; i += 256) m = fmaxf(m, __ldg(&gmax[(size_t)b * nblocks + i]));
+  s_max[threadIdx.x] = m;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (threadIdx.x < o) s_max[threadIdx.x] = fmaxf(s_max[threadIdx.x], s_max[threadIdx.x + o]);
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    double sum = 0.0;
+    for (int i = 0; i < DG_BLK; ++i) sum += partial[(size_t)b * DG_BLK + i];
+    diag[(size_t)b * stride] = (float)sqrt(sum / (double)plane);
+    diag[(size_t)b * stride + 1] = cmax * s_max[0];
+  }
+}
+
+cudaError_t epr_launch_diagnostics(const epr_plan_s* p, int batch, const float* tau, const float* es, float* diag,
+                                   int stride, cudaStream_t st) {
+  const unsigned plane = (unsigned)p->nx * p->ny;
+  if (p->solver == EPR_LOCAL) {                       // the non-local splat has already refreshed p->gmax for this τ
+    const cudaError_t e = epr_launch_grad_blockmax(p, batch, tau, st);
+    if (e != cudaSuccess) return e;
+  }
+  float cmax = 0.f;
+  for (int s = 0; s < p->n_bins; ++s) cmax = fmaxf(cmax, 0.5f * p->lines.a[s] * p->lines.gamma[s]);
+  k_diag_partial<<<dim3(DG_BLK, batch), 256, 0, st>>>(p->n_bins, plane, es, p->diag_partial);
+  k_diag_final<<<batch, 256, 0, st>>>(plane, (p->nx / 16) * (p->ny / 16), cmax, p->diag_partial, p->gmax, diag, stride);
+  return cudaGetLastError();
+}

@@ -348,6 +348,35 @@ def test_retrieve_non_power_of_two_columns_several_lines(E, ny, nx, n_lines):
     assert rel_l2(got, ref) < TOL_PHASE
 
 
+@pytest.mark.parametrize("name,n", [("C1", None), ("C3", 256), ("C4", 128)])
+def test_diagnostics_history(E, name, n):
+    """epr_set_diagnostics: residual RMS and largest unclamped shift per iteration against the oracle's histories
+    (PAPER.md:53-55, 231); switching it off restores the plain result bit for bit."""
+    import torch
+    w = make_workload(name, n=n, batch=2)
+    plan = E.epr_plan(w.nx, w.ny, w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
+                      max_batch=2, max_shift_px=w.max_shift_px)
+    d = _dev(w.d)
+    out = torch.empty_like(d)
+    diag = torch.zeros(2, w.iterations, 2, device="cuda")
+    E.epr_set_diagnostics(plan, diag)
+    E.epr_retrieve(plan, d, out, w.iterations, w.step)
+    got = diag.cpu().numpy()
+    E.epr_set_diagnostics(plan, None)
+    out2 = torch.empty_like(d)
+    E.epr_retrieve(plan, d, out2, w.iterations, w.step)
+    assert torch.equal(out, out2)
+    plan.destroy()
+    lines = O.derive_lines(w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta)
+    for j in range(2):
+        h, sh = [], []
+        O.retrieve(w.d[j].astype(np.float64), lines, w.solver, w.iterations, w.step, S=w.max_shift_px, history=h,
+                   shift_history=sh)
+        h, sh = np.array(h), np.array(sh)
+        assert np.max(np.abs(got[j, :, 0] - h)) < 2e-3 * h[0]          # e is a small difference of O(1) planes in fp32
+        assert np.max(np.abs(got[j, :, 1] - sh) / sh) < 1e-3
+
+
 def test_retrieve_outputs_and_host_path(E):
     import torch
     w = make_workload("C1")

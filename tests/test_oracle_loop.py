@@ -125,3 +125,25 @@ def test_local_solver_degrades_beyond_one_pixel_nonlocal_stays_stable():
     O.retrieve(d, lines, "nonlocal", iterations=8, step=0.4, history=h_non)
     assert h_non[-1] < h_non[0]
     assert not (h_loc[-1] < h_non[-1])
+
+
+def test_max_shift_closed_form_and_history():
+    """I = exp(c x) (one line): u_x = a c exactly wherever the central difference does not straddle the periodic seam,
+    u_y = 0; the indicator is not clamped.  The histories have one entry per iteration."""
+    lines = _mono(50.0)
+    ny, nx, c = 8, 64, 0.03
+    tau = -c * np.tile(np.arange(nx, dtype=np.float64), (ny, 1))          # I = exp(c x)
+    ux, uy = O.ray_map(np.exp(-tau), lines.a[0], np.inf)
+    assert np.max(np.abs(ux[:, 1:-1] - lines.a[0] * c)) < 1e-10 and np.max(np.abs(uy)) == 0.0
+    seam = lines.a[0] * c * (nx - 2) / 2.0                                 # |D0| across the wrap: (x_0 - x_{n-2}) / 2
+    assert abs(O.max_shift(tau, lines) - seam) < 1e-9 * seam
+    d = 1.0 + 0.01 * _smooth(32, 32, 3)
+    h, sh = [], []
+    O.retrieve(d, lines, "local", iterations=3, step=1.0, history=h, shift_history=sh)
+    assert len(h) == len(sh) == 3 and all(v > 0 for v in sh)
+    E = np.array([80.0, 120.0])
+    l2 = O.derive_lines(6.5e-6, 2.0, E, [0.5, 0.5], [800.0, 1200.0])
+    t2 = 0.1 * (1.0 + _smooth(16, 16, 9))
+    per_line = [max(np.max(np.abs(l2.a[s] * l2.gamma[s] * O.d0x(t2))), np.max(np.abs(l2.a[s] * l2.gamma[s] * O.d0y(t2))))
+                for s in range(2)]
+    assert abs(O.max_shift(t2, l2) - max(per_line)) < 1e-12             # D0 ln I_s = −γ_s D0 τ (Eq. (7))
