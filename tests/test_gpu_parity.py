@@ -377,6 +377,32 @@ def test_diagnostics_history(E, name, n):
         assert np.max(np.abs(got[j, :, 1] - sh) / sh) < 1e-3
 
 
+@pytest.mark.parametrize("ny,nx,n_lines", [(16, 16, 1), (32, 48, 3), (48, 16, 8), (80, 160, 5)])
+def test_retrieve_nonlocal_grids_smaller_than_a_tile(E, ny, nx, n_lines):
+    """Grids smaller than one 128 x 64 detector tile, started (opt.init = 1) from a τ⁰ whose shifts span several pixels
+    and hit the clamp: every source reaches the tile through several periodic images (R7), the block-maximum samples
+    and the staged residual rows wrap more than once."""
+    import torch
+    rng = np.random.default_rng(100 * ny + nx)
+    y, x = np.meshgrid(np.arange(ny) * 2 * np.pi / ny, np.arange(nx) * 2 * np.pi / nx, indexing="ij")
+    d = (1.0 + 0.15 * np.cos(y + 0.3) * np.sin(2 * x) + 0.1 * np.cos(3 * y - x) + 0.01 * rng.normal(size=(ny, nx)))
+    d = d.astype(np.float32)[None]
+    tau0 = (0.12 * (1.0 + np.cos(y + 1.0) * np.cos(x)) + 0.05 * np.sin(2 * y + x)).astype(np.float32)[None]
+    e = np.linspace(60.0, 140.0, n_lines) if n_lines > 1 else np.array([100.0])
+    wt = np.exp(-0.5 * ((e - 100.0) / 20.0) ** 2)
+    db = 200.0 * e / 100.0
+    L_m, S, its = 40.0, 6.0, 2
+    lines = O.derive_lines(6.5e-6, L_m, e, wt, db)
+    assert O.max_shift(tau0[0].astype(np.float64), lines) > S        # several pixels, some clamped
+    ref = O.retrieve(d[0].astype(np.float64), lines, "nonlocal", its, 0.4, S=S, tau0=tau0[0].astype(np.float64))
+    plan = E.epr_plan(nx, ny, 6.5e-6, L_m, e, wt, db, "nonlocal", max_batch=1, max_shift_px=S, init=1)
+    out = _dev(tau0.copy())
+    E.epr_retrieve(plan, _dev(d), out, its, 0.4)
+    got = out.cpu().numpy()[0]
+    plan.destroy()
+    assert rel_l2(got, ref) < TOL_PHASE
+
+
 def test_retrieve_outputs_and_host_path(E):
     import torch
     w = make_workload("C1")
