@@ -384,31 +384,43 @@ __device__ __forceinline__ void sw_scatter(const float2 (&u)[PassGeom<N, R, TPC>
 // Same pass structure as Engine (STRIDE = 4 columns per tile), on the swizzled layout.
 //  run_first: first-pass inputs already in registers (read by the caller from the LINEAR tile, followed by a barrier)
 //  the last pass leaves its outputs in registers (element index of uL[c][q] is (t + c·TPC) + q·PL).
-template <int N, int TPC, bool INV, bool REV> struct EngineSw {
+// barrier of the threads that share a tile: the whole CTA (GROUP = 0, __syncthreads) or a named barrier `id` of GROUP
+// threads (two 512-thread groups of one CTA working on different tiles)
+template <int GROUP> __device__ __forceinline__ void tile_sync(int id) {
+  if constexpr (GROUP == 0) __syncthreads();
+  else asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(GROUP) : "memory");
+}
+
+template <int N, int TPC, bool INV, bool REV, int GROUP = 0> struct EngineSw {
   using E = Engine<N, TPC, 4, INV, REV>;
   static constexpr int NP = E::NP, R0 = E::R0, RL = E::RL, PL = E::PL;
   using G0 = typename E::G0;
   using GL = typename E::GL;
   static_assert(NP >= 2, "at least two passes");
 
-  template <int I> __device__ static __forceinline__ void middle(float2* s, int c, int t, const float2* __restrict__ tw) {
+  template <int I> __device__ static __forceinline__ void middle(float2* s, int c, int t, const float2* __restrict__ tw, int bar) {
     if constexpr (I < NP - 1) {
       constexpr int R = sched_radix(N, I, REV), P = sched_P(N, I, REV);
       float2 u[PassGeom<N, R, TPC>::CNT][R];
       sw_gather<N, R, TPC>(u, s, c, t);
-      __syncthreads();
+      tile_sync<GROUP>(bar);
       bfly<N, P, R, TPC, INV>(u, t, tw + tw_offset(N, I, REV));
       sw_scatter<N, P, R, TPC>(u, s, c, t);
-      __syncthreads();
-      middle<I + 1>(s, c, t, tw);
+      tile_sync<GROUP>(bar);
+      middle<I + 1>(s, c, t, tw, bar);
     }
   }
+  struct NoHook { __device__ __forceinline__ void operator()() const {} };
+  // hook: called once by every thread after its first-pass scatter, before the first barrier (a place where one
+  // thread can do a little bookkeeping while the others are still computing)
+  template <class HOOK = NoHook>
   __device__ static __forceinline__ void run(float2 (&u0)[G0::CNT][R0], float2 (&uL)[GL::CNT][RL], float2* s, int c, int t,
-                                             const float2* __restrict__ tw) {
+                                             const float2* __restrict__ tw, int bar = 0, HOOK hook = HOOK()) {
     bfly<N, 1, R0, TPC, INV>(u0, t, tw);
     sw_scatter<N, 1, R0, TPC>(u0, s, c, t);
-    __syncthreads();
-    middle<1>(s, c, t, tw);
+    hook();
+    tile_sync<GROUP>(bar);
+    middle<1>(s, c, t, tw, bar);
     sw_gather<N, RL, TPC>(uL, s, c, t);
     bfly<N, PL, RL, TPC, INV>(uL, t, tw + tw_offset(N, NP - 1, REV));
   }

@@ -5,6 +5,7 @@
 // and X[nx/2] (im), so a plane of nx/2 complex columns holds the whole half spectrum.
 // H_s(θ) = 1 / (1 + a_s λ(θ)) with λ = λx[kx] + λy[ky] from two 1-D tables (discrete or continuous symbol, R5);
 // the 1/(nx·ny) normalisation is folded into H.
+#include <type_traits>
 #include "epr_fft.cuh"
 #include "epr_internal.h"
 #include "epr_math.cuh"
@@ -490,6 +491,129 @@ k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
   }
 }
 
+// ------------------------------------------------------------------------------------------------ columns, TMA, two groups
+// One line per output tile (the one-line loop, the initial guess, epr_precondition) at ny = 2048: in k_cols_tma a CTA
+// loads, transforms and stores ONE tile, and a fifth of its warp time is spent at the mbarrier waiting for that tile
+// (both CTAs of an SM often wait together).  Here one persistent CTA per SM runs TWO groups of 512 threads on
+// different tiles with THREE 64 KB tile buffers: tile k (k = 0, 1, 2, … in this CTA's static sequence) lives in buffer
+// k mod 3 and is processed by group k mod 2; the group that finishes tile k stores it and, as soon as the TMA unit has
+// read the buffer, requests tile k + 3 into it — which the OTHER group will need only after finishing tile k + 1.
+// The groups drift half a tile apart after the first wait, so every later tile has landed before it is wanted.
+// Groups synchronise on named barriers (1 + group); the engine is the same swizzled in-place one.
+template <int N>
+__global__ void __launch_bounds__(2 * ColTmaCfg<N>::NT, 1)
+k_cols_tma2(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_out, EprLines L, int M,
+            int mode, float scale, int tiles_x, int ntiles, const float* __restrict__ lam_x,
+            const float* __restrict__ lam_y, const float2* __restrict__ tw, const float2* __restrict__ tw_inv) {
+  using C = ColTmaCfg<N>;
+  constexpr int GT = C::NT;                                // threads per group
+  using EF = EngineSw<N, C::TPC, false, false, GT>;
+  using EI = EngineSw<N, C::TPC, true, true, GT>;
+  static_assert(EF::RL == EI::R0 && EF::GL::CNT == EI::G0::CNT && EF::PL == EI::G0::T, "schedules must mirror");
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + 3 * C::TILE);
+  const int g = threadIdx.x / GT, lt = threadIdx.x - g * GT;
+  const int c = lt % C::W, t = lt / C::W;
+  const int nb = L.n_bins;
+  auto tile_of = [&](int k) { return (int)blockIdx.x + k * (int)gridDim.x; };
+  auto load_tile = [&](int k) {             // one thread: request tile k of this CTA's sequence into buffer k % 3
+    const int T = tile_of(k), bx = T % tiles_x, pl = T / tiles_x;
+    float2* dst = reinterpret_cast<float2*>(smem_raw + (k % 3) * C::TILE);
+    eprtma::fence_proxy_async();
+    eprtma::mbar_expect_tx(&bar[k % 3], (unsigned)C::TILE);
+#pragma unroll
+    for (int b = 0; b < N / C::BOX; ++b)
+      eprtma::tensor_g2s_2d(dst + b * C::BOX * C::W, &map_in, 2 * bx * C::W, pl * N + b * C::BOX, &bar[k % 3]);
+  };
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < 3; ++i) eprtma::mbar_init(&bar[i], 1);
+    eprtma::mbar_fence_init();
+    for (int k = 0; k < 3; ++k)
+      if (tile_of(k) < ntiles) load_tile(k);
+  }
+  __syncthreads();
+  int pending = -1;                        // thread 0 of a group: tile to request into the buffer stored last
+  auto work = [&](auto bid_tag) {
+    constexpr int BID = decltype(bid_tag)::value;          // named barrier of this group (compile time: no R2UR per barrier)
+    for (int k = g; tile_of(k) < ntiles; k += 2) {
+      const int T = tile_of(k), bx = T % tiles_x, oplane = T / tiles_x;
+      const int kx = bx * C::W + c;
+      const float lx = __ldg(&lam_x[kx]);
+      const float a = (mode == 2) ? L.abar : L.a[oplane % nb];
+      float2* sm = reinterpret_cast<float2*>(smem_raw + (k % 3) * C::TILE);
+      // Refill of the buffer this group stored last: by then the TMA unit has read it (the wait returns at once), and
+      // the request still leaves the other group, which wants that tile, about half a tile of lead.
+      auto refill = [&]() {
+        if (lt == 0 && pending >= 0) { eprtma::bulk_wait_read<0>(); load_tile(pending); pending = -1; }
+      };
+      eprtma::mbar_wait(&bar[k % 3], (unsigned)(k / 3) & 1u);
+      float2 u0[EF::G0::CNT][EF::R0], uL[EF::GL::CNT][EF::RL], acc[EF::GL::CNT][EF::RL];
+#pragma unroll
+      for (int cc = 0; cc < EF::G0::CNT; ++cc)
+#pragma unroll
+        for (int r = 0; r < EF::R0; ++r) u0[cc][r] = sm[(t + cc * C::TPC + r * EF::G0::T) * C::W + c];   // LINEAR tile
+      tile_sync<GT>(BID);                     // every thread has its inputs: the tile may be overwritten in place
+      EF::run(u0, uL, sm, c, t, tw, BID, refill);
+      if (bx == 0) {
+        // tile 0 holds the packed column kx = 0 (see k_cols_tma)
+        tile_sync<GT>(BID);
+#pragma unroll
+        for (int cc = 0; cc < EF::GL::CNT; ++cc)
+#pragma unroll
+          for (int q = 0; q < EF::RL; ++q) sm[(t + cc * C::TPC + q * EF::PL) * C::W + c] = uL[cc][q];
+        tile_sync<GT>(BID);
+        if (c == 0) {
+          const float lxN = __ldg(&lam_x[M]);
+          for (int ky = t; ky <= N / 2; ky += C::TPC) {
+            const int km = (ky == 0) ? 0 : N - ky;
+            const float2 ck = sm[ky * C::W], cm = sm[km * C::W];
+            const float ly = __ldg(&lam_y[ky]);
+            const float h0 = scale / (1.f + a * (lx + ly)), hN = scale / (1.f + a * (lxN + ly));
+            const float2 A = make_float2(0.5f * (ck.x + cm.x), 0.5f * (ck.y - cm.y));
+            const float2 B = make_float2(0.5f * (ck.y + cm.y), -0.5f * (ck.x - cm.x));
+            sm[ky * C::W] = make_float2(h0 * A.x - hN * B.y, h0 * A.y + hN * B.x);
+            if (km != ky) sm[km * C::W] = make_float2(h0 * A.x + hN * B.y, -h0 * A.y + hN * B.x);
+          }
+        }
+        tile_sync<GT>(BID);
+#pragma unroll
+        for (int cc = 0; cc < EF::GL::CNT; ++cc)
+#pragma unroll
+          for (int q = 0; q < EF::RL; ++q) uL[cc][q] = sm[(t + cc * C::TPC + q * EF::PL) * C::W + c];
+      }
+      const float alx = fmaf(a, lx, 1.f);
+#pragma unroll
+      for (int cc = 0; cc < EF::GL::CNT; ++cc) {
+#pragma unroll
+        for (int q = 0; q < EF::RL; ++q) {
+          const float h = (kx == 0) ? 1.f : __fdividef(scale, fmaf(a, __ldg(&lam_y[t + cc * C::TPC + q * EF::PL]), alx));
+          acc[cc][q].x = h * uL[cc][q].x; acc[cc][q].y = h * uL[cc][q].y;
+        }
+      }
+      tile_sync<GT>(BID);                     // all reads of the tile done before the inverse writes it
+      float2 uo[EI::GL::CNT][EI::RL];
+      EI::run(acc, uo, sm, c, t, tw_inv, BID);
+      tile_sync<GT>(BID);                     // last-pass gathers done: the tile is rewritten in LINEAR order for the TMA store
+#pragma unroll
+      for (int cc = 0; cc < EI::GL::CNT; ++cc)
+#pragma unroll
+        for (int q = 0; q < EI::RL; ++q) sm[(t + cc * C::TPC + q * EI::PL) * C::W + c] = uo[cc][q];
+      eprtma::fence_proxy_async();            // generic-proxy writes → visible to the async proxy
+      tile_sync<GT>(BID);
+      if (lt == 0) {
+#pragma unroll
+        for (int b = 0; b < N / C::BOX; ++b)
+          eprtma::tensor_s2g_2d(&map_out, 2 * bx * C::W, oplane * N + b * C::BOX, sm + b * C::BOX * C::W);
+        eprtma::bulk_commit();
+        pending = tile_of(k + 3) < ntiles ? k + 3 : -1;      // refilled from the next tile's first pass (see `refill`)
+      }
+    }
+  };
+  if (g == 0) work(std::integral_constant<int, 1>{}); else work(std::integral_constant<int, 2>{});
+  if (lt == 0 && pending >= 0) { eprtma::bulk_wait_read<0>(); load_tile(pending); }   // (cannot happen: kept for safety)
+  if (lt == 0) eprtma::bulk_wait<0>();      // the CTA's stores are complete before it exits
+}
+
 // ------------------------------------------------------------------------------------------------ columns, TMA, any ny
 // ny ≥ 256 that is not a power of two (2160 = 9 boxes of 240 rows): the 4-column tile arrives by TMA in LINEAR order in
 // its own buffer(s) and the padded engine of k_cols works beside it, so that — several lines — the load of line s + 1
@@ -741,6 +865,20 @@ static bool launch_cols_tma(const epr_plan_s* p, int oplanes, int mode, const fl
     }
     const CUtensorMap& mo = (out == p->spec) ? p->map_spec : p->map_spec_sum;
     dim3 grid(M / C::W, oplanes);
+    if constexpr (2 * C::NT == 1024) {
+      // one line per tile and enough tiles to keep every SM's two groups busy: persistent two-group kernel
+      static int sms = 0, two = -1;
+      if (two < 0) { const char* e = getenv("EPR_COLS2"); two = e ? atoi(e) : 1; }
+      if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+      const int ntiles = (M / C::W) * oplanes;
+      if (two && !(mode == 1 && p->n_bins > 1) && ntiles >= 8 * sms) {
+        constexpr size_t smem2 = 3 * C::TILE + 32;
+        static bool attr2 = false;
+        if (!attr2) { cudaFuncSetAttribute(k_cols_tma2<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2); attr2 = true; }
+        k_cols_tma2<N><<<sms, 2 * C::NT, smem2, st>>>(p->map_spec, mo, p->lines, M, mode, scale, M / C::W, ntiles, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+        return true;
+      }
+    }
     if (mode == 1 && p->n_bins > 1)
       k_cols_tma<N, true><<<grid, C::NT, C::smem(true), st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
     else
