@@ -50,6 +50,7 @@ typedef struct {
   int output;         /* 0: τ (default); 1: phase φ of line out_bin; 2: total intensity Σ_s I_s */
   int out_bin;
   const double* mu_rel; /* γ_s override (relative attenuation per line, length n_bins) or NULL   R11 */
+  int nonlocal_wkb1;  /* non-local solver: add the local WKB1 term of Eq. (1) to the ray-map prediction (default 0)  R4 */
 } epr_options;
 
 void epr_default_options(epr_options* opt);

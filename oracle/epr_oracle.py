@@ -112,6 +112,18 @@ def lap5(g):
 # --------------------------------------------------------------------------------------
 # a1-L  local O(L^2) closure, Eq. (1)
 # --------------------------------------------------------------------------------------
+def wkb1_term(I, alpha):
+    """The diffraction-pressure (WKB1) term of Eq. (1), (eps²/4) ∂i(I ∂iQ) with Q = ∇²√I/√I
+    (Eq. (S15)): flux form on the 5-point stencils (R3), coefficient alpha²/4 in pixel units.
+    Eq. (1) SUBTRACTS it from the prediction."""
+    I = np.asarray(I, dtype=np.float64)
+    A = np.sqrt(I)
+    Q = lap5(A) / A
+    Fx = 0.5 * (_xp(I) + I) * (_xp(Q) - Q)   # flux through the face x+1/2
+    Fy = 0.5 * (_yp(I) + I) * (_yp(Q) - Q)   # flux through the face y+1/2
+    return 0.25 * alpha * alpha * ((Fx - _xm(Fx)) + (Fy - _ym(Fy)))
+
+
 def closure(I, a, alpha, order=2, wkb1=True):
     """P = I − eps ∂i(I ∂iφ) + (eps²/2) ∂i∂j(I ∂iφ ∂jφ) − (eps²/4) ∂i(I ∂iQ)   Eq. (1) PAPER.md:146.
 
@@ -130,12 +142,7 @@ def closure(I, a, alpha, order=2, wkb1=True):
         Sxy = I * gx * gy
         P = P + 0.5 * a * a * (d2x(Sxx) + d2y(Syy) + 2.0 * d0x(d0y(Sxy)))
         if wkb1:
-            A = np.sqrt(I)
-            Q = lap5(A) / A
-            Fx = 0.5 * (_xp(I) + I) * (_xp(Q) - Q)   # flux through the face x+1/2
-            Fy = 0.5 * (_yp(I) + I) * (_yp(Q) - Q)   # flux through the face y+1/2
-            div = (Fx - _xm(Fx)) + (Fy - _ym(Fy))
-            P = P - 0.25 * alpha * alpha * div
+            P = P - wkb1_term(I, alpha)
     return P
 
 
@@ -256,9 +263,12 @@ def project(T, lines: Lines, tol=1e-14, max_iter=200):
 # --------------------------------------------------------------------------------------
 # forward model  τ → Σ_s F_s[I_s]   Eq. (5)
 # --------------------------------------------------------------------------------------
-def forward(tau, lines: Lines, solver="local", order=2, wkb1=True, S=16.0):
+def forward(tau, lines: Lines, solver="local", order=2, wkb1=True, S=16.0, nonlocal_wkb1=False):
     """I_det ≈ Σ_s F_s[I_s], F_s ∈ {P_{m,s}, ℳ_s} (Eq. (5)) with
-    I_s = f_s e^{−γ_s τ} (Eq. (7)).  Returns (P_sum, [P_s], [(ux_s, uy_s)] or None)."""
+    I_s = f_s e^{−γ_s τ} (Eq. (7)).  Returns (P_sum, [P_s], [(ux_s, uy_s)] or None).
+    nonlocal_wkb1 (variant of reading R4, off by default): the ray map carries the WKB0 transport to all orders; the
+    leading wave-optics correction of Eq. (1), −(eps²/4) ∂i(I ∂iQ), is added to it as the same LOCAL term
+    ("when complemented by the second-order corrections", PAPER.md:173)."""
     Is = line_intensities(tau, lines)
     P_bins, maps = [], []
     for s in range(lines.n_bins):
@@ -267,7 +277,10 @@ def forward(tau, lines: Lines, solver="local", order=2, wkb1=True, S=16.0):
         else:
             ux, uy = ray_map(Is[s], lines.a[s], S)
             maps.append((ux, uy))
-            P_bins.append(splat(Is[s], ux, uy))
+            P_s = splat(Is[s], ux, uy)
+            if nonlocal_wkb1:
+                P_s = P_s - wkb1_term(Is[s], lines.alpha[s])
+            P_bins.append(P_s)
     P = np.sum(P_bins, axis=0)
     return P, P_bins, (maps if solver != "local" else None)
 
@@ -307,7 +320,7 @@ def max_shift(tau, lines: Lines):
 
 
 def retrieve(d, lines: Lines, solver="local", iterations=10, step=1.0, order=2, wkb1=True,
-             symbol=0, S=16.0, i_min=1e-6, tau0=None, history=None, shift_history=None):
+             symbol=0, S=16.0, i_min=1e-6, tau0=None, history=None, shift_history=None, nonlocal_wkb1=False):
     """The batched per-projection correction loop for one projection:
     per-line predictions and their sum, detector residual, positivity-weighted split, transport
     back (identity | adjoint Eq. (4)), per-line FFT-diagonal preconditioner update, projection
@@ -317,7 +330,7 @@ def retrieve(d, lines: Lines, solver="local", iterations=10, step=1.0, order=2, 
     n = lines.n_bins
     for _ in range(iterations):
         Is = line_intensities(tau, lines)
-        P, P_bins, maps = forward(tau, lines, solver, order, wkb1, S)
+        P, P_bins, maps = forward(tau, lines, solver, order, wkb1, S, nonlocal_wkb1)
         e = d - P
         if history is not None:
             history.append(float(np.sqrt(np.mean(e * e))))

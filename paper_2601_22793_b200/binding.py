@@ -26,7 +26,7 @@ class Options(C.Structure):
     """Mirror of `epr_options` (include/epr.h)."""
     _fields_ = [("order", C.c_int), ("wkb1", C.c_int), ("symbol", C.c_int), ("max_shift_px", C.c_float),
                 ("i_min", C.c_float), ("newton_iters", C.c_int), ("init", C.c_int), ("output", C.c_int),
-                ("out_bin", C.c_int), ("mu_rel", C.POINTER(C.c_double))]
+                ("out_bin", C.c_int), ("mu_rel", C.POINTER(C.c_double)), ("nonlocal_wkb1", C.c_int)]
 
 
 def lib_path():
@@ -137,7 +137,7 @@ class Plan:
 
 def epr_plan(nx, ny, pixel_m, L_m, energy_keV, weight, delta_over_beta, solver="local", max_batch=1, **opts):
     """epr_plan of include/epr.h.  `opts`: fields of epr_options (order, wkb1, symbol, max_shift_px, i_min,
-    newton_iters, init, output, out_bin, mu_rel)."""
+    newton_iters, init, output, out_bin, mu_rel, nonlocal_wkb1)."""
     lib = load_library()
     E = np.ascontiguousarray(np.atleast_1d(energy_keV), dtype=np.float64)
     w = np.ascontiguousarray(np.atleast_1d(weight), dtype=np.float64)

@@ -24,9 +24,9 @@ static const double HC_KEV_M = 1.2398419843e-9;
     if (e_ != cudaSuccess) FAIL(p, EPR_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
   } while (0)
 // Kernel families, for launch counting and the optional per-kernel CUDA-event timing (epr_profile_*).
-enum { K_FWD_LOCAL = 0, K_SPLAT, K_RESIDUAL, K_GATHER, K_ROWS_R2C, K_COLS, K_ROWS_C2R, K_PRED_OUT, K_OUTPUT, K_RESAMPLE, K_DIAG, K_COUNT };
+enum { K_FWD_LOCAL = 0, K_SPLAT, K_RESIDUAL, K_GATHER, K_ROWS_R2C, K_COLS, K_ROWS_C2R, K_PRED_OUT, K_OUTPUT, K_RESAMPLE, K_DIAG, K_WKB1, K_COUNT };
 static const char* const K_NAMES[K_COUNT] = {"k_forward_local", "k_splat", "k_residual", "k_gather", "k_rows_r2c",
-                                              "k_cols", "k_rows_c2r", "k_pred_out", "k_output", "k_resample", "k_diagnostics"};
+                                              "k_cols", "k_rows_c2r", "k_pred_out", "k_output", "k_resample", "k_diagnostics", "k_wkb1_sub"};
 struct EprProf {
   struct Rec { int tag; cudaEvent_t a, b; };
   std::vector<Rec> recs;
@@ -54,7 +54,7 @@ struct EprProf {
 extern "C" void epr_default_options(epr_options* o) {
   if (!o) return;
   o->order = 2; o->wkb1 = 1; o->symbol = 0; o->max_shift_px = 16.f; o->i_min = 1e-6f; o->newton_iters = 4;
-  o->init = 0; o->output = 0; o->out_bin = 0; o->mu_rel = NULL;
+  o->init = 0; o->output = 0; o->out_bin = 0; o->mu_rel = NULL; o->nonlocal_wkb1 = 0;
 }
 
 extern "C" const char* epr_version(void) { return "epr-b200 0.1 (sm_100a)"; }
@@ -335,6 +335,7 @@ extern "C" epr_status epr_forward(epr_plan_t p, int batch, const float* tau, flo
     if ((st = ensure_raymap(p)) != EPR_OK) return st;
     KL(p, K_SPLAT, cs, epr_launch_splat(p, batch, tau, NULL, NULL, p->raymap, p->pred, 0, NULL, cs));
     p->launches += 1;                                  // k_grad_blockmax, launched ahead of the splat
+    if (p->opt.nonlocal_wkb1) KL(p, K_WKB1, cs, epr_launch_wkb1_sub(p, batch, tau, p->pred, cs));
     KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, P_sum, P_bins, cs));
     p->raymap_batch = batch;
   }
@@ -413,7 +414,12 @@ static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* ta
       if (p->diag && it < p->diag_cap)
         KL(p, K_DIAG, cs, epr_launch_diagnostics(p, nb, tau, p->res, p->diag + ((size_t)b_first * p->diag_cap + it) * 2, p->diag_cap * 2, cs));
     } else {
-      if (p->n_bins == 1) {
+      if (p->opt.nonlocal_wkb1) {                      // variant: splat, WKB1 term, then the separate residual kernel
+        KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->pred, 0, NULL, cs));
+        p->launches += 1;
+        KL(p, K_WKB1, cs, epr_launch_wkb1_sub(p, nb, tau, p->pred, cs));
+        KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, p->res, cs));
+      } else if (p->n_bins == 1) {
         KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->res, 2, d, cs));       // a0 + a1-N + a2 fused
         p->launches += 1;                                  // k_grad_blockmax, launched ahead of the splat
       } else {

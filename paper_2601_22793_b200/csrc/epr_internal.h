@@ -116,4 +116,6 @@ cudaError_t epr_launch_downsample(const epr_plan_s* p, int batch, int m, const f
 // diag[b·stride + 0] = RMS_px(Σ_s es[b][s]), diag[b·stride + 1] = max_s |c_s| · max|D⁰τ| (unclamped shift, px)
 cudaError_t epr_launch_diagnostics(const epr_plan_s* p, int batch, const float* tau, const float* es, float* diag,
                                    int stride, cudaStream_t st);
+// pred[b][s] −= f_s (α_s²/4) ∂i(Î ∂iQ): the WKB1 term of Eq. (1) for the non-local forward (opt.nonlocal_wkb1)
+cudaError_t epr_launch_wkb1_sub(const epr_plan_s* p, int batch, const float* tau, float* pred, cudaStream_t st);
 cudaError_t epr_launch_output(const epr_plan_s* p, int batch, const float* tau, float* out, cudaStream_t st);

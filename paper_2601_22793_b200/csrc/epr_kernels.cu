@@ -1166,3 +1166,55 @@ cudaError_t epr_launch_diagnostics(const epr_plan_s* p, int batch, const float* 
   k_diag_final<<<batch, 256, 0, st>>>(plane, (p->nx / 16) * (p->ny / 16), cmax, p->diag_partial, p->gmax, diag, stride);
   return cudaGetLastError();
 }
+
+// =====================================================================================================
+// Variant of reading R4 (opt.nonlocal_wkb1, off by default): the leading wave-optics correction of Eq. (1)
+// PAPER.md:146, −(ε²/4) ∂i(I ∂iQ) with Q = ∇²√I/√I (Eq. (S15)), added to the ray-map prediction as the
+// same LOCAL term ("when complemented by the second-order corrections"):
+//   pred[b][s] −= f_s (α_s²/4) Σ_i D⁻_i( ½(Î[+1] + Î) D⁺_i Q ),  Î = A², A = 1 + Ad, Ad = expm1(−γ_s τ/2), Q = ∇²₅Ad / A.
+// The paper finds the term "consistently negligible"; this is a plain tile kernel, not a tuned one.
+// CTA = 32 x 8 pixels; Ad on the tile + 2, Q on the tile + 1, both in shared memory.
+// =====================================================================================================
+#define WK_TX 32
+#define WK_TY 8
+__global__ void __launch_bounds__(256) k_wkb1_sub(EprLines L, int nx, int ny, const float* __restrict__ tau,
+                                                  float* __restrict__ pred) {
+  __shared__ float s_ad[WK_TY + 4][WK_TX + 4], s_q[WK_TY + 2][WK_TX + 2];
+  const int tid = threadIdx.x, b = blockIdx.z;
+  const int x0 = blockIdx.x * WK_TX, y0 = blockIdx.y * WK_TY;
+  const unsigned plane = (unsigned)nx * (unsigned)ny;
+  const float* tb = tau + (size_t)b * plane;
+  for (int s = 0; s < L.n_bins; ++s) {
+    const float cg = -0.5f * L.gamma[s];
+    __syncthreads();                                   // the previous line's tiles are no longer read
+    for (int i = tid; i < (WK_TY + 4) * (WK_TX + 4); i += 256) {
+      const int ly = i / (WK_TX + 4), lx = i - ly * (WK_TX + 4);
+      s_ad[ly][lx] = epr_expm1(cg * __ldg(tb + (unsigned)wrapm(y0 - 2 + ly, ny) * nx + wrapm(x0 - 2 + lx, nx)));
+    }
+    __syncthreads();
+    for (int i = tid; i < (WK_TY + 2) * (WK_TX + 2); i += 256) {
+      const int ly = i / (WK_TX + 2), lx = i - ly * (WK_TX + 2);
+      const float ac = s_ad[ly + 1][lx + 1];
+      s_q[ly][lx] = __fdividef(((s_ad[ly + 1][lx + 2] - ac) + (s_ad[ly + 1][lx] - ac)) +
+                               ((s_ad[ly][lx + 1] - ac) + (s_ad[ly + 2][lx + 1] - ac)), 1.f + ac);
+    }
+    __syncthreads();
+    const int tx = tid & (WK_TX - 1), ty = tid / WK_TX;
+    const int gx = x0 + tx, gy = y0 + ty;
+    if (gx < nx && gy < ny) {
+      auto I = [&](int dy, int dx) { const float a = 1.f + s_ad[ty + 2 + dy][tx + 2 + dx]; return a * a; };
+      auto Q = [&](int dy, int dx) { return s_q[ty + 1 + dy][tx + 1 + dx]; };
+      const float Ic = I(0, 0), Qc = Q(0, 0);
+      const float fxp = 0.5f * (I(0, 1) + Ic) * (Q(0, 1) - Qc), fxm = 0.5f * (Ic + I(0, -1)) * (Qc - Q(0, -1));
+      const float fyp = 0.5f * (I(1, 0) + Ic) * (Q(1, 0) - Qc), fym = 0.5f * (Ic + I(-1, 0)) * (Qc - Q(-1, 0));
+      float* o = pred + ((size_t)b * L.n_bins + s) * plane + (unsigned)gy * nx + gx;
+      *o -= L.f[s] * L.q4[s] * ((fxp - fxm) + (fyp - fym));
+    }
+  }
+}
+
+cudaError_t epr_launch_wkb1_sub(const epr_plan_s* p, int batch, const float* tau, float* pred, cudaStream_t st) {
+  dim3 grid((p->nx + WK_TX - 1) / WK_TX, (p->ny + WK_TY - 1) / WK_TY, batch);
+  k_wkb1_sub<<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, tau, pred);
+  return cudaGetLastError();
+}

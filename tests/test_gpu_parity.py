@@ -403,6 +403,32 @@ def test_retrieve_nonlocal_grids_smaller_than_a_tile(E, ny, nx, n_lines):
     assert rel_l2(got, ref) < TOL_PHASE
 
 
+def test_nonlocal_wkb1_variant(E):
+    """opt.nonlocal_wkb1 (variant of R4): forward model and retrieval with the WKB1 term of Eq. (1) added
+    to the ray-map prediction, at a δ/β small enough for the term to matter."""
+    import torch
+    ny, nx, S = 160, 96, 8.0
+    en, wt, db = np.array([80.0, 100.0, 120.0]), np.array([0.3, 0.4, 0.3]), np.array([8.0, 10.0, 12.0])
+    lines = O.derive_lines(6.5e-6, 20.0, en, wt, db)
+    tau = _tau_field(ny, nx, 5, amp=0.3)[None]
+    plan = E.epr_plan(nx, ny, 6.5e-6, 20.0, en, wt, db, "nonlocal", max_batch=1, max_shift_px=S, nonlocal_wkb1=1)
+    P = torch.empty((1, ny, nx), device="cuda")
+    Pb = torch.empty((1, 3, ny, nx), device="cuda")
+    E.epr_forward(plan, _dev(tau), P, Pb)
+    ref, ref_bins, _ = O.forward(tau[0].astype(np.float64), lines, "nonlocal", S=S, nonlocal_wkb1=True)
+    plain, _, _ = O.forward(tau[0].astype(np.float64), lines, "nonlocal", S=S)
+    assert rel_l2(ref, plain) > 100 * TOL_OP                         # the term is far above the tolerance here
+    assert rel_l2(P.cpu().numpy()[0], ref) < TOL_OP
+    for s in range(3):
+        assert rel_l2(Pb.cpu().numpy()[0, s], ref_bins[s]) < TOL_OP
+    d = np.float32(ref + 0.002 * np.random.default_rng(3).normal(size=ref.shape))[None]
+    out = torch.empty((1, ny, nx), device="cuda")
+    E.epr_retrieve(plan, _dev(d), out, 5, 0.4)
+    plan.destroy()
+    want = O.retrieve(d[0].astype(np.float64), lines, "nonlocal", 5, 0.4, S=S, nonlocal_wkb1=True)
+    assert rel_l2(out.cpu().numpy()[0], want) < TOL_PHASE
+
+
 def test_retrieve_outputs_and_host_path(E):
     import torch
     w = make_workload("C1")

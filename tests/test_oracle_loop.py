@@ -147,3 +147,23 @@ def test_max_shift_closed_form_and_history():
     per_line = [max(np.max(np.abs(l2.a[s] * l2.gamma[s] * O.d0x(t2))), np.max(np.abs(l2.a[s] * l2.gamma[s] * O.d0y(t2))))
                 for s in range(2)]
     assert abs(O.max_shift(t2, l2) - max(per_line)) < 1e-12             # D0 ln I_s = −γ_s D0 τ (Eq. (7))
+
+
+def test_nonlocal_wkb1_variant_keeps_mass_and_vanishes_for_exponentials():
+    """Variant of R4: the WKB1 term of Eq. (1) added to the ray-map prediction.  It is a discrete
+    divergence, so the total intensity is still conserved; for I = exp(cx + dy) the quantum potential Q is constant
+    (interior) and the term vanishes; and it is exactly the term the local closure subtracts."""
+    E = np.array([80.0, 120.0])
+    lines = O.derive_lines(6.5e-6, 8.0, E, [0.4, 0.6], [8.0, 12.0])          # small δ/β: α²/4 = (a/db)² is not small
+    tau = 0.3 * (1.0 + _smooth(24, 32, 11))
+    P0, b0, _ = O.forward(tau, lines, "nonlocal", S=8.0)
+    P1, b1, _ = O.forward(tau, lines, "nonlocal", S=8.0, nonlocal_wkb1=True)
+    Is = O.line_intensities(tau, lines)
+    assert np.linalg.norm(P1 - P0) > 1e-4 * np.linalg.norm(P0 - np.sum(Is, axis=0))   # the variant does something
+    for s in range(2):
+        assert abs(b1[s].sum() - Is[s].sum()) < 1e-12 * Is[s].sum()
+        loc = O.closure(Is[s], lines.a[s], lines.alpha[s], 2, False) - O.closure(Is[s], lines.a[s], lines.alpha[s], 2, True)
+        assert np.max(np.abs((b0[s] - b1[s]) - loc)) < 1e-13
+    y, x = np.meshgrid(np.arange(16.0), np.arange(16.0), indexing="ij")
+    W = O.wkb1_term(np.exp(0.03 * x - 0.02 * y), 3.0)
+    assert np.max(np.abs(W[3:-3, 3:-3])) < 1e-12
