@@ -213,15 +213,19 @@ def test_full_size_periodic_tiling(E, name):
     lines = O.derive_lines(w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta)
     ref = O.retrieve(w.d[0].astype(np.float64), lines, w.solver, w.iterations, w.step, S=w.max_shift_px)
     big = np.tile(w.d[0], (4, 4))[None]
-    d = _dev(np.concatenate([big, big]))
+    # one line: a batch of 8 selects the kernels bench.py's batch of 32 runs (128-row march, two-group column kernel:
+    # both need a launch that fills the GPU); 8 lines: a batch of 2 already does
+    nbatch = 8 if w.n_bins == 1 else 2
+    d = _dev(np.concatenate([big] * nbatch))
     plan = E.epr_plan(2048, 2048, w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
-                      max_batch=2, max_shift_px=w.max_shift_px)
+                      max_batch=nbatch, max_shift_px=w.max_shift_px)
     out = torch.empty_like(d)
     E.epr_retrieve(plan, d, out, w.iterations, w.step)
     got = out.cpu().numpy()
     plan.destroy()
     assert rel_l2(got[0], np.tile(ref, (4, 4))) < TOL_PHASE
-    assert np.array_equal(got[0], got[1])                      # batch entries are independent and deterministic
+    for j in range(1, nbatch):
+        assert np.array_equal(got[0], got[j])                  # batch entries are independent and deterministic
 
 
 def test_retrieve_graph_replay_matches_eager(E):
