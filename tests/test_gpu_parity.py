@@ -366,6 +366,13 @@ def test_diagnostics_history(E, name, n):
     E.epr_set_diagnostics(plan, diag)
     E.epr_retrieve(plan, d, out, w.iterations, w.step)
     got = diag.cpu().numpy()
+    # the host path works through the batch in chunks: every chunk must land in its own rows of the array
+    diag_h = torch.zeros_like(diag)
+    E.epr_set_diagnostics(plan, diag_h)
+    dh = torch.from_numpy(w.d).pin_memory()
+    oh = torch.empty_like(dh).pin_memory()
+    E.epr_retrieve_host(plan, dh, oh, w.iterations, w.step)
+    assert torch.equal(diag_h, diag) and torch.equal(oh.cuda(), out)
     E.epr_set_diagnostics(plan, None)
     out2 = torch.empty_like(d)
     E.epr_retrieve(plan, d, out2, w.iterations, w.step)
