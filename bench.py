@@ -133,6 +133,15 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def override_lines(w, n):
+    """Retrieval with n spectral lines on the config's detector data (only the spectral discretisation the retrieval
+    assumes changes): E = linspace(60, 140) keV, Gaussian weights (sigma 20 keV), delta/beta proportional to E."""
+    db100 = float(w.delta_over_beta[np.argmin(np.abs(w.energy_keV - 100.0))])
+    e = np.linspace(60.0, 140.0, n) if n > 1 else np.array([100.0])
+    wt = np.exp(-0.5 * ((e - 100.0) / 20.0) ** 2)
+    w.energy_keV, w.weight, w.delta_over_beta = e, wt / wt.sum(), db100 * e / 100.0
+
+
 def fine_shift_clamp(w, m):
     """S in pixels of the grid refined m times (the library accepts at most 30)."""
     return float(min(30.0, m * w.max_shift_px))
@@ -155,6 +164,8 @@ def run_reference(args, rank):
         return
     from epr_inputs import make_workload
     w = make_workload(args.config, batch=1, distinct=1)
+    if args.lines > 0:
+        override_lines(w, args.lines)
     for _ in range(args.warmup):
         oracle_time_one(w, m=args.oversample)
     t = [oracle_time_one(w, m=args.oversample) for _ in range(args.steps)]
@@ -182,6 +193,9 @@ def main():
     ap.add_argument("--distinct", type=int, default=2, help="distinct simulated projections (rest: new noise only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--lines", type=int, default=0,
+                    help="retrieve with this many spectral lines (60-140 keV, Gaussian weights) instead of the config's own "
+                         "discretisation, e.g. --config C2 --lines 5: the paper's 'local L2 poly' rows (PAPER.md:116-119)")
     ap.add_argument("--oversample", type=int, default=1,
                     help="run the loop on the grid refined this many times (PAPER.md:79; epr_retrieve_oversampled)")
     args = ap.parse_args()
@@ -208,6 +222,8 @@ def main():
 
     B = args.batch
     w = make_workload(args.config, batch=B, distinct=min(args.distinct, B))
+    if args.lines > 0:
+        override_lines(w, args.lines)
     if world > 1:                                   # every rank gets its own noise realisations
         rng = np.random.default_rng(4000 + rank)
         w.d = np.ascontiguousarray(w.d[rng.permutation(B)])

@@ -9,160 +9,11 @@
 // a2, the detector residual (a3 is the identity for the local solver).
 //   P_s/f_s − 1 = J − a ∇²₅J + (a²/2)[D²x(Î gx²) + D²y(Î gy²) + 2 D⁰xD⁰y(Î gx gy)] − (α²/4) Σ_i D⁻_i(Ī_i D⁺_i Q)
 //   with A = exp(−γτ/2) = 1 + Ad,  Î = I/f = A²,  J = Î − 1 = Ad(2+Ad),  g = −γ D⁰τ,  Q = ∇²₅A / A.
-//   FUSE (n_bins == 1): out = e = (d − 1) − (P − 1);  otherwise out[b][s] = P_s − f_s for k_residual.
-// One CTA = 128x8 output pixels, each thread a strip of 4 in x.  Stage 1: τ and Ad (halo 2) in shared memory;
-// stage 2: Î gx², Î gy², Î gx gy, Q (halo 1); stage 3: the closure from float4 shared loads.  The kernel is
-// bound by fp32 issue (≈ 100 instructions per pixel), not by HBM (12 B/px): see DESIGN.md.
+//   One line: out = e = (d − 1) − (P − 1);  several lines: out[b][s] = P_s − f_s for k_residual.
+// The kernel is bound by fp32 issue (≈ 90 instructions per pixel and line), not by HBM: see DESIGN.md.
 // =====================================================================================================
-#define FL_TX 128
-#define FL_TY 8
-#define FL_PW (FL_TX + 8)            // row pitch: 4 columns of (aligned) halo on each side, 2 used
-#define FL_R1 (FL_TY + 4)            // rows with halo 2
-#define FL_R2 (FL_TY + 2)            // rows with halo 1
-
-struct Strip6 { float m, v0, v1, v2, v3, p; };     // values at columns c-1, c..c+3, c+4 of one row
-__device__ __forceinline__ Strip6 ld6(const float* row, int c) {
-  const float4 v = *reinterpret_cast<const float4*>(row + c);
-  return Strip6{row[c - 1], v.x, v.y, v.z, v.w, row[c + 4]};
-}
-__device__ __forceinline__ float4 ld4(const float* row, int c) { return *reinterpret_cast<const float4*>(row + c); }
-
-template <bool FUSE>
-__global__ void __launch_bounds__(256) k_forward_local(EprLines L, int nx, int ny, int order, int wkb1,
-                                                       const float* __restrict__ tau, const float* __restrict__ d,
-                                                       float* __restrict__ out) {
-  __shared__ __align__(16) float s_tau[FL_R1][FL_PW], s_ad[FL_R1][FL_PW];
-  __shared__ __align__(16) float s_sxx[FL_R2][FL_PW], s_syy[FL_R2][FL_PW], s_sxy[FL_R2][FL_PW], s_q[FL_R2][FL_PW];
-  const int b = blockIdx.z, tid = threadIdx.x;
-  const int x0 = blockIdx.x * FL_TX, y0 = blockIdx.y * FL_TY;
-  const unsigned plane = (unsigned)nx * (unsigned)ny;
-  const float* tb = tau + (size_t)b * plane;
-
-  // stage 0: τ tile, rows y0-2 .. y0+TY+1, columns x0-4 .. x0+TX+3 as whole float4 groups (nx % 4 == 0)
-  for (int i = tid; i < FL_R1 * (FL_PW / 4); i += 256) {
-    const int ly = i / (FL_PW / 4), g = i - ly * (FL_PW / 4);
-    const int gy = wrapm(y0 - 2 + ly, ny), gx = wrapm(x0 - 4 + 4 * g, nx);
-    *reinterpret_cast<float4*>(&s_tau[ly][4 * g]) = __ldg(reinterpret_cast<const float4*>(tb + (unsigned)gy * nx + gx));
-  }
-  for (int s = 0; s < L.n_bins; ++s) {
-    const float gam = L.gamma[s], cg = -0.5f * gam;
-    __syncthreads();
-    // stage 1: Ad = expm1(−γτ/2)
-    for (int i = tid; i < FL_R1 * (FL_PW / 4); i += 256) {
-      const int ly = i / (FL_PW / 4), g = i - ly * (FL_PW / 4);
-      const float4 t = *reinterpret_cast<const float4*>(&s_tau[ly][4 * g]);
-      *reinterpret_cast<float4*>(&s_ad[ly][4 * g]) =
-          make_float4(epr_expm1(cg * t.x), epr_expm1(cg * t.y), epr_expm1(cg * t.z), epr_expm1(cg * t.w));
-    }
-    __syncthreads();
-    if (order == 2) {
-      // stage 2 on rows 1..TY+2 (halo 1): interior float4 groups 1..TX/4, plus the two halo columns 3 and TX+4
-      for (int i = tid; i < FL_R2 * (FL_TX / 4 + 1); i += 256) {
-        const int r2 = i / (FL_TX / 4 + 1), g = i - r2 * (FL_TX / 4 + 1);
-        const int ly = r2 + 1;
-        if (g < FL_TX / 4) {
-          const int c = 4 * (g + 1);
-          const Strip6 t0 = ld6(s_tau[ly], c), a0 = ld6(s_ad[ly], c);
-          const float4 tn = ld4(s_tau[ly - 1], c), ts = ld4(s_tau[ly + 1], c);
-          const float4 an = ld4(s_ad[ly - 1], c), as = ld4(s_ad[ly + 1], c);
-          float4 oxx, oyy, oxy, oq;
-#define ST2(o, tw, te, tnn, tss, aw, ac, ae, ann, ass)                                  \
-          {                                                                              \
-            const float gx = cg * ((te) - (tw)), gy = cg * ((tss) - (tnn));              \
-            const float A = 1.f + (ac), I = A * A, igx = I * gx;                          \
-            oxx.o = igx * gx; oxy.o = igx * gy; oyy.o = I * gy * gy;                      \
-            oq.o = __fdividef((((ae) - (ac)) + ((aw) - (ac))) + (((ann) - (ac)) + ((ass) - (ac))), A); \
-          }
-          ST2(x, t0.m, t0.v1, tn.x, ts.x, a0.m, a0.v0, a0.v1, an.x, as.x)
-          ST2(y, t0.v0, t0.v2, tn.y, ts.y, a0.v0, a0.v1, a0.v2, an.y, as.y)
-          ST2(z, t0.v1, t0.v3, tn.z, ts.z, a0.v1, a0.v2, a0.v3, an.z, as.z)
-          ST2(w, t0.v2, t0.p, tn.w, ts.w, a0.v2, a0.v3, a0.p, an.w, as.w)
-          *reinterpret_cast<float4*>(&s_sxx[r2][c]) = oxx;
-          *reinterpret_cast<float4*>(&s_syy[r2][c]) = oyy;
-          *reinterpret_cast<float4*>(&s_sxy[r2][c]) = oxy;
-          *reinterpret_cast<float4*>(&s_q[r2][c]) = oq;
-        } else {
-#pragma unroll
-          for (int side = 0; side < 2; ++side) {
-            const int c = side ? FL_TX + 4 : 3;
-            const float gx = cg * (s_tau[ly][c + 1] - s_tau[ly][c - 1]), gy = cg * (s_tau[ly + 1][c] - s_tau[ly - 1][c]);
-            const float ac = s_ad[ly][c], A = 1.f + ac, I = A * A, igx = I * gx;
-            s_sxx[r2][c] = igx * gx; s_sxy[r2][c] = igx * gy; s_syy[r2][c] = I * gy * gy;
-            s_q[r2][c] = __fdividef(((s_ad[ly][c + 1] - ac) + (s_ad[ly][c - 1] - ac)) + ((s_ad[ly - 1][c] - ac) + (s_ad[ly + 1][c] - ac)), A);
-          }
-        }
-      }
-    }
-    __syncthreads();
-    // stage 3: one strip of 4 outputs per thread (TX/4 = 32 strips per row x TY rows = 256)
-    {
-      const int ty = tid >> 5, c = 4 * ((tid & 31) + 1);
-      const int gx0 = x0 + c - 4, gyy = y0 + ty;
-      if (gx0 < nx && gyy < ny) {
-        const int l1 = ty + 2, l2 = ty + 1;
-        const Strip6 a0 = ld6(s_ad[l1], c);
-        const float4 an = ld4(s_ad[l1 - 1], c), as = ld4(s_ad[l1 + 1], c);
-        const float av[6] = {a0.m, a0.v0, a0.v1, a0.v2, a0.v3, a0.p};
-        const float anv[4] = {an.x, an.y, an.z, an.w}, asv[4] = {as.x, as.y, as.z, as.w};
-        float v[4];
-        float Jr[6], Ir[6];
-#pragma unroll
-        for (int k = 0; k < 6; ++k) { Jr[k] = av[k] * (2.f + av[k]); Ir[k] = Jr[k] + 1.f; }
-        float Jn[4], Js[4];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) { Jn[k] = anv[k] * (2.f + anv[k]); Js[k] = asv[k] * (2.f + asv[k]); }
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const float Jc = Jr[k + 1];
-          const float lapJ = ((Jr[k + 2] - Jc) + (Jr[k] - Jc)) + ((Jn[k] - Jc) + (Js[k] - Jc));
-          v[k] = fmaf(-L.a[s], lapJ, Jc);
-        }
-        if (order == 2) {
-          const Strip6 xx = ld6(s_sxx[l2], c);
-          const float4 yn = ld4(s_syy[l2 - 1], c), yc = ld4(s_syy[l2], c), ys = ld4(s_syy[l2 + 1], c);
-          const Strip6 xyn = ld6(s_sxy[l2 - 1], c), xys = ld6(s_sxy[l2 + 1], c);
-          const float xxv[6] = {xx.m, xx.v0, xx.v1, xx.v2, xx.v3, xx.p};
-          const float ynv[4] = {yn.x, yn.y, yn.z, yn.w}, ycv[4] = {yc.x, yc.y, yc.z, yc.w}, ysv[4] = {ys.x, ys.y, ys.z, ys.w};
-          const float xnv[6] = {xyn.m, xyn.v0, xyn.v1, xyn.v2, xyn.v3, xyn.p}, xsv[6] = {xys.m, xys.v0, xys.v1, xys.v2, xys.v3, xys.p};
-#pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            const float sxx = (xxv[k + 2] - xxv[k + 1]) + (xxv[k] - xxv[k + 1]);
-            const float syy = (ysv[k] - ycv[k]) + (ynv[k] - ycv[k]);
-            const float sxy2 = 0.5f * ((xsv[k + 2] - xsv[k]) - (xnv[k + 2] - xnv[k]));      // 2 · D⁰xD⁰y
-            v[k] = fmaf(L.a2h[s], (sxx + syy) + sxy2, v[k]);
-          }
-          if (wkb1) {
-            const Strip6 q0 = ld6(s_q[l2], c);
-            const float4 qn = ld4(s_q[l2 - 1], c), qs = ld4(s_q[l2 + 1], c);
-            const float qv[6] = {q0.m, q0.v0, q0.v1, q0.v2, q0.v3, q0.p};
-            const float qnv[4] = {qn.x, qn.y, qn.z, qn.w}, qsv[4] = {qs.x, qs.y, qs.z, qs.w};
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-              const float Ic = Ir[k + 1], Qc = qv[k + 1];
-              const float In = Jn[k] + 1.f, Is = Js[k] + 1.f;
-              const float div = 0.5f * (((Ir[k + 2] + Ic) * (qv[k + 2] - Qc) - (Ic + Ir[k]) * (Qc - qv[k]))
-                                        + ((Is + Ic) * (qsv[k] - Qc) - (Ic + In) * (Qc - qnv[k])));
-              v[k] = fmaf(-L.q4[s], div, v[k]);
-            }
-          }
-        }
-        const unsigned o = (unsigned)gyy * nx + gx0;
-        if (FUSE) {
-          const float4 dd = __ldg(reinterpret_cast<const float4*>(d + (size_t)b * plane + o));
-          *reinterpret_cast<float4*>(out + (size_t)b * plane + o) =
-              make_float4((dd.x - 1.f) - v[0], (dd.y - 1.f) - v[1], (dd.z - 1.f) - v[2], (dd.w - 1.f) - v[3]);
-        } else {
-          const float f = L.f[s];
-          *reinterpret_cast<float4*>(out + ((size_t)b * L.n_bins + s) * plane + o) =
-              make_float4(f * v[0], f * v[1], f * v[2], f * v[3]);
-        }
-      }
-    }
-  }
-}
-
 // -----------------------------------------------------------------------------------------------------
-// k_local_march — the fused closure + residual for one spectral line (the hot configuration), register marching.
+// k_local_march — the closure (fused with the residual for one spectral line, the hot configuration), register marching.
 // A warp owns a band of 128 columns (lane l: 4 consecutive pixels; lanes 0 and 31 are halo providers, lanes
 // 1..30 write 120 output columns) and marches down LM_MR output rows.  Every row of τ and d is fetched ONCE
 // (cp.async ring, see below); all x-neighbours come from warp shuffles and all y-neighbours from rolling
@@ -217,7 +68,8 @@ __device__ __forceinline__ W6 window(const F4& v) {
   return r;
 }
 
-template <int LM_MR, int LM_WPC>
+// PRED (several lines): blockIdx.z = projection · n_bins + line; out[b][s] = P_s − f_s = f_s v for k_residual, no d.
+template <int LM_MR, int LM_WPC, bool PRED>
 __global__ void __launch_bounds__(32 * LM_WPC) k_local_march(EprLines L, int nx, int ny, int order, int wkb1,
                                                      const float* __restrict__ tau, const float* __restrict__ d,
                                                      float* __restrict__ out) {
@@ -227,13 +79,15 @@ __global__ void __launch_bounds__(32 * LM_WPC) k_local_march(EprLines L, int nx,
   if (band * LM_BW >= nx) return;
   const int y0 = blockIdx.y * LM_MR;
   const unsigned plane = (unsigned)nx * (unsigned)ny;
-  const float* tb = tau + (size_t)blockIdx.z * plane;
-  const float* db = d + (size_t)blockIdx.z * plane;
+  const int ls = PRED ? (int)(blockIdx.z % L.n_bins) : 0;                  // spectral line
+  const size_t bz = PRED ? blockIdx.z / L.n_bins : blockIdx.z;             // projection
+  const float* tb = tau + bz * plane;
+  const float* db = PRED ? nullptr : d + bz * plane;
   float* ob = out + (size_t)blockIdx.z * plane;
   const int xw = wrapm(xs, nx);
   const bool writer = lane >= 1 && lane <= 30 && xs < nx;
-  const float cg = -0.5f * L.gamma[0], a = L.a[0], q4 = L.q4[0];
-  const float c2 = L.a2h[0] * cg * cg;
+  const float cg = -0.5f * L.gamma[ls], a = L.a[ls], q4 = L.q4[ls], fs = L.f[ls];
+  const float c2 = L.a2h[ls] * cg * cg;
   const bool o2 = order == 2, wk = o2 && wkb1;
 
   F4 t_a, t_b, t_c, A_b, dA_lo, J_a, J_b, H_a, Q_a, ACC_a, ACC_b;
@@ -247,7 +101,7 @@ __global__ void __launch_bounds__(32 * LM_WPC) k_local_march(EprLines L, int nx,
   // row pointers advance by one row per request (τ rows wrap periodically, d / out rows never leave the plane)
   int yr = wrapm(y0 - 2, ny);
   const float* tp = tb + (unsigned)yr * nx + xw;
-  const float* dp = db + (unsigned)y0 * nx + xs;
+  const float* dp = PRED ? nullptr : db + (unsigned)y0 * nx + xs;
   float* op = ob + (unsigned)y0 * nx + xs;
 #pragma unroll
   for (int i = 0; i < LM_D - 1; ++i) {
@@ -266,7 +120,7 @@ __global__ void __launch_bounds__(32 * LM_WPC) k_local_march(EprLines L, int nx,
         cp_async16(&ring_t[sl][tid], tp);
         tp += nx;
         if (++yr == ny) { yr = 0; tp -= plane; }
-        if (ahead >= 4) {                            // d row of output row y0 − 4 + ahead
+        if (!PRED && ahead >= 4) {                   // d row of output row y0 − 4 + ahead
           if (y0 - 4 + ahead < ny && writer) cp_async16(&ring_d[sl][tid], dp);
           dp += nx;
         }
@@ -274,7 +128,9 @@ __global__ void __launch_bounds__(32 * LM_WPC) k_local_march(EprLines L, int nx,
       cp_async_commit();
       cp_async_wait<LM_D - 1>();
     }
-    const float4 tv = ring_t[step % LM_D][tid], dd = ring_d[step % LM_D][tid];
+    const float4 tv = ring_t[step % LM_D][tid];
+    float4 dd = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (!PRED) dd = ring_d[step % LM_D][tid];
     // ---- rotate ----
     t_a = t_b; t_b = t_c;
     t_c.v[0] = tv.x; t_c.v[1] = tv.y; t_c.v[2] = tv.z; t_c.v[3] = tv.w;
@@ -360,9 +216,14 @@ __global__ void __launch_bounds__(32 * LM_WPC) k_local_march(EprLines L, int nx,
     // ---- output row o = n − 2 = m − 1 ----
     const int o = n - 2;
     if (step >= 4 && o < ny && writer) {
-      *reinterpret_cast<float4*>(op + (unsigned)(step - 4) * nx) =
-          make_float4((dd.x - 1.f) - (J_a.v[0] + ACC_a.v[0]), (dd.y - 1.f) - (J_a.v[1] + ACC_a.v[1]),
-                      (dd.z - 1.f) - (J_a.v[2] + ACC_a.v[2]), (dd.w - 1.f) - (J_a.v[3] + ACC_a.v[3]));
+      if (PRED)
+        *reinterpret_cast<float4*>(op + (unsigned)(step - 4) * nx) =
+            make_float4(fs * (J_a.v[0] + ACC_a.v[0]), fs * (J_a.v[1] + ACC_a.v[1]), fs * (J_a.v[2] + ACC_a.v[2]),
+                        fs * (J_a.v[3] + ACC_a.v[3]));
+      else
+        *reinterpret_cast<float4*>(op + (unsigned)(step - 4) * nx) =
+            make_float4((dd.x - 1.f) - (J_a.v[0] + ACC_a.v[0]), (dd.y - 1.f) - (J_a.v[1] + ACC_a.v[1]),
+                        (dd.z - 1.f) - (J_a.v[2] + ACC_a.v[2]), (dd.w - 1.f) - (J_a.v[3] + ACC_a.v[3]));
     }
     // ---- rotate the row windows ----
     A_b = A_c; dA_lo = dA_hi; J_a = J_b; J_b = J_c; H_a = H_b; Q_a = Q_b; ACC_a = ACC_b; ACC_b = ACC_c;
@@ -371,26 +232,23 @@ __global__ void __launch_bounds__(32 * LM_WPC) k_local_march(EprLines L, int nx,
 
 cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float* tau, const float* d_fuse, float* out,
                                      cudaStream_t st) {
-  if (d_fuse) {
-    const int bands = (p->nx + LM_BW - 1) / LM_BW;
-    static int sms = 0;
-    if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
-    // the tallest row block that still gives every SM about a dozen warps (all CTAs resident at once: no tail wave)
-    const long long need = 12ll * sms;
-    if ((long long)bands * ((p->ny + 127) / 128) * batch >= need) {
-      dim3 grid(bands, (p->ny + 127) / 128, batch);
-      k_local_march<128, 1><<<grid, 32, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, d_fuse, out);
-    } else if ((long long)bands * ((p->ny + 63) / 64) * batch >= need) {
-      dim3 grid((bands + 1) / 2, (p->ny + 63) / 64, batch);
-      k_local_march<64, 2><<<grid, 64, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, d_fuse, out);
-    } else {
-      dim3 grid((bands + 3) / 4, (p->ny + 31) / 32, batch);
-      k_local_march<32, 4><<<grid, 128, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, d_fuse, out);
-    }
-    return cudaGetLastError();
-  }
-  dim3 grid((p->nx + FL_TX - 1) / FL_TX, (p->ny + FL_TY - 1) / FL_TY, batch);
-  k_forward_local<false><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, nullptr, out);
+  // one line fused with the residual (d_fuse), or line by line into pred (several lines: blockIdx.z = projection · n_bins + line)
+  const int bands = (p->nx + LM_BW - 1) / LM_BW;
+  const int nz = d_fuse ? batch : batch * p->n_bins;
+  static int sms = 0;
+  if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+  // the tallest row block that still gives every SM about a dozen warps (all CTAs resident at once: no tail wave)
+  const long long need = 12ll * sms;
+#define EPR_MARCH(MR, WPC, GX, GY, NT)                                                                               \
+  do {                                                                                                              \
+    dim3 grid(GX, GY, nz);                                                                                          \
+    if (d_fuse) k_local_march<MR, WPC, false><<<grid, NT, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, d_fuse, out); \
+    else k_local_march<MR, WPC, true><<<grid, NT, 0, st>>>(p->lines, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, nullptr, out);       \
+  } while (0)
+  if ((long long)bands * ((p->ny + 127) / 128) * nz >= need) EPR_MARCH(128, 1, bands, (p->ny + 127) / 128, 32);
+  else if ((long long)bands * ((p->ny + 63) / 64) * nz >= need) EPR_MARCH(64, 2, (bands + 1) / 2, (p->ny + 63) / 64, 64);
+  else EPR_MARCH(32, 4, (bands + 3) / 4, (p->ny + 31) / 32, 128);
+#undef EPR_MARCH
   return cudaGetLastError();
 }
 
@@ -472,11 +330,10 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
                                                     const float* __restrict__ gmax) {
   extern __shared__ __align__(16) unsigned char st_raw[];
   unsigned* s_acc = reinterpret_cast<unsigned*>(st_raw);                              // [ST_AROWS][ST_AP]
-  float* s_tau = reinterpret_cast<float*>(st_raw + ST_AP * ST_AROWS * sizeof(unsigned));   // [RH + 2][TP]
+  float* s_tau = reinterpret_cast<float*>(st_raw + ST_AP * ST_AROWS * sizeof(unsigned));   // [ST_H + 2 H + 2][TP]
   const int b = blockIdx.z, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   constexpr int NW = ST_NT / 32;
   const int x0 = blockIdx.x * ST_W, y0 = blockIdx.y * ST_H;
-  const int RW = ST_W + 2 * H, RH = ST_H + 2 * H;      // source region: columns x0 − H …, rows y0 − H …
   const int Ha = (H + 1 + 3) & ~3;                     // τ tile halo in x, rounded up to whole 16-byte chunks
   const int TP = ST_W + 2 * Ha;                        // τ tile pitch; tile column of tile-relative x is x + Ha
   const unsigned plane = (unsigned)nx * (unsigned)ny;
@@ -753,7 +610,7 @@ cudaError_t epr_launch_splat(const epr_plan_s* p, int batch, const float* tau, c
 // =====================================================================================================
 // a2  detector residual and positivity-weighted split (reading R8), deviation form:
 //   e = (d − 1) − Σ_s (P_s − f_s);   w_s = P_s⁺ / Σ_t P_t⁺ (fallback f_s);   es_s = w_s e
-//   pred holds P_s − f_s (float), written by k_forward_local or k_splat_tile.
+//   pred holds P_s − f_s (float), written by k_local_march (several lines) or k_splat_tile.
 // =====================================================================================================
 // one thread = 4 consecutive pixels (plane % 4 == 0)
 __global__ void __launch_bounds__(256) k_residual(EprLines L, unsigned plane, const float* __restrict__ d,
