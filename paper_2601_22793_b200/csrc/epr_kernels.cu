@@ -315,25 +315,25 @@ cudaError_t epr_launch_grad_blockmax(const epr_plan_s* p, int batch, const float
 //   (d − 1) − (P − f): the detector residual a2 fused into the flush.
 // =====================================================================================================
 #define ST_W 128
-#define ST_H 64
+#define ST_H 64                       // tile height (template parameter TH of the kernel: 64, or 32 for large S)
 #define ST_AP (ST_W + 8)              // accumulator pitch: 4 columns of (aligned) border left, 1 used right
 #define ST_AROWS (ST_H + 2)           // one border row above and below: out-of-tile corners land there, unflushed
 
 // FROM_TAU: sources and ray map from the τ tile staged in shared memory (the loop's configuration);
 // otherwise (epr_transport) both are read from global planes.
 // ST_NT threads per CTA: 512 when two CTAs fit an SM, 1024 when the halo (large S) leaves room for one only
-template <bool FROM_TAU, bool MAP_OUT, int ST_NT>
+template <bool FROM_TAU, bool MAP_OUT, int ST_NT, int TH>
 __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny, float S, int H,
                                                     const float* __restrict__ tau, const float* __restrict__ I_bins,
                                                     const float2* __restrict__ map_in, float2* __restrict__ map_out,
                                                     float* __restrict__ out, int out_mode, const float* __restrict__ d,
                                                     const float* __restrict__ gmax) {
   extern __shared__ __align__(16) unsigned char st_raw[];
-  unsigned* s_acc = reinterpret_cast<unsigned*>(st_raw);                              // [ST_AROWS][ST_AP]
-  float* s_tau = reinterpret_cast<float*>(st_raw + ST_AP * ST_AROWS * sizeof(unsigned));   // [ST_H + 2 H + 2][TP]
+  unsigned* s_acc = reinterpret_cast<unsigned*>(st_raw);                              // [(TH + 2)][ST_AP]
+  float* s_tau = reinterpret_cast<float*>(st_raw + ST_AP * (TH + 2) * sizeof(unsigned));   // [TH + 2 H + 2][TP]
   const int b = blockIdx.z, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   constexpr int NW = ST_NT / 32;
-  const int x0 = blockIdx.x * ST_W, y0 = blockIdx.y * ST_H;
+  const int x0 = blockIdx.x * ST_W, y0 = blockIdx.y * TH;
   const int Ha = (H + 1 + 3) & ~3;                     // τ tile halo in x, rounded up to whole 16-byte chunks
   const int TP = ST_W + 2 * Ha;                        // τ tile pitch; tile column of tile-relative x is x + Ha
   const unsigned plane = (unsigned)nx * (unsigned)ny;
@@ -346,12 +346,12 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
     if (tid == 0) { s_maxd = 0u; s_maxd_in = 0u; }
     __syncthreads();
     const int nbx = nx >> 4, nby = ny >> 4;
-    const int nsx = (ST_W + 2 * H + 15) / 16 + 1, nsy = (ST_H + 2 * H + 15) / 16 + 1;
+    const int nsx = (ST_W + 2 * H + 15) / 16 + 1, nsy = (TH + 2 * H + 15) / 16 + 1;
     const float* gm = gmax + (size_t)b * nbx * nby;
     for (int i = tid; i < nsx * nsy; i += ST_NT) {
       const int j = i / nsx, ii = i - j * nsx;
-      const int px = min(-H + 16 * ii, ST_W - 1 + H), py = min(-H + 16 * j, ST_H - 1 + H);   // tile-relative sample
-      const bool inside = (unsigned)px < ST_W && (unsigned)py < ST_H;
+      const int px = min(-H + 16 * ii, ST_W - 1 + H), py = min(-H + 16 * j, TH - 1 + H);   // tile-relative sample
+      const bool inside = (unsigned)px < ST_W && (unsigned)py < TH;
       const float v = __ldg(&gm[(wrapm(y0 + py, ny) >> 4) * nbx + (wrapm(x0 + px, nx) >> 4)]);
       atomicMax(inside ? &s_maxd_in : &s_maxd, __float_as_uint(v));
     }
@@ -359,12 +359,12 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
     float csmax = 0.f;
     for (int s = 0; s < L.n_bins; ++s) csmax = fmaxf(csmax, 0.5f * L.a[s] * L.gamma[s]);
     const int Hl = min(H, (int)fminf(csmax * __uint_as_float(s_maxd), S) + 1);      // widest ring of any line
-    // τ tile rows y0 − Hl − 1 … y0 + ST_H + Hl (tile rows H − Hl … H + ST_H + 1 + Hl), columns x0 − Ha …:
+    // τ tile rows y0 − Hl − 1 … y0 + TH + Hl (tile rows H − Hl … H + TH + 1 + Hl), columns x0 − Ha …:
     // 16-byte cp.async chunks (nx % 4 == 0: a chunk never straddles the wrap), spread evenly over the threads
     const float* tb = tau + (size_t)b * plane;
-    const int cpr = TP / 4, nrows = ST_H + 2 + 2 * Hl;
+    const int cpr = TP / 4, nrows = TH + 2 + 2 * Hl;
     const float inv_cpr = 1.f / (float)cpr;
-    const bool big = nx >= 2 * (ST_W + 2 * Ha) && ny >= 2 * (ST_H + 2 * H + 2);
+    const bool big = nx >= 2 * (ST_W + 2 * Ha) && ny >= 2 * (TH + 2 * H + 2);
     for (int i = tid; i < nrows * cpr; i += ST_NT) {
       const int r = (int)(((float)i + 0.5f) * inv_cpr), cx = i - r * cpr;
       const int ly = H - Hl + r;
@@ -376,7 +376,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
   }
   // one line with the residual fused (out_mode 2): the d values of this thread's flush groups are requested now, so that
   // the flush does not wait on them (the load used to be 21 % of the kernel's stall samples)
-  constexpr int NFL = ST_W * ST_H / 4 / ST_NT;         // flush groups (4 pixels) per thread
+  constexpr int NFL = ST_W * TH / 4 / ST_NT;         // flush groups (4 pixels) per thread
   float4 dpre[NFL];
   if (out_mode == 2) {
 #pragma unroll
@@ -391,7 +391,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
   for (int s = 0; s < L.n_bins; ++s) {
     const size_t pl = ((size_t)b * L.n_bins + s) * plane;
     __syncthreads();                                   // previous bin flushed
-    for (int i = tid; i < ST_AP * ST_AROWS / 4; i += ST_NT) reinterpret_cast<uint4*>(s_acc)[i] = make_uint4(0u, 0u, 0u, 0u);
+    for (int i = tid; i < ST_AP * (TH + 2) / 4; i += ST_NT) reinterpret_cast<uint4*>(s_acc)[i] = make_uint4(0u, 0u, 0u, 0u);
     if (FROM_TAU && s == 0) cp_async_wait<0>();
     __syncthreads();
     const float cs = -0.5f * L.a[s] * L.gamma[s], gam = L.gamma[s], fixFf = (float)L.fixF[s];
@@ -399,16 +399,16 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
     // a source at distance D from the tile reaches it only if ⌊|u|⌋ + 1 ≥ D
     int He = H;
     if (FROM_TAU) He = min(H, (int)fminf(fabsf(cs) * __uint_as_float(s_maxd), S) + 1);
-    const int RWe = ST_W + 2 * He, RHe = ST_H + 2 * He;
+    const int RWe = ST_W + 2 * He, RHe = TH + 2 * He;
     // Every periodic image of a source pixel inside the region is a distinct candidate: its targets differ by whole
     // periods, and exactly one image puts a given corner on a given detector pixel — that IS the periodic wrap (R7).
     if (FROM_TAU) {
-      // (1) The tile's own ST_W x ST_H sources (nearly all of them hit): a warp owns a 32-column strip and marches
+      // (1) The tile's own ST_W x TH sources (nearly all of them hit): a warp owns a 32-column strip and marches
       // down its rows with the column's τ values in registers (3 shared loads per source instead of 5, no index
       // arithmetic: one address per array advances by a row); the loads of row r + 1 are issued before the atomics
       // of row r.  32-bit shared addresses are formed once (the compiler otherwise rebuilds them per source).
       // The clamp of u is skipped when |c_s| · max|D⁰τ| over the tile cannot exceed S.
-      constexpr int RG = NW / 4, ROWS = ST_H / RG;
+      constexpr int RG = NW / 4, ROWS = TH / RG;
       const int x = (warp & 3) * 32 + lane, yb = (warp >> 2) * ROWS;
       const unsigned TP4 = 4u * TP;
       const unsigned rb0 = (unsigned)__cvta_generic_to_shared(s_tau) + 4u * (unsigned)((yb + H + 1) * TP + x + Ha);
@@ -438,8 +438,8 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
           const float totf = (float)tot, te = totf * (1.f - dy), td = totf * dy, ex = 1.f - dx;
           const int c00 = __float2int_rn(te * ex), c10 = __float2int_rn(te * dx), c01 = __float2int_rn(td * ex);
           const int c11 = tot - c00 - c10 - c01;
-          // ax = x + fx ∈ [−1, ST_W − 1], ay ∈ [−1, ST_H − 1]: all four corners are inside the bordered accumulator
-          if ((unsigned)(x + fx + 1) <= ST_W && (unsigned)(yb + r + fy + 1) <= ST_H) {
+          // ax = x + fx ∈ [−1, ST_W − 1], ay ∈ [−1, TH − 1]: all four corners are inside the bordered accumulator
+          if ((unsigned)(x + fx + 1) <= ST_W && (unsigned)(yb + r + fy + 1) <= TH) {
             const unsigned a0 = ab + 4u * (unsigned)(fy * ST_AP + fx);
             red_shared_u32(a0, (unsigned)c00);
             red_shared_u32(a0 + 4, (unsigned)c10);
@@ -455,13 +455,13 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
     }
     // (2) FROM_TAU: the ring of width He around the tile (two bands of He rows, two of He columns), few of whose
     // sources reach the tile; otherwise (epr_transport): the whole region, row-major.
-    const int n_tb = 2 * He * RWe, n_walk = FROM_TAU ? n_tb + 2 * ST_H * He : RWe * RHe;
+    const int n_tb = 2 * He * RWe, n_walk = FROM_TAU ? n_tb + 2 * TH * He : RWe * RHe;
     const float inv_rw = 1.f / (float)RWe, inv_2he = 1.f / (float)(2 * He);
     for (int i = tid; i < n_walk; i += ST_NT) {
       int sx, sy;                                      // quotients by float reciprocal: exact for these ranges
       if (!FROM_TAU || i < n_tb) {
         sy = (int)(((float)i + 0.5f) * inv_rw); sx = i - sy * RWe;
-        if (FROM_TAU && sy >= He) sy += ST_H;
+        if (FROM_TAU && sy >= He) sy += TH;
       } else {
         const int j = i - n_tb;
         sy = (int)(((float)j + 0.5f) * inv_2he); sx = j - sy * 2 * He;
@@ -477,7 +477,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
         tc = tp[0];
         ux = fminf(fmaxf(cs * (tp[1] - tp[-1]), -S), S);
         uy = fminf(fmaxf(cs * (tp[TP] - tp[-TP]), -S), S);
-        if (MAP_OUT && (unsigned)tx0 < ST_W && (unsigned)ty0 < ST_H && x0 + tx0 < nx && y0 + ty0 < ny)
+        if (MAP_OUT && (unsigned)tx0 < ST_W && (unsigned)ty0 < TH && x0 + tx0 < nx && y0 + ty0 < ny)
           map_out[pl + (unsigned)(y0 + ty0) * nx + (x0 + tx0)] = make_float2(ux, uy);
       } else {
         gidx = (unsigned)wrapm(y0 + ty0, ny) * nx + wrapm(x0 + tx0, nx);
@@ -486,7 +486,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       }
       const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
       const int ax = tx0 + fx, ay = ty0 + fy;          // top-left target, tile coordinates
-      if ((unsigned)(ax + 1) > ST_W || (unsigned)(ay + 1) > ST_H) continue;      // cannot touch this tile
+      if ((unsigned)(ax + 1) > ST_W || (unsigned)(ay + 1) > TH) continue;      // cannot touch this tile
       const float dx = ux - (float)fx, dy = uy - (float)fy;
       int tot;                                         // signed: epr_transport accepts planes of either sign
       if (FROM_TAU) {
@@ -502,7 +502,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       const float totf = (float)tot, te = totf * (1.f - dy), td = totf * dy, ex = 1.f - dx;
       const int c00 = __float2int_rn(te * ex), c10 = __float2int_rn(te * dx), c01 = __float2int_rn(td * ex);
       const int c11 = tot - c00 - c10 - c01;
-      // ax ∈ [−1, ST_W − 1], ay ∈ [−1, ST_H − 1]: all four corners are inside the bordered accumulator
+      // ax ∈ [−1, ST_W − 1], ay ∈ [−1, TH − 1]: all four corners are inside the bordered accumulator
       unsigned* a0 = s_acc + (ay + 1) * ST_AP + (ax + 4);
       atomicAdd(a0, (unsigned)c00);
       atomicAdd(a0 + 1, (unsigned)c10);
@@ -542,7 +542,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
     // and overwrites them with e_s, so the N prediction planes never come back from HBM.
     const float off = 1.f + L.fsum_dev;
     float* ob = out + (size_t)b * L.n_bins * plane;
-    for (int i = tid; i < ST_W * ST_H / 4; i += ST_NT) {
+    for (int i = tid; i < ST_W * TH / 4; i += ST_NT) {
       const int ty = i / (ST_W / 4), tx = 4 * (i - ty * (ST_W / 4));
       const int gx = x0 + tx, gy = y0 + ty;
       if (gx >= nx || gy >= ny) continue;
@@ -574,32 +574,41 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
   }
 }
 
+template <bool FROM_TAU, bool MAP_OUT, int NT, int TH>
+static cudaError_t launch_splat_v(const epr_plan_s* p, int batch, int H, size_t smem, const float* tau, const float* I_bins,
+                                  const float2* map_in, float2* map_out, float* out, int out_mode, const float* d,
+                                  cudaStream_t st) {
+  static size_t attr = 0;
+  if (smem > attr) {
+    cudaFuncSetAttribute(k_splat_tile<FROM_TAU, MAP_OUT, NT, TH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attr = smem;
+  }
+  dim3 grid((p->nx + ST_W - 1) / ST_W, (p->ny + TH - 1) / TH, batch);
+  k_splat_tile<FROM_TAU, MAP_OUT, NT, TH><<<grid, NT, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, H, tau, I_bins,
+                                                                   map_in, map_out, out, out_mode, d, p->gmax);
+  return cudaGetLastError();
+}
+
 template <bool FROM_TAU, bool MAP_OUT>
 static cudaError_t launch_splat_t(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
                                   float2* map_out, float* out, int out_mode, const float* d, cudaStream_t st) {
   const int H = (int)ceilf(p->opt.max_shift_px) + 1;
   const int Ha = (H + 1 + 3) & ~3;
-  const size_t smem = (size_t)ST_AP * ST_AROWS * sizeof(unsigned) +
-                      (FROM_TAU ? (size_t)(ST_W + 2 * Ha) * (ST_H + 2 * H + 2) * sizeof(float) : 0);
-  static size_t attr[2] = {0, 0};
-  const int big = smem > 113 * 1024 ? 1 : 0;            // more than half of the 227 KB an SM offers
-  if (smem > attr[big]) {
-    if (big) cudaFuncSetAttribute(k_splat_tile<FROM_TAU, MAP_OUT, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    else cudaFuncSetAttribute(k_splat_tile<FROM_TAU, MAP_OUT, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr[big] = smem;
-  }
-  dim3 grid((p->nx + ST_W - 1) / ST_W, (p->ny + ST_H - 1) / ST_H, batch);
+  auto smem_of = [&](int th) {
+    return (size_t)ST_AP * (th + 2) * sizeof(unsigned) + (FROM_TAU ? (size_t)(ST_W + 2 * Ha) * (th + 2 * H + 2) * sizeof(float) : 0);
+  };
   if (FROM_TAU) {                                      // block maxima of |D⁰τ| (also used by the gather of this τ)
     const cudaError_t e = epr_launch_grad_blockmax(p, batch, tau, st);
     if (e != cudaSuccess) return e;
   }
-  if (big)
-    k_splat_tile<FROM_TAU, MAP_OUT, 1024><<<grid, 1024, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, H, tau, I_bins,
-                                                                    map_in, map_out, out, out_mode, d, p->gmax);
-  else
-    k_splat_tile<FROM_TAU, MAP_OUT, 512><<<grid, 512, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, H, tau, I_bins,
-                                                                  map_in, map_out, out, out_mode, d, p->gmax);
-  return cudaGetLastError();
+  const size_t half = 113 * 1024;                      // half of the 227 KB an SM offers: two CTAs per SM
+  // 128 x 64 tiles with 512 threads when two CTAs fit an SM; large S (C5: S = 24): 128 x 32 tiles still bring two;
+  // beyond that one 1024-thread CTA per SM
+  if (smem_of(ST_H) <= half)
+    return launch_splat_v<FROM_TAU, MAP_OUT, 512, ST_H>(p, batch, H, smem_of(ST_H), tau, I_bins, map_in, map_out, out, out_mode, d, st);
+  if (smem_of(ST_H / 2) <= half)
+    return launch_splat_v<FROM_TAU, MAP_OUT, 512, ST_H / 2>(p, batch, H, smem_of(ST_H / 2), tau, I_bins, map_in, map_out, out, out_mode, d, st);
+  return launch_splat_v<FROM_TAU, MAP_OUT, 1024, ST_H>(p, batch, H, smem_of(ST_H), tau, I_bins, map_in, map_out, out, out_mode, d, st);
 }
 
 cudaError_t epr_launch_splat(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
