@@ -234,7 +234,8 @@ template <int N, int R, int TPC> struct PassGeom {
 
 // Butterfly + Stockham scatter of one thread's butterflies held in u[c][r] (inputs x[j + r·T], j = t + c·TPC):
 // twiddle (P > 1), radix-R DFT; afterwards u[c][q] is output element j0 + q·P, j0 = (j − j%P)·R + j%P.
-template <int N, int P, int R, int TPC, bool INV>
+// TWS: the twiddle table lives in shared memory (plain loads) instead of global memory (read-only path)
+template <int N, int P, int R, int TPC, bool INV, bool TWS = false>
 __device__ __forceinline__ void bfly(float2 (&u)[PassGeom<N, R, TPC>::CNT][R], int t, const float2* __restrict__ tw) {
   using G = PassGeom<N, R, TPC>;
 #pragma unroll
@@ -244,7 +245,7 @@ __device__ __forceinline__ void bfly(float2 (&u)[PassGeom<N, R, TPC>::CNT][R], i
       if constexpr (P > 1) {
         const int k = j % P;
 #pragma unroll
-        for (int r = 1; r < R; ++r) u[c][r] = cmul(u[c][r], conj_if<INV>(__ldg(&tw[(r - 1) * P + k])));
+        for (int r = 1; r < R; ++r) u[c][r] = cmul(u[c][r], conj_if<INV>(TWS ? tw[(r - 1) * P + k] : __ldg(&tw[(r - 1) * P + k])));
       }
       dft<R, INV>(u[c]);
     }
@@ -281,7 +282,7 @@ __device__ __forceinline__ void smem_scatter(const float2 (&u)[PassGeom<N, R, TP
 // Usage (n = NP passes):  first pass inputs come from registers (filled by the caller from global memory:
 // element index of u[c][r] is (t + c·TPC) + r·T0), last pass outputs stay in registers (element index of
 // u[c][q] is (t + c·TPC) + q·PL).  Passes in between go through shared memory.
-template <int N, int TPC, int STRIDE, bool INV, bool REV> struct Engine {
+template <int N, int TPC, int STRIDE, bool INV, bool REV, bool TWS = false> struct Engine {
   static constexpr int NP = num_passes(N);
   static constexpr int R0 = sched_radix(N, 0, REV);                 // first radix
   static constexpr int RL = sched_radix(N, NP - 1, REV);            // last radix
@@ -295,7 +296,7 @@ template <int N, int TPC, int STRIDE, bool INV, bool REV> struct Engine {
       float2 u[PassGeom<N, R, TPC>::CNT][R];
       smem_gather<N, R, TPC, STRIDE>(u, s, off, t);
       __syncthreads();
-      bfly<N, P, R, TPC, INV>(u, t, tw + tw_offset(N, I, REV));
+      bfly<N, P, R, TPC, INV, TWS>(u, t, tw + tw_offset(N, I, REV));
       smem_scatter<N, P, R, TPC, STRIDE>(u, s, off, t);
       __syncthreads();
       middle<I + 1>(s, off, t, tw);
@@ -306,18 +307,18 @@ template <int N, int TPC, int STRIDE, bool INV, bool REV> struct Engine {
   __device__ static __forceinline__ void run(float2 (&u0)[G0::CNT][R0], float2 (&uL)[GL::CNT][RL], float2* s, int off, int t,
                                              const float2* __restrict__ tw) {
     if constexpr (NP == 1) {
-      bfly<N, 1, R0, TPC, INV>(u0, t, tw);
+      bfly<N, 1, R0, TPC, INV, TWS>(u0, t, tw);
 #pragma unroll
       for (int c = 0; c < G0::CNT; ++c)
 #pragma unroll
         for (int r = 0; r < R0; ++r) uL[c][r] = u0[c][r];
     } else {
-      bfly<N, 1, R0, TPC, INV>(u0, t, tw);
+      bfly<N, 1, R0, TPC, INV, TWS>(u0, t, tw);
       smem_scatter<N, 1, R0, TPC, STRIDE>(u0, s, off, t);
       __syncthreads();
       middle<1>(s, off, t, tw);
       smem_gather<N, RL, TPC, STRIDE>(uL, s, off, t);
-      bfly<N, PL, RL, TPC, INV>(uL, t, tw + tw_offset(N, NP - 1, REV));
+      bfly<N, PL, RL, TPC, INV, TWS>(uL, t, tw + tw_offset(N, NP - 1, REV));
     }
   }
 };

@@ -623,7 +623,11 @@ template <int N> struct ColTmaPadCfg {
   using C = ColCfg<N>;
   static constexpr size_t LIN = (size_t)N * C::W * sizeof(float2);
   static constexpr size_t WORK = (C::SMEM + 15) / 16 * 16;
-  static constexpr size_t smem(bool sum) { return (sum ? 2 : 1) * LIN + WORK + 16; }
+  // several lines: the forward twiddle table (used once per line) goes to shared memory when it still fits — with
+  // ~210 KB of shared memory carved out, the L1 that is left (hit rate 29 %) cannot hold the tables
+  static constexpr size_t TWB = (size_t)tw_total(N, false) * sizeof(float2);
+  static constexpr bool TWS = 2 * LIN + WORK + 16 + TWB <= 227 * 1024;
+  static constexpr size_t smem(bool sum) { return (sum ? 2 : 1) * LIN + WORK + 16 + ((sum && TWS) ? TWB : 0); }
 };
 
 template <int N, bool SUM>
@@ -633,13 +637,19 @@ k_cols_tmap(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
             const float2* __restrict__ tw, const float2* __restrict__ tw_inv) {
   using C = ColCfg<N>;
   using P = ColTmaPadCfg<N>;
-  using EF = Engine<N, C::TPC, C::W, false, false>;
+  constexpr bool TWS = SUM && P::TWS;
+  using EF = Engine<N, C::TPC, C::W, false, false, TWS>;
   using EI = Engine<N, C::TPC, C::W, true, true>;
   static_assert(EF::RL == EI::R0 && EF::GL::CNT == EI::G0::CNT && EF::PL == EI::G0::T, "schedules must mirror");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   constexpr int NBUF = SUM ? 2 : 1;
   float2* work = reinterpret_cast<float2*>(smem_raw + NBUF * P::LIN);
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + NBUF * P::LIN + P::WORK);
+  float2* tw_s = reinterpret_cast<float2*>(smem_raw + NBUF * P::LIN + P::WORK + 16);
+  if (TWS) {                                 // visible to everybody after the __syncthreads that follows the barrier init
+    for (int i = threadIdx.x; i < tw_total(N, false); i += C::NT) tw_s[i] = __ldg(&tw[i]);
+  }
+  const float2* twf = TWS ? tw_s : tw;
   const int c = threadIdx.x % C::W, t = threadIdx.x / C::W;
   const int kx0 = blockIdx.x * C::W, kx = kx0 + c;
   const int oplane = blockIdx.y;
@@ -680,7 +690,7 @@ k_cols_tmap(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
         u0[cc][r] = v;
       }
     }
-    EF::run(u0, uL, work, c, t, tw);
+    EF::run(u0, uL, work, c, t, twf);
     if (blockIdx.x == 0) {
       // tile 0 holds the packed column kx = 0: C = F0 + i FM (both Hermitian in ky).  With A = ½(C[ky] + C*[−ky]),
       // B = −(i/2)(C[ky] − C*[−ky]):  C'[ky] = H(0,ky) A + i H(M,ky) B,  C'[−ky] = H(0,ky) A* + i H(M,ky) B*.
