@@ -328,10 +328,12 @@ def test_resampling_round_trip_is_exact(E):
         assert np.max(np.abs(out.cpu().numpy() - dn)) < 5e-7
 
 
-@pytest.mark.parametrize("ny,nx,n_lines", [(2160, 32, 3), (2160, 64, 8), (320, 64, 5), (2560, 32, 3)])
+@pytest.mark.parametrize("ny,nx,n_lines", [(2160, 32, 3), (2160, 64, 8), (320, 64, 5), (2560, 32, 3), (4096, 32, 3), (32, 4096, 1)])
 def test_retrieve_non_power_of_two_columns_several_lines(E, ny, nx, n_lines):
     """The Fourier-space sum over lines (R10) on column lengths that are not powers of two: 2160 and 320 take the
-    TMA-staged padded column kernel with two tiles in flight, 2560 (two tiles would not fit an SM) the direct one."""
+    TMA-staged padded column kernel with two tiles in flight, 2560 (two tiles would not fit an SM) the direct one; 4096
+    rows (the x2 oversampled grid of a 2048 detector) with several lines take the direct kernel as well, 4096 columns the
+    2048-point row transforms."""
     import torch
     rng = np.random.default_rng(ny + nx + n_lines)
     y, x = np.meshgrid(np.arange(ny) * 2 * np.pi / ny, np.arange(nx) * 2 * np.pi / nx, indexing="ij")
