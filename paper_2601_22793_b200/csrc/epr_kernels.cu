@@ -1,4 +1,5 @@
 // epr_kernels.cu — stencil, splat, gather and pointwise kernels of the EPR iteration (sm_100a).
+#include <cstdlib>
 #include <type_traits>
 #include "epr_internal.h"
 #include "epr_math.cuh"
@@ -317,7 +318,8 @@ cudaError_t epr_launch_grad_blockmax(const epr_plan_s* p, int batch, const float
 #define ST_W 128
 #define ST_H 64                       // tile height (template parameter TH of the kernel: 64, or 32 for large S)
 #define ST_AP (ST_W + 8)              // accumulator pitch: 4 columns of (aligned) border left, 1 used right
-#define ST_AROWS (ST_H + 2)           // one border row above and below: out-of-tile corners land there, unflushed
+#define ST_AROWS (ST_H + 2)
+#define ST_LCAP 2048                  // capacity of the ring-candidate list (several lines); beyond it the ring is walked           // one border row above and below: out-of-tile corners land there, unflushed
 
 // FROM_TAU: sources and ray map from the τ tile staged in shared memory (the loop's configuration);
 // otherwise (epr_transport) both are read from global planes.
@@ -327,7 +329,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
                                                     const float* __restrict__ tau, const float* __restrict__ I_bins,
                                                     const float2* __restrict__ map_in, float2* __restrict__ map_out,
                                                     float* __restrict__ out, int out_mode, const float* __restrict__ d,
-                                                    const float* __restrict__ gmax) {
+                                                    const float* __restrict__ gmax, int use_list) {
   extern __shared__ __align__(16) unsigned char st_raw[];
   unsigned* s_acc = reinterpret_cast<unsigned*>(st_raw);                              // [(TH + 2)][ST_AP]
   float* s_tau = reinterpret_cast<float*>(st_raw + ST_AP * (TH + 2) * sizeof(unsigned));   // [TH + 2 H + 2][TP]
@@ -341,7 +343,10 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
   // Largest |D⁰τ| (times 2) among the sources in the ring of width H around the tile (s_maxd) and in the tile itself
   // (s_maxd_in), from the 16x16-block maxima of k_grad_blockmax: a source at distance D from the tile reaches it only
   // if ⌊|u|⌋ + 1 ≥ D, so the ring that has to be walked (and loaded) is He ≤ H wide.
-  __shared__ unsigned s_maxd, s_maxd_in;
+  __shared__ unsigned s_maxd, s_maxd_in, s_cnt;
+  // several lines: the few ring sources that can reach the tile at all, found once (see below), 16 bits each
+  unsigned short* s_list = reinterpret_cast<unsigned short*>(st_raw + ST_AP * (TH + 2) * sizeof(unsigned) +
+                                                             (size_t)TP * (TH + 2 * H + 2) * sizeof(float));
   if (FROM_TAU) {
     if (tid == 0) { s_maxd = 0u; s_maxd_in = 0u; }
     __syncthreads();
@@ -373,6 +378,39 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       cp_async16(s_tau + ly * TP + 4 * cx, tb + (unsigned)gy * nx + gx);
     }
     cp_async_commit();
+    if (use_list) {
+      // Ring candidates of ALL lines in one walk.  u_s = c_s D⁰τ with c_s < 0 for every line, so the shift of any line
+      // is the strongest line's shift scaled by t ∈ (0, 1]: ⌊u_s⌋ lies between min(⌊u_max⌋, 0) and max(⌊u_max⌋, −1) on
+      // each axis (fp32 products and the clamp are monotone in |c_s|).  A source none of whose possible targets touches
+      // the tile is dropped here once instead of being rejected by every line; the per-line walk below repeats the
+      // exact test on what is left (a few per cent of the tile's own sources).
+      if (tid == 0) s_cnt = 0u;
+      cp_async_wait<0>();
+      __syncthreads();
+      const int RWl = ST_W + 2 * Hl, n_tbl = 2 * Hl * RWl, n_wl = n_tbl + 2 * TH * Hl;
+      const float inv_rwl = 1.f / (float)RWl, inv_2hl = 1.f / (float)(2 * Hl);
+      for (int i = tid; i < n_wl; i += ST_NT) {
+        int sx, sy;
+        if (i < n_tbl) {
+          sy = (int)(((float)i + 0.5f) * inv_rwl); sx = i - sy * RWl;
+          if (sy >= Hl) sy += TH;
+        } else {
+          const int j = i - n_tbl;
+          sy = (int)(((float)j + 0.5f) * inv_2hl); sx = j - sy * 2 * Hl;
+          sy += Hl;
+          if (sx >= Hl) sx += ST_W;
+        }
+        const int tx0 = sx - Hl, ty0 = sy - Hl;
+        const float* tp = s_tau + (ty0 + H + 1) * TP + (tx0 + Ha);
+        const float ux = fminf(fmaxf(-csmax * (tp[1] - tp[-1]), -S), S);
+        const float uy = fminf(fmaxf(-csmax * (tp[TP] - tp[-TP]), -S), S);
+        const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
+        if (tx0 + max(fx, -1) >= -1 && tx0 + min(fx, 0) <= ST_W - 1 && ty0 + max(fy, -1) >= -1 && ty0 + min(fy, 0) <= TH - 1) {
+          const unsigned k = atomicAdd(&s_cnt, 1u);
+          if (k < ST_LCAP) s_list[k] = (unsigned short)(((ty0 + 64) << 8) | (tx0 + 64));
+        }
+      }
+    }
   }
   // one line with the residual fused (out_mode 2): the d values of this thread's flush groups are requested now, so that
   // the flush does not wait on them (the load used to be 21 % of the kernel's stall samples)
@@ -455,11 +493,15 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
     }
     // (2) FROM_TAU: the ring of width He around the tile (two bands of He rows, two of He columns), few of whose
     // sources reach the tile; otherwise (epr_transport): the whole region, row-major.
-    const int n_tb = 2 * He * RWe, n_walk = FROM_TAU ? n_tb + 2 * TH * He : RWe * RHe;
+    const bool listed = FROM_TAU && use_list && s_cnt <= ST_LCAP;      // s_cnt is final: barriers above (uniform)
+    const int n_tb = 2 * He * RWe, n_walk = listed ? (int)s_cnt : FROM_TAU ? n_tb + 2 * TH * He : RWe * RHe;
     const float inv_rw = 1.f / (float)RWe, inv_2he = 1.f / (float)(2 * He);
     for (int i = tid; i < n_walk; i += ST_NT) {
       int sx, sy;                                      // quotients by float reciprocal: exact for these ranges
-      if (!FROM_TAU || i < n_tb) {
+      if (listed) {
+        const unsigned e = s_list[i];
+        sx = (int)(e & 255u) - 64 + He; sy = (int)(e >> 8) - 64 + He;
+      } else if (!FROM_TAU || i < n_tb) {
         sy = (int)(((float)i + 0.5f) * inv_rw); sx = i - sy * RWe;
         if (FROM_TAU && sy >= He) sy += TH;
       } else {
@@ -584,8 +626,11 @@ static cudaError_t launch_splat_v(const epr_plan_s* p, int batch, int H, size_t 
     attr = smem;
   }
   dim3 grid((p->nx + ST_W - 1) / ST_W, (p->ny + TH - 1) / TH, batch);
+  // several lines share one list of ring candidates (the coordinates are packed in 8 bits each: H ≤ 64)
+  static const bool list_off = getenv("EPR_SPLAT_LIST") && atoi(getenv("EPR_SPLAT_LIST")) == 0;
+  const int use_list = FROM_TAU && p->lines.n_bins > 1 && H <= 64 && !list_off;
   k_splat_tile<FROM_TAU, MAP_OUT, NT, TH><<<grid, NT, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, H, tau, I_bins,
-                                                                   map_in, map_out, out, out_mode, d, p->gmax);
+                                                                   map_in, map_out, out, out_mode, d, p->gmax, use_list);
   return cudaGetLastError();
 }
 
@@ -595,7 +640,7 @@ static cudaError_t launch_splat_t(const epr_plan_s* p, int batch, const float* t
   const int H = (int)ceilf(p->opt.max_shift_px) + 1;
   const int Ha = (H + 1 + 3) & ~3;
   auto smem_of = [&](int th) {
-    return (size_t)ST_AP * (th + 2) * sizeof(unsigned) + (FROM_TAU ? (size_t)(ST_W + 2 * Ha) * (th + 2 * H + 2) * sizeof(float) : 0);
+    return (size_t)ST_AP * (th + 2) * sizeof(unsigned) + (FROM_TAU ? (size_t)(ST_W + 2 * Ha) * (th + 2 * H + 2) * sizeof(float) + ST_LCAP * sizeof(unsigned short) : 0);
   };
   if (FROM_TAU) {                                      // block maxima of |D⁰τ| (also used by the gather of this τ)
     const cudaError_t e = epr_launch_grad_blockmax(p, batch, tau, st);
