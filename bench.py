@@ -14,6 +14,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -159,6 +160,51 @@ def oracle_time_one(w, j=0, m=1):
     return time.perf_counter() - t0
 
 
+def cufft_compare(epr, plan, B, reps=5):
+    """Comparison point only (north_star: "a cuFFT-based variant is kept only as a reported comparison point"): the
+    a4 preconditioner q_s = IFFT2(H_s FFT2(r_s)), H_s = 1/(1 + a_s λ) with the discrete 5-point symbol (PAPER.md:51,
+    reading R5), once through epr_precondition (the library's own row/column FFT kernels) and once through cuFFT
+    (torch.fft.rfft2 · H · irfft2) on the same device planes.  Nothing on the product path calls this."""
+    import torch
+    nb, ny, nx = plan.n_bins, plan.ny, plan.nx
+    Bc = max(1, min(B, 256 // max(nb, 1), 16))     # planes of both variants plus the cuFFT spectra stay within a few GB
+    g = torch.Generator(device="cuda").manual_seed(7)
+    r = torch.randn((Bc, nb, ny, nx), device="cuda", dtype=torch.float32, generator=g)
+    q = torch.empty_like(r)
+    a = torch.tensor(plan.lines()["a"], device="cuda", dtype=torch.float64)
+    th_y = 2 * math.pi * torch.fft.fftfreq(ny, device="cuda", dtype=torch.float64)
+    th_x = 2 * math.pi * torch.fft.rfftfreq(nx, device="cuda", dtype=torch.float64)
+    lam = (2 - 2 * torch.cos(th_y))[:, None] + (2 - 2 * torch.cos(th_x))[None, :]
+    H = (1.0 / (1.0 + a[:, None, None] * lam[None])).to(torch.float32)          # [nb][ny][nx/2+1]
+
+    def ours():
+        epr.epr_precondition(plan, r, q)
+
+    def cufft():
+        return torch.fft.irfft2(torch.fft.rfft2(r) * H, s=(ny, nx))
+
+    def timed(fn):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+    t_ours, t_cufft = timed(ours), timed(cufft)
+    ref = cufft()
+    diff = float(torch.linalg.vector_norm((q - ref).double()) / torch.linalg.vector_norm(ref.double()))
+    del r, q, ref, H
+    torch.cuda.empty_cache()
+    return {"op": "epr_precondition (a4) on %d x %d line(s) x %dx%d" % (Bc, nb, ny, nx),
+            "ours_us_per_plane": 1e3 * t_ours / (Bc * nb), "cufft_us_per_plane": 1e3 * t_cufft / (Bc * nb),
+            "cufft_over_ours": t_cufft / t_ours, "rel_l2_between": diff,
+            "note": "cuFFT leg = torch.fft.rfft2 * H -> irfft2 (library kernels, comparison point only)"}
+
+
 def run_reference(args, rank):
     if rank != 0:
         return
@@ -193,6 +239,8 @@ def main():
     ap.add_argument("--distinct", type=int, default=2, help="distinct simulated projections (rest: new noise only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cufft-compare", action="store_true",
+                    help="skip the preconditioner-through-cuFFT comparison point (rank 0, outside every timed region)")
     ap.add_argument("--lines", type=int, default=0,
                     help="retrieve with this many spectral lines (60-140 keV, Gaussian weights) instead of the config's own "
                          "discretisation, e.g. --config C2 --lines 5: the paper's 'local L2 poly' rows (PAPER.md:116-119)")
@@ -300,6 +348,10 @@ def main():
     prof = plan.profile_read()
     plan.profile(False)
 
+    cmp_cufft = None
+    if rank == 0 and m == 1 and not args.no_cufft_compare:
+        cmp_cufft = cufft_compare(epr, plan, B)
+
     if rank == 0:
         peak, peak_src = peaks()
         per_kernel = []
@@ -344,6 +396,8 @@ def main():
             "clocks": clk.summary(),
             "roofline": roofline,
         }
+        if cmp_cufft is not None:
+            result["cufft_compare"] = cmp_cufft
         if not args.no_cpu_baseline:
             t1 = oracle_time_one(w, m=m)
             result["cpu_baseline"] = {"value": 1.0 / t1, "unit": UNIT, "cores": 1, "kind": "oracle",
