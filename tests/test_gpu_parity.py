@@ -141,6 +141,37 @@ def test_forward_nonlocal_splat_mass_and_adjoint(E, ny, nx, spec, L):
     plan.destroy()
 
 
+def test_forward_nonlocal_uniform_large_shift_several_lines(E):
+    """Several lines share one list of ring candidates per detector tile (k_splat_tile); a triangle-wave τ gives a
+    constant 14-pixel shift on both axes at the strongest line, so that about 2900 ring sources reach every 128x64
+    tile — more than the list holds (2048) — and the kernel has to fall back to walking the ring line by line.
+    The weaker lines (unequal a_s) reach the tile from a narrower ring.  Result against the oracle, mass included."""
+    import torch
+    ny = nx = 256
+    en, w, db = SPECTRA["poly3_unequal_a"]
+    S, c = 16.0, 0.002
+    l0 = O.derive_lines(6.5e-6, 1.0, en, w, db)
+    L = 14.0 / (c * float(np.max(l0.a * l0.gamma)))            # a_s is linear in L
+    lines = O.derive_lines(6.5e-6, L, en, w, db)
+    assert abs(float(np.max(lines.a * lines.gamma)) * c - 14.0) < 1e-9
+    tri = np.abs(np.arange(nx) - nx / 2)
+    tau = (c * (tri[None, :] + tri[:, None]) + 0.05).astype(np.float32)[None]
+    plan = E.epr_plan(nx, ny, 6.5e-6, L, en, w, db, "nonlocal", max_batch=1, max_shift_px=S)
+    P = torch.empty((1, ny, nx), device="cuda")
+    Pb = torch.empty((1, 3, ny, nx), device="cuda")
+    E.epr_forward(plan, _dev(tau), P, Pb)
+    ref, ref_bins, maps = O.forward(tau[0].astype(np.float64), lines, "nonlocal", S=S)
+    Is = O.line_intensities(tau[0].astype(np.float64), lines)
+    shifts = sorted(float(np.abs(maps[s][0]).max()) for s in range(3))
+    assert shifts[-1] > 13.9 and shifts[0] < 0.8 * shifts[-1]
+    assert rel_l2(P.cpu().numpy()[0], ref) < TOL_OP
+    for s in range(3):
+        got = Pb.cpu().numpy()[0, s]
+        assert rel_l2(got, ref_bins[s]) < TOL_OP
+        assert abs(got.astype(np.float64).sum() - Is[s].sum()) <= TOL_MASS * Is[s].sum()
+    plan.destroy()
+
+
 def test_transport_signed_planes_and_wrap(E):
     """The linear splat accepts planes of either sign (fixed point is signed), and mass that leaves one side of a
     multi-tile grid enters the other (R7): compare with the oracle on a 320 x 320 grid (3 x 5 detector tiles, ragged in x)."""
