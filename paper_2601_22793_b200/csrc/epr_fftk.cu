@@ -206,10 +206,10 @@ __global__ void __launch_bounds__(RowCfg<M>::NT, (RowCfg<M>::NT <= 128) ? C2R_MI
           if (i + C::TPC < M && !tau_is_zero) tnext = dst[i + C::TPC];
           const float2 v = s[i];
           float d0, d1;
-          if (!epr_project_increment_small_nb(L, tau.x, step * v.x, newton_iters, i_min, d0))
+          if (!epr_project_increment_small_nb2(L, tau, make_float2(step * v.x, step * v.y), newton_iters, i_min, d0, d1)) {
             d0 = epr_project_increment(tau.x, step * v.x, s_f, s_gamma, L.n_bins, L.gamma_max, newton_iters, i_min);
-          if (!epr_project_increment_small_nb(L, tau.y, step * v.y, newton_iters, i_min, d1))
             d1 = epr_project_increment(tau.y, step * v.y, s_f, s_gamma, L.n_bins, L.gamma_max, newton_iters, i_min);
+          }
           tau.x += d0; tau.y += d1;
           dst[i] = tau;
         }

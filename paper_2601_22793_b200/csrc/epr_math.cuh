@@ -97,7 +97,9 @@ __device__ __forceinline__ bool epr_project_increment_small(const EprLines& L, f
   }
   const float rc1 = -__fdividef(1.f, G1);            // 1 / c1
   float delta = dT * rc1;                            // y = ΔT / c1: first order
-  if (!(fabsf(delta) * L.gamma_max < 0.01f && G0 + dT >= i_min)) return false;
+  // straight-line code (no early return): the caller runs two pixels through it back to back and the two chains of
+  // exponentials and divisions interleave; a result with ok == false is discarded
+  const bool ok = fabsf(delta) * L.gamma_max < 0.01f && G0 + dT >= i_min;
   if (newton_iters > 0) {
     // No loop, no divergence: second-order series reversion δ₁ = y − (c2/c1) y² (relative error (γ y)²/3 < 4e-5), then
     // ONE Newton step on the cubic, which squares it (< 1e-9: below fp32).  The loop this replaces took three
@@ -109,18 +111,25 @@ __device__ __forceinline__ bool epr_project_increment_small(const EprLines& L, f
     delta -= __fdividef(F, dF);
   }
   delta_out = delta;
-  return true;
+  return ok;
 }
 
-// the line counts with an unrolled instance: 8 (BASELINE configs C4, C5), 5 and 10 (the paper's own runs)
-__device__ __forceinline__ bool epr_project_increment_small_nb(const EprLines& L, float tau, float dT, int newton_iters,
-                                                               float i_min, float& delta_out) {
+// the line counts with an unrolled instance: 8 (BASELINE configs C4, C5), 5 and 10 (the paper's own runs);
+// two pixels at once (the C2R epilogue's float2): both small-step solutions in one basic block; false if either needs
+// the general routine (the caller then takes it for both: the general routine repeats the small test itself)
+__device__ __forceinline__ bool epr_project_increment_small_nb2(const EprLines& L, float2 tau, float2 dT, int newton_iters,
+                                                                float i_min, float& d0, float& d1) {
+  bool ok0, ok1;
   switch (L.n_bins) {
-    case 8: return epr_project_increment_small<8>(L, tau, dT, newton_iters, i_min, delta_out);
-    case 5: return epr_project_increment_small<5>(L, tau, dT, newton_iters, i_min, delta_out);
-    case 10: return epr_project_increment_small<10>(L, tau, dT, newton_iters, i_min, delta_out);
+    case 8: ok0 = epr_project_increment_small<8>(L, tau.x, dT.x, newton_iters, i_min, d0);
+            ok1 = epr_project_increment_small<8>(L, tau.y, dT.y, newton_iters, i_min, d1); break;
+    case 5: ok0 = epr_project_increment_small<5>(L, tau.x, dT.x, newton_iters, i_min, d0);
+            ok1 = epr_project_increment_small<5>(L, tau.y, dT.y, newton_iters, i_min, d1); break;
+    case 10: ok0 = epr_project_increment_small<10>(L, tau.x, dT.x, newton_iters, i_min, d0);
+             ok1 = epr_project_increment_small<10>(L, tau.y, dT.y, newton_iters, i_min, d1); break;
     default: return false;
   }
+  return ok0 && ok1;
 }
 
 // Projection to the single-thickness manifold, Eq. (7) + PAPER.md:233 (R10), as an increment:
