@@ -544,10 +544,20 @@ extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_
   if (iterations < 0 || !(step > 0.f)) FAIL(p, EPR_EINVAL, "epr_retrieve_host: iterations must be >= 0 and step > 0");
   const size_t plane = (size_t)p->nx * p->ny;
   // Host chunks are smaller than the device work batch so that the copies of chunk i±1 overlap the loop of chunk i:
-  // about 256 MB of input per chunk (EPR_HOST_CHUNK overrides), at least 4 chunks per call when the batch allows
+  // about 256 MB of input per chunk (EPR_HOST_CHUNK overrides), at least min_chunks chunks per call when the batch allows
   // (C2, batch 64: chunks of 8 / 12 / 16 / 24 projections give 1012 / 1044 / 1060 / 987 projections/s end to end).
+  // How many chunks a small batch is cut into follows the share of the copies: r = copy time / loop time per projection,
+  // from 8 B/px over the host link (about 50 GB/s) against (iterations + 1) x the loop's algorithmic bytes at about
+  // 2.5 TB/s.  Copies that are a small share (several lines: r < 0.1) are not worth loops over one or two projections,
+  // whose launches underfill the GPU (measured, batch 4: C4 120.7 / 133.8 / 138.7 and C5 80.8 / 88.8 / 90.9 projections/s
+  // with chunks of 1 / 2 / 4; C3, batch 8, r = 0.37: 464 / 542 / 542 / 500 with chunks of 1 / 2 / 4 / 8).
+  const int nbn = p->n_bins;
+  const double bpp = (p->solver == EPR_LOCAL) ? (nbn == 1 ? 40.0 : 24.0 + 24.0 * nbn) : (nbn == 1 ? 52.0 : 28.0 + 24.0 * nbn);
+  const double r = (8.0 / 50.0) / ((iterations + 1) * bpp / 2500.0);
+  const int min_chunks = r >= 0.3 ? 4 : r >= 0.15 ? 2 : 1;
   int wbch = (int)(((size_t)256 << 20) / (plane * sizeof(float)));
-  if (wbch > (batch + 3) / 4) wbch = (batch + 3) / 4;
+  if (wbch > (batch + min_chunks - 1) / min_chunks) wbch = (batch + min_chunks - 1) / min_chunks;
+  if (nbn == 1 && wbch < 2) wbch = 2;              // one plane per launch leaves most SMs idle
   { const char* env = getenv("EPR_HOST_CHUNK"); if (env && atoi(env) > 0) wbch = atoi(env); }
   if (wbch < 1) wbch = 1;
   if (wbch > p->work_batch) wbch = p->work_batch;
