@@ -350,7 +350,10 @@ def main():
 
     cmp_cufft = None
     if rank == 0 and m == 1 and not args.no_cufft_compare:
-        cmp_cufft = cufft_compare(epr, plan, B)
+        try:
+            cmp_cufft = cufft_compare(epr, plan, B)
+        except Exception as exc:                    # a comparison point must never cost the bench line
+            cmp_cufft = {"error": f"{type(exc).__name__}: {exc}"[:200]}
 
     if rank == 0:
         peak, peak_src = peaks()
