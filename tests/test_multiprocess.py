@@ -53,3 +53,31 @@ def test_two_rank_gloo_sharding(tmp_path):
     mp.spawn(_worker, args=(world, _free_port(), total, str(tmp_path)), nprocs=world, join=True)
     got = np.concatenate([np.load(tmp_path / f"r{k}.npy") for k in range(world)])
     assert np.array_equal(got, np.arange(total, dtype=np.float32) * 2.0)
+
+
+def _run_bench(env_extra, *args):
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, **env_extra)
+    return subprocess.run([sys.executable, os.path.join(root, "bench.py"), *args], cwd=root, env=env,
+                          capture_output=True, text=True, timeout=600)
+
+
+def test_bench_reference_arm_contract():
+    """`bench.py --impl reference` (the oracle on the host cores) prints ONE JSON line with the base contract's keys on
+    rank 0; under a multi-rank launch the other ranks exit 0 without work or output."""
+    import json
+    res = _run_bench({"RANK": "0", "WORLD_SIZE": "1"}, "--impl", "reference", "--config", "C1", "--steps", "1", "--warmup", "0")
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [ln for ln in res.stdout.splitlines() if ln.strip()]
+    assert len(lines) == 1
+    j = json.loads(lines[0])
+    assert j["impl"] == "reference" and j["unit"] == "projections/s" and j["higher_is_better"] is True
+    assert j["value"] > 0 and j["steps"] == 1 and j["dtype"] == "f64" and j["data"] == "synthetic"
+    assert j["cpu_baseline"]["kind"] == "oracle" and j["cpu_baseline"]["value"] == j["value"]
+    assert j["e2e"] == {"value": j["value"], "unit": j["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert j["config"]["workload"].startswith("C1")
+    other = _run_bench({"RANK": "1", "WORLD_SIZE": "2", "LOCAL_RANK": "1"}, "--impl", "reference", "--config", "C1",
+                       "--gpus", "2", "--steps", "1", "--warmup", "0")
+    assert other.returncode == 0 and other.stdout.strip() == ""
