@@ -456,7 +456,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
         unsigned rb = rb0, ab = ab0;
         float tn = lds_f32(rb - TP4), tc = lds_f32(rb), ts = lds_f32(rb + TP4), tl = lds_f32(rb - 4), tr = lds_f32(rb + 4);
         float2* mo = MAP_OUT ? map_out + pl + (size_t)(y0 + yb) * nx + (x0 + x) : nullptr;
-#pragma unroll 2
+#pragma unroll 8
         for (int r = 0; r < ROWS; ++r) {
           rb += TP4;                                   // one row beyond the strip at the last r: still inside the τ tile
           const float ts2 = lds_f32(rb + TP4), tl2 = lds_f32(rb - 4), tr2 = lds_f32(rb + 4);
