@@ -167,3 +167,96 @@ def test_nonlocal_wkb1_variant_keeps_mass_and_vanishes_for_exponentials():
     y, x = np.meshgrid(np.arange(16.0), np.arange(16.0), indexing="ij")
     W = O.wkb1_term(np.exp(0.03 * x - 0.02 * y), 3.0)
     assert np.max(np.abs(W[3:-3, 3:-3])) < 1e-12
+
+
+# --------------------------------------------------------------------------------------------------------------------
+# Closed-form pins of the polychromatic loop body: per-line filter coefficient, positivity-weighted
+# split, weighted-mean Paganin start, positivity floor.  Each of them is a number worked out by hand from the paper's
+# statement of the step, not a second call of the routine under test.
+# --------------------------------------------------------------------------------------------------------------------
+def _three_unequal_lines(L=3.0):
+    E = np.array([70.0, 100.0, 130.0])
+    lines = O.derive_lines(6.5e-6, L, E, [0.3, 0.45, 0.25], [600.0, 1000.0, 1500.0])
+    assert np.ptp(lines.a) > 0.2 * lines.a.mean() and np.ptp(lines.gamma) > 0.3          # unequal a_s and γ_s
+    return lines
+
+
+def _lam(ny, nx, my, mx):
+    """Discrete 5-point symbol of the mode cos(2π(mx x/nx + my y/ny)), written out (R5)."""
+    return (2.0 - 2.0 * np.cos(2 * np.pi * mx / nx)) + (2.0 - 2.0 * np.cos(2 * np.pi * my / ny))
+
+
+@pytest.mark.parametrize("solver", ["local", "nonlocal"])
+def test_one_iteration_from_constant_start_closed_form(solver):
+    """PAPER.md:231 "split [the residual] across spectral lines with positivity-weighted weights … apply a per-line
+    FFT-diagonal inverse".  Start from a CONSTANT τ⁰ = c: every P_s = I_s = f_s e^{−γ_s c} is constant (all differences
+    vanish, zero shift = identity transport), so w_s = I_s/T⁰ with T⁰ = Σ_s I_s, and for d = T⁰ + ε cos(θ·r) one
+    iteration gives   Σ_s I_s = T⁰ + step·ε·cos(θ·r)·Σ_s w_s/(1 + a_s λ(θ))   — each line filtered with ITS OWN a_s."""
+    lines = _three_unequal_lines()
+    ny, nx, my, mx, c, eps, step = 24, 32, 2, 3, 0.8, 1e-3, 0.7
+    y, x = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    mode = np.cos(2 * np.pi * (mx * x / nx + my * y / ny))
+    I0 = lines.f * np.exp(-lines.gamma * c)
+    T0 = I0.sum()
+    d = T0 + eps * mode
+    tau = O.retrieve(d, lines, solver, iterations=1, step=step, tau0=np.full((ny, nx), c))
+    got = np.sum(O.line_intensities(tau, lines), axis=0)
+    w = I0 / T0
+    gain = float(np.sum(w / (1.0 + lines.a * _lam(ny, nx, my, mx))))
+    want = T0 + step * eps * mode * gain
+    assert np.max(np.abs(got - want)) < 1e-12
+    # the pin has teeth: the weighted-mean coefficient, or weights f_s, would be off by far more than the tolerance
+    wrong_a = float(np.sum(w / (1.0 + lines.abar * _lam(ny, nx, my, mx))))
+    wrong_w = float(np.sum(lines.f / (1.0 + lines.a * _lam(ny, nx, my, mx))))
+    assert abs(wrong_a - gain) * step * eps > 1e-7 and abs(wrong_w - gain) * step * eps > 1e-7
+
+
+def test_paganin_init_several_lines_uses_weighted_mean_coefficient():
+    """R9 with PAPER.md:51: the start is ONE linear Paganin solve with ā = Σ_s f_s a_s, so for d = 1 + ε cos(θ·r) the
+    total intensity of the start is 1 + ε cos(θ·r)/(1 + ā λ(θ)), ā worked out here from the physical constants."""
+    lines = _three_unequal_lines()
+    ny, nx, my, mx, eps = 20, 28, 1, 4, 2e-3
+    y, x = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    mode = np.cos(2 * np.pi * (mx * x / nx + my * y / ny))
+    E, wgt, db = np.array([70.0, 100.0, 130.0]), np.array([0.3, 0.45, 0.25]), np.array([600.0, 1000.0, 1500.0])
+    a_s = 3.0 * O.HC_KEV_M / (2 * np.pi * E) / (6.5e-6) ** 2 * db / 2.0          # (L/k_s p²)·db_s/2
+    abar = float(np.sum(wgt / wgt.sum() * a_s))
+    tau = O.paganin_init(1.0 + eps * mode, lines)
+    got = np.sum(O.line_intensities(tau, lines), axis=0)
+    assert np.max(np.abs(got - (1.0 + eps * mode / (1.0 + abar * _lam(ny, nx, my, mx))))) < 1e-13
+    assert abs(1.0 / (1.0 + a_s[0] * _lam(ny, nx, my, mx)) - 1.0 / (1.0 + abar * _lam(ny, nx, my, mx))) * eps > 1e-6
+
+
+def test_split_weights_hand_computed():
+    """R8 ("positivity-weighted"): w_s = P_s⁺/Σ_t P_t⁺.  (0.3, 0.1) → (0.75, 0.25); a negative prediction
+    gets no share: (−0.2, 0.5) → (0, 1); both non-positive → the spectral fractions f_s."""
+    lines = O.derive_lines(6.5e-6, 3.0, [80.0, 120.0], [0.4, 0.6], [800.0, 1200.0])
+    P = [np.array([[0.3, -0.2, -0.1, 0.0]]), np.array([[0.1, 0.5, -0.3, 0.0]])]
+    w = O.split_weights(P, lines)
+    assert np.allclose(w[0][0, :2], [0.75, 0.0], atol=1e-15) and np.allclose(w[1][0, :2], [0.25, 1.0], atol=1e-15)
+    assert np.allclose(w[0][0, 2:], 0.4, atol=1e-15) and np.allclose(w[1][0, 2:], 0.6, atol=1e-15)
+
+
+@pytest.mark.parametrize("n_lines", [1, 3])
+def test_positivity_floor_returns_tau_of_i_min(n_lines):
+    """PAPER.md:225 "nonnegative spectral components": the total intensity is floored at i_min before it is put back on
+    the manifold Eq. (7).  With a vanishing propagation distance the filter is the identity, so step = 1 from a constant
+    start gives Σ_s I_s = d pixel by pixel; a pixel of d forced to −1 must come back at exactly the τ with
+    Σ_s f_s e^{−γ_s τ} = i_min (one line: τ = −ln i_min), in the start (R9) and in the loop."""
+    if n_lines == 1:
+        lines = O.derive_lines(6.5e-6, 1e-12, [100.0], [1.0], [1000.0])
+    else:
+        lines = _three_unequal_lines(L=1e-12)
+    assert np.max(lines.a) < 1e-9
+    i_min = 1e-3
+    d = np.full((8, 12), 0.9)
+    d[3, 5] = -1.0
+    for tau in (O.paganin_init(d, lines, i_min=i_min),
+                O.retrieve(d, lines, "local", iterations=1, step=1.0, i_min=i_min, tau0=np.full(d.shape, 0.2)),
+                O.retrieve(d, lines, "nonlocal", iterations=1, step=1.0, i_min=i_min, tau0=np.full(d.shape, 0.2))):
+        assert np.all(np.isfinite(tau))
+        T = np.sum(O.line_intensities(tau, lines), axis=0)
+        assert abs(T[3, 5] - i_min) < 1e-12 * i_min * 1e3
+        assert np.max(np.abs(np.delete(T.ravel(), 3 * 12 + 5) - 0.9)) < 1e-9
+        if n_lines == 1:
+            assert abs(tau[3, 5] + np.log(i_min)) < 1e-12
