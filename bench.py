@@ -59,17 +59,33 @@ def max_over_ranks(value, device):
     return float(t.item())
 
 
-def measured_traffic(kernel, nb, solver):
-    """DRAM bytes per pixel per launch of `kernel` from the committed `ncu --set full` capture
-    (profiles/r1_dram_traffic.json: dram__bytes_read.sum + dram__bytes_write.sum divided by the pixels of that launch),
-    or None when that kernel / configuration was not captured."""
-    path = os.path.join(ROOT, "profiles", "r1_dram_traffic.json")
+TRAFFIC_FILE = os.path.join("profiles", "r2_dram_traffic.json")
+
+
+def measured_traffic(epr, kernel, nb, solver, config, algorithmic_bytes_per_launch):
+    """DRAM bytes per launch of `kernel` from the committed `ncu --set full` capture (TRAFFIC_FILE: per kernel and
+    configuration, dram__bytes_read.sum + dram__bytes_write.sum of one launch divided by that launch's algorithmic
+    bytes), scaled to this run's launch size.  The capture names the library version it was taken from; when the
+    library loaded now reports another version the number is stale and null is returned instead.
+    Returns (bytes per launch or None, provenance string)."""
+    path = os.path.join(ROOT, TRAFFIC_FILE)
     try:
-        tab = json.load(open(path))["bytes_per_px"]
+        tab = json.load(open(path))
     except Exception:
-        return None
-    key = f"{kernel}:{solver}:{nb}"
-    return tab.get(key)
+        return None, f"{TRAFFIC_FILE} absent"
+    lib_now = epr.load_library().epr_version().decode()
+    if tab.get("lib_version") != lib_now:
+        return None, f"{TRAFFIC_FILE} was captured from '{tab.get('lib_version')}', library is '{lib_now}': stale, dropped"
+    ratio = tab.get("dram_over_algorithmic", {}).get(f"{config}:{kernel}")
+    if ratio is None:
+        return None, f"{TRAFFIC_FILE} has no capture of {kernel} at {config}"
+    return ratio * algorithmic_bytes_per_launch, f"{TRAFFIC_FILE} ({tab.get('command', 'ncu --set full')}; {tab.get('lib_version')})"
+
+
+def expected_launches_per_step(kernel, w, m):
+    """Launches of a kernel family in one epr_retrieve over a batch that fits the plan's work batch."""
+    it = w.iterations
+    return {"k_rows_r2c": it + 1, "k_cols": it + 1, "k_rows_c2r": it + 1, "k_resample": 2}.get(kernel, it)
 
 
 def peaks():
@@ -160,6 +176,62 @@ def oracle_time_one(w, j=0, m=1):
     return time.perf_counter() - t0
 
 
+def _oracle_sample_worker(a):
+    """One host process of the bounded oracle sample: the initial Paganin solve alone (iterations = 0) and the initial
+    solve plus ONE correction iteration on one projection; returns the two wall times."""
+    (d, pixel_m, L_m, energy, weight, db, solver, step, S) = a
+    from oracle import epr_oracle as O
+    lines = O.derive_lines(pixel_m, L_m, energy, weight, db)
+    d64 = d.astype(np.float64)
+    t0 = time.perf_counter()
+    O.retrieve(d64, lines, solver, 0, step, S=S)
+    t1 = time.perf_counter()
+    O.retrieve(d64, lines, solver, 1, step, S=S)
+    t2 = time.perf_counter()
+    return t1 - t0, t2 - t1
+
+
+def host_procs(w):
+    """All host cores, unless the host's free memory cannot hold that many oracle processes (one fp64 retrieval keeps
+    about 5 planes per line alive: ~45 planes of 8 bytes per pixel for 8 lines)."""
+    cores = os.cpu_count() or 1
+    try:
+        import psutil
+        need = 8.0 * w.nx * w.ny * (6 * w.n_bins + 8) * 1.5
+        cores = max(1, min(cores, int(psutil.virtual_memory().available * 0.6 / need)))
+    except Exception:
+        pass
+    return cores
+
+
+def oracle_sample(w, procs):
+    """Bounded sample of the oracle for the expensive configurations (a full 8-line retrieval takes minutes per
+    projection): `procs` host processes (multiprocessing, one projection each, all running at once, so that memory
+    bandwidth contention is in the number) time the initial solve and the initial solve + 1 iteration; the cost of the
+    workload's `iterations` is extrapolated linearly, t = t_init + iterations · (t_1 − t_init) — every iteration of the
+    oracle does the same work.  Returns the cpu_baseline object."""
+    import multiprocessing as mp
+    B = w.d.shape[0]
+    idx = [0, B // 2, B - 1] if B >= 3 else list(range(B))           # BASELINE.md §3: projections 0 / 31 / 63 of C5
+    jobs = [(w.d[idx[k % len(idx)]], w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver, w.step,
+             w.max_shift_px) for k in range(procs)]
+    t0 = time.perf_counter()
+    if procs == 1:
+        res = [_oracle_sample_worker(jobs[0])]
+    else:
+        with mp.get_context("spawn").Pool(procs) as pool:
+            res = pool.map(_oracle_sample_worker, jobs)
+    wall = time.perf_counter() - t0
+    t_init = max(r[0] for r in res)
+    t_one = max(r[1] for r in res)
+    t_full = t_init + w.iterations * max(t_one - t_init, 0.0)
+    return {"value": procs / t_full, "unit": UNIT, "cores": procs, "kind": "oracle",
+            "sample": f"{procs} process(es) x 1 projection ({w.ny}x{w.nx}, {w.n_bins} line(s)) at once: initial solve "
+                      f"{t_init:.2f} s, initial solve + 1 iteration {t_one:.2f} s (slowest process); extrapolated to "
+                      f"{w.iterations} iterations = {t_full:.1f} s per projection per process; sample wall {wall:.1f} s; "
+                      f"numpy fp64, host has {os.cpu_count()} cores"}
+
+
 def cufft_compare(epr, plan, B, reps=5):
     """Comparison point only (north_star: "a cuFFT-based variant is kept only as a reported comparison point"): the
     a4 preconditioner q_s = IFFT2(H_s FFT2(r_s)), H_s = 1/(1 + a_s λ) with the discrete 5-point symbol (PAPER.md:51,
@@ -229,55 +301,22 @@ def run_reference(args, rank):
     }))
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C2")
-    ap.add_argument("--batch", type=int, default=64)
-    ap.add_argument("--distinct", type=int, default=2, help="distinct simulated projections (rest: new noise only)")
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-cufft-compare", action="store_true",
-                    help="skip the preconditioner-through-cuFFT comparison point (rank 0, outside every timed region)")
-    ap.add_argument("--lines", type=int, default=0,
-                    help="retrieve with this many spectral lines (60-140 keV, Gaussian weights) instead of the config's own "
-                         "discretisation, e.g. --config C2 --lines 5: the paper's 'local L2 poly' rows (PAPER.md:116-119)")
-    ap.add_argument("--oversample", type=int, default=1,
-                    help="run the loop on the grid refined this many times (PAPER.md:79; epr_retrieve_oversampled)")
-    args = ap.parse_args()
-    args.warmup = max(args.warmup, 0)
-
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
-        run_reference(args, rank)
-        return
-
+def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, lines=0, m=1, cufft=False):
+    """Time one configuration: K steps of epr_retrieve over B resident projections (CUDA events on the launch stream),
+    the same through epr_retrieve_host with pinned host buffers, and a profiling pass with the in-library per-kernel
+    events.  Returns the pieces of the JSON line for this configuration (everything already reduced over ranks)."""
     import torch
     import torch.distributed as dist
-    import paper_2601_22793_b200 as epr
     from epr_inputs import make_workload
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    args.warmup = max(args.warmup, 3)
-
-    B = args.batch
-    w = make_workload(args.config, batch=B, distinct=min(args.distinct, B))
-    if args.lines > 0:
-        override_lines(w, args.lines)
+    w = make_workload(name, batch=B, distinct=min(distinct, B))
+    if lines > 0:
+        override_lines(w, lines)
     if world > 1:                                   # every rank gets its own noise realisations
         rng = np.random.default_rng(4000 + rank)
         w.d = np.ascontiguousarray(w.d[rng.permutation(B)])
     plane = w.nx * w.ny
     nb = w.n_bins
-    m = args.oversample
     plan = epr.epr_plan(m * w.nx, m * w.ny, w.pixel_m / m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
                         max_batch=B, max_shift_px=w.max_shift_px if m == 1 else fine_shift_clamp(w, m))
     d_host = torch.from_numpy(w.d).pin_memory()
@@ -313,11 +352,11 @@ def main():
     flush = None
     if in_bytes <= 2 * 126e6:
         flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         step()
     barrier()
     l0 = plan.launches
-    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     with ClockSampler(local) as clk:
         for e0, e1 in evs:
             if flush is not None:
@@ -329,85 +368,162 @@ def main():
     ms = sum(e0.elapsed_time(e1) for e0, e1 in evs)
     launches = plan.launches - l0
     ms = max_over_ranks(ms, torch.device("cuda", local))
-    value = world * B * args.steps / (ms * 1e-3)
+    value = world * B * steps / (ms * 1e-3)
 
     # ---- end to end through the public host API: pinned host buffers, H2D + loop + D2H inside the timed region
     step_host()
     barrier()
     t0 = time.perf_counter()
-    for _ in range(args.steps):
+    for _ in range(steps):
         step_host()
     e2e_s = time.perf_counter() - t0
     e2e_s = max_over_ranks(e2e_s, torch.device("cuda", local))
-    e2e = world * B * args.steps / e2e_s
+    e2e = world * B * steps / e2e_s
 
     # ---- per-kernel device times (CUDA events around every launch, on the launch stream), same K steps
     plan.profile(True)
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     prof = plan.profile_read()
     plan.profile(False)
+    flags = plan.read_flags()
 
     cmp_cufft = None
-    if rank == 0 and m == 1 and not args.no_cufft_compare:
+    if rank == 0 and m == 1 and cufft:
         try:
             cmp_cufft = cufft_compare(epr, plan, B)
         except Exception as exc:                    # a comparison point must never cost the bench line
             cmp_cufft = {"error": f"{type(exc).__name__}: {exc}"[:200]}
 
-    if rank == 0:
-        peak, peak_src = peaks()
-        per_kernel = []
-        for name, (tot_ms, cnt) in prof.items():
-            bpp = kernel_bytes_per_px(name, nb, w.solver)
-            # px per launch: every launch covers the whole batch; r2c covers nb planes per projection in the loop
-            launches_per_step = cnt / args.steps
-            px = B * plane * m * m                  # pixels of the computational grid
-            if name == "k_rows_r2c":
-                # (iterations launches of nb planes + 1 init launch of 1 plane) per step
-                px = px * (w.iterations * nb + 1) / (w.iterations + 1)
-            if name == "k_resample":                # replication: R 4/m² + W 4; block mean: R 4 + W 4/m²; one launch each
-                bpp = 4.0 + 4.0 / (m * m)
-            avg_ms = tot_ms / cnt
-            gbs = bpp * px / (avg_ms * 1e-3) / 1e9
-            per_kernel.append({"kernel": name, "launches_per_step": launches_per_step, "avg_ms": avg_ms,
-                               "share": None, "algorithmic_bytes_per_launch": bpp * px, "achieved_gbs": gbs,
-                               "frac": gbs / peak})
-        tot = sum(k["avg_ms"] * k["launches_per_step"] for k in per_kernel)
-        for k in per_kernel:
-            k["share"] = k["avg_ms"] * k["launches_per_step"] / tot
-        per_kernel.sort(key=lambda k: -k["share"])
-        dom = per_kernel[0]
-        tpp = measured_traffic(dom["kernel"], nb, w.solver)
-        traffic = None if tpp is None else tpp * dom["algorithmic_bytes_per_launch"] / kernel_bytes_per_px(dom["kernel"], nb, w.solver)
-        roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved_gbs"], "peak": peak,
-                    "unit": "GB/s", "frac": dom["frac"], "traffic": traffic, "peak_source": peak_src,
-                    "per_kernel": per_kernel}
-        result = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"{args.config}: {w.ny}x{w.nx}, {nb} line(s), {w.solver} solver, "
-                                   f"{w.iterations} iterations, step {w.step}"
-                                   + (f", oversampling {m} (computational grid {m * w.ny}x{m * w.nx})" if m > 1 else ""),
-                       "batch_per_gpu": B, "work_batch": None,
-                       "l2": (f"inputs {in_bytes / 1e6:.0f} MB per step > 2 x 126 MB L2: no flush needed" if flush is None else
-                              f"inputs {in_bytes / 1e6:.0f} MB per step: L2 flushed (256 MB overwrite) between timed steps"),
-                       "ms_per_iteration_per_projection": ms / args.steps / B / (w.iterations + 1)},
-            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": B * plane * 4, "d2h_bytes_per_step": B * plane * 4},
-            "gpu_launches": int(launches) * world,
-            "clocks": clk.summary(),
-            "roofline": roofline,
-        }
-        if cmp_cufft is not None:
-            result["cufft_compare"] = cmp_cufft
-        if not args.no_cpu_baseline:
-            t1 = oracle_time_one(w, m=m)
-            result["cpu_baseline"] = {"value": 1.0 / t1, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                      "sample": f"1 of the {B} projections ({w.ny}x{w.nx}, all {w.iterations} "
-                                                f"iterations) in {t1:.1f} s, numpy fp64, host has {os.cpu_count()} cores"}
-        print(json.dumps(result))
+    peak, peak_src = peaks()
+    per_kernel = []
+    for kname, (tot_ms, cnt) in prof.items():
+        bpp = kernel_bytes_per_px(kname, nb, w.solver)
+        # px per launch: every launch covers the whole batch; r2c covers nb planes per projection in the loop
+        launches_per_step = cnt / steps
+        px = B * plane * m * m                  # pixels of the computational grid
+        if kname == "k_rows_r2c":
+            # (iterations launches of nb planes + 1 init launch of 1 plane) per step
+            px = px * (w.iterations * nb + 1) / (w.iterations + 1)
+        if kname == "k_resample":                # replication: R 4/m² + W 4; block mean: R 4 + W 4/m²; one launch each
+            bpp = 4.0 + 4.0 / (m * m)
+        # a batch larger than the plan's work batch goes through the loop in passes: launches cover B / passes projections
+        passes = max(1, round(launches_per_step / expected_launches_per_step(kname, w, m)))
+        px = px / passes
+        avg_ms = tot_ms / cnt
+        gbs = bpp * px / (avg_ms * 1e-3) / 1e9
+        per_kernel.append({"kernel": kname, "launches_per_step": launches_per_step, "avg_ms": avg_ms,
+                           "share": None, "algorithmic_bytes_per_launch": bpp * px, "achieved_gbs": gbs,
+                           "frac": gbs / peak})
+    tot = sum(k["avg_ms"] * k["launches_per_step"] for k in per_kernel)
+    for k in per_kernel:
+        k["share"] = k["avg_ms"] * k["launches_per_step"] / tot
+    per_kernel.sort(key=lambda k: -k["share"])
+    dom = per_kernel[0]
+    traffic, traffic_src = measured_traffic(epr, dom["kernel"], nb, w.solver, name, dom["algorithmic_bytes_per_launch"])
+    # whole-iteration view: algorithmic bytes of one iteration (sum over the loop's kernels) over the time per iteration
+    roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved_gbs"], "peak": peak,
+                "unit": "GB/s", "frac": dom["frac"], "traffic": traffic, "traffic_source": traffic_src,
+                "peak_source": peak_src, "per_kernel": per_kernel}
+    res = {
+        "value": value, "unit": UNIT, "ms_per_step": ms / steps, "steps": steps, "warmup": warmup,
+        "config": {"workload": f"{name}: {w.ny}x{w.nx}, {nb} line(s), {w.solver} solver, "
+                               f"{w.iterations} iterations, step {w.step}"
+                               + (f", oversampling {m} (computational grid {m * w.ny}x{m * w.nx})" if m > 1 else ""),
+                   "batch_per_gpu": B, "distinct_projections": min(distinct, B),
+                   "l2": (f"inputs {in_bytes / 1e6:.0f} MB per step > 2 x 126 MB L2: no flush needed" if flush is None else
+                          f"inputs {in_bytes / 1e6:.0f} MB per step: L2 flushed (256 MB overwrite) between timed steps"),
+                   "ms_per_iteration_per_projection": ms / steps / B / (w.iterations + 1)},
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": B * plane * 4, "d2h_bytes_per_step": B * plane * 4,
+                "api": "epr_retrieve_host (pinned host buffers, chunks double-buffered on three streams)"},
+        "gpu_launches": int(launches) * world,
+        "clocks": clk.summary(),
+        "roofline": roofline,
+        "flags": flags,
+    }
+    if cmp_cufft is not None:
+        res["cufft_compare"] = cmp_cufft
     plan.destroy()
+    del d, out, d_host, out_host, flush
+    torch.cuda.empty_cache()
+    return res, w
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C2")
+    ap.add_argument("--batch", type=int, default=0, help="projections per GPU and step (default: 64 for C2 / C5, 16 for C3, 8 for C4)")
+    ap.add_argument("--distinct", type=int, default=2, help="distinct simulated projections (rest: new noise only)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cufft-compare", action="store_true",
+                    help="skip the preconditioner-through-cuFFT comparison point (rank 0, outside every timed region)")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="headline configuration only: skip the C3 / C4 / C5 sub-results of the default run")
+    ap.add_argument("--lines", type=int, default=0,
+                    help="retrieve with this many spectral lines (60-140 keV, Gaussian weights) instead of the config's own "
+                         "discretisation, e.g. --config C2 --lines 5: the paper's 'local L2 poly' rows (PAPER.md:116-119)")
+    ap.add_argument("--oversample", type=int, default=1,
+                    help="run the loop on the grid refined this many times (PAPER.md:79; epr_retrieve_oversampled)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_2601_22793_b200 as epr
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    args.warmup = max(args.warmup, 3)
+    default_batch = {"C1": 64, "C2": 64, "C3": 16, "C4": 8, "C5": 64}
+    B = args.batch if args.batch > 0 else default_batch[args.config]
+
+    head, w = measure_config(epr, args.config, B, args.steps, args.warmup, args.distinct, rank, world, local,
+                             lines=args.lines, m=args.oversample, cufft=not args.no_cufft_compare)
+    result = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+              "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+              "vs_baseline": None, "dtype": "f32", "data": "synthetic"}
+    for k in ("config", "e2e", "gpu_launches", "clocks", "roofline", "flags", "cufft_compare"):
+        if k in head:
+            result[k] = head[k]
+    if rank == 0 and not args.no_cpu_baseline:
+        t1 = oracle_time_one(w, m=args.oversample)
+        result["cpu_baseline"] = {"value": 1.0 / t1, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                  "sample": f"1 of the {B} projections ({w.ny}x{w.nx}, all {w.iterations} "
+                                            f"iterations) in {t1:.1f} s, numpy fp64, host has {os.cpu_count()} cores"}
+    del w
+
+    # ---- the other BASELINE.json configurations, each measured the same way (same protocol, fewer steps), in the same
+    # line: C3 (non-local, one line), C4 (non-local, 8 lines), C5 (2560 x 2160, 8 lines, batch 64 — more than the
+    # plan's work batch holds, so the device call passes through HBM in sub-batches and the host call streams chunks)
+    default_run = (args.config == "C2" and args.lines == 0 and args.oversample == 1 and args.batch == 0)
+    if default_run and not args.no_other_configs:
+        other = {}
+        for name, ob, osteps in (("C3", 16, 3), ("C4", 8, 3), ("C5", 64, 2)):
+            try:
+                r, ow = measure_config(epr, name, ob, osteps, 3, args.distinct, rank, world, local)
+                if rank == 0 and not args.no_cpu_baseline:
+                    r["cpu_baseline"] = oracle_sample(ow, host_procs(ow) if name == "C5" else 1)
+                del ow
+                other[name] = r
+            except Exception as exc:                # a sub-result must never cost the headline
+                other[name] = {"error": f"{type(exc).__name__}: {exc}"[:300]}
+        result["other_configs"] = other
+    if rank == 0:
+        print(json.dumps(result))
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()

@@ -14,7 +14,9 @@
  *    return; epr_plan / epr_destroy / epr_retrieve_host may synchronise.
  *  - Every call returns an epr_status; nothing throws or exits.  On EPR_EINVAL / EPR_ESIZE nothing has been
  *    enqueued.  epr_last_error(plan) gives a NUL-terminated message owned by the plan.
- *  - A plan is not thread-safe; distinct plans are independent.
+ *  - A plan is not thread-safe; distinct plans are independent, also across threads and devices: a plan belongs to
+ *    the CUDA device that was current in epr_plan, every call runs there (whatever device is current in the caller)
+ *    and restores the caller's device.
  *  - d is the flat-field-normalised detector intensity (≈ 1 in the empty beam; Σ_s f_s = 1).
  *  - The state of the iteration is the nominal thickness field τ of Eq. (7):
  *    I_s = f_s exp(−γ_s τ).  The phase of line s is φ_s = −(δ_s/2β_s) γ_s τ (Eq. (6)).
@@ -126,10 +128,23 @@ epr_status epr_retrieve_oversampled(epr_plan_t plan, int factor, int batch, cons
 epr_status epr_set_diagnostics(epr_plan_t plan, float* diag, int capacity_iters);
 
 /* epr_retrieve_host — same, with HOST buffers (pinned for full speed): copies d host→device, runs the loop,
- *   copies the result device→host, in chunks of max_batch projections with copies overlapped with compute;
- *   returns after the last copy has completed.  `batch` may exceed max_batch. */
+ *   copies the result device→host.  The batch is cut into chunks of about 256 MB of input (never more than the plan's
+ *   work batch; environment EPR_HOST_CHUNK = projections per chunk overrides) that travel on three private streams, so
+ *   that the copy in of chunk i + 1 and the copy out of chunk i − 1 overlap the loop of chunk i; the first and last
+ *   chunks are smaller (their copies overlap nothing).  `batch` may exceed max_batch.  The call first waits for all
+ *   work enqueued earlier on the device (cudaDeviceSynchronize) and returns after its last copy has completed. */
 epr_status epr_retrieve_host(epr_plan_t plan, int batch, const float* d_host, float* out_host, int iterations,
                              float step);
+
+/* epr_read_flags — conditions kernels detected since the flags were last cleared (synchronises the device).
+ *   EPR_FLAG_SPLAT_OVERFLOW: the non-local forward accumulates each line's detector plane in 32-bit fixed point (unit
+ *   2^-26 of the flat field; order-independent, exactly mass conserving).  A detector pixel of one line that collects
+ *   32x the flat field or more leaves that range; the flag is raised when an accumulator reads negative, i.e. for
+ *   totals in [32, 64)x (it wraps silently beyond 64x, and epr_transport, whose planes may be negative, never raises
+ *   it).  Physical caustics of the paper's regime stay below ~10x.
+ *   *flags receives the bits; clear != 0 resets them. */
+#define EPR_FLAG_SPLAT_OVERFLOW 1u
+epr_status epr_read_flags(epr_plan_t plan, unsigned* flags, int clear);
 
 /* Per-line scalars the plan derived (HOST arrays of length n_bins, any may be NULL): f_s, γ_s, a_s, α_s. */
 epr_status epr_plan_lines(epr_plan_t plan, double* f, double* gamma, double* a, double* alpha);

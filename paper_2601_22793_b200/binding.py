@@ -13,7 +13,8 @@ _LIB = None
 
 EXPORTS = ["epr_default_options", "epr_plan", "epr_forward", "epr_adjoint", "epr_transport", "epr_precondition",
            "epr_retrieve", "epr_retrieve_oversampled", "epr_set_diagnostics", "epr_retrieve_host", "epr_plan_lines", "epr_launch_count", "epr_destroy",
-           "epr_last_error", "epr_version", "epr_profile_enable", "epr_profile_read"]
+           "epr_last_error", "epr_version", "epr_profile_enable", "epr_profile_read", "epr_read_flags"]
+EPR_FLAG_SPLAT_OVERFLOW = 1
 
 
 class EprError(RuntimeError):
@@ -63,6 +64,8 @@ def load_library():
     lib.epr_profile_enable.restype = ci
     lib.epr_profile_read.argtypes = [vp, ci, C.POINTER(C.c_char_p), C.POINTER(cd), C.POINTER(C.c_longlong), ci]
     lib.epr_profile_read.restype = ci
+    lib.epr_read_flags.argtypes = [vp, C.POINTER(C.c_uint), ci]
+    lib.epr_read_flags.restype = ci
     lib.epr_last_error.argtypes = [vp]
     lib.epr_last_error.restype = C.c_char_p
     lib.epr_version.restype = C.c_char_p
@@ -122,6 +125,12 @@ class Plan:
         cnt = (C.c_longlong * n)()
         k = load_library().epr_profile_read(self._h, n, names, ms, cnt, 1 if reset else 0)
         return {names[i].decode(): (float(ms[i]), int(cnt[i])) for i in range(k)}
+
+    def read_flags(self, clear=True):
+        """EPR_FLAG_* bits raised by kernels since the last clear (epr_read_flags; synchronises)."""
+        v = C.c_uint(0)
+        self._check(load_library().epr_read_flags(self._h, C.byref(v), 1 if clear else 0))
+        return int(v.value)
 
     def destroy(self):
         if self._h is not None:
@@ -228,7 +237,8 @@ def epr_retrieve_host(plan, d_host, out_host, iterations, step):
             if a.dtype != np.float32 or not a.flags.c_contiguous:
                 raise TypeError(f"{name}: expected C-contiguous float32")
             return C.c_void_p(a.ctypes.data), a.shape
-        if a.is_cuda or a.dtype.is_floating_point is False or not a.is_contiguous():
+        import torch
+        if not isinstance(a, torch.Tensor) or a.is_cuda or a.dtype != torch.float32 or not a.is_contiguous():
             raise TypeError(f"{name}: expected a contiguous float32 host tensor")
         return C.c_void_p(a.data_ptr()), tuple(a.shape)
     pd, sd = hp(d_host, "d_host")

@@ -51,13 +51,25 @@ struct EprProf {
     }                                                                          \
   } while (0)
 
+// Every entry point runs on the plan's device (function attributes, workspaces and streams belong to it) and restores
+// the caller's current device on return.
+struct DevGuard {
+  int prev = -1;
+  explicit DevGuard(const epr_plan_s* p) {
+    if (!p) return;
+    int cur = 0;
+    if (cudaGetDevice(&cur) == cudaSuccess && cur != p->device) { prev = cur; cudaSetDevice(p->device); }
+  }
+  ~DevGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 extern "C" void epr_default_options(epr_options* o) {
   if (!o) return;
   o->order = 2; o->wkb1 = 1; o->symbol = 0; o->max_shift_px = 16.f; o->i_min = 1e-6f; o->newton_iters = 4;
   o->init = 0; o->output = 0; o->out_bin = 0; o->mu_rel = NULL; o->nonlocal_wkb1 = 0;
 }
 
-extern "C" const char* epr_version(void) { return "epr-b200 0.1 (sm_100a)"; }
+extern "C" const char* epr_version(void) { return "epr-b200 0.2.0 (sm_100a)"; }
 
 extern "C" const char* epr_last_error(epr_plan_t p) { return p ? p->err : "null plan"; }
 
@@ -156,6 +168,8 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
   *out = p;                                   // returned even on failure so that the caller can read the message
   p->nx = nx; p->ny = ny; p->n_bins = n_bins; p->max_batch = max_batch; p->solver = (int)solver; p->opt = o;
   p->opt.mu_rel = NULL;
+  CU(p, cudaGetDevice(&p->device));
+  CU(p, cudaDeviceGetAttribute(&p->sms, cudaDevAttrMultiProcessorCount, p->device));
   p->graph_mode = 1;
   { const char* g = getenv("EPR_GRAPH"); if (g) p->graph_mode = atoi(g); }
 
@@ -221,6 +235,8 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
   p->work_batch = work;
   const size_t wb = (size_t)work;
   cudaError_t e = cudaSuccess;
+  if (e == cudaSuccess) e = cudaMalloc((void**)&p->d_flags, 4 * sizeof(unsigned));
+  if (e == cudaSuccess) e = cudaMemset(p->d_flags, 0, 4 * sizeof(unsigned));
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->tau, wb * plane * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->pred, wb * n_bins * plane * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->res, wb * n_bins * plane * sizeof(float));
@@ -259,6 +275,7 @@ extern "C" epr_status epr_profile_enable(epr_plan_t p, int on) {
 extern "C" int epr_profile_read(epr_plan_t p, int max_kernels, const char** names, double* total_ms, long long* count,
                                 int reset) {
   if (!p || !p->prof) return 0;
+  DevGuard dg(p);
   EprProf* pr = (EprProf*)p->prof;
   cudaDeviceSynchronize();
   for (auto& r : pr->recs) {
@@ -291,11 +308,23 @@ extern "C" epr_status epr_plan_lines(epr_plan_t p, double* f, double* gamma, dou
   return EPR_OK;
 }
 
+extern "C" epr_status epr_read_flags(epr_plan_t p, unsigned* flags, int clear) {
+  if (!p) return EPR_EINVAL;
+  if (!flags) FAIL(p, EPR_EINVAL, "epr_read_flags: NULL pointer");
+  DevGuard dg(p);
+  CU(p, cudaDeviceSynchronize());
+  CU(p, cudaMemcpy(flags, p->d_flags, sizeof(unsigned), cudaMemcpyDeviceToHost));
+  if (clear) CU(p, cudaMemset(p->d_flags, 0, sizeof(unsigned)));
+  return EPR_OK;
+}
+
 extern "C" epr_status epr_destroy(epr_plan_t p) {
   if (!p) return EPR_EINVAL;
+  DevGuard dg(p);
   cudaDeviceSynchronize();
   cudaFree(p->tw_row); cudaFree(p->tw_r2c); cudaFree(p->tw_col); cudaFree(p->tw_col_inv); cudaFree(p->lam_x); cudaFree(p->lam_y);
   cudaFree(p->tau); cudaFree(p->pred); cudaFree(p->res); cudaFree(p->res2); cudaFree(p->spec); cudaFree(p->spec_sum);
+  cudaFree(p->d_flags);
   cudaFree(p->raymap); cudaFree(p->gmax); cudaFree(p->os_d); cudaFree(p->os_out); cudaFree(p->diag_partial);
   if (p->graph_exec) cudaGraphExecDestroy(p->graph_exec);
   if (p->prof) { epr_profile_read(p, 0, NULL, NULL, NULL, 1); delete (EprProf*)p->prof; }
@@ -315,7 +344,7 @@ static epr_status check_call(epr_plan_t p, int batch) {
 // ----------------------------------------------------------------------------------------------- operators
 static epr_status ensure_raymap(epr_plan_t p) {
   if (p->raymap) return EPR_OK;
-  const size_t n = (size_t)p->work_batch * p->n_bins * p->nx * p->ny;
+  const size_t n = (size_t)p->max_batch * p->n_bins * p->nx * p->ny;       // the whole batch: epr_adjoint / epr_transport follow
   cudaError_t e = cudaMalloc((void**)&p->raymap, n * sizeof(float2));
   if (e != cudaSuccess) FAIL(p, EPR_ENOMEM, "ray map storage: %s", cudaGetErrorString(e));
   return EPR_OK;
@@ -324,27 +353,32 @@ static epr_status ensure_raymap(epr_plan_t p) {
 extern "C" epr_status epr_forward(epr_plan_t p, int batch, const float* tau, float* P_sum, float* P_bins, void* stream) {
   epr_status st = check_call(p, batch);
   if (st != EPR_OK) return st;
+  DevGuard dg(p);
   if (!tau || !P_sum) FAIL(p, EPR_EINVAL, "epr_forward: NULL tau or P_sum");
-  if (batch > p->work_batch) FAIL(p, EPR_EINVAL, "epr_forward: batch %d exceeds the plan's work batch %d", batch, p->work_batch);
   cudaStream_t cs = (cudaStream_t)stream;
   const size_t plane = (size_t)p->nx * p->ny;
-  if (p->solver == EPR_LOCAL) {
-    KL(p, K_FWD_LOCAL, cs, epr_launch_forward_local(p, batch, tau, NULL, p->pred, cs));
-    KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, P_sum, P_bins, cs));
-  } else {
-    if ((st = ensure_raymap(p)) != EPR_OK) return st;
-    KL(p, K_SPLAT, cs, epr_launch_splat(p, batch, tau, NULL, NULL, p->raymap, p->pred, 0, NULL, cs));
-    p->launches += 1;                                  // k_grad_blockmax, launched ahead of the splat
-    if (p->opt.nonlocal_wkb1) KL(p, K_WKB1, cs, epr_launch_wkb1_sub(p, batch, tau, p->pred, cs));
-    KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, batch, p->pred, P_sum, P_bins, cs));
-    p->raymap_batch = batch;
+  if (p->solver == EPR_NONLOCAL && (st = ensure_raymap(p)) != EPR_OK) return st;
+  for (int b0 = 0; b0 < batch; b0 += p->work_batch) {         // the prediction workspace holds work_batch projections
+    const int nb = (batch - b0 < p->work_batch) ? batch - b0 : p->work_batch;
+    const float* t = tau + (size_t)b0 * plane;
+    float* Ps = P_sum + (size_t)b0 * plane;
+    float* Pb = P_bins ? P_bins + (size_t)b0 * p->n_bins * plane : NULL;
+    if (p->solver == EPR_LOCAL) {
+      KL(p, K_FWD_LOCAL, cs, epr_launch_forward_local(p, nb, t, NULL, p->pred, cs));
+    } else {
+      KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, t, NULL, NULL, p->raymap + (size_t)b0 * p->n_bins * plane, p->pred, 0, NULL, cs));
+      if (p->opt.nonlocal_wkb1) KL(p, K_WKB1, cs, epr_launch_wkb1_sub(p, nb, t, p->pred, cs));
+    }
+    KL(p, K_PRED_OUT, cs, epr_launch_pred_out(p, nb, p->pred, Ps, Pb, cs));
   }
+  if (p->solver == EPR_NONLOCAL) p->raymap_batch = batch;
   return EPR_OK;
 }
 
 extern "C" epr_status epr_adjoint(epr_plan_t p, int batch, const float* e_bins, float* r_bins, void* stream) {
   epr_status st = check_call(p, batch);
   if (st != EPR_OK) return st;
+  DevGuard dg(p);
   if (!e_bins || !r_bins) FAIL(p, EPR_EINVAL, "epr_adjoint: NULL pointer");
   cudaStream_t cs = (cudaStream_t)stream;
   const size_t n = (size_t)batch * p->n_bins * p->nx * p->ny;
@@ -361,6 +395,7 @@ extern "C" epr_status epr_adjoint(epr_plan_t p, int batch, const float* e_bins, 
 extern "C" epr_status epr_transport(epr_plan_t p, int batch, const float* I_bins, float* P_bins, void* stream) {
   epr_status st = check_call(p, batch);
   if (st != EPR_OK) return st;
+  DevGuard dg(p);
   if (!I_bins || !P_bins) FAIL(p, EPR_EINVAL, "epr_transport: NULL pointer");
   if (p->solver != EPR_NONLOCAL) FAIL(p, EPR_EINVAL, "epr_transport: non-local plans only");
   if (!p->raymap || p->raymap_batch < batch) FAIL(p, EPR_EINVAL, "epr_transport: no ray map stored for batch %d (call epr_forward first)", batch);
@@ -374,6 +409,7 @@ extern "C" epr_status epr_transport(epr_plan_t p, int batch, const float* I_bins
 extern "C" epr_status epr_precondition(epr_plan_t p, int batch, const float* r_bins, float* q_bins, void* stream) {
   epr_status st = check_call(p, batch);
   if (st != EPR_OK) return st;
+  DevGuard dg(p);
   if (!r_bins || !q_bins) FAIL(p, EPR_EINVAL, "epr_precondition: NULL pointer");
   cudaStream_t cs = (cudaStream_t)stream;
   const size_t plane = (size_t)p->nx * p->ny;
@@ -416,15 +452,12 @@ static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* ta
     } else {
       if (p->opt.nonlocal_wkb1) {                      // variant: splat, WKB1 term, then the separate residual kernel
         KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->pred, 0, NULL, cs));
-        p->launches += 1;
         KL(p, K_WKB1, cs, epr_launch_wkb1_sub(p, nb, tau, p->pred, cs));
         KL(p, K_RESIDUAL, cs, epr_launch_residual(p, nb, d, p->pred, p->res, cs));
       } else if (p->n_bins == 1) {
         KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->res, 2, d, cs));       // a0 + a1-N + a2 fused
-        p->launches += 1;                                  // k_grad_blockmax, launched ahead of the splat
       } else {
         KL(p, K_SPLAT, cs, epr_launch_splat(p, nb, tau, NULL, NULL, NULL, p->res, 3, d, cs));       // a0 + a1-N + a2 fused
-        p->launches += 1;                                  // k_grad_blockmax, launched ahead of the splat
       }
       if (p->diag && it < p->diag_cap)
         KL(p, K_DIAG, cs, epr_launch_diagnostics(p, nb, tau, p->res, p->diag + ((size_t)b_first * p->diag_cap + it) * 2, p->diag_cap * 2, cs));
@@ -456,6 +489,7 @@ static epr_status retrieve_device(epr_plan_t p, int batch, const float* d, float
 // Per-iteration diagnostics of the following retrievals: residual RMS and largest shift component (device array).
 extern "C" epr_status epr_set_diagnostics(epr_plan_t p, float* diag, int capacity_iters) {
   if (!p) return EPR_EINVAL;
+  DevGuard dg(p);
   if (diag && capacity_iters < 1) FAIL(p, EPR_EINVAL, "epr_set_diagnostics: capacity_iters must be >= 1");
   if (diag) {
     cudaError_t e = cudaSuccess;
@@ -474,6 +508,7 @@ extern "C" epr_status epr_retrieve_oversampled(epr_plan_t p, int factor, int bat
                                                int iterations, float step, void* stream) {
   epr_status st = check_call(p, batch);
   if (st != EPR_OK) return st;
+  DevGuard dg(p);
   if (!d || !out) FAIL(p, EPR_EINVAL, "epr_retrieve_oversampled: NULL pointer");
   if (iterations < 0 || !(step > 0.f)) FAIL(p, EPR_EINVAL, "epr_retrieve_oversampled: iterations must be >= 0 and step > 0");
   if (factor < 1 || factor > 8 || p->nx % (4 * factor) != 0 || p->ny % factor != 0)
@@ -500,6 +535,7 @@ extern "C" epr_status epr_retrieve(epr_plan_t p, int batch, const float* d, floa
                                    void* stream) {
   epr_status st = check_call(p, batch);
   if (st != EPR_OK) return st;
+  DevGuard dg(p);
   if (!d || !out) FAIL(p, EPR_EINVAL, "epr_retrieve: NULL pointer");
   if (iterations < 0 || !(step > 0.f)) FAIL(p, EPR_EINVAL, "epr_retrieve: iterations must be >= 0 and step > 0");
   cudaStream_t cs = (cudaStream_t)stream;
@@ -507,7 +543,12 @@ extern "C" epr_status epr_retrieve(epr_plan_t p, int batch, const float* d, floa
   // captured once into a CUDA graph and replayed while the call's arguments stay the same.  Never under profiling
   // (events are recorded around every launch) and never on the legacy default stream (capture is illegal there).
   const size_t work = (size_t)batch * p->n_bins * p->nx * p->ny;
-  const bool use_graph = !p->prof_on && !p->diag && cs != 0 && (p->graph_mode == 2 || (p->graph_mode == 1 && work <= ((size_t)1 << 20)));
+  bool use_graph = !p->prof_on && !p->diag && cs != 0 && cs != cudaStreamLegacy && cs != cudaStreamPerThread &&
+                   (p->graph_mode == 2 || (p->graph_mode == 1 && work <= ((size_t)1 << 20)));
+  if (use_graph) {                                     // a stream the caller is capturing already: just enqueue into it
+    cudaStreamCaptureStatus cst = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(cs, &cst) != cudaSuccess || cst != cudaStreamCaptureStatusNone) { cudaGetLastError(); use_graph = false; }
+  }
   if (!use_graph) return retrieve_device(p, batch, d, out, iterations, step, 0, cs);
   if (p->graph_exec && p->graph_d == d && p->graph_out == out && p->graph_batch == batch && p->graph_iters == iterations &&
       p->graph_step == step) {
@@ -521,16 +562,25 @@ extern "C" epr_status epr_retrieve(epr_plan_t p, int batch, const float* d, floa
     p->graph_warm = 1;
     return retrieve_device(p, batch, d, out, iterations, step, 0, cs);
   }
+  // Capture is an optimisation: whatever goes wrong with it (a stream that cannot be captured, a launcher doing
+  // first-use setup inside the capture, instantiation failure) ends in the eager path, never in an error.
   const long long l0 = p->launches;
-  CU(p, cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal));
+  if (cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+    cudaGetLastError();
+    return retrieve_device(p, batch, d, out, iterations, step, 0, cs);
+  }
   st = retrieve_device(p, batch, d, out, iterations, step, 0, cs);
   cudaGraph_t graph = NULL;
   cudaError_t ce = cudaStreamEndCapture(cs, &graph);
-  if (st != EPR_OK) { if (graph) cudaGraphDestroy(graph); return st; }
-  if (ce != cudaSuccess || !graph) FAIL(p, EPR_ECUDA, "graph capture: %s", cudaGetErrorString(ce));
-  ce = cudaGraphInstantiate(&p->graph_exec, graph, 0);
-  cudaGraphDestroy(graph);
-  if (ce != cudaSuccess) { p->graph_exec = NULL; FAIL(p, EPR_ECUDA, "graph instantiate: %s", cudaGetErrorString(ce)); }
+  if (st == EPR_OK && ce == cudaSuccess && graph) ce = cudaGraphInstantiate(&p->graph_exec, graph, 0);
+  if (graph) cudaGraphDestroy(graph);
+  if (st != EPR_OK || ce != cudaSuccess || !p->graph_exec) {
+    cudaGetLastError();
+    p->graph_exec = NULL;
+    p->launches = l0;
+    p->graph_mode = 0;                                 // do not try again on this plan
+    return retrieve_device(p, batch, d, out, iterations, step, 0, cs);
+  }
   p->graph_d = d; p->graph_out = out; p->graph_batch = batch; p->graph_iters = iterations; p->graph_step = step;
   p->graph_launches = p->launches - l0;
   CU(p, cudaGraphLaunch(p->graph_exec, cs));
@@ -540,6 +590,7 @@ extern "C" epr_status epr_retrieve(epr_plan_t p, int batch, const float* d, floa
 extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_host, float* out_host, int iterations,
                                         float step) {
   if (!p) return EPR_EINVAL;
+  DevGuard dg(p);
   if (batch < 1 || !d_host || !out_host) FAIL(p, EPR_EINVAL, "epr_retrieve_host: bad batch or NULL pointer");
   if (iterations < 0 || !(step > 0.f)) FAIL(p, EPR_EINVAL, "epr_retrieve_host: iterations must be >= 0 and step > 0");
   const size_t plane = (size_t)p->nx * p->ny;
@@ -577,6 +628,9 @@ extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_
     for (int i = 0; i < 6; ++i) CU(p, cudaEventCreateWithFlags(&p->hev[i], cudaEventDisableTiming));
   }
   cudaStream_t s_in = p->hstream[0], s_cmp = p->hstream[1], s_out = p->hstream[2];
+  // The call works on private streams and on the plan's shared workspaces: whatever earlier calls on this plan enqueued
+  // on the caller's streams (they only enqueue and return) must have finished first.
+  CU(p, cudaDeviceSynchronize());
   // Tapered schedule: the first copy in and the last copy out cannot overlap any compute, so the first and the last
   // chunks are small (wbch/4, wbch/2, wbch, …, wbch, wbch/2, wbch/4) when the batch holds at least three full chunks.
   const bool taper = wbch >= 4 && batch >= 3 * wbch;

@@ -797,10 +797,8 @@ int GFN(epr_fftg_has_)(int n) {
 }
 
 // persistent grid: as many CTAs as are resident at once (occupancy x SMs), at most one per row group
-template <typename K> static int row_grid(K kernel, int nt, size_t smem, int ngroups) {
-  int dev = 0, sms = 0, occ = 0;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+template <typename K> static int row_grid(K kernel, int sms, int nt, size_t smem, int ngroups) {
+  int occ = 0;
   cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, nt, smem);
   const int g = sms * (occ > 0 ? occ : 1);
@@ -815,10 +813,10 @@ cudaError_t GFN(epr_fftg_rows_r2c_)(const epr_plan_s* p, int planes, const float
   case n_: {                                                                                                    \
     using C = RowCfg<n_ / 2>;                                                                                   \
     constexpr size_t smem = (size_t)C::ROWS * C::PL * sizeof(float2);                                           \
-    static bool attr = false;                                                                                   \
-    if (!attr) {                                                                                                \
+    static EprPerDevice attr = {};                                                                              \
+    if (!attr.at(p)) {                                                                                          \
       cudaFuncSetAttribute(k_rows_r2c_direct<n_ / 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);   \
-      attr = true;                                                                                              \
+      attr.at(p) = 1;                                                                                           \
     }                                                                                                           \
     dim3 grid((p->ny + C::ROWS - 1) / C::ROWS, planes);                                                         \
     k_rows_r2c_direct<n_ / 2><<<grid, C::NT, smem, st>>>(p->ny, in, in_offset, p->tw_row, p->tw_r2c, spec);      \
@@ -834,8 +832,9 @@ template <int M, int EPI>
 static void launch_c2r(const epr_plan_s* p, int nrows, const float2* spec, float step, int tau_is_zero, float* q_or_tau,
                        cudaStream_t st) {
   using C = RowCfg<M>;
-  static int full = 0;
-  if (!full) full = row_grid(k_rows_c2r<M, EPI>, C::NT, C::SMEM, 1 << 30);
+  static EprPerDevice fullv = {};                        // resident CTAs of this kernel on the plan's device
+  if (!fullv.at(p)) fullv.at(p) = row_grid(k_rows_c2r<M, EPI>, p->sms, C::NT, C::SMEM, 1 << 30);
+  const int full = (int)fullv.at(p);
   const int ngroups = (nrows + C::ROWS - 1) / C::ROWS;
   k_rows_c2r<M, EPI><<<ngroups < full ? ngroups : full, C::NT, C::SMEM, st>>>(
       p->lines, nrows, spec, p->tw_row, p->tw_r2c, step, tau_is_zero, p->opt.newton_iters, p->opt.i_min, q_or_tau);
@@ -866,25 +865,25 @@ static bool launch_cols_tma(const epr_plan_s* p, int oplanes, int mode, const fl
     const int M = p->nx / 2;
     if (!p->tma_ok || M % C::W != 0 || spec != p->spec || (out != p->spec && out != p->spec_sum)) return false;
     if (mode == 1 && p->n_bins > 1 && C::smem(true) > 227 * 1024) return false;     // two tiles of 4096 rows do not fit an SM
-    static bool attr = false;
-    if (!attr) {
+    static EprPerDevice attr = {};
+    if (!attr.at(p)) {
       cudaFuncSetAttribute(k_cols_tma<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem(false));
       if (C::smem(true) <= 227 * 1024)
         cudaFuncSetAttribute(k_cols_tma<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem(true));
-      attr = true;
+      attr.at(p) = 1;
     }
     const CUtensorMap& mo = (out == p->spec) ? p->map_spec : p->map_spec_sum;
     dim3 grid(M / C::W, oplanes);
     if constexpr (2 * C::NT == 1024) {
       // one line per tile and enough tiles to keep every SM's two groups busy: persistent two-group kernel
-      static int sms = 0, two = -1;
+      static int two = -1;                               // process-wide developer switch (environment), not device state
       if (two < 0) { const char* e = getenv("EPR_COLS2"); two = e ? atoi(e) : 1; }
-      if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+      const int sms = p->sms;
       const int ntiles = (M / C::W) * oplanes;
       if (two && !(mode == 1 && p->n_bins > 1) && ntiles >= 8 * sms) {
         constexpr size_t smem2 = 3 * C::TILE + 32;
-        static bool attr2 = false;
-        if (!attr2) { cudaFuncSetAttribute(k_cols_tma2<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2); attr2 = true; }
+        static EprPerDevice attr2 = {};
+        if (!attr2.at(p)) { cudaFuncSetAttribute(k_cols_tma2<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2); attr2.at(p) = 1; }
         k_cols_tma2<N><<<sms, 2 * C::NT, smem2, st>>>(p->map_spec, mo, p->lines, M, mode, scale, M / C::W, ntiles, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
         return true;
       }
@@ -901,13 +900,13 @@ static bool launch_cols_tma(const epr_plan_s* p, int oplanes, int mode, const fl
     const bool sum = mode == 1 && p->n_bins > 1;
     if (!p->tma_ok || M % C::W != 0 || spec != p->spec || (out != p->spec && out != p->spec_sum)) return false;
     if (P::smem(sum) > 227 * 1024) return false;
-    static bool attr = false;
-    if (!attr) {
+    static EprPerDevice attr = {};
+    if (!attr.at(p)) {
       if (P::smem(false) <= 227 * 1024)
         cudaFuncSetAttribute(k_cols_tmap<N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::smem(false));
       if (P::smem(true) <= 227 * 1024)
         cudaFuncSetAttribute(k_cols_tmap<N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::smem(true));
-      attr = true;
+      attr.at(p) = 1;
     }
     const CUtensorMap& mo = (out == p->spec) ? p->map_spec : p->map_spec_sum;
     dim3 grid(M / C::W, oplanes);
@@ -930,11 +929,11 @@ cudaError_t GFN(epr_fftg_cols_)(const epr_plan_s* p, int planes, int mode, const
   case n_: {                                                                                                    \
     using C = ColCfg<n_>;                                                                                       \
     if (launch_cols_tma<n_>(p, oplanes, mode, spec, out, scale, st)) break;                                     \
-    static bool attr = false;                                                                                   \
-    if (!attr) {                                                                                                \
+    static EprPerDevice attr = {};                                                                              \
+    if (!attr.at(p)) {                                                                                          \
       cudaFuncSetAttribute(k_cols<n_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);       \
       cudaFuncSetAttribute(k_cols<n_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);        \
-      attr = true;                                                                                              \
+      attr.at(p) = 1;                                                                                           \
     }                                                                                                           \
     dim3 grid((M + C::W - 1) / C::W, oplanes);                                                                  \
     if (mode == 1 && p->n_bins > 1)                                                                             \

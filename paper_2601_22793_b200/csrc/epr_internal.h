@@ -31,6 +31,8 @@ struct EprLines {
 };
 
 struct epr_plan_s {
+  int device;                  // CUDA device the plan was built on: every entry point runs there (DevGuard in epr_api.cu)
+  int sms;                     // its SM count
   int nx, ny, n_bins, max_batch;
   int work_batch;              // projections processed per pass of the loop (workspaces are sized for it)
   int solver;                  // EPR_LOCAL / EPR_NONLOCAL
@@ -55,13 +57,14 @@ struct epr_plan_s {
   CUtensorMap map_spec_sum;
   int tma_ok;                  // descriptors valid (ny ≥ 256, nx % 8 == 0)
   int tma_box_rows;            // rows per TMA box: the largest divisor of ny that is ≤ 256 (256 for powers of two, 240 for 2160)
+  unsigned* d_flags;           // device word of EPR_FLAG_* bits raised by kernels (epr_read_flags)
   float* gmax;                 // [work_batch][ny/16][nx/16] block maxima of |D⁰τ| (non-local: k_grad_blockmax)
   float* diag;                 // caller's diagnostics array [batch][diag_cap][2] (device) or NULL (epr_set_diagnostics)
   int diag_cap;
   double* diag_partial;        // [work_batch][64] partial sums of squares
   float* os_d;                 // [work_batch][ny][nx] up-sampled detector images (lazy, epr_retrieve_oversampled)
   float* os_out;               // [work_batch][ny][nx] fine-grid result before down-sampling (lazy)
-  float2* raymap;              // [work_batch][n_bins][ny][nx] stored u_s (lazy, epr_forward non-local)
+  float2* raymap;              // [max_batch][n_bins][ny][nx] stored u_s (lazy, epr_forward non-local)
   int raymap_batch;            // batch of the stored map (0 = none)
   // host staging for epr_retrieve_host
   float* stage_in[2];
@@ -82,6 +85,19 @@ struct epr_plan_s {
   int prof_on;                 // per-kernel event timing enabled
   void* prof;                  // EprProf*
   char err[256];
+};
+
+// A launcher that enqueues more than one kernel reports the extra ones here, next to the launch itself
+// (epr_launch_count / bench.py's gpu_launches; the C-ABI layer counts one per launcher call).
+static inline void epr_note_extra_launch(const epr_plan_s* p, int n = 1) { const_cast<epr_plan_s*>(p)->launches += n; }
+
+// Per-device one-time setup (cudaFuncSetAttribute, occupancy queries) of a launcher: function attributes belong to the
+// device, so every call site keeps one flag / value per device ordinal instead of one per process.  The calls guarded
+// this way are idempotent, so two threads racing on the first use of a device both do the same harmless work.
+#define EPR_MAX_DEVICES 64
+struct EprPerDevice {
+  long long v[EPR_MAX_DEVICES];
+  long long& at(const epr_plan_s* p) { return v[(unsigned)p->device % EPR_MAX_DEVICES]; }
 };
 
 // ---- launchers (epr_kernels.cu / epr_fftk.cu); all return cudaGetLastError() ----

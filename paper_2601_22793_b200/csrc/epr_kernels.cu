@@ -236,8 +236,7 @@ cudaError_t epr_launch_forward_local(const epr_plan_s* p, int batch, const float
   // one line fused with the residual (d_fuse), or line by line into pred (several lines: blockIdx.z = projection · n_bins + line)
   const int bands = (p->nx + LM_BW - 1) / LM_BW;
   const int nz = d_fuse ? batch : batch * p->n_bins;
-  static int sms = 0;
-  if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); }
+  const int sms = p->sms;
   // the tallest row block that still gives every SM about a dozen warps (all CTAs resident at once: no tail wave)
   const long long need = 12ll * sms;
 #define EPR_MARCH(MR, WPC, GX, GY, NT)                                                                               \
@@ -329,7 +328,8 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
                                                     const float* __restrict__ tau, const float* __restrict__ I_bins,
                                                     const float2* __restrict__ map_in, float2* __restrict__ map_out,
                                                     float* __restrict__ out, int out_mode, const float* __restrict__ d,
-                                                    const float* __restrict__ gmax, int use_list) {
+                                                    const float* __restrict__ gmax, int use_list,
+                                                    unsigned* __restrict__ flags) {
   extern __shared__ __align__(16) unsigned char st_raw[];
   unsigned* s_acc = reinterpret_cast<unsigned*>(st_raw);                              // [(TH + 2)][ST_AP]
   float* s_tau = reinterpret_cast<float*>(st_raw + ST_AP * (TH + 2) * sizeof(unsigned));   // [TH + 2 H + 2][TP]
@@ -566,8 +566,15 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       if (out_mode == 1) {
         o = make_float4((float)(int)v.x * sc, (float)(int)v.y * sc, (float)(int)v.z * sc, (float)(int)v.w * sc);
       } else {
-        o = make_float4(fmaf((float)((int)v.x - Fi), sc, corr), fmaf((float)((int)v.y - Fi), sc, corr),
-                        fmaf((float)((int)v.z - Fi), sc, corr), fmaf((float)((int)v.w - Fi), sc, corr));
+        // Sources from τ are positive, so an accumulator that reads negative has passed 32x the flat field (u32 fixed
+        // point, 1.0 = 2^26, wraps at 64x): reported through the plan's flag word (epr_read_flags), never silently.
+        if ((v.x | v.y | v.z | v.w) & 0x80000000u) atomicOr(flags, EPR_FLAG_SPLAT_OVERFLOW);
+        // An EMPTY detector pixel (no source reaches it: the shadow side of a caustic) is written as exactly −f_s, so that
+        // P_s = f_s + (P_s − f_s) is exactly 0 downstream and the split's decision "Σ_t P_t⁺ = 0 → w_s = f_s" (R8) is
+        // taken on the integers, where an empty pixel is exactly empty — (float)(−Fi) alone would leave ±3e-8 there.
+        const float nf = -L.f[s];
+        o = make_float4(v.x ? fmaf((float)((int)v.x - Fi), sc, corr) : nf, v.y ? fmaf((float)((int)v.y - Fi), sc, corr) : nf,
+                        v.z ? fmaf((float)((int)v.z - Fi), sc, corr) : nf, v.w ? fmaf((float)((int)v.w - Fi), sc, corr) : nf);
         if (out_mode == 2) {
           const float4 dd = dpre[k];
           const float off = 1.f + L.fsum_dev;
@@ -620,17 +627,17 @@ template <bool FROM_TAU, bool MAP_OUT, int NT, int TH>
 static cudaError_t launch_splat_v(const epr_plan_s* p, int batch, int H, size_t smem, const float* tau, const float* I_bins,
                                   const float2* map_in, float2* map_out, float* out, int out_mode, const float* d,
                                   cudaStream_t st) {
-  static size_t attr = 0;
-  if (smem > attr) {
+  static EprPerDevice attr = {};                         // largest dynamic shared memory set so far, per device
+  if ((long long)smem > attr.at(p)) {
     cudaFuncSetAttribute(k_splat_tile<FROM_TAU, MAP_OUT, NT, TH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr = smem;
+    attr.at(p) = (long long)smem;
   }
   dim3 grid((p->nx + ST_W - 1) / ST_W, (p->ny + TH - 1) / TH, batch);
   // several lines share one list of ring candidates (the coordinates are packed in 8 bits each: H ≤ 64)
   static const bool list_off = getenv("EPR_SPLAT_LIST") && atoi(getenv("EPR_SPLAT_LIST")) == 0;
   const int use_list = FROM_TAU && p->lines.n_bins > 1 && H <= 64 && !list_off;
   k_splat_tile<FROM_TAU, MAP_OUT, NT, TH><<<grid, NT, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, H, tau, I_bins,
-                                                                   map_in, map_out, out, out_mode, d, p->gmax, use_list);
+                                                                   map_in, map_out, out, out_mode, d, p->gmax, use_list, p->d_flags);
   return cudaGetLastError();
 }
 
@@ -645,6 +652,7 @@ static cudaError_t launch_splat_t(const epr_plan_s* p, int batch, const float* t
   if (FROM_TAU) {                                      // block maxima of |D⁰τ| (also used by the gather of this τ)
     const cudaError_t e = epr_launch_grad_blockmax(p, batch, tau, st);
     if (e != cudaSuccess) return e;
+    epr_note_extra_launch(p);
   }
   const size_t half = 113 * 1024;                      // half of the 227 KB an SM offers: two CTAs per SM
   // 128 x 64 tiles with 512 threads when two CTAs fit an SM; large S (C5: S = 24): 128 x 32 tiles still bring two;
@@ -861,6 +869,10 @@ __global__ void __launch_bounds__(GT_NT, 2) k_gather_tile(EprLines L, int nx, in
       const float* row = tb + (unsigned)gy * nx;
       dtx[k] = __ldg(row + xp) - __ldg(row + xm);
       dty[k] = __ldg(tb + (unsigned)yp * nx + gx) - __ldg(tb + (unsigned)ym * nx + gx);
+      // Pixels outside the image (ragged last tile) only keep the lanes busy: their shifts must be ZERO, not those of
+      // column 0 / row ny − 1, whose gradients the tile's block maxima (and so the staged halo Hg) do not bound — the
+      // corner loads below are unpredicated and would leave the staged tile.
+      if (!xin || y0 + yy + 4 * k >= ny) dtx[k] = dty[k] = 0.f;
     }
   }
   unsigned nfill = 0u;                                 // bit i: parity of the fills of buffer i (lines served by global loads skip theirs)
@@ -927,11 +939,11 @@ cudaError_t epr_launch_gather(const epr_plan_s* p, int batch, const float* tau, 
     // Several lines only: with one line there is nothing to stage ahead and nothing to share, and the direct kernel
     // below measures faster (14.1 vs 15.5 us per 2048² plane).
     constexpr size_t smem = 2 * (size_t)GT_ER * GT_EP * sizeof(float);
-    static bool attr = false;
-    if (!attr) {
+    static EprPerDevice attr = {};
+    if (!attr.at(p)) {
       cudaFuncSetAttribute(k_gather_tile<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
       cudaFuncSetAttribute(k_gather_tile<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-      attr = true;
+      attr.at(p) = 1;
     }
     dim3 grid((p->nx + GT_W - 1) / GT_W, (p->ny + GT_H - 1) / GT_H, batch);
     if (p->nx >= 2 * GT_EP && p->ny >= 2 * GT_ER)
@@ -1072,9 +1084,11 @@ cudaError_t epr_launch_diagnostics(const epr_plan_s* p, int batch, const float* 
   if (p->solver == EPR_LOCAL) {                       // the non-local splat has already refreshed p->gmax for this τ
     const cudaError_t e = epr_launch_grad_blockmax(p, batch, tau, st);
     if (e != cudaSuccess) return e;
+    epr_note_extra_launch(p);
   }
   float cmax = 0.f;
   for (int s = 0; s < p->n_bins; ++s) cmax = fmaxf(cmax, 0.5f * p->lines.a[s] * p->lines.gamma[s]);
+  epr_note_extra_launch(p);                            // two kernels below
   k_diag_partial<<<dim3(DG_BLK, batch), 256, 0, st>>>(p->n_bins, plane, es, p->diag_partial);
   k_diag_final<<<batch, 256, 0, st>>>(plane, (p->nx / 16) * (p->ny / 16), cmax, p->diag_partial, p->gmax, diag, stride);
   return cudaGetLastError();

@@ -55,3 +55,19 @@ def test_product_does_not_import_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 text = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in text.replace("no oracle", ""), f"{f} mentions the oracle"
+
+
+def test_host_binding_rejects_non_float32_buffers():
+    """epr_retrieve_host takes float32 host buffers only: a float64 or 2-byte tensor of the right shape would make the
+    library read / write the wrong number of bytes.  The check sits in the binding, ahead of the library call."""
+    import numpy as np
+    import torch
+    from paper_2601_22793_b200 import binding
+
+    class FakePlan:
+        ny, nx, _h = 4, 8, None
+
+    for bad in (torch.zeros((1, 4, 8), dtype=torch.float64), torch.zeros((1, 4, 8), dtype=torch.float16),
+                torch.zeros((1, 4, 8), dtype=torch.bfloat16), np.zeros((1, 4, 8), dtype=np.float64)):
+        with pytest.raises(TypeError):
+            binding.epr_retrieve_host(FakePlan(), bad, bad, 1, 1.0)
