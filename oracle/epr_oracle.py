@@ -71,22 +71,22 @@ def derive_lines(pixel_m, L_m, energy_keV, weight, delta_over_beta, mu_rel=None)
 
 
 # --------------------------------------------------------------------------------------
-# periodic finite differences (R1-R3, R7)
+# periodic finite differences (R1-R3, R7); they act on the LAST TWO axes ([…][y][x]), so a stack of planes works too
 # --------------------------------------------------------------------------------------
 def _xp(g):  # g[y][x+1]
-    return np.roll(g, -1, axis=1)
+    return np.roll(g, -1, axis=-1)
 
 
 def _xm(g):  # g[y][x-1]
-    return np.roll(g, 1, axis=1)
+    return np.roll(g, 1, axis=-1)
 
 
 def _yp(g):  # g[y+1][x]
-    return np.roll(g, -1, axis=0)
+    return np.roll(g, -1, axis=-2)
 
 
 def _ym(g):  # g[y-1][x]
-    return np.roll(g, 1, axis=0)
+    return np.roll(g, 1, axis=-2)
 
 
 def d0x(g):
@@ -383,3 +383,191 @@ def retrieve_oversampled(d, lines_fine: Lines, m, solver="local", iterations=10,
     down-sample τ.  m = 1 is `retrieve`."""
     tau = retrieve(upsample(d, m), lines_fine, solver, iterations, step, order, wkb1, symbol, S, i_min)
     return downsample(tau, m)
+
+
+# --------------------------------------------------------------------------------------
+# x-dependent effective spectrum (PAPER.md:57, 216-221 Eq. (6) + remark, 227-229 Eq. (7), 431-441 §9.2;
+# SURVEY.md §8(f) rank 2; reading R17)
+# --------------------------------------------------------------------------------------
+# The paper parameterises I_s(r) = f_s(x) exp(−γ_s(x) τ(r)) and φ_s = (db_s(x)/2) ln I_s with 1-D profiles in the
+# horizontal detector coordinate x ("slow spatial variations of the effective spectrum", §9.2), and promises the
+# "file format and the blockwise interpolation strategy" in a Supporting Information that PAPER.md does not contain
+# (PAPER.md:221).  Reading R17 (DESIGN.md):
+#   (a) the profiles are given on n_blocks equal blocks of columns; the value of column x is the LINEAR interpolation
+#       between the two nearest block centres, constant outside the outermost centres; one block = uniform spectrum
+#       (§9.2 "single block");
+#   (b) the variation is slow, so the per-line scalars are FROZEN at the pixel's own column: every stencil of the local
+#       closure sees the neighbouring τ through the scalars of the centre column (no derivative of f_s, γ_s, db_s is
+#       ever taken — the empty beam must stay d = 1), and a source pixel of the ray map carries the mass and the shift
+#       of its own column's scalars;
+#   (c) the FFT-diagonal preconditioner cannot have an x-dependent coefficient; it is applied once per block with that
+#       block's a_s and the results are blended with the interpolation weights of (a): "blockwise interpolation".
+@dataclass
+class Profiles:
+    n_bins: int
+    n_blocks: int
+    nx: int
+    alpha: np.ndarray     # [n_bins]            L/(k_s p²): the lines keep their energies, PAPER.md:142, 164
+    wblk: np.ndarray      # [n_blocks][nx]      interpolation weights of (a); Σ_b wblk[b][x] = 1
+    f_blk: np.ndarray     # [n_blocks][n_bins]  per-block scalars
+    gamma_blk: np.ndarray
+    a_blk: np.ndarray
+    abar_blk: np.ndarray  # [n_blocks]          Σ_s f_s a_s per block (initial guess, R9)
+    f: np.ndarray         # [n_bins][nx]        per-column scalars
+    gamma: np.ndarray
+    db: np.ndarray
+    a: np.ndarray
+
+    def column(self, x) -> Lines:
+        """The uniform-spectrum scalars of column x, as a `Lines`."""
+        return Lines(self.n_bins, None, None, self.alpha, self.db[:, x], self.a[:, x], self.f[:, x], self.gamma[:, x])
+
+
+def block_weights(nx, n_blocks):
+    """(a): block b covers columns [b nx/n_blocks, (b+1) nx/n_blocks) (nx divisible by n_blocks), centre
+    c_b = (b + ½) nx/n_blocks − ½ in pixel-centre coordinates; hat-function weights, clamped at both ends."""
+    assert nx % n_blocks == 0
+    wb = nx // n_blocks
+    c = (np.arange(n_blocks) + 0.5) * wb - 0.5
+    x = np.arange(nx, dtype=np.float64)
+    w = np.zeros((n_blocks, nx))
+    if n_blocks == 1:
+        w[0] = 1.0
+        return w
+    t = np.clip((x - c[0]) / wb, 0.0, n_blocks - 1.0)       # position in units of blocks
+    b0 = np.minimum(np.floor(t).astype(int), n_blocks - 2)
+    fr = t - b0
+    w[b0, np.arange(nx)] = 1.0 - fr
+    w[b0 + 1, np.arange(nx)] += fr
+    return w
+
+
+def derive_profiles(pixel_m, L_m, energy_keV, nx, weight_blk, db_blk, mu_rel_blk=None) -> Profiles:
+    """Per-block scalars like `derive_lines` (weight_blk, db_blk, mu_rel_blk: [n_blocks][n_bins]) and their per-column
+    interpolation.  γ keeps ONE normalisation for the whole detector, so that τ is one thickness field: with
+    g_s^{(b)} = 1/(E_s db_s^{(b)}) (R11) or mu_rel, γ_s^{(b)} = g_s^{(b)}/G, G = mean_b Σ_s f_s^{(b)} g_s^{(b)};
+    uniform profiles reduce to R11."""
+    E = np.atleast_1d(np.asarray(energy_keV, dtype=np.float64))
+    wt = np.atleast_2d(np.asarray(weight_blk, dtype=np.float64))
+    db = np.atleast_2d(np.asarray(db_blk, dtype=np.float64))
+    nblk, n = wt.shape
+    assert db.shape == (nblk, n) and E.size == n
+    k = 2.0 * np.pi * E / HC_KEV_M
+    alpha = L_m / (k * pixel_m * pixel_m)
+    f_blk = wt / wt.sum(axis=1, keepdims=True)
+    g = (1.0 / (E[None, :] * db)) if mu_rel_blk is None else np.atleast_2d(np.asarray(mu_rel_blk, dtype=np.float64))
+    G = np.mean(np.sum(f_blk * g, axis=1))
+    gamma_blk = g / G
+    a_blk = alpha[None, :] * db / 2.0
+    w = block_weights(nx, nblk)
+    col = lambda v: np.einsum("bx,bs->sx", w, v)            # noqa: E731  Σ_b wblk[b][x] v[b][s]
+    dbx = col(db)
+    return Profiles(n, nblk, nx, alpha, w, f_blk, gamma_blk, a_blk, np.sum(f_blk * a_blk, axis=1),
+                    col(f_blk), col(gamma_blk), dbx, alpha[:, None] * dbx / 2.0)
+
+
+def line_intensities_x(tau, prof: Profiles):
+    """I_s = f_s(x) exp(−γ_s(x) τ)   Eq. (7) PAPER.md:227 with the x-dependent profiles."""
+    tau = np.asarray(tau, dtype=np.float64)
+    return [prof.f[s][None, :] * np.exp(-prof.gamma[s][None, :] * tau) for s in range(prof.n_bins)]
+
+
+def closure_x(tau, prof: Profiles, s, order=2, wkb1=True):
+    """(b): P_s(y, x) = closure(f_s(x) e^{−γ_s(x) τ}; a_s(x), α_s) evaluated AT column x — the Eq. (1) closure of the
+    uniform case with the scalars of the centre column.  The stencil has radius 2, so for every column a strip of the
+    five columns x−2 … x+2 (periodic, R7) is enough; the strips are stacked as [x][y][k] and the centre k = 2 is kept."""
+    tau = np.asarray(tau, dtype=np.float64)
+    strips = np.stack([np.roll(tau, -k, axis=1) for k in (-2, -1, 0, 1, 2)], axis=-1)      # [y][x][k] = τ[y][x+k]
+    strips = np.transpose(strips, (1, 0, 2))                                                # [x][y][k]
+    I = prof.f[s][:, None, None] * np.exp(-prof.gamma[s][:, None, None] * strips)
+    P = closure(I, prof.a[s][:, None, None], prof.alpha[s], order=order, wkb1=wkb1)
+    return P[:, :, 2].T
+
+
+def ray_map_x(tau, prof: Profiles, s, S):
+    """(b): u_s = a_s(x) D⁰ ln I_s with the scalars of the source's own column frozen, i.e. D⁰ ln I_s = −γ_s(x) D⁰τ
+    (Eq. (2) PAPER.md:164-167 with Eq. (6), (7)); each component clamped to ±S (R6)."""
+    tau = np.asarray(tau, dtype=np.float64)
+    c = (prof.a[s] * prof.gamma[s])[None, :]
+    return np.clip(-c * d0x(tau), -S, S), np.clip(-c * d0y(tau), -S, S)
+
+
+def forward_x(tau, prof: Profiles, solver="local", order=2, wkb1=True, S=16.0):
+    """Eq. (5) PAPER.md:209-212 with the x-dependent spectrum: returns (P_sum, [P_s], [(ux_s, uy_s)] or None)."""
+    Is = line_intensities_x(tau, prof)
+    P_bins, maps = [], []
+    for s in range(prof.n_bins):
+        if solver == "local":
+            P_bins.append(closure_x(tau, prof, s, order=order, wkb1=wkb1))
+        else:
+            ux, uy = ray_map_x(tau, prof, s, S)
+            maps.append((ux, uy))
+            P_bins.append(splat(Is[s], ux, uy))
+    return np.sum(P_bins, axis=0), P_bins, (maps if solver != "local" else None)
+
+
+def split_weights_x(P_bins, prof: Profiles):
+    """R8 with the fallback f_s(x) of the detector pixel's column."""
+    Pp = [np.maximum(P, 0.0) for P in P_bins]
+    den = np.sum(Pp, axis=0)
+    ok = den > 0.0
+    safe = np.where(ok, den, 1.0)
+    return [np.where(ok, Pp[s] / safe, prof.f[s][None, :]) for s in range(prof.n_bins)]
+
+
+def precondition_x(r, a_blk, wblk, symbol=0):
+    """(c) blockwise interpolation of the FFT-diagonal inverse: q = Σ_b wblk[b][x] ·
+    IFFT2(FFT2(r)/(1 + a^{(b)} λ)); a_blk: [n_blocks] coefficients of ONE line (or the ā of the initial guess)."""
+    r = np.asarray(r, dtype=np.float64)
+    q = np.zeros_like(r)
+    for b in range(len(a_blk)):
+        q += wblk[b][None, :] * precondition(r, a_blk[b], symbol)
+    return q
+
+
+def project_x(T, prof: Profiles, tol=1e-14, max_iter=200):
+    """Solve Σ_s f_s(x) exp(−γ_s(x) τ) = T per pixel (R10 with the column's scalars); Newton as in `project`."""
+    T = np.asarray(T, dtype=np.float64)
+    f = prof.f[:, None, :]
+    g = prof.gamma[:, None, :]
+    if prof.n_bins == 1:
+        return -np.log(T / f[0]) / g[0]
+    gbar = np.sum(f * g, axis=0) / np.sum(f, axis=0)
+    tau = -np.log(T / np.sum(f, axis=0)) / gbar
+    for _ in range(max_iter):
+        Es = f * np.exp(-g * tau[None])
+        step = (np.sum(Es, axis=0) - T) / (-np.sum(g * Es, axis=0))
+        tau = tau - step
+        if np.max(np.abs(step)) < tol:
+            break
+    return tau
+
+
+def paganin_init_x(d, prof: Profiles, symbol=0, i_min=1e-6):
+    """R9 with (c): the linear Paganin solve with the weighted-mean coefficient ā^{(b)} of every block, blended."""
+    T0 = np.maximum(precondition_x(d, prof.abar_blk, prof.wblk, symbol), i_min)
+    return project_x(T0, prof)
+
+
+def retrieve_x(d, prof: Profiles, solver="local", iterations=10, step=1.0, order=2, wkb1=True, symbol=0, S=16.0,
+               i_min=1e-6, tau0=None, history=None):
+    """The correction loop of PAPER.md:231-233 with the x-dependent effective spectrum of Eq. (6)/(7) (reading R17):
+    the same steps as `retrieve`, every per-line scalar taken at the pixel's column, the filter blockwise."""
+    d = np.asarray(d, dtype=np.float64)
+    tau = paganin_init_x(d, prof, symbol, i_min) if tau0 is None else np.asarray(tau0, np.float64).copy()
+    n = prof.n_bins
+    for _ in range(iterations):
+        Is = line_intensities_x(tau, prof)
+        P, P_bins, maps = forward_x(tau, prof, solver, order, wkb1, S)
+        e = d - P
+        if history is not None:
+            history.append(float(np.sqrt(np.mean(e * e))))
+        w = split_weights_x(P_bins, prof)
+        for s in range(n):
+            r = w[s] * e
+            if solver != "local":
+                r = gather(r, maps[s][0], maps[s][1])
+            Is[s] = Is[s] + step * precondition_x(r, prof.a_blk[:, s], prof.wblk, symbol)
+        T = np.maximum(np.sum(Is, axis=0), i_min)
+        tau = project_x(T, prof)
+    return tau

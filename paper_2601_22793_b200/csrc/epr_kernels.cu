@@ -568,7 +568,9 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       } else {
         // Sources from τ are positive, so an accumulator that reads negative has passed 32x the flat field (u32 fixed
         // point, 1.0 = 2^26, wraps at 64x): reported through the plan's flag word (epr_read_flags), never silently.
-        if ((v.x | v.y | v.z | v.w) & 0x80000000u) atomicOr(flags, EPR_FLAG_SPLAT_OVERFLOW);
+        // (The exact-remainder corner may be a few units NEGATIVE when a weight vanishes, so a pixel fed by such corners
+        // alone legitimately reads −1 … −8 units: those are not overflows, hence the offset.)
+        if (((v.x + 1024u) | (v.y + 1024u) | (v.z + 1024u) | (v.w + 1024u)) & 0x80000000u) atomicOr(flags, EPR_FLAG_SPLAT_OVERFLOW);
         // An EMPTY detector pixel (no source reaches it: the shadow side of a caustic) is written as exactly −f_s, so that
         // P_s = f_s + (P_s − f_s) is exactly 0 downstream and the split's decision "Σ_t P_t⁺ = 0 → w_s = f_s" (R8) is
         // taken on the integers, where an empty pixel is exactly empty — (float)(−Fi) alone would leave ±3e-8 there.
