@@ -33,7 +33,8 @@ typedef struct epr_plan_s* epr_plan_t;
 typedef enum {
   EPR_OK = 0,
   EPR_EINVAL = 1, /* bad argument (NULL pointer, non-positive size / energy / weight / step, batch > max_batch …) */
-  EPR_ESIZE = 2,  /* unsupported grid: nx, ny must be one of the sizes with a compiled FFT (16 … 4096) */
+  EPR_ESIZE = 2,  /* unsupported grid: nx or ny has a prime factor other than 2, 3, 5, or exceeds the largest supported
+                     length (8192; 4096 for the sizes with a compiled transform), see epr_plan */
   EPR_ECUDA = 3,  /* a CUDA runtime call failed; message in epr_last_error */
   EPR_ENOMEM = 4  /* device allocation failed */
 } epr_status;
@@ -64,6 +65,11 @@ void epr_default_options(epr_options* opt);
  *                 internally to Σ f_s = 1), δ_s/β_s.
  *   solver        EPR_LOCAL: Taylor/WKB closure Eq. (1); EPR_NONLOCAL: ray map Eq. (2) + splat Eq. (3).
  *   max_batch     largest `batch` later calls may pass (workspaces are sized for it).
+ * Grids: nx, ny >= 8 with prime factors in {2, 3, 5} (anything else: EPR_ESIZE; padding is the caller's job, R7).
+ *   The tuned kernels run on 16-pixel-aligned grids whose lengths have a compiled transform (16, 32, 48, 64, 80, 96, 128,
+ *   160, 256, 320, 384, 512, 640, 768, 1024, 1280, 1536, 1920, 2048, 2160, 2560, 3072, 3200, 4096); every other smooth
+ *   grid up to 8192 per axis (250, 1080, 3000, odd lengths such as 375, …) runs the general path: the same steps, one
+ *   pixel per thread, run-time-radix FFT — correct to the same tolerances, about 3x slower per pixel.
  * Derived: k_s = 2πE_s/(hc); α_s = L/(k_s p²); a_s = α_s δ_s/(2β_s); γ_s ∝ 1/(E_s δ_s/β_s), Σ f_s γ_s = 1. */
 epr_status epr_plan(epr_plan_t* plan, int nx, int ny, double pixel_m, double L_m, int n_bins,
                     const double* energy_keV, const double* weight, const double* delta_over_beta,
@@ -124,7 +130,7 @@ epr_status epr_retrieve_oversampled(epr_plan_t plan, int factor, int batch, cons
  *     diag[b][n][1] = the regime indicator η of PAPER.md:53 in the sup norm: the largest unclamped shift component
  *                     max_s max_r |a_s D⁰ ln I_s| in pixels of the plan's grid (η < 1: local regime).
  *   Costs two small kernels and one pass over the residual planes per iteration; keep it off in timed runs.  While it
- *   is on, retrievals are not captured into CUDA graphs. */
+ *   is on, retrievals are not captured into CUDA graphs.  Tuned path only (EPR_EINVAL on a general-path plan). */
 epr_status epr_set_diagnostics(epr_plan_t plan, float* diag, int capacity_iters);
 
 /* epr_retrieve_host — same, with HOST buffers (pinned for full speed): copies d host→device, runs the loop,
@@ -135,6 +141,26 @@ epr_status epr_set_diagnostics(epr_plan_t plan, float* diag, int capacity_iters)
  *   work enqueued earlier on the device (cudaDeviceSynchronize) and returns after its last copy has completed. */
 epr_status epr_retrieve_host(epr_plan_t plan, int batch, const float* d_host, float* out_host, int iterations,
                              float step);
+
+/* epr_plan_profiles — x-dependent effective spectrum           PAPER.md:216-221 (Eq. (6) + remark), 227-229 (Eq. (7)), 431-441 (§9.2)
+ *   "I_s(r) = f_s(x) exp(−γ_s(x) τ(r))", "db_s(x) = δ_s(x)/β_s(x) may be x-dependent if an x-dependent effective spectrum
+ *   is used": the spectrum varies slowly across the horizontal detector coordinate x.  The paper's "blockwise
+ *   interpolation strategy" is not printed; reading R17:
+ *   (a) the profiles are given on n_blocks equal blocks of columns (n_blocks divides nx, <= 64); the value of column x is the
+ *       linear interpolation between the two nearest block centres, constant outside the outermost centres;
+ *   (b) per-line scalars are frozen at the pixel's own column: the closure stencil sees neighbouring τ through the centre
+ *       column's scalars, a ray-map source carries the mass and shift of its own column (no derivative of a profile);
+ *   (c) the FFT-diagonal filter is applied once per block with that block's a_s and blended with the weights of (a).
+ *   weight, delta_over_beta, mu_rel: HOST arrays [n_blocks][n_bins] (mu_rel may be NULL: γ_s ∝ 1/(E_s δ_s/β_s), R11); weights
+ *   are normalised per block; γ keeps ONE normalisation for the whole detector (block mean of Σ_s f_s γ_s = 1).  The energies,
+ *   L, pixel and options are the plan's.  n_blocks = 1 is the uniform spectrum ("single block", §9.2).  After this call the
+ *   plan runs the general path (see epr_plan); epr_set_diagnostics and opt.nonlocal_wkb1 are not available on it.
+ *   Synchronises the device. */
+epr_status epr_plan_profiles(epr_plan_t plan, int n_blocks, const double* weight, const double* delta_over_beta,
+                             const double* mu_rel);
+
+/* Per-column scalars the plan uses (HOST arrays [n_bins][nx], any may be NULL): f_s(x), γ_s(x), a_s(x). */
+epr_status epr_plan_columns(epr_plan_t plan, double* f, double* gamma, double* a);
 
 /* epr_read_flags — conditions kernels detected since the flags were last cleared (synchronises the device).
  *   EPR_FLAG_SPLAT_OVERFLOW: the non-local forward accumulates each line's detector plane in 32-bit fixed point (unit

@@ -13,7 +13,8 @@ _LIB = None
 
 EXPORTS = ["epr_default_options", "epr_plan", "epr_forward", "epr_adjoint", "epr_transport", "epr_precondition",
            "epr_retrieve", "epr_retrieve_oversampled", "epr_set_diagnostics", "epr_retrieve_host", "epr_plan_lines", "epr_launch_count", "epr_destroy",
-           "epr_last_error", "epr_version", "epr_profile_enable", "epr_profile_read", "epr_read_flags"]
+           "epr_last_error", "epr_version", "epr_profile_enable", "epr_profile_read", "epr_read_flags",
+           "epr_plan_profiles", "epr_plan_columns"]
 EPR_FLAG_SPLAT_OVERFLOW = 1
 
 
@@ -64,6 +65,10 @@ def load_library():
     lib.epr_profile_enable.restype = ci
     lib.epr_profile_read.argtypes = [vp, ci, C.POINTER(C.c_char_p), C.POINTER(cd), C.POINTER(C.c_longlong), ci]
     lib.epr_profile_read.restype = ci
+    lib.epr_plan_profiles.argtypes = [vp, ci, C.POINTER(cd), C.POINTER(cd), C.POINTER(cd)]
+    lib.epr_plan_profiles.restype = ci
+    lib.epr_plan_columns.argtypes = [vp, C.POINTER(cd), C.POINTER(cd), C.POINTER(cd)]
+    lib.epr_plan_columns.restype = ci
     lib.epr_read_flags.argtypes = [vp, C.POINTER(C.c_uint), ci]
     lib.epr_read_flags.restype = ci
     lib.epr_last_error.argtypes = [vp]
@@ -126,6 +131,13 @@ class Plan:
         k = load_library().epr_profile_read(self._h, n, names, ms, cnt, 1 if reset else 0)
         return {names[i].decode(): (float(ms[i]), int(cnt[i])) for i in range(k)}
 
+    def columns(self):
+        """Per-column scalars the plan uses: dict of float64 arrays [n_bins][nx] f, gamma, a (epr_plan_columns)."""
+        arrs = [np.zeros((self.n_bins, self.nx)) for _ in range(3)]
+        ptrs = [a.ctypes.data_as(C.POINTER(C.c_double)) for a in arrs]
+        self._check(load_library().epr_plan_columns(self._h, *ptrs))
+        return dict(zip(("f", "gamma", "a"), arrs))
+
     def read_flags(self, clear=True):
         """EPR_FLAG_* bits raised by kernels since the last clear (epr_read_flags; synchronises)."""
         v = C.c_uint(0)
@@ -175,6 +187,22 @@ def epr_plan(nx, ny, pixel_m, L_m, energy_keV, weight, delta_over_beta, solver="
             lib.epr_destroy(h)
         raise EprError(st, msg)
     return Plan(h, int(nx), int(ny), int(E.size), sv, int(max_batch))
+
+
+def epr_plan_profiles(plan, weight_blk, delta_over_beta_blk, mu_rel_blk=None):
+    """epr_plan_profiles of include/epr.h: [n_blocks][n_bins] arrays (x-dependent effective spectrum, reading R17)."""
+    w = np.ascontiguousarray(np.atleast_2d(weight_blk), dtype=np.float64)
+    db = np.ascontiguousarray(np.atleast_2d(delta_over_beta_blk), dtype=np.float64)
+    if w.shape != db.shape or w.shape[1] != plan.n_bins:
+        raise ValueError("weight_blk, delta_over_beta_blk: expected [n_blocks][n_bins]")
+    dp = C.POINTER(C.c_double)
+    mu = None
+    if mu_rel_blk is not None:
+        mu = np.ascontiguousarray(np.atleast_2d(mu_rel_blk), dtype=np.float64)
+        if mu.shape != w.shape:
+            raise ValueError("mu_rel_blk: expected [n_blocks][n_bins]")
+    plan._check(load_library().epr_plan_profiles(plan._h, int(w.shape[0]), w.ctypes.data_as(dp), db.ctypes.data_as(dp),
+                                                 mu.ctypes.data_as(dp) if mu is not None else None))
 
 
 def epr_forward(plan, tau, P_sum, P_bins=None):

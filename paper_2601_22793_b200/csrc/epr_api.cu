@@ -24,9 +24,9 @@ static const double HC_KEV_M = 1.2398419843e-9;
     if (e_ != cudaSuccess) FAIL(p, EPR_ECUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
   } while (0)
 // Kernel families, for launch counting and the optional per-kernel CUDA-event timing (epr_profile_*).
-enum { K_FWD_LOCAL = 0, K_SPLAT, K_RESIDUAL, K_GATHER, K_ROWS_R2C, K_COLS, K_ROWS_C2R, K_PRED_OUT, K_OUTPUT, K_RESAMPLE, K_DIAG, K_WKB1, K_COUNT };
+enum { K_FWD_LOCAL = 0, K_SPLAT, K_RESIDUAL, K_GATHER, K_ROWS_R2C, K_COLS, K_ROWS_C2R, K_PRED_OUT, K_OUTPUT, K_RESAMPLE, K_DIAG, K_WKB1, K_UPDATE, K_COUNT };
 static const char* const K_NAMES[K_COUNT] = {"k_forward_local", "k_splat", "k_residual", "k_gather", "k_rows_r2c",
-                                              "k_cols", "k_rows_c2r", "k_pred_out", "k_output", "k_resample", "k_diagnostics", "k_wkb1_sub"};
+                                              "k_cols", "k_rows_c2r", "k_pred_out", "k_output", "k_resample", "k_diagnostics", "k_wkb1_sub", "k_update"};
 struct EprProf {
   struct Rec { int tag; cudaEvent_t a, b; };
   std::vector<Rec> recs;
@@ -50,6 +50,10 @@ struct EprProf {
       ((EprProf*)(p)->prof)->recs.push_back(rec_);                             \
     }                                                                          \
   } while (0)
+
+static cudaError_t gen_r2c(epr_plan_t p, int planes, const float* in, float off, cudaStream_t cs);
+static cudaError_t gen_cols(epr_plan_t p, int planes, int mode, int blk, float2* out, cudaStream_t cs);
+static cudaError_t gen_c2r(epr_plan_t p, int planes, const float2* spec, float* q, cudaStream_t cs);
 
 // Every entry point runs on the plan's device (function attributes, workspaces and streams belong to it) and restores
 // the caller's current device on return.
@@ -139,6 +143,85 @@ static bool make_spec_map(CUtensorMap* map, void* base, int nx, size_t rows, int
             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// Per-column tables of the general path from per-block scalars (reading R17(a)): block b
+// covers columns [b nx/n_blocks, (b+1) nx/n_blocks), centre c_b = (b + ½) nx/n_blocks − ½; the value of column x is the
+// linear interpolation between the two nearest centres, constant outside the outermost ones.  f_blk, gamma_blk, db_blk:
+// [n_blocks][n_bins] (f normalised per block, γ with its one global normalisation).  Also the per-block filter
+// coefficients a_s^{(b)} = α_s db_s^{(b)}/2, ā^{(b)} = Σ_s f_s^{(b)} a_s^{(b)} (R17(c)) and the block-filter workspace.
+static epr_status set_columns(epr_plan_s* p, int n_blocks, const double* f_blk, const double* gamma_blk, const double* db_blk) {
+  const int nx = p->nx, nb = p->n_bins;
+  const int wb = nx / n_blocks;
+  std::vector<double> w((size_t)n_blocks * nx, 0.0);
+  for (int x = 0; x < nx; ++x) {
+    if (n_blocks == 1) { w[x] = 1.0; continue; }
+    double t = ((double)x - (0.5 * wb - 0.5)) / (double)wb;            // position in units of blocks from the first centre
+    t = t < 0.0 ? 0.0 : (t > n_blocks - 1.0 ? n_blocks - 1.0 : t);
+    int b0 = (int)floor(t);
+    if (b0 > n_blocks - 2) b0 = n_blocks - 2;
+    const double fr = t - b0;
+    w[(size_t)b0 * nx + x] = 1.0 - fr;
+    w[(size_t)(b0 + 1) * nx + x] += fr;
+  }
+  free(p->h_col);
+  p->h_col = (double*)malloc(sizeof(double) * 3 * nb * nx);
+  if (!p->h_col) FAIL(p, EPR_ENOMEM, "column tables");
+  double *hf = p->h_col, *hg = hf + (size_t)nb * nx, *ha = hg + (size_t)nb * nx;
+  for (int s = 0; s < nb; ++s)
+    for (int x = 0; x < nx; ++x) {
+      double f = 0, g = 0, db = 0;
+      for (int b = 0; b < n_blocks; ++b) {
+        const double wv = w[(size_t)b * nx + x];
+        f += wv * f_blk[b * nb + s]; g += wv * gamma_blk[b * nb + s]; db += wv * db_blk[b * nb + s];
+      }
+      hf[(size_t)s * nx + x] = f; hg[(size_t)s * nx + x] = g; ha[(size_t)s * nx + x] = p->h_alpha[s] * db / 2.0;
+    }
+  // one device allocation: f, γ, a, fixCorr (float [nb][nx]), fixFi (u32 [nb][nx]), fsum_dev (float [nx]), wblk (float [n_blocks][nx])
+  const size_t n1 = (size_t)nb * nx;
+  std::vector<float> host(5 * n1 + nx + (size_t)n_blocks * nx);
+  float *df = host.data(), *dg = df + n1, *da = dg + n1, *dc = da + n1;
+  unsigned* dF = reinterpret_cast<unsigned*>(dc + n1);
+  float *ds = reinterpret_cast<float*>(dF + n1), *dw = ds + nx;
+  for (int x = 0; x < nx; ++x) ds[x] = 0.f;
+  for (size_t i = 0; i < n1; ++i) {
+    df[i] = (float)hf[i]; dg[i] = (float)hg[i]; da[i] = (float)ha[i];
+    const double fix = (double)df[i] * EPR_FIX_ONE;                    // the device uses the fp32-rounded f_s(x) consistently
+    dF[i] = (unsigned)llrint(fix);
+    dc[i] = (float)((double)dF[i] / EPR_FIX_ONE - (double)df[i]);
+  }
+  for (int x = 0; x < nx; ++x) {
+    double fs = 0;
+    for (int s = 0; s < nb; ++s) fs += (double)df[(size_t)s * nx + x];
+    ds[x] = (float)(fs - 1.0);
+  }
+  for (size_t i = 0; i < (size_t)n_blocks * nx; ++i) dw[i] = (float)w[i];
+  cudaFree(p->cols_store);
+  p->cols_store = NULL;
+  CU(p, cudaMalloc(&p->cols_store, host.size() * sizeof(float)));
+  CU(p, cudaMemcpy(p->cols_store, host.data(), host.size() * sizeof(float), cudaMemcpyHostToDevice));
+  float* base = (float*)p->cols_store;
+  p->cols.f = base; p->cols.gamma = base + n1; p->cols.a = base + 2 * n1; p->cols.fixCorr = base + 3 * n1;
+  p->cols.fixFi = reinterpret_cast<const unsigned*>(base + 4 * n1);
+  p->cols.fsum_dev = base + 5 * n1; p->cols.wblk = base + 5 * n1 + nx;
+  for (int b = 0; b < n_blocks; ++b) {
+    double abar = 0;
+    for (int s = 0; s < nb; ++s) {
+      const double a = p->h_alpha[s] * db_blk[b * nb + s] / 2.0;
+      p->a_blk[b][s] = (float)a;
+      abar += f_blk[b * nb + s] * a;
+    }
+    p->abar_blk[b] = (float)abar;
+  }
+  if (!p->qblk || n_blocks > p->n_blocks) {
+    cudaFree(p->qblk);
+    p->qblk = NULL;
+    cudaError_t e = cudaMalloc((void**)&p->qblk, (size_t)n_blocks * p->work_batch * nx * p->ny * sizeof(float));
+    if (e != cudaSuccess) FAIL(p, e == cudaErrorMemoryAllocation ? EPR_ENOMEM : EPR_ECUDA, "block-filter workspace: %s", cudaGetErrorString(e));
+  }
+  p->n_blocks = n_blocks;
+  p->general = 1;
+  return EPR_OK;
+}
+
 extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, double L_m, int n_bins,
                                const double* energy_keV, const double* weight, const double* delta_over_beta,
                                epr_solver solver, int max_batch, const epr_options* opt) {
@@ -147,7 +230,7 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
   if (!energy_keV || !weight || !delta_over_beta) return EPR_EINVAL;
   if (n_bins < 1 || n_bins > EPR_MAX_BINS || max_batch < 1 || !(pixel_m > 0) || !(L_m > 0)) return EPR_EINVAL;
   if (solver != EPR_LOCAL && solver != EPR_NONLOCAL) return EPR_EINVAL;
-  if (nx < 16 || ny < 16) return EPR_EINVAL;
+  if (nx < 8 || ny < 8) return EPR_EINVAL;
   double wsum = 0;
   for (int s = 0; s < n_bins; ++s) {
     if (!(energy_keV[s] > 0) || !(weight[s] > 0) || !(delta_over_beta[s] > 0)) return EPR_EINVAL;
@@ -160,7 +243,12 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
       o.max_shift_px > 30.f || !(o.i_min > 0) || o.newton_iters < 0 || o.newton_iters > 32 || o.output < 0 ||
       o.output > 2 || o.out_bin < 0 || o.out_bin >= n_bins)
     return EPR_EINVAL;
-  if (!epr_fft_size_supported(nx) || !epr_fft_size_supported(ny)) return EPR_ESIZE;
+  // Grids: the tuned kernels take the sizes with a compiled FFT on 16-pixel-aligned grids; every other {2,3,5}-smooth
+  // grid (8 … 8192 per axis) runs the general path (epr_general.cu), with the run-time-radix FFT where needed.
+  const bool tuned_fft = nx % 2 == 0 && epr_fft_size_supported(nx) && epr_fft_size_supported(ny);
+  const bool aligned = nx % 16 == 0 && ny % 16 == 0;
+  if (!tuned_fft && !(epr_fftgen_supported(nx) && epr_fftgen_supported(ny))) return EPR_ESIZE;
+  if ((!tuned_fft || !aligned) && o.nonlocal_wkb1) return EPR_EINVAL;      // variant R4 exists on the tuned path only
 
   epr_plan_s* p = (epr_plan_s*)aligned_alloc(64, (sizeof(epr_plan_s) + 63) / 64 * 64);   // CUtensorMap members: 64-byte aligned
   if (!p) return EPR_ENOMEM;
@@ -216,10 +304,18 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
   L.fsum_dev = (float)(fs - 1.0);
 
   const int M = nx / 2;
-  CU(p, upload(&p->tw_row, pass_twiddles(M, false)));
-  CU(p, upload(&p->tw_r2c, twiddles(nx, M)));
-  CU(p, upload(&p->tw_col, pass_twiddles(ny, false)));
-  CU(p, upload(&p->tw_col_inv, pass_twiddles(ny, true)));
+  p->fft_generic = tuned_fft ? 0 : 1;
+  p->general = (!tuned_fft || !aligned) ? 1 : 0;
+  p->n_blocks = 1;
+  if (tuned_fft) {
+    CU(p, upload(&p->tw_row, pass_twiddles(M, false)));
+    CU(p, upload(&p->tw_r2c, twiddles(nx, M)));
+    CU(p, upload(&p->tw_col, pass_twiddles(ny, false)));
+    CU(p, upload(&p->tw_col_inv, pass_twiddles(ny, true)));
+  } else {
+    CU(p, upload(&p->tw_gen_x, twiddles(nx, nx)));
+    CU(p, upload(&p->tw_gen_y, twiddles(ny, ny)));
+  }
   CU(p, upload(&p->lam_x, lambda_table(nx, M + 1, o.symbol)));
   CU(p, upload(&p->lam_y, lambda_table(ny, ny, o.symbol)));
 
@@ -241,20 +337,27 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->pred, wb * n_bins * plane * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc((void**)&p->res, wb * n_bins * plane * sizeof(float));
   if (e == cudaSuccess && solver == EPR_NONLOCAL) e = cudaMalloc((void**)&p->res2, wb * n_bins * plane * sizeof(float));
-  if (e == cudaSuccess && solver == EPR_NONLOCAL) e = cudaMalloc((void**)&p->gmax, wb * (size_t)(nx / 16) * (ny / 16) * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc((void**)&p->spec, wb * n_bins * plane * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc((void**)&p->spec_sum, wb * plane * sizeof(float));
+  if (e == cudaSuccess && solver == EPR_NONLOCAL) e = cudaMalloc((void**)&p->gmax, wb * (size_t)((nx + 15) / 16) * ((ny + 15) / 16) * sizeof(float));
+  const size_t spf = p->fft_generic ? epr_fftgen_spec_floats(p) : plane;     // floats per spectrum plane
+  if (e == cudaSuccess) e = cudaMalloc((void**)&p->spec, wb * n_bins * spf * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&p->spec_sum, wb * spf * sizeof(float));
   if (e != cudaSuccess) FAIL(p, e == cudaErrorMemoryAllocation ? EPR_ENOMEM : EPR_ECUDA, "workspace: %s", cudaGetErrorString(e));
   // TMA descriptors for the column kernel (power-of-two ny ≥ 256, whole 4-column tiles): the spectra seen as
   // [rows = planes·ny][nx floats], box = 8 floats (4 complex columns) x 256 rows, no swizzle.
   p->tma_ok = 0;
-  if (ny >= 256 && nx % 8 == 0) {
+  if (tuned_fft && ny >= 256 && nx % 8 == 0) {
     int br = 256;
     while (ny % br != 0) --br;                       // 256 for powers of two, 240 for 2160, 160 for 320
     p->tma_box_rows = br;
     if (br >= 64 && make_spec_map(&p->map_spec, p->spec, nx, (size_t)wb * n_bins * ny, br) &&
         make_spec_map(&p->map_spec_sum, p->spec_sum, nx, (size_t)wb * ny, br))
       p->tma_ok = 1;
+  }
+  if (p->general) {                                    // constant columns: the uniform spectrum on the general path
+    double fb[EPR_MAX_BINS], gb[EPR_MAX_BINS], dbb[EPR_MAX_BINS];
+    for (int s = 0; s < n_bins; ++s) { fb[s] = p->h_f[s]; gb[s] = p->h_gamma[s]; dbb[s] = p->h_db[s]; }
+    epr_status st = set_columns(p, 1, fb, gb, dbb);
+    if (st != EPR_OK) return st;
   }
   return EPR_OK;
 }
@@ -308,6 +411,58 @@ extern "C" epr_status epr_plan_lines(epr_plan_t p, double* f, double* gamma, dou
   return EPR_OK;
 }
 
+// x-dependent effective spectrum (reading R17): replaces the plan's uniform
+// spectrum by n_blocks block profiles; the plan then runs the general path.
+extern "C" epr_status epr_plan_profiles(epr_plan_t p, int n_blocks, const double* weight, const double* delta_over_beta,
+                                        const double* mu_rel) {
+  if (!p) return EPR_EINVAL;
+  DevGuard dg(p);
+  if (!weight || !delta_over_beta) FAIL(p, EPR_EINVAL, "epr_plan_profiles: NULL pointer");
+  if (n_blocks < 1 || n_blocks > EPR_MAX_BLOCKS || p->nx % n_blocks != 0)
+    FAIL(p, EPR_EINVAL, "epr_plan_profiles: n_blocks = %d must be in 1..%d and divide nx = %d", n_blocks, EPR_MAX_BLOCKS, p->nx);
+  if (p->opt.nonlocal_wkb1) FAIL(p, EPR_EINVAL, "epr_plan_profiles: opt.nonlocal_wkb1 is not available with an x-dependent spectrum");
+  if (p->diag) FAIL(p, EPR_EINVAL, "epr_plan_profiles: switch diagnostics off first (not available on the general path)");
+  const int nb = p->n_bins;
+  std::vector<double> f((size_t)n_blocks * nb), g((size_t)n_blocks * nb), db((size_t)n_blocks * nb);
+  double G = 0;
+  for (int b = 0; b < n_blocks; ++b) {
+    double wsum = 0;
+    for (int s = 0; s < nb; ++s) {
+      const double w = weight[b * nb + s], d = delta_over_beta[b * nb + s];
+      if (!(w > 0) || !(d > 0) || (mu_rel && !(mu_rel[b * nb + s] > 0)))
+        FAIL(p, EPR_EINVAL, "epr_plan_profiles: weights, delta/beta and mu_rel must be positive (block %d, line %d)", b, s);
+      wsum += w;
+    }
+    for (int s = 0; s < nb; ++s) {
+      f[b * nb + s] = weight[b * nb + s] / wsum;
+      db[b * nb + s] = delta_over_beta[b * nb + s];
+      // γ_s ∝ 1/(E_s db_s) (R11) or the caller's relative attenuation; E_s from α_s = L/(k_s p²): 1/E_s ∝ α_s
+      g[b * nb + s] = mu_rel ? mu_rel[b * nb + s] : p->h_alpha[s] / db[b * nb + s];
+      G += f[b * nb + s] * g[b * nb + s];
+    }
+  }
+  G /= n_blocks;                                       // ONE normalisation for the whole detector: τ is one thickness field
+  for (auto& v : g) v /= G;
+  CU(p, cudaDeviceSynchronize());                      // the tables may be in use by enqueued work
+  epr_status st = set_columns(p, n_blocks, f.data(), g.data(), db.data());
+  if (st != EPR_OK) return st;
+  if (p->graph_exec) { cudaGraphExecDestroy(p->graph_exec); p->graph_exec = NULL; }
+  return EPR_OK;
+}
+
+extern "C" epr_status epr_plan_columns(epr_plan_t p, double* f, double* gamma, double* a) {
+  if (!p) return EPR_EINVAL;
+  const size_t n = (size_t)p->n_bins * p->nx;
+  for (int s = 0; s < p->n_bins; ++s)
+    for (int x = 0; x < p->nx; ++x) {
+      const size_t i = (size_t)s * p->nx + x;
+      if (f) f[i] = p->h_col ? p->h_col[i] : p->h_f[s];
+      if (gamma) gamma[i] = p->h_col ? p->h_col[n + i] : p->h_gamma[s];
+      if (a) a[i] = p->h_col ? p->h_col[2 * n + i] : p->h_a[s];
+    }
+  return EPR_OK;
+}
+
 extern "C" epr_status epr_read_flags(epr_plan_t p, unsigned* flags, int clear) {
   if (!p) return EPR_EINVAL;
   if (!flags) FAIL(p, EPR_EINVAL, "epr_read_flags: NULL pointer");
@@ -324,7 +479,8 @@ extern "C" epr_status epr_destroy(epr_plan_t p) {
   cudaDeviceSynchronize();
   cudaFree(p->tw_row); cudaFree(p->tw_r2c); cudaFree(p->tw_col); cudaFree(p->tw_col_inv); cudaFree(p->lam_x); cudaFree(p->lam_y);
   cudaFree(p->tau); cudaFree(p->pred); cudaFree(p->res); cudaFree(p->res2); cudaFree(p->spec); cudaFree(p->spec_sum);
-  cudaFree(p->d_flags);
+  cudaFree(p->d_flags); cudaFree(p->cols_store); cudaFree(p->qblk); cudaFree(p->tw_gen_x); cudaFree(p->tw_gen_y);
+  free(p->h_col);
   cudaFree(p->raymap); cudaFree(p->gmax); cudaFree(p->os_d); cudaFree(p->os_out); cudaFree(p->diag_partial);
   if (p->graph_exec) cudaGraphExecDestroy(p->graph_exec);
   if (p->prof) { epr_profile_read(p, 0, NULL, NULL, NULL, 1); delete (EprProf*)p->prof; }
@@ -363,6 +519,16 @@ extern "C" epr_status epr_forward(epr_plan_t p, int batch, const float* tau, flo
     const float* t = tau + (size_t)b0 * plane;
     float* Ps = P_sum + (size_t)b0 * plane;
     float* Pb = P_bins ? P_bins + (size_t)b0 * p->n_bins * plane : NULL;
+    if (p->general) {
+      if (p->solver == EPR_LOCAL) {
+        KL(p, K_FWD_LOCAL, cs, epr_gen_forward_local(p, nb, t, p->pred, cs));
+      } else {
+        KL(p, K_SPLAT, cs, epr_gen_splat(p, nb, t, NULL, NULL, p->raymap + (size_t)b0 * p->n_bins * plane, (unsigned*)p->pred, cs));
+        KL(p, K_SPLAT, cs, epr_gen_fix2float(p, nb, (unsigned*)p->pred, 0, cs));
+      }
+      KL(p, K_PRED_OUT, cs, epr_gen_pred_out(p, nb, p->pred, Ps, Pb, cs));
+      continue;
+    }
     if (p->solver == EPR_LOCAL) {
       KL(p, K_FWD_LOCAL, cs, epr_launch_forward_local(p, nb, t, NULL, p->pred, cs));
     } else {
@@ -388,7 +554,8 @@ extern "C" epr_status epr_adjoint(epr_plan_t p, int batch, const float* e_bins, 
   }
   if (e_bins == r_bins) FAIL(p, EPR_EINVAL, "epr_adjoint: the gather cannot run in place");
   if (!p->raymap || p->raymap_batch < batch) FAIL(p, EPR_EINVAL, "epr_adjoint: no ray map stored for batch %d (call epr_forward first)", batch);
-  KL(p, K_GATHER, cs, epr_launch_gather(p, batch, NULL, p->raymap, e_bins, r_bins, 0, cs));
+  if (p->general) KL(p, K_GATHER, cs, epr_gen_gather(p, batch, NULL, p->raymap, e_bins, r_bins, cs));
+  else KL(p, K_GATHER, cs, epr_launch_gather(p, batch, NULL, p->raymap, e_bins, r_bins, 0, cs));
   return EPR_OK;
 }
 
@@ -402,6 +569,11 @@ extern "C" epr_status epr_transport(epr_plan_t p, int batch, const float* I_bins
   cudaStream_t cs = (cudaStream_t)stream;
   const size_t plane = (size_t)p->nx * p->ny;
   if (I_bins == P_bins) FAIL(p, EPR_EINVAL, "epr_transport: the splat cannot run in place");
+  if (p->general) {                                    // the caller's output planes serve as the fixed-point accumulators
+    KL(p, K_SPLAT, cs, epr_gen_splat(p, batch, NULL, I_bins, p->raymap, NULL, (unsigned*)P_bins, cs));
+    KL(p, K_SPLAT, cs, epr_gen_fix2float(p, batch, (unsigned*)P_bins, 1, cs));
+    return EPR_OK;
+  }
   KL(p, K_SPLAT, cs, epr_launch_splat(p, batch, NULL, I_bins, p->raymap, NULL, P_bins, 1, NULL, cs));
   return EPR_OK;
 }
@@ -417,9 +589,76 @@ extern "C" epr_status epr_precondition(epr_plan_t p, int batch, const float* r_b
     const int nb = (batch - b0 < p->work_batch) ? batch - b0 : p->work_batch;
     const int planes = nb * p->n_bins;
     const size_t off = (size_t)b0 * p->n_bins * plane;
+    if (p->general) {
+      // per-line filter of every block, blended with the interpolation weights (R17(c)); the input may alias the output,
+      // so several blocks accumulate in a workspace first
+      for (int b = 0; b < p->n_blocks; ++b) {
+        KL(p, K_ROWS_R2C, cs, gen_r2c(p, planes, r_bins + off, 0.f, cs));
+        KL(p, K_COLS, cs, gen_cols(p, planes, 0, b, p->spec, cs));
+        if (p->n_blocks == 1) { KL(p, K_ROWS_C2R, cs, gen_c2r(p, planes, p->spec, q_bins + off, cs)); break; }
+        KL(p, K_ROWS_C2R, cs, gen_c2r(p, planes, p->spec, p->pred, cs));
+        KL(p, K_UPDATE, cs, epr_gen_blend(p, planes, b, p->pred, p->res, b > 0, cs));
+      }
+      if (p->n_blocks > 1) CU(p, cudaMemcpyAsync(q_bins + off, p->res, (size_t)planes * plane * sizeof(float), cudaMemcpyDeviceToDevice, cs));
+      continue;
+    }
     KL(p, K_ROWS_R2C, cs, epr_launch_rows_r2c(p, planes, r_bins + off, 0.f, p->spec, cs));
     KL(p, K_COLS, cs, epr_launch_cols(p, planes, 0, p->spec, p->spec, cs));
     KL(p, K_ROWS_C2R, cs, epr_launch_rows_c2r(p, planes, p->spec, 0, 1.f, 0, q_bins + off, cs));
+  }
+  return EPR_OK;
+}
+
+// ----------------------------------------------------------------------------------------------- general path
+// FFT back end of the general path: the tuned row / column kernels when both sizes have a compiled transform, the
+// run-time-radix ones otherwise.  The filter of block b uses that block's coefficients (R17(c)).
+static cudaError_t gen_r2c(epr_plan_t p, int planes, const float* in, float off, cudaStream_t cs) {
+  return p->fft_generic ? epr_fftgen_rows_r2c(p, planes, in, off, p->spec, cs) : epr_launch_rows_r2c(p, planes, in, off, p->spec, cs);
+}
+static cudaError_t gen_cols(epr_plan_t p, int planes, int mode, int blk, float2* out, cudaStream_t cs) {
+  EprLines lb = p->lines;
+  for (int s = 0; s < p->n_bins; ++s) lb.a[s] = p->a_blk[blk][s];
+  lb.abar = p->abar_blk[blk];
+  return p->fft_generic ? epr_fftgen_cols(p, planes, mode, p->spec, out, cs, &lb) : epr_launch_cols(p, planes, mode, p->spec, out, cs, &lb);
+}
+static cudaError_t gen_c2r(epr_plan_t p, int planes, const float2* spec, float* q, cudaStream_t cs) {
+  return p->fft_generic ? epr_fftgen_rows_c2r(p, planes, spec, q, cs) : epr_launch_rows_c2r(p, planes, spec, 0, 1.f, 0, q, cs);
+}
+
+// One pass of the loop over nb <= work_batch projections on the general path (same steps as retrieve_chunk).
+static epr_status retrieve_chunk_general(epr_plan_t p, int nb, const float* d, float* tau, int iterations, float step,
+                                         cudaStream_t cs) {
+  const size_t plane = (size_t)p->nx * p->ny;
+  const int planes = nb * p->n_bins;
+  const size_t bstride = (size_t)p->work_batch * plane;            // qblk[b] holds work_batch planes
+  if (p->opt.init == 0) {
+    // initial guess (R9, R17(c)): T⁰ − 1 = Σ_b wblk[b][x] IFFT(FFT(d − 1)/(1 + ā^{(b)} λ)), floored, projected
+    KL(p, K_ROWS_R2C, cs, gen_r2c(p, nb, d, -1.f, cs));
+    for (int b = 0; b < p->n_blocks; ++b) {
+      KL(p, K_COLS, cs, gen_cols(p, nb, 2, b, p->spec_sum, cs));
+      KL(p, K_ROWS_C2R, cs, gen_c2r(p, nb, p->spec_sum, p->qblk + b * bstride, cs));
+    }
+    KL(p, K_UPDATE, cs, epr_gen_update(p, nb, p->qblk, bstride, 1.f, 1, tau, cs));
+  }
+  for (int it = 0; it < iterations; ++it) {
+    const float* r;
+    if (p->solver == EPR_LOCAL) {
+      KL(p, K_FWD_LOCAL, cs, epr_gen_forward_local(p, nb, tau, p->pred, cs));                   // a0 + a1-L
+      KL(p, K_RESIDUAL, cs, epr_gen_residual(p, nb, d, p->pred, p->res, cs));                   // a2 (a3 = identity)
+      r = p->res;
+    } else {
+      KL(p, K_SPLAT, cs, epr_gen_splat(p, nb, tau, NULL, NULL, NULL, (unsigned*)p->res, cs));   // a0 + a1-N
+      KL(p, K_SPLAT, cs, epr_gen_fix2float(p, nb, (unsigned*)p->res, 0, cs));
+      KL(p, K_RESIDUAL, cs, epr_gen_residual(p, nb, d, p->res, p->res, cs));                    // a2, in place
+      KL(p, K_GATHER, cs, epr_gen_gather(p, nb, tau, NULL, p->res, p->res2, cs));               // a3
+      r = p->res2;
+    }
+    KL(p, K_ROWS_R2C, cs, gen_r2c(p, planes, r, 0.f, cs));                                      // a4
+    for (int b = 0; b < p->n_blocks; ++b) {
+      KL(p, K_COLS, cs, gen_cols(p, planes, 1, b, p->spec_sum, cs));                            // Σ_s in Fourier space (R10), block b
+      KL(p, K_ROWS_C2R, cs, gen_c2r(p, nb, p->spec_sum, p->qblk + b * bstride, cs));
+    }
+    KL(p, K_UPDATE, cs, epr_gen_update(p, nb, p->qblk, bstride, step, 0, tau, cs));             // a5 + a6
   }
   return EPR_OK;
 }
@@ -429,6 +668,7 @@ extern "C" epr_status epr_precondition(epr_plan_t p, int batch, const float* r_b
 // b_first: index of the chunk's first projection within the caller's batch (row of the diagnostics array).
 static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* tau, int iterations, float step,
                                  int b_first, cudaStream_t cs) {
+  if (p->general) return retrieve_chunk_general(p, nb, d, tau, iterations, step, cs);
   const size_t plane = (size_t)p->nx * p->ny;
   const int planes = nb * p->n_bins;
   if (p->opt.init == 0) {
@@ -481,7 +721,7 @@ static epr_status retrieve_device(epr_plan_t p, int batch, const float* d, float
     if (p->opt.init == 1 && tau != o) CU(p, cudaMemcpyAsync(tau, o, (size_t)nb * plane * sizeof(float), cudaMemcpyDeviceToDevice, cs));
     epr_status st = retrieve_chunk(p, nb, d + (size_t)b0 * plane, tau, iterations, step, b_first + b0, cs);
     if (st != EPR_OK) return st;
-    if (p->opt.output != 0) KL(p, K_OUTPUT, cs, epr_launch_output(p, nb, tau, o, cs));
+    if (p->opt.output != 0) KL(p, K_OUTPUT, cs, p->general ? epr_gen_output(p, nb, tau, o, cs) : epr_launch_output(p, nb, tau, o, cs));
   }
   return EPR_OK;
 }
@@ -490,6 +730,7 @@ static epr_status retrieve_device(epr_plan_t p, int batch, const float* d, float
 extern "C" epr_status epr_set_diagnostics(epr_plan_t p, float* diag, int capacity_iters) {
   if (!p) return EPR_EINVAL;
   DevGuard dg(p);
+  if (diag && p->general) FAIL(p, EPR_EINVAL, "epr_set_diagnostics: not available on the general path (x-dependent spectrum or unaligned grid)");
   if (diag && capacity_iters < 1) FAIL(p, EPR_EINVAL, "epr_set_diagnostics: capacity_iters must be >= 1");
   if (diag) {
     cudaError_t e = cudaSuccess;

@@ -5,14 +5,14 @@
 #ifdef EPR_FFT_DEV          /* developer build: only group 0 (2048, 16, 32) is compiled */
 #define EPR_FFT_GROUPS(G) G(0)
 #else
-#define EPR_FFT_GROUPS(G) G(0) G(1) G(2) G(3) G(4) G(5) G(6)
+#define EPR_FFT_GROUPS(G) G(0) G(1) G(2) G(3) G(4) G(5) G(6) G(7) G(8) G(9) G(10)
 #endif
 
 #define G(g)                                                                                                          \
   int epr_fftg_has_##g(int n);                                                                                        \
   cudaError_t epr_fftg_rows_r2c_##g(const epr_plan_s*, int, const float*, float, float2*, cudaStream_t);               \
   cudaError_t epr_fftg_rows_c2r_##g(const epr_plan_s*, int, const float2*, int, float, int, float*, cudaStream_t);     \
-  cudaError_t epr_fftg_cols_##g(const epr_plan_s*, int, int, const float2*, float2*, cudaStream_t);
+  cudaError_t epr_fftg_cols_##g(const epr_plan_s*, int, int, const float2*, float2*, cudaStream_t, const EprLines*);
 EPR_FFT_GROUPS(G)
 #undef G
 
@@ -39,8 +39,9 @@ cudaError_t epr_launch_rows_c2r(const epr_plan_s* p, int planes, const float2* s
   return cudaErrorInvalidValue;
 }
 
-cudaError_t epr_launch_cols(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st) {
-#define G(g) if (epr_fftg_has_##g(p->ny)) return epr_fftg_cols_##g(p, planes, mode, spec, out, st);
+cudaError_t epr_launch_cols(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st,
+                            const EprLines* lines_override) {
+#define G(g) if (epr_fftg_has_##g(p->ny)) return epr_fftg_cols_##g(p, planes, mode, spec, out, st, lines_override);
   EPR_FFT_GROUPS(G)
 #undef G
   return cudaErrorInvalidValue;

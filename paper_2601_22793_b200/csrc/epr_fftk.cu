@@ -768,7 +768,7 @@ k_cols_tmap(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
 // The instantiations are split into EPR_FFT_NGROUPS translation units (this file compiled once per group with
 // -DEPR_FFT_GROUP=g, in parallel: see build.py); epr_fftd.cu routes a size to the group that holds it.
 #ifndef EPR_FFT_GROUP
-#error "compile with -DEPR_FFT_GROUP=<0..6> (paper_2601_22793_b200/build.py does)"
+#error "compile with -DEPR_FFT_GROUP=<0..10> (paper_2601_22793_b200/build.py does)"
 #endif
 #if EPR_FFT_GROUP == 0
 #define EPR_FFT_SIZES(X) X(2048) X(16) X(32)
@@ -782,8 +782,16 @@ k_cols_tmap(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ 
 #define EPR_FFT_SIZES(X) X(512) X(320) X(128)
 #elif EPR_FFT_GROUP == 5
 #define EPR_FFT_SIZES(X) X(256) X(160)
-#else
+#elif EPR_FFT_GROUP == 6
 #define EPR_FFT_SIZES(X) X(4096)
+#elif EPR_FFT_GROUP == 7
+#define EPR_FFT_SIZES(X) X(1536) X(384)
+#elif EPR_FFT_GROUP == 8
+#define EPR_FFT_SIZES(X) X(1920) X(640)
+#elif EPR_FFT_GROUP == 9
+#define EPR_FFT_SIZES(X) X(3072) X(768)
+#else
+#define EPR_FFT_SIZES(X) X(3200) X(1280)
 #endif
 #define EPR_CAT2(a, b) a##b
 #define EPR_CAT(a, b) EPR_CAT2(a, b)
@@ -858,8 +866,8 @@ cudaError_t GFN(epr_fftg_rows_c2r_)(const epr_plan_s* p, int planes, const float
 }
 
 template <int N>
-static bool launch_cols_tma(const epr_plan_s* p, int oplanes, int mode, const float2* spec, float2* out, float scale,
-                            cudaStream_t st) {
+static bool launch_cols_tma(const epr_plan_s* p, const EprLines& LL, int oplanes, int mode, const float2* spec, float2* out,
+                            float scale, cudaStream_t st) {
   if constexpr (N >= 256 && (N & (N - 1)) == 0) {
     using C = ColTmaCfg<N>;
     const int M = p->nx / 2;
@@ -884,14 +892,14 @@ static bool launch_cols_tma(const epr_plan_s* p, int oplanes, int mode, const fl
         constexpr size_t smem2 = 3 * C::TILE + 32;
         static EprPerDevice attr2 = {};
         if (!attr2.at(p)) { cudaFuncSetAttribute(k_cols_tma2<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2); attr2.at(p) = 1; }
-        k_cols_tma2<N><<<sms, 2 * C::NT, smem2, st>>>(p->map_spec, mo, p->lines, M, mode, scale, M / C::W, ntiles, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+        k_cols_tma2<N><<<sms, 2 * C::NT, smem2, st>>>(p->map_spec, mo, LL, M, mode, scale, M / C::W, ntiles, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
         return true;
       }
     }
     if (mode == 1 && p->n_bins > 1)
-      k_cols_tma<N, true><<<grid, C::NT, C::smem(true), st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+      k_cols_tma<N, true><<<grid, C::NT, C::smem(true), st>>>(p->map_spec, mo, LL, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
     else
-      k_cols_tma<N, false><<<grid, C::NT, C::smem(false), st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+      k_cols_tma<N, false><<<grid, C::NT, C::smem(false), st>>>(p->map_spec, mo, LL, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
     return true;
   } else if constexpr (N >= 256) {
     using C = ColCfg<N>;
@@ -911,16 +919,18 @@ static bool launch_cols_tma(const epr_plan_s* p, int oplanes, int mode, const fl
     const CUtensorMap& mo = (out == p->spec) ? p->map_spec : p->map_spec_sum;
     dim3 grid(M / C::W, oplanes);
     if (sum)
-      k_cols_tmap<N, true><<<grid, C::NT, P::smem(true), st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->tma_box_rows, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+      k_cols_tmap<N, true><<<grid, C::NT, P::smem(true), st>>>(p->map_spec, mo, LL, M, mode, scale, p->tma_box_rows, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
     else
-      k_cols_tmap<N, false><<<grid, C::NT, P::smem(false), st>>>(p->map_spec, mo, p->lines, M, mode, scale, p->tma_box_rows, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+      k_cols_tmap<N, false><<<grid, C::NT, P::smem(false), st>>>(p->map_spec, mo, LL, M, mode, scale, p->tma_box_rows, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
     return true;
   } else {
     return false;
   }
 }
 
-cudaError_t GFN(epr_fftg_cols_)(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st) {
+cudaError_t GFN(epr_fftg_cols_)(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st,
+                                const EprLines* lines_override) {
+  const EprLines& LL = lines_override ? *lines_override : p->lines;     // block filters pass their own a[] / abar
   const int M = p->nx / 2;
   const int oplanes = (mode == 1) ? planes / p->n_bins : planes;
   const float scale = (float)(1.0 / ((double)p->nx * (double)p->ny));
@@ -928,7 +938,7 @@ cudaError_t GFN(epr_fftg_cols_)(const epr_plan_s* p, int planes, int mode, const
 #define X(n_)                                                                                                   \
   case n_: {                                                                                                    \
     using C = ColCfg<n_>;                                                                                       \
-    if (launch_cols_tma<n_>(p, oplanes, mode, spec, out, scale, st)) break;                                     \
+    if (launch_cols_tma<n_>(p, LL, oplanes, mode, spec, out, scale, st)) break;                                     \
     static EprPerDevice attr = {};                                                                              \
     if (!attr.at(p)) {                                                                                          \
       cudaFuncSetAttribute(k_cols<n_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);       \
@@ -937,9 +947,9 @@ cudaError_t GFN(epr_fftg_cols_)(const epr_plan_s* p, int planes, int mode, const
     }                                                                                                           \
     dim3 grid((M + C::W - 1) / C::W, oplanes);                                                                  \
     if (mode == 1 && p->n_bins > 1)                                                                             \
-      k_cols<n_, true><<<grid, C::NT, C::SMEM, st>>>(p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv, spec, out); \
+      k_cols<n_, true><<<grid, C::NT, C::SMEM, st>>>(LL, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv, spec, out); \
     else                                                                                                        \
-      k_cols<n_, false><<<grid, C::NT, C::SMEM, st>>>(p->lines, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv, spec, out); \
+      k_cols<n_, false><<<grid, C::NT, C::SMEM, st>>>(LL, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv, spec, out); \
   } break;
     EPR_FFT_SIZES(X)
 #undef X

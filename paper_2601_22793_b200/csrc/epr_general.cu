@@ -1,0 +1,367 @@
+// epr_general.cu — the GENERAL path of the EPR iteration (sm_100a): the same steps a0 … a6 as epr_kernels.cu, with
+//   * every per-line scalar read per COLUMN from small device tables — the x-dependent effective spectrum
+//     f_s(x), γ_s(x), db_s(x) of PAPER.md:216-221 (Eq. (6) + remark), 227-229 (Eq. (7)), 431-441 (§9.2), reading R17:
+//     the scalars are frozen at the pixel's own column (no derivative of a profile is ever taken) and the
+//     FFT-diagonal filter is applied per block and blended (epr_api.cu);
+//   * no alignment requirement on the grid: any nx, ny >= 8 (one pixel per thread, scalar accesses), so that it also
+//     serves {2,3,5}-smooth grids the tuned kernels do not take (nx % 4 != 0, ny % 16 != 0, …).
+// The tuned kernels of epr_kernels.cu remain the path of the uniform spectrum on aligned grids; these kernels favour
+// plain structure over the last factor of two (they are bound by instruction issue at about 3x the tuned cost).
+// Arithmetic is the same deviation form: state τ, J = expm1(−γτ), data d − 1, predictions P_s − f_s(x),
+// splat in u32 fixed point with the exact-remainder corner.
+#include "epr_internal.h"
+#include "epr_math.cuh"
+
+#define GN_TX 32
+#define GN_TY 8
+
+// =====================================================================================================
+// a1-L  local O(L²) closure, Eq. (1) PAPER.md:146 (readings R1-R3), scalars of the CENTRE column (R17(b)):
+//   P_s/f_s − 1 = J − a ∇²₅J + (a²/2)[D²x(Î gx²) + D²y(Î gy²) + 2 D⁰xD⁰y(Î gx gy)] − (α²/4) Σ_i D⁻_i(Ī_i D⁺_i Q)
+//   A = exp(−γτ/2) = 1 + Ad, Î = A², J = Ad(2 + Ad), g = −γ D⁰τ, Q = ∇²₅A / A; neighbour values formed with the centre's γ.
+// One thread = one pixel, every line; τ tile + 2 in shared memory.
+// =====================================================================================================
+__global__ void __launch_bounds__(GN_TX * GN_TY) k_gen_local(EprLines L, EprColumns C, int nx, int ny, int order, int wkb1,
+                                                            const float* __restrict__ tau, float* __restrict__ pred) {
+  __shared__ float s_t[GN_TY + 4][GN_TX + 4];
+  const int tid = threadIdx.y * GN_TX + threadIdx.x, b = blockIdx.z;
+  const int x0 = blockIdx.x * GN_TX, y0 = blockIdx.y * GN_TY;
+  const size_t plane = (size_t)nx * ny;
+  const float* tb = tau + (size_t)b * plane;
+  for (int i = tid; i < (GN_TY + 4) * (GN_TX + 4); i += GN_TX * GN_TY) {
+    const int ly = i / (GN_TX + 4), lx = i - ly * (GN_TX + 4);
+    s_t[ly][lx] = __ldg(tb + (size_t)wrapm(y0 - 2 + ly, ny) * nx + wrapm(x0 - 2 + lx, nx));
+  }
+  __syncthreads();
+  const int x = x0 + threadIdx.x, y = y0 + threadIdx.y;
+  if (x >= nx || y >= ny) return;
+  // τ on the 5 x 5 neighbourhood (corners unused)
+  float t[5][5];
+#pragma unroll
+  for (int j = 0; j < 5; ++j)
+#pragma unroll
+    for (int i = 0; i < 5; ++i) t[j][i] = s_t[threadIdx.y + j][threadIdx.x + i];
+  const bool o2 = order == 2, wk = o2 && wkb1;
+  for (int s = 0; s < L.n_bins; ++s) {
+    const float gam = __ldg(&C.gamma[(size_t)s * nx + x]), a = __ldg(&C.a[(size_t)s * nx + x]), fs = __ldg(&C.f[(size_t)s * nx + x]);
+    const float cg = -0.5f * gam, c2 = 0.5f * a * a * cg * cg, q4 = L.q4[s];
+    // Ad on the 13-point diamond |dx| + |dy| <= 2 (index [dy + 2][dx + 2])
+    float A[5][5];
+#pragma unroll
+    for (int j = 0; j < 5; ++j)
+#pragma unroll
+      for (int i = 0; i < 5; ++i)
+        A[j][i] = (abs(i - 2) + abs(j - 2) <= 2) ? epr_expm1(cg * t[j][i]) : 0.f;
+    auto J = [&](int dy, int dx) { const float v = A[dy + 2][dx + 2]; return v * (2.f + v); };
+    auto Ih = [&](int dy, int dx) { const float v = 1.f + A[dy + 2][dx + 2]; return v * v; };
+    const float J0 = J(0, 0);
+    float v = J0 - a * (((J(0, 1) - J0) + (J(0, -1) - J0)) + ((J(1, 0) - J0) + (J(-1, 0) - J0)));
+    if (o2) {
+      auto tx = [&](int dy, int dx) { return t[dy + 2][dx + 3] - t[dy + 2][dx + 1]; };
+      auto ty = [&](int dy, int dx) { return t[dy + 3][dx + 2] - t[dy + 1][dx + 2]; };
+      auto Sxx = [&](int dx) { const float g = tx(0, dx); return Ih(0, dx) * g * g; };
+      auto Syy = [&](int dy) { const float g = ty(dy, 0); return Ih(dy, 0) * g * g; };
+      auto Sxy = [&](int dy, int dx) { return Ih(dy, dx) * tx(dy, dx) * ty(dy, dx); };
+      const float sx0 = Sxx(0), sy0 = Syy(0);
+      const float d2x = (Sxx(1) - sx0) - (sx0 - Sxx(-1)), d2y = (Syy(1) - sy0) - (sy0 - Syy(-1));
+      const float cross = 0.5f * ((Sxy(1, 1) - Sxy(1, -1)) - (Sxy(-1, 1) - Sxy(-1, -1)));
+      v = fmaf(c2, d2x + d2y + cross, v);
+      if (wk) {
+        auto Q = [&](int dy, int dx) {
+          const float ac = A[dy + 2][dx + 2];
+          return __fdividef(((A[dy + 2][dx + 3] - ac) + (A[dy + 2][dx + 1] - ac)) + ((A[dy + 3][dx + 2] - ac) + (A[dy + 1][dx + 2] - ac)), 1.f + ac);
+        };
+        const float Q0 = Q(0, 0), I0 = Ih(0, 0);
+        const float fxp = 0.5f * (Ih(0, 1) + I0) * (Q(0, 1) - Q0), fxm = 0.5f * (I0 + Ih(0, -1)) * (Q0 - Q(0, -1));
+        const float fyp = 0.5f * (Ih(1, 0) + I0) * (Q(1, 0) - Q0), fym = 0.5f * (I0 + Ih(-1, 0)) * (Q0 - Q(-1, 0));
+        v = fmaf(-q4, (fxp - fxm) + (fyp - fym), v);
+      }
+    }
+    pred[((size_t)b * L.n_bins + s) * plane + (size_t)y * nx + x] = fs * v;
+  }
+}
+
+cudaError_t epr_gen_forward_local(const epr_plan_s* p, int batch, const float* tau, float* pred, cudaStream_t st) {
+  dim3 grid((p->nx + GN_TX - 1) / GN_TX, (p->ny + GN_TY - 1) / GN_TY, batch), blk(GN_TX, GN_TY);
+  k_gen_local<<<grid, blk, 0, st>>>(p->lines, p->cols, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, pred);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// a1-N  ray map (Eq. (2), clamp R6) + mass-conserving bilinear splat, scalars of
+// the SOURCE's column (R17(b)).  One thread = one source pixel, every line; the 4-way scatter goes to a u32 fixed-point
+// plane in global memory (unit 2^-26, zero-initialised by the launcher) with native integer atomics: order-independent
+// (bit-reproducible) and exactly mass conserving — the 4th corner takes the integer remainder, as in k_splat_tile.
+// =====================================================================================================
+template <bool FROM_TAU>
+__global__ void __launch_bounds__(256) k_gen_splat(EprLines L, EprColumns C, int nx, int ny, float S,
+                                                   const float* __restrict__ tau, const float* __restrict__ I_bins,
+                                                   const float2* __restrict__ map_in, float2* __restrict__ map_out,
+                                                   unsigned* __restrict__ acc) {
+  const int x = blockIdx.x * 64 + (threadIdx.x & 63), y = blockIdx.y * 4 + (threadIdx.x >> 6), b = blockIdx.z;
+  if (x >= nx || y >= ny) return;
+  const size_t plane = (size_t)nx * ny, pix = (size_t)y * nx + x;
+  float tc = 0.f, dtx = 0.f, dty = 0.f;
+  if (FROM_TAU) {
+    const float* tb = tau + (size_t)b * plane;
+    const int xm = x == 0 ? nx - 1 : x - 1, xp = x + 1 == nx ? 0 : x + 1;
+    const int ym = y == 0 ? ny - 1 : y - 1, yp = y + 1 == ny ? 0 : y + 1;
+    tc = __ldg(tb + pix);
+    dtx = __ldg(tb + (size_t)y * nx + xp) - __ldg(tb + (size_t)y * nx + xm);
+    dty = __ldg(tb + (size_t)yp * nx + x) - __ldg(tb + (size_t)ym * nx + x);
+  }
+  for (int s = 0; s < L.n_bins; ++s) {
+    const size_t pl = ((size_t)b * L.n_bins + s) * plane;
+    float ux, uy;
+    int tot;
+    if (FROM_TAU) {
+      const float gam = __ldg(&C.gamma[(size_t)s * nx + x]), a = __ldg(&C.a[(size_t)s * nx + x]), fs = __ldg(&C.f[(size_t)s * nx + x]);
+      const float cs = -0.5f * a * gam;                 // u = a D⁰ ln I_s = −a γ D⁰τ
+      ux = fminf(fmaxf(cs * dtx, -S), S);
+      uy = fminf(fmaxf(cs * dty, -S), S);
+      if (map_out) map_out[pl + pix] = make_float2(ux, uy);
+      const float xe = -gam * tc;
+      const float J = fabsf(xe) < 0.35f ? epr_expm1_small(xe) : epr_exp_fast(xe) - 1.f;
+      tot = (int)__ldg(&C.fixFi[(size_t)s * nx + x]) + __float2int_rn(fs * 67108864.f * J);
+    } else {
+      const float2 m = __ldg(&map_in[pl + pix]);
+      ux = m.x; uy = m.y;
+      tot = __float2int_rn(__ldg(&I_bins[pl + pix]) * 67108864.f);
+    }
+    const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
+    const float dx = ux - (float)fx, dy = uy - (float)fy;
+    const float totf = (float)tot, te = totf * (1.f - dy), td = totf * dy, ex = 1.f - dx;
+    const int c00 = __float2int_rn(te * ex), c10 = __float2int_rn(te * dx), c01 = __float2int_rn(td * ex);
+    const int c11 = tot - c00 - c10 - c01;
+    const int ix0 = wrapm(x + fx, nx), iy0 = wrapm(y + fy, ny);
+    const int ix1 = ix0 + 1 == nx ? 0 : ix0 + 1, iy1 = iy0 + 1 == ny ? 0 : iy0 + 1;
+    unsigned* ap = acc + pl;
+    atomicAdd(ap + (size_t)iy0 * nx + ix0, (unsigned)c00);
+    atomicAdd(ap + (size_t)iy0 * nx + ix1, (unsigned)c10);
+    atomicAdd(ap + (size_t)iy1 * nx + ix0, (unsigned)c01);
+    atomicAdd(ap + (size_t)iy1 * nx + ix1, (unsigned)c11);
+  }
+}
+
+cudaError_t epr_gen_splat(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
+                          float2* map_out, unsigned* acc, cudaStream_t st) {
+  const size_t n = (size_t)batch * p->n_bins * p->nx * p->ny;
+  cudaError_t e = cudaMemsetAsync(acc, 0, n * sizeof(unsigned), st);
+  if (e != cudaSuccess) return e;
+  dim3 grid((p->nx + 63) / 64, (p->ny + 3) / 4, batch);
+  if (tau) k_gen_splat<true><<<grid, 256, 0, st>>>(p->lines, p->cols, p->nx, p->ny, p->opt.max_shift_px, tau, nullptr, nullptr, map_out, acc);
+  else k_gen_splat<false><<<grid, 256, 0, st>>>(p->lines, p->cols, p->nx, p->ny, p->opt.max_shift_px, nullptr, I_bins, map_in, nullptr, acc);
+  return cudaGetLastError();
+}
+
+// fixed point -> float in place.  mode 0: P_s − f_s(x) of the detector pixel's column (an EMPTY pixel is written as exactly
+// −f_s(x), so that P_s = 0 exactly downstream: the split's fallback decision, R8); mode 1: P_s (epr_transport, signed).
+__global__ void __launch_bounds__(256) k_gen_fix2float(int n_bins, EprColumns C, int nx, size_t plane, int mode,
+                                                       unsigned* __restrict__ acc, unsigned* __restrict__ flags) {
+  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
+  if (i >= plane) return;
+  const int x = (int)(i % (size_t)nx);
+  const float sc = 1.0f / (float)EPR_FIX_ONE;
+  for (int s = 0; s < n_bins; ++s) {
+    unsigned* ap = acc + ((size_t)blockIdx.y * n_bins + s) * plane + i;
+    const unsigned v = *ap;
+    float o;
+    if (mode == 1) {
+      o = (float)(int)v * sc;
+    } else {
+      if ((v + 1024u) & 0x80000000u) atomicOr(flags, EPR_FLAG_SPLAT_OVERFLOW);
+      const int Fi = (int)__ldg(&C.fixFi[(size_t)s * nx + x]);
+      o = v ? fmaf((float)((int)v - Fi), sc, __ldg(&C.fixCorr[(size_t)s * nx + x])) : -__ldg(&C.f[(size_t)s * nx + x]);
+    }
+    *reinterpret_cast<float*>(ap) = o;
+  }
+}
+
+cudaError_t epr_gen_fix2float(const epr_plan_s* p, int batch, unsigned* acc, int mode, cudaStream_t st) {
+  const size_t plane = (size_t)p->nx * p->ny;
+  dim3 grid((unsigned)((plane + 255) / 256), batch);
+  k_gen_fix2float<<<grid, 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, mode, acc, p->d_flags);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// a2  residual and positivity-weighted split (R8) with the column's f_s(x):
+//   e = (d − 1) − Σ_s (P_s − f_s) − (Σ_s (float)f_s(x) − 1);  w_s = P_s⁺/Σ_t P_t⁺ (fallback f_s(x));  es_s = w_s e.  pred may alias es.
+// =====================================================================================================
+__global__ void __launch_bounds__(256) k_gen_residual(int n_bins, EprColumns C, int nx, size_t plane, const float* __restrict__ d,
+                                                      const float* pred, float* es) {
+  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
+  if (i >= plane) return;
+  const int x = (int)(i % (size_t)nx), b = blockIdx.y;
+  const size_t base = (size_t)b * n_bins * plane + i;
+  float pd[EPR_MAX_BINS], sum = 0.f, den = 0.f;
+  for (int s = 0; s < n_bins; ++s) {
+    pd[s] = pred[base + (size_t)s * plane];
+    sum += pd[s];
+    pd[s] = fmaxf(__ldg(&C.f[(size_t)s * nx + x]) + pd[s], 0.f);      // P_s⁺
+    den += pd[s];
+  }
+  const float e = (__ldg(&d[(size_t)b * plane + i]) - (1.f + __ldg(&C.fsum_dev[x]))) - sum;
+  const float q = den > 0.f ? e / den : 0.f;
+  for (int s = 0; s < n_bins; ++s)
+    es[base + (size_t)s * plane] = den > 0.f ? pd[s] * q : __ldg(&C.f[(size_t)s * nx + x]) * e;
+}
+
+cudaError_t epr_gen_residual(const epr_plan_s* p, int batch, const float* d, const float* pred, float* es, cudaStream_t st) {
+  const size_t plane = (size_t)p->nx * p->ny;
+  dim3 grid((unsigned)((plane + 255) / 256), batch);
+  k_gen_residual<<<grid, 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, d, pred, es);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// a3  adjoint gather, Eq. (4), with the SAME x0, y0, w as the splat: the map of the pixel's own column.
+// =====================================================================================================
+__global__ void __launch_bounds__(256) k_gen_gather(EprLines L, EprColumns C, int nx, int ny, float S, const float* __restrict__ tau,
+                                                    const float2* __restrict__ map_in, const float* __restrict__ es,
+                                                    float* __restrict__ r) {
+  const int x = blockIdx.x * 64 + (threadIdx.x & 63), y = blockIdx.y * 4 + (threadIdx.x >> 6), b = blockIdx.z;
+  if (x >= nx || y >= ny) return;
+  const size_t plane = (size_t)nx * ny, pix = (size_t)y * nx + x;
+  float dtx = 0.f, dty = 0.f;
+  if (!map_in) {
+    const float* tb = tau + (size_t)b * plane;
+    const int xm = x == 0 ? nx - 1 : x - 1, xp = x + 1 == nx ? 0 : x + 1;
+    const int ym = y == 0 ? ny - 1 : y - 1, yp = y + 1 == ny ? 0 : y + 1;
+    dtx = __ldg(tb + (size_t)y * nx + xp) - __ldg(tb + (size_t)y * nx + xm);
+    dty = __ldg(tb + (size_t)yp * nx + x) - __ldg(tb + (size_t)ym * nx + x);
+  }
+  for (int s = 0; s < L.n_bins; ++s) {
+    const size_t pl = ((size_t)b * L.n_bins + s) * plane;
+    float ux, uy;
+    if (map_in) {
+      const float2 m = __ldg(&map_in[pl + pix]);
+      ux = m.x; uy = m.y;
+    } else {
+      const float cs = -0.5f * __ldg(&C.a[(size_t)s * nx + x]) * __ldg(&C.gamma[(size_t)s * nx + x]);
+      ux = fminf(fmaxf(cs * dtx, -S), S);
+      uy = fminf(fmaxf(cs * dty, -S), S);
+    }
+    const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
+    const float dx = ux - (float)fx, dy = uy - (float)fy;
+    const int ix0 = wrapm(x + fx, nx), iy0 = wrapm(y + fy, ny);
+    const int ix1 = ix0 + 1 == nx ? 0 : ix0 + 1, iy1 = iy0 + 1 == ny ? 0 : iy0 + 1;
+    const float* eb = es + pl;
+    const float e00 = __ldg(eb + (size_t)iy0 * nx + ix0), e10 = __ldg(eb + (size_t)iy0 * nx + ix1);
+    const float e01 = __ldg(eb + (size_t)iy1 * nx + ix0), e11 = __ldg(eb + (size_t)iy1 * nx + ix1);
+    const float t0 = fmaf(dx, e10 - e00, e00), t1 = fmaf(dx, e11 - e01, e01);
+    r[pl + pix] = fmaf(dy, t1 - t0, t0);
+  }
+}
+
+cudaError_t epr_gen_gather(const epr_plan_s* p, int batch, const float* tau, const float2* map_in, const float* es, float* r,
+                           cudaStream_t st) {
+  dim3 grid((p->nx + 63) / 64, (p->ny + 3) / 4, batch);
+  k_gen_gather<<<grid, 256, 0, st>>>(p->lines, p->cols, p->nx, p->ny, p->opt.max_shift_px, tau, map_in, es, r);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// a5 + a6  relaxed update and projection to the single-thickness manifold (R10) as an increment, with
+// the scalars of the pixel's column:  ΔT = step · Σ_b wblk[b][x] q_b  (R17(c): block filters blended),
+//   τ += δ,  Σ_s f_s(x) e^{−γ_s(x) τ} expm1(−γ_s(x) δ) = ΔT,  floored so that Σ_s I_s + ΔT >= i_min.
+// =====================================================================================================
+__global__ void __launch_bounds__(256) k_gen_update(int n_bins, EprColumns C, int nx, size_t plane, int n_blocks,
+                                                    const float* __restrict__ qblk, size_t blk_stride, float step,
+                                                    int tau_is_zero, int newton_iters, float i_min, float* __restrict__ tau) {
+  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
+  if (i >= plane) return;
+  const int x = (int)(i % (size_t)nx), b = blockIdx.y;
+  float q = 0.f;
+  for (int k = 0; k < n_blocks; ++k) {
+    const float w = __ldg(&C.wblk[(size_t)k * nx + x]);
+    if (w != 0.f) q = fmaf(w, __ldg(&qblk[(size_t)k * blk_stride + (size_t)b * plane + i]), q);
+  }
+  float* tp = tau + (size_t)b * plane + i;
+  const float t = tau_is_zero ? 0.f : *tp;
+  float delta;
+  if (n_bins == 1) {
+    const float g = __ldg(&C.gamma[x]);                 // one line: f = 1; δ = −log1p(ΔT e^{γτ})/γ in closed form
+    delta = epr_project_increment_mono(g * t, step * q, i_min) / g;
+  } else {
+    float f[EPR_MAX_BINS], g[EPR_MAX_BINS], gmax = 0.f;
+    for (int s = 0; s < n_bins; ++s) {
+      f[s] = __ldg(&C.f[(size_t)s * nx + x]);
+      g[s] = __ldg(&C.gamma[(size_t)s * nx + x]);
+      gmax = fmaxf(gmax, g[s]);
+    }
+    delta = epr_project_increment(t, step * q, f, g, n_bins, gmax, newton_iters, i_min);
+  }
+  *tp = t + delta;
+}
+
+cudaError_t epr_gen_update(const epr_plan_s* p, int batch, const float* qblk, size_t blk_stride, float step, int tau_is_zero,
+                           float* tau, cudaStream_t st) {
+  const size_t plane = (size_t)p->nx * p->ny;
+  dim3 grid((unsigned)((plane + 255) / 256), batch);
+  k_gen_update<<<grid, 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, p->n_blocks, qblk, blk_stride, step, tau_is_zero,
+                                      p->opt.newton_iters, p->opt.i_min, tau);
+  return cudaGetLastError();
+}
+
+// out (+)= wblk[b][x] q over `planes` planes (epr_precondition with block filters)
+__global__ void __launch_bounds__(256) k_gen_blend(const float* __restrict__ w, int nx, size_t n, const float* __restrict__ q,
+                                                   float* __restrict__ out, int accumulate) {
+  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
+  if (i >= n) return;
+  const float v = __ldg(&w[i % (size_t)nx]) * __ldg(&q[i]);
+  out[i] = accumulate ? out[i] + v : v;
+}
+
+cudaError_t epr_gen_blend(const epr_plan_s* p, int planes, int b, const float* q, float* out, int accumulate, cudaStream_t st) {
+  const size_t n = (size_t)planes * p->nx * p->ny;
+  k_gen_blend<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p->cols.wblk + (size_t)b * p->nx, p->nx, n, q, out, accumulate);
+  return cudaGetLastError();
+}
+
+// epr_forward output: P_s = f_s(x) + (P_s − f_s), P = Σ_s P_s
+__global__ void __launch_bounds__(256) k_gen_pred_out(int n_bins, EprColumns C, int nx, size_t plane, const float* __restrict__ pred,
+                                                      float* __restrict__ P_sum, float* __restrict__ P_bins) {
+  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
+  if (i >= plane) return;
+  const int x = (int)(i % (size_t)nx), b = blockIdx.y;
+  const size_t base = (size_t)b * n_bins * plane + i;
+  float sum = 0.f;
+  for (int s = 0; s < n_bins; ++s) {
+    const float v = __ldg(&C.f[(size_t)s * nx + x]) + __ldg(&pred[base + (size_t)s * plane]);
+    sum += v;
+    if (P_bins) P_bins[base + (size_t)s * plane] = v;
+  }
+  if (P_sum) P_sum[(size_t)b * plane + i] = sum;
+}
+
+cudaError_t epr_gen_pred_out(const epr_plan_s* p, int batch, const float* pred, float* P_sum, float* P_bins, cudaStream_t st) {
+  const size_t plane = (size_t)p->nx * p->ny;
+  dim3 grid((unsigned)((plane + 255) / 256), batch);
+  k_gen_pred_out<<<grid, 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, pred, P_sum, P_bins);
+  return cudaGetLastError();
+}
+
+// output conversion with the column's scalars: τ | φ of line out_bin = −(db_s(x)/2) γ_s(x) τ (Eq. (6)) | Σ_s I_s (Eq. (7))
+__global__ void __launch_bounds__(256) k_gen_output(int n_bins, EprColumns C, int nx, size_t n, int mode, int bin, float inv_alpha,
+                                                    const float* __restrict__ tau, float* __restrict__ out) {
+  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
+  if (i >= n) return;
+  const int x = (int)(i % (size_t)nx);
+  const float t = tau[i];
+  float v = t;
+  if (mode == 1) v = -(__ldg(&C.a[(size_t)bin * nx + x]) * inv_alpha) * __ldg(&C.gamma[(size_t)bin * nx + x]) * t;   // db/2 = a/α
+  else if (mode == 2) {
+    v = 0.f;
+    for (int s = 0; s < n_bins; ++s) v += __ldg(&C.f[(size_t)s * nx + x]) * expf(-__ldg(&C.gamma[(size_t)s * nx + x]) * t);
+  }
+  out[i] = v;
+}
+
+cudaError_t epr_gen_output(const epr_plan_s* p, int batch, const float* tau, float* out, cudaStream_t st) {
+  const size_t n = (size_t)p->nx * p->ny * batch;
+  const int sb = p->opt.out_bin;
+  k_gen_output<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p->n_bins, p->cols, p->nx, n, p->opt.output, sb,
+                                                             (float)(1.0 / p->h_alpha[sb]), tau, out);
+  return cudaGetLastError();
+}

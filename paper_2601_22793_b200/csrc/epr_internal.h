@@ -30,6 +30,19 @@ struct EprLines {
   float fsum_dev;               // Σ_s (float)f_s − 1: rounding of the fp32 fractions, removed from the residual
 };
 
+// Per-column scalars of the GENERAL path (x-dependent effective spectrum, PAPER.md:216-229 / §9.2, reading R17; also
+// used with constant columns for grids the tuned kernels do not take).  Device pointers, [n_bins][nx] unless stated.
+struct EprColumns {
+  const float* f;          // f_s(x), Σ_s f_s(x) = 1                                  Eq. (7)
+  const float* gamma;      // γ_s(x)                                                   Eq. (7)
+  const float* a;          // a_s(x) = α_s db_s(x)/2                                   Eq. (1)+(6)
+  const unsigned* fixFi;   // rint(f_s(x) 2^26): fixed-point baseline of the splat
+  const float* fixCorr;    // rint(f_s(x) 2^26) 2^-26 − f_s(x)
+  const float* fsum_dev;   // [nx]  Σ_s (float)f_s(x) − 1
+  const float* wblk;       // [n_blocks][nx] interpolation weights of the block filters (R17(c))
+};
+#define EPR_MAX_BLOCKS 64
+
 struct epr_plan_s {
   int device;                  // CUDA device the plan was built on: every entry point runs there (DevGuard in epr_api.cu)
   int sms;                     // its SM count
@@ -81,6 +94,18 @@ struct epr_plan_s {
   long long graph_launches;    // kernel launches inside the graph
   int graph_warm;              // an eager pass has run (function attributes are set)
   int graph_mode;              // 0 off, 1 on for launch-bound sizes (default), 2 always (EPR_GRAPH)
+  // ---- general path (epr_general.cu): any {2,3,5}-smooth grid >= 8, x-dependent spectrum ----
+  int general;                 // 1: the loop and the operators run the general kernels
+  int fft_generic;             // 1: run-time-radix FFT (size not in the tuned table); spectra are [ny][nx/2 + 1] then
+  int n_blocks;                // blocks of the x-dependent spectrum (1 = uniform)
+  EprColumns cols;             // device tables (owned by the plan: cols_store)
+  void* cols_store;            // one allocation behind `cols`
+  double* h_col;               // host copy [3][n_bins][nx]: f, γ, a per column (epr_plan_columns)
+  float a_blk[EPR_MAX_BLOCKS][EPR_MAX_BINS];   // a_s of block b
+  float abar_blk[EPR_MAX_BLOCKS];              // Σ_s f_s a_s of block b (initial guess)
+  float* qblk;                 // [n_blocks][work_batch][ny][nx] filtered residual sums per block
+  float2* tw_gen_x;            // exp(−2πi m/nx), m < nx   (run-time-radix FFT)
+  float2* tw_gen_y;            // exp(−2πi m/ny), m < ny
   long long launches;
   int prof_on;                 // per-kernel event timing enabled
   void* prof;                  // EprProf*
@@ -122,7 +147,9 @@ cudaError_t epr_launch_rows_r2c(const epr_plan_s* p, int planes, const float* in
                                 cudaStream_t st);
 // mode 0: per-plane filter with bin = plane % n_bins (out has `planes` planes);
 // mode 1: sum over bins (out has planes / n_bins planes);  mode 2: single filter with abar (init).
-cudaError_t epr_launch_cols(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st);
+// lines_override != NULL: the per-line filter coefficients a[] / abar are taken from it instead of p->lines (block filters)
+cudaError_t epr_launch_cols(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st,
+                            const EprLines* lines_override = nullptr);
 // epilogue 0: write q; 1: τ update (Newton projection) with step; init0: treat τ as 0 (initial guess)
 cudaError_t epr_launch_rows_c2r(const epr_plan_s* p, int planes, const float2* spec, int epilogue, float step,
                                 int tau_is_zero, float* q_or_tau, cudaStream_t st);
@@ -135,3 +162,32 @@ cudaError_t epr_launch_diagnostics(const epr_plan_s* p, int batch, const float* 
 // pred[b][s] −= f_s (α_s²/4) ∂i(Î ∂iQ): the WKB1 term of Eq. (1) for the non-local forward (opt.nonlocal_wkb1)
 cudaError_t epr_launch_wkb1_sub(const epr_plan_s* p, int batch, const float* tau, float* pred, cudaStream_t st);
 cudaError_t epr_launch_output(const epr_plan_s* p, int batch, const float* tau, float* out, cudaStream_t st);
+
+// ---- general path (epr_general.cu / epr_fftgen.cu) ----
+// a1-L: pred[b][s] = P_s − f_s(x), every line, per-column scalars frozen at the centre column (R17(b))
+cudaError_t epr_gen_forward_local(const epr_plan_s* p, int batch, const float* tau, float* pred, cudaStream_t st);
+// a1-N: acc[b][s] (u32 fixed point, zeroed here) += splat of line s; sources from τ (I_bins NULL; the ray map goes to map_out if
+// given) or from I_bins with the stored map_in (epr_transport)
+cudaError_t epr_gen_splat(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
+                          float2* map_out, unsigned* acc, cudaStream_t st);
+// fixed-point planes -> float, in place: mode 0: P_s − f_s(x); mode 1: P_s (transport)
+cudaError_t epr_gen_fix2float(const epr_plan_s* p, int batch, unsigned* acc_inout, int mode, cudaStream_t st);
+// a2: es[b][s] = w_s e from pred[b][s] = P_s − f_s (float; may alias es), fallback f_s(x)
+cudaError_t epr_gen_residual(const epr_plan_s* p, int batch, const float* d, const float* pred, float* es, cudaStream_t st);
+// a3: gather with the map recomputed from τ (map_in NULL) or stored
+cudaError_t epr_gen_gather(const epr_plan_s* p, int batch, const float* tau, const float2* map_in, const float* es, float* r,
+                           cudaStream_t st);
+// a5 + a6: τ += δ(τ, step Σ_b wblk[b][x] q_b) with the column's scalars; qblk = [n_blocks][batch] planes
+cudaError_t epr_gen_update(const epr_plan_s* p, int batch, const float* qblk, size_t blk_stride, float step, int tau_is_zero,
+                           float* tau, cudaStream_t st);
+// out (+)= wblk[b][x] · q   (epr_precondition on an x-dependent plan)
+cudaError_t epr_gen_blend(const epr_plan_s* p, int planes, int b, const float* q, float* out, int accumulate, cudaStream_t st);
+cudaError_t epr_gen_pred_out(const epr_plan_s* p, int batch, const float* pred, float* P_sum, float* P_bins, cudaStream_t st);
+cudaError_t epr_gen_output(const epr_plan_s* p, int batch, const float* tau, float* out, cudaStream_t st);
+// run-time-radix FFT (any {2,3,5}-smooth nx, ny): spectra [planes][ny][nx/2 + 1]
+int epr_fftgen_supported(int n);
+size_t epr_fftgen_spec_floats(const epr_plan_s* p);     // floats per spectrum plane
+cudaError_t epr_fftgen_rows_r2c(const epr_plan_s* p, int planes, const float* in, float in_offset, float2* spec, cudaStream_t st);
+cudaError_t epr_fftgen_cols(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st,
+                            const EprLines* lines_override);
+cudaError_t epr_fftgen_rows_c2r(const epr_plan_s* p, int planes, const float2* spec, float* q, cudaStream_t st);

@@ -518,7 +518,7 @@ def test_argument_errors(E):
     import torch
     en, w, db = SPECTRA["mono"]
     with pytest.raises(E.EprError) as ei:
-        E.epr_plan(250, 256, 6.5e-6, 1.0, en, w, db)            # 250 = 2·5³ is not in the supported size table
+        E.epr_plan(224, 256, 6.5e-6, 1.0, en, w, db)            # 224 = 2⁵·7: a prime factor outside {2, 3, 5}
     assert ei.value.status == 2
     with pytest.raises(E.EprError):
         E.epr_plan(256, 256, -1.0, 1.0, en, w, db)
