@@ -331,13 +331,7 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
             epr.epr_retrieve_oversampled(plan, m, d, out, w.iterations, w.step)
 
     def step_host():
-        if m == 1:
-            epr.epr_retrieve_host(plan, d_host, out_host, w.iterations, w.step)
-        else:                                       # no chunked host variant of the oversampled call: plain copies
-            d.copy_(d_host, non_blocking=True)
-            step()
-            out_host.copy_(out, non_blocking=True)
-            torch.cuda.synchronize()
+        epr.epr_retrieve_host(plan, d_host, out_host, w.iterations, w.step, factor=m)
 
     def barrier():
         torch.cuda.synchronize()

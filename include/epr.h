@@ -133,6 +133,16 @@ epr_status epr_retrieve_oversampled(epr_plan_t plan, int factor, int batch, cons
  *   is on, retrievals are not captured into CUDA graphs.  Tuned path only (EPR_EINVAL on a general-path plan). */
 epr_status epr_set_diagnostics(epr_plan_t plan, float* diag, int capacity_iters);
 
+/* epr_shift_histogram — the regime diagnostic of Fig. 6
+ *   "the distribution of estimated WKB0 transverse shifts (in detector-pixel units) for each sampling energy (spectral
+ *   line) on a representative radiograph": for every projection b and line s the histogram over the pixels of
+ *   η = ‖Δ_s‖/p = ‖a_s D⁰ ln I_s‖ (Euclidean norm, not clamped; pixels of the plan's grid) of the thickness field tau
+ *   (e.g. the result of epr_retrieve).  Bin k counts η ∈ [k·bin_px, (k+1)·bin_px), the last bin is open-ended.
+ *   tau  [batch][ny][nx] DEVICE in;  hist [batch][n_bins][n_hist] DEVICE unsigned out (overwritten);  2 <= n_hist <= 1024.
+ *   η < 1 over most of the field: local regime; a significant fraction above 1: use the non-local solver. */
+epr_status epr_shift_histogram(epr_plan_t plan, int batch, const float* tau, int n_hist, float bin_px, unsigned* hist,
+                               void* stream);
+
 /* epr_retrieve_host — same, with HOST buffers (pinned for full speed): copies d host→device, runs the loop,
  *   copies the result device→host.  The batch is cut into chunks of about 256 MB of input (never more than the plan's
  *   work batch; environment EPR_HOST_CHUNK = projections per chunk overrides) that travel on three private streams, so
@@ -171,6 +181,12 @@ epr_status epr_plan_columns(epr_plan_t plan, double* f, double* gamma, double* a
  *   *flags receives the bits; clear != 0 resets them. */
 #define EPR_FLAG_SPLAT_OVERFLOW 1u
 epr_status epr_read_flags(epr_plan_t plan, unsigned* flags, int clear);
+
+/* epr_retrieve_oversampled_host — epr_retrieve_oversampled with HOST buffers on the detector grid
+ *   d_host, out_host [batch][ny/factor][nx/factor]; the same chunked schedule as epr_retrieve_host (copies of neighbouring
+ *   chunks overlap the loop), every chunk replicated, retrieved and block-averaged on the device. */
+epr_status epr_retrieve_oversampled_host(epr_plan_t plan, int factor, int batch, const float* d_host, float* out_host,
+                                         int iterations, float step);
 
 /* Per-line scalars the plan derived (HOST arrays of length n_bins, any may be NULL): f_s, γ_s, a_s, α_s. */
 epr_status epr_plan_lines(epr_plan_t plan, double* f, double* gamma, double* a, double* alpha);

@@ -571,3 +571,21 @@ def retrieve_x(d, prof: Profiles, solver="local", iterations=10, step=1.0, order
         T = np.maximum(np.sum(Is, axis=0), i_min)
         tau = project_x(T, prof)
     return tau
+
+
+# --------------------------------------------------------------------------------------
+# regime diagnostic: per-line distribution of the eikonal shift (Fig. 6)
+# --------------------------------------------------------------------------------------
+def shift_histogram(tau, lines: Lines, n_hist, bin_px):
+    """"the distribution of estimated WKB0 transverse shifts (in detector-pixel units) for each sampling energy (spectral
+    line) on a representative radiograph": for every line the histogram of η(r) = ‖Δ_s(r)‖/p =
+    ‖a_s D⁰ ln I_s‖ (Eq. (2), Euclidean norm, NOT clamped) over the pixels, bins [k·bin_px, (k+1)·bin_px),
+    the last bin open-ended.  Returns integer counts [n_bins][n_hist] (each row sums to the number of pixels)."""
+    Is = line_intensities(tau, lines)
+    out = np.zeros((lines.n_bins, n_hist), dtype=np.int64)
+    for s in range(lines.n_bins):
+        ux, uy = ray_map(Is[s], lines.a[s], np.inf)
+        eta = np.sqrt(ux * ux + uy * uy)
+        k = np.minimum(np.floor(eta / bin_px).astype(np.int64), n_hist - 1)
+        out[s] = np.bincount(k.ravel(), minlength=n_hist)
+    return out

@@ -14,7 +14,8 @@ _LIB = None
 EXPORTS = ["epr_default_options", "epr_plan", "epr_forward", "epr_adjoint", "epr_transport", "epr_precondition",
            "epr_retrieve", "epr_retrieve_oversampled", "epr_set_diagnostics", "epr_retrieve_host", "epr_plan_lines", "epr_launch_count", "epr_destroy",
            "epr_last_error", "epr_version", "epr_profile_enable", "epr_profile_read", "epr_read_flags",
-           "epr_plan_profiles", "epr_plan_columns"]
+           "epr_plan_profiles", "epr_plan_columns", "epr_shift_histogram",
+           "epr_retrieve_oversampled_host"]
 EPR_FLAG_SPLAT_OVERFLOW = 1
 
 
@@ -57,6 +58,8 @@ def load_library():
     lib.epr_retrieve_oversampled.argtypes = [vp, ci, ci, vp, vp, ci, cf, vp]
     lib.epr_set_diagnostics.argtypes = [vp, vp, ci]
     lib.epr_retrieve_host.argtypes = [vp, ci, vp, vp, ci, cf]
+    lib.epr_retrieve_oversampled_host.argtypes = [vp, ci, ci, vp, vp, ci, cf]
+    lib.epr_retrieve_oversampled_host.restype = ci
     lib.epr_plan_lines.argtypes = [vp, C.POINTER(cd), C.POINTER(cd), C.POINTER(cd), C.POINTER(cd)]
     lib.epr_launch_count.argtypes = [vp]
     lib.epr_launch_count.restype = C.c_longlong
@@ -69,6 +72,8 @@ def load_library():
     lib.epr_plan_profiles.restype = ci
     lib.epr_plan_columns.argtypes = [vp, C.POINTER(cd), C.POINTER(cd), C.POINTER(cd)]
     lib.epr_plan_columns.restype = ci
+    lib.epr_shift_histogram.argtypes = [vp, ci, vp, ci, cf, vp, vp]
+    lib.epr_shift_histogram.restype = ci
     lib.epr_read_flags.argtypes = [vp, C.POINTER(C.c_uint), ci]
     lib.epr_read_flags.restype = ci
     lib.epr_last_error.argtypes = [vp]
@@ -248,6 +253,16 @@ def epr_retrieve_oversampled(plan, factor, d, out, iterations, step):
                                                         int(iterations), float(step), _stream()))
 
 
+def epr_shift_histogram(plan, tau, n_hist, bin_px):
+    """Per-line histogram of the unclamped shift norm of `tau` (epr_shift_histogram): int32 CUDA tensor [batch][n_bins][n_hist]."""
+    import torch
+    b = tau.shape[0]
+    hist = torch.zeros((b, plan.n_bins, int(n_hist)), dtype=torch.int32, device=tau.device)
+    plan._check(load_library().epr_shift_histogram(plan._h, b, _dev(tau, (b, plan.ny, plan.nx), "tau"), int(n_hist), float(bin_px),
+                                                   C.c_void_p(hist.data_ptr()), _stream()))
+    return hist
+
+
 def epr_set_diagnostics(plan, diag):
     """diag: contiguous float32 CUDA tensor [batch][capacity_iters][2] (kept alive by the caller), or None to switch off."""
     if diag is None:
@@ -258,8 +273,9 @@ def epr_set_diagnostics(plan, diag):
     plan._check(load_library().epr_set_diagnostics(plan._h, _dev(diag, None, "diag"), int(diag.shape[1])))
 
 
-def epr_retrieve_host(plan, d_host, out_host, iterations, step):
-    """HOST buffers (pinned float32 torch tensors or C-contiguous numpy arrays), copies inside the call."""
+def epr_retrieve_host(plan, d_host, out_host, iterations, step, factor=1):
+    """HOST buffers (pinned float32 torch tensors or C-contiguous numpy arrays), copies inside the call.
+    factor > 1: epr_retrieve_oversampled_host — buffers on the detector grid [batch][ny/factor][nx/factor]."""
     def hp(a, name):
         if isinstance(a, np.ndarray):
             if a.dtype != np.float32 or not a.flags.c_contiguous:
@@ -271,6 +287,12 @@ def epr_retrieve_host(plan, d_host, out_host, iterations, step):
         return C.c_void_p(a.data_ptr()), tuple(a.shape)
     pd, sd = hp(d_host, "d_host")
     po, so = hp(out_host, "out_host")
-    if tuple(sd) != tuple(so) or tuple(sd[1:]) != (plan.ny, plan.nx):
-        raise ValueError("d_host / out_host must both be [batch][ny][nx]")
-    plan._check(load_library().epr_retrieve_host(plan._h, int(sd[0]), pd, po, int(iterations), float(step)))
+    factor = int(factor)
+    if factor < 1 or plan.ny % factor or plan.nx % factor:
+        raise ValueError("factor must divide the plan's grid")
+    if tuple(sd) != tuple(so) or tuple(sd[1:]) != (plan.ny // factor, plan.nx // factor):
+        raise ValueError("d_host / out_host must both be [batch][ny / factor][nx / factor]")
+    if factor == 1:
+        plan._check(load_library().epr_retrieve_host(plan._h, int(sd[0]), pd, po, int(iterations), float(step)))
+    else:
+        plan._check(load_library().epr_retrieve_oversampled_host(plan._h, factor, int(sd[0]), pd, po, int(iterations), float(step)))

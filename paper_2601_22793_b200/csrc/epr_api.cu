@@ -726,6 +726,19 @@ static epr_status retrieve_device(epr_plan_t p, int batch, const float* d, float
   return EPR_OK;
 }
 
+// Per-line distribution of the eikonal shift of a given thickness field (Fig. 6).
+extern "C" epr_status epr_shift_histogram(epr_plan_t p, int batch, const float* tau, int n_hist, float bin_px, unsigned* hist,
+                                          void* stream) {
+  epr_status st = check_call(p, batch);
+  if (st != EPR_OK) return st;
+  DevGuard dg(p);
+  if (!tau || !hist) FAIL(p, EPR_EINVAL, "epr_shift_histogram: NULL pointer");
+  if (n_hist < 2 || n_hist > 1024 || !(bin_px > 0.f)) FAIL(p, EPR_EINVAL, "epr_shift_histogram: n_hist must be in 2..1024 and bin_px > 0");
+  cudaStream_t cs = (cudaStream_t)stream;
+  KL(p, K_DIAG, cs, epr_launch_shift_hist(p, batch, tau, n_hist, bin_px, hist, cs));
+  return EPR_OK;
+}
+
 // Per-iteration diagnostics of the following retrievals: residual RMS and largest shift component (device array).
 extern "C" epr_status epr_set_diagnostics(epr_plan_t p, float* diag, int capacity_iters) {
   if (!p) return EPR_EINVAL;
@@ -744,6 +757,32 @@ extern "C" epr_status epr_set_diagnostics(epr_plan_t p, float* diag, int capacit
   return EPR_OK;
 }
 
+static epr_status ensure_oversampling_buffers(epr_plan_t p) {
+  if (p->os_d) return EPR_OK;
+  const size_t plane = (size_t)p->nx * p->ny;
+  cudaError_t e = cudaMalloc((void**)&p->os_d, (size_t)p->work_batch * plane * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&p->os_out, (size_t)p->work_batch * plane * sizeof(float));
+  if (e != cudaSuccess) FAIL(p, e == cudaErrorMemoryAllocation ? EPR_ENOMEM : EPR_ECUDA, "oversampling buffers: %s", cudaGetErrorString(e));
+  return EPR_OK;
+}
+
+static epr_status check_oversampling(epr_plan_t p, int factor, const char* who) {
+  if (factor < 1 || factor > 8 || p->nx % (4 * factor) != 0 || p->ny % factor != 0)
+    FAIL(p, EPR_EINVAL, "%s: factor %d must be in 1..8 and divide the plan's grid %d x %d (nx / factor a multiple of 4)", who, factor, p->nx, p->ny);
+  if (p->opt.init != 0) FAIL(p, EPR_EINVAL, "%s: opt.init = 1 (caller-supplied start) is not supported", who);
+  return EPR_OK;
+}
+
+// replicate -> loop -> block mean for nb <= work_batch projections (coarse in / out may be any device buffers)
+static epr_status retrieve_oversampled_chunk(epr_plan_t p, int factor, int nb, const float* d_coarse, float* out_coarse,
+                                             int iterations, float step, int b_first, cudaStream_t cs) {
+  KL(p, K_RESAMPLE, cs, epr_launch_upsample(p, nb, factor, d_coarse, p->os_d, cs));
+  epr_status st = retrieve_device(p, nb, p->os_d, p->os_out, iterations, step, b_first, cs);
+  if (st != EPR_OK) return st;
+  KL(p, K_RESAMPLE, cs, epr_launch_downsample(p, nb, factor, p->os_out, out_coarse, cs));
+  return EPR_OK;
+}
+
 // The loop on an oversampled grid (reading R16): the plan is the FINE grid's.
 extern "C" epr_status epr_retrieve_oversampled(epr_plan_t p, int factor, int batch, const float* d, float* out,
                                                int iterations, float step, void* stream) {
@@ -752,22 +791,14 @@ extern "C" epr_status epr_retrieve_oversampled(epr_plan_t p, int factor, int bat
   DevGuard dg(p);
   if (!d || !out) FAIL(p, EPR_EINVAL, "epr_retrieve_oversampled: NULL pointer");
   if (iterations < 0 || !(step > 0.f)) FAIL(p, EPR_EINVAL, "epr_retrieve_oversampled: iterations must be >= 0 and step > 0");
-  if (factor < 1 || factor > 8 || p->nx % (4 * factor) != 0 || p->ny % factor != 0)
-    FAIL(p, EPR_EINVAL, "epr_retrieve_oversampled: factor %d must be in 1..8 and divide the plan's grid %d x %d (nx / factor a multiple of 4)", factor, p->nx, p->ny);
-  if (p->opt.init != 0) FAIL(p, EPR_EINVAL, "epr_retrieve_oversampled: opt.init = 1 (caller-supplied start) is not supported");
+  if ((st = check_oversampling(p, factor, "epr_retrieve_oversampled")) != EPR_OK) return st;
+  if ((st = ensure_oversampling_buffers(p)) != EPR_OK) return st;
   cudaStream_t cs = (cudaStream_t)stream;
   const size_t plane = (size_t)p->nx * p->ny, cplane = plane / ((size_t)factor * factor);
-  if (!p->os_d) {
-    cudaError_t e = cudaMalloc((void**)&p->os_d, (size_t)p->work_batch * plane * sizeof(float));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&p->os_out, (size_t)p->work_batch * plane * sizeof(float));
-    if (e != cudaSuccess) FAIL(p, e == cudaErrorMemoryAllocation ? EPR_ENOMEM : EPR_ECUDA, "oversampling buffers: %s", cudaGetErrorString(e));
-  }
   for (int b0 = 0; b0 < batch; b0 += p->work_batch) {
     const int nb = (batch - b0 < p->work_batch) ? batch - b0 : p->work_batch;
-    KL(p, K_RESAMPLE, cs, epr_launch_upsample(p, nb, factor, d + (size_t)b0 * cplane, p->os_d, cs));
-    st = retrieve_device(p, nb, p->os_d, p->os_out, iterations, step, b0, cs);
+    st = retrieve_oversampled_chunk(p, factor, nb, d + (size_t)b0 * cplane, out + (size_t)b0 * cplane, iterations, step, b0, cs);
     if (st != EPR_OK) return st;
-    KL(p, K_RESAMPLE, cs, epr_launch_downsample(p, nb, factor, p->os_out, out + (size_t)b0 * cplane, cs));
   }
   return EPR_OK;
 }
@@ -828,13 +859,12 @@ extern "C" epr_status epr_retrieve(epr_plan_t p, int batch, const float* d, floa
   return EPR_OK;
 }
 
-extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_host, float* out_host, int iterations,
-                                        float step) {
-  if (!p) return EPR_EINVAL;
-  DevGuard dg(p);
+// factor = 1: the plan's grid; factor > 1: host buffers on the detector grid, the loop on the plan's (fine) grid (R16)
+static epr_status retrieve_host_impl(epr_plan_t p, int factor, int batch, const float* d_host, float* out_host, int iterations,
+                                     float step) {
   if (batch < 1 || !d_host || !out_host) FAIL(p, EPR_EINVAL, "epr_retrieve_host: bad batch or NULL pointer");
   if (iterations < 0 || !(step > 0.f)) FAIL(p, EPR_EINVAL, "epr_retrieve_host: iterations must be >= 0 and step > 0");
-  const size_t plane = (size_t)p->nx * p->ny;
+  const size_t plane = (size_t)p->nx * p->ny / ((size_t)factor * factor);       // a plane of the HOST buffers
   // Host chunks are smaller than the device work batch so that the copies of chunk i±1 overlap the loop of chunk i:
   // about 256 MB of input per chunk (EPR_HOST_CHUNK overrides), at least min_chunks chunks per call when the batch allows
   // (C2, batch 64: chunks of 8 / 12 / 16 / 24 projections give 1012 / 1044 / 1060 / 987 projections/s end to end).
@@ -845,7 +875,7 @@ extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_
   // with chunks of 1 / 2 / 4; C3, batch 8, r = 0.37: 464 / 542 / 542 / 500 with chunks of 1 / 2 / 4 / 8).
   const int nbn = p->n_bins;
   const double bpp = (p->solver == EPR_LOCAL) ? (nbn == 1 ? 40.0 : 24.0 + 24.0 * nbn) : (nbn == 1 ? 52.0 : 28.0 + 24.0 * nbn);
-  const double r = (8.0 / 50.0) / ((iterations + 1) * bpp / 2500.0);
+  const double r = (8.0 / 50.0) / ((iterations + 1) * bpp * factor * factor / 2500.0);
   const int min_chunks = r >= 0.3 ? 4 : r >= 0.15 ? 2 : 1;
   int wbch = (int)(((size_t)256 << 20) / (plane * sizeof(float)));
   if (wbch > (batch + min_chunks - 1) / min_chunks) wbch = (batch + min_chunks - 1) / min_chunks;
@@ -853,7 +883,7 @@ extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_
   { const char* env = getenv("EPR_HOST_CHUNK"); if (env && atoi(env) > 0) wbch = atoi(env); }
   if (wbch < 1) wbch = 1;
   if (wbch > p->work_batch) wbch = p->work_batch;
-  if (p->stage_in[0] && p->stage_chunk < wbch) {           // staging buffers too small for this call: re-allocate
+  if (p->stage_in[0] && p->stage_floats < (size_t)wbch * plane) {           // staging buffers too small for this call: re-allocate
     CU(p, cudaDeviceSynchronize());
     for (int i = 0; i < 2; ++i) { cudaFree(p->stage_in[i]); cudaFree(p->stage_out[i]); p->stage_in[i] = p->stage_out[i] = NULL; }
   }
@@ -863,6 +893,7 @@ extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_
       CU(p, cudaMalloc((void**)&p->stage_out[i], (size_t)wbch * plane * sizeof(float)));
     }
     p->stage_chunk = wbch;
+    p->stage_floats = (size_t)wbch * plane;
   }
   if (!p->hstream[0]) {
     for (int i = 0; i < 3; ++i) CU(p, cudaStreamCreateWithFlags(&p->hstream[i], cudaStreamNonBlocking));
@@ -900,7 +931,8 @@ extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_
       CU(p, cudaMemcpyAsync(p->stage_out[buf], out_host + (size_t)b0 * plane, bytes, cudaMemcpyHostToDevice, s_in));
     CU(p, cudaEventRecord(ev_in, s_in));
     CU(p, cudaStreamWaitEvent(s_cmp, ev_in, 0));
-    epr_status st = retrieve_device(p, nb, p->stage_in[buf], p->stage_out[buf], iterations, step, b0, s_cmp);
+    epr_status st = factor == 1 ? retrieve_device(p, nb, p->stage_in[buf], p->stage_out[buf], iterations, step, b0, s_cmp)
+                                : retrieve_oversampled_chunk(p, factor, nb, p->stage_in[buf], p->stage_out[buf], iterations, step, b0, s_cmp);
     if (st != EPR_OK) return st;
     CU(p, cudaEventRecord(ev_cmp, s_cmp));
     CU(p, cudaStreamWaitEvent(s_out, ev_cmp, 0));
@@ -910,4 +942,23 @@ extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_
   CU(p, cudaStreamSynchronize(s_out));
   CU(p, cudaStreamSynchronize(s_cmp));
   return EPR_OK;
+}
+
+extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_host, float* out_host, int iterations,
+                                        float step) {
+  if (!p) return EPR_EINVAL;
+  DevGuard dg(p);
+  return retrieve_host_impl(p, 1, batch, d_host, out_host, iterations, step);
+}
+
+// Host buffers on the DETECTOR grid, the loop on the oversampled grid of the plan (R16): the same chunked,
+// overlapped schedule; every chunk is replicated, retrieved and block-averaged on the device.
+extern "C" epr_status epr_retrieve_oversampled_host(epr_plan_t p, int factor, int batch, const float* d_host, float* out_host,
+                                                    int iterations, float step) {
+  if (!p) return EPR_EINVAL;
+  DevGuard dg(p);
+  epr_status st = check_oversampling(p, factor, "epr_retrieve_oversampled_host");
+  if (st != EPR_OK) return st;
+  if ((st = ensure_oversampling_buffers(p)) != EPR_OK) return st;
+  return retrieve_host_impl(p, factor, batch, d_host, out_host, iterations, step);
 }

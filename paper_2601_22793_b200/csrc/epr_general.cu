@@ -365,3 +365,46 @@ cudaError_t epr_gen_output(const epr_plan_s* p, int batch, const float* tau, flo
                                                              (float)(1.0 / p->h_alpha[sb]), tau, out);
   return cudaGetLastError();
 }
+
+// =====================================================================================================
+// Regime diagnostic (Fig. 6): per projection and line, the histogram over the pixels of
+// η = ‖Δ_s‖/p = a_s γ_s ‖D⁰τ‖ (Euclidean norm of the UNCLAMPED eikonal shift, Eq. (2)), bins [k·bin_px, (k+1)·bin_px), the last
+// one open-ended.  hist: [batch][n_bins][n_hist] unsigned, accumulated (the launcher zeroes it).  Works on both paths: the
+// scalars come from the column tables when the plan has them, from the uniform per-line scalars otherwise.
+// One thread = one pixel; counts are collected per CTA in shared memory first.
+// =====================================================================================================
+__global__ void __launch_bounds__(256) k_shift_hist(EprLines L, EprColumns C, int use_cols, int nx, int ny, int n_hist,
+                                                    float inv_bin, const float* __restrict__ tau, unsigned* __restrict__ hist) {
+  extern __shared__ unsigned s_h[];                     // [n_bins][n_hist]
+  const int nb = L.n_bins, b = blockIdx.z;
+  for (int i = threadIdx.x; i < nb * n_hist; i += 256) s_h[i] = 0u;
+  __syncthreads();
+  const int x = blockIdx.x * 64 + (threadIdx.x & 63), y = blockIdx.y * 4 + (threadIdx.x >> 6);
+  if (x < nx && y < ny) {
+    const float* tb = tau + (size_t)b * nx * ny;
+    const int xm = x == 0 ? nx - 1 : x - 1, xp = x + 1 == nx ? 0 : x + 1;
+    const int ym = y == 0 ? ny - 1 : y - 1, yp = y + 1 == ny ? 0 : y + 1;
+    const float dtx = __ldg(tb + (size_t)y * nx + xp) - __ldg(tb + (size_t)y * nx + xm);
+    const float dty = __ldg(tb + (size_t)yp * nx + x) - __ldg(tb + (size_t)ym * nx + x);
+    const float g = 0.5f * sqrtf(dtx * dtx + dty * dty);                      // ‖D⁰τ‖
+    for (int s = 0; s < nb; ++s) {
+      const float c = use_cols ? __ldg(&C.a[(size_t)s * nx + x]) * __ldg(&C.gamma[(size_t)s * nx + x]) : L.a[s] * L.gamma[s];
+      const int k = min((int)(c * g * inv_bin), n_hist - 1);
+      atomicAdd(&s_h[s * n_hist + k], 1u);
+    }
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < nb * n_hist; i += 256)
+    if (s_h[i]) atomicAdd(&hist[(size_t)b * nb * n_hist + i], s_h[i]);
+}
+
+cudaError_t epr_launch_shift_hist(const epr_plan_s* p, int batch, const float* tau, int n_hist, float bin_px, unsigned* hist,
+                                  cudaStream_t st) {
+  const size_t n = (size_t)batch * p->n_bins * n_hist;
+  cudaError_t e = cudaMemsetAsync(hist, 0, n * sizeof(unsigned), st);
+  if (e != cudaSuccess) return e;
+  dim3 grid((p->nx + 63) / 64, (p->ny + 3) / 4, batch);
+  k_shift_hist<<<grid, 256, (size_t)p->n_bins * n_hist * sizeof(unsigned), st>>>(p->lines, p->cols, p->general, p->nx, p->ny, n_hist,
+                                                                                  1.f / bin_px, tau, hist);
+  return cudaGetLastError();
+}

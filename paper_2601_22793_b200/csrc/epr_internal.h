@@ -83,6 +83,7 @@ struct epr_plan_s {
   float* stage_in[2];
   float* stage_out[2];
   int stage_chunk;             // projections the staging buffers hold
+  size_t stage_floats;         // floats each staging buffer holds
   cudaStream_t hstream[3];     // copy-in, compute, copy-out
   cudaEvent_t hev[6];          // per buffer: in-done, compute-done, out-done
   // CUDA graph of the last epr_retrieve (same buffers, batch, iterations, step): replayed instead of re-enqueued
@@ -191,3 +192,6 @@ cudaError_t epr_fftgen_rows_r2c(const epr_plan_s* p, int planes, const float* in
 cudaError_t epr_fftgen_cols(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st,
                             const EprLines* lines_override);
 cudaError_t epr_fftgen_rows_c2r(const epr_plan_s* p, int planes, const float2* spec, float* q, cudaStream_t st);
+// per-line histogram of the unclamped shift norm (Fig. 6); hist [batch][n_bins][n_hist], zeroed by the launcher
+cudaError_t epr_launch_shift_hist(const epr_plan_s* p, int batch, const float* tau, int n_hist, float bin_px, unsigned* hist,
+                                  cudaStream_t st);

@@ -738,3 +738,66 @@ def test_splat_overflow_flag(E):
     assert plan.read_flags(clear=False) & EPR_FLAG_SPLAT_OVERFLOW
     assert plan.read_flags() & EPR_FLAG_SPLAT_OVERFLOW and plan.read_flags() == 0      # cleared by the read
     plan.destroy()
+
+
+def test_oversampled_host_path_and_shift_histogram(E):
+    """epr_retrieve_oversampled_host (detector-grid host buffers, chunked: batch 5 > max_batch 2) equals the device call bit
+    for bit; epr_shift_histogram of the result against the oracle's per-line histogram (Fig. 6): the bin of a
+    pixel is decided by a float, so the counts may differ by the pixels whose fp64 value lies within 1e-4 of a bin edge."""
+    import torch
+    w = make_workload("C4", n=64, batch=5)
+    m = 2
+    plan = E.epr_plan(m * w.nx, m * w.ny, w.pixel_m / m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
+                      max_batch=2, max_shift_px=24.0)
+    dh = torch.from_numpy(w.d).pin_memory()
+    oh = torch.empty_like(dh).pin_memory()
+    E.epr_retrieve_host(plan, dh, oh, 3, w.step, factor=m)
+    for j0 in (0, 2, 4):
+        d = _dev(w.d[j0:j0 + 2])
+        out = torch.empty_like(d)
+        E.epr_retrieve_oversampled(plan, m, d, out, 3, w.step)
+        assert torch.equal(out.cpu(), oh[j0:j0 + 2])
+    plan.destroy()
+    # histogram on a plan of the detector grid, from the retrieved τ
+    plan = E.epr_plan(w.nx, w.ny, w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver, max_batch=5)
+    tau = oh.cuda()
+    n_hist, bin_px = 64, 0.25
+    hist = E.epr_shift_histogram(plan, tau, n_hist, bin_px).cpu().numpy()
+    plan.destroy()
+    lines = O.derive_lines(w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta)
+    for j in range(5):
+        t64 = oh[j].numpy().astype(np.float64)
+        ref = O.shift_histogram(t64, lines, n_hist, bin_px)
+        assert np.all(hist[j].sum(axis=1) == w.nx * w.ny)
+        for s in range(w.n_bins):
+            ux, uy = O.ray_map(O.line_intensities(t64, lines)[s], lines.a[s], np.inf)
+            eta = np.sqrt(ux * ux + uy * uy) / bin_px
+            near_edge = int(np.sum(np.abs(eta - np.rint(eta)) < 1e-4 * np.maximum(eta, 1.0)))
+            assert np.sum(np.abs(hist[j, s].astype(np.int64) - ref[s])) <= 2 * near_edge
+        assert ref[0].argmax() != ref[-1].argmax() or ref[0].max() != ref[-1].max()
+
+
+def test_two_plans_on_two_devices(E):
+    """A plan belongs to the device that was current in epr_plan; launcher state (function attributes, occupancy) is kept
+    per device.  Runs when two GPUs are visible: one plan each, interleaved calls from the OTHER device's context, results
+    equal to the one-device result."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two visible GPUs")
+    w = make_workload("C3", n=256)
+    outs = []
+    plans = []
+    for dev in (0, 1):
+        with torch.cuda.device(dev):
+            plans.append(E.epr_plan(w.nx, w.ny, w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
+                                    max_batch=1, max_shift_px=w.max_shift_px))
+    for dev in (0, 1):
+        d = torch.from_numpy(w.d[:1]).to(f"cuda:{dev}")
+        out = torch.empty_like(d)
+        with torch.cuda.device(1 - dev):                           # the caller's current device is the OTHER one; the
+            E.epr_retrieve(plans[dev], d, out, w.iterations, w.step)   # default stream handle (0) means the plan's device
+        torch.cuda.synchronize(dev)
+        outs.append(out.cpu())
+    for p in plans:
+        p.destroy()
+    assert torch.equal(outs[0], outs[1])

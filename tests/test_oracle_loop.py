@@ -260,3 +260,25 @@ def test_positivity_floor_returns_tau_of_i_min(n_lines):
         assert np.max(np.abs(np.delete(T.ravel(), 3 * 12 + 5) - 0.9)) < 1e-9
         if n_lines == 1:
             assert abs(tau[3, 5] + np.log(i_min)) < 1e-12
+
+
+def test_shift_histogram_closed_form():
+    """η = ‖Δ‖/p per line.  τ = −(c x + e y) (I_s = f_s exp(γ_s (c x + e y))) gives the same shift
+    a_s γ_s √(c² + e²) at every pixel whose central differences do not straddle the periodic seam, so each line's
+    histogram is one spike of (nx − 2)(ny − 2) pixels in a bin known in closed form; the seam pixels (larger differences)
+    land in higher bins; every row sums to the number of pixels."""
+    E = np.array([80.0, 120.0])
+    lines = O.derive_lines(6.5e-6, 2.0, E, [0.5, 0.5], [800.0, 1200.0])
+    ny, nx, c, e = 12, 20, 0.003, 0.004
+    y, x = np.meshgrid(np.arange(ny, dtype=np.float64), np.arange(nx, dtype=np.float64), indexing="ij")
+    tau = -(c * x + e * y) + 1.0
+    n_hist, bin_px = 40, 0.05
+    h = O.shift_histogram(tau, lines, n_hist, bin_px)
+    assert h.shape == (2, n_hist) and np.all(h.sum(axis=1) == nx * ny)
+    for s in range(2):
+        eta = lines.a[s] * lines.gamma[s] * np.hypot(c, e)
+        k = int(np.floor(eta / bin_px))
+        assert 0 < k < n_hist - 1
+        assert h[s, k] == (nx - 2) * (ny - 2)
+        assert h[s, :k].sum() == 0 and h[s, k + 1:].sum() == nx * ny - (nx - 2) * (ny - 2)   # seam pixels: larger shifts
+    assert int(np.argmax(h[0])) != int(np.argmax(h[1]))              # the lines differ (Fig. 6: one curve per line)
