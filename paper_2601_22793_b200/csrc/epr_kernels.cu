@@ -140,7 +140,10 @@ __global__ void __launch_bounds__(32 * LM_WPC) k_local_march(EprLines L, int nx,
     {
       const float x0 = cg * t_c.v[0], x1 = cg * t_c.v[1], x2 = cg * t_c.v[2], x3 = cg * t_c.v[3];
       const float mx = fmaxf(fmaxf(fabsf(x0), fabsf(x1)), fmaxf(fabsf(x2), fabsf(x3)));
-      if (__any_sync(0xffffffffu, mx >= 0.35f)) {        // rare (thick object): both branches of epr_expm1
+      if (!__any_sync(0xffffffffu, mx >= 0.09f)) {       // weak absorption (most rows): a shorter series is exact in fp32
+        A_c.v[0] = epr_expm1_tiny(x0); A_c.v[1] = epr_expm1_tiny(x1);
+        A_c.v[2] = epr_expm1_tiny(x2); A_c.v[3] = epr_expm1_tiny(x3);
+      } else if (__any_sync(0xffffffffu, mx >= 0.35f)) {  // rare (thick object): both branches of epr_expm1
         A_c.v[0] = epr_expm1(x0); A_c.v[1] = epr_expm1(x1); A_c.v[2] = epr_expm1(x2); A_c.v[3] = epr_expm1(x3);
       } else {
         A_c.v[0] = epr_expm1_small(x0); A_c.v[1] = epr_expm1_small(x1);
@@ -414,24 +417,35 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
   }
   // one line with the residual fused (out_mode 2): the d values of this thread's flush groups are requested now, so that
   // the flush does not wait on them (the load used to be 21 % of the kernel's stall samples)
+  // Flush geometry: a thread owns the same NFL groups of 4 pixels for every line — column group tid % 32, rows
+  // fty + FRS·k — so the shared-memory offsets are immediates and the global offset advances by FRS·nx per group
+  // (the generic index arithmetic i = tid + k·NT → (ty, tx) cost 21 of the 66 instructions of a group).
   constexpr int NFL = ST_W * TH / 4 / ST_NT;         // flush groups (4 pixels) per thread
+  constexpr int FRS = ST_NT / (ST_W / 4);            // rows between a thread's consecutive groups
+  const int ftx = 4 * (tid % (ST_W / 4)), fty = tid / (ST_W / 4);
+  const bool fxin = x0 + ftx < nx;
+  const int frows = ny - y0 - fty;                   // group k is inside the image iff fxin && FRS·k < frows
+  const unsigned fg0 = (unsigned)(y0 + fty) * nx + (x0 + ftx), fgs = (unsigned)FRS * nx;
+  unsigned* facc = s_acc + (fty + 1) * ST_AP + 4 + ftx;
   float4 dpre[NFL];
   if (out_mode == 2) {
+    const float* dg = d + (size_t)b * plane + fg0;
 #pragma unroll
     for (int k = 0; k < NFL; ++k) {
-      const int i = tid + k * ST_NT;
-      const int ty = i / (ST_W / 4), tx = 4 * (i - ty * (ST_W / 4));
       dpre[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (x0 + tx < nx && y0 + ty < ny)
-        dpre[k] = __ldg(reinterpret_cast<const float4*>(d + (size_t)b * plane + (unsigned)(y0 + ty) * nx + (x0 + tx)));
+      if (fxin && FRS * k < frows) dpre[k] = __ldg(reinterpret_cast<const float4*>(dg + k * fgs));
     }
   }
   for (int s = 0; s < L.n_bins; ++s) {
     const size_t pl = ((size_t)b * L.n_bins + s) * plane;
-    __syncthreads();                                   // previous bin flushed
-    for (int i = tid; i < ST_AP * (TH + 2) / 4; i += ST_NT) reinterpret_cast<uint4*>(s_acc)[i] = make_uint4(0u, 0u, 0u, 0u);
-    if (FROM_TAU && s == 0) cp_async_wait<0>();
-    __syncthreads();
+    // The accumulator tile is zeroed once; afterwards the flush of a line zeroes what it reads (and the unflushed
+    // border), so a line costs two barriers — after the scatter, after the flush — and no separate clearing pass.
+    if (s == 0) {
+      __syncthreads();                                 // (the candidate list above reads the τ tile; s_acc is untouched so far)
+      for (int i = tid; i < ST_AP * (TH + 2) / 4; i += ST_NT) reinterpret_cast<uint4*>(s_acc)[i] = make_uint4(0u, 0u, 0u, 0u);
+      if (FROM_TAU) cp_async_wait<0>();
+    }
+    __syncthreads();                                   // accumulators clear (first line) / previous line flushed and cleared
     const float cs = -0.5f * L.a[s] * L.gamma[s], gam = L.gamma[s], fixFf = (float)L.fixF[s];
     const int Fi = (int)L.fixFi[s];
     // a source at distance D from the tile reaches it only if ⌊|u|⌋ + 1 ≥ D
@@ -554,14 +568,20 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
     __syncthreads();
     // flush the tile: 4 pixels per thread per pass
     const float sc = 1.0f / (float)EPR_FIX_ONE, corr = L.fixCorr[s];
+    float* ol = out + pl + fg0;
+    // border cells (4 columns left and right of every row, the rows above and below): out-of-tile corners, never flushed
+    if (tid < 2 * (TH + 2)) {
+      const int r = tid >> 1;
+      *reinterpret_cast<uint4*>(s_acc + r * ST_AP + ((tid & 1) ? ST_W + 4 : 0)) = make_uint4(0u, 0u, 0u, 0u);
+    } else if (tid < 2 * (TH + 2) + 2 * (ST_W / 4)) {
+      const int j = tid - 2 * (TH + 2), r = (j & 1) ? TH + 1 : 0;
+      *reinterpret_cast<uint4*>(s_acc + r * ST_AP + 4 + 4 * (j >> 1)) = make_uint4(0u, 0u, 0u, 0u);
+    }
 #pragma unroll
     for (int k = 0; k < NFL; ++k) {
-      const int i = tid + k * ST_NT;
-      const int ty = i / (ST_W / 4), tx = 4 * (i - ty * (ST_W / 4));
-      const int gx = x0 + tx, gy = y0 + ty;
-      if (gx >= nx || gy >= ny) continue;
-      const uint4 v = *reinterpret_cast<const uint4*>(s_acc + (ty + 1) * ST_AP + 4 + tx);
-      const unsigned g = (unsigned)gy * nx + gx;
+      const uint4 v = *reinterpret_cast<const uint4*>(facc + k * FRS * ST_AP);
+      *reinterpret_cast<uint4*>(facc + k * FRS * ST_AP) = make_uint4(0u, 0u, 0u, 0u);      // cleared for the next line
+      if (!(fxin && FRS * k < frows)) continue;
       float4 o;
       if (out_mode == 1) {
         o = make_float4((float)(int)v.x * sc, (float)(int)v.y * sc, (float)(int)v.z * sc, (float)(int)v.w * sc);
@@ -570,7 +590,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
         // point, 1.0 = 2^26, wraps at 64x): reported through the plan's flag word (epr_read_flags), never silently.
         // (The exact-remainder corner may be a few units NEGATIVE when a weight vanishes, so a pixel fed by such corners
         // alone legitimately reads −1 … −8 units: those are not overflows, hence the offset.)
-        if (((v.x + 1024u) | (v.y + 1024u) | (v.z + 1024u) | (v.w + 1024u)) & 0x80000000u) atomicOr(flags, EPR_FLAG_SPLAT_OVERFLOW);
+        if (min(min((int)v.x, (int)v.y), min((int)v.z, (int)v.w)) < -1024) atomicOr(flags, EPR_FLAG_SPLAT_OVERFLOW);
         // An EMPTY detector pixel (no source reaches it: the shadow side of a caustic) is written as exactly −f_s, so that
         // P_s = f_s + (P_s − f_s) is exactly 0 downstream and the split's decision "Σ_t P_t⁺ = 0 → w_s = f_s" (R8) is
         // taken on the integers, where an empty pixel is exactly empty — (float)(−Fi) alone would leave ±3e-8 there.
@@ -583,7 +603,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
           o = make_float4((dd.x - off) - o.x, (dd.y - off) - o.y, (dd.z - off) - o.z, (dd.w - off) - o.w);
         }
       }
-      *reinterpret_cast<float4*>(out + pl + g) = o;
+      *reinterpret_cast<float4*>(ol + k * fgs) = o;
     }
   }
   if (out_mode == 3) {
@@ -592,12 +612,12 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
     // P_s − f_s it stored above (same thread, same addresses: program order makes them visible; they are still in L2)
     // and overwrites them with e_s, so the N prediction planes never come back from HBM.
     const float off = 1.f + L.fsum_dev;
-    float* ob = out + (size_t)b * L.n_bins * plane;
-    for (int i = tid; i < ST_W * TH / 4; i += ST_NT) {
-      const int ty = i / (ST_W / 4), tx = 4 * (i - ty * (ST_W / 4));
-      const int gx = x0 + tx, gy = y0 + ty;
-      if (gx >= nx || gy >= ny) continue;
-      float* og = ob + (unsigned)gy * nx + gx;
+    float* ob = out + (size_t)b * L.n_bins * plane + fg0;
+    const float* dg = d + (size_t)b * plane + fg0;
+#pragma unroll 1
+    for (int k = 0; k < NFL; ++k) {
+      if (!(fxin && FRS * k < frows)) continue;
+      float* og = ob + k * fgs;
       float4 sum = make_float4(0.f, 0.f, 0.f, 0.f), den = sum;
       #pragma unroll 4                                  // four independent L2 loads in flight per thread (8: slower)
       for (int s = 0; s < L.n_bins; ++s) {
@@ -606,19 +626,21 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
         sum.x += pd.x; sum.y += pd.y; sum.z += pd.z; sum.w += pd.w;
         den.x += fmaxf(f + pd.x, 0.f); den.y += fmaxf(f + pd.y, 0.f); den.z += fmaxf(f + pd.z, 0.f); den.w += fmaxf(f + pd.w, 0.f);
       }
-      const float4 dd = __ldg(reinterpret_cast<const float4*>(d + (size_t)b * plane + (unsigned)gy * nx + gx));
+      const float4 dd = __ldg(reinterpret_cast<const float4*>(dg + k * fgs));
       const float4 e = make_float4((dd.x - off) - sum.x, (dd.y - off) - sum.y, (dd.z - off) - sum.z, (dd.w - off) - sum.w);
+      // e_s = P_s⁺ q + f_s fb:  q = e/Σ_t P_t⁺, fb = 0 where the sum is positive;  q = 0, fb = e (weights f_s) where it is not
       const float4 q = make_float4(den.x > 0.f ? e.x / den.x : 0.f, den.y > 0.f ? e.y / den.y : 0.f,
                                    den.z > 0.f ? e.z / den.z : 0.f, den.w > 0.f ? e.w / den.w : 0.f);
+      const float4 fb = make_float4(den.x > 0.f ? 0.f : e.x, den.y > 0.f ? 0.f : e.y, den.z > 0.f ? 0.f : e.z, den.w > 0.f ? 0.f : e.w);
       #pragma unroll 4
       for (int s = 0; s < L.n_bins; ++s) {
         const float4 pd = __ldcg(reinterpret_cast<const float4*>(og + (size_t)s * plane));
         const float f = L.f[s];
         float4 o;
-        o.x = den.x > 0.f ? fmaxf(f + pd.x, 0.f) * q.x : f * e.x;
-        o.y = den.y > 0.f ? fmaxf(f + pd.y, 0.f) * q.y : f * e.y;
-        o.z = den.z > 0.f ? fmaxf(f + pd.z, 0.f) * q.z : f * e.z;
-        o.w = den.w > 0.f ? fmaxf(f + pd.w, 0.f) * q.w : f * e.w;
+        o.x = fmaf(fmaxf(f + pd.x, 0.f), q.x, f * fb.x);
+        o.y = fmaf(fmaxf(f + pd.y, 0.f), q.y, f * fb.y);
+        o.z = fmaf(fmaxf(f + pd.z, 0.f), q.z, f * fb.z);
+        o.w = fmaf(fmaxf(f + pd.w, 0.f), q.w, f * fb.w);
         *reinterpret_cast<float4*>(og + (size_t)s * plane) = o;
       }
     }

@@ -24,6 +24,14 @@ __device__ __forceinline__ float epr_expm1_small(float x) {
   return fmaf(x * x, q, x);
 }
 
+// Taylor degree 5 for |x| < 0.09: truncation x^6/720, 1e-8 relative to x at the limit (below fp32 rounding)
+__device__ __forceinline__ float epr_expm1_tiny(float x) {
+  float q = fmaf(x, 8.33333333e-3f, 4.16666667e-2f);
+  q = fmaf(x, q, 1.66666667e-1f);
+  q = fmaf(x, q, 0.5f);
+  return fmaf(x * x, q, x);
+}
+
 // e^x by the MUFU exponential alone (ex2.approx.ftz, 2^-22 relative; no denormal rescue: callers' results saturate)
 __device__ __forceinline__ float epr_exp_fast(float x) {
   float y;
