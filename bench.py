@@ -45,6 +45,9 @@ def kernel_bytes_per_px(name, nb, solver):
         "k_output": 8,
         "k_resample": 8,                        # replaced per call by 4 + 4/m² (see main)
         "k_pred_out": 4 * nb + 4,
+        "k_update": 16,                         # general path: R two block-filtered planes (non-zero weights), R tau, W tau
+        "k_diagnostics": 4 * nb + 4,
+        "k_wkb1_sub": 4 + 8 * nb,
     }[name]
 
 
@@ -82,9 +85,12 @@ def measured_traffic(epr, kernel, nb, solver, config, algorithmic_bytes_per_laun
     return ratio * algorithmic_bytes_per_launch, f"{TRAFFIC_FILE} ({tab.get('command', 'ncu --set full')}; {tab.get('lib_version')})"
 
 
-def expected_launches_per_step(kernel, w, m):
+def expected_launches_per_step(kernel, w, m, blocks=0):
     """Launches of a kernel family in one epr_retrieve over a batch that fits the plan's work batch."""
     it = w.iterations
+    if blocks > 0:                                  # general path: block filters, splat = scatter + conversion
+        return {"k_rows_r2c": it + 1, "k_cols": (it + 1) * blocks, "k_rows_c2r": (it + 1) * blocks, "k_update": it + 1,
+                "k_splat": 2 * it, "k_resample": 2}.get(kernel, it)
     return {"k_rows_r2c": it + 1, "k_cols": it + 1, "k_rows_c2r": it + 1, "k_resample": 2}.get(kernel, it)
 
 
@@ -301,7 +307,17 @@ def run_reference(args, rank):
     }))
 
 
-def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, lines=0, m=1, cufft=False):
+def block_profiles(w, n_blocks):
+    """Synthetic x-dependent effective spectrum for `--blocks` (beam hardening stronger at the centre of a
+    cylindrical container): the weights tilt towards the high-energy lines and delta/beta rises by up to 10 % at the centre."""
+    t = 1.0 - np.abs(np.linspace(-1.0, 1.0, n_blocks))[:, None]            # 0 at the edges, 1 at the centre
+    e = (np.asarray(w.energy_keV, dtype=np.float64) - 100.0) / 40.0
+    wt = np.asarray(w.weight, dtype=np.float64)[None, :] * (1.0 + 0.4 * t * e[None, :])
+    db = np.asarray(w.delta_over_beta, dtype=np.float64)[None, :] * (1.0 + 0.1 * t)
+    return wt, db
+
+
+def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, lines=0, m=1, cufft=False, blocks=0):
     """Time one configuration: K steps of epr_retrieve over B resident projections (CUDA events on the launch stream),
     the same through epr_retrieve_host with pinned host buffers, and a profiling pass with the in-library per-kernel
     events.  Returns the pieces of the JSON line for this configuration (everything already reduced over ranks)."""
@@ -319,6 +335,8 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
     nb = w.n_bins
     plan = epr.epr_plan(m * w.nx, m * w.ny, w.pixel_m / m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
                         max_batch=B, max_shift_px=w.max_shift_px if m == 1 else fine_shift_clamp(w, m))
+    if blocks > 0:                                  # x-dependent effective spectrum (reading R17): the general path
+        epr.epr_plan_profiles(plan, *block_profiles(w, blocks))
     d_host = torch.from_numpy(w.d).pin_memory()
     out_host = torch.empty_like(d_host).pin_memory()
     d = d_host.cuda()
@@ -402,7 +420,9 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
         if kname == "k_resample":                # replication: R 4/m² + W 4; block mean: R 4 + W 4/m²; one launch each
             bpp = 4.0 + 4.0 / (m * m)
         # a batch larger than the plan's work batch goes through the loop in passes: launches cover B / passes projections
-        passes = max(1, round(launches_per_step / expected_launches_per_step(kname, w, m)))
+        passes = max(1, round(launches_per_step / expected_launches_per_step(kname, w, m, blocks)))
+        if blocks > 0 and kname == "k_rows_c2r":
+            bpp = 8                                 # general path: plain inverse transform (R spectrum, W q)
         px = px / passes
         avg_ms = tot_ms / cnt
         gbs = bpp * px / (avg_ms * 1e-3) / 1e9
@@ -423,7 +443,8 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
         "value": value, "unit": UNIT, "ms_per_step": ms / steps, "steps": steps, "warmup": warmup,
         "config": {"workload": f"{name}: {w.ny}x{w.nx}, {nb} line(s), {w.solver} solver, "
                                f"{w.iterations} iterations, step {w.step}"
-                               + (f", oversampling {m} (computational grid {m * w.ny}x{m * w.nx})" if m > 1 else ""),
+                               + (f", oversampling {m} (computational grid {m * w.ny}x{m * w.nx})" if m > 1 else "")
+                               + (f", x-dependent spectrum on {blocks} blocks (general path)" if blocks > 0 else ""),
                    "batch_per_gpu": B, "distinct_projections": min(distinct, B),
                    "l2": (f"inputs {in_bytes / 1e6:.0f} MB per step > 2 x 126 MB L2: no flush needed" if flush is None else
                           f"inputs {in_bytes / 1e6:.0f} MB per step: L2 flushed (256 MB overwrite) between timed steps"),
@@ -460,6 +481,8 @@ def main():
     ap.add_argument("--lines", type=int, default=0,
                     help="retrieve with this many spectral lines (60-140 keV, Gaussian weights) instead of the config's own "
                          "discretisation, e.g. --config C2 --lines 5: the paper's 'local L2 poly' rows (PAPER.md:116-119)")
+    ap.add_argument("--blocks", type=int, default=0,
+                    help="x-dependent effective spectrum on this many blocks (PAPER.md:431-441; epr_plan_profiles, general path)")
     ap.add_argument("--oversample", type=int, default=1,
                     help="run the loop on the grid refined this many times (PAPER.md:79; epr_retrieve_oversampled)")
     args = ap.parse_args()
@@ -486,7 +509,7 @@ def main():
     B = args.batch if args.batch > 0 else default_batch[args.config]
 
     head, w = measure_config(epr, args.config, B, args.steps, args.warmup, args.distinct, rank, world, local,
-                             lines=args.lines, m=args.oversample, cufft=not args.no_cufft_compare)
+                             lines=args.lines, m=args.oversample, cufft=not args.no_cufft_compare, blocks=args.blocks)
     result = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
               "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
               "vs_baseline": None, "dtype": "f32", "data": "synthetic"}
@@ -503,12 +526,14 @@ def main():
     # ---- the other BASELINE.json configurations, each measured the same way (same protocol, fewer steps), in the same
     # line: C3 (non-local, one line), C4 (non-local, 8 lines), C5 (2560 x 2160, 8 lines, batch 64 — more than the
     # plan's work batch holds, so the device call passes through HBM in sub-batches and the host call streams chunks)
-    default_run = (args.config == "C2" and args.lines == 0 and args.oversample == 1 and args.batch == 0)
+    default_run = (args.config == "C2" and args.lines == 0 and args.oversample == 1 and args.batch == 0 and args.blocks == 0)
     if default_run and not args.no_other_configs:
         other = {}
-        for name, ob, osteps in (("C3", 16, 3), ("C4", 8, 3), ("C5", 64, 2)):
+        # the splat's ring width and candidate list depend on the data: these batches hold more distinct projections
+        # (C5: 8 different rotation angles of the phantom) than the headline's local solver needs
+        for name, ob, osteps, odist in (("C3", 16, 3, 4), ("C4", 8, 3, 4), ("C5", 64, 2, 8)):
             try:
-                r, ow = measure_config(epr, name, ob, osteps, 3, args.distinct, rank, world, local)
+                r, ow = measure_config(epr, name, ob, osteps, 3, max(args.distinct, odist), rank, world, local)
                 if rank == 0 and not args.no_cpu_baseline:
                     r["cpu_baseline"] = oracle_sample(ow, host_procs(ow) if name == "C5" else 1)
                 del ow

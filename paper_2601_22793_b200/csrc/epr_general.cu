@@ -14,6 +14,13 @@
 
 #define GN_TX 32
 #define GN_TY 8
+// pointwise kernels: one thread = one pixel; x = blockIdx.x·256 + threadIdx.x, y = blockIdx.y, projection (or plane) = blockIdx.z
+// — the column (for the per-column tables) comes without a division
+#define GN_PIX(nx)                                                              \
+  const int x = blockIdx.x * 256 + threadIdx.x;                                 \
+  if (x >= (nx)) return;                                                        \
+  const size_t i = (size_t)blockIdx.y * (nx) + x;
+static inline dim3 gn_grid(const epr_plan_s* p, int nz) { return dim3((p->nx + 255) / 256, p->ny, nz); }
 
 // =====================================================================================================
 // a1-L  local O(L²) closure, Eq. (1) PAPER.md:146 (readings R1-R3), scalars of the CENTRE column (R17(b)):
@@ -42,16 +49,29 @@ __global__ void __launch_bounds__(GN_TX * GN_TY) k_gen_local(EprLines L, EprColu
 #pragma unroll
     for (int i = 0; i < 5; ++i) t[j][i] = s_t[threadIdx.y + j][threadIdx.x + i];
   const bool o2 = order == 2, wk = o2 && wkb1;
+  float tmax = 0.f;                                    // largest |τ| of the diamond: picks the series of expm1 per warp and line
+#pragma unroll
+  for (int j = 0; j < 5; ++j)
+#pragma unroll
+    for (int i = 0; i < 5; ++i)
+      if (abs(i - 2) + abs(j - 2) <= 2) tmax = fmaxf(tmax, fabsf(t[j][i]));
   for (int s = 0; s < L.n_bins; ++s) {
     const float gam = __ldg(&C.gamma[(size_t)s * nx + x]), a = __ldg(&C.a[(size_t)s * nx + x]), fs = __ldg(&C.f[(size_t)s * nx + x]);
     const float cg = -0.5f * gam, c2 = 0.5f * a * a * cg * cg, q4 = L.q4[s];
-    // Ad on the 13-point diamond |dx| + |dy| <= 2 (index [dy + 2][dx + 2])
+    // Ad on the 13-point diamond |dx| + |dy| <= 2 (index [dy + 2][dx + 2]): every neighbour seen through THIS column's γ, so
+    // nothing can be shared with the neighbouring threads; the series is as short as the warp's largest argument allows
     float A[5][5];
+    const float amax = fabsf(cg) * tmax;
+    const int tier = __any_sync(__activemask(), amax >= 0.35f) ? 2 : (__any_sync(__activemask(), amax >= 0.09f) ? 1 : 0);
+    auto fill = [&](auto fn) {
 #pragma unroll
-    for (int j = 0; j < 5; ++j)
+      for (int j = 0; j < 5; ++j)
 #pragma unroll
-      for (int i = 0; i < 5; ++i)
-        A[j][i] = (abs(i - 2) + abs(j - 2) <= 2) ? epr_expm1(cg * t[j][i]) : 0.f;
+        for (int i = 0; i < 5; ++i) A[j][i] = (abs(i - 2) + abs(j - 2) <= 2) ? fn(cg * t[j][i]) : 0.f;
+    };
+    if (tier == 0) fill([](float v) { return epr_expm1_tiny(v); });
+    else if (tier == 1) fill([](float v) { return epr_expm1_small(v); });
+    else fill([](float v) { return epr_expm1(v); });
     auto J = [&](int dy, int dx) { const float v = A[dy + 2][dx + 2]; return v * (2.f + v); };
     auto Ih = [&](int dy, int dx) { const float v = 1.f + A[dy + 2][dx + 2]; return v * v; };
     const float J0 = J(0, 0);
@@ -158,12 +178,10 @@ cudaError_t epr_gen_splat(const epr_plan_s* p, int batch, const float* tau, cons
 // −f_s(x), so that P_s = 0 exactly downstream: the split's fallback decision, R8); mode 1: P_s (epr_transport, signed).
 __global__ void __launch_bounds__(256) k_gen_fix2float(int n_bins, EprColumns C, int nx, size_t plane, int mode,
                                                        unsigned* __restrict__ acc, unsigned* __restrict__ flags) {
-  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
-  if (i >= plane) return;
-  const int x = (int)(i % (size_t)nx);
+  GN_PIX(nx)
   const float sc = 1.0f / (float)EPR_FIX_ONE;
   for (int s = 0; s < n_bins; ++s) {
-    unsigned* ap = acc + ((size_t)blockIdx.y * n_bins + s) * plane + i;
+    unsigned* ap = acc + ((size_t)blockIdx.z * n_bins + s) * plane + i;
     const unsigned v = *ap;
     float o;
     if (mode == 1) {
@@ -179,8 +197,7 @@ __global__ void __launch_bounds__(256) k_gen_fix2float(int n_bins, EprColumns C,
 
 cudaError_t epr_gen_fix2float(const epr_plan_s* p, int batch, unsigned* acc, int mode, cudaStream_t st) {
   const size_t plane = (size_t)p->nx * p->ny;
-  dim3 grid((unsigned)((plane + 255) / 256), batch);
-  k_gen_fix2float<<<grid, 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, mode, acc, p->d_flags);
+  k_gen_fix2float<<<gn_grid(p, batch), 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, mode, acc, p->d_flags);
   return cudaGetLastError();
 }
 
@@ -190,27 +207,27 @@ cudaError_t epr_gen_fix2float(const epr_plan_s* p, int batch, unsigned* acc, int
 // =====================================================================================================
 __global__ void __launch_bounds__(256) k_gen_residual(int n_bins, EprColumns C, int nx, size_t plane, const float* __restrict__ d,
                                                       const float* pred, float* es) {
-  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
-  if (i >= plane) return;
-  const int x = (int)(i % (size_t)nx), b = blockIdx.y;
+  GN_PIX(nx)
+  const int b = blockIdx.z;
   const size_t base = (size_t)b * n_bins * plane + i;
-  float pd[EPR_MAX_BINS], sum = 0.f, den = 0.f;
-  for (int s = 0; s < n_bins; ++s) {
-    pd[s] = pred[base + (size_t)s * plane];
-    sum += pd[s];
-    pd[s] = fmaxf(__ldg(&C.f[(size_t)s * nx + x]) + pd[s], 0.f);      // P_s⁺
-    den += pd[s];
+  float sum = 0.f, den = 0.f;
+  for (int s = 0; s < n_bins; ++s) {                    // two passes over the lines (the second hits L1/L2): no per-thread array
+    const float pd = pred[base + (size_t)s * plane];
+    sum += pd;
+    den += fmaxf(__ldg(&C.f[(size_t)s * nx + x]) + pd, 0.f);           // P_s⁺
   }
   const float e = (__ldg(&d[(size_t)b * plane + i]) - (1.f + __ldg(&C.fsum_dev[x]))) - sum;
   const float q = den > 0.f ? e / den : 0.f;
-  for (int s = 0; s < n_bins; ++s)
-    es[base + (size_t)s * plane] = den > 0.f ? pd[s] * q : __ldg(&C.f[(size_t)s * nx + x]) * e;
+  for (int s = 0; s < n_bins; ++s) {
+    const float f = __ldg(&C.f[(size_t)s * nx + x]);
+    const float pp = fmaxf(f + pred[base + (size_t)s * plane], 0.f);
+    es[base + (size_t)s * plane] = den > 0.f ? pp * q : f * e;
+  }
 }
 
 cudaError_t epr_gen_residual(const epr_plan_s* p, int batch, const float* d, const float* pred, float* es, cudaStream_t st) {
   const size_t plane = (size_t)p->nx * p->ny;
-  dim3 grid((unsigned)((plane + 255) / 256), batch);
-  k_gen_residual<<<grid, 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, d, pred, es);
+  k_gen_residual<<<gn_grid(p, batch), 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, d, pred, es);
   return cudaGetLastError();
 }
 
@@ -269,9 +286,8 @@ cudaError_t epr_gen_gather(const epr_plan_s* p, int batch, const float* tau, con
 __global__ void __launch_bounds__(256) k_gen_update(int n_bins, EprColumns C, int nx, size_t plane, int n_blocks,
                                                     const float* __restrict__ qblk, size_t blk_stride, float step,
                                                     int tau_is_zero, int newton_iters, float i_min, float* __restrict__ tau) {
-  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
-  if (i >= plane) return;
-  const int x = (int)(i % (size_t)nx), b = blockIdx.y;
+  GN_PIX(nx)
+  const int b = blockIdx.z;
   float q = 0.f;
   for (int k = 0; k < n_blocks; ++k) {
     const float w = __ldg(&C.wblk[(size_t)k * nx + x]);
@@ -298,33 +314,30 @@ __global__ void __launch_bounds__(256) k_gen_update(int n_bins, EprColumns C, in
 cudaError_t epr_gen_update(const epr_plan_s* p, int batch, const float* qblk, size_t blk_stride, float step, int tau_is_zero,
                            float* tau, cudaStream_t st) {
   const size_t plane = (size_t)p->nx * p->ny;
-  dim3 grid((unsigned)((plane + 255) / 256), batch);
-  k_gen_update<<<grid, 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, p->n_blocks, qblk, blk_stride, step, tau_is_zero,
+  k_gen_update<<<gn_grid(p, batch), 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, p->n_blocks, qblk, blk_stride, step, tau_is_zero,
                                       p->opt.newton_iters, p->opt.i_min, tau);
   return cudaGetLastError();
 }
 
 // out (+)= wblk[b][x] q over `planes` planes (epr_precondition with block filters)
-__global__ void __launch_bounds__(256) k_gen_blend(const float* __restrict__ w, int nx, size_t n, const float* __restrict__ q,
+__global__ void __launch_bounds__(256) k_gen_blend(const float* __restrict__ w, int nx, size_t plane, const float* __restrict__ q,
                                                    float* __restrict__ out, int accumulate) {
-  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
-  if (i >= n) return;
-  const float v = __ldg(&w[i % (size_t)nx]) * __ldg(&q[i]);
-  out[i] = accumulate ? out[i] + v : v;
+  GN_PIX(nx)
+  const size_t j = (size_t)blockIdx.z * plane + i;
+  const float v = __ldg(&w[x]) * __ldg(&q[j]);
+  out[j] = accumulate ? out[j] + v : v;
 }
 
 cudaError_t epr_gen_blend(const epr_plan_s* p, int planes, int b, const float* q, float* out, int accumulate, cudaStream_t st) {
-  const size_t n = (size_t)planes * p->nx * p->ny;
-  k_gen_blend<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p->cols.wblk + (size_t)b * p->nx, p->nx, n, q, out, accumulate);
+  k_gen_blend<<<gn_grid(p, planes), 256, 0, st>>>(p->cols.wblk + (size_t)b * p->nx, p->nx, (size_t)p->nx * p->ny, q, out, accumulate);
   return cudaGetLastError();
 }
 
 // epr_forward output: P_s = f_s(x) + (P_s − f_s), P = Σ_s P_s
 __global__ void __launch_bounds__(256) k_gen_pred_out(int n_bins, EprColumns C, int nx, size_t plane, const float* __restrict__ pred,
                                                       float* __restrict__ P_sum, float* __restrict__ P_bins) {
-  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
-  if (i >= plane) return;
-  const int x = (int)(i % (size_t)nx), b = blockIdx.y;
+  GN_PIX(nx)
+  const int b = blockIdx.z;
   const size_t base = (size_t)b * n_bins * plane + i;
   float sum = 0.f;
   for (int s = 0; s < n_bins; ++s) {
@@ -337,17 +350,16 @@ __global__ void __launch_bounds__(256) k_gen_pred_out(int n_bins, EprColumns C, 
 
 cudaError_t epr_gen_pred_out(const epr_plan_s* p, int batch, const float* pred, float* P_sum, float* P_bins, cudaStream_t st) {
   const size_t plane = (size_t)p->nx * p->ny;
-  dim3 grid((unsigned)((plane + 255) / 256), batch);
-  k_gen_pred_out<<<grid, 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, pred, P_sum, P_bins);
+  k_gen_pred_out<<<gn_grid(p, batch), 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, pred, P_sum, P_bins);
   return cudaGetLastError();
 }
 
 // output conversion with the column's scalars: τ | φ of line out_bin = −(db_s(x)/2) γ_s(x) τ (Eq. (6)) | Σ_s I_s (Eq. (7))
-__global__ void __launch_bounds__(256) k_gen_output(int n_bins, EprColumns C, int nx, size_t n, int mode, int bin, float inv_alpha,
-                                                    const float* __restrict__ tau, float* __restrict__ out) {
-  const size_t i = (size_t)blockIdx.x * 256 + threadIdx.x;
-  if (i >= n) return;
-  const int x = (int)(i % (size_t)nx);
+__global__ void __launch_bounds__(256) k_gen_output(int n_bins, EprColumns C, int nx, size_t plane, int mode, int bin, float inv_alpha,
+                                                    const float* __restrict__ tau_b, float* __restrict__ out_b) {
+  GN_PIX(nx)
+  const float* tau = tau_b + (size_t)blockIdx.z * plane;
+  float* out = out_b + (size_t)blockIdx.z * plane;
   const float t = tau[i];
   float v = t;
   if (mode == 1) v = -(__ldg(&C.a[(size_t)bin * nx + x]) * inv_alpha) * __ldg(&C.gamma[(size_t)bin * nx + x]) * t;   // db/2 = a/α
@@ -359,9 +371,9 @@ __global__ void __launch_bounds__(256) k_gen_output(int n_bins, EprColumns C, in
 }
 
 cudaError_t epr_gen_output(const epr_plan_s* p, int batch, const float* tau, float* out, cudaStream_t st) {
-  const size_t n = (size_t)p->nx * p->ny * batch;
+  const size_t n = (size_t)p->nx * p->ny;
   const int sb = p->opt.out_bin;
-  k_gen_output<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(p->n_bins, p->cols, p->nx, n, p->opt.output, sb,
+  k_gen_output<<<gn_grid(p, batch), 256, 0, st>>>(p->n_bins, p->cols, p->nx, n, p->opt.output, sb,
                                                              (float)(1.0 / p->h_alpha[sb]), tau, out);
   return cudaGetLastError();
 }
