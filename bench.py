@@ -90,7 +90,7 @@ def expected_launches_per_step(kernel, w, m, blocks=0):
     it = w.iterations
     if blocks > 0:                                  # general path: block filters, splat = scatter + conversion
         return {"k_rows_r2c": it + 1, "k_cols": (it + 1) * blocks, "k_rows_c2r": (it + 1) * blocks, "k_update": it + 1,
-                "k_splat": 2 * it, "k_resample": 2}.get(kernel, it)
+                "k_splat": it if (w.nx % 16 == 0 and w.ny % 16 == 0) else 2 * it, "k_resample": 2}.get(kernel, it)
     return {"k_rows_r2c": it + 1, "k_cols": it + 1, "k_rows_c2r": it + 1, "k_resample": 2}.get(kernel, it)
 
 

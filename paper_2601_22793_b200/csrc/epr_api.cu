@@ -52,7 +52,7 @@ struct EprProf {
   } while (0)
 
 static cudaError_t gen_r2c(epr_plan_t p, int planes, const float* in, float off, cudaStream_t cs);
-static cudaError_t gen_cols(epr_plan_t p, int planes, int mode, int blk, float2* out, cudaStream_t cs);
+static cudaError_t gen_cols(epr_plan_t p, int planes, int mode, int blk, float2* out, cudaStream_t cs, int stage);
 static cudaError_t gen_c2r(epr_plan_t p, int planes, const float2* spec, float* q, cudaStream_t cs);
 
 // Every entry point runs on the plan's device (function attributes, workspaces and streams belong to it) and restores
@@ -202,6 +202,14 @@ static epr_status set_columns(epr_plan_s* p, int n_blocks, const double* f_blk, 
   p->cols.f = base; p->cols.gamma = base + n1; p->cols.a = base + 2 * n1; p->cols.fixCorr = base + 3 * n1;
   p->cols.fixFi = reinterpret_cast<const unsigned*>(base + 4 * n1);
   p->cols.fsum_dev = base + 5 * n1; p->cols.wblk = base + 5 * n1 + nx;
+  // bounds for the tuned non-local kernels (ring width, staged halo, clamp test): the largest a_s(x) γ_s(x) of every line
+  p->lines_bound = p->lines;
+  for (int s = 0; s < nb; ++s) {
+    float m = 0.f;
+    for (int x = 0; x < nx; ++x) m = fmaxf(m, da[(size_t)s * nx + x] * dg[(size_t)s * nx + x]);
+    p->lines_bound.a[s] = m * 1.000001f;               // (the kernels form a·γ in fp32 from the two table entries)
+    p->lines_bound.gamma[s] = 1.f;
+  }
   for (int b = 0; b < n_blocks; ++b) {
     double abar = 0;
     for (int s = 0; s < nb; ++s) {
@@ -594,7 +602,7 @@ extern "C" epr_status epr_precondition(epr_plan_t p, int batch, const float* r_b
       // so several blocks accumulate in a workspace first
       for (int b = 0; b < p->n_blocks; ++b) {
         KL(p, K_ROWS_R2C, cs, gen_r2c(p, planes, r_bins + off, 0.f, cs));
-        KL(p, K_COLS, cs, gen_cols(p, planes, 0, b, p->spec, cs));
+        KL(p, K_COLS, cs, gen_cols(p, planes, 0, b, p->spec, cs, 0));
         if (p->n_blocks == 1) { KL(p, K_ROWS_C2R, cs, gen_c2r(p, planes, p->spec, q_bins + off, cs)); break; }
         KL(p, K_ROWS_C2R, cs, gen_c2r(p, planes, p->spec, p->pred, cs));
         KL(p, K_UPDATE, cs, epr_gen_blend(p, planes, b, p->pred, p->res, b > 0, cs));
@@ -615,11 +623,17 @@ extern "C" epr_status epr_precondition(epr_plan_t p, int batch, const float* r_b
 static cudaError_t gen_r2c(epr_plan_t p, int planes, const float* in, float off, cudaStream_t cs) {
   return p->fft_generic ? epr_fftgen_rows_r2c(p, planes, in, off, p->spec, cs) : epr_launch_rows_r2c(p, planes, in, off, p->spec, cs);
 }
-static cudaError_t gen_cols(epr_plan_t p, int planes, int mode, int blk, float2* out, cudaStream_t cs) {
+static cudaError_t gen_cols(epr_plan_t p, int planes, int mode, int blk, float2* out, cudaStream_t cs, int stage) {
   EprLines lb = p->lines;
   for (int s = 0; s < p->n_bins; ++s) lb.a[s] = p->a_blk[blk][s];
   lb.abar = p->abar_blk[blk];
-  return p->fft_generic ? epr_fftgen_cols(p, planes, mode, p->spec, out, cs, &lb) : epr_launch_cols(p, planes, mode, p->spec, out, cs, &lb);
+  return p->fft_generic ? epr_fftgen_cols(p, planes, mode, p->spec, out, cs, &lb) : epr_launch_cols(p, planes, mode, p->spec, out, cs, &lb, stage);
+}
+// Several block filters on the same residuals: transform the columns once, then filter + sum + inverse per block
+// (the TMA column kernel's stages; power-of-two ny in 256 … 2048 on grids with TMA descriptors).
+static bool cols_staged(epr_plan_t p) {
+  const int ny = p->ny;
+  return p->n_blocks > 1 && !p->fft_generic && p->tma_ok && ny >= 256 && ny <= 2048 && (ny & (ny - 1)) == 0 && (p->nx / 2) % 4 == 0;
 }
 static cudaError_t gen_c2r(epr_plan_t p, int planes, const float2* spec, float* q, cudaStream_t cs) {
   return p->fft_generic ? epr_fftgen_rows_c2r(p, planes, spec, q, cs) : epr_launch_rows_c2r(p, planes, spec, 0, 1.f, 0, q, cs);
@@ -634,8 +648,10 @@ static epr_status retrieve_chunk_general(epr_plan_t p, int nb, const float* d, f
   if (p->opt.init == 0) {
     // initial guess (R9, R17(c)): T⁰ − 1 = Σ_b wblk[b][x] IFFT(FFT(d − 1)/(1 + ā^{(b)} λ)), floored, projected
     KL(p, K_ROWS_R2C, cs, gen_r2c(p, nb, d, -1.f, cs));
+    const int st2 = cols_staged(p) ? 2 : 0;
+    if (st2) KL(p, K_COLS, cs, gen_cols(p, nb, 0, 0, p->spec, cs, 1));                          // columns transformed once
     for (int b = 0; b < p->n_blocks; ++b) {
-      KL(p, K_COLS, cs, gen_cols(p, nb, 2, b, p->spec_sum, cs));
+      KL(p, K_COLS, cs, gen_cols(p, nb, 2, b, p->spec_sum, cs, st2));
       KL(p, K_ROWS_C2R, cs, gen_c2r(p, nb, p->spec_sum, p->qblk + b * bstride, cs));
     }
     KL(p, K_UPDATE, cs, epr_gen_update(p, nb, p->qblk, bstride, 1.f, 1, tau, cs));
@@ -646,6 +662,11 @@ static epr_status retrieve_chunk_general(epr_plan_t p, int nb, const float* d, f
       KL(p, K_FWD_LOCAL, cs, epr_gen_forward_local(p, nb, tau, p->pred, cs));                   // a0 + a1-L
       KL(p, K_RESIDUAL, cs, epr_gen_residual(p, nb, d, p->pred, p->res, cs));                   // a2 (a3 = identity)
       r = p->res;
+    } else if (p->nx % 16 == 0 && p->ny % 16 == 0) {
+      // 16-pixel-aligned grid: the tuned tile kernels, reading the per-column tables (a0 + a1-N + a2 fused, then a3)
+      KL(p, K_SPLAT, cs, epr_launch_splat_cols(p, nb, tau, p->res, p->n_bins == 1 ? 2 : 3, d, cs));
+      KL(p, K_GATHER, cs, epr_launch_gather_cols(p, nb, tau, p->res, p->res2, cs));
+      r = p->res2;
     } else {
       KL(p, K_SPLAT, cs, epr_gen_splat(p, nb, tau, NULL, NULL, NULL, (unsigned*)p->res, cs));   // a0 + a1-N
       KL(p, K_SPLAT, cs, epr_gen_fix2float(p, nb, (unsigned*)p->res, 0, cs));
@@ -654,8 +675,10 @@ static epr_status retrieve_chunk_general(epr_plan_t p, int nb, const float* d, f
       r = p->res2;
     }
     KL(p, K_ROWS_R2C, cs, gen_r2c(p, planes, r, 0.f, cs));                                      // a4
+    const int st2 = cols_staged(p) ? 2 : 0;
+    if (st2) KL(p, K_COLS, cs, gen_cols(p, planes, 0, 0, p->spec, cs, 1));                      // columns transformed once
     for (int b = 0; b < p->n_blocks; ++b) {
-      KL(p, K_COLS, cs, gen_cols(p, planes, 1, b, p->spec_sum, cs));                            // Σ_s in Fourier space (R10), block b
+      KL(p, K_COLS, cs, gen_cols(p, planes, 1, b, p->spec_sum, cs, st2));                       // Σ_s in Fourier space (R10), block b
       KL(p, K_ROWS_C2R, cs, gen_c2r(p, nb, p->spec_sum, p->qblk + b * bstride, cs));
     }
     KL(p, K_UPDATE, cs, epr_gen_update(p, nb, p->qblk, bstride, step, 0, tau, cs));             // a5 + a6

@@ -12,7 +12,7 @@
   int epr_fftg_has_##g(int n);                                                                                        \
   cudaError_t epr_fftg_rows_r2c_##g(const epr_plan_s*, int, const float*, float, float2*, cudaStream_t);               \
   cudaError_t epr_fftg_rows_c2r_##g(const epr_plan_s*, int, const float2*, int, float, int, float*, cudaStream_t);     \
-  cudaError_t epr_fftg_cols_##g(const epr_plan_s*, int, int, const float2*, float2*, cudaStream_t, const EprLines*);
+  cudaError_t epr_fftg_cols_##g(const epr_plan_s*, int, int, const float2*, float2*, cudaStream_t, const EprLines*, int);
 EPR_FFT_GROUPS(G)
 #undef G
 
@@ -40,8 +40,8 @@ cudaError_t epr_launch_rows_c2r(const epr_plan_s* p, int planes, const float2* s
 }
 
 cudaError_t epr_launch_cols(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st,
-                            const EprLines* lines_override) {
-#define G(g) if (epr_fftg_has_##g(p->ny)) return epr_fftg_cols_##g(p, planes, mode, spec, out, st, lines_override);
+                            const EprLines* lines_override, int stage) {
+#define G(g) if (epr_fftg_has_##g(p->ny)) return epr_fftg_cols_##g(p, planes, mode, spec, out, st, lines_override, stage);
   EPR_FFT_GROUPS(G)
 #undef G
   return cudaErrorInvalidValue;

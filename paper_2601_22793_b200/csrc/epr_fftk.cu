@@ -379,19 +379,24 @@ template <int N> struct ColTmaCfg {
   static constexpr size_t TILE = (size_t)N * W * sizeof(float2);
   // SUM (several lines per output tile): two tiles, so that the load of line s+1 overlaps the transform of line s
   static constexpr size_t smem(bool sum) { return (sum ? 2 : 1) * TILE + 16; }   // + two mbarriers
+  static constexpr size_t smem3() { return 3 * TILE + 32; }
 };
 
-template <int N, bool SUM>
+// NBUF tile buffers: 1 (one line per output tile), 2 (several lines: the load of line s + 1 under the transform of line s), 3 (stage 2
+// of the block filters: no transform per line, so the loads are the whole cost and two of them are kept in flight)
+template <int N, bool SUM, int NBUF = (SUM ? 2 : 1)>
 __global__ void __launch_bounds__(ColTmaCfg<N>::NT, (SUM || ColTmaCfg<N>::NT > 512) ? 1 : 2)
 k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_out, EprLines L, int M,
            int mode, float scale, const float* __restrict__ lam_x, const float* __restrict__ lam_y,
-           const float2* __restrict__ tw, const float2* __restrict__ tw_inv) {
+           const float2* __restrict__ tw, const float2* __restrict__ tw_inv, int stage) {
+  // stage 0: the whole operator.  Block filters of an x-dependent spectrum (R17(c)) apply several filters to the same
+  // residuals, so the forward transform is done once — stage 1: out[plane] = FFT_y(spec[plane]), stored in frequency order —
+  // and every block then runs stage 2: the input tiles are already transformed (filter, Σ_s, inverse only).
   using C = ColTmaCfg<N>;
   using EF = EngineSw<N, C::TPC, false, false>;
   using EI = EngineSw<N, C::TPC, true, true>;
   static_assert(EF::RL == EI::R0 && EF::GL::CNT == EI::G0::CNT && EF::PL == EI::G0::T, "schedules must mirror");
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  constexpr int NBUF = SUM ? 2 : 1;
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + NBUF * C::TILE);
   const int c = threadIdx.x % C::W, t = threadIdx.x / C::W;
   const int kx0 = blockIdx.x * C::W, kx = kx0 + c;
@@ -399,7 +404,10 @@ k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
   const int nb = L.n_bins;
   const int nloop = SUM ? nb : 1;
   const float lx = __ldg(&lam_x[kx]);
-  if (threadIdx.x == 0) { eprtma::mbar_init(&bar[0], 1); eprtma::mbar_init(&bar[1], 1); eprtma::mbar_fence_init(); }
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < (NBUF < 2 ? 2 : NBUF); ++i) eprtma::mbar_init(&bar[i], 1);
+    eprtma::mbar_fence_init();
+  }
   __syncthreads();
   auto load_tile = [&](int sl) {            // one thread: request line sl of this output tile into buffer sl % NBUF
     const int iplane = (mode == 1) ? oplane * nb + sl : oplane;
@@ -410,7 +418,8 @@ k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
     for (int bx = 0; bx < N / C::BOX; ++bx)
       eprtma::tensor_g2s_2d(dst + bx * C::BOX * C::W, &map_in, 2 * kx0, iplane * N + bx * C::BOX, &bar[sl % NBUF]);
   };
-  if (threadIdx.x == 0) load_tile(0);
+  if (threadIdx.x == 0)
+    for (int i = 0; i < (NBUF > 1 ? NBUF - 1 : 1) && i < nloop; ++i) load_tile(i);
   float2 acc[EF::GL::CNT][EF::RL];
   if (SUM) {
 #pragma unroll
@@ -421,25 +430,51 @@ k_cols_tma(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ C
   for (int sl = 0; sl < nloop; ++sl) {
     const float a = (mode == 2) ? L.abar : L.a[(mode == 1) ? sl : (oplane % nb)];
     float2* sm = reinterpret_cast<float2*>(smem_raw + (sl % NBUF) * C::TILE);
-    // the other buffer was last read during line sl − 1, which every thread left through the barrier closing it
-    if (SUM && threadIdx.x == 0 && sl + 1 < nloop) load_tile(sl + 1);
+    // buffer (sl − 1) % NBUF was last read during line sl − 1, which every thread left through the barrier closing it
+    if (SUM && threadIdx.x == 0 && sl + NBUF - 1 < nloop) load_tile(sl + NBUF - 1);
     eprtma::mbar_wait(&bar[sl % NBUF], (sl / NBUF) & 1);
     float2 u0[EF::G0::CNT][EF::R0], uL[EF::GL::CNT][EF::RL];
+    if (stage != 2) {
 #pragma unroll
-    for (int cc = 0; cc < EF::G0::CNT; ++cc)
+      for (int cc = 0; cc < EF::G0::CNT; ++cc)
 #pragma unroll
-      for (int r = 0; r < EF::R0; ++r) u0[cc][r] = sm[(t + cc * C::TPC + r * EF::G0::T) * C::W + c];   // LINEAR tile
-    __syncthreads();                       // every thread has its inputs: the tile may be overwritten in place
-    EF::run(u0, uL, sm, c, t, tw);
-    if (blockIdx.x == 0) {
-      // tile 0 holds the packed column kx = 0: C = F0 + i FM (both Hermitian in ky).  With A = ½(C[ky] + C*[−ky]),
-      // B = −(i/2)(C[ky] − C*[−ky]):  C'[ky] = H(0,ky) A + i H(M,ky) B,  C'[−ky] = H(0,ky) A* + i H(M,ky) B*.
+        for (int r = 0; r < EF::R0; ++r) u0[cc][r] = sm[(t + cc * C::TPC + r * EF::G0::T) * C::W + c];   // LINEAR tile
+      __syncthreads();                     // every thread has its inputs: the tile may be overwritten in place
+      EF::run(u0, uL, sm, c, t, tw);
+    } else {                               // the tile holds the transformed column in frequency order
+#pragma unroll
+      for (int cc = 0; cc < EF::GL::CNT; ++cc)
+#pragma unroll
+        for (int q = 0; q < EF::RL; ++q) uL[cc][q] = sm[(t + cc * C::TPC + q * EF::PL) * C::W + c];
+    }
+    if (stage == 1) {                      // forward only: frequency order back into the tile, TMA store, done (SUM is false)
       __syncthreads();
 #pragma unroll
       for (int cc = 0; cc < EF::GL::CNT; ++cc)
 #pragma unroll
         for (int q = 0; q < EF::RL; ++q) sm[(t + cc * C::TPC + q * EF::PL) * C::W + c] = uL[cc][q];
+      eprtma::fence_proxy_async();
       __syncthreads();
+      if (threadIdx.x == 0) {
+#pragma unroll
+        for (int bx = 0; bx < N / C::BOX; ++bx)
+          eprtma::tensor_s2g_2d(&map_out, 2 * kx0, oplane * N + bx * C::BOX, sm + bx * C::BOX * C::W);
+        eprtma::bulk_commit();
+        eprtma::bulk_wait<0>();
+      }
+      return;
+    }
+    if (blockIdx.x == 0) {
+      // tile 0 holds the packed column kx = 0: C = F0 + i FM (both Hermitian in ky).  With A = ½(C[ky] + C*[−ky]),
+      // B = −(i/2)(C[ky] − C*[−ky]):  C'[ky] = H(0,ky) A + i H(M,ky) B,  C'[−ky] = H(0,ky) A* + i H(M,ky) B*.
+      __syncthreads();
+      if (stage != 2) {
+#pragma unroll
+        for (int cc = 0; cc < EF::GL::CNT; ++cc)
+#pragma unroll
+          for (int q = 0; q < EF::RL; ++q) sm[(t + cc * C::TPC + q * EF::PL) * C::W + c] = uL[cc][q];
+        __syncthreads();
+      }
       if (c == 0) {
         const float lxN = __ldg(&lam_x[M]);
         for (int ky = t; ky <= N / 2; ky += C::TPC) {
@@ -867,7 +902,7 @@ cudaError_t GFN(epr_fftg_rows_c2r_)(const epr_plan_s* p, int planes, const float
 
 template <int N>
 static bool launch_cols_tma(const epr_plan_s* p, const EprLines& LL, int oplanes, int mode, const float2* spec, float2* out,
-                            float scale, cudaStream_t st) {
+                            float scale, cudaStream_t st, int stage) {
   if constexpr (N >= 256 && (N & (N - 1)) == 0) {
     using C = ColTmaCfg<N>;
     const int M = p->nx / 2;
@@ -888,7 +923,7 @@ static bool launch_cols_tma(const epr_plan_s* p, const EprLines& LL, int oplanes
       if (two < 0) { const char* e = getenv("EPR_COLS2"); two = e ? atoi(e) : 1; }
       const int sms = p->sms;
       const int ntiles = (M / C::W) * oplanes;
-      if (two && !(mode == 1 && p->n_bins > 1) && ntiles >= 8 * sms) {
+      if (two && stage == 0 && !(mode == 1 && p->n_bins > 1) && ntiles >= 8 * sms) {
         constexpr size_t smem2 = 3 * C::TILE + 32;
         static EprPerDevice attr2 = {};
         if (!attr2.at(p)) { cudaFuncSetAttribute(k_cols_tma2<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2); attr2.at(p) = 1; }
@@ -896,12 +931,17 @@ static bool launch_cols_tma(const epr_plan_s* p, const EprLines& LL, int oplanes
         return true;
       }
     }
-    if (mode == 1 && p->n_bins > 1)
-      k_cols_tma<N, true><<<grid, C::NT, C::smem(true), st>>>(p->map_spec, mo, LL, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+    if (mode == 1 && p->n_bins > 1 && stage == 2 && C::smem3() <= 227 * 1024) {
+      static EprPerDevice attr3 = {};
+      if (!attr3.at(p)) { cudaFuncSetAttribute(k_cols_tma<N, true, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem3()); attr3.at(p) = 1; }
+      k_cols_tma<N, true, 3><<<grid, C::NT, C::smem3(), st>>>(p->map_spec, mo, LL, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv, stage);
+    } else if (mode == 1 && p->n_bins > 1)
+      k_cols_tma<N, true><<<grid, C::NT, C::smem(true), st>>>(p->map_spec, mo, LL, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv, stage);
     else
-      k_cols_tma<N, false><<<grid, C::NT, C::smem(false), st>>>(p->map_spec, mo, LL, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv);
+      k_cols_tma<N, false><<<grid, C::NT, C::smem(false), st>>>(p->map_spec, mo, LL, M, mode, scale, p->lam_x, p->lam_y, p->tw_col, p->tw_col_inv, stage);
     return true;
   } else if constexpr (N >= 256) {
+    if (stage != 0) return false;
     using C = ColCfg<N>;
     using P = ColTmaPadCfg<N>;
     const int M = p->nx / 2;
@@ -929,7 +969,7 @@ static bool launch_cols_tma(const epr_plan_s* p, const EprLines& LL, int oplanes
 }
 
 cudaError_t GFN(epr_fftg_cols_)(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st,
-                                const EprLines* lines_override) {
+                                const EprLines* lines_override, int stage) {
   const EprLines& LL = lines_override ? *lines_override : p->lines;     // block filters pass their own a[] / abar
   const int M = p->nx / 2;
   const int oplanes = (mode == 1) ? planes / p->n_bins : planes;
@@ -938,7 +978,8 @@ cudaError_t GFN(epr_fftg_cols_)(const epr_plan_s* p, int planes, int mode, const
 #define X(n_)                                                                                                   \
   case n_: {                                                                                                    \
     using C = ColCfg<n_>;                                                                                       \
-    if (launch_cols_tma<n_>(p, LL, oplanes, mode, spec, out, scale, st)) break;                                     \
+    if (launch_cols_tma<n_>(p, LL, oplanes, mode, spec, out, scale, st, stage)) break;                              \
+    if (stage != 0) return cudaErrorNotSupported;           /* staged block filters: TMA column kernel only */     \
     static EprPerDevice attr = {};                                                                              \
     if (!attr.at(p)) {                                                                                          \
       cudaFuncSetAttribute(k_cols<n_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);       \

@@ -300,13 +300,37 @@ __global__ void __launch_bounds__(256) k_gen_update(int n_bins, EprColumns C, in
     const float g = __ldg(&C.gamma[x]);                 // one line: f = 1; δ = −log1p(ΔT e^{γτ})/γ in closed form
     delta = epr_project_increment_mono(g * t, step * q, i_min) / g;
   } else {
-    float f[EPR_MAX_BINS], g[EPR_MAX_BINS], gmax = 0.f;
+    // converging iterations (|γ_max δ| < 0.01): the moments G_k = Σ_s I_s γ_s^k of the column's lines once, the cubic of
+    // F(δ) = Σ_s I_s expm1(−γ_s δ) − ΔT solved without a loop (series reversion + one Newton step) — the arithmetic of
+    // epr_project_increment_small (epr_math.cuh) with run-time line count and per-column scalars
+    const float dT = step * q;
+    float G0 = 0.f, G1 = 0.f, G2 = 0.f, G3 = 0.f, gmax = 0.f;
+#pragma unroll 4
     for (int s = 0; s < n_bins; ++s) {
-      f[s] = __ldg(&C.f[(size_t)s * nx + x]);
-      g[s] = __ldg(&C.gamma[(size_t)s * nx + x]);
-      gmax = fmaxf(gmax, g[s]);
+      const float g = __ldg(&C.gamma[(size_t)s * nx + x]);
+      const float pI = __ldg(&C.f[(size_t)s * nx + x]) * epr_exp_fast(-g * t);
+      gmax = fmaxf(gmax, g);
+      G0 += pI;
+      float pg = pI * g; G1 += pg;
+      pg *= g; G2 += pg;
+      G3 = fmaf(pg, g, G3);
     }
-    delta = epr_project_increment(t, step * q, f, g, n_bins, gmax, newton_iters, i_min);
+    const float rc1 = -__fdividef(1.f, G1);
+    delta = dT * rc1;
+    if (fabsf(delta) * gmax < 0.01f && G0 + dT >= i_min && newton_iters > 0) {
+      const float c1 = -G1, c2 = 0.5f * G2, c3 = -1.66666667e-1f * G3;
+      delta = fmaf(-(c2 * rc1) * delta, delta, delta);
+      const float F = fmaf(fmaf(fmaf(c3, delta, c2), delta, c1), delta, -dT);
+      const float dF = fmaf(fmaf(3.f * c3, delta, 2.f * c2), delta, c1);
+      delta -= __fdividef(F, dF);
+    } else {
+      float f[EPR_MAX_BINS], g[EPR_MAX_BINS];
+      for (int s = 0; s < n_bins; ++s) {
+        f[s] = __ldg(&C.f[(size_t)s * nx + x]);
+        g[s] = __ldg(&C.gamma[(size_t)s * nx + x]);
+      }
+      delta = epr_project_increment(t, dT, f, g, n_bins, gmax, newton_iters, i_min);
+    }
   }
   *tp = t + delta;
 }

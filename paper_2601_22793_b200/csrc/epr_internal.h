@@ -100,6 +100,7 @@ struct epr_plan_s {
   int fft_generic;             // 1: run-time-radix FFT (size not in the tuned table); spectra are [ny][nx/2 + 1] then
   int n_blocks;                // blocks of the x-dependent spectrum (1 = uniform)
   EprColumns cols;             // device tables (owned by the plan: cols_store)
+  EprLines lines_bound;        // `lines` with a[s] = max_x a_s(x) γ_s(x), gamma[s] = 1: bounds for the tuned kernels' ring / halo / clamp tests
   void* cols_store;            // one allocation behind `cols`
   double* h_col;               // host copy [3][n_bins][nx]: f, γ, a per column (epr_plan_columns)
   float a_blk[EPR_MAX_BLOCKS][EPR_MAX_BINS];   // a_s of block b
@@ -149,8 +150,11 @@ cudaError_t epr_launch_rows_r2c(const epr_plan_s* p, int planes, const float* in
 // mode 0: per-plane filter with bin = plane % n_bins (out has `planes` planes);
 // mode 1: sum over bins (out has planes / n_bins planes);  mode 2: single filter with abar (init).
 // lines_override != NULL: the per-line filter coefficients a[] / abar are taken from it instead of p->lines (block filters)
+// stage 0: whole operator; 1: forward column transform only (out[plane] = FFT_y(spec[plane]), frequency order, mode 0);
+// 2: the input planes are already column-transformed (filter, Σ_s, inverse) — TMA column kernel only (power-of-two ny in
+// 256 … 2048 with TMA descriptors), cudaErrorNotSupported otherwise
 cudaError_t epr_launch_cols(const epr_plan_s* p, int planes, int mode, const float2* spec, float2* out, cudaStream_t st,
-                            const EprLines* lines_override = nullptr);
+                            const EprLines* lines_override = nullptr, int stage = 0);
 // epilogue 0: write q; 1: τ update (Newton projection) with step; init0: treat τ as 0 (initial guess)
 cudaError_t epr_launch_rows_c2r(const epr_plan_s* p, int planes, const float2* spec, int epilogue, float step,
                                 int tau_is_zero, float* q_or_tau, cudaStream_t st);
@@ -195,3 +199,7 @@ cudaError_t epr_fftgen_rows_c2r(const epr_plan_s* p, int planes, const float2* s
 // per-line histogram of the unclamped shift norm (Fig. 6); hist [batch][n_bins][n_hist], zeroed by the launcher
 cudaError_t epr_launch_shift_hist(const epr_plan_s* p, int batch, const float* tau, int n_hist, float bin_px, unsigned* hist,
                                   cudaStream_t st);
+// tuned splat / gather of the loop with per-column tables (general path on 16-pixel-aligned grids)
+cudaError_t epr_launch_splat_cols(const epr_plan_s* p, int batch, const float* tau, float* out, int out_mode, const float* d,
+                                  cudaStream_t st);
+cudaError_t epr_launch_gather_cols(const epr_plan_s* p, int batch, const float* tau, const float* es, float* r, cudaStream_t st);

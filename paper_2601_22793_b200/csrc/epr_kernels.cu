@@ -326,8 +326,11 @@ cudaError_t epr_launch_grad_blockmax(const epr_plan_s* p, int batch, const float
 // FROM_TAU: sources and ray map from the τ tile staged in shared memory (the loop's configuration);
 // otherwise (epr_transport) both are read from global planes.
 // ST_NT threads per CTA: 512 when two CTAs fit an SM, 1024 when the halo (large S) leaves room for one only
-template <bool FROM_TAU, bool MAP_OUT, int ST_NT, int TH>
-__global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny, float S, int H,
+// COLS: x-dependent effective spectrum (reading R17): the per-line scalars of a SOURCE come from its own column's tables C
+// (mass f_s(x), γ_s(x), shift coefficient a_s(x)γ_s(x)), the baseline / split fractions of a DETECTOR pixel from its column;
+// L then only carries bounds (a[s]·gamma[s] = max over columns of a_s(x)γ_s(x)) for the ring width and the clamp test.
+template <bool FROM_TAU, bool MAP_OUT, int ST_NT, int TH, bool COLS = false>
+__global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, EprColumns C, int nx, int ny, float S, int H,
                                                     const float* __restrict__ tau, const float* __restrict__ I_bins,
                                                     const float2* __restrict__ map_in, float2* __restrict__ map_out,
                                                     float* __restrict__ out, int out_mode, const float* __restrict__ d,
@@ -462,6 +465,15 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       // The clamp of u is skipped when |c_s| · max|D⁰τ| over the tile cannot exceed S.
       constexpr int RG = NW / 4, ROWS = TH / RG;
       const int x = (warp & 3) * 32 + lane, yb = (warp >> 2) * ROWS;
+      float csx = cs, gamx = gam, fixFfx = fixFf;      // scalars of THIS thread's source column
+      int Fix = Fi;
+      if (COLS) {
+        const size_t ci = (size_t)s * nx + wrapm(x0 + x, nx);
+        gamx = __ldg(&C.gamma[ci]);
+        csx = -0.5f * __ldg(&C.a[ci]) * gamx;
+        fixFfx = __ldg(&C.f[ci]) * 67108864.f;
+        Fix = (int)__ldg(&C.fixFi[ci]);
+      }
       const unsigned TP4 = 4u * TP;
       const unsigned rb0 = (unsigned)__cvta_generic_to_shared(s_tau) + 4u * (unsigned)((yb + H + 1) * TP + x + Ha);
       const unsigned ab0 = (unsigned)__cvta_generic_to_shared(s_acc) + 4u * (unsigned)((yb + 1) * ST_AP + x + 4);
@@ -475,7 +487,7 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
           rb += TP4;                                   // one row beyond the strip at the last r: still inside the τ tile
           const float ts2 = lds_f32(rb + TP4), tl2 = lds_f32(rb - 4), tr2 = lds_f32(rb + 4);
           const float gx = tr - tl, gy = ts - tn;
-          float ux = cs * gx, uy = cs * gy;
+          float ux = csx * gx, uy = csx * gy;
           if (CLAMP) { ux = fminf(fmaxf(ux, -S), S); uy = fminf(fmaxf(uy, -S), S); }
           if (MAP_OUT) {
             if (x0 + x < nx && y0 + yb + r < ny) *mo = make_float2(ux, uy);
@@ -483,10 +495,10 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
           }
           const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
           const float dx = ux - (float)fx, dy = uy - (float)fy;
-          const float xe = -gam * tc;
+          const float xe = -gamx * tc;
           float J = epr_expm1_small(xe);               // MUFU branch only where a lane of the warp needs it
           if (__any_sync(0xffffffffu, fabsf(xe) >= 0.35f)) J = fabsf(xe) < 0.35f ? J : epr_exp_fast(xe) - 1.f;
-          const int tot = Fi + __float2int_rn(fixFf * J);
+          const int tot = Fix + __float2int_rn(fixFfx * J);
           const float totf = (float)tot, te = totf * (1.f - dy), td = totf * dy, ex = 1.f - dx;
           const int c00 = __float2int_rn(te * ex), c10 = __float2int_rn(te * dx), c01 = __float2int_rn(td * ex);
           const int c11 = tot - c00 - c10 - c01;
@@ -527,12 +539,21 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       const int tx0 = sx - He, ty0 = sy - He;          // source pixel relative to the tile
       float ux, uy, tc = 0.f;
       unsigned gidx = 0;
+      float csx = cs, gamx = gam, fixFfx = fixFf;      // scalars of the source's column
+      int Fix = Fi;
+      if (COLS && FROM_TAU) {
+        const size_t ci = (size_t)s * nx + wrapm(x0 + tx0, nx);
+        gamx = __ldg(&C.gamma[ci]);
+        csx = -0.5f * __ldg(&C.a[ci]) * gamx;
+        fixFfx = __ldg(&C.f[ci]) * 67108864.f;
+        Fix = (int)__ldg(&C.fixFi[ci]);
+      }
       if (FROM_TAU) {
         // u = a D⁰ ln I_s = −a γ D⁰τ, clamped to ±S
         const float* tp = s_tau + (ty0 + H + 1) * TP + (tx0 + Ha);
         tc = tp[0];
-        ux = fminf(fmaxf(cs * (tp[1] - tp[-1]), -S), S);
-        uy = fminf(fmaxf(cs * (tp[TP] - tp[-TP]), -S), S);
+        ux = fminf(fmaxf(csx * (tp[1] - tp[-1]), -S), S);
+        uy = fminf(fmaxf(csx * (tp[TP] - tp[-TP]), -S), S);
         if (MAP_OUT && (unsigned)tx0 < ST_W && (unsigned)ty0 < TH && x0 + tx0 < nx && y0 + ty0 < ny)
           map_out[pl + (unsigned)(y0 + ty0) * nx + (x0 + tx0)] = make_float2(ux, uy);
       } else {
@@ -548,9 +569,9 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       if (FROM_TAU) {
         // the same arithmetic as the interior walk, operation for operation: a source is an interior source of its
         // own tile and a ring source of its neighbours, and all of them must agree on its four corner masses
-        const float xe = -gam * tc;
+        const float xe = -gamx * tc;
         const float J = fabsf(xe) < 0.35f ? epr_expm1_small(xe) : epr_exp_fast(xe) - 1.f;
-        tot = Fi + __float2int_rn(fixFf * J);
+        tot = Fix + __float2int_rn(fixFfx * J);
       } else {
         tot = __float2int_rn(__ldg(&I_bins[pl + gidx]) * 67108864.f);
       }
@@ -594,13 +615,25 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
         // An EMPTY detector pixel (no source reaches it: the shadow side of a caustic) is written as exactly −f_s, so that
         // P_s = f_s + (P_s − f_s) is exactly 0 downstream and the split's decision "Σ_t P_t⁺ = 0 → w_s = f_s" (R8) is
         // taken on the integers, where an empty pixel is exactly empty — (float)(−Fi) alone would leave ±3e-8 there.
-        const float nf = -L.f[s];
-        o = make_float4(v.x ? fmaf((float)((int)v.x - Fi), sc, corr) : nf, v.y ? fmaf((float)((int)v.y - Fi), sc, corr) : nf,
-                        v.z ? fmaf((float)((int)v.z - Fi), sc, corr) : nf, v.w ? fmaf((float)((int)v.w - Fi), sc, corr) : nf);
+        if (COLS) {                                    // baseline, its fp32 remainder and f_s of the four DETECTOR columns
+          const size_t ci = (size_t)s * nx + (x0 + ftx);
+          const uint4 F4 = __ldg(reinterpret_cast<const uint4*>(C.fixFi + ci));
+          const float4 c4 = __ldg(reinterpret_cast<const float4*>(C.fixCorr + ci)), f4 = __ldg(reinterpret_cast<const float4*>(C.f + ci));
+          o = make_float4(v.x ? fmaf((float)((int)v.x - (int)F4.x), sc, c4.x) : -f4.x, v.y ? fmaf((float)((int)v.y - (int)F4.y), sc, c4.y) : -f4.y,
+                          v.z ? fmaf((float)((int)v.z - (int)F4.z), sc, c4.z) : -f4.z, v.w ? fmaf((float)((int)v.w - (int)F4.w), sc, c4.w) : -f4.w);
+        } else {
+          const float nf = -L.f[s];
+          o = make_float4(v.x ? fmaf((float)((int)v.x - Fi), sc, corr) : nf, v.y ? fmaf((float)((int)v.y - Fi), sc, corr) : nf,
+                          v.z ? fmaf((float)((int)v.z - Fi), sc, corr) : nf, v.w ? fmaf((float)((int)v.w - Fi), sc, corr) : nf);
+        }
         if (out_mode == 2) {
           const float4 dd = dpre[k];
-          const float off = 1.f + L.fsum_dev;
-          o = make_float4((dd.x - off) - o.x, (dd.y - off) - o.y, (dd.z - off) - o.z, (dd.w - off) - o.w);
+          float4 off = make_float4(1.f + L.fsum_dev, 1.f + L.fsum_dev, 1.f + L.fsum_dev, 1.f + L.fsum_dev);
+          if (COLS) {
+            const float4 fd = __ldg(reinterpret_cast<const float4*>(C.fsum_dev + (x0 + ftx)));
+            off = make_float4(1.f + fd.x, 1.f + fd.y, 1.f + fd.z, 1.f + fd.w);
+          }
+          o = make_float4((dd.x - off.x) - o.x, (dd.y - off.y) - o.y, (dd.z - off.z) - o.z, (dd.w - off.w) - o.w);
         }
       }
       *reinterpret_cast<float4*>(ol + k * fgs) = o;
@@ -611,7 +644,17 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
     // PAPER.md:231, reading R8 — the arithmetic of k_residual, in place.  Every thread re-reads exactly the values
     // P_s − f_s it stored above (same thread, same addresses: program order makes them visible; they are still in L2)
     // and overwrites them with e_s, so the N prediction planes never come back from HBM.
-    const float off = 1.f + L.fsum_dev;
+    float4 off = make_float4(1.f + L.fsum_dev, 1.f + L.fsum_dev, 1.f + L.fsum_dev, 1.f + L.fsum_dev);
+    if (COLS && fxin) {
+      const float4 fd = __ldg(reinterpret_cast<const float4*>(C.fsum_dev + (x0 + ftx)));
+      off = make_float4(1.f + fd.x, 1.f + fd.y, 1.f + fd.z, 1.f + fd.w);
+    }
+    // f_s of the thread's four detector columns: the line's scalar, or (COLS) the columns' table entries
+    auto f4_of = [&](int s) {
+      if (COLS) return __ldg(reinterpret_cast<const float4*>(C.f + (size_t)s * nx + (x0 + ftx)));
+      const float f = L.f[s];
+      return make_float4(f, f, f, f);
+    };
     float* ob = out + (size_t)b * L.n_bins * plane + fg0;
     const float* dg = d + (size_t)b * plane + fg0;
 #pragma unroll 1
@@ -622,12 +665,12 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       #pragma unroll 4                                  // four independent L2 loads in flight per thread (8: slower)
       for (int s = 0; s < L.n_bins; ++s) {
         const float4 pd = __ldcg(reinterpret_cast<const float4*>(og + (size_t)s * plane));
-        const float f = L.f[s];
+        const float4 f = f4_of(s);
         sum.x += pd.x; sum.y += pd.y; sum.z += pd.z; sum.w += pd.w;
-        den.x += fmaxf(f + pd.x, 0.f); den.y += fmaxf(f + pd.y, 0.f); den.z += fmaxf(f + pd.z, 0.f); den.w += fmaxf(f + pd.w, 0.f);
+        den.x += fmaxf(f.x + pd.x, 0.f); den.y += fmaxf(f.y + pd.y, 0.f); den.z += fmaxf(f.z + pd.z, 0.f); den.w += fmaxf(f.w + pd.w, 0.f);
       }
       const float4 dd = __ldg(reinterpret_cast<const float4*>(dg + k * fgs));
-      const float4 e = make_float4((dd.x - off) - sum.x, (dd.y - off) - sum.y, (dd.z - off) - sum.z, (dd.w - off) - sum.w);
+      const float4 e = make_float4((dd.x - off.x) - sum.x, (dd.y - off.y) - sum.y, (dd.z - off.z) - sum.z, (dd.w - off.w) - sum.w);
       // e_s = P_s⁺ q + f_s fb:  q = e/Σ_t P_t⁺, fb = 0 where the sum is positive;  q = 0, fb = e (weights f_s) where it is not
       const float4 q = make_float4(den.x > 0.f ? e.x / den.x : 0.f, den.y > 0.f ? e.y / den.y : 0.f,
                                    den.z > 0.f ? e.z / den.z : 0.f, den.w > 0.f ? e.w / den.w : 0.f);
@@ -635,37 +678,38 @@ __global__ void __launch_bounds__(ST_NT) k_splat_tile(EprLines L, int nx, int ny
       #pragma unroll 4
       for (int s = 0; s < L.n_bins; ++s) {
         const float4 pd = __ldcg(reinterpret_cast<const float4*>(og + (size_t)s * plane));
-        const float f = L.f[s];
+        const float4 f = f4_of(s);
         float4 o;
-        o.x = fmaf(fmaxf(f + pd.x, 0.f), q.x, f * fb.x);
-        o.y = fmaf(fmaxf(f + pd.y, 0.f), q.y, f * fb.y);
-        o.z = fmaf(fmaxf(f + pd.z, 0.f), q.z, f * fb.z);
-        o.w = fmaf(fmaxf(f + pd.w, 0.f), q.w, f * fb.w);
+        o.x = fmaf(fmaxf(f.x + pd.x, 0.f), q.x, f.x * fb.x);
+        o.y = fmaf(fmaxf(f.y + pd.y, 0.f), q.y, f.y * fb.y);
+        o.z = fmaf(fmaxf(f.z + pd.z, 0.f), q.z, f.z * fb.z);
+        o.w = fmaf(fmaxf(f.w + pd.w, 0.f), q.w, f.w * fb.w);
         *reinterpret_cast<float4*>(og + (size_t)s * plane) = o;
       }
     }
   }
 }
 
-template <bool FROM_TAU, bool MAP_OUT, int NT, int TH>
+template <bool FROM_TAU, bool MAP_OUT, int NT, int TH, bool COLS>
 static cudaError_t launch_splat_v(const epr_plan_s* p, int batch, int H, size_t smem, const float* tau, const float* I_bins,
                                   const float2* map_in, float2* map_out, float* out, int out_mode, const float* d,
                                   cudaStream_t st) {
   static EprPerDevice attr = {};                         // largest dynamic shared memory set so far, per device
   if ((long long)smem > attr.at(p)) {
-    cudaFuncSetAttribute(k_splat_tile<FROM_TAU, MAP_OUT, NT, TH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_splat_tile<FROM_TAU, MAP_OUT, NT, TH, COLS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr.at(p) = (long long)smem;
   }
   dim3 grid((p->nx + ST_W - 1) / ST_W, (p->ny + TH - 1) / TH, batch);
   // several lines share one list of ring candidates (the coordinates are packed in 8 bits each: H ≤ 64)
   static const bool list_off = getenv("EPR_SPLAT_LIST") && atoi(getenv("EPR_SPLAT_LIST")) == 0;
   const int use_list = FROM_TAU && p->lines.n_bins > 1 && H <= 64 && !list_off;
-  k_splat_tile<FROM_TAU, MAP_OUT, NT, TH><<<grid, NT, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, H, tau, I_bins,
-                                                                   map_in, map_out, out, out_mode, d, p->gmax, use_list, p->d_flags);
+  k_splat_tile<FROM_TAU, MAP_OUT, NT, TH, COLS><<<grid, NT, smem, st>>>(COLS ? p->lines_bound : p->lines, p->cols, p->nx, p->ny,
+                                                                         p->opt.max_shift_px, H, tau, I_bins, map_in, map_out, out,
+                                                                         out_mode, d, p->gmax, use_list, p->d_flags);
   return cudaGetLastError();
 }
 
-template <bool FROM_TAU, bool MAP_OUT>
+template <bool FROM_TAU, bool MAP_OUT, bool COLS = false>
 static cudaError_t launch_splat_t(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
                                   float2* map_out, float* out, int out_mode, const float* d, cudaStream_t st) {
   const int H = (int)ceilf(p->opt.max_shift_px) + 1;
@@ -682,10 +726,10 @@ static cudaError_t launch_splat_t(const epr_plan_s* p, int batch, const float* t
   // 128 x 64 tiles with 512 threads when two CTAs fit an SM; large S (C5: S = 24): 128 x 32 tiles still bring two;
   // beyond that one 1024-thread CTA per SM
   if (smem_of(ST_H) <= half)
-    return launch_splat_v<FROM_TAU, MAP_OUT, 512, ST_H>(p, batch, H, smem_of(ST_H), tau, I_bins, map_in, map_out, out, out_mode, d, st);
+    return launch_splat_v<FROM_TAU, MAP_OUT, 512, ST_H, COLS>(p, batch, H, smem_of(ST_H), tau, I_bins, map_in, map_out, out, out_mode, d, st);
   if (smem_of(ST_H / 2) <= half)
-    return launch_splat_v<FROM_TAU, MAP_OUT, 512, ST_H / 2>(p, batch, H, smem_of(ST_H / 2), tau, I_bins, map_in, map_out, out, out_mode, d, st);
-  return launch_splat_v<FROM_TAU, MAP_OUT, 1024, ST_H>(p, batch, H, smem_of(ST_H), tau, I_bins, map_in, map_out, out, out_mode, d, st);
+    return launch_splat_v<FROM_TAU, MAP_OUT, 512, ST_H / 2, COLS>(p, batch, H, smem_of(ST_H / 2), tau, I_bins, map_in, map_out, out, out_mode, d, st);
+  return launch_splat_v<FROM_TAU, MAP_OUT, 1024, ST_H, COLS>(p, batch, H, smem_of(ST_H), tau, I_bins, map_in, map_out, out, out_mode, d, st);
 }
 
 cudaError_t epr_launch_splat(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,
@@ -693,6 +737,12 @@ cudaError_t epr_launch_splat(const epr_plan_s* p, int batch, const float* tau, c
   if (!tau) return launch_splat_t<false, false>(p, batch, tau, I_bins, map_in, map_out, out, out_mode, d, st);
   if (map_out) return launch_splat_t<true, true>(p, batch, tau, I_bins, map_in, map_out, out, out_mode, d, st);
   return launch_splat_t<true, false>(p, batch, tau, I_bins, map_in, map_out, out, out_mode, d, st);
+}
+
+// The loop's splat with the per-column tables of an x-dependent spectrum (16-pixel-aligned grids; reading R17(b))
+cudaError_t epr_launch_splat_cols(const epr_plan_s* p, int batch, const float* tau, float* out, int out_mode, const float* d,
+                                  cudaStream_t st) {
+  return launch_splat_t<true, false, true>(p, batch, tau, nullptr, nullptr, nullptr, out, out_mode, d, st);
 }
 
 // =====================================================================================================
@@ -768,8 +818,8 @@ cudaError_t epr_launch_pred_out(const epr_plan_s* p, int batch, const float* pre
 // a3  adjoint ℳ*_s: bilinear gather at the mapped coordinates, Eq. (4), with the SAME
 //     x0, y0, w as the splat of this iteration (ray map recomputed from τ, or the stored one).
 // =====================================================================================================
-template <bool BIG>          // BIG: nx, ny > 32 ≥ |shift| + 1, so one conditional add wraps an index
-__global__ void __launch_bounds__(256) k_gather(EprLines L, int nx, int ny, float S, const float* __restrict__ tau,
+template <bool BIG, bool COLS = false>          // BIG: nx, ny > 32 ≥ |shift| + 1, so one conditional add wraps an index; COLS: per-column a_s γ_s
+__global__ void __launch_bounds__(256) k_gather(EprLines L, EprColumns C, int nx, int ny, float S, const float* __restrict__ tau,
                                                 const float2* __restrict__ map_in, const float* __restrict__ es,
                                                 float* __restrict__ r) {
   // one thread = 4 consecutive pixels of one row (nx % 4 == 0)
@@ -794,7 +844,13 @@ __global__ void __launch_bounds__(256) k_gather(EprLines L, int nx, int ny, floa
   float* rb = r + p0 + row + x;
   const float2* mb = map_in ? map_in + p0 + row + x : nullptr;
   for (int s = 0; s < L.n_bins; ++s, eb += plane, rb += plane) {
-    const float c = -0.5f * L.a[s] * L.gamma[s];
+    float c4[4];
+    c4[0] = c4[1] = c4[2] = c4[3] = -0.5f * L.a[s] * L.gamma[s];
+    if (COLS) {                                        // the pixel's own column (the map of the splat of this column's sources)
+      const float4 a4 = __ldg(reinterpret_cast<const float4*>(C.a + (size_t)s * nx + x));
+      const float4 g4 = __ldg(reinterpret_cast<const float4*>(C.gamma + (size_t)s * nx + x));
+      c4[0] = -0.5f * a4.x * g4.x; c4[1] = -0.5f * a4.y * g4.y; c4[2] = -0.5f * a4.z * g4.z; c4[3] = -0.5f * a4.w * g4.w;
+    }
     float o[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
@@ -803,8 +859,8 @@ __global__ void __launch_bounds__(256) k_gather(EprLines L, int nx, int ny, floa
         const float2 m = __ldg(mb + k);
         ux = m.x; uy = m.y;
       } else {
-        ux = fminf(fmaxf(c * dtx[k], -S), S);
-        uy = fminf(fmaxf(c * dty[k], -S), S);
+        ux = fminf(fmaxf(c4[k] * dtx[k], -S), S);
+        uy = fminf(fmaxf(c4[k] * dty[k], -S), S);
       }
       const int fx = __float2int_rd(ux), fy = __float2int_rd(uy);
       const float dx = ux - (float)fx, dy = uy - (float)fy;
@@ -838,8 +894,8 @@ __global__ void __launch_bounds__(256) k_gather(EprLines L, int nx, int ny, floa
 #define GT_NT 512
 #define GT_PPT (GT_W * GT_H / GT_NT)   // pixels per thread (rows y = (tid >> 7) + 4 k of column tid & 127)
 
-template <bool BIG>          // BIG: nx, ny ≥ 2 (tile + halo), so one conditional add wraps an index
-__global__ void __launch_bounds__(GT_NT, 2) k_gather_tile(EprLines L, int nx, int ny, float S, const float* __restrict__ tau,
+template <bool BIG, bool COLS = false>          // BIG: nx, ny ≥ 2 (tile + halo), so one conditional add wraps an index
+__global__ void __launch_bounds__(GT_NT, 2) k_gather_tile(EprLines L, EprColumns C, int nx, int ny, float S, const float* __restrict__ tau,
                                                         const float* __restrict__ gmax, const float* __restrict__ es,
                                                         float* __restrict__ r) {
   extern __shared__ __align__(128) float s_e[];       // [2][GT_ER][GT_EP]
@@ -902,7 +958,9 @@ __global__ void __launch_bounds__(GT_NT, 2) k_gather_tile(EprLines L, int nx, in
   unsigned nfill = 0u;                                 // bit i: parity of the fills of buffer i (lines served by global loads skip theirs)
   for (int s = 0; s < L.n_bins; ++s) {
     if (s + 1 < L.n_bins) stage(s + 1);                // buffer (s + 1) & 1 was released by the barrier ending line s − 1
-    const float c = -0.5f * L.a[s] * L.gamma[s];
+    // COLS: L carries the bound max_x a_s(x) γ_s(x) (halo, clamp test); the thread's pixels share its column's coefficient
+    const float cb = -0.5f * L.a[s] * L.gamma[s];
+    const float c = COLS ? -0.5f * __ldg(&C.a[(size_t)s * nx + (xin ? x0 + x : 0)]) * __ldg(&C.gamma[(size_t)s * nx + (xin ? x0 + x : 0)]) : cb;
     const int Hg = halo(s);
     if (Hg <= GT_HG) {                                 // phase parity = how often this buffer has been filled before
       eprtma::mbar_wait(&s_bar[s & 1], (nfill >> (s & 1)) & 1u);
@@ -931,7 +989,7 @@ __global__ void __launch_bounds__(GT_NT, 2) k_gather_tile(EprLines L, int nx, in
           if (FULL || (xin && y0 + yy + 4 * k < ny)) rb[k * nx4] = fmaf(dy, t1 - t0, t0);
         }
       };
-      const bool clamp = fabsf(c) * maxd > S, full = x0 + GT_W <= nx && y0 + GT_H <= ny;
+      const bool clamp = fabsf(cb) * maxd > S, full = x0 + GT_W <= nx && y0 + GT_H <= ny;
       if (clamp) { if (full) body(std::true_type{}, std::true_type{}); else body(std::true_type{}, std::false_type{}); }
       else { if (full) body(std::false_type{}, std::true_type{}); else body(std::false_type{}, std::false_type{}); }
     } else if (xin) {
@@ -956,8 +1014,10 @@ __global__ void __launch_bounds__(GT_NT, 2) k_gather_tile(EprLines L, int nx, in
   }
 }
 
-cudaError_t epr_launch_gather(const epr_plan_s* p, int batch, const float* tau, const float2* map_in, const float* es,
-                              float* r, int gmax_fresh, cudaStream_t st) {
+template <bool COLS>
+static cudaError_t launch_gather_t(const epr_plan_s* p, int batch, const float* tau, const float2* map_in, const float* es,
+                                   float* r, int gmax_fresh, cudaStream_t st) {
+  const EprLines& LL = COLS ? p->lines_bound : p->lines;
   if (tau && !map_in && gmax_fresh && p->gmax && p->n_bins > 1) {
     // the loop: p->gmax holds the block maxima of this τ (written ahead of the splat of the same iteration).
     // Several lines only: with one line there is nothing to stage ahead and nothing to share, and the direct kernel
@@ -965,21 +1025,31 @@ cudaError_t epr_launch_gather(const epr_plan_s* p, int batch, const float* tau, 
     constexpr size_t smem = 2 * (size_t)GT_ER * GT_EP * sizeof(float);
     static EprPerDevice attr = {};
     if (!attr.at(p)) {
-      cudaFuncSetAttribute(k_gather_tile<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-      cudaFuncSetAttribute(k_gather_tile<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      cudaFuncSetAttribute(k_gather_tile<true, COLS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      cudaFuncSetAttribute(k_gather_tile<false, COLS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
       attr.at(p) = 1;
     }
     dim3 grid((p->nx + GT_W - 1) / GT_W, (p->ny + GT_H - 1) / GT_H, batch);
     if (p->nx >= 2 * GT_EP && p->ny >= 2 * GT_ER)
-      k_gather_tile<true><<<grid, GT_NT, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, tau, p->gmax, es, r);
+      k_gather_tile<true, COLS><<<grid, GT_NT, smem, st>>>(LL, p->cols, p->nx, p->ny, p->opt.max_shift_px, tau, p->gmax, es, r);
     else
-      k_gather_tile<false><<<grid, GT_NT, smem, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, tau, p->gmax, es, r);
+      k_gather_tile<false, COLS><<<grid, GT_NT, smem, st>>>(LL, p->cols, p->nx, p->ny, p->opt.max_shift_px, tau, p->gmax, es, r);
     return cudaGetLastError();
   }
   dim3 grid((p->nx / 4 + 63) / 64, (p->ny + 3) / 4, batch);
-  if (p->nx > 32 && p->ny > 32) k_gather<true><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, tau, map_in, es, r);
-  else k_gather<false><<<grid, 256, 0, st>>>(p->lines, p->nx, p->ny, p->opt.max_shift_px, tau, map_in, es, r);
+  if (p->nx > 32 && p->ny > 32) k_gather<true, COLS><<<grid, 256, 0, st>>>(LL, p->cols, p->nx, p->ny, p->opt.max_shift_px, tau, map_in, es, r);
+  else k_gather<false, COLS><<<grid, 256, 0, st>>>(LL, p->cols, p->nx, p->ny, p->opt.max_shift_px, tau, map_in, es, r);
   return cudaGetLastError();
+}
+
+cudaError_t epr_launch_gather(const epr_plan_s* p, int batch, const float* tau, const float2* map_in, const float* es,
+                              float* r, int gmax_fresh, cudaStream_t st) {
+  return launch_gather_t<false>(p, batch, tau, map_in, es, r, gmax_fresh, st);
+}
+
+// the loop's gather with the per-column tables of an x-dependent spectrum (after epr_launch_splat_cols on the same τ)
+cudaError_t epr_launch_gather_cols(const epr_plan_s* p, int batch, const float* tau, const float* es, float* r, cudaStream_t st) {
+  return launch_gather_t<true>(p, batch, tau, nullptr, es, r, 1, st);
 }
 
 // Final output conversion: τ | φ of one line (Eq. (6): φ_s = −(db_s/2) γ_s τ) | Σ_s I_s (Eq. (7)).

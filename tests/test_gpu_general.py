@@ -247,3 +247,28 @@ def test_profiles_output_modes_and_host_path(E):
     for j in range(3):
         want = -(prof.db[2][None, :] / 2.0) * prof.gamma[2][None, :] * refs[j]
         assert_close(oh[j].numpy(), want, TOL_PHASE)
+
+
+@pytest.mark.parametrize("solver,step,L,S", [("local", 1.0, 0.3, 16.0), ("nonlocal", 0.4, 8.0, 6.0)])
+@pytest.mark.parametrize("n_lines", [3, 1])
+def test_retrieve_profiles_staged_column_transforms(E, solver, step, L, S, n_lines):
+    """ny = 256 (power of two, TMA column kernel): with several blocks the columns are transformed ONCE per iteration and every
+    block filter runs on the transformed spectra (stage 1 / stage 2 of k_cols_tma), also for the initial solve; 64 x 256 grid,
+    4 blocks, against retrieve_x."""
+    import torch
+    nx, ny, nblk = 64, 256, 4
+    en, wt, db, mu_rel, prof = _profiles(nx, nblk, L, n_lines, True)
+    d = _data(ny, nx, 31)
+    ref = O.retrieve_x(d.astype(np.float64), prof, solver, 4, step, S=S)
+    plan = E.epr_plan(nx, ny, 6.5e-6, L, en, wt[0], db[0], solver, max_batch=1, max_shift_px=S)
+    E.epr_plan_profiles(plan, wt, db, mu_rel)
+    dd = _dev(d[None])
+    out = torch.empty_like(dd)
+    l0 = plan.launches
+    E.epr_retrieve(plan, dd, out, 4, step)
+    got = out.cpu().numpy()[0]
+    n_launch = plan.launches - l0
+    plan.destroy()
+    assert_close(got, ref, TOL_PHASE, f"staged columns, {solver}, {n_lines} line(s)")
+    # 5 solves x (1 row pass + 1 staged column pass + 4 x (block filter + inverse rows) + 1 update) + forward-model launches
+    assert n_launch >= 5 * (1 + 1 + 2 * nblk + 1)
