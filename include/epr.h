@@ -33,8 +33,7 @@ typedef struct epr_plan_s* epr_plan_t;
 typedef enum {
   EPR_OK = 0,
   EPR_EINVAL = 1, /* bad argument (NULL pointer, non-positive size / energy / weight / step, batch > max_batch …) */
-  EPR_ESIZE = 2,  /* unsupported grid: nx or ny has a prime factor other than 2, 3, 5, or exceeds the largest supported
-                     length (8192; 4096 for the sizes with a compiled transform), see epr_plan */
+  EPR_ESIZE = 2,  /* unsupported grid: nx or ny has a prime factor other than 2, 3, 5, or exceeds 8192 (see epr_plan) */
   EPR_ECUDA = 3,  /* a CUDA runtime call failed; message in epr_last_error */
   EPR_ENOMEM = 4  /* device allocation failed */
 } epr_status;
@@ -69,7 +68,7 @@ void epr_default_options(epr_options* opt);
  *   The tuned kernels run on 16-pixel-aligned grids whose lengths have a compiled transform (16, 32, 48, 64, 80, 96, 128,
  *   160, 256, 320, 384, 512, 640, 768, 1024, 1280, 1536, 1920, 2048, 2160, 2560, 3072, 3200, 4096); every other smooth
  *   grid up to 8192 per axis (250, 1080, 3000, odd lengths such as 375, …) runs the general path: the same steps, one
- *   pixel per thread, run-time-radix FFT — correct to the same tolerances, about 3x slower per pixel.
+ *   pixel per thread, run-time-radix FFT — correct to the same tolerances, 2x (non-local) to 5x (local) slower per pixel.
  * Derived: k_s = 2πE_s/(hc); α_s = L/(k_s p²); a_s = α_s δ_s/(2β_s); γ_s ∝ 1/(E_s δ_s/β_s), Σ f_s γ_s = 1. */
 epr_status epr_plan(epr_plan_t* plan, int nx, int ny, double pixel_m, double L_m, int n_bins,
                     const double* energy_keV, const double* weight, const double* delta_over_beta,

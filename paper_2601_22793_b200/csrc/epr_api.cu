@@ -73,7 +73,7 @@ extern "C" void epr_default_options(epr_options* o) {
   o->init = 0; o->output = 0; o->out_bin = 0; o->mu_rel = NULL; o->nonlocal_wkb1 = 0;
 }
 
-extern "C" const char* epr_version(void) { return "epr-b200 0.2.0 (sm_100a)"; }
+extern "C" const char* epr_version(void) { return "epr-b200 0.2.1 (sm_100a)"; }
 
 extern "C" const char* epr_last_error(epr_plan_t p) { return p ? p->err : "null plan"; }
 
@@ -304,6 +304,11 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
     L.pj_b[s] = (float)log2(p->h_f[s]);
     L.pj_g2[s] = (float)(p->h_gamma[s] * p->h_gamma[s]);
     L.pj_g3[s] = (float)(p->h_gamma[s] * p->h_gamma[s] * p->h_gamma[s]);
+  }
+  for (int k = 0; k < 8; ++k) {
+    double g = 0;
+    for (int s = 0; s < n_bins; ++s) g += (double)L.f[s] * pow(p->h_gamma[s], k);
+    L.pj_G[k] = (float)g;
   }
   L.gamma_max = 0.f;
   for (int s = 0; s < n_bins; ++s) L.gamma_max = fmaxf(L.gamma_max, L.gamma[s]);

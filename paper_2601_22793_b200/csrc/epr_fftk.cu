@@ -206,7 +206,10 @@ __global__ void __launch_bounds__(RowCfg<M>::NT, (RowCfg<M>::NT <= 128) ? C2R_MI
           if (i + C::TPC < M && !tau_is_zero) tnext = dst[i + C::TPC];
           const float2 v = s[i];
           float d0, d1;
-          if (!epr_project_increment_small_nb2(L, tau, make_float2(step * v.x, step * v.y), newton_iters, i_min, d0, d1)) {
+          if (tau_is_zero) {                 // the initial guess: constant moments, no exponential of τ
+            d0 = epr_project_increment_tau0(L, step * v.x, s_f, s_gamma, newton_iters, i_min);
+            d1 = epr_project_increment_tau0(L, step * v.y, s_f, s_gamma, newton_iters, i_min);
+          } else if (!epr_project_increment_small_nb2(L, tau, make_float2(step * v.x, step * v.y), newton_iters, i_min, d0, d1)) {
             d0 = epr_project_increment(tau.x, step * v.x, s_f, s_gamma, L.n_bins, L.gamma_max, newton_iters, i_min);
             d1 = epr_project_increment(tau.y, step * v.y, s_f, s_gamma, L.n_bins, L.gamma_max, newton_iters, i_min);
           }

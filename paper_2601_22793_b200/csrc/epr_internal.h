@@ -25,6 +25,7 @@ struct EprLines {
   float pj_b[EPR_MAX_BINS];     // log2(f_s)
   float pj_g2[EPR_MAX_BINS];    // γ_s²
   float pj_g3[EPR_MAX_BINS];    // γ_s³
+  float pj_G[8];                // Σ_s f_s γ_s^k, k = 0..7: the moments of the projection at τ = 0 (initial guess)
   float abar;                   // Σ f_s a_s (initial guess, R9)
   float gamma_max;              // max_s γ_s (range test of the projection's polynomial form)
   float fsum_dev;               // Σ_s (float)f_s − 1: rounding of the fp32 fractions, removed from the residual

@@ -230,3 +230,43 @@ static __device__ __noinline__ float epr_project_increment(float tau, float dT, 
   }
   return delta;
 }
+
+// The projection of the INITIAL guess (τ = 0, R9): I_s = f_s, so the moments G_k = Σ_s f_s γ_s^k are constants of the plan
+// (L.pj_G) and no exponential of τ is needed: Newton on the degree-7 polynomial for |γ_max δ| < 0.25, on the exact sum
+// Σ_s f_s expm1(−γ_s δ) = ΔT beyond (thick objects).  Same tiers, start and stopping rule as epr_project_increment.
+static __device__ __noinline__ float epr_project_increment_tau0(const EprLines& L, float dT, const float* __restrict__ f,
+                                                                const float* __restrict__ gamma, int newton_iters, float i_min) {
+  const float G0 = L.pj_G[0], G1 = L.pj_G[1];
+  if (G0 + dT < i_min) dT = i_min - G0;
+  float delta = -epr_log1p(__fdividef(dT, G0)) * __fdividef(G0, G1);
+  if (fabsf(delta) * L.gamma_max < 0.25f) {
+    const float c1 = -G1, c2 = 0.5f * L.pj_G[2], c3 = -1.66666667e-1f * L.pj_G[3], c4 = 4.16666667e-2f * L.pj_G[4],
+                c5 = -8.33333333e-3f * L.pj_G[5], c6 = 1.38888889e-3f * L.pj_G[6], c7 = -1.98412698e-4f * L.pj_G[7];
+    for (int it = 0; it < newton_iters; ++it) {
+      float P = c7, dP = 0.f;
+      dP = fmaf(dP, delta, P); P = fmaf(P, delta, c6);
+      dP = fmaf(dP, delta, P); P = fmaf(P, delta, c5);
+      dP = fmaf(dP, delta, P); P = fmaf(P, delta, c4);
+      dP = fmaf(dP, delta, P); P = fmaf(P, delta, c3);
+      dP = fmaf(dP, delta, P); P = fmaf(P, delta, c2);
+      dP = fmaf(dP, delta, P); P = fmaf(P, delta, c1);
+      const float F = fmaf(P, delta, -dT), dF = fmaf(dP, delta, P);
+      const float stp = __fdividef(F, dF);
+      delta -= stp;
+      if (fabsf(stp) <= 1e-7f * fabsf(delta) + 1e-12f) break;
+    }
+    return delta;
+  }
+  for (int it = 0; it < newton_iters; ++it) {
+    float F = -dT, dF = 0.f;
+    for (int s = 0; s < L.n_bins; ++s) {
+      const float em = epr_expm1(-gamma[s] * delta);
+      F = fmaf(f[s], em, F);
+      dF = fmaf(-gamma[s] * f[s], 1.f + em, dF);
+    }
+    const float stp = __fdividef(F, dF);
+    delta -= stp;
+    if (fabsf(stp) <= 1e-7f * fabsf(delta) + 1e-12f) break;
+  }
+  return delta;
+}
