@@ -470,7 +470,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="C2")
-    ap.add_argument("--batch", type=int, default=0, help="projections per GPU and step (default: 64 for C2 / C5, 16 for C3, 8 for C4)")
+    ap.add_argument("--batch", type=int, default=0, help="projections per GPU and step (default: 64 for C2 / C3 / C5, 8 for C4)")
     ap.add_argument("--distinct", type=int, default=2, help="distinct simulated projections (rest: new noise only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -505,7 +505,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     args.warmup = max(args.warmup, 3)
-    default_batch = {"C1": 64, "C2": 64, "C3": 16, "C4": 8, "C5": 64}
+    default_batch = {"C1": 64, "C2": 64, "C3": 64, "C4": 8, "C5": 64}
     B = args.batch if args.batch > 0 else default_batch[args.config]
 
     head, w = measure_config(epr, args.config, B, args.steps, args.warmup, args.distinct, rank, world, local,
@@ -531,7 +531,7 @@ def main():
         other = {}
         # the splat's ring width and candidate list depend on the data: these batches hold more distinct projections
         # (C5: 8 different rotation angles of the phantom) than the headline's local solver needs
-        for name, ob, osteps, odist in (("C3", 16, 3, 4), ("C4", 8, 3, 4), ("C5", 64, 2, 8)):
+        for name, ob, osteps, odist in (("C3", 64, 3, 4), ("C4", 8, 3, 4), ("C5", 64, 2, 8)):
             try:
                 r, ow = measure_config(epr, name, ob, osteps, 3, max(args.distinct, odist), rank, world, local)
                 if rank == 0 and not args.no_cpu_baseline:

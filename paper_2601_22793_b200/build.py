@@ -33,7 +33,7 @@ def _compile(unit, nvcc, force, verbose, hdr_t):
     src_p = os.path.join(CSRC, src)
     if not force and os.path.exists(obj) and os.path.getmtime(obj) > max(os.path.getmtime(src_p), hdr_t):
         return obj, ""
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + extra + ["-c", src, "-o", obj]
+    cmd = [nvcc] + NVCC_FLAGS + os.environ.get("EPR_NVCC_EXTRA", "").split() + (["-Xptxas", "-v"] if verbose else []) + extra + ["-c", src, "-o", obj]
     res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
     if res.returncode != 0:
         raise RuntimeError(f"nvcc failed on {src} {extra}:\n" + res.stdout + res.stderr)

@@ -911,6 +911,10 @@ static epr_status retrieve_host_impl(epr_plan_t p, int factor, int batch, const 
   { const char* env = getenv("EPR_HOST_CHUNK"); if (env && atoi(env) > 0) wbch = atoi(env); }
   if (wbch < 1) wbch = 1;
   if (wbch > p->work_batch) wbch = p->work_batch;
+  if (!getenv("EPR_HOST_CHUNK")) {                    // equal chunks: 16 projections in chunks of at most 15 go as 8 + 8, not 15 + 1
+    const int nch = (batch + wbch - 1) / wbch;
+    wbch = (batch + nch - 1) / nch;
+  }
   if (p->stage_in[0] && p->stage_floats < (size_t)wbch * plane) {           // staging buffers too small for this call: re-allocate
     CU(p, cudaDeviceSynchronize());
     for (int i = 0; i < 2; ++i) { cudaFree(p->stage_in[i]); cudaFree(p->stage_out[i]); p->stage_in[i] = p->stage_out[i] = NULL; }

@@ -52,7 +52,10 @@ struct RowPipe {
 // One row group per CTA, many CTAs per SM: the forward row transform has no epilogue to hide a load behind and
 // measures faster this way (6.7 vs 7.3 us per 2048² plane) than through the TMA stage, which is kept for C2R.
 template <int M>
-__global__ void __launch_bounds__(RowCfg<M>::NT) k_rows_r2c_direct(int ny, const float* __restrict__ in, float in_offset,
+#ifndef R2C_MINB
+#define R2C_MINB 1
+#endif
+__global__ void __launch_bounds__(RowCfg<M>::NT, (RowCfg<M>::NT <= 128) ? R2C_MINB : 1) k_rows_r2c_direct(int ny, const float* __restrict__ in, float in_offset,
                                                             const float2* __restrict__ tw, const float2* __restrict__ tw2,
                                                             float2* __restrict__ spec) {
   using C = RowCfg<M>;

@@ -272,3 +272,40 @@ def test_retrieve_profiles_staged_column_transforms(E, solver, step, L, S, n_lin
     assert_close(got, ref, TOL_PHASE, f"staged columns, {solver}, {n_lines} line(s)")
     # 5 solves x (1 row pass + 1 staged column pass + 4 x (block filter + inverse rows) + 1 update) + forward-model launches
     assert n_launch >= 5 * (1 + 1 + 2 * nblk + 1)
+
+
+def test_profiles_on_the_oversampled_grid_and_graph_replay(E):
+    """The x-dependent spectrum combined with the oversampled loop (PAPER.md:79 + §9.2: the paper's production set-up): plan on
+    the x2 grid with block profiles, replicate -> retrieve_x -> block mean against the oracle; and on a side stream the
+    launch-bound general-path retrieval is captured into a CUDA graph and replayed bit for bit."""
+    import torch
+    nxd, nyd, m, L = 80, 48, 2, 0.3
+    en, wt, db, mu_rel, _ = _profiles(m * nxd, 4, L, 3, True)
+    prof_f = O.derive_profiles(6.5e-6 / m, L, en, m * nxd, wt, db, mu_rel)
+    d = _data(nyd, nxd, 41)
+    ref = O.downsample(O.retrieve_x(O.upsample(d.astype(np.float64), m), prof_f, "local", 3, 1.0), m)
+    plan = E.epr_plan(m * nxd, m * nyd, 6.5e-6 / m, L, en, wt[0], db[0], "local", max_batch=1)
+    E.epr_plan_profiles(plan, wt, db, mu_rel)
+    dd = _dev(d[None])
+    out = torch.empty_like(dd)
+    E.epr_retrieve_oversampled(plan, m, dd, out, 3, 1.0)
+    assert_close(out.cpu().numpy()[0], ref, TOL_PHASE, "profiles on the x2 grid")
+    plan.destroy()
+    # graph capture of the general path (160 x 96, non-local, run-time memset + atomics inside the capture on 150 x 90)
+    for nx, ny in ((160, 96), (150, 90)):
+        en, wt, db, mu_rel, prof = _profiles(nx, 5, 8.0, 3, False)
+        plan = E.epr_plan(nx, ny, 6.5e-6, 8.0, en, wt[0], db[0], "nonlocal", max_batch=1, max_shift_px=6.0)
+        E.epr_plan_profiles(plan, wt, db, mu_rel)
+        dd = _dev(_data(ny, nx, 5)[None])
+        ref = torch.empty_like(dd)
+        E.epr_retrieve(plan, dd, ref, 3, 0.4)                  # default stream: eager
+        torch.cuda.synchronize()
+        side = torch.cuda.Stream()
+        out = torch.empty_like(dd)
+        with torch.cuda.stream(side):
+            for _ in range(3):                                 # eager warm pass, capture + launch, replay
+                out.zero_()
+                E.epr_retrieve(plan, dd, out, 3, 0.4)
+                side.synchronize()
+                assert torch.equal(out, ref)
+        plan.destroy()
