@@ -8,17 +8,17 @@ import it.
 
 Every function cites the PAPER.md passage (line, section / equation) it follows.  Where the
 paper is silent the reading taken is the one listed in DESIGN.md ("Readings", R1..R16, which
-restate SURVEY.md §8(c); R16 is the oversampled grid of SURVEY.md §8(f)).
+restate SURVEY.md §8(c); R16 is the oversampled grid and R17 the x-dependent effective spectrum of SURVEY.md §8(f)).
 
 Conventions: pixel units; arrays are `[row = y][col = x]`, x fastest
 (PAPER.md:185-191 write `P_s(y0, x0)`); every index is periodic (R7).
 
-Parity pins: every function below is pinned by `tests/test_oracle_operators.py`, `tests/test_oracle_loop.py` and
-`tests/test_oracle_oversample.py` against closed
-forms, invariants, brute force or a library routine used in a different way (see the table in
-DESIGN.md).  The *discretisation readings* R1..R14 themselves are "parity unpinned" against
-the paper's own (unavailable) implementation: the paper prints no numeric intermediate or
-final value.
+Parity pins: every function below is pinned by `tests/test_oracle_operators.py`, `tests/test_oracle_loop.py`,
+`tests/test_oracle_oversample.py` and `tests/test_oracle_profiles.py` against closed forms, invariants, brute force
+from the definition or a library routine used in a different way (table in DESIGN.md §8; a mutation check of the pins is
+described there).  The *readings* R1..R17 themselves (finite-difference scheme, weights, start, projection, oversampling
+transfer, blockwise interpolation of an x-dependent spectrum) are "parity unpinned" against the paper's own (unavailable)
+implementation: the paper prints no numeric intermediate or final value.
 """
 from __future__ import annotations
 
