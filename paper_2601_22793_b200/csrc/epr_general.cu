@@ -229,9 +229,43 @@ __global__ void __launch_bounds__(256) k_gen_residual(int n_bins, EprColumns C, 
   }
 }
 
+// the same for four consecutive pixels per thread (nx % 4 == 0): 16-byte accesses
+__global__ void __launch_bounds__(256) k_gen_residual4(int n_bins, EprColumns C, int nx, size_t plane, const float* __restrict__ d,
+                                                       const float* pred, float* es) {
+  const int x = 4 * (blockIdx.x * 256 + threadIdx.x);
+  if (x >= nx) return;
+  const size_t i = (size_t)blockIdx.y * nx + x;
+  const int b = blockIdx.z;
+  const size_t base = (size_t)b * n_bins * plane + i;
+  float4 sum = make_float4(0.f, 0.f, 0.f, 0.f), den = sum;
+  for (int s = 0; s < n_bins; ++s) {
+    const float4 pd = *reinterpret_cast<const float4*>(pred + base + (size_t)s * plane);
+    const float4 f = __ldg(reinterpret_cast<const float4*>(C.f + (size_t)s * nx + x));
+    sum.x += pd.x; sum.y += pd.y; sum.z += pd.z; sum.w += pd.w;
+    den.x += fmaxf(f.x + pd.x, 0.f); den.y += fmaxf(f.y + pd.y, 0.f); den.z += fmaxf(f.z + pd.z, 0.f); den.w += fmaxf(f.w + pd.w, 0.f);
+  }
+  const float4 dd = __ldg(reinterpret_cast<const float4*>(d + (size_t)b * plane + i));
+  const float4 fd = __ldg(reinterpret_cast<const float4*>(C.fsum_dev + x));
+  const float4 e = make_float4((dd.x - (1.f + fd.x)) - sum.x, (dd.y - (1.f + fd.y)) - sum.y, (dd.z - (1.f + fd.z)) - sum.z, (dd.w - (1.f + fd.w)) - sum.w);
+  const float4 q = make_float4(den.x > 0.f ? e.x / den.x : 0.f, den.y > 0.f ? e.y / den.y : 0.f, den.z > 0.f ? e.z / den.z : 0.f, den.w > 0.f ? e.w / den.w : 0.f);
+  for (int s = 0; s < n_bins; ++s) {
+    const float4 pd = *reinterpret_cast<const float4*>(pred + base + (size_t)s * plane);
+    const float4 f = __ldg(reinterpret_cast<const float4*>(C.f + (size_t)s * nx + x));
+    float4 o;
+    o.x = den.x > 0.f ? fmaxf(f.x + pd.x, 0.f) * q.x : f.x * e.x;
+    o.y = den.y > 0.f ? fmaxf(f.y + pd.y, 0.f) * q.y : f.y * e.y;
+    o.z = den.z > 0.f ? fmaxf(f.z + pd.z, 0.f) * q.z : f.z * e.z;
+    o.w = den.w > 0.f ? fmaxf(f.w + pd.w, 0.f) * q.w : f.w * e.w;
+    *reinterpret_cast<float4*>(es + base + (size_t)s * plane) = o;
+  }
+}
+
 cudaError_t epr_gen_residual(const epr_plan_s* p, int batch, const float* d, const float* pred, float* es, cudaStream_t st) {
   const size_t plane = (size_t)p->nx * p->ny;
-  k_gen_residual<<<gn_grid(p, batch), 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, d, pred, es);
+  if (p->nx % 4 == 0)
+    k_gen_residual4<<<dim3((p->nx / 4 + 255) / 256, p->ny, batch), 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, d, pred, es);
+  else
+    k_gen_residual<<<gn_grid(p, batch), 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, d, pred, es);
   return cudaGetLastError();
 }
 
@@ -287,63 +321,91 @@ cudaError_t epr_gen_gather(const epr_plan_s* p, int batch, const float* tau, con
 // the scalars of the pixel's column:  ΔT = step · Σ_b wblk[b][x] q_b  (R17(c): block filters blended),
 //   τ += δ,  Σ_s f_s(x) e^{−γ_s(x) τ} expm1(−γ_s(x) δ) = ΔT,  floored so that Σ_s I_s + ΔT >= i_min.
 // =====================================================================================================
+// δ of one pixel of column x: given τ and ΔT, Σ_s f_s(x) e^{−γ_s(x) τ} expm1(−γ_s(x) δ) = ΔT (floored)
+__device__ __forceinline__ float gen_delta(int n_bins, const EprColumns& C, int nx, int x, float t, float dT, int newton_iters, float i_min) {
+  if (n_bins == 1) {
+    const float g = __ldg(&C.gamma[x]);                 // one line: f = 1; δ = −log1p(ΔT e^{γτ})/γ in closed form
+    return epr_project_increment_mono(g * t, dT, i_min) / g;
+  }
+  // converging iterations (|γ_max δ| < 0.01): the moments G_k = Σ_s I_s γ_s^k of the column's lines once, the cubic of
+  // F(δ) = Σ_s I_s expm1(−γ_s δ) − ΔT solved without a loop (series reversion + one Newton step) — the arithmetic of
+  // epr_project_increment_small (epr_math.cuh) with run-time line count and per-column scalars
+  float G0 = 0.f, G1 = 0.f, G2 = 0.f, G3 = 0.f, gmax = 0.f;
+#pragma unroll 4
+  for (int s = 0; s < n_bins; ++s) {
+    const float g = __ldg(&C.gamma[(size_t)s * nx + x]);
+    const float pI = __ldg(&C.f[(size_t)s * nx + x]) * epr_exp_fast(-g * t);
+    gmax = fmaxf(gmax, g);
+    G0 += pI;
+    float pg = pI * g; G1 += pg;
+    pg *= g; G2 += pg;
+    G3 = fmaf(pg, g, G3);
+  }
+  const float rc1 = -__fdividef(1.f, G1);
+  float delta = dT * rc1;
+  if (fabsf(delta) * gmax < 0.01f && G0 + dT >= i_min && newton_iters > 0) {
+    const float c1 = -G1, c2 = 0.5f * G2, c3 = -1.66666667e-1f * G3;
+    delta = fmaf(-(c2 * rc1) * delta, delta, delta);
+    const float F = fmaf(fmaf(fmaf(c3, delta, c2), delta, c1), delta, -dT);
+    const float dF = fmaf(fmaf(3.f * c3, delta, 2.f * c2), delta, c1);
+    return delta - __fdividef(F, dF);
+  }
+  float f[EPR_MAX_BINS], g[EPR_MAX_BINS];
+  for (int s = 0; s < n_bins; ++s) {
+    f[s] = __ldg(&C.f[(size_t)s * nx + x]);
+    g[s] = __ldg(&C.gamma[(size_t)s * nx + x]);
+  }
+  return epr_project_increment(t, dT, f, g, n_bins, gmax, newton_iters, i_min);
+}
+
+// V pixels per thread: 1 (any nx) or 4 (nx % 4 == 0: 16-byte accesses)
+template <int V>
 __global__ void __launch_bounds__(256) k_gen_update(int n_bins, EprColumns C, int nx, size_t plane, int n_blocks,
                                                     const float* __restrict__ qblk, size_t blk_stride, float step,
                                                     int tau_is_zero, int newton_iters, float i_min, float* __restrict__ tau) {
-  GN_PIX(nx)
+  const int x = V * (blockIdx.x * 256 + threadIdx.x);
+  if (x >= nx) return;
+  const size_t i = (size_t)blockIdx.y * nx + x;
   const int b = blockIdx.z;
-  float q = 0.f;
+  float q[V], t[V];
+#pragma unroll
+  for (int v = 0; v < V; ++v) q[v] = 0.f;
   for (int k = 0; k < n_blocks; ++k) {
-    const float w = __ldg(&C.wblk[(size_t)k * nx + x]);
-    if (w != 0.f) q = fmaf(w, __ldg(&qblk[(size_t)k * blk_stride + (size_t)b * plane + i]), q);
+    const float* wp = C.wblk + (size_t)k * nx + x;
+    const float* qp = qblk + (size_t)k * blk_stride + (size_t)b * plane + i;
+    if (V == 4) {
+      const float4 w = __ldg(reinterpret_cast<const float4*>(wp));
+      if (w.x != 0.f || w.y != 0.f || w.z != 0.f || w.w != 0.f) {
+        const float4 qq = __ldg(reinterpret_cast<const float4*>(qp));
+        q[0] = fmaf(w.x, qq.x, q[0]); q[1 % V] = fmaf(w.y, qq.y, q[1 % V]); q[2 % V] = fmaf(w.z, qq.z, q[2 % V]); q[3 % V] = fmaf(w.w, qq.w, q[3 % V]);
+      }
+    } else {
+      const float w = __ldg(wp);
+      if (w != 0.f) q[0] = fmaf(w, __ldg(qp), q[0]);
+    }
   }
   float* tp = tau + (size_t)b * plane + i;
-  const float t = tau_is_zero ? 0.f : *tp;
-  float delta;
-  if (n_bins == 1) {
-    const float g = __ldg(&C.gamma[x]);                 // one line: f = 1; δ = −log1p(ΔT e^{γτ})/γ in closed form
-    delta = epr_project_increment_mono(g * t, step * q, i_min) / g;
+  if (V == 4) {
+    const float4 tv = tau_is_zero ? make_float4(0.f, 0.f, 0.f, 0.f) : *reinterpret_cast<const float4*>(tp);
+    t[0] = tv.x; t[1 % V] = tv.y; t[2 % V] = tv.z; t[3 % V] = tv.w;
   } else {
-    // converging iterations (|γ_max δ| < 0.01): the moments G_k = Σ_s I_s γ_s^k of the column's lines once, the cubic of
-    // F(δ) = Σ_s I_s expm1(−γ_s δ) − ΔT solved without a loop (series reversion + one Newton step) — the arithmetic of
-    // epr_project_increment_small (epr_math.cuh) with run-time line count and per-column scalars
-    const float dT = step * q;
-    float G0 = 0.f, G1 = 0.f, G2 = 0.f, G3 = 0.f, gmax = 0.f;
-#pragma unroll 4
-    for (int s = 0; s < n_bins; ++s) {
-      const float g = __ldg(&C.gamma[(size_t)s * nx + x]);
-      const float pI = __ldg(&C.f[(size_t)s * nx + x]) * epr_exp_fast(-g * t);
-      gmax = fmaxf(gmax, g);
-      G0 += pI;
-      float pg = pI * g; G1 += pg;
-      pg *= g; G2 += pg;
-      G3 = fmaf(pg, g, G3);
-    }
-    const float rc1 = -__fdividef(1.f, G1);
-    delta = dT * rc1;
-    if (fabsf(delta) * gmax < 0.01f && G0 + dT >= i_min && newton_iters > 0) {
-      const float c1 = -G1, c2 = 0.5f * G2, c3 = -1.66666667e-1f * G3;
-      delta = fmaf(-(c2 * rc1) * delta, delta, delta);
-      const float F = fmaf(fmaf(fmaf(c3, delta, c2), delta, c1), delta, -dT);
-      const float dF = fmaf(fmaf(3.f * c3, delta, 2.f * c2), delta, c1);
-      delta -= __fdividef(F, dF);
-    } else {
-      float f[EPR_MAX_BINS], g[EPR_MAX_BINS];
-      for (int s = 0; s < n_bins; ++s) {
-        f[s] = __ldg(&C.f[(size_t)s * nx + x]);
-        g[s] = __ldg(&C.gamma[(size_t)s * nx + x]);
-      }
-      delta = epr_project_increment(t, dT, f, g, n_bins, gmax, newton_iters, i_min);
-    }
+    t[0] = tau_is_zero ? 0.f : *tp;
   }
-  *tp = t + delta;
+#pragma unroll
+  for (int v = 0; v < V; ++v) t[v] += gen_delta(n_bins, C, nx, x + v, t[v], step * q[v], newton_iters, i_min);
+  if (V == 4) *reinterpret_cast<float4*>(tp) = make_float4(t[0], t[1 % V], t[2 % V], t[3 % V]);
+  else *tp = t[0];
 }
 
 cudaError_t epr_gen_update(const epr_plan_s* p, int batch, const float* qblk, size_t blk_stride, float step, int tau_is_zero,
                            float* tau, cudaStream_t st) {
   const size_t plane = (size_t)p->nx * p->ny;
-  k_gen_update<<<gn_grid(p, batch), 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, p->n_blocks, qblk, blk_stride, step, tau_is_zero,
-                                      p->opt.newton_iters, p->opt.i_min, tau);
+  if (p->nx % 4 == 0)
+    k_gen_update<4><<<dim3((p->nx / 4 + 255) / 256, p->ny, batch), 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, p->n_blocks, qblk, blk_stride,
+                                                                                 step, tau_is_zero, p->opt.newton_iters, p->opt.i_min, tau);
+  else
+    k_gen_update<1><<<gn_grid(p, batch), 256, 0, st>>>(p->n_bins, p->cols, p->nx, plane, p->n_blocks, qblk, blk_stride, step, tau_is_zero,
+                                                       p->opt.newton_iters, p->opt.i_min, tau);
   return cudaGetLastError();
 }
 
