@@ -32,7 +32,8 @@ def _data(ny, nx, seed, amp=0.1):
 
 # (nx, ny): sizes SURVEY.md §8(b) / VERDICT name — 1536², 1920 x 1080, 3200 x 256 (the paper's 3104-wide radiographs
 # padded to 2^7·5²), 250 = 2·5³ — plus an odd length, a tiny grid and a non-multiple of 4
-GRIDS = [(1536, 1536), (1920, 1080), (3200, 256), (250, 256), (256, 250), (375, 40), (8, 24), (90, 150), (1080, 48)]
+GRIDS = [(1536, 1536), (1920, 1080), (3200, 256), (250, 256), (256, 250), (375, 40), (8, 24), (90, 150), (1080, 48),
+         (8192, 16), (16, 8192), (6561, 8)]            # the longest lengths the run-time-radix FFT takes (8192 = 2^13, 6561 = 3^8)
 
 
 @pytest.mark.parametrize("nx,ny", GRIDS)

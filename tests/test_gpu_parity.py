@@ -802,3 +802,70 @@ def test_two_plans_on_two_devices(E):
     for p in plans:
         p.destroy()
     assert torch.equal(outs[0], outs[1])
+
+
+@pytest.mark.parametrize("n_lines", [2, 16])
+def test_retrieve_fewest_and_most_lines(E, n_lines):
+    """2 lines and the maximum the plan accepts (16: every per-line array of the kernels' parameter block in use), non-local."""
+    w = make_workload("C4", n=128)
+    e = np.linspace(60.0, 140.0, n_lines)
+    wt = np.exp(-0.5 * ((e - 100.0) / 20.0) ** 2)
+    w.energy_keV, w.weight, w.delta_over_beta = e, wt / wt.sum(), 200.0 * e / 100.0
+    got, refs = _run_retrieve(E, w, iterations=6)
+    assert_close(got[0], refs[0], TOL_PHASE)
+
+
+@pytest.mark.parametrize("S", [0.0, 30.0])
+def test_shift_clamp_extremes(E, S):
+    """max_shift_px = 0 (every shift clamped to zero: the transport degenerates to the identity, R6) and 30 (the largest the
+    library accepts: one 1024-thread CTA per SM in the splat), against the oracle with the same clamp; one and three lines."""
+    import torch
+    for spec in ("mono", "poly3_unequal_a"):
+        en, w, db = SPECTRA[spec]
+        ny, nx, L = 128, 256, 200.0
+        tau = _tau_field(ny, nx, 6, amp=0.5)[None]
+        lines = O.derive_lines(6.5e-6, L, en, w, db)
+        assert O.max_shift(tau[0].astype(np.float64), lines) > 31.0          # the clamp binds at either extreme
+        plan = E.epr_plan(nx, ny, 6.5e-6, L, en, w, db, "nonlocal", max_batch=1, max_shift_px=S)
+        P = torch.empty((1, ny, nx), device="cuda")
+        Pb = torch.empty((1, len(en), ny, nx), device="cuda")
+        E.epr_forward(plan, _dev(tau), P, Pb)
+        ref, ref_bins, _ = O.forward(tau[0].astype(np.float64), lines, "nonlocal", S=S)
+        assert_close(P.cpu().numpy()[0], ref, TOL_OP)
+        if S == 0.0:
+            Is = O.line_intensities(tau[0].astype(np.float64), lines)
+            assert_close(Pb.cpu().numpy()[0, 0], Is[0], TOL_OP)               # identity transport
+        d = np.float32(ref * (1.0 + 0.01 * np.cos(np.arange(nx) * 0.1))[None, :])[None]
+        out = _dev(tau.copy())
+        plan.destroy()
+        plan = E.epr_plan(nx, ny, 6.5e-6, L, en, w, db, "nonlocal", max_batch=1, max_shift_px=S, init=1)
+        E.epr_retrieve(plan, _dev(d), out, 2, 0.4)
+        plan.destroy()
+        want = O.retrieve(d[0].astype(np.float64), lines, "nonlocal", 2, 0.4, S=S, tau0=tau[0].astype(np.float64))
+        assert_close(out.cpu().numpy()[0], want, TOL_PHASE)
+
+
+def test_argument_errors_more(E):
+    import torch
+    en, w, db = SPECTRA["mono"]
+    e17 = np.linspace(60.0, 140.0, 17)
+    for kw in (dict(max_shift_px=31.0), dict(newton_iters=-1), dict(order=3), dict(output=3), dict(out_bin=1), dict(i_min=0.0)):
+        with pytest.raises(E.EprError) as ei:
+            E.epr_plan(64, 64, 6.5e-6, 1.0, en, w, db, "nonlocal", **kw)
+        assert ei.value.status == 1
+    with pytest.raises(E.EprError):
+        E.epr_plan(64, 64, 6.5e-6, 1.0, e17, np.ones(17), np.full(17, 1000.0))      # more than 16 lines
+    with pytest.raises(E.EprError):
+        E.epr_plan(64, 64, 6.5e-6, 1.0, en, [0.0], db)                              # non-positive weight
+    plan = E.epr_plan(64, 64, 6.5e-6, 1.0, en, w, db, max_batch=2)
+    empty = torch.ones((0, 64, 64), device="cuda")
+    with pytest.raises(E.EprError):
+        E.epr_retrieve(plan, empty, torch.empty_like(empty), 1, 1.0)                # empty batch
+    d = torch.ones((1, 64, 64), device="cuda")
+    with pytest.raises(E.EprError):
+        E.epr_retrieve(plan, d, torch.empty_like(d), -1, 1.0)                       # negative iteration count
+    with pytest.raises(E.EprError):
+        E.epr_plan_profiles(plan, np.ones((3, 1)), np.full((3, 1), 1000.0))         # 3 blocks do not divide nx = 64
+    with pytest.raises(E.EprError):
+        E.epr_shift_histogram(plan, d, 1, 0.1)                                      # fewer than 2 bins
+    plan.destroy()
