@@ -276,7 +276,7 @@ __global__ void __launch_bounds__(256) k_grad_blockmax(int nx, int ny, const flo
   auto row4 = [&](int y) { return __ldg(reinterpret_cast<const float4*>(tb + (size_t)(y < 0 ? y + ny : (y >= ny ? y - ny : y)) * nx + xs)); };
   float4 n = row4(y0 - 1), c = row4(y0);
   float m = 0.f;
-#pragma unroll 4
+#pragma unroll 8
   for (int r = 0; r < 16; ++r) {
     const float4 s4 = row4(y0 + r + 1);
     float l = __shfl_up_sync(0xffffffffu, c.w, 1), rr = __shfl_down_sync(0xffffffffu, c.x, 1);
