@@ -492,8 +492,19 @@ def ray_map_x(tau, prof: Profiles, s, S):
     return np.clip(-c * d0x(tau), -S, S), np.clip(-c * d0y(tau), -S, S)
 
 
-def forward_x(tau, prof: Profiles, solver="local", order=2, wkb1=True, S=16.0):
-    """Eq. (5) PAPER.md:209-212 with the x-dependent spectrum: returns (P_sum, [P_s], [(ux_s, uy_s)] or None)."""
+def wkb1_term_x(tau, prof: Profiles, s):
+    """(b): the WKB1 term of Eq. (1) PAPER.md:146 (`wkb1_term`, R3) evaluated AT column x on I = f_s(x) e^{−γ_s(x) τ} with
+    the scalars of the centre column, on the same five-column strips as `closure_x` (the term has radius 2)."""
+    tau = np.asarray(tau, dtype=np.float64)
+    strips = np.stack([np.roll(tau, -k, axis=1) for k in (-2, -1, 0, 1, 2)], axis=-1)      # [y][x][k] = τ[y][x+k]
+    strips = np.transpose(strips, (1, 0, 2))                                                # [x][y][k]
+    I = prof.f[s][:, None, None] * np.exp(-prof.gamma[s][:, None, None] * strips)
+    return wkb1_term(I, prof.alpha[s])[:, :, 2].T
+
+
+def forward_x(tau, prof: Profiles, solver="local", order=2, wkb1=True, S=16.0, nonlocal_wkb1=False):
+    """Eq. (5) PAPER.md:209-212 with the x-dependent spectrum: returns (P_sum, [P_s], [(ux_s, uy_s)] or None).
+    nonlocal_wkb1: the variant of reading R4 (see `forward`), the local term taken at the detector pixel's column."""
     Is = line_intensities_x(tau, prof)
     P_bins, maps = [], []
     for s in range(prof.n_bins):
@@ -502,8 +513,21 @@ def forward_x(tau, prof: Profiles, solver="local", order=2, wkb1=True, S=16.0):
         else:
             ux, uy = ray_map_x(tau, prof, s, S)
             maps.append((ux, uy))
-            P_bins.append(splat(Is[s], ux, uy))
+            P_s = splat(Is[s], ux, uy)
+            if nonlocal_wkb1:
+                P_s = P_s - wkb1_term_x(tau, prof, s)
+            P_bins.append(P_s)
     return np.sum(P_bins, axis=0), P_bins, (maps if solver != "local" else None)
+
+
+def max_shift_x(tau, prof: Profiles):
+    """`max_shift` with the x-dependent spectrum: the largest component of the unclamped shift of `ray_map_x` over pixels
+    and lines (regime indicator of PAPER.md:53-55 in the sup norm)."""
+    m = 0.0
+    for s in range(prof.n_bins):
+        ux, uy = ray_map_x(tau, prof, s, np.inf)
+        m = max(m, float(np.max(np.abs(ux))), float(np.max(np.abs(uy))))
+    return m
 
 
 def split_weights_x(P_bins, prof: Profiles):
@@ -550,7 +574,7 @@ def paganin_init_x(d, prof: Profiles, symbol=0, i_min=1e-6):
 
 
 def retrieve_x(d, prof: Profiles, solver="local", iterations=10, step=1.0, order=2, wkb1=True, symbol=0, S=16.0,
-               i_min=1e-6, tau0=None, history=None):
+               i_min=1e-6, tau0=None, history=None, shift_history=None, nonlocal_wkb1=False):
     """The correction loop of PAPER.md:231-233 with the x-dependent effective spectrum of Eq. (6)/(7) (reading R17):
     the same steps as `retrieve`, every per-line scalar taken at the pixel's column, the filter blockwise."""
     d = np.asarray(d, dtype=np.float64)
@@ -558,10 +582,12 @@ def retrieve_x(d, prof: Profiles, solver="local", iterations=10, step=1.0, order
     n = prof.n_bins
     for _ in range(iterations):
         Is = line_intensities_x(tau, prof)
-        P, P_bins, maps = forward_x(tau, prof, solver, order, wkb1, S)
+        P, P_bins, maps = forward_x(tau, prof, solver, order, wkb1, S, nonlocal_wkb1)
         e = d - P
         if history is not None:
             history.append(float(np.sqrt(np.mean(e * e))))
+        if shift_history is not None:
+            shift_history.append(max_shift_x(tau, prof))
         w = split_weights_x(P_bins, prof)
         for s in range(n):
             r = w[s] * e

@@ -204,3 +204,57 @@ def test_split_fallback_uses_the_columns_fraction():
     for x in (2, 3, 6, 7):
         assert np.allclose([w[s][0, x] for s in range(3)], prof.f[:, x], atol=1e-15)
     assert abs(prof.f[0, 2] - prof.f[0, 6]) > 0.01
+
+
+def test_nonlocal_wkb1_x_brute_force_and_uniform_reduction():
+    """Variant of R4 with the x-dependent spectrum: column x of the subtracted term is column x of the uniform-spectrum
+    `wkb1_term` evaluated on the WHOLE plane with the scalars of column x; the term is exactly what the frozen-coefficient
+    local closure subtracts; identical blocks give the uniform-spectrum variant."""
+    ny, nx = 12, 20
+    en, wt, db = np.array([80.0, 120.0]), np.array([0.4, 0.6]), np.array([8.0, 12.0])   # small δ/β: α²/4 is not small
+    t = np.linspace(0.0, 1.0, 4)[:, None]
+    prof = O.derive_profiles(6.5e-6, 8.0, en, nx, wt[None, :] * (1.0 + 0.5 * t), db[None, :] * (1.0 + 0.3 * t))
+    tau = 0.3 * (1.0 + 0.5 * _smooth(ny, nx, 21))
+    P0, b0, _ = O.forward_x(tau, prof, "nonlocal", S=8.0)
+    P1, b1, _ = O.forward_x(tau, prof, "nonlocal", S=8.0, nonlocal_wkb1=True)
+    assert np.linalg.norm(P1 - P0) > 1e-4 * np.linalg.norm(P0 - 1.0)                    # the variant does something
+    for s in range(2):
+        for x in range(nx):
+            I = prof.f[s, x] * np.exp(-prof.gamma[s, x] * tau)
+            want = O.wkb1_term(I, prof.alpha[s])[:, x]
+            assert np.max(np.abs((b0[s] - b1[s])[:, x] - want)) < 1e-15          # a difference of O(1) planes; term ~ 3e-4
+        loc = O.closure_x(tau, prof, s, 2, False) - O.closure_x(tau, prof, s, 2, True)
+        assert np.max(np.abs((b0[s] - b1[s]) - loc)) < 1e-13
+    uni = O.derive_profiles(6.5e-6, 8.0, en, nx, [wt] * 4, [db] * 4)
+    lines = O.derive_lines(6.5e-6, 8.0, en, wt, db)
+    d = 1.0 + 0.1 * _smooth(ny, nx, 3)
+    t_x = O.retrieve_x(d, uni, "nonlocal", 3, 0.4, S=8.0, nonlocal_wkb1=True)
+    t_u = O.retrieve(d, lines, "nonlocal", 3, 0.4, S=8.0, nonlocal_wkb1=True)
+    assert np.max(np.abs(t_x - t_u)) < 1e-13
+    assert np.max(np.abs(t_u - O.retrieve(d, lines, "nonlocal", 3, 0.4, S=8.0))) > 1e-6
+
+
+def test_max_shift_x_plain_loops_and_histories():
+    """Regime indicator with the x-dependent spectrum: the largest |a_s(x) γ_s(x) D⁰τ| over pixels, lines and the two
+    axes, written out in plain loops; `retrieve_x` records it and the residual RMS once per iteration, and identical
+    blocks give the uniform-spectrum histories."""
+    ny, nx = 10, 16
+    prof, _, _ = _varying(nx, 4, L=300.0, mu=True)
+    tau = 0.2 * (1.0 + 0.5 * _smooth(ny, nx, 17))
+    want = 0.0
+    for s in range(3):
+        for y in range(ny):
+            for x in range(nx):
+                c = prof.a[s, x] * prof.gamma[s, x]
+                want = max(want, c * abs(tau[y, (x + 1) % nx] - tau[y, (x - 1) % nx]) / 2.0,
+                           c * abs(tau[(y + 1) % ny, x] - tau[(y - 1) % ny, x]) / 2.0)
+    assert abs(O.max_shift_x(tau, prof) - want) < 1e-14 * want and want > 0.1
+    uni = O.derive_profiles(6.5e-6, 20.0, E3, nx, [W3] * 2, [DB3] * 2)
+    lines = O.derive_lines(6.5e-6, 20.0, E3, W3, DB3)
+    d = 1.0 + 0.1 * _smooth(ny, nx, 4)
+    hx, sx, hu, su = [], [], [], []
+    O.retrieve_x(d, uni, "nonlocal", 3, 0.4, S=8.0, history=hx, shift_history=sx)
+    O.retrieve(d, lines, "nonlocal", 3, 0.4, S=8.0, history=hu, shift_history=su)
+    assert len(hx) == 3 and len(sx) == 3
+    assert np.allclose(hx, hu, rtol=1e-11, atol=0) and np.allclose(sx, su, rtol=1e-11, atol=0)
+    assert abs(sx[0] - O.max_shift(O.paganin_init(d, lines), lines)) < 1e-12 * sx[0]
