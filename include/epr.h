@@ -129,7 +129,8 @@ epr_status epr_retrieve_oversampled(epr_plan_t plan, int factor, int batch, cons
  *     diag[b][n][1] = the regime indicator η of PAPER.md:53 in the sup norm: the largest unclamped shift component
  *                     max_s max_r |a_s D⁰ ln I_s| in pixels of the plan's grid (η < 1: local regime).
  *   Costs two small kernels and one pass over the residual planes per iteration; keep it off in timed runs.  While it
- *   is on, retrievals are not captured into CUDA graphs.  Tuned path only (EPR_EINVAL on a general-path plan). */
+ *   is on, retrievals are not captured into CUDA graphs.  On a plan with an x-dependent spectrum the shift uses the
+ *   scalars of the pixel's own column, a_s(x) γ_s(x) (R17(b)). */
 epr_status epr_set_diagnostics(epr_plan_t plan, float* diag, int capacity_iters);
 
 /* epr_shift_histogram — the regime diagnostic of Fig. 6
@@ -163,7 +164,8 @@ epr_status epr_retrieve_host(epr_plan_t plan, int batch, const float* d_host, fl
  *   weight, delta_over_beta, mu_rel: HOST arrays [n_blocks][n_bins] (mu_rel may be NULL: γ_s ∝ 1/(E_s δ_s/β_s), R11); weights
  *   are normalised per block; γ keeps ONE normalisation for the whole detector (block mean of Σ_s f_s γ_s = 1).  The energies,
  *   L, pixel and options are the plan's.  n_blocks = 1 is the uniform spectrum ("single block", §9.2).  After this call the
- *   plan runs the general path (see epr_plan); epr_set_diagnostics and opt.nonlocal_wkb1 are not available on it.
+ *   plan runs the general path (see epr_plan); every option and entry point stays available (opt.nonlocal_wkb1 takes the
+ *   WKB1 term at the detector pixel's column, epr_set_diagnostics the shift of the pixel's own column).
  *   Synchronises the device. */
 epr_status epr_plan_profiles(epr_plan_t plan, int n_blocks, const double* weight, const double* delta_over_beta,
                              const double* mu_rel);

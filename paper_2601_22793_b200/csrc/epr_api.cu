@@ -256,7 +256,6 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
   const bool tuned_fft = nx % 2 == 0 && epr_fft_size_supported(nx) && epr_fft_size_supported(ny);
   const bool aligned = nx % 16 == 0 && ny % 16 == 0;
   if (!tuned_fft && !(epr_fftgen_supported(nx) && epr_fftgen_supported(ny))) return EPR_ESIZE;
-  if ((!tuned_fft || !aligned) && o.nonlocal_wkb1) return EPR_EINVAL;      // variant R4 exists on the tuned path only
 
   epr_plan_s* p = (epr_plan_s*)aligned_alloc(64, (sizeof(epr_plan_s) + 63) / 64 * 64);   // CUtensorMap members: 64-byte aligned
   if (!p) return EPR_ENOMEM;
@@ -433,8 +432,6 @@ extern "C" epr_status epr_plan_profiles(epr_plan_t p, int n_blocks, const double
   if (!weight || !delta_over_beta) FAIL(p, EPR_EINVAL, "epr_plan_profiles: NULL pointer");
   if (n_blocks < 1 || n_blocks > EPR_MAX_BLOCKS || p->nx % n_blocks != 0)
     FAIL(p, EPR_EINVAL, "epr_plan_profiles: n_blocks = %d must be in 1..%d and divide nx = %d", n_blocks, EPR_MAX_BLOCKS, p->nx);
-  if (p->opt.nonlocal_wkb1) FAIL(p, EPR_EINVAL, "epr_plan_profiles: opt.nonlocal_wkb1 is not available with an x-dependent spectrum");
-  if (p->diag) FAIL(p, EPR_EINVAL, "epr_plan_profiles: switch diagnostics off first (not available on the general path)");
   const int nb = p->n_bins;
   std::vector<double> f((size_t)n_blocks * nb), g((size_t)n_blocks * nb), db((size_t)n_blocks * nb);
   double G = 0;
@@ -538,6 +535,7 @@ extern "C" epr_status epr_forward(epr_plan_t p, int batch, const float* tau, flo
       } else {
         KL(p, K_SPLAT, cs, epr_gen_splat(p, nb, t, NULL, NULL, p->raymap + (size_t)b0 * p->n_bins * plane, (unsigned*)p->pred, cs));
         KL(p, K_SPLAT, cs, epr_gen_fix2float(p, nb, (unsigned*)p->pred, 0, cs));
+        if (p->opt.nonlocal_wkb1) KL(p, K_WKB1, cs, epr_gen_wkb1_sub(p, nb, t, p->pred, cs));
       }
       KL(p, K_PRED_OUT, cs, epr_gen_pred_out(p, nb, p->pred, Ps, Pb, cs));
       continue;
@@ -646,7 +644,7 @@ static cudaError_t gen_c2r(epr_plan_t p, int planes, const float2* spec, float* 
 
 // One pass of the loop over nb <= work_batch projections on the general path (same steps as retrieve_chunk).
 static epr_status retrieve_chunk_general(epr_plan_t p, int nb, const float* d, float* tau, int iterations, float step,
-                                         cudaStream_t cs) {
+                                         int b_first, cudaStream_t cs) {
   const size_t plane = (size_t)p->nx * p->ny;
   const int planes = nb * p->n_bins;
   const size_t bstride = (size_t)p->work_batch * plane;            // qblk[b] holds work_batch planes
@@ -669,15 +667,26 @@ static epr_status retrieve_chunk_general(epr_plan_t p, int nb, const float* d, f
       r = p->res;
     } else if (p->nx % 16 == 0 && p->ny % 16 == 0) {
       // 16-pixel-aligned grid: the tuned tile kernels, reading the per-column tables (a0 + a1-N + a2 fused, then a3)
-      KL(p, K_SPLAT, cs, epr_launch_splat_cols(p, nb, tau, p->res, p->n_bins == 1 ? 2 : 3, d, cs));
-      KL(p, K_GATHER, cs, epr_launch_gather_cols(p, nb, tau, p->res, p->res2, cs));
+      if (p->opt.nonlocal_wkb1) {                      // variant: splat, WKB1 term, then the separate residual kernel
+        KL(p, K_SPLAT, cs, epr_launch_splat_cols(p, nb, tau, p->pred, 0, NULL, cs));
+        KL(p, K_WKB1, cs, epr_gen_wkb1_sub(p, nb, tau, p->pred, cs));
+        KL(p, K_RESIDUAL, cs, epr_gen_residual(p, nb, d, p->pred, p->res, cs));
+      } else {
+        KL(p, K_SPLAT, cs, epr_launch_splat_cols(p, nb, tau, p->res, p->n_bins == 1 ? 2 : 3, d, cs));
+      }
       r = p->res2;
     } else {
       KL(p, K_SPLAT, cs, epr_gen_splat(p, nb, tau, NULL, NULL, NULL, (unsigned*)p->res, cs));   // a0 + a1-N
       KL(p, K_SPLAT, cs, epr_gen_fix2float(p, nb, (unsigned*)p->res, 0, cs));
+      if (p->opt.nonlocal_wkb1) KL(p, K_WKB1, cs, epr_gen_wkb1_sub(p, nb, tau, p->res, cs));
       KL(p, K_RESIDUAL, cs, epr_gen_residual(p, nb, d, p->res, p->res, cs));                    // a2, in place
-      KL(p, K_GATHER, cs, epr_gen_gather(p, nb, tau, NULL, p->res, p->res2, cs));               // a3
       r = p->res2;
+    }
+    if (p->diag && it < p->diag_cap)                   // e_s are in p->res on every branch
+      KL(p, K_DIAG, cs, epr_gen_diagnostics(p, nb, tau, p->res, p->diag + ((size_t)b_first * p->diag_cap + it) * 2, p->diag_cap * 2, cs));
+    if (p->solver != EPR_LOCAL) {                      // a3
+      if (p->nx % 16 == 0 && p->ny % 16 == 0) KL(p, K_GATHER, cs, epr_launch_gather_cols(p, nb, tau, p->res, p->res2, cs));
+      else KL(p, K_GATHER, cs, epr_gen_gather(p, nb, tau, NULL, p->res, p->res2, cs));
     }
     KL(p, K_ROWS_R2C, cs, gen_r2c(p, planes, r, 0.f, cs));                                      // a4
     const int st2 = cols_staged(p) ? 2 : 0;
@@ -696,7 +705,7 @@ static epr_status retrieve_chunk_general(epr_plan_t p, int nb, const float* d, f
 // b_first: index of the chunk's first projection within the caller's batch (row of the diagnostics array).
 static epr_status retrieve_chunk(epr_plan_t p, int nb, const float* d, float* tau, int iterations, float step,
                                  int b_first, cudaStream_t cs) {
-  if (p->general) return retrieve_chunk_general(p, nb, d, tau, iterations, step, cs);
+  if (p->general) return retrieve_chunk_general(p, nb, d, tau, iterations, step, b_first, cs);
   const size_t plane = (size_t)p->nx * p->ny;
   const int planes = nb * p->n_bins;
   if (p->opt.init == 0) {
@@ -771,12 +780,11 @@ extern "C" epr_status epr_shift_histogram(epr_plan_t p, int batch, const float* 
 extern "C" epr_status epr_set_diagnostics(epr_plan_t p, float* diag, int capacity_iters) {
   if (!p) return EPR_EINVAL;
   DevGuard dg(p);
-  if (diag && p->general) FAIL(p, EPR_EINVAL, "epr_set_diagnostics: not available on the general path (x-dependent spectrum or unaligned grid)");
   if (diag && capacity_iters < 1) FAIL(p, EPR_EINVAL, "epr_set_diagnostics: capacity_iters must be >= 1");
   if (diag) {
     cudaError_t e = cudaSuccess;
-    if (!p->diag_partial) e = cudaMalloc((void**)&p->diag_partial, (size_t)p->work_batch * 64 * sizeof(double));
-    if (e == cudaSuccess && !p->gmax)
+    if (!p->diag_partial) e = cudaMalloc((void**)&p->diag_partial, (size_t)p->work_batch * 128 * sizeof(double));   // 64 x {Σe², max}
+    if (e == cudaSuccess && !p->gmax && !p->general)
       e = cudaMalloc((void**)&p->gmax, (size_t)p->work_batch * (p->nx / 16) * (p->ny / 16) * sizeof(float));
     if (e != cudaSuccess) FAIL(p, e == cudaErrorMemoryAllocation ? EPR_ENOMEM : EPR_ECUDA, "diagnostics buffers: %s", cudaGetErrorString(e));
   }

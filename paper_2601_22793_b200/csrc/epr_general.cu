@@ -28,8 +28,10 @@ static inline dim3 gn_grid(const epr_plan_s* p, int nz) { return dim3((p->nx + 2
 //   A = exp(−γτ/2) = 1 + Ad, Î = A², J = Ad(2 + Ad), g = −γ D⁰τ, Q = ∇²₅A / A; neighbour values formed with the centre's γ.
 // One thread = one pixel, every line; τ tile + 2 in shared memory.
 // =====================================================================================================
+// term_only (variant of reading R4, opt.nonlocal_wkb1): pred −= f_s(x)(α²/4) Σ_i D⁻_i(Ī_i D⁺_i Q) alone — the WKB1 term
+// added to the ray-map prediction as the same LOCAL term ("when complemented by the second-order corrections").
 __global__ void __launch_bounds__(GN_TX * GN_TY) k_gen_local(EprLines L, EprColumns C, int nx, int ny, int order, int wkb1,
-                                                            const float* __restrict__ tau, float* __restrict__ pred) {
+                                                            int term_only, const float* __restrict__ tau, float* pred) {
   __shared__ float s_t[GN_TY + 4][GN_TX + 4];
   const int tid = threadIdx.y * GN_TX + threadIdx.x, b = blockIdx.z;
   const int x0 = blockIdx.x * GN_TX, y0 = blockIdx.y * GN_TY;
@@ -79,8 +81,8 @@ __global__ void __launch_bounds__(GN_TX * GN_TY) k_gen_local(EprLines L, EprColu
     auto J = [&](int dy, int dx) { const float v = A[dy + 2][dx + 2]; return v * (2.f + v); };
     auto Ih = [&](int dy, int dx) { const float v = 1.f + A[dy + 2][dx + 2]; return v * v; };
     const float J0 = J(0, 0);
-    float v = J0 - a * (((J(0, 1) - J0) + (J(0, -1) - J0)) + ((J(1, 0) - J0) + (J(-1, 0) - J0)));
-    if (o2) {
+    float v = term_only ? 0.f : J0 - a * (((J(0, 1) - J0) + (J(0, -1) - J0)) + ((J(1, 0) - J0) + (J(-1, 0) - J0)));
+    if (o2 && !term_only) {
       auto tx = [&](int dy, int dx) { return t[dy + 2][dx + 3] - t[dy + 2][dx + 1]; };
       auto ty = [&](int dy, int dx) { return t[dy + 3][dx + 2] - t[dy + 1][dx + 2]; };
       auto Sxx = [&](int dx) { const float g = tx(0, dx); return Ih(0, dx) * g * g; };
@@ -90,24 +92,31 @@ __global__ void __launch_bounds__(GN_TX * GN_TY) k_gen_local(EprLines L, EprColu
       const float d2x = (Sxx(1) - sx0) - (sx0 - Sxx(-1)), d2y = (Syy(1) - sy0) - (sy0 - Syy(-1));
       const float cross = 0.5f * ((Sxy(1, 1) - Sxy(1, -1)) - (Sxy(-1, 1) - Sxy(-1, -1)));
       v = fmaf(c2, d2x + d2y + cross, v);
-      if (wk) {
-        auto Q = [&](int dy, int dx) {
-          const float ac = A[dy + 2][dx + 2];
-          return __fdividef(((A[dy + 2][dx + 3] - ac) + (A[dy + 2][dx + 1] - ac)) + ((A[dy + 3][dx + 2] - ac) + (A[dy + 1][dx + 2] - ac)), 1.f + ac);
-        };
-        const float Q0 = Q(0, 0), I0 = Ih(0, 0);
-        const float fxp = 0.5f * (Ih(0, 1) + I0) * (Q(0, 1) - Q0), fxm = 0.5f * (I0 + Ih(0, -1)) * (Q0 - Q(0, -1));
-        const float fyp = 0.5f * (Ih(1, 0) + I0) * (Q(1, 0) - Q0), fym = 0.5f * (I0 + Ih(-1, 0)) * (Q0 - Q(-1, 0));
-        v = fmaf(-q4, (fxp - fxm) + (fyp - fym), v);
-      }
     }
-    pred[((size_t)b * L.n_bins + s) * plane + (size_t)y * nx + x] = fs * v;
+    if (wk) {
+      auto Q = [&](int dy, int dx) {
+        const float ac = A[dy + 2][dx + 2];
+        return __fdividef(((A[dy + 2][dx + 3] - ac) + (A[dy + 2][dx + 1] - ac)) + ((A[dy + 3][dx + 2] - ac) + (A[dy + 1][dx + 2] - ac)), 1.f + ac);
+      };
+      const float Q0 = Q(0, 0), I0 = Ih(0, 0);
+      const float fxp = 0.5f * (Ih(0, 1) + I0) * (Q(0, 1) - Q0), fxm = 0.5f * (I0 + Ih(0, -1)) * (Q0 - Q(0, -1));
+      const float fyp = 0.5f * (Ih(1, 0) + I0) * (Q(1, 0) - Q0), fym = 0.5f * (I0 + Ih(-1, 0)) * (Q0 - Q(-1, 0));
+      v = fmaf(-q4, (fxp - fxm) + (fyp - fym), v);
+    }
+    float* o = pred + ((size_t)b * L.n_bins + s) * plane + (size_t)y * nx + x;
+    *o = term_only ? fmaf(fs, v, *o) : fs * v;
   }
 }
 
 cudaError_t epr_gen_forward_local(const epr_plan_s* p, int batch, const float* tau, float* pred, cudaStream_t st) {
   dim3 grid((p->nx + GN_TX - 1) / GN_TX, (p->ny + GN_TY - 1) / GN_TY, batch), blk(GN_TX, GN_TY);
-  k_gen_local<<<grid, blk, 0, st>>>(p->lines, p->cols, p->nx, p->ny, p->opt.order, p->opt.wkb1, tau, pred);
+  k_gen_local<<<grid, blk, 0, st>>>(p->lines, p->cols, p->nx, p->ny, p->opt.order, p->opt.wkb1, 0, tau, pred);
+  return cudaGetLastError();
+}
+
+cudaError_t epr_gen_wkb1_sub(const epr_plan_s* p, int batch, const float* tau, float* pred, cudaStream_t st) {
+  dim3 grid((p->nx + GN_TX - 1) / GN_TX, (p->ny + GN_TY - 1) / GN_TY, batch), blk(GN_TX, GN_TY);
+  k_gen_local<<<grid, blk, 0, st>>>(p->lines, p->cols, p->nx, p->ny, 2, 1, 1, tau, pred);
   return cudaGetLastError();
 }
 
@@ -508,5 +517,75 @@ cudaError_t epr_launch_shift_hist(const epr_plan_s* p, int batch, const float* t
   dim3 grid((p->nx + 63) / 64, (p->ny + 3) / 4, batch);
   k_shift_hist<<<grid, 256, (size_t)p->n_bins * n_hist * sizeof(unsigned), st>>>(p->lines, p->cols, p->general, p->nx, p->ny, n_hist,
                                                                                   1.f / bin_px, tau, hist);
+  return cudaGetLastError();
+}
+
+// =====================================================================================================
+// Diagnostics of the loop on the general path (epr_set_diagnostics; never in timed runs): per projection, the RMS of the
+// detector residual e = Σ_s e_s and the regime indicator as the largest UNCLAMPED shift
+// component max_s a_s(x) γ_s(x) · max(|D⁰xτ|, |D⁰yτ|) with the scalars of the pixel's own column (R17(b)).
+// Two launches, fixed summation order (bit-reproducible): 64 partial sums / maxima per projection, then one thread each.
+// =====================================================================================================
+#define GD_BLK 64
+__global__ void __launch_bounds__(256) k_gen_diag_partial(int n_bins, EprColumns C, int nx, int ny, const float* __restrict__ tau,
+                                                          const float* __restrict__ es, double* __restrict__ partial) {
+  __shared__ double s_sum[256];
+  __shared__ float s_max[256];
+  const int b = blockIdx.y;
+  const size_t plane = (size_t)nx * ny;
+  const float* tb = tau + (size_t)b * plane;
+  const float* eb = es + (size_t)b * n_bins * plane;
+  double acc = 0.0;
+  float m = 0.f;
+  for (int x = threadIdx.x; x < nx; x += 256) {
+    float c = 0.f;
+    for (int s = 0; s < n_bins; ++s) c = fmaxf(c, __ldg(&C.a[(size_t)s * nx + x]) * __ldg(&C.gamma[(size_t)s * nx + x]));
+    const int xm = x == 0 ? nx - 1 : x - 1, xp = x + 1 == nx ? 0 : x + 1;
+    for (int y = blockIdx.x; y < ny; y += GD_BLK) {
+      const int ym = y == 0 ? ny - 1 : y - 1, yp = y + 1 == ny ? 0 : y + 1;
+      const size_t i = (size_t)y * nx + x;
+      float e = 0.f;
+      for (int s = 0; s < n_bins; ++s) e += __ldg(eb + (size_t)s * plane + i);
+      acc += (double)e * e;
+      const float dtx = __ldg(tb + (size_t)y * nx + xp) - __ldg(tb + (size_t)y * nx + xm);
+      const float dty = __ldg(tb + (size_t)yp * nx + x) - __ldg(tb + (size_t)ym * nx + x);
+      m = fmaxf(m, 0.5f * c * fmaxf(fabsf(dtx), fabsf(dty)));
+    }
+  }
+  s_sum[threadIdx.x] = acc;
+  s_max[threadIdx.x] = m;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (threadIdx.x < o) {
+      s_sum[threadIdx.x] += s_sum[threadIdx.x + o];
+      s_max[threadIdx.x] = fmaxf(s_max[threadIdx.x], s_max[threadIdx.x + o]);
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    partial[((size_t)b * GD_BLK + blockIdx.x) * 2] = s_sum[0];
+    partial[((size_t)b * GD_BLK + blockIdx.x) * 2 + 1] = (double)s_max[0];
+  }
+}
+
+__global__ void __launch_bounds__(32) k_gen_diag_reduce(int batch, size_t plane, const double* __restrict__ partial,
+                                                        float* __restrict__ diag, int stride) {
+  const int b = blockIdx.x * 32 + threadIdx.x;
+  if (b >= batch) return;
+  double sum = 0.0, m = 0.0;
+  for (int i = 0; i < GD_BLK; ++i) {
+    sum += partial[((size_t)b * GD_BLK + i) * 2];
+    m = fmax(m, partial[((size_t)b * GD_BLK + i) * 2 + 1]);
+  }
+  diag[(size_t)b * stride] = (float)sqrt(sum / (double)plane);
+  diag[(size_t)b * stride + 1] = (float)m;
+}
+
+// partial: [batch][GD_BLK][2] doubles (epr_set_diagnostics allocates it)
+cudaError_t epr_gen_diagnostics(const epr_plan_s* p, int batch, const float* tau, const float* es, float* diag, int stride,
+                                cudaStream_t st) {
+  epr_note_extra_launch(p);                              // two kernels
+  k_gen_diag_partial<<<dim3(GD_BLK, batch), 256, 0, st>>>(p->n_bins, p->cols, p->nx, p->ny, tau, es, p->diag_partial);
+  k_gen_diag_reduce<<<(batch + 31) / 32, 32, 0, st>>>(batch, (size_t)p->nx * p->ny, p->diag_partial, diag, stride);
   return cudaGetLastError();
 }

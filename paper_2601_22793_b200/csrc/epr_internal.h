@@ -172,6 +172,11 @@ cudaError_t epr_launch_output(const epr_plan_s* p, int batch, const float* tau, 
 // ---- general path (epr_general.cu / epr_fftgen.cu) ----
 // a1-L: pred[b][s] = P_s − f_s(x), every line, per-column scalars frozen at the centre column (R17(b))
 cudaError_t epr_gen_forward_local(const epr_plan_s* p, int batch, const float* tau, float* pred, cudaStream_t st);
+// variant of R4 (opt.nonlocal_wkb1): pred[b][s] −= f_s(x)(α_s²/4) ∂i(Î ∂iQ) with the centre column's scalars
+cudaError_t epr_gen_wkb1_sub(const epr_plan_s* p, int batch, const float* tau, float* pred, cudaStream_t st);
+// diagnostics (epr_set_diagnostics): diag[b·stride + {0, 1}] = residual RMS of Σ_s es[b][s], largest unclamped shift component
+cudaError_t epr_gen_diagnostics(const epr_plan_s* p, int batch, const float* tau, const float* es, float* diag, int stride,
+                                cudaStream_t st);
 // a1-N: acc[b][s] (u32 fixed point, zeroed here) += splat of line s; sources from τ (I_bins NULL; the ray map goes to map_out if
 // given) or from I_bins with the stored map_in (epr_transport)
 cudaError_t epr_gen_splat(const epr_plan_s* p, int batch, const float* tau, const float* I_bins, const float2* map_in,

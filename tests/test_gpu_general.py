@@ -310,3 +310,90 @@ def test_profiles_on_the_oversampled_grid_and_graph_replay(E):
                 side.synchronize()
                 assert torch.equal(out, ref)
         plan.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# variants on the general path: opt.nonlocal_wkb1 (R4) and epr_set_diagnostics
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nx,ny,blocks", [(90, 150, 0), (96, 160, 4), (90, 150, 3)])
+def test_nonlocal_wkb1_variant_general_path(E, nx, ny, blocks):
+    """opt.nonlocal_wkb1 (variant of R4) on a grid the tuned kernels do not take (blocks = 0: uniform
+    spectrum) and with block profiles on an aligned and on an unaligned grid: the WKB1 term of Eq. (1) at the detector
+    pixel's column (oracle: forward / forward_x with nonlocal_wkb1), at a δ/β small enough for the term to matter."""
+    import torch
+    S, L = 8.0, 20.0
+    en, wt, db = np.array([80.0, 100.0, 120.0]), np.array([0.3, 0.4, 0.3]), np.array([8.0, 10.0, 12.0])
+    tau = _tau_field(ny, nx, 5, amp=0.3)[None]
+    plan = E.epr_plan(nx, ny, 6.5e-6, L, en, wt, db, "nonlocal", max_batch=1, max_shift_px=S, nonlocal_wkb1=1)
+    if blocks:
+        t = np.linspace(0.0, 1.0, blocks)[:, None]
+        wb, dbb = wt[None, :] * (1.0 + t * np.array([0.5, 0.0, -0.4])[None, :]), db[None, :] * (1.0 + 0.3 * t)
+        E.epr_plan_profiles(plan, wb, dbb, None)
+        prof = O.derive_profiles(6.5e-6, L, en, nx, wb, dbb)
+        fwd = lambda t64, **kw: O.forward_x(t64, prof, "nonlocal", S=S, **kw)
+        ret = lambda d64: O.retrieve_x(d64, prof, "nonlocal", 4, 0.4, S=S, nonlocal_wkb1=True)
+    else:
+        lines = O.derive_lines(6.5e-6, L, en, wt, db)
+        fwd = lambda t64, **kw: O.forward(t64, lines, "nonlocal", S=S, **kw)
+        ret = lambda d64: O.retrieve(d64, lines, "nonlocal", 4, 0.4, S=S, nonlocal_wkb1=True)
+    P = torch.empty((1, ny, nx), device="cuda")
+    Pb = torch.empty((1, 3, ny, nx), device="cuda")
+    E.epr_forward(plan, _dev(tau), P, Pb)
+    ref, ref_bins, _ = fwd(tau[0].astype(np.float64), nonlocal_wkb1=True)
+    plain, _, _ = fwd(tau[0].astype(np.float64))
+    assert rel_l2(ref, plain) > 100 * TOL_OP                         # the term is far above the tolerance here
+    assert_close(P.cpu().numpy()[0], ref, TOL_OP)
+    for s in range(3):
+        assert_close(Pb.cpu().numpy()[0, s], ref_bins[s], TOL_OP)
+    d = np.float32(ref + 0.002 * np.random.default_rng(3).normal(size=ref.shape))[None]
+    out = torch.empty((1, ny, nx), device="cuda")
+    E.epr_retrieve(plan, _dev(d), out, 4, 0.4)
+    plan.destroy()
+    assert_close(out.cpu().numpy()[0], ret(d[0].astype(np.float64)), TOL_PHASE)
+
+
+@pytest.mark.parametrize("nx,ny,blocks,solver,step,L", [(90, 150, 0, "local", 1.0, 0.3), (90, 150, 0, "nonlocal", 0.4, 8.0),
+                                                         (160, 96, 5, "local", 1.0, 0.3), (160, 96, 5, "nonlocal", 0.4, 8.0),
+                                                         (150, 90, 5, "nonlocal", 0.4, 8.0)])
+def test_diagnostics_general_path(E, nx, ny, blocks, solver, step, L):
+    """epr_set_diagnostics on the general path: residual RMS and largest unclamped shift per iteration against the oracle's
+    histories, uniform spectrum on an unaligned grid and block profiles (shift with the scalars of the
+    pixel's own column); the host path writes every chunk into its own rows; switching it off restores the plain result."""
+    import torch
+    its, S = 4, 6.0
+    if blocks:
+        en, wt, db, mu_rel, prof = _profiles(nx, blocks, L, 3, True)
+        w0, db0 = wt[0], db[0]
+    else:
+        en, w0, db0 = E3, W3, DB3
+        lines = O.derive_lines(6.5e-6, L, en, w0, db0)
+    d = np.stack([_data(ny, nx, 11), _data(ny, nx, 12, amp=0.2)])
+    plan = E.epr_plan(nx, ny, 6.5e-6, L, en, w0, db0, solver, max_batch=2, max_shift_px=S)
+    if blocks:
+        E.epr_plan_profiles(plan, wt, db, mu_rel)
+    dd = _dev(d)
+    out = torch.empty_like(dd)
+    diag = torch.zeros(2, its, 2, device="cuda")
+    E.epr_set_diagnostics(plan, diag)
+    E.epr_retrieve(plan, dd, out, its, step)
+    got = diag.cpu().numpy()
+    diag_h = torch.zeros_like(diag)
+    E.epr_set_diagnostics(plan, diag_h)
+    dh = torch.from_numpy(d).pin_memory()
+    oh = torch.empty_like(dh).pin_memory()
+    E.epr_retrieve_host(plan, dh, oh, its, step)
+    assert torch.equal(diag_h, diag) and torch.equal(oh.cuda(), out)
+    E.epr_set_diagnostics(plan, None)
+    out2 = torch.empty_like(dd)
+    E.epr_retrieve(plan, dd, out2, its, step)
+    assert torch.equal(out, out2)
+    plan.destroy()
+    for j in range(2):
+        h, sh = [], []
+        if blocks:
+            O.retrieve_x(d[j].astype(np.float64), prof, solver, its, step, S=S, history=h, shift_history=sh)
+        else:
+            O.retrieve(d[j].astype(np.float64), lines, solver, its, step, S=S, history=h, shift_history=sh)
+        h, sh = np.array(h), np.array(sh)
+        assert np.max(np.abs(got[j, :, 0] - h)) < 2e-3 * h[0]          # e is a small difference of O(1) planes in fp32
+        assert np.max(np.abs(got[j, :, 1] - sh) / sh) < 1e-3
