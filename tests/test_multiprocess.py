@@ -81,3 +81,10 @@ def test_bench_reference_arm_contract():
     other = _run_bench({"RANK": "1", "WORLD_SIZE": "2", "LOCAL_RANK": "1"}, "--impl", "reference", "--config", "C1",
                        "--gpus", "2", "--steps", "1", "--warmup", "0")
     assert other.returncode == 0 and other.stdout.strip() == ""
+    # a budget too small for whole projections: each step runs the first iterations only and says so
+    res = _run_bench({"RANK": "0", "WORLD_SIZE": "1"}, "--impl", "reference", "--config", "C1", "--steps", "3", "--warmup", "1",
+                     "--ref-budget", "0.01")
+    assert res.returncode == 0, res.stderr[-2000:]
+    j = json.loads(res.stdout.strip())
+    assert j["config"]["iterations_run_per_step"] == 1 and "extrapolated" in j["cpu_baseline"]["sample"]
+    assert j["value"] > 0 and j["config"]["ms_per_projection_extrapolated"] > j["ms_per_step"]
