@@ -202,6 +202,35 @@ long long epr_launch_count(epr_plan_t plan);
 epr_status epr_profile_enable(epr_plan_t plan, int on);
 int epr_profile_read(epr_plan_t plan, int max_kernels, const char** names, double* total_ms, long long* count, int reset);
 
+/* epr_residual_rms_static — the residual RMS of epr_set_diagnostics without a plan and WITHOUT ANY ALLOCATION
+ *                                                                                              PAPER.md:231, 95
+ *   rms[b] = sqrt( mean over the ny·nx pixels of ( Σ_s e_bins[b][s] )² ) — for e_s the per-line residuals of one loop
+ *   iteration (their sum is the detector residual e = d − Σ_s P_s, "form the detector residual" PAPER.md:231) this is
+ *   diag[b][n][0] of epr_set_diagnostics, the quantity whose decay over n is the convergence history of PAPER.md:95.
+ *   Pass n_bins = 1 to take the RMS of a plane that is already summed.
+ *     e_bins [batch][n_bins][ny][nx]  DEVICE in;   rms [batch]  DEVICE out;   1 <= n_bins <= 16;  nx·ny < 2^32, any shape.
+ * For whom: callers that cannot call cudaMalloc where they want this number — a monitoring hook inside a process whose
+ *   device memory has all been given to one pool (the reconstruction framework's allocator, or plans sized at start-up),
+ *   where a late cudaMalloc fails or fragments that pool; and acquisition-rate loops, which cannot take the device-wide
+ *   stall a cudaMalloc / cudaFree may cause.  The plan-based diagnostic allocates its reduction scratch on first use;
+ *   this call does not: it calls no cudaMalloc, cudaFree or any library routine that allocates, needs no plan, and only
+ *   enqueues two kernels on `stream`.
+ * How: the scratch (64 doubles per projection) lives in a fixed array inside libepr.so, sized for EPR_STATIC_MAX_BATCH
+ *   projections = 512 KiB.  Each GPU that loads this library's code holds its own copy of those 512 KiB until the process
+ *   ends.  batch > EPR_STATIC_MAX_BATCH returns EPR_ESIZE (nothing enqueued); split larger batches into several calls.
+ * Device and first call: the call works on the CURRENT device, which must own e_bins and rms (EPR_EINVAL otherwise).  The
+ *   first call on each device looks up where the array sits on that device and remembers it; that first call is also
+ *   when the runtime may load the library's code onto the device, so make it once during set-up, before any stream
+ *   capture and before the latency-critical part of the run.  Later calls on that device do no set-up.
+ * Shared scratch: all calls on a device use the same array, and it keeps whatever the previous call left there.  Nothing in
+ *   it needs to be zero (every slot a call reads it has written first), so back-to-back calls on ONE stream are safe; two
+ *   calls whose kernels may overlap on the GPU — different streams without an event between them, or different host
+ *   threads — race on the array and return garbage.  Order them yourself.
+ * Errors: epr_static_last_error() gives the message of the last failed epr_residual_rms_static of the calling thread. */
+#define EPR_STATIC_MAX_BATCH 1024
+epr_status epr_residual_rms_static(int batch, int n_bins, int nx, int ny, const float* e_bins, float* rms, void* stream);
+const char* epr_static_last_error(void);
+
 epr_status epr_destroy(epr_plan_t plan);
 const char* epr_last_error(epr_plan_t plan);
 const char* epr_version(void);

@@ -15,7 +15,8 @@ EXPORTS = ["epr_default_options", "epr_plan", "epr_forward", "epr_adjoint", "epr
            "epr_retrieve", "epr_retrieve_oversampled", "epr_set_diagnostics", "epr_retrieve_host", "epr_plan_lines", "epr_launch_count", "epr_destroy",
            "epr_last_error", "epr_version", "epr_profile_enable", "epr_profile_read", "epr_read_flags",
            "epr_plan_profiles", "epr_plan_columns", "epr_shift_histogram",
-           "epr_retrieve_oversampled_host"]
+           "epr_retrieve_oversampled_host", "epr_residual_rms_static", "epr_static_last_error"]
+EPR_STATIC_MAX_BATCH = 1024
 EPR_FLAG_SPLAT_OVERFLOW = 1
 
 
@@ -76,6 +77,10 @@ def load_library():
     lib.epr_shift_histogram.restype = ci
     lib.epr_read_flags.argtypes = [vp, C.POINTER(C.c_uint), ci]
     lib.epr_read_flags.restype = ci
+    lib.epr_residual_rms_static.argtypes = [ci, ci, ci, ci, vp, vp, vp]
+    lib.epr_residual_rms_static.restype = ci
+    lib.epr_static_last_error.argtypes = []
+    lib.epr_static_last_error.restype = C.c_char_p
     lib.epr_last_error.argtypes = [vp]
     lib.epr_last_error.restype = C.c_char_p
     lib.epr_version.restype = C.c_char_p
@@ -261,6 +266,23 @@ def epr_shift_histogram(plan, tau, n_hist, bin_px):
     plan._check(load_library().epr_shift_histogram(plan._h, b, _dev(tau, (b, plan.ny, plan.nx), "tau"), int(n_hist), float(bin_px),
                                                    C.c_void_p(hist.data_ptr()), _stream()))
     return hist
+
+
+def epr_residual_rms_static(e_bins, rms):
+    """epr_residual_rms_static of include/epr.h: RMS over the pixels of Σ_s e_bins[b][s], written to rms[b].
+
+    For callers that must not allocate device memory (all of it already belongs to a pool, or a cudaMalloc stall is not
+    acceptable in the loop): the reduction scratch is a fixed 512 KiB array inside libepr.so, so neither the library nor
+    this wrapper allocates — `rms` ([batch], float32, CUDA) is the caller's, like `e_bins` ([batch][n_bins][ny][nx]).
+    batch <= EPR_STATIC_MAX_BATCH.  Runs on the current device and torch's current stream; calls share the scratch, so
+    keep them on one stream (or order them with events).  Make the first call on a device during set-up."""
+    if e_bins.dim() != 4:
+        raise ValueError("e_bins: expected [batch][n_bins][ny][nx]")
+    b, n_bins, ny, nx = (int(v) for v in e_bins.shape)
+    st = load_library().epr_residual_rms_static(b, n_bins, nx, ny, _dev(e_bins, None, "e_bins"), _dev(rms, (b,), "rms"),
+                                                 _stream())
+    if st != 0:
+        raise EprError(st, load_library().epr_static_last_error().decode())
 
 
 def epr_set_diagnostics(plan, diag):

@@ -16,7 +16,8 @@ LIB = os.path.join(HERE, "libepr.so")
 FFT_GROUPS = 11
 # (source, object stem, extra flags)
 UNITS = [("epr_api.cu", "epr_api", []), ("epr_kernels.cu", "epr_kernels", []), ("epr_fftd.cu", "epr_fftd", []),
-         ("epr_general.cu", "epr_general", []), ("epr_fftgen.cu", "epr_fftgen", [])] + \
+         ("epr_general.cu", "epr_general", []), ("epr_fftgen.cu", "epr_fftgen", []),
+         ("epr_static.cu", "epr_static", [])] + \
         [("epr_fftk.cu", f"epr_fftk_g{g}", [f"-DEPR_FFT_GROUP={g}"]) for g in range(FFT_GROUPS)]
 HEADERS = ["epr_internal.h", "epr_math.cuh", "epr_fft.cuh", "epr_tma.cuh", os.path.join("..", "..", "include", "epr.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
