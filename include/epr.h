@@ -33,7 +33,7 @@ typedef struct epr_plan_s* epr_plan_t;
 typedef enum {
   EPR_OK = 0,
   EPR_EINVAL = 1, /* bad argument (NULL pointer, non-positive size / energy / weight / step, batch > max_batch …) */
-  EPR_ESIZE = 2,  /* unsupported grid: nx or ny has a prime factor other than 2, 3, 5, or exceeds 8192 (see epr_plan) */
+  EPR_ESIZE = 2,  /* unsupported grid: nx or ny below 8, with a prime factor other than 2, 3, 5, or above 8192 (see epr_plan) */
   EPR_ECUDA = 3,  /* a CUDA runtime call failed; message in epr_last_error */
   EPR_ENOMEM = 4  /* device allocation failed */
 } epr_status;
@@ -166,7 +166,11 @@ epr_status epr_retrieve_host(epr_plan_t plan, int batch, const float* d_host, fl
  *   L, pixel and options are the plan's.  n_blocks = 1 is the uniform spectrum ("single block", §9.2).  After this call the
  *   plan runs the general path (see epr_plan); every option and entry point stays available (opt.nonlocal_wkb1 takes the
  *   WKB1 term at the detector pixel's column, epr_set_diagnostics the shift of the pixel's own column).
- *   Synchronises the device. */
+ *   Synchronises the device.  A ray map stored by an earlier epr_forward is dropped (call epr_forward again before
+ *   epr_adjoint / epr_transport); epr_plan_lines keeps returning the uniform scalars of epr_plan — read the ones in use with
+ *   epr_plan_columns.  The filter workspace (n_blocks planes per projection of the work batch) is allocated here; when it does
+ *   not fit, the plan's work batch is halved until it does (larger batches simply take more passes).  If the call fails
+ *   (EPR_ENOMEM, EPR_ECUDA) the plan is unchanged and stays usable with its previous spectrum. */
 epr_status epr_plan_profiles(epr_plan_t plan, int n_blocks, const double* weight, const double* delta_over_beta,
                              const double* mu_rel);
 
@@ -189,7 +193,8 @@ epr_status epr_read_flags(epr_plan_t plan, unsigned* flags, int clear);
 epr_status epr_retrieve_oversampled_host(epr_plan_t plan, int factor, int batch, const float* d_host, float* out_host,
                                          int iterations, float step);
 
-/* Per-line scalars the plan derived (HOST arrays of length n_bins, any may be NULL): f_s, γ_s, a_s, α_s. */
+/* Per-line scalars epr_plan derived (HOST arrays of length n_bins, any may be NULL): f_s, γ_s, a_s, α_s.  Not changed by
+ * epr_plan_profiles (see there). */
 epr_status epr_plan_lines(epr_plan_t plan, double* f, double* gamma, double* a, double* alpha);
 
 /* Number of kernel launches the plan has enqueued so far (for bench.py's gpu_launches). */

@@ -162,10 +162,11 @@ static epr_status set_columns(epr_plan_s* p, int n_blocks, const double* f_blk, 
     w[(size_t)b0 * nx + x] = 1.0 - fr;
     w[(size_t)(b0 + 1) * nx + x] += fr;
   }
-  free(p->h_col);
-  p->h_col = (double*)malloc(sizeof(double) * 3 * nb * nx);
-  if (!p->h_col) FAIL(p, EPR_ENOMEM, "column tables");
-  double *hf = p->h_col, *hg = hf + (size_t)nb * nx, *ha = hg + (size_t)nb * nx;
+  // Everything new is built beside the old state and swapped in only when all of it exists: a failed allocation leaves
+  // the plan exactly as it was (old tables, old n_blocks, old workspace), still usable.
+  double* h_col_new = (double*)malloc(sizeof(double) * 3 * nb * nx);
+  if (!h_col_new) FAIL(p, EPR_ENOMEM, "column tables");
+  double *hf = h_col_new, *hg = hf + (size_t)nb * nx, *ha = hg + (size_t)nb * nx;
   for (int s = 0; s < nb; ++s)
     for (int x = 0; x < nx; ++x) {
       double f = 0, g = 0, db = 0;
@@ -194,10 +195,37 @@ static epr_status set_columns(epr_plan_s* p, int n_blocks, const double* f_blk, 
     ds[x] = (float)(fs - 1.0);
   }
   for (size_t i = 0; i < (size_t)n_blocks * nx; ++i) dw[i] = (float)w[i];
+  void* store_new = NULL;
+  float* qblk_new = NULL;
+  // the general path puts work_batch · n_bins planes into gridDim.y / .z (limit 65535): small grids with a huge batch
+  int work_new = p->work_batch;
+  if (work_new > 65535 / nb) work_new = 65535 / nb;
+  const bool need_q = !p->qblk || n_blocks > p->n_blocks;
+  cudaError_t ce = cudaMalloc(&store_new, host.size() * sizeof(float));
+  if (ce == cudaSuccess) ce = cudaMemcpy(store_new, host.data(), host.size() * sizeof(float), cudaMemcpyHostToDevice);
+  // block-filter workspace: n_blocks planes per projection of the work batch.  The plan's work batch was sized without
+  // it; when it does not fit, the work batch is halved until it does (batches are processed in passes of work_batch).
+  while (ce == cudaSuccess && need_q) {
+    ce = cudaMalloc((void**)&qblk_new, (size_t)n_blocks * work_new * nx * p->ny * sizeof(float));
+    if (ce != cudaErrorMemoryAllocation || work_new == 1) break;
+    cudaGetLastError();
+    ce = cudaSuccess;
+    work_new = (work_new + 1) / 2;
+  }
+  if (ce != cudaSuccess) {
+    cudaGetLastError();
+    cudaFree(store_new); cudaFree(qblk_new); free(h_col_new);
+    FAIL(p, ce == cudaErrorMemoryAllocation ? EPR_ENOMEM : EPR_ECUDA, "column tables / block-filter workspace (%d blocks): %s",
+         n_blocks, cudaGetErrorString(ce));
+  }
+  if (p->graph_exec) { cudaGraphExecDestroy(p->graph_exec); p->graph_exec = NULL; }   // it references the old tables
+  free(p->h_col);
+  p->h_col = h_col_new;
   cudaFree(p->cols_store);
-  p->cols_store = NULL;
-  CU(p, cudaMalloc(&p->cols_store, host.size() * sizeof(float)));
-  CU(p, cudaMemcpy(p->cols_store, host.data(), host.size() * sizeof(float), cudaMemcpyHostToDevice));
+  p->cols_store = store_new;
+  if (need_q) { cudaFree(p->qblk); p->qblk = qblk_new; }
+  p->work_batch = work_new;
+  p->raymap_batch = 0;                                 // a stored ray map belongs to the previous scalars
   float* base = (float*)p->cols_store;
   p->cols.f = base; p->cols.gamma = base + n1; p->cols.a = base + 2 * n1; p->cols.fixCorr = base + 3 * n1;
   p->cols.fixFi = reinterpret_cast<const unsigned*>(base + 4 * n1);
@@ -219,12 +247,6 @@ static epr_status set_columns(epr_plan_s* p, int n_blocks, const double* f_blk, 
     }
     p->abar_blk[b] = (float)abar;
   }
-  if (!p->qblk || n_blocks > p->n_blocks) {
-    cudaFree(p->qblk);
-    p->qblk = NULL;
-    cudaError_t e = cudaMalloc((void**)&p->qblk, (size_t)n_blocks * p->work_batch * nx * p->ny * sizeof(float));
-    if (e != cudaSuccess) FAIL(p, e == cudaErrorMemoryAllocation ? EPR_ENOMEM : EPR_ECUDA, "block-filter workspace: %s", cudaGetErrorString(e));
-  }
   p->n_blocks = n_blocks;
   p->general = 1;
   return EPR_OK;
@@ -238,7 +260,8 @@ extern "C" epr_status epr_plan(epr_plan_t* out, int nx, int ny, double pixel_m, 
   if (!energy_keV || !weight || !delta_over_beta) return EPR_EINVAL;
   if (n_bins < 1 || n_bins > EPR_MAX_BINS || max_batch < 1 || !(pixel_m > 0) || !(L_m > 0)) return EPR_EINVAL;
   if (solver != EPR_LOCAL && solver != EPR_NONLOCAL) return EPR_EINVAL;
-  if (nx < 8 || ny < 8) return EPR_EINVAL;
+  if (nx < 1 || ny < 1) return EPR_EINVAL;
+  if (nx < 8 || ny < 8) return EPR_ESIZE;              // include/epr.h: grids below 8 are unsupported sizes
   double wsum = 0;
   for (int s = 0; s < n_bins; ++s) {
     if (!(energy_keV[s] > 0) || !(weight[s] > 0) || !(delta_over_beta[s] > 0)) return EPR_EINVAL;

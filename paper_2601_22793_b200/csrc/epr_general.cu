@@ -484,11 +484,12 @@ cudaError_t epr_gen_output(const epr_plan_s* p, int batch, const float* tau, flo
 // scalars come from the column tables when the plan has them, from the uniform per-line scalars otherwise.
 // One thread = one pixel; counts are collected per CTA in shared memory first.
 // =====================================================================================================
-__global__ void __launch_bounds__(256) k_shift_hist(EprLines L, EprColumns C, int use_cols, int nx, int ny, int n_hist,
-                                                    float inv_bin, const float* __restrict__ tau, unsigned* __restrict__ hist) {
-  extern __shared__ unsigned s_h[];                     // [n_bins][n_hist]
+__global__ void __launch_bounds__(256) k_shift_hist(EprLines L, EprColumns C, int use_cols, int nx, int ny, int n_hist, int s0,
+                                                    int ns, float inv_bin, const float* __restrict__ tau,
+                                                    unsigned* __restrict__ hist) {
+  extern __shared__ unsigned s_h[];                     // [ns][n_hist]: lines s0 … s0 + ns − 1
   const int nb = L.n_bins, b = blockIdx.z;
-  for (int i = threadIdx.x; i < nb * n_hist; i += 256) s_h[i] = 0u;
+  for (int i = threadIdx.x; i < ns * n_hist; i += 256) s_h[i] = 0u;
   __syncthreads();
   const int x = blockIdx.x * 64 + (threadIdx.x & 63), y = blockIdx.y * 4 + (threadIdx.x >> 6);
   if (x < nx && y < ny) {
@@ -498,25 +499,39 @@ __global__ void __launch_bounds__(256) k_shift_hist(EprLines L, EprColumns C, in
     const float dtx = __ldg(tb + (size_t)y * nx + xp) - __ldg(tb + (size_t)y * nx + xm);
     const float dty = __ldg(tb + (size_t)yp * nx + x) - __ldg(tb + (size_t)ym * nx + x);
     const float g = 0.5f * sqrtf(dtx * dtx + dty * dty);                      // ‖D⁰τ‖
-    for (int s = 0; s < nb; ++s) {
+    for (int j = 0; j < ns; ++j) {
+      const int s = s0 + j;
       const float c = use_cols ? __ldg(&C.a[(size_t)s * nx + x]) * __ldg(&C.gamma[(size_t)s * nx + x]) : L.a[s] * L.gamma[s];
       const int k = min((int)(c * g * inv_bin), n_hist - 1);
-      atomicAdd(&s_h[s * n_hist + k], 1u);
+      atomicAdd(&s_h[j * n_hist + k], 1u);
     }
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < nb * n_hist; i += 256)
-    if (s_h[i]) atomicAdd(&hist[(size_t)b * nb * n_hist + i], s_h[i]);
+  for (int i = threadIdx.x; i < ns * n_hist; i += 256)
+    if (s_h[i]) atomicAdd(&hist[((size_t)b * nb + s0) * n_hist + i], s_h[i]);
 }
 
+// The per-CTA counters stay within the 48 KB of shared memory every kernel may use without opting in: the lines are
+// taken in passes of at most 12288 / n_hist (16 lines x 1024 bins = 64 KB goes in two passes of 12 and 4 lines).
 cudaError_t epr_launch_shift_hist(const epr_plan_s* p, int batch, const float* tau, int n_hist, float bin_px, unsigned* hist,
                                   cudaStream_t st) {
   const size_t n = (size_t)batch * p->n_bins * n_hist;
   cudaError_t e = cudaMemsetAsync(hist, 0, n * sizeof(unsigned), st);
   if (e != cudaSuccess) return e;
-  dim3 grid((p->nx + 63) / 64, (p->ny + 3) / 4, batch);
-  k_shift_hist<<<grid, 256, (size_t)p->n_bins * n_hist * sizeof(unsigned), st>>>(p->lines, p->cols, p->general, p->nx, p->ny, n_hist,
-                                                                                  1.f / bin_px, tau, hist);
+  const int per_pass = (48 * 1024 / (int)sizeof(unsigned)) / n_hist;        // n_hist <= 1024: at least 12
+  bool first = true;
+  for (int b0 = 0; b0 < batch; b0 += 65535) {                               // gridDim.z <= 65535
+    const int nbat = batch - b0 < 65535 ? batch - b0 : 65535;
+    dim3 grid((p->nx + 63) / 64, (p->ny + 3) / 4, nbat);
+    for (int s0 = 0; s0 < p->n_bins; s0 += per_pass) {
+      const int ns = p->n_bins - s0 < per_pass ? p->n_bins - s0 : per_pass;
+      if (!first) epr_note_extra_launch(p);
+      first = false;
+      k_shift_hist<<<grid, 256, (size_t)ns * n_hist * sizeof(unsigned), st>>>(
+          p->lines, p->cols, p->general, p->nx, p->ny, n_hist, s0, ns, 1.f / bin_px, tau + (size_t)b0 * p->nx * p->ny,
+          hist + (size_t)b0 * p->n_bins * n_hist);
+    }
+  }
   return cudaGetLastError();
 }
 

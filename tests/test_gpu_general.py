@@ -73,10 +73,10 @@ def test_retrieve_any_smooth_grid(E, nx, ny, solver, step, L):
 
 def test_argument_errors_sizes(E):
     en, w, db = SPECTRA["mono"]
-    for nx, ny in ((14, 16), (16, 7 * 16), (4, 64), (64, 4)):      # prime factor 7; below 8
+    for nx, ny in ((14, 16), (16, 7 * 16), (4, 64), (64, 4), (0, 64), (64, -8)):   # prime factor 7; below 8; not positive
         with pytest.raises(E.EprError) as ei:
             E.epr_plan(nx, ny, 6.5e-6, 1.0, en, w, db)
-        assert ei.value.status == (1 if min(nx, ny) < 8 else 2)
+        assert ei.value.status == (1 if min(nx, ny) < 1 else 2)        # EPR_EINVAL / EPR_ESIZE as include/epr.h says
     E.epr_plan(250, 16, 6.5e-6, 1.0, en, w, db).destroy()          # 250 = 2·5³ plans
 
 

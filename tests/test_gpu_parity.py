@@ -741,6 +741,35 @@ def test_splat_overflow_flag(E):
     plan.destroy()
 
 
+def test_shift_histogram_largest_documented_shape(E):
+    """epr_shift_histogram at the largest shape include/epr.h documents, 16 lines x 1024 bins (64 KB of per-CTA counters: the
+    launcher takes the lines in passes that fit 48 KB of shared memory), and at 13 x 1024 and 16 x 800, against the
+    oracle's histogram with the same near-edge allowance as below."""
+    n = 16
+    en = np.linspace(50.0, 150.0, n)
+    wt = np.exp(-0.5 * ((en - 100.0) / 30.0) ** 2)
+    db = 300.0 * en / 100.0
+    ny, nx = 96, 160
+    tau = np.stack([_tau_field(ny, nx, 21, amp=0.2), _tau_field(ny, nx, 22, amp=0.1)])
+    for n_lines, n_hist in ((16, 1024), (13, 1024), (16, 800)):
+        plan = E.epr_plan(nx, ny, 6.5e-6, 8.0, en[:n_lines], wt[:n_lines], db[:n_lines], "nonlocal", max_batch=2)
+        lines = O.derive_lines(6.5e-6, 8.0, en[:n_lines], wt[:n_lines], db[:n_lines])
+        bin_px = float(1.05 * O.max_shift(tau[0].astype(np.float64), lines) * np.sqrt(2.0) / n_hist)
+        hist = E.epr_shift_histogram(plan, _dev(tau), n_hist, bin_px).cpu().numpy()
+        plan.destroy()
+        assert hist.shape == (2, n_lines, n_hist)
+        for j in range(2):
+            t64 = tau[j].astype(np.float64)
+            ref = O.shift_histogram(t64, lines, n_hist, bin_px)
+            assert np.all(hist[j].sum(axis=1) == nx * ny)
+            assert np.count_nonzero(ref[0]) > n_hist // 8                   # the counts really spread over the bins
+            for s in range(n_lines):
+                ux, uy = O.ray_map(O.line_intensities(t64, lines)[s], lines.a[s], np.inf)
+                eta = np.sqrt(ux * ux + uy * uy) / bin_px
+                near_edge = int(np.sum(np.abs(eta - np.rint(eta)) < 1e-4 * np.maximum(eta, 1.0)))
+                assert np.sum(np.abs(hist[j, s].astype(np.int64) - ref[s])) <= 2 * near_edge, (n_lines, n_hist, j, s)
+
+
 def test_oversampled_host_path_and_shift_histogram(E):
     """epr_retrieve_oversampled_host (detector-grid host buffers, chunked: batch 5 > max_batch 2) equals the device call bit
     for bit; epr_shift_histogram of the result against the oracle's per-line histogram (Fig. 6): the bin of a
