@@ -282,3 +282,37 @@ def test_shift_histogram_closed_form():
         assert h[s, k] == (nx - 2) * (ny - 2)
         assert h[s, :k].sum() == 0 and h[s, k + 1:].sum() == nx * ny - (nx - 2) * (ny - 2)   # seam pixels: larger shifts
     assert int(np.argmax(h[0])) != int(np.argmax(h[1]))              # the lines differ (Fig. 6: one curve per line)
+
+
+def test_phase_is_eq6_written_out():
+    """Eq. (6) PAPER.md:216 with Eq. (7): φ_s = (db_s/2) ln(I_s / f_s) = (db_s/2)(ln I_s − ln f_s), db_s = δ_s/β_s
+    retyped here, I_s from `line_intensities`.  One line (γ = 1, f = 1): φ = (δ/2β) ln e^{−τ}.  A thicker object gives a more
+    NEGATIVE phase (δ > 0: the wave is advanced in matter), which fixes the sign."""
+    db = [800.0, 1200.0]
+    lines = O.derive_lines(6.5e-6, 2.0, [80.0, 120.0], [0.4, 0.6], db)
+    tau = 0.3 * (1.2 + _smooth(16, 24, 31))
+    Is = O.line_intensities(tau, lines)
+    for s in range(2):
+        want = (db[s] / 2.0) * (np.log(Is[s]) - np.log(lines.f[s]))
+        assert np.max(np.abs(O.phase(tau, lines, s) - want)) < 1e-12 * np.max(np.abs(want))
+    one = O.derive_lines(6.5e-6, 2.0, [100.0], [1.0], [1000.0])
+    assert np.max(np.abs(O.phase(tau, one) - 500.0 * np.log(np.exp(-tau)))) < 1e-11
+    assert np.all(O.phase(tau, one) < 0.0) and np.all(O.phase(2.0 * tau, one) < O.phase(tau, one))
+
+
+@pytest.mark.parametrize("solver", ["local", "nonlocal"])
+def test_residual_history_is_the_rms(solver):
+    """PAPER.md:231 "form the detector residual", PAPER.md:95 (convergence history): `history[n]` is the root mean square of
+    e = d − Σ_s P_s over the pixels.  From a CONSTANT start τ⁰ every operator leaves the constant planes I_s alone, so
+    Σ_s P_s = T⁰ = Σ_s f_s e^{−γ_s τ⁰} exactly; with d = T⁰ + ε cos(θ·r) over whole periods the first entry is ε/√2
+    (a mean of |e| would give 2ε/π)."""
+    lines = _three_unequal_lines(L=1.0)
+    ny, nx, eps, tau0 = 16, 24, 0.03, 0.2
+    T0 = float(np.sum(lines.f * np.exp(-lines.gamma * tau0)))
+    y, x = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    d = T0 + eps * np.cos(2 * np.pi * (3 * x / nx + 2 * y / ny))
+    h = []
+    O.retrieve(d, lines, solver, iterations=2, step=0.5, tau0=np.full((ny, nx), tau0), history=h)
+    assert len(h) == 2
+    assert abs(h[0] - eps / np.sqrt(2.0)) < 1e-13
+    assert abs(h[0] - 2 * eps / np.pi) > 1e-3

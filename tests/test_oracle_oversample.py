@@ -91,3 +91,22 @@ def test_fine_pixel_scalars_scale_as_the_square_of_the_factor():
     l1, l2 = _lines(6.5e-6, 3), _lines(6.5e-6 / 2, 3)
     assert np.allclose(l2.alpha, 4.0 * l1.alpha, rtol=1e-14) and np.allclose(l2.a, 4.0 * l1.a, rtol=1e-14)
     assert np.allclose(l2.gamma, l1.gamma, rtol=1e-14)
+
+
+def test_factor_one_nonlocal_hands_the_clamp_through():
+    """PAPER.md:167 ("the internal pixel size on the oversampled grid"): S counts pixels of the grid the loop runs on and is
+    handed to it unchanged.  With a clamp that BINDS (largest shift of the start > S) factor 1 must be the plain
+    non-local loop with the same S — and not the loop with 2 S."""
+    ny, nx, S = 16, 24, 0.1
+    y, x = np.meshgrid(np.arange(ny) * 2 * np.pi / ny, np.arange(nx) * 2 * np.pi / nx, indexing="ij")
+    d = 1.0 + 0.3 * np.cos(2 * x + y) + 0.2 * np.sin(3 * y - x)
+    lines = O.derive_lines(6.5e-6, 30.0, [100.0], [1.0], [1000.0])
+    tau0 = O.paganin_init(d, lines)
+    assert 2 * S < O.max_shift(tau0, lines)                                # the clamp binds at S and still at 2 S
+    plain = O.retrieve(d, lines, "nonlocal", 3, 0.4, S=S)
+    assert np.array_equal(O.retrieve_oversampled(d, lines, 1, "nonlocal", 3, 0.4, S=S), plain)
+    assert np.max(np.abs(O.retrieve(d, lines, "nonlocal", 3, 0.4, S=2 * S) - plain)) > 1e-6
+    # and at factor 2: the fine loop written out with the same S
+    fine = O.derive_lines(6.5e-6 / 2, 30.0, [100.0], [1.0], [1000.0])
+    want = O.downsample(O.retrieve(O.upsample(d, 2), fine, "nonlocal", 2, 0.4, S=S), 2)
+    assert np.array_equal(O.retrieve_oversampled(d, fine, 2, "nonlocal", 2, 0.4, S=S), want)

@@ -213,7 +213,10 @@ def test_nonlocal_wkb1_x_brute_force_and_uniform_reduction():
     ny, nx = 12, 20
     en, wt, db = np.array([80.0, 120.0]), np.array([0.4, 0.6]), np.array([8.0, 12.0])   # small δ/β: α²/4 is not small
     t = np.linspace(0.0, 1.0, 4)[:, None]
-    prof = O.derive_profiles(6.5e-6, 8.0, en, nx, wt[None, :] * (1.0 + 0.5 * t), db[None, :] * (1.0 + 0.3 * t))
+    # line-dependent tilts of the weights: after the per-block normalisation f_s(x) really varies with x
+    prof = O.derive_profiles(6.5e-6, 8.0, en, nx, wt[None, :] * (1.0 + t * np.array([0.8, -0.5])[None, :]),
+                             db[None, :] * (1.0 + 0.3 * t))
+    assert np.ptp(prof.f[0]) > 0.1 and np.ptp(prof.gamma[0]) > 0.01
     tau = 0.3 * (1.0 + 0.5 * _smooth(ny, nx, 21))
     P0, b0, _ = O.forward_x(tau, prof, "nonlocal", S=8.0)
     P1, b1, _ = O.forward_x(tau, prof, "nonlocal", S=8.0, nonlocal_wkb1=True)
@@ -258,3 +261,40 @@ def test_max_shift_x_plain_loops_and_histories():
     assert len(hx) == 3 and len(sx) == 3
     assert np.allclose(hx, hu, rtol=1e-11, atol=0) and np.allclose(sx, su, rtol=1e-11, atol=0)
     assert abs(sx[0] - O.max_shift(O.paganin_init(d, lines), lines)) < 1e-12 * sx[0]
+
+
+def test_positivity_floor_with_profiles():
+    """PAPER.md:225 "nonnegative spectral components", Eq. (7) PAPER.md:227 with the column's scalars: the total intensity
+    is floored at i_min before it is put back on the manifold, in the start (R9) and in the loop.  Vanishing propagation
+    distance: every filter is the identity (the block weights sum to one), so step = 1 from a constant start gives
+    Σ_s I_s = d pixel by pixel; a pixel of d forced to −1 must come back at the τ with Σ_s f_s(x) e^{−γ_s(x) τ} = i_min for
+    ITS column, found here by bracketing (brentq) on the column's scalars."""
+    from scipy.optimize import brentq
+    ny, nx, i_min = 8, 12, 1e-3
+    prof, _, _ = _varying(nx, 4, L=1e-12, mu=True)
+    assert np.max(prof.a) < 1e-9 and np.ptp(prof.gamma[0]) > 0.05
+    d = np.full((ny, nx), 0.9)
+    d[3, 5] = -1.0
+    f5, g5 = prof.f[:, 5], prof.gamma[:, 5]
+    want = brentq(lambda t: float(np.sum(f5 * np.exp(-g5 * t))) - i_min, 0.0, 1e3, xtol=1e-14, rtol=1e-14)
+    for tau in (O.paganin_init_x(d, prof, i_min=i_min),
+                O.retrieve_x(d, prof, "local", iterations=1, step=1.0, i_min=i_min, tau0=np.full(d.shape, 0.2)),
+                O.retrieve_x(d, prof, "nonlocal", iterations=1, step=1.0, i_min=i_min, tau0=np.full(d.shape, 0.2))):
+        assert np.all(np.isfinite(tau))
+        assert abs(tau[3, 5] - want) < 1e-10 * want
+        T = np.sum(O.line_intensities_x(tau, prof), axis=0)
+        assert np.max(np.abs(np.delete(T.ravel(), 3 * nx + 5) - 0.9)) < 1e-9
+
+
+@pytest.mark.parametrize("solver", ["local", "nonlocal"])
+def test_residual_history_with_profiles_is_the_rms(solver):
+    """`retrieve_x(history=…)`: root mean square of e = d − Σ_s P_s.  Constant start τ⁰: Σ_s P_s is the
+    column's T⁰(x) = Σ_s f_s(x) e^{−γ_s(x) τ⁰}; d = T⁰(x) + ε cos(θ·r) over whole periods gives ε/√2 first."""
+    ny, nx, eps, tau0 = 16, 24, 0.03, 0.2
+    prof, _, _ = _varying(nx, 4, L=1.0, mu=True)
+    T0 = np.sum(prof.f * np.exp(-prof.gamma * tau0), axis=0)[None, :]
+    y, x = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    d = T0 + eps * np.cos(2 * np.pi * (3 * x / nx + 2 * y / ny))
+    h = []
+    O.retrieve_x(d, prof, solver, iterations=2, step=0.5, tau0=np.full((ny, nx), tau0), history=h)
+    assert len(h) == 2 and abs(h[0] - eps / np.sqrt(2.0)) < 1e-12 and abs(h[0] - 2 * eps / np.pi) > 1e-3
