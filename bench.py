@@ -170,16 +170,34 @@ def fine_shift_clamp(w, m):
     return float(min(30.0, m * w.max_shift_px))
 
 
+def workload_string(name, w, m=1, blocks=0):
+    """`config.workload` of both arms (the driver compares the two strings)."""
+    return (f"{name}: {w.ny}x{w.nx}, {w.n_bins} line(s), {w.solver} solver, {w.iterations} iterations, step {w.step}"
+            + (f", oversampling {m} (computational grid {m * w.ny}x{m * w.nx})" if m > 1 else "")
+            + (f", x-dependent spectrum on {blocks} blocks (general path)" if blocks > 0 else ""))
+
+
 def oracle_time_one(w, j=0, m=1):
-    """The oracle as it stands, one projection of the workload, on the host cores (numpy: 1 thread)."""
+    """The oracle as it stands, one projection of the workload, on the host cores (numpy: 1 thread).  Returns (seconds,
+    the oracle's result): the result is compared with the GPU's output for the same projection (`parity`)."""
     from oracle import epr_oracle as O
     lines = O.derive_lines(w.pixel_m / m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta)
     t0 = time.perf_counter()
     if m == 1:
-        O.retrieve(w.d[j].astype(np.float64), lines, w.solver, w.iterations, w.step, S=w.max_shift_px)
+        tau = O.retrieve(w.d[j].astype(np.float64), lines, w.solver, w.iterations, w.step, S=w.max_shift_px)
     else:
-        O.retrieve_oversampled(w.d[j].astype(np.float64), lines, m, w.solver, w.iterations, w.step, S=fine_shift_clamp(w, m))
-    return time.perf_counter() - t0
+        tau = O.retrieve_oversampled(w.d[j].astype(np.float64), lines, m, w.solver, w.iterations, w.step, S=fine_shift_clamp(w, m))
+    return time.perf_counter() - t0, tau
+
+
+def parity_of(gpu_tau, oracle_tau):
+    """The oracle acting as checker, outside every timed region: the GPU's result for one projection of the timed
+    batch against the oracle's for the same input (north_star: retrieved thickness / phase within 1e-4 relative L2)."""
+    g = np.asarray(gpu_tau, dtype=np.float64)
+    r = np.asarray(oracle_tau, dtype=np.float64)
+    return {"rel_l2": float(np.linalg.norm(g - r) / np.linalg.norm(r)),
+            "max_rel": float(np.max(np.abs(g - r)) / np.max(np.abs(r))), "tolerance_rel_l2": 1e-4,
+            "what": "tau of projection 0 of the timed batch, all iterations: GPU (epr_retrieve) vs the fp64 oracle"}
 
 
 def _oracle_sample_worker(a):
@@ -309,10 +327,10 @@ def run_reference(args, rank):
     if args.lines > 0:
         override_lines(w, args.lines)
     m = args.oversample
-    c0 = oracle_time_iters(w, 0, m)
+    c0 = float(np.median([oracle_time_iters(w, 0, m) for _ in range(3)]))     # initial solve alone: median of three
     c1 = oracle_time_iters(w, 1, m)
     t_iter = max(c1 - c0, 1e-3)
-    per_step = args.ref_budget / max(1, args.steps + args.warmup)
+    per_step = (args.ref_budget - 4 * c0 - t_iter) / max(1, args.steps + args.warmup)
     n_it = int(max(1, min(w.iterations, (per_step - c0) // t_iter)))
     for _ in range(args.warmup):
         oracle_time_iters(w, n_it, m)
@@ -325,14 +343,16 @@ def run_reference(args, rank):
     else:
         sample = (f"1 projection {w.ny}x{w.nx} per step: initial solve + the first {n_it} of {w.iterations} iterations "
                   f"({float(np.mean(t)):.2f} s per step measured), extrapolated linearly to all iterations with the initial "
-                  f"solve of the calibration ({c0:.2f} s); numpy fp64 oracle; run bounded to {args.ref_budget:.0f} s")
+                  f"solve of the calibration ({c0:.2f} s, median of 3); numpy fp64 oracle; run bounded to {args.ref_budget:.0f} s")
+    # ONE time base in the line: value, ms_per_step, cpu_baseline and e2e all describe the full workload (extrapolated where
+    # the budget cut the iterations); what was actually timed per step sits in config.ms_per_step_measured
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(t)), "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{args.config}: {w.ny}x{w.nx}, {w.n_bins} line(s), {w.solver}, {w.iterations} iterations"
-                               + (f", oversampling {args.oversample}" if args.oversample > 1 else ""),
-                   "iterations_run_per_step": n_it, "ms_per_projection_extrapolated": 1e3 * tot / args.steps},
+        "config": {"workload": workload_string(args.config, w, m),
+                   "iterations_run_per_step": n_it, "ms_per_step_measured": 1e3 * float(np.mean(t)),
+                   "extrapolated": bool(n_it != w.iterations)},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
@@ -348,7 +368,8 @@ def block_profiles(w, n_blocks):
     return wt, db
 
 
-def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, lines=0, m=1, cufft=False, blocks=0):
+def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, lines=0, m=1, cufft=False, blocks=0, n=None,
+                   S_fine=None):
     """Time one configuration: K steps of epr_retrieve over B resident projections (CUDA events on the launch stream),
     the same through epr_retrieve_host with pinned host buffers, and a profiling pass with the in-library per-kernel
     events.  Returns the pieces of the JSON line for this configuration (everything already reduced over ranks)."""
@@ -356,7 +377,7 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
     import torch.distributed as dist
     from epr_inputs import make_workload
 
-    w = make_workload(name, batch=B, distinct=min(distinct, B))
+    w = make_workload(name, n=n, batch=B, distinct=min(distinct, B))
     if lines > 0:
         override_lines(w, lines)
     if world > 1:                                   # every rank gets its own noise realisations
@@ -365,7 +386,7 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
     plane = w.nx * w.ny
     nb = w.n_bins
     plan = epr.epr_plan(m * w.nx, m * w.ny, w.pixel_m / m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
-                        max_batch=B, max_shift_px=w.max_shift_px if m == 1 else fine_shift_clamp(w, m))
+                        max_batch=B, max_shift_px=w.max_shift_px if m == 1 else (S_fine or fine_shift_clamp(w, m)))
     if blocks > 0:                                  # x-dependent effective spectrum (reading R17): the general path
         epr.epr_plan_profiles(plan, *block_profiles(w, blocks))
     d_host = torch.from_numpy(w.d).pin_memory()
@@ -413,7 +434,10 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
     ms = max_over_ranks(ms, torch.device("cuda", local))
     value = world * B * steps / (ms * 1e-3)
 
-    # ---- end to end through the public host API: pinned host buffers, H2D + loop + D2H inside the timed region
+    # ---- end to end through the public host API: pinned host buffers, H2D + loop + D2H inside the timed region.
+    # (i) per call: every epr_retrieve_host waits for its own last copy; (ii) the streaming session of PAPER.md:245
+    # (epr_retrieve_host_async x K, one epr_host_wait): the K batches follow each other as the chunks of a scan do, every
+    # copy in and every copy out still inside the timed region — the headline e2e where the API offers it (factor 1)
     step_host()
     barrier()
     t0 = time.perf_counter()
@@ -421,7 +445,19 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
         step_host()
     e2e_s = time.perf_counter() - t0
     e2e_s = max_over_ranks(e2e_s, torch.device("cuda", local))
-    e2e = world * B * steps / e2e_s
+    e2e_call = world * B * steps / e2e_s
+    e2e, e2e_api = e2e_call, "epr_retrieve_host (pinned host buffers, chunks double-buffered on three streams), one call per step"
+    if m == 1:
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            epr.epr_retrieve_host(plan, d_host, out_host, w.iterations, w.step, wait=False)
+        epr.epr_host_wait(plan)
+        e2e_s = time.perf_counter() - t0
+        e2e_s = max_over_ranks(e2e_s, torch.device("cuda", local))
+        e2e = world * B * steps / e2e_s
+        e2e_api = (f"epr_retrieve_host_async x {steps} + epr_host_wait (streaming session: pinned host buffers, chunks "
+                   "double-buffered on three streams across consecutive batches); per_call = epr_retrieve_host, one call per step")
 
     # ---- per-kernel device times (CUDA events around every launch, on the launch stream), same K steps
     plan.profile(True)
@@ -472,16 +508,13 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
                 "peak_source": peak_src, "per_kernel": per_kernel}
     res = {
         "value": value, "unit": UNIT, "ms_per_step": ms / steps, "steps": steps, "warmup": warmup,
-        "config": {"workload": f"{name}: {w.ny}x{w.nx}, {nb} line(s), {w.solver} solver, "
-                               f"{w.iterations} iterations, step {w.step}"
-                               + (f", oversampling {m} (computational grid {m * w.ny}x{m * w.nx})" if m > 1 else "")
-                               + (f", x-dependent spectrum on {blocks} blocks (general path)" if blocks > 0 else ""),
+        "config": {"workload": workload_string(name, w, m, blocks),
                    "batch_per_gpu": B, "distinct_projections": min(distinct, B),
                    "l2": (f"inputs {in_bytes / 1e6:.0f} MB per step > 2 x 126 MB L2: no flush needed" if flush is None else
                           f"inputs {in_bytes / 1e6:.0f} MB per step: L2 flushed (256 MB overwrite) between timed steps"),
                    "ms_per_iteration_per_projection": ms / steps / B / (w.iterations + 1)},
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": B * plane * 4, "d2h_bytes_per_step": B * plane * 4,
-                "api": "epr_retrieve_host (pinned host buffers, chunks double-buffered on three streams)"},
+                "per_call": e2e_call, "api": e2e_api},
         "gpu_launches": int(launches) * world,
         "clocks": clk.summary(),
         "roofline": roofline,
@@ -489,10 +522,55 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
     }
     if cmp_cufft is not None:
         res["cufft_compare"] = cmp_cufft
+    if m > 1:
+        res["config"]["max_shift_fine_px"] = float(S_fine or fine_shift_clamp(w, m))
+    step()
+    torch.cuda.synchronize()
+    res["_tau0"] = out[0].cpu().numpy()             # for `parity` (popped before the line is printed)
     plan.destroy()
     del d, out, d_host, out_host, flush
     torch.cuda.empty_cache()
     return res, w
+
+
+def measure_c1(epr, local, calls=200):
+    """BASELINE.json configs[0] (C1: ONE 256 x 256 projection, local solver, 10 iterations — launch-bound): microseconds per
+    epr_retrieve on a non-default stream, launched kernel by kernel (EPR_GRAPH = 0 at plan time) and as the CUDA graph the
+    library captures on the second identical call and replays afterwards (include/epr.h, epr_retrieve)."""
+    import torch
+    from epr_inputs import make_workload
+    w = make_workload("C1")
+    d = torch.from_numpy(w.d).cuda()
+    out = torch.empty_like(d)
+    st = torch.cuda.Stream()
+    res = {}
+    for mode, env in (("eager", "0"), ("graph", "1")):
+        os.environ["EPR_GRAPH"] = env
+        plan = epr.epr_plan(w.nx, w.ny, w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver, max_batch=1)
+        os.environ.pop("EPR_GRAPH")
+        with torch.cuda.stream(st):
+            for _ in range(5):
+                epr.epr_retrieve(plan, d, out, w.iterations, w.step)
+            st.synchronize()
+            l0 = plan.launches
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0 = time.perf_counter()
+            e0.record(st)
+            for _ in range(calls):
+                epr.epr_retrieve(plan, d, out, w.iterations, w.step)
+            e1.record(st)
+            st.synchronize()
+            wall = time.perf_counter() - t0
+        res[mode] = {"us_per_retrieval_device": 1e3 * e0.elapsed_time(e1) / calls, "us_per_retrieval_wall": 1e6 * wall / calls,
+                     "kernel_launches_per_retrieval": (plan.launches - l0) / calls}
+        plan.destroy()
+    res["config"] = {"workload": workload_string("C1", w), "batch": 1, "calls": calls,
+                     "l2": "one 256 KB plane: deliberately L2-resident (the configuration is launch-bound, not HBM-bound)"}
+    res["value"] = 1e6 / res["graph"]["us_per_retrieval_device"]
+    res["unit"] = UNIT
+    res["summary"] = [round(res["value"], 1), None, f"graph {res['graph']['us_per_retrieval_device']:.0f} us / eager "
+                      f"{res['eager']['us_per_retrieval_device']:.0f} us per retrieval", None, None]
+    return res
 
 
 def main():
@@ -548,16 +626,29 @@ def main():
     for k in ("config", "e2e", "gpu_launches", "clocks", "roofline", "flags", "cufft_compare"):
         if k in head:
             result[k] = head[k]
+    tau_gpu = head.pop("_tau0")
     if rank == 0 and not args.no_cpu_baseline:
-        t1 = oracle_time_one(w, m=args.oversample)
+        t1, tau_ref = oracle_time_one(w, m=args.oversample)
         result["cpu_baseline"] = {"value": 1.0 / t1, "unit": UNIT, "cores": 1, "kind": "oracle",
                                   "sample": f"1 of the {B} projections ({w.ny}x{w.nx}, all {w.iterations} "
                                             f"iterations) in {t1:.1f} s, numpy fp64, host has {os.cpu_count()} cores"}
-    del w
+        result["parity"] = parity_of(tau_gpu, tau_ref)
+        del tau_ref
+    del w, tau_gpu
 
+    def compact(r):
+        """[projections/s device-resident, through host buffers, dominant kernel, its HBM fraction, median SM MHz]"""
+        if "error" in r:
+            return r["error"][:80]
+        return [round(r["value"], 1), round(r["e2e"]["value"], 1), r["roofline"]["kernel"], round(r["roofline"]["frac"], 3),
+                r["clocks"].get("sm_mhz")]
+
+    summary = {args.config: compact(head)}
     # ---- the other BASELINE.json configurations, each measured the same way (same protocol, fewer steps), in the same
     # line: C3 (non-local, one line), C4 (non-local, 8 lines), C5 (2560 x 2160, 8 lines, batch 64 — more than the
-    # plan's work batch holds, so the device call passes through HBM in sub-batches and the host call streams chunks)
+    # plan's work batch holds, so the device call passes through HBM in sub-batches and the host call streams chunks);
+    # then the SURVEY.md §8(f) shapes: the oversampled loop (PAPER.md:79) and the x-dependent spectrum (PAPER.md:431-441),
+    # and BASELINE.json configs[0] (C1: one 256 x 256 retrieval, launch-bound, eager and as a replayed CUDA graph)
     default_run = (args.config == "C2" and args.lines == 0 and args.oversample == 1 and args.batch == 0 and args.blocks == 0)
     if default_run and not args.no_other_configs:
         other = {}
@@ -566,13 +657,46 @@ def main():
         for name, ob, osteps, odist in (("C3", 64, 3, 4), ("C4", 8, 3, 4), ("C5", 64, 2, 8)):
             try:
                 r, ow = measure_config(epr, name, ob, osteps, 3, max(args.distinct, odist), rank, world, local)
+                tau_gpu = r.pop("_tau0")
                 if rank == 0 and not args.no_cpu_baseline:
-                    r["cpu_baseline"] = oracle_sample(ow, host_procs(ow) if name == "C5" else 1)
-                del ow
+                    if name == "C3":               # one line: the full 20 iterations of one projection fit the budget
+                        t1, tau_ref = oracle_time_one(ow)
+                        r["cpu_baseline"] = {"value": 1.0 / t1, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                             "sample": f"1 of the {ob} projections ({ow.ny}x{ow.nx}, all {ow.iterations} "
+                                                       f"iterations) in {t1:.1f} s, numpy fp64"}
+                        r["parity"] = parity_of(tau_gpu, tau_ref)
+                        del tau_ref
+                    else:
+                        r["cpu_baseline"] = oracle_sample(ow, host_procs(ow) if name == "C5" else 1)
+                del ow, tau_gpu
                 other[name] = r
             except Exception as exc:                # a sub-result must never cost the headline
                 other[name] = {"error": f"{type(exc).__name__}: {exc}"[:300]}
+            summary[name] = compact(other[name])
+        extra = (("C2_x2", dict(name="C2", B=8, m=2)),                                     # local, x2: 4096 x 4096
+                 ("C3_1024_x4", dict(name="C3", B=8, m=4, n=1024, S_fine=30.0)),            # non-local, x4: 4096 x 4096
+                 ("C2_blocks4", dict(name="C2", B=16, blocks=4)), ("C4_blocks4", dict(name="C4", B=4, blocks=4)))
+        for key, kw in extra:
+            try:
+                r, ow = measure_config(epr, kw["name"], kw["B"], 2, 3, 2, rank, world, local, m=kw.get("m", 1),
+                                       blocks=kw.get("blocks", 0), n=kw.get("n"), S_fine=kw.get("S_fine"))
+                r.pop("_tau0")
+                r["roofline"].pop("per_kernel", None)            # keep the line short: the headline configs carry the tables
+                del ow
+                other[key] = r
+            except Exception as exc:
+                other[key] = {"error": f"{type(exc).__name__}: {exc}"[:300]}
+            summary[key] = compact(other[key])
+        try:
+            other["C1"] = measure_c1(epr, local)
+            summary["C1"] = other["C1"]["summary"]
+        except Exception as exc:
+            other["C1"] = {"error": f"{type(exc).__name__}: {exc}"[:300]}
+            summary["C1"] = other["C1"]["error"][:80]
         result["other_configs"] = other
+    # LAST in the line, so that a reader who keeps only its tail still sees every configuration
+    result["summary"] = {"columns": ["projections/s device-resident", "projections/s through host buffers", "dominant kernel",
+                                     "its fraction of the HBM peak", "median SM MHz"], **summary}
     if rank == 0:
         print(json.dumps(result))
     if world > 1:

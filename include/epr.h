@@ -63,7 +63,9 @@ void epr_default_options(epr_options* opt);
  *   energy_keV, weight, delta_over_beta   HOST arrays of length n_bins: E_s, spectral weight (normalised
  *                 internally to Σ f_s = 1), δ_s/β_s.
  *   solver        EPR_LOCAL: Taylor/WKB closure Eq. (1); EPR_NONLOCAL: ray map Eq. (2) + splat Eq. (3).
- *   max_batch     largest `batch` later calls may pass (workspaces are sized for it).
+ *   max_batch     largest `batch` later calls may pass.  The loop's workspaces are sized for a WORK BATCH = max_batch, capped
+ *                 so that they stay below 12 GB (environment EPR_WORK_BATCH = projections, read here, overrides); larger
+ *                 batches pass through the loop in passes of that many projections — same results, bit for bit.
  * Grids: nx, ny >= 8 with prime factors in {2, 3, 5} (anything else: EPR_ESIZE; padding is the caller's job, R7).
  *   The tuned kernels run on 16-pixel-aligned grids whose lengths have a compiled transform (16, 32, 48, 64, 80, 96, 128,
  *   160, 256, 320, 384, 512, 640, 768, 1024, 1280, 1536, 1920, 2048, 2160, 2560, 3072, 3200, 4096); every other smooth
@@ -148,9 +150,43 @@ epr_status epr_shift_histogram(epr_plan_t plan, int batch, const float* tau, int
  *   work batch; environment EPR_HOST_CHUNK = projections per chunk overrides) that travel on three private streams, so
  *   that the copy in of chunk i + 1 and the copy out of chunk i − 1 overlap the loop of chunk i; the first and last
  *   chunks are smaller (their copies overlap nothing).  `batch` may exceed max_batch.  The call first waits for all
- *   work enqueued earlier on the device (cudaDeviceSynchronize) and returns after its last copy has completed. */
+ *   work enqueued earlier on the device (cudaDeviceSynchronize) and returns after its last copy has completed.
+ *   Tunables (environment, read at every call): small batches are cut into 1, 2 or 4 chunks according to the share of
+ *   the copies in the call, estimated from EPR_HOST_LINK_GBS (host link, default 50 GB/s — a B200 on PCIe 5 x16) and
+ *   EPR_LOOP_GBS (rate at which the loop moves its algorithmic bytes, default 2500 GB/s, measured on B200); set them for
+ *   another host link or GPU.  They only change the chunking, never the result. */
 epr_status epr_retrieve_host(epr_plan_t plan, int batch, const float* d_host, float* out_host, int iterations,
                              float step);
+
+/* epr_retrieve_host_async / epr_host_wait — epr_retrieve_host as a STREAMING SESSION
+ *   "large acquisitions processed in chunks": a scan is thousands of radiographs handed over batch after batch.
+ *   epr_retrieve_host_async enqueues one batch exactly like epr_retrieve_host (same chunks, same results bit for bit) but
+ *   returns without waiting; consecutive async calls on a plan form a session in which the copy in of the next batch's first
+ *   chunk overlaps the last loop of the previous batch and its last copy out overlaps the next batch's first loop.  Only the
+ *   first call of a session waits for work enqueued earlier on the device.  epr_host_wait returns when everything enqueued
+ *   in the session has completed — every out_host is valid from then on — and closes it; a plain epr_retrieve_host does the
+ *   same before it starts.  d_host and out_host must stay valid (and should be pinned) until epr_host_wait.  Between the
+ *   first async call and epr_host_wait make NO other call on this plan except epr_retrieve_host_async (the session uses
+ *   the plan's workspaces on private streams).  opt.init = 1 and epr_set_diagnostics work as in epr_retrieve_host (the
+ *   diagnostics rows are indexed per call: give every call its own array or read it before the next call). */
+epr_status epr_retrieve_host_async(epr_plan_t plan, int batch, const float* d_host, float* out_host, int iterations,
+                                   float step);
+epr_status epr_host_wait(epr_plan_t plan);
+
+/* epr_retrieve_host_multi — ONE host batch over several plans, one per GPU
+ *   "when two GPUs are available ...": projections are independent, so plan k (normally created on device k; all plans on
+ *   the same grid with the same physics) receives the contiguous, balanced range of the batch that rank k of n_plans gets —
+ *   the first batch % n_plans plans take one projection more — as one streaming call on its own device, and the call
+ *   returns when all of them have finished.  No data crosses between GPUs.  HOST buffers [batch][ny][nx], pinned for
+ *   overlap.  Plans may also share a device (two pipelines on one GPU).  Returns the first error of any plan (its message
+ *   is in that plan's epr_last_error). */
+epr_status epr_retrieve_host_multi(epr_plan_t* plans, int n_plans, int batch, const float* d_host, float* out_host,
+                                   int iterations, float step);
+
+/* epr_shard_range — the split epr_retrieve_host_multi (and a one-process-per-GPU launcher) uses: part k of `parts` gets the
+ *   projections [*start, *stop) of `total`; contiguous, balanced, the first total % parts parts take one more.  Host
+ *   arithmetic only: needs no device.  EPR_EINVAL for total < 0, parts < 1, k outside 0..parts−1 or NULL pointers. */
+epr_status epr_shard_range(int total, int k, int parts, int* start, int* stop);
 
 /* epr_plan_profiles — x-dependent effective spectrum           PAPER.md:216-221 (Eq. (6) + remark), 227-229 (Eq. (7)), 431-441 (§9.2)
  *   "I_s(r) = f_s(x) exp(−γ_s(x) τ(r))", "db_s(x) = δ_s(x)/β_s(x) may be x-dependent if an x-dependent effective spectrum

@@ -6,5 +6,5 @@ cudaStream_t).  Every step of the path runs in the hand-written sm_100a kernels 
 """
 from .binding import (EPR_LOCAL, EPR_NONLOCAL, EprError, Options, Plan, epr_adjoint, epr_forward, epr_plan, epr_plan_profiles,  # noqa: F401
                       epr_precondition, epr_retrieve, epr_retrieve_host, epr_retrieve_oversampled, epr_set_diagnostics, epr_shift_histogram, epr_transport, lib_path,
-                      EPR_STATIC_MAX_BATCH, epr_residual_rms_static,
+                      EPR_STATIC_MAX_BATCH, epr_residual_rms_static, epr_host_wait, epr_retrieve_host_multi, epr_shard_range,
                       load_library)

@@ -15,7 +15,8 @@ EXPORTS = ["epr_default_options", "epr_plan", "epr_forward", "epr_adjoint", "epr
            "epr_retrieve", "epr_retrieve_oversampled", "epr_set_diagnostics", "epr_retrieve_host", "epr_plan_lines", "epr_launch_count", "epr_destroy",
            "epr_last_error", "epr_version", "epr_profile_enable", "epr_profile_read", "epr_read_flags",
            "epr_plan_profiles", "epr_plan_columns", "epr_shift_histogram",
-           "epr_retrieve_oversampled_host", "epr_residual_rms_static", "epr_static_last_error"]
+           "epr_retrieve_oversampled_host", "epr_residual_rms_static", "epr_static_last_error",
+           "epr_retrieve_host_async", "epr_host_wait", "epr_retrieve_host_multi", "epr_shard_range"]
 EPR_STATIC_MAX_BATCH = 1024
 EPR_FLAG_SPLAT_OVERFLOW = 1
 
@@ -59,6 +60,14 @@ def load_library():
     lib.epr_retrieve_oversampled.argtypes = [vp, ci, ci, vp, vp, ci, cf, vp]
     lib.epr_set_diagnostics.argtypes = [vp, vp, ci]
     lib.epr_retrieve_host.argtypes = [vp, ci, vp, vp, ci, cf]
+    lib.epr_retrieve_host_async.argtypes = [vp, ci, vp, vp, ci, cf]
+    lib.epr_retrieve_host_async.restype = ci
+    lib.epr_host_wait.argtypes = [vp]
+    lib.epr_host_wait.restype = ci
+    lib.epr_retrieve_host_multi.argtypes = [C.POINTER(vp), ci, ci, vp, vp, ci, cf]
+    lib.epr_retrieve_host_multi.restype = ci
+    lib.epr_shard_range.argtypes = [ci, ci, ci, C.POINTER(ci), C.POINTER(ci)]
+    lib.epr_shard_range.restype = ci
     lib.epr_retrieve_oversampled_host.argtypes = [vp, ci, ci, vp, vp, ci, cf]
     lib.epr_retrieve_oversampled_host.restype = ci
     lib.epr_plan_lines.argtypes = [vp, C.POINTER(cd), C.POINTER(cd), C.POINTER(cd), C.POINTER(cd)]
@@ -295,26 +304,61 @@ def epr_set_diagnostics(plan, diag):
     plan._check(load_library().epr_set_diagnostics(plan._h, _dev(diag, None, "diag"), int(diag.shape[1])))
 
 
-def epr_retrieve_host(plan, d_host, out_host, iterations, step, factor=1):
+def _host_ptr(a, name):
+    if isinstance(a, np.ndarray):
+        if a.dtype != np.float32 or not a.flags.c_contiguous:
+            raise TypeError(f"{name}: expected C-contiguous float32")
+        return C.c_void_p(a.ctypes.data), a.shape
+    import torch
+    if not isinstance(a, torch.Tensor) or a.is_cuda or a.dtype != torch.float32 or not a.is_contiguous():
+        raise TypeError(f"{name}: expected a contiguous float32 host tensor")
+    return C.c_void_p(a.data_ptr()), tuple(a.shape)
+
+
+def epr_retrieve_host(plan, d_host, out_host, iterations, step, factor=1, wait=True):
     """HOST buffers (pinned float32 torch tensors or C-contiguous numpy arrays), copies inside the call.
-    factor > 1: epr_retrieve_oversampled_host — buffers on the detector grid [batch][ny/factor][nx/factor]."""
-    def hp(a, name):
-        if isinstance(a, np.ndarray):
-            if a.dtype != np.float32 or not a.flags.c_contiguous:
-                raise TypeError(f"{name}: expected C-contiguous float32")
-            return C.c_void_p(a.ctypes.data), a.shape
-        import torch
-        if not isinstance(a, torch.Tensor) or a.is_cuda or a.dtype != torch.float32 or not a.is_contiguous():
-            raise TypeError(f"{name}: expected a contiguous float32 host tensor")
-        return C.c_void_p(a.data_ptr()), tuple(a.shape)
-    pd, sd = hp(d_host, "d_host")
-    po, so = hp(out_host, "out_host")
+    factor > 1: epr_retrieve_oversampled_host — buffers on the detector grid [batch][ny/factor][nx/factor].
+    wait=False: epr_retrieve_host_async — the call only enqueues; keep the buffers alive and call epr_host_wait(plan)."""
+    pd, sd = _host_ptr(d_host, "d_host")
+    po, so = _host_ptr(out_host, "out_host")
     factor = int(factor)
     if factor < 1 or plan.ny % factor or plan.nx % factor:
         raise ValueError("factor must divide the plan's grid")
     if tuple(sd) != tuple(so) or tuple(sd[1:]) != (plan.ny // factor, plan.nx // factor):
         raise ValueError("d_host / out_host must both be [batch][ny / factor][nx / factor]")
-    if factor == 1:
+    if not wait:
+        if factor != 1:
+            raise ValueError("the streaming session takes buffers on the plan's grid (factor = 1)")
+        plan._check(load_library().epr_retrieve_host_async(plan._h, int(sd[0]), pd, po, int(iterations), float(step)))
+    elif factor == 1:
         plan._check(load_library().epr_retrieve_host(plan._h, int(sd[0]), pd, po, int(iterations), float(step)))
     else:
         plan._check(load_library().epr_retrieve_oversampled_host(plan._h, factor, int(sd[0]), pd, po, int(iterations), float(step)))
+
+
+def epr_shard_range(total, k, parts):
+    """epr_shard_range of include/epr.h: (start, stop) of part k — host arithmetic, works without a device."""
+    a, b = C.c_int(0), C.c_int(0)
+    st = load_library().epr_shard_range(int(total), int(k), int(parts), C.byref(a), C.byref(b))
+    if st != 0:
+        raise EprError(st, "epr_shard_range: total >= 0, parts >= 1 and 0 <= k < parts required")
+    return int(a.value), int(b.value)
+
+
+def epr_host_wait(plan):
+    """epr_host_wait of include/epr.h: returns when every epr_retrieve_host(..., wait=False) of the session has completed."""
+    plan._check(load_library().epr_host_wait(plan._h))
+
+
+def epr_retrieve_host_multi(plans, d_host, out_host, iterations, step):
+    """epr_retrieve_host_multi of include/epr.h: ONE host batch split over `plans` (one per GPU), no exchange between them."""
+    pd, sd = _host_ptr(d_host, "d_host")
+    po, so = _host_ptr(out_host, "out_host")
+    p0 = plans[0]
+    if tuple(sd) != tuple(so) or tuple(sd[1:]) != (p0.ny, p0.nx):
+        raise ValueError("d_host / out_host must both be [batch][ny][nx]")
+    hs = (C.c_void_p * len(plans))(*[p._h.value for p in plans])
+    st = load_library().epr_retrieve_host_multi(hs, len(plans), int(sd[0]), pd, po, int(iterations), float(step))
+    if st != 0:
+        msgs = [load_library().epr_last_error(p._h).decode() for p in plans]
+        raise EprError(st, "; ".join(m for m in msgs if m))

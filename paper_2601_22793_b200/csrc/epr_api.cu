@@ -919,8 +919,24 @@ extern "C" epr_status epr_retrieve(epr_plan_t p, int batch, const float* d, floa
 }
 
 // factor = 1: the plan's grid; factor > 1: host buffers on the detector grid, the loop on the plan's (fine) grid (R16)
+// Closes a streaming session: waits for everything epr_retrieve_host_async enqueued on the plan's private streams.
+static epr_status host_wait(epr_plan_t p) {
+  if (!p->hsession) return EPR_OK;
+  p->hsession = 0;
+  p->hchunk = 0;
+  CU(p, cudaStreamSynchronize(p->hstream[2]));
+  CU(p, cudaStreamSynchronize(p->hstream[1]));
+  CU(p, cudaStreamSynchronize(p->hstream[0]));
+  return EPR_OK;
+}
+
+// async = 0: one self-contained call (waits for earlier device work on entry, returns when its last copy is done).
+// async = 1: a call of a streaming session (chunk k + 1 is prepared while chunk k is processed): only the FIRST
+// call of a session waits for earlier device work, no call waits at its end, and the chunk counter — which decides the
+// staging buffer and the events a chunk must wait for — runs on across calls, so that the first copy in of call k + 1
+// overlaps the last loop of call k and the last copy out of call k overlaps the first loop of call k + 1.
 static epr_status retrieve_host_impl(epr_plan_t p, int factor, int batch, const float* d_host, float* out_host, int iterations,
-                                     float step) {
+                                     float step, int async) {
   if (batch < 1 || !d_host || !out_host) FAIL(p, EPR_EINVAL, "epr_retrieve_host: bad batch or NULL pointer");
   if (iterations < 0 || !(step > 0.f)) FAIL(p, EPR_EINVAL, "epr_retrieve_host: iterations must be >= 0 and step > 0");
   const size_t plane = (size_t)p->nx * p->ny / ((size_t)factor * factor);       // a plane of the HOST buffers
@@ -934,7 +950,11 @@ static epr_status retrieve_host_impl(epr_plan_t p, int factor, int batch, const 
   // with chunks of 1 / 2 / 4; C3, batch 8, r = 0.37: 464 / 542 / 542 / 500 with chunks of 1 / 2 / 4 / 8).
   const int nbn = p->n_bins;
   const double bpp = (p->solver == EPR_LOCAL) ? (nbn == 1 ? 40.0 : 24.0 + 24.0 * nbn) : (nbn == 1 ? 52.0 : 28.0 + 24.0 * nbn);
-  const double r = (8.0 / 50.0) / ((iterations + 1) * bpp * factor * factor / 2500.0);
+  // the two rates are tunables stated in include/epr.h (epr_retrieve_host): environment EPR_HOST_LINK_GBS, EPR_LOOP_GBS
+  double link_gbs = 50.0, loop_gbs = 2500.0;
+  { const char* e1 = getenv("EPR_HOST_LINK_GBS"); if (e1 && atof(e1) > 0) link_gbs = atof(e1); }
+  { const char* e2 = getenv("EPR_LOOP_GBS"); if (e2 && atof(e2) > 0) loop_gbs = atof(e2); }
+  const double r = (8.0 / link_gbs) / ((iterations + 1) * bpp * factor * factor / loop_gbs);
   const int min_chunks = r >= 0.3 ? 4 : r >= 0.15 ? 2 : 1;
   int wbch = (int)(((size_t)256 << 20) / (plane * sizeof(float)));
   if (wbch > (batch + min_chunks - 1) / min_chunks) wbch = (batch + min_chunks - 1) / min_chunks;
@@ -945,6 +965,10 @@ static epr_status retrieve_host_impl(epr_plan_t p, int factor, int batch, const 
   if (!getenv("EPR_HOST_CHUNK")) {                    // equal chunks: 16 projections in chunks of at most 15 go as 8 + 8, not 15 + 1
     const int nch = (batch + wbch - 1) / wbch;
     wbch = (batch + nch - 1) / nch;
+  }
+  if (!async || (p->stage_in[0] && p->stage_floats < (size_t)wbch * plane)) {
+    const epr_status ws = host_wait(p);     // a self-contained call, or new staging buffers: the open session (if any) ends here
+    if (ws != EPR_OK) return ws;
   }
   if (p->stage_in[0] && p->stage_floats < (size_t)wbch * plane) {           // staging buffers too small for this call: re-allocate
     CU(p, cudaDeviceSynchronize());
@@ -965,7 +989,9 @@ static epr_status retrieve_host_impl(epr_plan_t p, int factor, int batch, const 
   cudaStream_t s_in = p->hstream[0], s_cmp = p->hstream[1], s_out = p->hstream[2];
   // The call works on private streams and on the plan's shared workspaces: whatever earlier calls on this plan enqueued
   // on the caller's streams (they only enqueue and return) must have finished first.
-  CU(p, cudaDeviceSynchronize());
+  if (!p->hsession) CU(p, cudaDeviceSynchronize());
+  const bool head_taper = !p->hsession;     // inside a session the previous call's last loop covers this call's first copy
+  if (async) p->hsession = 1;
   // Tapered schedule: the first copy in and the last copy out cannot overlap any compute, so the first and the last
   // chunks are small (wbch/4, wbch/2, wbch, …, wbch, wbch/2, wbch/4) when the batch holds at least three full chunks.
   const bool taper = wbch >= 4 && batch >= 3 * wbch;
@@ -975,16 +1001,18 @@ static epr_status retrieve_host_impl(epr_plan_t p, int factor, int batch, const 
     const int left = batch - b0;
     nb = wbch;
     if (taper) {
-      if (chunk < 2) nb = head[chunk];
+      if (chunk < 2) { if (head_taper) nb = head[chunk]; }
+      else if (async) { }                  // a session never knows its last call: no small chunks at the end of a call
       else if (left <= wbch / 4) nb = left;
       else if (left <= wbch / 4 + wbch / 2) nb = left - wbch / 4;
       else if (left < wbch + wbch / 4 + wbch / 2) nb = left - (wbch / 4 + wbch / 2);
     }
     if (nb > left) nb = left;
-    const int buf = chunk & 1;
+    const long long seq = async ? p->hchunk++ : (long long)chunk;         // position in the session / in this call
+    const int buf = (int)(seq & 1);
     cudaEvent_t ev_in = p->hev[buf * 3 + 0], ev_cmp = p->hev[buf * 3 + 1], ev_out = p->hev[buf * 3 + 2];
     const size_t bytes = (size_t)nb * plane * sizeof(float);
-    if (chunk >= 2) {                       // buffers of chunk-2 must be free: its compute read stage_in, its D2H read stage_out
+    if (seq >= 2) {                       // buffers of chunk-2 must be free: its compute read stage_in, its D2H read stage_out
       CU(p, cudaStreamWaitEvent(s_in, ev_cmp, 0));
       if (p->opt.init == 1) CU(p, cudaStreamWaitEvent(s_in, ev_out, 0));
       CU(p, cudaStreamWaitEvent(s_cmp, ev_out, 0));
@@ -1002,6 +1030,7 @@ static epr_status retrieve_host_impl(epr_plan_t p, int factor, int batch, const 
     CU(p, cudaMemcpyAsync(out_host + (size_t)b0 * plane, p->stage_out[buf], bytes, cudaMemcpyDeviceToHost, s_out));
     CU(p, cudaEventRecord(ev_out, s_out));
   }
+  if (async) return EPR_OK;
   CU(p, cudaStreamSynchronize(s_out));
   CU(p, cudaStreamSynchronize(s_cmp));
   return EPR_OK;
@@ -1011,7 +1040,59 @@ extern "C" epr_status epr_retrieve_host(epr_plan_t p, int batch, const float* d_
                                         float step) {
   if (!p) return EPR_EINVAL;
   DevGuard dg(p);
-  return retrieve_host_impl(p, 1, batch, d_host, out_host, iterations, step);
+  return retrieve_host_impl(p, 1, batch, d_host, out_host, iterations, step, 0);
+}
+
+extern "C" epr_status epr_retrieve_host_async(epr_plan_t p, int batch, const float* d_host, float* out_host, int iterations,
+                                              float step) {
+  if (!p) return EPR_EINVAL;
+  DevGuard dg(p);
+  return retrieve_host_impl(p, 1, batch, d_host, out_host, iterations, step, 1);
+}
+
+extern "C" epr_status epr_host_wait(epr_plan_t p) {
+  if (!p) return EPR_EINVAL;
+  DevGuard dg(p);
+  return host_wait(p);
+}
+
+// Contiguous, balanced split of `total` independent projections over `parts`: part k gets [*start, *stop); the first
+// total % parts parts take one more.  Pure host arithmetic (no device needed).
+extern "C" epr_status epr_shard_range(int total, int k, int parts, int* start, int* stop) {
+  if (total < 0 || parts < 1 || k < 0 || k >= parts || !start || !stop) return EPR_EINVAL;
+  const int base = total / parts, rem = total % parts;
+  *start = k * base + (k < rem ? k : rem);
+  *stop = *start + base + (k < rem ? 1 : 0);
+  return EPR_OK;
+}
+
+// One host batch over several plans (one per GPU): plan k takes a contiguous, balanced range of the batch
+// (the split of epr_inputs.shard_range) as one streaming call, then all are awaited.
+extern "C" epr_status epr_retrieve_host_multi(epr_plan_t* plans, int n_plans, int batch, const float* d_host, float* out_host,
+                                              int iterations, float step) {
+  if (!plans || n_plans < 1) return EPR_EINVAL;
+  for (int k = 0; k < n_plans; ++k) {
+    if (!plans[k]) return EPR_EINVAL;
+    if (plans[k]->nx != plans[0]->nx || plans[k]->ny != plans[0]->ny) FAIL(plans[k], EPR_EINVAL, "epr_retrieve_host_multi: plans of different grids");
+  }
+  if (batch < 1 || !d_host || !out_host) FAIL(plans[0], EPR_EINVAL, "epr_retrieve_host_multi: bad batch or NULL pointer");
+  const size_t plane = (size_t)plans[0]->nx * plans[0]->ny;
+  epr_status first = EPR_OK;
+  for (int k = 0; k < n_plans; ++k) {
+    int b0 = 0, b1 = 0;
+    epr_shard_range(batch, k, n_plans, &b0, &b1);
+    if (b1 == b0) continue;
+    DevGuard dg(plans[k]);
+    const epr_status st = retrieve_host_impl(plans[k], 1, (int)(b1 - b0), d_host + (size_t)b0 * plane, out_host + (size_t)b0 * plane,
+                                             iterations, step, 1);
+    if (st != EPR_OK && first == EPR_OK) first = st;
+  }
+  for (int k = 0; k < n_plans; ++k) {
+    DevGuard dg(plans[k]);
+    const epr_status st = host_wait(plans[k]);
+    if (st != EPR_OK && first == EPR_OK) first = st;
+  }
+  return first;
 }
 
 // Host buffers on the DETECTOR grid, the loop on the oversampled grid of the plan (R16): the same chunked,
@@ -1023,5 +1104,5 @@ extern "C" epr_status epr_retrieve_oversampled_host(epr_plan_t p, int factor, in
   epr_status st = check_oversampling(p, factor, "epr_retrieve_oversampled_host");
   if (st != EPR_OK) return st;
   if ((st = ensure_oversampling_buffers(p)) != EPR_OK) return st;
-  return retrieve_host_impl(p, factor, batch, d_host, out_host, iterations, step);
+  return retrieve_host_impl(p, factor, batch, d_host, out_host, iterations, step, 0);
 }

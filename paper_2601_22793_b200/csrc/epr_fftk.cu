@@ -925,11 +925,9 @@ static bool launch_cols_tma(const epr_plan_s* p, const EprLines& LL, int oplanes
     dim3 grid(M / C::W, oplanes);
     if constexpr (2 * C::NT == 1024) {
       // one line per tile and enough tiles to keep every SM's two groups busy: persistent two-group kernel
-      static int two = -1;                               // process-wide developer switch (environment), not device state
-      if (two < 0) { const char* e = getenv("EPR_COLS2"); two = e ? atoi(e) : 1; }
       const int sms = p->sms;
       const int ntiles = (M / C::W) * oplanes;
-      if (two && stage == 0 && !(mode == 1 && p->n_bins > 1) && ntiles >= 8 * sms) {
+      if (stage == 0 && !(mode == 1 && p->n_bins > 1) && ntiles >= 8 * sms) {
         constexpr size_t smem2 = 3 * C::TILE + 32;
         static EprPerDevice attr2 = {};
         if (!attr2.at(p)) { cudaFuncSetAttribute(k_cols_tma2<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2); attr2.at(p) = 1; }

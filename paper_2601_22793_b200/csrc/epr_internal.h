@@ -87,6 +87,8 @@ struct epr_plan_s {
   size_t stage_floats;         // floats each staging buffer holds
   cudaStream_t hstream[3];     // copy-in, compute, copy-out
   cudaEvent_t hev[6];          // per buffer: in-done, compute-done, out-done
+  int hsession;                // 1 while epr_retrieve_host_async calls are outstanding (closed by epr_host_wait)
+  long long hchunk;            // chunks enqueued in the open session (buffer = hchunk & 1)
   // CUDA graph of the last epr_retrieve (same buffers, batch, iterations, step): replayed instead of re-enqueued
   cudaGraphExec_t graph_exec;
   const float* graph_d;

@@ -701,8 +701,7 @@ static cudaError_t launch_splat_v(const epr_plan_s* p, int batch, int H, size_t 
   }
   dim3 grid((p->nx + ST_W - 1) / ST_W, (p->ny + TH - 1) / TH, batch);
   // several lines share one list of ring candidates (the coordinates are packed in 8 bits each: H ≤ 64)
-  static const bool list_off = getenv("EPR_SPLAT_LIST") && atoi(getenv("EPR_SPLAT_LIST")) == 0;
-  const int use_list = FROM_TAU && p->lines.n_bins > 1 && H <= 64 && !list_off;
+  const int use_list = FROM_TAU && p->lines.n_bins > 1 && H <= 64;
   k_splat_tile<FROM_TAU, MAP_OUT, NT, TH, COLS><<<grid, NT, smem, st>>>(COLS ? p->lines_bound : p->lines, p->cols, p->nx, p->ny,
                                                                          p->opt.max_shift_px, H, tau, I_bins, map_in, map_out, out,
                                                                          out_mode, d, p->gmax, use_list, p->d_flags);

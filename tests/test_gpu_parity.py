@@ -514,6 +514,102 @@ def test_retrieve_outputs_and_host_path(E):
     plan.destroy()
 
 
+@pytest.mark.parametrize("name", ["C3", "C4"])
+def test_retrieve_device_batch_larger_than_the_work_batch(E, name, monkeypatch):
+    """epr_retrieve on DEVICE buffers with batch > the plan's work batch (what bench.py's C5 sub-result times: 64 projections
+    in passes of 16): EPR_WORK_BATCH = 2 at plan time, batch 5 → passes of 2, 2, 1, each projection against the oracle."""
+    import torch
+    w = make_workload(name, n=128, batch=5)
+    monkeypatch.setenv("EPR_WORK_BATCH", "2")
+    plan = E.epr_plan(w.nx, w.ny, w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
+                      max_batch=5, max_shift_px=w.max_shift_px)
+    monkeypatch.delenv("EPR_WORK_BATCH")
+    d = _dev(w.d)
+    out = torch.empty_like(d)
+    E.epr_retrieve(plan, d, out, w.iterations, w.step)
+    got = out.cpu().numpy()
+    # the same call on a plan whose work batch holds everything: the passes change nothing, bit for bit
+    whole = E.epr_plan(w.nx, w.ny, w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
+                       max_batch=5, max_shift_px=w.max_shift_px)
+    out2 = torch.empty_like(d)
+    E.epr_retrieve(whole, d, out2, w.iterations, w.step)
+    assert torch.equal(out, out2)
+    plan.destroy()
+    whole.destroy()
+    lines = O.derive_lines(w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta)
+    for j in range(5):
+        ref = O.retrieve(w.d[j].astype(np.float64), lines, w.solver, w.iterations, w.step, S=w.max_shift_px)
+        assert_close(got[j], ref, TOL_PHASE, f"{name} projection {j}")
+
+
+@pytest.mark.parametrize("solver", ["local", "nonlocal"])
+def test_retrieve_host_with_caller_supplied_start(E, solver):
+    """epr_retrieve_host with opt.init = 1: out_host holds τ⁰ on entry and travels to the device beside d in every chunk
+    (batch 5 > max_batch 2: three chunks)."""
+    import torch
+    w = make_workload("C3" if solver == "nonlocal" else "C1", n=128, batch=5)
+    rng = np.random.default_rng(9)
+    y, x = np.meshgrid(np.arange(w.ny) * 2 * np.pi / w.ny, np.arange(w.nx) * 2 * np.pi / w.nx, indexing="ij")
+    tau0 = np.stack([(0.02 + 0.01 * j) * (1.0 + np.cos(x + j) * np.sin(2 * y)) + 0.001 * rng.normal(size=x.shape)
+                     for j in range(5)]).astype(np.float32)
+    its, step = 3, 0.3                                                    # under-relaxed: the start is still visible
+    plan = E.epr_plan(w.nx, w.ny, w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, solver, max_batch=2,
+                      max_shift_px=w.max_shift_px, init=1)
+    dh = torch.from_numpy(w.d).pin_memory()
+    oh = torch.from_numpy(tau0.copy()).pin_memory()
+    E.epr_retrieve_host(plan, dh, oh, its, step)
+    plan.destroy()
+    lines = O.derive_lines(w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta)
+    for j in range(5):
+        ref = O.retrieve(w.d[j].astype(np.float64), lines, solver, its, step, S=w.max_shift_px,
+                         tau0=tau0[j].astype(np.float64))
+        start = O.retrieve(w.d[j].astype(np.float64), lines, solver, its, step, S=w.max_shift_px)
+        assert rel_l2(ref, start) > 10 * TOL_PHASE                     # the start matters after 3 iterations
+        assert_close(oh[j].numpy(), ref, TOL_PHASE, f"{solver} projection {j}")
+
+
+@pytest.mark.parametrize("name", ["C1", "C3"])
+def test_host_streaming_session_and_multi_plan(E, name):
+    """epr_retrieve_host_async / epr_host_wait (the next chunk is prepared while the current one is processed):
+    three batches of different sizes enqueued back to back, one wait — every result equals the plain epr_retrieve_host call
+    bit for bit (same chunks, same kernels; only the waiting differs), and so does a plain call that follows an open session.
+    epr_retrieve_host_multi: ONE host batch over two plans (here both on this GPU; one per device in production) — plan 0
+    gets projections [0, 3), plan 1 [3, 5), the split of epr_inputs.shard_range — again the same bits."""
+    import torch
+    from epr_inputs import shard_range
+    w = make_workload(name, n=128, batch=11)
+    its = 4
+    mk = lambda mb: E.epr_plan(w.nx, w.ny, w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
+                               max_batch=mb, max_shift_px=w.max_shift_px)
+    plan = mk(2)
+    dh = torch.from_numpy(w.d).pin_memory()
+    want = torch.empty_like(dh).pin_memory()
+    E.epr_retrieve_host(plan, dh, want, its, w.step)
+    lines = O.derive_lines(w.pixel_m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta)
+    ref = O.retrieve(w.d[10].astype(np.float64), lines, w.solver, its, w.step, S=w.max_shift_px)
+    assert_close(want[10].numpy(), ref, TOL_PHASE)
+    got = torch.full_like(dh, float("nan")).pin_memory()
+    for a, b in ((0, 5), (5, 6), (6, 11)):                              # 5, 1 and 5 projections: 3 + 1 + 3 chunks of <= 2
+        E.epr_retrieve_host(plan, dh[a:b], got[a:b], its, w.step, wait=False)
+    E.epr_host_wait(plan)
+    assert torch.equal(got, want)
+    got2 = torch.full_like(dh, float("nan")).pin_memory()
+    E.epr_retrieve_host(plan, dh[:4], got2[:4], its, w.step, wait=False)   # session left open …
+    E.epr_retrieve_host(plan, dh[4:], got2[4:], its, w.step)               # … a plain call closes it first
+    assert torch.equal(got2, want)
+    E.epr_host_wait(plan)                                                   # nothing open: returns at once
+    other = mk(2)
+    got3 = torch.full((5, w.ny, w.nx), float("nan")).pin_memory()
+    E.epr_retrieve_host_multi([plan, other], dh[:5], got3, its, w.step)
+    assert shard_range(5, 0, 2) == (0, 3) and shard_range(5, 1, 2) == (3, 5)
+    assert torch.equal(got3, want[:5])
+    got4 = torch.full((1, w.ny, w.nx), float("nan")).pin_memory()          # fewer projections than plans: plan 1 idles
+    E.epr_retrieve_host_multi([plan, other], dh[7:8], got4, its, w.step)
+    assert torch.equal(got4, want[7:8])
+    plan.destroy()
+    other.destroy()
+
+
 def test_argument_errors(E):
     import torch
     en, w, db = SPECTRA["mono"]
