@@ -377,12 +377,13 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
     import torch.distributed as dist
     from epr_inputs import make_workload
 
-    w = make_workload(name, n=n, batch=B, distinct=min(distinct, B))
+    # N > 1: ONE seeded batch of N x B projections, rank k retrieves its contiguous share [lo, hi) (shard_range; no
+    # data-path collective: projections are independent) — generated by the rank that needs it
+    from epr_inputs import shard_range
+    lo, hi = shard_range(world * B, rank, world)
+    w = make_workload(name, n=n, batch=hi - lo, distinct=min(distinct, B), first=lo)
     if lines > 0:
         override_lines(w, lines)
-    if world > 1:                                   # every rank gets its own noise realisations
-        rng = np.random.default_rng(4000 + rank)
-        w.d = np.ascontiguousarray(w.d[rng.permutation(B)])
     plane = w.nx * w.ny
     nb = w.n_bins
     plan = epr.epr_plan(m * w.nx, m * w.ny, w.pixel_m / m, w.L_m, w.energy_keV, w.weight, w.delta_over_beta, w.solver,
@@ -509,7 +510,8 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
     res = {
         "value": value, "unit": UNIT, "ms_per_step": ms / steps, "steps": steps, "warmup": warmup,
         "config": {"workload": workload_string(name, w, m, blocks),
-                   "batch_per_gpu": B, "distinct_projections": min(distinct, B),
+                   "batch_per_gpu": B, "global_batch": world * B, "sharding": "contiguous ranges of one seeded batch, no collective",
+                   "distinct_projections": min(distinct, B),
                    "l2": (f"inputs {in_bytes / 1e6:.0f} MB per step > 2 x 126 MB L2: no flush needed" if flush is None else
                           f"inputs {in_bytes / 1e6:.0f} MB per step: L2 flushed (256 MB overwrite) between timed steps"),
                    "ms_per_iteration_per_projection": ms / steps / B / (w.iterations + 1)},

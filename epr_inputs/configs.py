@@ -72,10 +72,12 @@ def _max_phase_gradient(t_px, pixel_m, energy_keV):
     return float(max(gx.max(), gy.max()))
 
 
-def make_workload(name, n=None, batch=None, noise=True, distinct=None):
+def make_workload(name, n=None, batch=None, noise=True, distinct=None, first=0):
     """Build workload `name` (C1..C5).  n: override grid (n x n, or (ny, nx)); batch: override batch.
     distinct: number of distinct simulated projections (the rest of the batch re-draws only the
-    Poisson noise of projection j % distinct) — bounds host-side generation time for large batches."""
+    Poisson noise of projection j % distinct) — bounds host-side generation time for large batches.
+    first: the batch is the slice [first, first + batch) of one larger seeded batch (projection j of that batch has the
+    same image and the same noise whoever generates it): what rank k of a multi-GPU run gets from `shard_range`."""
     c = CONFIGS[name]
     num = int(name[1:])
     ny, nx = c["ny"], c["nx"]
@@ -102,8 +104,9 @@ def make_workload(name, n=None, batch=None, noise=True, distinct=None):
     clean = [fresnel_detector(t, PIXEL_M, L_m, E, w) for t in phantoms]
     d = np.empty((B, ny, nx), dtype=np.float32)
     for j in range(B):
-        img = clean[j % n_distinct]
-        d[j] = poisson_noise(img, PHOTONS, 2000 + num + 7919 * j) if noise else img.astype(np.float32)
+        g = int(first) + j                                # index in the global batch
+        img = clean[g % n_distinct]
+        d[j] = poisson_noise(img, PHOTONS, 2000 + num + 7919 * g) if noise else img.astype(np.float32)
 
     db = c["db100"] * E / 100.0
     return Workload(name=name, nx=nx, ny=ny, batch=B, pixel_m=PIXEL_M, L_m=L_m, energy_keV=E, weight=w,

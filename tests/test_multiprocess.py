@@ -69,6 +69,20 @@ def test_library_shard_range_is_the_same_split():
             E.epr_shard_range(*bad)
 
 
+def test_ranks_generate_their_share_of_one_seeded_batch():
+    """bench.py --gpus N: ONE seeded batch of N x B projections, rank k generates and retrieves the range shard_range gives
+    it (make_workload(first=lo)); put together the shares are the batch a single process would have generated."""
+    from epr_inputs import make_workload
+    whole = make_workload("C1", n=32, batch=7, distinct=2)
+    parts = []
+    for k in range(3):
+        lo, hi = shard_range(7, k, 3)
+        part = make_workload("C1", n=32, batch=hi - lo, distinct=2, first=lo)
+        assert part.L_m == whole.L_m
+        parts.append(part.d)
+    assert np.array_equal(np.concatenate(parts), whole.d)
+
+
 def test_two_rank_gloo_sharding(tmp_path):
     world, total = 2, 7
     mp.spawn(_worker, args=(world, _free_port(), total, str(tmp_path)), nprocs=world, join=True)
