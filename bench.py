@@ -62,7 +62,7 @@ def max_over_ranks(value, device):
     return float(t.item())
 
 
-TRAFFIC_FILE = os.path.join("profiles", "r2_dram_traffic.json")
+TRAFFIC_FILE = os.path.join("profiles", "r3_dram_traffic.json")
 
 
 def measured_traffic(epr, kernel, nb, solver, config, algorithmic_bytes_per_launch):
@@ -83,6 +83,27 @@ def measured_traffic(epr, kernel, nb, solver, config, algorithmic_bytes_per_laun
     if ratio is None:
         return None, f"{TRAFFIC_FILE} has no capture of {kernel} at {config}"
     return ratio * algorithmic_bytes_per_launch, f"{TRAFFIC_FILE} ({tab.get('command', 'ncu --set full')}; {tab.get('lib_version')})"
+
+
+def issue_ceiling(epr, kernel, config, sm_mhz, px_lines_per_launch, avg_ms):
+    """The secondary ceiling SURVEY.md §8(d) names, for kernels that instruction issue bounds rather than HBM: executed warp
+    instructions per pixel and line and the IPC of the committed `ncu --set full` capture (TRAFFIC_FILE, version-checked like
+    `traffic`), and the fraction of the SM's issue peak THIS run reached — instructions of one launch (inst_per_px_line x pixel-lines
+    / 32) over what 148 SMs issuing 4 warp instructions per clock at the sampled SM clock could issue in the measured launch time."""
+    try:
+        tab = json.load(open(os.path.join(ROOT, TRAFFIC_FILE)))
+    except Exception:
+        return None
+    if tab.get("lib_version") != epr.load_library().epr_version().decode():
+        return None
+    ent = tab.get("issue", {}).get(f"{config}:{kernel}")
+    if ent is None or not sm_mhz:
+        return None
+    warp_inst = ent["inst_per_px_line"] * px_lines_per_launch / 32.0
+    peak = 4.0 * 148 * sm_mhz * 1e6 * (avg_ms * 1e-3)
+    return {"inst_per_px_line": ent["inst_per_px_line"], "ipc_ncu": ent["ipc"], "frac_of_issue_peak": warp_inst / peak,
+            "derivation": "inst_per_px_line x pixel-lines per launch / 32 warp instructions over 4 per clock x 148 SMs x the sampled SM "
+                          f"clock ({sm_mhz:.0f} MHz) x the launch time measured in this run; counts from {TRAFFIC_FILE}"}
 
 
 def expected_launches_per_step(kernel, w, m, blocks=0):
@@ -494,7 +515,7 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
         px = px / passes
         avg_ms = tot_ms / cnt
         gbs = bpp * px / (avg_ms * 1e-3) / 1e9
-        per_kernel.append({"kernel": kname, "launches_per_step": launches_per_step, "avg_ms": avg_ms,
+        per_kernel.append({"kernel": kname, "launches_per_step": launches_per_step, "avg_ms": avg_ms, "passes": passes,
                            "share": None, "algorithmic_bytes_per_launch": bpp * px, "achieved_gbs": gbs,
                            "frac": gbs / peak})
     tot = sum(k["avg_ms"] * k["launches_per_step"] for k in per_kernel)
@@ -507,6 +528,10 @@ def measure_config(epr, name, B, steps, warmup, distinct, rank, world, local, li
     roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["achieved_gbs"], "peak": peak,
                 "unit": "GB/s", "frac": dom["frac"], "traffic": traffic, "traffic_source": traffic_src,
                 "peak_source": peak_src, "per_kernel": per_kernel}
+    issue = issue_ceiling(epr, dom["kernel"], name, clk.summary().get("sm_mhz"), B * plane * m * m * nb / dom.get("passes", 1),
+                          dom["avg_ms"])
+    if issue is not None:
+        roofline["issue"] = issue
     res = {
         "value": value, "unit": UNIT, "ms_per_step": ms / steps, "steps": steps, "warmup": warmup,
         "config": {"workload": workload_string(name, w, m, blocks),
